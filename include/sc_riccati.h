@@ -1,0 +1,146 @@
+/* sc_riccati.h — C ABI of the B200-native Riccati-parametrised Eilenberger sweep.
+ *
+ * What it computes (all citations are PAPER.md:<line> = arXiv 2205.15000 "SuperConga"):
+ *   for every Fermi angle phi_k (:189) and every energy (Matsubara i*eps_n, or eps + i*delta, :98) the
+ *   coherence functions gamma, gamma-tilde are marched along straight trajectories R(s) = R_min + s v_F
+ *   (Eq. 23 :153) through a 2-D grain with specular walls (:155, :161), solving the Riccati equations
+ *   (Eq. 25-26 :169-172) with the closed-form step for piecewise-constant Delta, A (the "stepping
+ *   method", :982).  From g = (1 - gamma gamma~)/(1 + gamma gamma~) (Eq. 24 :165) it accumulates the
+ *   gap-equation right-hand side (Eq. 22 :144), the current density (Eq. 8 :69), the Eilenberger
+ *   free-energy term I(R) (Eq. 19 :128) and the LDOS (Eq. 14 :100); the induced vector potential is
+ *   Eq. D1 (:1009) and the self-consistency update is Algorithm 1 (:203-205) with the Picard or
+ *   Barzilai-Borwein accelerator (App. E :1066-1127).  Readings of silent passages: DESIGN.md §3.
+ *
+ * Units (:104-112, Table II :1204-1230): energies in 2 pi kB Tc, lengths in xi0 (v_F = 1), t = T/Tc,
+ * A in Phi0/(pi xi0), j in j0, free-energy density in (2 pi kB Tc)^2 N_F.
+ *
+ * Conventions
+ *   Pointers marked "dev" are CUDA device pointers on opts.device, "host" are host pointers.  The
+ *   caller owns every field buffer; the context owns tables, boundary stores and scratch.  Nothing
+ *   returned has to be freed except the context (sc_destroy).  Every call enqueues on opts.cuda_stream
+ *   and returns without a host synchronisation, except sc_create, sc_ldos's table upload, the
+ *   sc_debug_* taps, and any call given a non-NULL stats pointer (one small D2H copy).
+ *   Grid layout: row-major [j][i], x_i = (i - (nx-1)/2) h, y_j = (j - (ny-1)/2) h.  Complex fields are
+ *   interleaved (re, im) fp64.  Outputs are exactly 0 outside the mask.
+ *   Errors: a status code is returned (never an exception or abort across the ABI); the message is
+ *   available from sc_last_error().  All kernels are sm_100a; there is no CPU fallback: without a CUDA
+ *   device sc_create returns SC_ERR_CUDA.
+ *   One context per host thread.
+ */
+#ifndef SC_RICCATI_H
+#define SC_RICCATI_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sc_ctx sc_ctx;
+
+typedef enum { SC_OK = 0, SC_ERR_ARG = 1, SC_ERR_GEOMETRY = 2, SC_ERR_STATE = 3,
+               SC_ERR_CUDA = 4, SC_ERR_NOMEM = 5, SC_ERR_NUMERIC = 6 } sc_status;
+
+/* Order-parameter basis functions eta(phi) on a circular Fermi surface, Table III (:1238-1246):
+ * s: 1;  d_{x2-y2}: sqrt2 cos 2phi;  d_xy: sqrt2 sin 2phi;  g: sqrt2 sin 4phi. */
+typedef enum { SC_SYM_S = 0, SC_SYM_DX2Y2 = 1, SC_SYM_DXY = 2, SC_SYM_G = 3 } sc_symmetry;
+
+typedef struct { int nx, ny; double h; } sc_grid;
+
+/* One CSG component of the grain (:411-448, :928-958), applied in list order: kind 0 = disc
+ * (cx, cy, r), kind 1 = convex polygon with nvert vertices in counter-clockwise order (host pointers,
+ * copied by sc_create).  add = 1 adds the area, add = 0 removes it. */
+typedef struct { int kind; int add; double cx, cy, r; int nvert; const double *vx, *vy; } sc_shape;
+
+typedef struct {
+    int n_angles;        /* N_phi, even; phi_k = 2 pi k / N_phi (:189) */
+    int n_matsubara;     /* N_eps; eps_n = t (n + 1/2), n = 0..N_eps-1 (:98) */
+    int precision;       /* 64 (default) or 32: arithmetic of the march; ABI buffers stay fp64 */
+    int stepper;         /* 0 = closed-form step (:982); 1 = implicit mid-point C4-C9 (:984-1001) (not yet built) */
+    int quadrature;      /* 0 = paper's rule: Boole / Simpson 3/8 / Simpson 1/3 / trapezoid by N_phi mod 4,3,2 (:189); 1 = trapezoid */
+    int charge_sign;     /* sigma_e = -1 for electrons (:43, :890) */
+    int bc_mode;         /* 0 = specular (:155); 1 = bulk: every start value is the local homogeneous solution */
+    double crystal_rotation; /* rotation of the crystal axes in full turns (:890) */
+    int device;          /* CUDA device ordinal */
+    void* cuda_stream;   /* cudaStream_t; NULL = default stream */
+} sc_opts;
+
+typedef struct {
+    double res_delta, res_j, res_A, res_fe;   /* Eq. 27 (:201), 2-norm; filled by sc_iterate */
+    double min_one_minus_abs_gamma;           /* min over nodes of 1 - max(|gamma|,|gamma~|) (invariant |gamma| < 1) */
+    long long n_updates;                      /* logical trajectory-step updates of the sweep: 2 * N_phi * N_eps * sum_t pieces */
+    long long n_updates_executed;             /* steps actually marched (Eq. 13 symmetry halves them) */
+    float ms;                                 /* device time of the call (CUDA events on the stream) */
+    int n_bad;                                /* interpolation points with no valid neighbour (must be 0) */
+} sc_sweep_stats;
+
+/* Build the trajectory tables for a grain (:153, :189, Fig. 2 :195).  mask: host, nx*ny bytes, 1 iff the
+ * grid point is strictly inside the CSG of `shapes` (checked: SC_ERR_GEOMETRY on disagreement).
+ * T_over_Tc = t.  kappa <= 0 means infinite penetration depth (A_ind = 0, :890). */
+sc_status sc_create(const sc_grid* grid, const unsigned char* mask, const sc_shape* shapes, int nshapes,
+                    double T_over_Tc, double kappa, sc_symmetry symmetry, const sc_opts* opts, sc_ctx** out);
+sc_status sc_destroy(sc_ctx* ctx);
+
+/* Set Delta(R) (dev, complex fp64 [ny][nx]) and the TOTAL vector potential A = A_ext + A_ind (dev fp64
+ * [ny][nx] each; NULL = 0).  Copies into context-owned buffers; does not touch the boundary stores. */
+sc_status sc_set_fields(sc_ctx* ctx, const void* delta, const double* Ax, const double* Ay);
+
+/* Boundary stores := local homogeneous solution at each trajectory end (Algorithm 1 "Initialize
+ * gamma_dD", :205; reading R8).  Needs fields.  Called implicitly by the first sweep. */
+sc_status sc_reset_boundary(sc_ctx* ctx);
+
+/* One Jacobi sweep at the Matsubara energies (:187 "update of the boundary values can be done in
+ * parallel"): reads boundary store A, writes B, swaps.  Outputs (dev, any may be NULL):
+ *   delta_new  complex [ny][nx]   Eq. 22 (:144), n >= 0 only and doubled
+ *   jx, jy     fp64   [ny][nx]    Eq. 8 (:69) in units of j0
+ *   fe_I       fp64   [ny][nx]    I(R) of Eq. 19 (:128)
+ * Repeated calls with unchanged fields are the paper's burn-in (:962). */
+sc_status sc_riccati_sweep(sc_ctx* ctx, void* delta_new, double* jx, double* jy, double* fe_I,
+                           sc_sweep_stats* stats);
+
+/* LDOS N(eps_m, R)/N_F = <Re g_n> (Eq. 14 :100) at eps_m + i*broadening for the current fields, after
+ * n_boundary_iters Jacobi sweeps from freshly reset stores (:366 burn-in).  energies: host, n_e values.
+ * ldos: dev fp64 [n_e][ny][nx].  The Matsubara boundary stores are not touched. */
+sc_status sc_ldos(sc_ctx* ctx, const double* energies, int n_e, double broadening, int n_boundary_iters,
+                  double* ldos, sc_sweep_stats* stats);
+
+/* A_ind = -(1/kappa^2) sum G_{|m'-m|,|n'-n|} (j - <j>_mask) (Eq. D1-D6 :1009-1021, :1040) on the whole
+ * grid (dev in, dev out); fe_magnetic (host, may be NULL) = (h^2/2) sum_mask j.A_ind (reading R18). */
+sc_status sc_update_vector_potential(sc_ctx* ctx, const double* jx, const double* jy,
+                                     double* Aind_x, double* Aind_y, double* fe_magnetic);
+
+/* Set the external vector potential used by sc_iterate (dev fp64 [ny][nx]; NULL = 0). */
+sc_status sc_set_external_field(sc_ctx* ctx, const double* Aext_x, const double* Aext_y);
+
+/* One self-consistency iteration (Algorithm 1 :203-205): fields := (delta, A_ext + A_ind); sweep; A-solve;
+ * x = (Re D, Im D, kappa^2 A_ind) <- x + alpha (g(x) - x) with accelerator 0 = Picard (E5 :1070, alpha =
+ * step) or 1 = Barzilai-Borwein (E8-E11 :1107-1115, first alpha = step, clipped to [1e-3, 100]).  burnin != 0
+ * keeps delta, A_ind fixed (:962).  delta_inout / Aind_*_inout: dev, updated in place. */
+sc_status sc_iterate(sc_ctx* ctx, int accelerator, double step, int burnin, void* delta_inout,
+                     double* Aind_x_inout, double* Aind_y_inout, sc_sweep_stats* stats);
+
+/* ---- parity / debug taps (synchronise) -------------------------------------------------------- */
+/* Geometry: lattice size N_rot, number of trajectories of angle k (all N_phi angles are addressable). */
+sc_status sc_debug_geometry(sc_ctx* ctx, int* n_rot, int* n_traj_total, long long* n_pieces_total);
+/* Tables of angle k (host out, caller-sized from sc_debug_geometry): per trajectory
+ *   it[6] = {t, jf, jl, elem_in, elem_out, 0}, dt[2] = {u_in, u_out}, gidx[4] (entry gather: global
+ *   directed-trajectory ids (angle-major, line order), -1 unused), gw[4] weights.  Returns count in *n. */
+sc_status sc_debug_tables(sc_ctx* ctx, int k, int* n, int* it, double* dt, int* gidx, double* gw);
+/* gamma (and gamma-tilde) at the nodes of trajectory `local` of angle k (k < N_phi/2) for Matsubara index
+ * n_energy, as marched by the LAST sweep's inputs (re-marches that one trajectory). host out, complex. */
+sc_status sc_debug_trajectory(sc_ctx* ctx, int k, int local, int n_energy, int* n_nodes, void* gamma, void* gamma_tilde);
+/* Per-angle energy-summed node sums of the last sweep for angle k on the rotated lattice [t][j] (host out,
+ * N_rot*N_rot each; SF complex): SF = sum gamma/(1+P), SG = sum Im g, SI (Eq. 19 numerator). */
+sc_status sc_debug_partial(sc_ctx* ctx, int k, void* SF, double* SG, double* SI);
+/* Device-math self test: max relative error of the fp64 reciprocal / rsqrt / exp / sincos building blocks
+ * against the CUDA math library on n random arguments (host out, 6 values). */
+sc_status sc_debug_math(sc_ctx* ctx, int n, double* max_rel_err);
+/* Register-resident DFMA microbenchmark: measured fp64 FMA instructions per second of the device (the
+ * roofline denominator of the march kernel). */
+sc_status sc_debug_fp64_peak(sc_ctx* ctx, double* dfma_per_s, double* sm_clock_mhz);
+
+const char* sc_last_error(const sc_ctx* ctx);
+const char* sc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SC_RICCATI_H */

@@ -1,0 +1,577 @@
+// sc_api.cu — C ABI of libsc_riccati.so (include/sc_riccati.h): context, tables, launches.
+// Product code: no CPU fallback; every numerical step runs in the kernels of sc_kernels.cuh.
+#include <cuda_runtime.h>
+#include <cufft.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <numeric>
+#include <string>
+#include <vector>
+
+#include "../../include/sc_riccati.h"
+#include "sc_geometry.hpp"
+#include "sc_kernels.cuh"
+#include "sc_field_kernels.cuh"
+
+#define SC_VERSION_STR "sc_riccati 0.1 (sm_100a)"
+
+namespace {
+
+template <typename T>
+struct DevBuf {
+    T* p = nullptr; size_t n = 0;
+    cudaError_t alloc(size_t count) {
+        release(); n = count;
+        if (!count) return cudaSuccess;
+        return cudaMalloc((void**)&p, count * sizeof(T));
+    }
+    cudaError_t upload(const std::vector<T>& v, cudaStream_t s) {
+        cudaError_t e = alloc(v.size());
+        if (e != cudaSuccess || v.empty()) return e;
+        return cudaMemcpyAsync(p, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice, s);
+    }
+    void release() { if (p) cudaFree(p); p = nullptr; n = 0; }
+    ~DevBuf() { release(); }
+};
+
+struct EnergySet {
+    std::vector<double> zr, zi, w; std::vector<int> partner;
+    DevBuf<double> d_zr, d_zi, d_w; DevBuf<int> d_partner;
+    int ne = 0;
+    sck::EnergyDev dev() const { return sck::EnergyDev{ne, d_zr.p, d_zi.p, d_w.p, d_partner.p}; }
+};
+
+}  // namespace
+
+struct sc_ctx {
+    std::string err;
+    sc_opts opt{};
+    sc_grid grid{};
+    double t = 0, kappa = -1; int sym = 0;
+    cudaStream_t stream = nullptr;
+    int n_sm = 148;
+    scgeo::Geometry geo;
+    // physical trajectories (k < N/2)
+    int G = 0; int smax = 0; long long n_nodes = 0; long long n_pieces_logical = 0;
+    std::vector<int> h_k, h_t, h_jf, h_nn, h_dF, h_dB, h_order, h_line_g;
+    std::vector<long long> h_noff;
+    DevBuf<int> d_k, d_t, d_jf, d_nn, d_dF, d_dB, d_order, d_line_g;
+    DevBuf<double> d_l0, d_l1;
+    DevBuf<long long> d_noff;
+    DevBuf<double> d_vx, d_vy, d_eta, d_W;
+    DevBuf<unsigned char> d_mask, d_ga_n;
+    DevBuf<int> d_ga_idx; DevBuf<double> d_ga_w;
+    // fallback rows
+    std::vector<int> fb_rows;
+    DevBuf<int> d_fb_rows; DevBuf<double> d_fb_px, d_fb_py, d_fb_dx, d_fb_dy, d_fb_eta;
+    DevBuf<double2> d_fb_D; DevBuf<double> d_fb_a;
+    // fields
+    DevBuf<double2> d_delta; DevBuf<double> d_Ax, d_Ay; bool have_A = false, have_fields = false;
+    DevBuf<double> d_Aext_x, d_Aext_y; bool have_Aext = false;
+    DevBuf<double2> d_ndD; DevBuf<double> d_nda; bool nodes_fresh = false;
+    // energies and stores
+    EnergySet mats;
+    DevBuf<double2> d_store[2]; int cur = 0; bool stores_valid = false;
+    // scratch
+    DevBuf<double2> d_scrT, d_scrG; long long scr_stride = 0; int n_slots = 0;
+    DevBuf<double> d_part; DevBuf<int> d_counter; DevBuf<int> d_nbad; DevBuf<double> d_statmax;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    // vector potential / driver state
+    scf::FieldState fs;
+};
+
+namespace {
+
+sc_status fail(sc_ctx* c, sc_status s, const std::string& m) { if (c) c->err = m; return s; }
+#define CU(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return fail(ctx, e_ == cudaErrorMemoryAllocation ? SC_ERR_NOMEM : SC_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); } while (0)
+
+sck::GridDev grid_dev(const sc_ctx* c) {
+    return sck::GridDev{c->grid.nx, c->grid.ny, c->grid.h, c->d_mask.p, c->d_delta.p,
+                        c->have_A ? c->d_Ax.p : nullptr, c->have_A ? c->d_Ay.p : nullptr};
+}
+sck::TrajDev traj_dev(const sc_ctx* c) {
+    return sck::TrajDev{c->G, c->d_k.p, c->d_t.p, c->d_jf.p, c->d_nn.p, c->d_l0.p, c->d_l1.p, c->d_noff.p, c->d_dF.p, c->d_dB.p};
+}
+
+sc_status upload_energies(sc_ctx* ctx, EnergySet& E) {
+    E.ne = (int)E.zr.size();
+    CU(E.d_zr.upload(E.zr, ctx->stream)); CU(E.d_zi.upload(E.zi, ctx->stream));
+    CU(E.d_w.upload(E.w, ctx->stream)); CU(E.d_partner.upload(E.partner, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return SC_OK;
+}
+
+sc_status ensure_nodes(sc_ctx* ctx) {
+    if (ctx->nodes_fresh) return SC_OK;
+    if (!ctx->have_fields) return fail(ctx, SC_ERR_STATE, "sc_set_fields has not been called");
+    const int wpb = 8;
+    sck::rotate_in_kernel<<<(ctx->G + wpb - 1) / wpb, wpb * 32, 0, ctx->stream>>>(
+        grid_dev(ctx), traj_dev(ctx), ctx->d_vx.p, ctx->d_vy.p, ctx->d_eta.p, ctx->geo.c, ctx->opt.charge_sign,
+        ctx->d_ndD.p, ctx->d_nda.p, ctx->d_nbad.p);
+    if (!ctx->fb_rows.empty()) {
+        const int n = (int)ctx->fb_rows.size();
+        sck::fallback_kernel<<<(n + 127) / 128, 128, 0, ctx->stream>>>(grid_dev(ctx), n, ctx->d_fb_rows.p, ctx->d_fb_px.p,
+            ctx->d_fb_py.p, ctx->d_fb_dx.p, ctx->d_fb_dy.p, ctx->d_fb_eta.p, ctx->opt.charge_sign, ctx->d_fb_D.p, ctx->d_fb_a.p);
+    }
+    CU(cudaGetLastError());
+    ctx->nodes_fresh = true;
+    return SC_OK;
+}
+
+sck::MarchArgs march_args(sc_ctx* ctx, const EnergySet& E, const double2* store_old, double2* store_new) {
+    sck::MarchArgs A{};
+    A.T = traj_dev(ctx); A.E = E.dev(); A.order = ctx->d_order.p; A.n_items = ctx->G; A.h = ctx->grid.h;
+    A.nd_D = ctx->d_ndD.p; A.nd_a = ctx->d_nda.p; A.bc_mode = ctx->opt.bc_mode;
+    A.ga_idx = ctx->d_ga_idx.p; A.ga_w = ctx->d_ga_w.p; A.ga_n = ctx->d_ga_n.p;
+    A.fb_D = ctx->d_fb_D.p; A.fb_a = ctx->d_fb_a.p;
+    A.store_old = store_old; A.store_new = store_new;
+    A.scr_T = ctx->d_scrT.p; A.scr_G = ctx->d_scrG.p; A.scr_stride = ctx->scr_stride;
+    A.part = ctx->d_part.p; A.ldos = nullptr; A.counter = ctx->d_counter.p; A.stat_max2 = ctx->d_statmax.p;
+    return A;
+}
+
+template <int MODE>
+sc_status launch_march(sc_ctx* ctx, const sck::MarchArgs& A, bool stats) {
+    CU(cudaMemsetAsync(ctx->d_counter.p, 0, sizeof(int), ctx->stream));
+    const int blocks = ctx->n_slots / sck::MARCH_WARPS;
+    if (stats) sck::march_kernel<MODE, true><<<blocks, sck::MARCH_WARPS * 32, 0, ctx->stream>>>(A);
+    else sck::march_kernel<MODE, false><<<blocks, sck::MARCH_WARPS * 32, 0, ctx->stream>>>(A);
+    CU(cudaGetLastError());
+    return SC_OK;
+}
+
+sc_status reset_stores(sc_ctx* ctx, const EnergySet& E, double2* store) {
+    const long long total = (long long)ctx->G * E.ne;
+    sck::reset_store_kernel<<<(unsigned)((total + 255) / 256), 256, 0, ctx->stream>>>(traj_dev(ctx), E.dev(), ctx->d_ndD.p, ctx->d_nda.p, store);
+    CU(cudaGetLastError());
+    return SC_OK;
+}
+
+sck::BackArgs back_args(sc_ctx* ctx, void* delta_new, double* jx, double* jy, double* feI, int ne_mats) {
+    sck::BackArgs B{};
+    B.G = grid_dev(ctx); B.nphi = ctx->geo.nphi; B.nrot = ctx->geo.nrot; B.c = ctx->geo.c;
+    B.vx = ctx->d_vx.p; B.vy = ctx->d_vy.p; B.eta = ctx->d_eta.p; B.W = ctx->d_W.p;
+    B.line_g = ctx->d_line_g.p; B.T = traj_dev(ctx); B.part = ctx->d_part.p;
+    B.t = ctx->t; B.sigma = ctx->opt.charge_sign;
+    double D = std::log(ctx->t);
+    for (int n = 0; n < ne_mats; ++n) D += 1.0 / (n + 0.5);
+    B.D = D;
+    B.delta_new = (double2*)delta_new; B.jx = jx; B.jy = jy; B.feI = feI; B.n_bad = ctx->d_nbad.p;
+    return B;
+}
+
+sc_status fill_stats(sc_ctx* ctx, sc_sweep_stats* st, int ne, bool had_stats) {
+    if (!st) return SC_OK;
+    CU(cudaEventRecord(ctx->ev1, ctx->stream));
+    CU(cudaEventSynchronize(ctx->ev1));
+    float ms = 0; CU(cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1));
+    st->ms = ms;
+    int nb = 0; CU(cudaMemcpy(&nb, ctx->d_nbad.p, sizeof(int), cudaMemcpyDeviceToHost));
+    st->n_bad = nb;
+    st->n_updates = 2LL * 2LL * ctx->n_pieces_logical * ne;     // gamma and gamma-tilde, both angles of every pair
+    st->n_updates_executed = 2LL * ctx->n_pieces_logical * ne;
+    if (had_stats) {
+        std::vector<double> m(ctx->n_slots);
+        CU(cudaMemcpy(m.data(), ctx->d_statmax.p, m.size() * sizeof(double), cudaMemcpyDeviceToHost));
+        double mx = 0; for (double v : m) mx = std::max(mx, v);
+        st->min_one_minus_abs_gamma = 1.0 - std::sqrt(mx);
+    }
+    return SC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* sc_version(void) { return SC_VERSION_STR; }
+const char* sc_last_error(const sc_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+sc_status sc_create(const sc_grid* grid, const unsigned char* mask, const sc_shape* shapes, int nshapes,
+                    double T_over_Tc, double kappa, sc_symmetry symmetry, const sc_opts* opts, sc_ctx** out) {
+    if (!out) return SC_ERR_ARG;
+    *out = nullptr;
+    sc_ctx* ctx = new sc_ctx();
+    *out = ctx;     // returned even on failure so that sc_last_error works; the caller still destroys it
+    if (!grid || !mask || !shapes || nshapes <= 0 || !opts) return fail(ctx, SC_ERR_ARG, "null argument");
+    if (grid->nx < 2 || grid->ny < 2 || !(grid->h > 0)) return fail(ctx, SC_ERR_ARG, "bad grid");
+    if (!(T_over_Tc > 0)) return fail(ctx, SC_ERR_ARG, "T/Tc must be positive");
+    if (opts->n_matsubara < 1) return fail(ctx, SC_ERR_ARG, "n_matsubara < 1");
+    if (opts->precision != 64 && opts->precision != 0) return fail(ctx, SC_ERR_ARG, "only precision=64 is built in this version");
+    if (opts->stepper != 0) return fail(ctx, SC_ERR_ARG, "only the closed-form stepper is built in this version");
+    ctx->opt = *opts; ctx->grid = *grid; ctx->t = T_over_Tc; ctx->kappa = kappa; ctx->sym = (int)symmetry;
+    if (ctx->opt.charge_sign == 0) ctx->opt.charge_sign = -1;
+    // ---- geometry (host) ----
+    scgeo::Geometry& Gm = ctx->geo;
+    Gm.nx = grid->nx; Gm.ny = grid->ny; Gm.h = grid->h; Gm.nphi = opts->n_angles;
+    for (int s = 0; s < nshapes; ++s) {
+        scgeo::ShapeH S{shapes[s].kind, shapes[s].add, shapes[s].cx, shapes[s].cy, shapes[s].r, {}, {}};
+        if (S.kind == 1) {
+            if (shapes[s].nvert < 3 || !shapes[s].vx || !shapes[s].vy) return fail(ctx, SC_ERR_ARG, "polygon needs >= 3 vertices");
+            S.vx.assign(shapes[s].vx, shapes[s].vx + shapes[s].nvert); S.vy.assign(shapes[s].vy, shapes[s].vy + shapes[s].nvert);
+        } else if (S.kind != 0) return fail(ctx, SC_ERR_ARG, "unknown shape kind");
+        Gm.shapes.push_back(S);
+    }
+    for (int j = 0; j < grid->ny; ++j)
+        for (int i = 0; i < grid->nx; ++i) {
+            const double x = (i - 0.5 * (grid->nx - 1)) * grid->h, y = (j - 0.5 * (grid->ny - 1)) * grid->h;
+            if ((mask[(size_t)j * grid->nx + i] != 0) != scgeo::in_grain(Gm.shapes, x, y))
+                return fail(ctx, SC_ERR_GEOMETRY, "mask disagrees with the shape list");
+        }
+    if (scgeo::build(Gm, ctx->sym, opts->crystal_rotation, opts->quadrature)) return fail(ctx, SC_ERR_GEOMETRY, Gm.err);
+    const int N = Gm.nphi, H = N / 2, NR = Gm.nrot;
+    for (size_t li = 0; li < Gm.line_count.size(); ++li)
+        if (Gm.line_count[li] > 1) return fail(ctx, SC_ERR_GEOMETRY, "lines crossing the grain more than once (holes, concave unions) are not built yet");
+
+    // ---- physical trajectories = directed trajectories of the first half of the angles ----
+    ctx->G = Gm.aoff[H];
+    if (ctx->G == 0) return fail(ctx, SC_ERR_GEOMETRY, "grain contains no lattice node");
+    const int G = ctx->G;
+    ctx->h_k.resize(G); ctx->h_t.resize(G); ctx->h_jf.resize(G); ctx->h_nn.resize(G); ctx->h_dF.resize(G); ctx->h_dB.resize(G);
+    ctx->h_noff.resize(G); ctx->h_line_g.assign((size_t)H * NR, -1);
+    std::vector<double> l0(G), l1(G);
+    long long nodes = 0, pieces = 0; int smax = 0;
+    for (int g = 0; g < G; ++g) {
+        const scgeo::DTraj& d = Gm.dt[g];
+        ctx->h_k[g] = d.k; ctx->h_t[g] = d.t; ctx->h_jf[g] = d.jf; ctx->h_nn[g] = d.jl - d.jf + 1;
+        l0[g] = (d.jf - Gm.c) * Gm.h - d.u_in; l1[g] = d.u_out - (d.jl - Gm.c) * Gm.h;
+        ctx->h_noff[g] = nodes; nodes += ctx->h_nn[g]; pieces += ctx->h_nn[g] + 1; smax = std::max(smax, ctx->h_nn[g]);
+        ctx->h_dF[g] = g;
+        const int mir = Gm.line_first[(size_t)(d.k + H) * NR + (NR - 1 - d.t)];
+        if (mir < 0) return fail(ctx, SC_ERR_GEOMETRY, "internal: mirror trajectory missing");
+        ctx->h_dB[g] = mir;
+        ctx->h_line_g[(size_t)d.k * NR + d.t] = g;
+    }
+    ctx->n_nodes = nodes; ctx->n_pieces_logical = pieces; ctx->smax = smax;
+    ctx->h_order.resize(G);
+    std::iota(ctx->h_order.begin(), ctx->h_order.end(), 0);
+    std::stable_sort(ctx->h_order.begin(), ctx->h_order.end(), [&](int a, int b) { return ctx->h_nn[a] > ctx->h_nn[b]; });
+
+    const int ND = (int)Gm.dt.size();
+    std::vector<int> ga_idx((size_t)ND * 4, 0); std::vector<double> ga_w((size_t)ND * 4, 0.0); std::vector<unsigned char> ga_n(ND, 0);
+    std::vector<double> fpx, fpy, fdx, fdy, feta;
+    for (int d = 0; d < ND; ++d) {
+        const scgeo::DTraj& D = Gm.dt[d];
+        ga_n[d] = (unsigned char)D.gn;
+        for (int i = 0; i < D.gn; ++i) { ga_idx[4 * d + i] = D.gidx[i]; ga_w[4 * d + i] = D.gw[i]; }
+        if (D.gn == 0) {
+            const double w = (D.t - Gm.c) * Gm.h;
+            ctx->fb_rows.push_back(d);
+            fpx.push_back(D.u_in * Gm.vx[D.k] - w * Gm.vy[D.k]); fpy.push_back(D.u_in * Gm.vy[D.k] + w * Gm.vx[D.k]);
+            fdx.push_back(D.mdir[0]); fdy.push_back(D.mdir[1]);
+            feta.push_back(scgeo::eta_of(ctx->sym, std::atan2(D.mdir[1], D.mdir[0]), opts->crystal_rotation));
+        }
+    }
+
+    // ---- device ---- (the host tables above stay inspectable through sc_debug_tables even when this fails)
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(ctx, SC_ERR_CUDA, "no CUDA device: this library has no CPU path");
+    CU(cudaSetDevice(opts->device));
+    cudaDeviceProp prop; CU(cudaGetDeviceProperties(&prop, opts->device));
+    ctx->n_sm = prop.multiProcessorCount;
+    ctx->stream = (cudaStream_t)opts->cuda_stream;
+    CU(cudaEventCreate(&ctx->ev0)); CU(cudaEventCreate(&ctx->ev1));
+
+    // ---- upload ----
+    cudaStream_t s = ctx->stream;
+    std::vector<unsigned char> hm(mask, mask + (size_t)grid->nx * grid->ny);
+    CU(ctx->d_mask.upload(hm, s));
+    CU(ctx->d_k.upload(ctx->h_k, s)); CU(ctx->d_t.upload(ctx->h_t, s)); CU(ctx->d_jf.upload(ctx->h_jf, s)); CU(ctx->d_nn.upload(ctx->h_nn, s));
+    CU(ctx->d_dF.upload(ctx->h_dF, s)); CU(ctx->d_dB.upload(ctx->h_dB, s)); CU(ctx->d_order.upload(ctx->h_order, s));
+    CU(ctx->d_line_g.upload(ctx->h_line_g, s)); CU(ctx->d_l0.upload(l0, s)); CU(ctx->d_l1.upload(l1, s)); CU(ctx->d_noff.upload(ctx->h_noff, s));
+    CU(ctx->d_vx.upload(Gm.vx, s)); CU(ctx->d_vy.upload(Gm.vy, s)); CU(ctx->d_eta.upload(Gm.eta, s)); CU(ctx->d_W.upload(Gm.W, s));
+    CU(ctx->d_ga_idx.upload(ga_idx, s)); CU(ctx->d_ga_w.upload(ga_w, s)); CU(ctx->d_ga_n.upload(ga_n, s));
+    CU(ctx->d_fb_rows.upload(ctx->fb_rows, s)); CU(ctx->d_fb_px.upload(fpx, s)); CU(ctx->d_fb_py.upload(fpy, s));
+    CU(ctx->d_fb_dx.upload(fdx, s)); CU(ctx->d_fb_dy.upload(fdy, s)); CU(ctx->d_fb_eta.upload(feta, s));
+    CU(ctx->d_fb_D.alloc(ND)); CU(ctx->d_fb_a.alloc(ND));
+    CU(cudaMemsetAsync(ctx->d_fb_D.p, 0, ND * sizeof(double2), s)); CU(cudaMemsetAsync(ctx->d_fb_a.p, 0, ND * sizeof(double), s));
+
+    const size_t ng = (size_t)grid->nx * grid->ny;
+    CU(ctx->d_delta.alloc(ng)); CU(ctx->d_Ax.alloc(ng)); CU(ctx->d_Ay.alloc(ng));
+    CU(ctx->d_ndD.alloc(nodes)); CU(ctx->d_nda.alloc(nodes));
+    CU(ctx->d_part.alloc((size_t)nodes * sck::RED_VALS));
+    CU(ctx->d_counter.alloc(1)); CU(ctx->d_nbad.alloc(1));
+    CU(cudaMemsetAsync(ctx->d_nbad.p, 0, sizeof(int), s));
+
+    // Matsubara energies eps_n = t(n+1/2) (:98), unit weights, self-partnered (z = i eps -> -conj z = z)
+    EnergySet& E = ctx->mats;
+    for (int n = 0; n < opts->n_matsubara; ++n) { E.zr.push_back(0.0); E.zi.push_back(T_over_Tc * (n + 0.5)); E.w.push_back(1.0); E.partner.push_back(n); }
+    if (sc_status st = upload_energies(ctx, E)) return st;
+    CU(ctx->d_store[0].alloc((size_t)ND * E.ne)); CU(ctx->d_store[1].alloc((size_t)ND * E.ne));
+
+    // persistent march grid: 2 CTAs of 8 warps per SM; per-warp scratch of (smax+1) pieces x 32 lanes
+    ctx->n_slots = ctx->n_sm * 2 * sck::MARCH_WARPS;
+    ctx->scr_stride = (long long)(smax + 2) * 32;
+    CU(ctx->d_scrT.alloc((size_t)ctx->n_slots * ctx->scr_stride)); CU(ctx->d_scrG.alloc((size_t)ctx->n_slots * ctx->scr_stride));
+    CU(ctx->d_statmax.alloc(ctx->n_slots));
+    CU(cudaMemsetAsync(ctx->d_statmax.p, 0, ctx->n_slots * sizeof(double), s));
+    CU(cudaStreamSynchronize(s));
+    return SC_OK;
+}
+
+sc_status sc_destroy(sc_ctx* ctx) {
+    if (!ctx) return SC_ERR_ARG;
+    if (ctx->ev0) cudaEventDestroy(ctx->ev0);
+    if (ctx->ev1) cudaEventDestroy(ctx->ev1);
+    scf::release(ctx->fs);
+    delete ctx;
+    return SC_OK;
+}
+
+sc_status sc_set_fields(sc_ctx* ctx, const void* delta, const double* Ax, const double* Ay) {
+    if (!ctx || !delta) return fail(ctx, SC_ERR_ARG, "null argument");
+    const size_t ng = (size_t)ctx->grid.nx * ctx->grid.ny;
+    CU(cudaMemcpyAsync(ctx->d_delta.p, delta, ng * sizeof(double2), cudaMemcpyDeviceToDevice, ctx->stream));
+    ctx->have_A = Ax && Ay;
+    if (ctx->have_A) {
+        CU(cudaMemcpyAsync(ctx->d_Ax.p, Ax, ng * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
+        CU(cudaMemcpyAsync(ctx->d_Ay.p, Ay, ng * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
+    }
+    ctx->have_fields = true; ctx->nodes_fresh = false;
+    return SC_OK;
+}
+
+sc_status sc_reset_boundary(sc_ctx* ctx) {
+    if (!ctx) return SC_ERR_ARG;
+    if (sc_status st = ensure_nodes(ctx)) return st;
+    if (sc_status st = reset_stores(ctx, ctx->mats, ctx->d_store[ctx->cur].p)) return st;
+    ctx->stores_valid = true;
+    return SC_OK;
+}
+
+sc_status sc_riccati_sweep(sc_ctx* ctx, void* delta_new, double* jx, double* jy, double* fe_I, sc_sweep_stats* stats) {
+    if (!ctx) return SC_ERR_ARG;
+    if (!ctx->have_fields) return fail(ctx, SC_ERR_STATE, "sc_riccati_sweep before sc_set_fields");
+    if (stats) { CU(cudaEventRecord(ctx->ev0, ctx->stream)); CU(cudaMemsetAsync(ctx->d_nbad.p, 0, sizeof(int), ctx->stream)); }
+    if (sc_status st = ensure_nodes(ctx)) return st;
+    if (!ctx->stores_valid) { if (sc_status st = sc_reset_boundary(ctx)) return st; }
+    sck::MarchArgs A = march_args(ctx, ctx->mats, ctx->d_store[ctx->cur].p, ctx->d_store[ctx->cur ^ 1].p);
+    if (sc_status st = launch_march<0>(ctx, A, stats != nullptr)) return st;
+    ctx->cur ^= 1;
+    sck::BackArgs B = back_args(ctx, delta_new, jx, jy, fe_I, ctx->mats.ne);
+    dim3 grd((ctx->grid.nx + 127) / 128, ctx->grid.ny);
+    sck::rotate_back_kernel<<<grd, 128, 0, ctx->stream>>>(B);
+    CU(cudaGetLastError());
+    return fill_stats(ctx, stats, ctx->mats.ne, true);
+}
+
+sc_status sc_ldos(sc_ctx* ctx, const double* energies, int n_e, double broadening, int n_boundary_iters,
+                  double* ldos, sc_sweep_stats* stats) {
+    if (!ctx || !energies || n_e < 1 || !ldos) return fail(ctx, SC_ERR_ARG, "bad argument");
+    if (!(broadening > 0)) return fail(ctx, SC_ERR_ARG, "broadening must be positive");
+    if (n_boundary_iters < 1) return fail(ctx, SC_ERR_ARG, "n_boundary_iters < 1");
+    if (!ctx->have_fields) return fail(ctx, SC_ERR_STATE, "sc_ldos before sc_set_fields");
+    if (stats) { CU(cudaEventRecord(ctx->ev0, ctx->stream)); CU(cudaMemsetAsync(ctx->d_nbad.p, 0, sizeof(int), ctx->stream)); }
+    if (sc_status st = ensure_nodes(ctx)) return st;
+    // internal energy list closed under eps -> -eps (gamma-tilde_k(eps) = conj gamma_{k+N/2}(-eps), Eq. 13 :95)
+    EnergySet E;
+    std::vector<int> out_idx(n_e);
+    for (int m = 0; m < n_e; ++m) { E.zr.push_back(energies[m]); E.zi.push_back(broadening); E.w.push_back(1.0); out_idx[m] = m; }
+    E.partner.assign(n_e, -1);
+    for (int m = 0; m < n_e; ++m) {
+        if (E.partner[m] >= 0) continue;
+        int best = -1; double bd = 1e-12 * (1.0 + std::fabs(energies[m]));
+        for (int q = 0; q < (int)E.zr.size(); ++q) if (std::fabs(E.zr[q] + energies[m]) <= bd) { best = q; break; }
+        if (best < 0) { best = (int)E.zr.size(); E.zr.push_back(-energies[m]); E.zi.push_back(broadening); E.w.push_back(0.0); E.partner.push_back(m); }
+        E.partner[m] = best; E.partner[best] = m;
+    }
+    if (sc_status st = upload_energies(ctx, E)) return st;
+    const int ND = (int)ctx->geo.dt.size();
+    DevBuf<double2> st0, st1;
+    CU(st0.alloc((size_t)ND * E.ne)); CU(st1.alloc((size_t)ND * E.ne));
+    if (sc_status st = reset_stores(ctx, E, st0.p)) return st;
+    double2* so = st0.p; double2* sn = st1.p;
+    for (int it = 0; it + 1 < n_boundary_iters; ++it) {
+        sck::MarchArgs A = march_args(ctx, E, so, sn);
+        if (sc_status st = launch_march<2>(ctx, A, false)) return st;
+        std::swap(so, sn);
+    }
+    // last sweep: per-energy Re g at every node, in batches of angle pairs sized to the free memory
+    const int H = ctx->geo.nphi / 2;
+    std::vector<long long> pair_nodes(H + 1, 0);
+    for (int g = 0; g < ctx->G; ++g) pair_nodes[ctx->h_k[g] + 1] += ctx->h_nn[g];
+    for (int p = 0; p < H; ++p) pair_nodes[p + 1] += pair_nodes[p];
+    size_t freeb = 0, totalb = 0; CU(cudaMemGetInfo(&freeb, &totalb));
+    const size_t budget = std::min<size_t>(freeb / 2, (size_t)48 << 30);
+    DevBuf<int> d_out_idx; CU(d_out_idx.upload(out_idx, ctx->stream));
+    // items are trajectory-sorted by length, not by pair: run the march over ALL pairs writing into a node
+    // window; windows are contiguous node ranges because node offsets are pair-major.
+    std::vector<int> item_by_pair(ctx->G); std::iota(item_by_pair.begin(), item_by_pair.end(), 0);
+    DevBuf<int> d_items; DevBuf<double> d_ldn;
+    int p0 = 0; bool first = true;
+    while (p0 < H) {
+        int p1 = p0 + 1;
+        while (p1 < H && (size_t)(pair_nodes[p1 + 1] - pair_nodes[p0]) * E.ne * sizeof(double) <= budget) ++p1;
+        const long long nwin = pair_nodes[p1] - pair_nodes[p0];
+        CU(d_ldn.alloc((size_t)nwin * E.ne));
+        std::vector<int> items;
+        for (int g : ctx->h_order) if (ctx->h_k[g] >= p0 && ctx->h_k[g] < p1) items.push_back(g);
+        CU(d_items.upload(items, ctx->stream));
+        sck::MarchArgs A = march_args(ctx, E, so, sn);
+        A.order = d_items.p; A.n_items = (int)items.size();
+        A.ldos = d_ldn.p - (size_t)pair_nodes[p0] * E.ne;       // node offsets are global
+        if (sc_status st = launch_march<1>(ctx, A, false)) return st;
+        sck::BackLdosArgs L{};
+        L.B = back_args(ctx, nullptr, nullptr, nullptr, nullptr, 1);
+        L.ne_out = n_e; L.out_idx = d_out_idx.p; L.partner = E.d_partner.p; L.ne = E.ne;
+        L.ldos_nodes = A.ldos; L.out = ldos; L.p0 = p0; L.p1 = p1; L.accumulate = first ? 0 : 1;
+        dim3 grd((n_e + 63) / 64, ctx->grid.nx, ctx->grid.ny);
+        sck::rotate_back_ldos_kernel<<<grd, 64, 0, ctx->stream>>>(L);
+        CU(cudaGetLastError());
+        CU(cudaStreamSynchronize(ctx->stream));     // d_ldn / d_items are re-used by the next batch
+        first = false; p0 = p1;
+    }
+    sc_status r = fill_stats(ctx, stats, E.ne, false);
+    if (stats) { stats->n_updates *= n_boundary_iters; stats->n_updates_executed *= n_boundary_iters; }
+    return r;
+}
+
+sc_status sc_set_external_field(sc_ctx* ctx, const double* Ax, const double* Ay) {
+    if (!ctx) return SC_ERR_ARG;
+    const size_t ng = (size_t)ctx->grid.nx * ctx->grid.ny;
+    ctx->have_Aext = Ax && Ay;
+    if (ctx->have_Aext) {
+        CU(ctx->d_Aext_x.alloc(ng)); CU(ctx->d_Aext_y.alloc(ng));
+        CU(cudaMemcpyAsync(ctx->d_Aext_x.p, Ax, ng * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
+        CU(cudaMemcpyAsync(ctx->d_Aext_y.p, Ay, ng * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
+    }
+    return SC_OK;
+}
+
+sc_status sc_update_vector_potential(sc_ctx* ctx, const double* jx, const double* jy, double* Ax, double* Ay, double* fe_mag) {
+    if (!ctx || !jx || !jy || !Ax || !Ay) return fail(ctx, SC_ERR_ARG, "null argument");
+    std::string e;
+    int rc = scf::vector_potential(ctx->fs, ctx->grid.nx, ctx->grid.ny, ctx->grid.h, ctx->d_mask.p, ctx->kappa, jx, jy, Ax, Ay, fe_mag, ctx->stream, e);
+    if (rc) return fail(ctx, rc == 2 ? SC_ERR_NOMEM : SC_ERR_CUDA, e);
+    return SC_OK;
+}
+
+sc_status sc_iterate(sc_ctx* ctx, int accelerator, double step, int burnin, void* delta_inout, double* Aix, double* Aiy, sc_sweep_stats* stats) {
+    if (!ctx || !delta_inout) return fail(ctx, SC_ERR_ARG, "null argument");
+    if (accelerator != 0 && accelerator != 1) return fail(ctx, SC_ERR_ARG, "accelerator must be 0 (Picard) or 1 (Barzilai-Borwein)");
+    const int nx = ctx->grid.nx, ny = ctx->grid.ny; const size_t ng = (size_t)nx * ny;
+    const bool withA = ctx->kappa > 0 && Aix && Aiy;
+    std::string e;
+    if (int rc = scf::ensure_driver(ctx->fs, ng, e)) return fail(ctx, rc == 2 ? SC_ERR_NOMEM : SC_ERR_CUDA, e);
+    if (stats) CU(cudaEventRecord(ctx->ev0, ctx->stream));
+    // total A = A_ext + A_ind
+    scf::FieldState& F = ctx->fs;
+    const double* Atx = nullptr; const double* Aty = nullptr;
+    if (ctx->have_Aext || (Aix && Aiy)) {
+        scf::add_fields(F.Atot_x, F.Atot_y, ctx->have_Aext ? ctx->d_Aext_x.p : nullptr, ctx->have_Aext ? ctx->d_Aext_y.p : nullptr, Aix, Aiy, ng, ctx->stream);
+        Atx = F.Atot_x; Aty = F.Atot_y;
+    }
+    if (sc_status st = sc_set_fields(ctx, delta_inout, Atx, Aty)) return st;
+    if (sc_status st = sc_riccati_sweep(ctx, F.dnew, F.jx, F.jy, F.feI, nullptr)) return st;
+    if (!burnin) {
+        if (withA) {
+            if (int rc = scf::vector_potential(F, nx, ny, ctx->grid.h, ctx->d_mask.p, ctx->kappa, F.jx, F.jy, F.gAx, F.gAy, nullptr, ctx->stream, e))
+                return fail(ctx, rc == 2 ? SC_ERR_NOMEM : SC_ERR_CUDA, e);
+        }
+        if (int rc = scf::mix(F, accelerator, step, ctx->kappa, withA, (double2*)delta_inout, Aix, Aiy, ctx->d_mask.p, ng, ctx->stream, e))
+            return fail(ctx, SC_ERR_CUDA, e);
+    }
+    if (stats) {
+        if (sc_status st = fill_stats(ctx, stats, ctx->mats.ne, false)) return st;
+        double r[4] = {0, 0, 0, 0};
+        if (!burnin) { if (int rc = scf::read_residuals(F, r, ctx->stream, e)) return fail(ctx, SC_ERR_CUDA, e); }
+        stats->res_delta = r[0]; stats->res_A = r[1]; stats->res_j = r[2]; stats->res_fe = r[3];
+        stats->min_one_minus_abs_gamma = 0.0;
+    }
+    return SC_OK;
+}
+
+// ---------------------------------------------------------------------------------------------- debug
+sc_status sc_debug_geometry(sc_ctx* ctx, int* n_rot, int* n_traj_total, long long* n_pieces_total) {
+    if (!ctx) return SC_ERR_ARG;
+    if (n_rot) *n_rot = ctx->geo.nrot;
+    if (n_traj_total) *n_traj_total = (int)ctx->geo.dt.size();
+    if (n_pieces_total) *n_pieces_total = 2 * ctx->n_pieces_logical;
+    return SC_OK;
+}
+
+sc_status sc_debug_tables(sc_ctx* ctx, int k, int* n, int* it, double* dt, int* gidx, double* gw) {
+    if (!ctx || k < 0 || k >= ctx->geo.nphi || !n) return fail(ctx, SC_ERR_ARG, "bad argument");
+    const int a = ctx->geo.aoff[k], b = ctx->geo.aoff[k + 1];
+    *n = b - a;
+    if (!it) return SC_OK;
+    for (int d = a; d < b; ++d) {
+        const scgeo::DTraj& D = ctx->geo.dt[d]; const int i = d - a;
+        it[6 * i + 0] = D.t; it[6 * i + 1] = D.jf; it[6 * i + 2] = D.jl; it[6 * i + 3] = D.elem_in; it[6 * i + 4] = D.elem_out; it[6 * i + 5] = 0;
+        dt[2 * i + 0] = D.u_in; dt[2 * i + 1] = D.u_out;
+        for (int q = 0; q < 4; ++q) { gidx[4 * i + q] = q < D.gn ? D.gidx[q] : -1; gw[4 * i + q] = q < D.gn ? D.gw[q] : 0.0; }
+    }
+    return SC_OK;
+}
+
+sc_status sc_debug_trajectory(sc_ctx* ctx, int k, int local, int n_energy, int* n_nodes, void* gamma, void* gamma_tilde) {
+    if (!ctx || k < 0 || k >= ctx->geo.nphi / 2) return fail(ctx, SC_ERR_ARG, "k must be < n_angles/2");
+    const int g = ctx->geo.aoff[k] + local;
+    if (local < 0 || g >= ctx->geo.aoff[k + 1] || n_energy < 0 || n_energy >= ctx->mats.ne) return fail(ctx, SC_ERR_ARG, "bad index");
+    if (!ctx->stores_valid) return fail(ctx, SC_ERR_STATE, "no sweep has been run");
+    const int nn = ctx->h_nn[g];
+    DevBuf<double2> dG, dGT; CU(dG.alloc(nn)); CU(dGT.alloc(nn));
+    // the last sweep read store[cur^1] (now the "new" side) and wrote store[cur]
+    sck::MarchArgs A = march_args(ctx, ctx->mats, ctx->d_store[ctx->cur ^ 1].p, nullptr);
+    sck::debug_traj_kernel<<<1, 32, 0, ctx->stream>>>(A, g, n_energy, dG.p, dGT.p);
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(gamma, dG.p, nn * sizeof(double2), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaMemcpyAsync(gamma_tilde, dGT.p, nn * sizeof(double2), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    if (n_nodes) *n_nodes = nn;
+    return SC_OK;
+}
+
+sc_status sc_debug_partial(sc_ctx* ctx, int k, void* SF, double* SG, double* SI) {
+    if (!ctx || k < 0 || k >= ctx->geo.nphi || !SF || !SG || !SI) return fail(ctx, SC_ERR_ARG, "bad argument");
+    const int H = ctx->geo.nphi / 2, NR = ctx->geo.nrot, p = k % H;
+    const int g0 = ctx->geo.aoff[p], g1 = ctx->geo.aoff[p + 1];
+    if (g1 == g0) return SC_OK;
+    const long long n0 = ctx->h_noff[g0], n1 = ctx->h_noff[g1 - 1] + ctx->h_nn[g1 - 1];
+    std::vector<double> buf((size_t)(n1 - n0) * sck::RED_VALS);
+    CU(cudaStreamSynchronize(ctx->stream));
+    CU(cudaMemcpy(buf.data(), ctx->d_part.p + (size_t)n0 * sck::RED_VALS, buf.size() * sizeof(double), cudaMemcpyDeviceToHost));
+    double* sf = (double*)SF;
+    std::fill(sf, sf + 2 * (size_t)NR * NR, 0.0); std::fill(SG, SG + (size_t)NR * NR, 0.0); std::fill(SI, SI + (size_t)NR * NR, 0.0);
+    for (int g = g0; g < g1; ++g)
+        for (int m = 0; m < ctx->h_nn[g]; ++m) {
+            const double* v = &buf[(size_t)(ctx->h_noff[g] - n0 + m) * sck::RED_VALS];
+            int t = ctx->h_t[g], j = ctx->h_jf[g] + m;
+            if (k < H) { const size_t q = (size_t)t * NR + j; sf[2 * q] = v[0]; sf[2 * q + 1] = v[1]; SG[q] = v[4]; SI[q] = v[5]; }
+            else { const size_t q = (size_t)(NR - 1 - t) * NR + (NR - 1 - j); sf[2 * q] = v[2]; sf[2 * q + 1] = -v[3]; SG[q] = -v[4]; SI[q] = v[5]; }
+        }
+    return SC_OK;
+}
+
+sc_status sc_debug_math(sc_ctx* ctx, int n, double* max_rel_err) {
+    if (!ctx || !max_rel_err) return SC_ERR_ARG;
+    DevBuf<double> d; CU(d.alloc(6)); CU(cudaMemsetAsync(d.p, 0, 6 * sizeof(double), ctx->stream));
+    sck::math_test_kernel<<<64, 128, 0, ctx->stream>>>(n, d.p);
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(max_rel_err, d.p, 6 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return SC_OK;
+}
+
+sc_status sc_debug_fp64_peak(sc_ctx* ctx, double* dfma_per_s, double* sm_clock_mhz) {
+    if (!ctx || !dfma_per_s) return SC_ERR_ARG;
+    DevBuf<double> d; CU(d.alloc(1));
+    const int iters = 20000, blocks = ctx->n_sm * 4, threads = 256;
+    sck::fp64_peak_kernel<<<blocks, threads, 0, ctx->stream>>>(iters / 10, d.p);    // warm-up
+    double best = 0;
+    for (int rep = 0; rep < 3; ++rep) {
+        CU(cudaEventRecord(ctx->ev0, ctx->stream));
+        sck::fp64_peak_kernel<<<blocks, threads, 0, ctx->stream>>>(iters, d.p);
+        CU(cudaEventRecord(ctx->ev1, ctx->stream));
+        CU(cudaEventSynchronize(ctx->ev1));
+        float ms = 0; CU(cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1));
+        best = std::max(best, (double)blocks * threads * (double)iters * 64.0 / (ms * 1e-3));
+    }
+    *dfma_per_s = best;
+    if (sm_clock_mhz) { int khz = 0; cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, ctx->opt.device); *sm_clock_mhz = khz / 1000.0; }
+    return SC_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,303 @@
+// sc_field_kernels.cuh — grid-field kernels around the sweep: vector-potential solve (a8) and the
+// self-consistency mixing (a9).  All reductions are two-stage with a fixed block count and a fixed
+// summation order (deterministic, no atomics).
+//
+// a8: A_ind = -(1/kappa^2) G (*) (j - <j>_mask)  (PAPER.md D1 :1009, :1040), G_{m,n} from the closed form
+// D3-D6 (:1014-1021).  The paper truncates an eigen-decomposition of G "to increase performance" (:1033);
+// here the cross-correlation is done exactly as a zero-padded (2nx x 2ny) FFT convolution (cuFFT D2Z/Z2D —
+// a library FFT, off the roofline-judged path): O(N^2 log N) instead of O(N^4).
+// a9: x = (Re D, Im D, kappa^2 A_x, kappa^2 A_y) (E3 :1053), d = g(x) - x (E4), Picard (E5) or
+// Barzilai-Borwein (E8-E11) with the step size kept on the device.
+#pragma once
+#include <cuda_runtime.h>
+#include <cufft.h>
+
+#include <cmath>
+#include <string>
+#include <vector>
+
+namespace scf {
+
+constexpr int RED_BLOCKS = 296;
+constexpr int RED_THREADS = 256;
+
+struct FieldState {
+    // vector potential
+    int nx = 0, ny = 0; double h = 0;
+    cufftHandle plan_f = 0, plan_b = 0; bool plans = false;
+    cufftDoubleComplex* Ghat = nullptr; double* pad = nullptr; cufftDoubleComplex* spec = nullptr;
+    double* red = nullptr;          // RED_BLOCKS * 8 partials + 16 results
+    // driver
+    size_t ng = 0;
+    double *Atot_x = nullptr, *Atot_y = nullptr, *jx = nullptr, *jy = nullptr, *feI = nullptr, *gAx = nullptr, *gAy = nullptr;
+    double2* dnew = nullptr;
+    double* d_prev = nullptr;       // 4*ng
+    double* d_cur = nullptr;        // 4*ng
+    double *prev_jx = nullptr, *prev_jy = nullptr, *prev_fe = nullptr;
+    double* state = nullptr;        // [0] alpha, [1] iteration index, [2..5] residuals (delta, A, j, fe)
+    bool driver = false, first = true;
+};
+
+inline void release(FieldState& F) {
+    if (F.plans) { cufftDestroy(F.plan_f); cufftDestroy(F.plan_b); }
+    void* ptrs[] = {F.Ghat, F.pad, F.spec, F.red, F.Atot_x, F.Atot_y, F.jx, F.jy, F.feI, F.gAx, F.gAy, F.dnew,
+                    F.d_prev, F.d_cur, F.prev_jx, F.prev_jy, F.prev_fe, F.state};
+    for (void* p : ptrs) if (p) cudaFree(p);
+    F = FieldState();
+}
+
+// ---- deterministic reductions --------------------------------------------------------------------
+template <typename Op>
+__global__ void reduce_stage1(size_t n, Op op, double* partial, int nout) {
+    __shared__ double sh[RED_THREADS];
+    for (int c = 0; c < nout; ++c) {
+        double s = 0.0;
+        for (size_t i = (size_t)blockIdx.x * RED_THREADS + threadIdx.x; i < n; i += (size_t)RED_BLOCKS * RED_THREADS) s += op(i, c);
+        sh[threadIdx.x] = s;
+        __syncthreads();
+        for (int o = RED_THREADS / 2; o; o >>= 1) { if (threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o]; __syncthreads(); }
+        if (threadIdx.x == 0) partial[(size_t)c * RED_BLOCKS + blockIdx.x] = sh[0];
+        __syncthreads();
+    }
+}
+__global__ void reduce_stage2(const double* partial, int nout, double* out) {
+    const int c = threadIdx.x;
+    if (c >= nout) return;
+    double s = 0.0;
+    for (int b = 0; b < RED_BLOCKS; ++b) s += partial[(size_t)c * RED_BLOCKS + b];
+    out[c] = s;
+}
+
+// ---- vector potential -------------------------------------------------------------------------------
+inline double G_closed(int m, int n, double h) {
+    // PAPER.md D3-D6 (:1014-1021), lengths in xi0
+    double acc = 0.0;
+    for (int sa = 1; sa >= -1; sa -= 2)
+        for (int sb = 1; sb >= -1; sb -= 2) {
+            const double p = 1.0 + 2.0 * sa * m, q = 1.0 + 2.0 * sb * n;      // (1+2m), (1+2n) with signed indices
+            const double mm = sa * (double)m, nn = sb * (double)n;
+            const double alpha = p * q * std::log(0.5 * p * p + 0.5 * q * q);
+            const double beta1 = (-2.0 * mm * mm + 2.0 * nn * nn + 4.0 * nn + 1.0) * std::atan(p / q);
+            const double beta2 = (-2.0 * nn * nn + 2.0 * mm * mm + 4.0 * mm + 1.0) * std::atan(q / p);
+            acc += alpha + beta1 + beta2;
+        }
+    const double PI_ = 3.14159265358979323846;
+    return h * h / (4.0 * PI_) * (2.0 * std::log(h) - std::log(2.0) - 3.0 + 0.25 * acc);
+}
+
+__global__ void pad_current_kernel(int nx, int ny, const unsigned char* mask, const double* j, const double* mean, int comp, double* pad) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, jj = blockIdx.y;
+    const int px = 2 * nx;
+    if (i >= px) return;
+    double v = 0.0;
+    if (i < nx && jj < ny) { const size_t q = (size_t)jj * nx + i; if (mask[q]) v = j[q] - mean[comp]; }
+    pad[(size_t)jj * px + i] = v;
+}
+__global__ void spec_mul_kernel(size_t n, cufftDoubleComplex* s, const cufftDoubleComplex* g) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const cufftDoubleComplex a = s[i], b = g[i];
+    s[i] = make_cuDoubleComplex(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+__global__ void crop_kernel(int nx, int ny, const double* pad, double scale, double* out) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    if (i >= nx) return;
+    out[(size_t)j * nx + i] = scale * pad[(size_t)j * 2 * nx + i];
+}
+
+struct MeanOp {
+    const unsigned char* mask; const double* jx; const double* jy;
+    __device__ double operator()(size_t i, int c) const { return mask[i] ? (c == 0 ? jx[i] : c == 1 ? jy[i] : 1.0) : 0.0; }
+};
+__global__ void mean_finish_kernel(double* r) { const double cnt = r[2] > 0 ? r[2] : 1.0; r[0] /= cnt; r[1] /= cnt; }
+struct FemagOp {
+    const unsigned char* mask; const double *jx, *jy, *ax, *ay;
+    __device__ double operator()(size_t i, int) const { return mask[i] ? jx[i] * ax[i] + jy[i] * ay[i] : 0.0; }
+};
+
+#define SCF_CU(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { err = std::string(#call) + ": " + cudaGetErrorString(e_); return e_ == cudaErrorMemoryAllocation ? 2 : 1; } } while (0)
+#define SCF_FFT(call) do { cufftResult r_ = (call); if (r_ != CUFFT_SUCCESS) { err = std::string(#call) + ": cufft error " + std::to_string((int)r_); return 1; } } while (0)
+
+inline int ensure_vp(FieldState& F, int nx, int ny, double h, cudaStream_t s, std::string& err) {
+    if (F.plans) return 0;
+    F.nx = nx; F.ny = ny; F.h = h;
+    const int px = 2 * nx, py = 2 * ny; const size_t nspec = (size_t)py * (px / 2 + 1);
+    SCF_CU(cudaMalloc((void**)&F.pad, (size_t)px * py * sizeof(double)));
+    SCF_CU(cudaMalloc((void**)&F.spec, nspec * sizeof(cufftDoubleComplex)));
+    SCF_CU(cudaMalloc((void**)&F.Ghat, nspec * sizeof(cufftDoubleComplex)));
+    if (!F.red) SCF_CU(cudaMalloc((void**)&F.red, (RED_BLOCKS * 8 + 16) * sizeof(double)));
+    SCF_FFT(cufftPlan2d(&F.plan_f, py, px, CUFFT_D2Z));
+    SCF_FFT(cufftPlan2d(&F.plan_b, py, px, CUFFT_Z2D));
+    SCF_FFT(cufftSetStream(F.plan_f, s)); SCF_FFT(cufftSetStream(F.plan_b, s));
+    F.plans = true;
+    // kernel table on the circular (2ny x 2nx) grid: K[dy][dx] = G_{|dx|,|dy|}; host evaluation of the closed form
+    std::vector<double> tab((size_t)nx * ny), K((size_t)px * py, 0.0);
+    for (int n = 0; n < ny; ++n) for (int m = 0; m < nx; ++m) tab[(size_t)n * nx + m] = G_closed(m, n, h);
+    for (int dy = -(ny - 1); dy <= ny - 1; ++dy)
+        for (int dx = -(nx - 1); dx <= nx - 1; ++dx)
+            K[(size_t)((dy + py) % py) * px + ((dx + px) % px)] = tab[(size_t)std::abs(dy) * nx + std::abs(dx)];
+    SCF_CU(cudaMemcpyAsync(F.pad, K.data(), K.size() * sizeof(double), cudaMemcpyHostToDevice, s));
+    SCF_FFT(cufftExecD2Z(F.plan_f, F.pad, F.Ghat));
+    SCF_CU(cudaStreamSynchronize(s));
+    return 0;
+}
+
+inline int vector_potential(FieldState& F, int nx, int ny, double h, const unsigned char* mask, double kappa,
+                            const double* jx, const double* jy, double* Ax, double* Ay, double* fe_mag,
+                            cudaStream_t s, std::string& err) {
+    const size_t ng = (size_t)nx * ny;
+    if (!(kappa > 0)) {       // infinite penetration depth: A_ind = 0 (:890)
+        SCF_CU(cudaMemsetAsync(Ax, 0, ng * sizeof(double), s)); SCF_CU(cudaMemsetAsync(Ay, 0, ng * sizeof(double), s));
+        if (fe_mag) *fe_mag = 0.0;
+        return 0;
+    }
+    if (int rc = ensure_vp(F, nx, ny, h, s, err)) return rc;
+    const int px = 2 * nx, py = 2 * ny; const size_t nspec = (size_t)py * (px / 2 + 1);
+    double* res = F.red + RED_BLOCKS * 8;
+    reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, MeanOp{mask, jx, jy}, F.red, 3);
+    reduce_stage2<<<1, 32, 0, s>>>(F.red, 3, res);
+    mean_finish_kernel<<<1, 1, 0, s>>>(res);
+    const double scale = -1.0 / (kappa * kappa) / ((double)px * py);
+    for (int comp = 0; comp < 2; ++comp) {
+        dim3 g1((px + 127) / 128, py);
+        pad_current_kernel<<<g1, 128, 0, s>>>(nx, ny, mask, comp ? jy : jx, res, comp, F.pad);
+        SCF_FFT(cufftExecD2Z(F.plan_f, F.pad, F.spec));
+        spec_mul_kernel<<<(unsigned)((nspec + 255) / 256), 256, 0, s>>>(nspec, F.spec, F.Ghat);
+        SCF_FFT(cufftExecZ2D(F.plan_b, F.spec, F.pad));
+        dim3 g2((nx + 127) / 128, ny);
+        crop_kernel<<<g2, 128, 0, s>>>(nx, ny, F.pad, scale, comp ? Ay : Ax);
+    }
+    SCF_CU(cudaGetLastError());
+    if (fe_mag) {
+        reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, FemagOp{mask, jx, jy, Ax, Ay}, F.red, 1);
+        reduce_stage2<<<1, 32, 0, s>>>(F.red, 1, res + 4);
+        double v = 0; SCF_CU(cudaMemcpyAsync(&v, res + 4, sizeof(double), cudaMemcpyDeviceToHost, s));
+        SCF_CU(cudaStreamSynchronize(s));
+        *fe_mag = 0.5 * h * h * v;
+    }
+    return 0;
+}
+
+// ---- driver ---------------------------------------------------------------------------------------
+inline int ensure_driver(FieldState& F, size_t ng, std::string& err) {
+    if (F.driver) return 0;
+    F.ng = ng;
+    double** bufs[] = {&F.Atot_x, &F.Atot_y, &F.jx, &F.jy, &F.feI, &F.gAx, &F.gAy, &F.prev_jx, &F.prev_jy, &F.prev_fe};
+    for (double** b : bufs) { SCF_CU(cudaMalloc((void**)b, ng * sizeof(double))); SCF_CU(cudaMemset(*b, 0, ng * sizeof(double))); }
+    SCF_CU(cudaMalloc((void**)&F.dnew, ng * sizeof(double2)));
+    SCF_CU(cudaMalloc((void**)&F.d_prev, 4 * ng * sizeof(double))); SCF_CU(cudaMalloc((void**)&F.d_cur, 4 * ng * sizeof(double)));
+    SCF_CU(cudaMalloc((void**)&F.state, 16 * sizeof(double))); SCF_CU(cudaMemset(F.state, 0, 16 * sizeof(double)));
+    if (!F.red) SCF_CU(cudaMalloc((void**)&F.red, (RED_BLOCKS * 8 + 16) * sizeof(double)));
+    F.driver = true; F.first = true;
+    return 0;
+}
+
+__global__ void add_fields_kernel(size_t n, double* ox, double* oy, const double* ax, const double* ay, const double* bx, const double* by) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    ox[i] = (ax ? ax[i] : 0.0) + (bx ? bx[i] : 0.0);
+    oy[i] = (ay ? ay[i] : 0.0) + (by ? by[i] : 0.0);
+}
+inline void add_fields(double* ox, double* oy, const double* ax, const double* ay, const double* bx, const double* by, size_t n, cudaStream_t s) {
+    add_fields_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(n, ox, oy, ax, ay, bx, by);
+}
+
+// d = g(x) - x for the concatenated iterate
+__global__ void diff_kernel(size_t ng, const double2* delta, const double2* dnew, const double* aix, const double* aiy,
+                            const double* gax, const double* gay, double k2, int withA, double* d) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= ng) return;
+    d[i] = dnew[i].x - delta[i].x; d[ng + i] = dnew[i].y - delta[i].y;
+    d[2 * ng + i] = withA ? k2 * (gax[i] - aix[i]) : 0.0;
+    d[3 * ng + i] = withA ? k2 * (gay[i] - aiy[i]) : 0.0;
+}
+struct DotOp {     // c = 0: dp.dd, 1: dp.dp, 2: dd.dd, with dd = d - dp
+    const double* d; const double* dp;
+    __device__ double operator()(size_t i, int c) const {
+        const double a = dp[i], b = d[i] - dp[i];
+        return c == 0 ? a * b : c == 1 ? a * a : b * b;
+    }
+};
+// state[0] = alpha, state[1] = iteration index i (reading R-BB: i starts at 0, first update uses alpha = step)
+__global__ void alpha_kernel(double* state, const double* dots, int accelerator, double step, int first) {
+    if (first) { state[0] = step; state[1] = 0.0; }
+    const int i = (int)state[1];
+    if (accelerator == 1 && i >= 1) {
+        const double dot = fabs(dots[0]);
+        double s = 1.0;
+        if (i & 1) { if (dot > 0) s = dots[1] / dot; } else { if (dots[2] > 0) s = dot / dots[2]; }
+        state[0] = fmin(fmax(state[0] * s, 1e-3), 100.0);
+    } else if (accelerator == 0) state[0] = step;
+    state[1] = i + 1;
+}
+struct NormOp {    // c: 0 |dx_delta|^2, 1 |x_delta|^2, 2 |dx_A|^2, 3 |x_A|^2 (before the update)
+    size_t ng; const double2* delta; const double* aix; const double* aiy; const double* d; const double* state; double k2; int withA;
+    __device__ double operator()(size_t i, int c) const {
+        const double al = state[0];
+        if (c == 0) return al * al * (d[i] * d[i] + d[ng + i] * d[ng + i]);
+        if (c == 1) return delta[i].x * delta[i].x + delta[i].y * delta[i].y;
+        if (!withA) return 0.0;
+        if (c == 2) return al * al * (d[2 * ng + i] * d[2 * ng + i] + d[3 * ng + i] * d[3 * ng + i]) / (k2 * k2);
+        return aix[i] * aix[i] + aiy[i] * aiy[i];
+    }
+};
+struct ObsNormOp {  // c: 0 |j - j_prev|^2, 1 |j_prev|^2, 2 |fe - fe_prev|^2, 3 |fe_prev|^2
+    const double *jx, *jy, *fe, *pjx, *pjy, *pfe;
+    __device__ double operator()(size_t i, int c) const {
+        if (c == 0) return (jx[i] - pjx[i]) * (jx[i] - pjx[i]) + (jy[i] - pjy[i]) * (jy[i] - pjy[i]);
+        if (c == 1) return pjx[i] * pjx[i] + pjy[i] * pjy[i];
+        if (c == 2) return (fe[i] - pfe[i]) * (fe[i] - pfe[i]);
+        return pfe[i] * pfe[i];
+    }
+};
+__global__ void residual_kernel(double* state, const double* n1, const double* n2) {
+    state[2] = n1[1] > 0 ? sqrt(n1[0] / n1[1]) : sqrt(n1[0]);
+    state[3] = n1[3] > 0 ? sqrt(n1[2] / n1[3]) : sqrt(n1[2]);
+    state[4] = n2[1] > 0 ? sqrt(n2[0] / n2[1]) : sqrt(n2[0]);
+    state[5] = n2[3] > 0 ? sqrt(n2[2] / n2[3]) : sqrt(n2[2]);
+}
+__global__ void update_kernel(size_t ng, double2* delta, double* aix, double* aiy, const double* d, const double* state,
+                              const unsigned char* mask, double k2, int withA) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= ng) return;
+    const double al = state[0];
+    const double m = mask[i] ? 1.0 : 0.0;
+    delta[i] = make_double2(m * (delta[i].x + al * d[i]), m * (delta[i].y + al * d[ng + i]));
+    if (withA) { aix[i] += al * d[2 * ng + i] / k2; aiy[i] += al * d[3 * ng + i] / k2; }
+}
+
+inline int mix(FieldState& F, int accelerator, double step, double kappa, bool withA, double2* delta, double* aix, double* aiy,
+               const unsigned char* mask, size_t ng, cudaStream_t s, std::string& err) {
+    const double k2 = withA ? kappa * kappa : 0.0;
+    const unsigned nb = (unsigned)((ng + 255) / 256);
+    double* res = F.red + RED_BLOCKS * 8;
+    diff_kernel<<<nb, 256, 0, s>>>(ng, delta, F.dnew, aix, aiy, F.gAx, F.gAy, k2, withA ? 1 : 0, F.d_cur);
+    if (!F.first && accelerator == 1) {
+        reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(4 * ng, DotOp{F.d_cur, F.d_prev}, F.red, 3);
+        reduce_stage2<<<1, 32, 0, s>>>(F.red, 3, res);
+    }
+    alpha_kernel<<<1, 1, 0, s>>>(F.state, res, accelerator, step, F.first ? 1 : 0);
+    reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, NormOp{ng, delta, aix, aiy, F.d_cur, F.state, k2, withA ? 1 : 0}, F.red, 4);
+    reduce_stage2<<<1, 32, 0, s>>>(F.red, 4, res + 4);
+    reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, ObsNormOp{F.jx, F.jy, F.feI, F.prev_jx, F.prev_jy, F.prev_fe}, F.red, 4);
+    reduce_stage2<<<1, 32, 0, s>>>(F.red, 4, res + 8);
+    residual_kernel<<<1, 1, 0, s>>>(F.state, res + 4, res + 8);
+    update_kernel<<<nb, 256, 0, s>>>(ng, delta, aix, aiy, F.d_cur, F.state, mask, k2 > 0 ? k2 : 1.0, withA ? 1 : 0);
+    SCF_CU(cudaMemcpyAsync(F.prev_jx, F.jx, ng * sizeof(double), cudaMemcpyDeviceToDevice, s));
+    SCF_CU(cudaMemcpyAsync(F.prev_jy, F.jy, ng * sizeof(double), cudaMemcpyDeviceToDevice, s));
+    SCF_CU(cudaMemcpyAsync(F.prev_fe, F.feI, ng * sizeof(double), cudaMemcpyDeviceToDevice, s));
+    std::swap(F.d_cur, F.d_prev);
+    F.first = false;
+    SCF_CU(cudaGetLastError());
+    return 0;
+}
+
+inline int read_residuals(FieldState& F, double r[4], cudaStream_t s, std::string& err) {
+    double st[6];
+    SCF_CU(cudaMemcpyAsync(st, F.state, 6 * sizeof(double), cudaMemcpyDeviceToHost, s));
+    SCF_CU(cudaStreamSynchronize(s));
+    r[0] = st[2]; r[1] = st[3]; r[2] = st[4]; r[3] = st[5];
+    return 0;
+}
+
+}  // namespace scf

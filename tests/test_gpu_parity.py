@@ -1,0 +1,208 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on identical seeded inputs.
+
+Tolerance (BASELINE.json north_star): 1e-9 relative in max-norm on Delta, j, g in FP64, with
+err = max|x_gpu - x_cpu| / max(max|x_cpu|, 1e-6) over the mask (reading A21).
+"""
+import numpy as np
+import pytest
+
+import oracle
+import workloads as wlmod
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-9
+
+
+def relerr(a, b):
+    a = np.asarray(a); b = np.asarray(b)
+    return float(np.max(np.abs(a - b)) / max(float(np.max(np.abs(b))), 1e-6))
+
+
+def dev(a, dtype=None):
+    return torch.as_tensor(np.ascontiguousarray(a), device="cuda") if a is not None else None
+
+
+@pytest.fixture(scope="module")
+def sc():
+    import paper_2205_15000_b200 as m
+    from paper_2205_15000_b200 import build
+    build.build()
+    return m
+
+
+class GpuRun:
+    def __init__(self, sc, wl, **kw):
+        self.wl = wl
+        self.ctx = sc.ScContext.from_workload(wl, **kw)
+        n = (wl.ny, wl.nx)
+        self.dn = torch.zeros(n, dtype=torch.complex128, device="cuda")
+        self.jx = torch.zeros(n, dtype=torch.float64, device="cuda")
+        self.jy = torch.zeros(n, dtype=torch.float64, device="cuda")
+        self.fe = torch.zeros(n, dtype=torch.float64, device="cuda")
+
+    def set_fields(self, delta, Ax, Ay):
+        self.ctx.sc_set_fields(dev(delta.astype(np.complex128)), dev(Ax), dev(Ay))
+
+    def sweep(self, stats=True):
+        st = self.ctx.sc_riccati_sweep(self.dn, self.jx, self.jy, self.fe, want_stats=stats)
+        torch.cuda.synchronize()
+        return dict(delta_new=self.dn.cpu().numpy(), jx=self.jx.cpu().numpy(), jy=self.jy.cpu().numpy(),
+                    fe_I=self.fe.cpu().numpy(), stats=st)
+
+
+def compare_sweeps(sc, wl, n_sweeps=2, **kw):
+    o = oracle.Oracle.from_workload(wl, **{k: v for k, v in kw.items() if k in ("bc_mode",)})
+    g = GpuRun(sc, wl, **kw)
+    Ax = wl.Aext_x if np.any(wl.Aext_x) else None
+    Ay = wl.Aext_y if np.any(wl.Aext_x) else None
+    g.set_fields(wl.delta0, Ax, Ay)
+    stores = None
+    worst = 0.0
+    for it in range(n_sweeps):
+        ro = o.sweep(wl.delta0, Ax, Ay, wl.n_energies, stores)
+        stores = ro["stores"]
+        rg = g.sweep()
+        for key in ("delta_new", "jx", "jy", "fe_I"):
+            e = relerr(rg[key], ro[key])
+            assert e < TOL, (it, key, e)
+            worst = max(worst, e)
+        assert rg["stats"].n_bad == 0 and ro["stats"]["n_bad"] == 0
+        assert rg["stats"].n_updates == ro["stats"]["n_updates"]
+        assert abs(rg["stats"].min_one_minus_abs_gamma - ro["stats"]["min_one_minus_abs_gamma"]) < 1e-9
+        assert np.all(rg["delta_new"][wl.mask == 0] == 0)
+    return o, g, stores, worst
+
+
+def test_math_building_blocks(sc):
+    wl = wlmod.make_workload(0)
+    ctx = sc.ScContext.from_workload(wl)
+    err = ctx.sc_debug_math(4000)
+    for k, v in err.items():
+        assert v < 2e-15, (k, v)
+
+
+def test_cfg0_full_sweeps_and_taps(sc):
+    wl = wlmod.make_workload(0)
+    o, g, stores, worst = compare_sweeps(sc, wl, n_sweeps=3)
+    # boundary stores: oracle gamma_end[d] == GPU gamma of trajectory d (via per-trajectory tap, last sweep)
+    Ax = Ay = None
+    z, w = o.matsubara(wl.n_energies)
+    # re-run the oracle's last sweep inputs: stores before the last sweep
+    st = None
+    for _ in range(2):
+        st = o.sweep(wl.delta0, None, None, wl.n_energies, st)["stores"]
+    for k in (0, 3, 7):
+        for local in (0, 5, o.ntraj_angle(k) - 1):
+            for n in (0, wl.n_energies - 1):
+                Go, GTo, _ = o.debug_trajectory(wl.delta0, Ax, Ay, k, local, z, n, st)
+                Gg, GTg = g.ctx.sc_debug_trajectory(k, local, n)
+                assert relerr(Gg, Go) < TOL and relerr(GTg, GTo) < TOL
+    # per-angle energy-summed node sums on the rotated lattice, both halves of the angle set
+    for k in (1, 9):
+        ro = o.sweep(wl.delta0, None, None, wl.n_energies, st, dbg_angle=k)
+        SF, SG, SI = g.ctx.sc_debug_partial(k)
+        assert relerr(SF, ro["dbg"]["SF"]) < TOL and relerr(SG, ro["dbg"]["SG"]) < TOL and relerr(SI, ro["dbg"]["SI"]) < TOL
+
+
+@pytest.mark.parametrize("cfg,kw,ns", [
+    (1, dict(pts_per_xi=6, n_angles=16, n_energies=40), 2),          # disc, vortex, A != 0, ragged energy tail
+    (2, dict(pts_per_xi=5, n_angles=32, n_energies=33, size_scale=0.5), 2),   # d-wave, [110] walls
+    (4, dict(pts_per_xi=5, n_angles=16, n_energies=64, size_scale=0.2), 1),   # many vortices, 2 full rounds
+])
+def test_reduced_configs(sc, cfg, kw, ns):
+    wl = wlmod.make_workload(cfg, **kw)
+    compare_sweeps(sc, wl, n_sweeps=ns)
+
+
+def test_bulk_boundary_mode(sc):
+    wl = wlmod.make_workload(1, pts_per_xi=5, n_angles=8, n_energies=8)
+    compare_sweeps(sc, wl, n_sweeps=1, bc_mode=1)
+
+
+def test_tiny_and_thin_grains(sc):
+    # 2x2 grain (one-node trajectories) and a thin rectangle (trajectories of very different lengths)
+    for shapes, n in (([wlmod.square(0.2)], (2, 2)), ([wlmod.Shape(kind=1, vx=[-1.5, 1.5, 1.5, -1.5], vy=[-0.2, -0.2, 0.2, 0.2])], (30, 4))):
+        nx, ny = n
+        h = 0.1
+        mask = wlmod.make_mask(shapes, nx, ny, h)
+        rng = np.random.default_rng(5)
+        d0 = (0.25 * (1 + 0.3 * rng.uniform(-1, 1, (ny, nx))) * np.exp(1j * rng.uniform(-1, 1, (ny, nx)))) * mask
+        A = 0.05 * rng.uniform(-1, 1, (ny, nx))
+        wl = wlmod.Workload("tiny", -1, nx, ny, h, shapes, mask, wlmod.SYM_DXY, 0.05, 12, 5, 0.4, -1.0, -1, d0, A, -A, 0.25)
+        compare_sweeps(sc, wl, n_sweeps=2)
+
+
+def test_repeat_sweeps_are_bitwise_deterministic(sc):
+    wl = wlmod.make_workload(1, pts_per_xi=6, n_angles=16, n_energies=40)
+    outs = []
+    for _ in range(2):
+        g = GpuRun(sc, wl)
+        g.set_fields(wl.delta0, wl.Aext_x, wl.Aext_y)
+        g.sweep(); r = g.sweep()
+        outs.append(r)
+    for key in ("delta_new", "jx", "jy", "fe_I"):
+        assert np.array_equal(outs[0][key], outs[1][key])
+
+
+def test_state_errors(sc):
+    wl = wlmod.make_workload(0)
+    ctx = sc.ScContext.from_workload(wl)
+    with pytest.raises(sc.ScError) as e:
+        ctx.sc_riccati_sweep()
+    assert e.value.status == 3       # SC_ERR_STATE: sweep before sc_set_fields
+
+
+def test_ldos_parity(sc):
+    wl = wlmod.make_workload(3, pts_per_xi=5, n_angles=16, size_scale=0.4, n_energies=9)
+    o = oracle.Oracle.from_workload(wl)
+    ctx = sc.ScContext.from_workload(wl)
+    ctx.sc_set_fields(dev(wl.delta0))
+    for energies, iters in ((wl.ldos_energies, 1), (wl.ldos_energies, 4), (np.array([0.0, 0.05, 0.11, -0.3]), 2)):
+        ref = o.ldos(wl.delta0, None, None, energies, wl.ldos_broadening * 2, iters)
+        out = torch.zeros((len(energies), wl.ny, wl.nx), dtype=torch.float64, device="cuda")
+        ctx.sc_ldos(energies, wl.ldos_broadening * 2, iters, out)
+        torch.cuda.synchronize()
+        assert relerr(out.cpu().numpy(), ref) < TOL
+        assert np.all(out.cpu().numpy()[:, wl.mask > 0] > 0)
+
+
+def test_vector_potential_parity(sc):
+    wl = wlmod.make_workload(1, pts_per_xi=4, n_angles=8, n_energies=8)
+    ctx = sc.ScContext.from_workload(wl)
+    rng = np.random.default_rng(11)
+    jx = rng.normal(size=(wl.ny, wl.nx)) * wl.mask; jy = rng.normal(size=(wl.ny, wl.nx)) * wl.mask
+    Ax = torch.zeros((wl.ny, wl.nx), dtype=torch.float64, device="cuda"); Ay = torch.zeros_like(Ax)
+    fe = ctx.sc_update_vector_potential(dev(jx), dev(jy), Ax, Ay, want_energy=True)
+    rx, ry = oracle.vector_potential(wl.mask, wl.h, wl.kappa, jx, jy)
+    assert relerr(Ax.cpu().numpy(), rx) < TOL and relerr(Ay.cpu().numpy(), ry) < TOL
+    ref_fe = 0.5 * wl.h ** 2 * float(np.sum((jx * rx + jy * ry)[wl.mask > 0]))
+    assert abs(fe - ref_fe) < 1e-9 * abs(ref_fe)
+
+
+@pytest.mark.parametrize("cfg,kw,acc,niter", [
+    (0, {}, 0, 20),                                                        # configs[0]: 20 Picard iterations
+    (1, dict(pts_per_xi=5, n_angles=16, n_energies=24), 1, 6),            # kappa = 2, Barzilai-Borwein, induced A
+])
+def test_self_consistent_iterations_match(sc, cfg, kw, acc, niter):
+    wl = wlmod.make_workload(cfg, **kw)
+    o = oracle.Oracle.from_workload(wl)
+    drv = oracle.Driver(o, wl.Aext_x, wl.Aext_y, wl.n_energies, accelerator=acc, step=1.0)
+    ctx = sc.ScContext.from_workload(wl)
+    ctx.sc_set_external_field(dev(wl.Aext_x), dev(wl.Aext_y))
+    d_g = dev(wl.delta0.astype(np.complex128)).clone()
+    ax_g = torch.zeros((wl.ny, wl.nx), dtype=torch.float64, device="cuda"); ay_g = torch.zeros_like(ax_g)
+    d_o = wl.delta0.copy(); ax_o = np.zeros((wl.ny, wl.nx)); ay_o = np.zeros((wl.ny, wl.nx))
+    for it in range(niter):
+        r = drv.iterate(d_o, ax_o, ay_o)
+        d_o, ax_o, ay_o = r["delta"], r["Aind_x"], r["Aind_y"]
+        st = ctx.sc_iterate(acc, 1.0, False, d_g, ax_g, ay_g, want_stats=True)
+        torch.cuda.synchronize()
+        # the fixed-point map amplifies rounding differences by at most alpha per iteration
+        tol = TOL * max(1.0, 3.0 ** min(it, 6)) if acc == 1 else TOL
+        assert relerr(d_g.cpu().numpy(), d_o) < tol, it
+        if wl.kappa > 0:
+            assert relerr(ax_g.cpu().numpy(), ax_o) < tol * 10, it
+        assert abs(st.res_delta - r["res_delta"]) < 1e-7 * max(r["res_delta"], 1e-3)
+    assert r["res_delta"] < 0.2
