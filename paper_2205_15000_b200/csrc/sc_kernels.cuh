@@ -494,7 +494,8 @@ __global__ void math_test_kernel(int n, double* err /*6*/) {
         const double y = 1.5707963 * (u1 - 0.5);                        // |y| <= pi/4
         double sn, cm1; scm::sincos_small(y, sn, cm1);
         e[4] = fmax(e[4], fabs(sn - sin(y)) / fmax(fabs(sin(y)), 1e-300));
-        e[5] = fmax(e[5], fabs(cm1 - (cos(y) - 1.0)) / fmax(fabs(cos(y) - 1.0), 1e-300));
+        const double sh = sin(0.5 * y), cref = -2.0 * sh * sh;              // cos y - 1 without cancellation
+        e[5] = fmax(e[5], fabs(cm1 - cref) / fmax(fabs(cref), 1e-300));
     }
     for (int c = 0; c < 6; ++c) {
         double v = e[c];
