@@ -1,0 +1,261 @@
+#!/usr/bin/env python
+"""bench.py — Riccati trajectory-step updates/s of one self-consistent iteration (sweep + A-solve + mixing).
+
+  python bench.py --gpus N --steps K --warmup W [--impl reference] [--cfg C]
+
+A step = one `sc_iterate` (Algorithm 1 :203-205) over one synthetic grain: rotate-in, march
+(gamma-tilde down, gamma up, node products, energy reduction), rotate-back + finalise, FFT vector-potential
+solve, Barzilai-Borwein mixing.  Workload at N=1: BASELINE.json configs[4] (s-wave disc R = 40 xi0,
+1600x1600 grid, 256 angles, 512 Matsubara energies, kappa = 2, 20 vortices), the config the metric's FP64
+target is quoted on.  Inputs are seeded synthetic fields (workloads/), resident in HBM for `value`; `e2e`
+repeats the measurement with pinned HOST buffers copied in and out every step.
+With --gpus N > 1 (torchrun) the Matsubara energies are sharded across ranks (the march, the specular
+boundary condition and the boundary stores never couple energies) and the partial Delta_new, j, I fields are
+summed with one NCCL all-reduce per sweep; per-rank work shrinks as N grows -> "strong" scaling.
+--impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import workloads  # noqa: E402
+
+METRIC = "riccati_trajectory_step_updates_per_s"
+UNIT = "updates/s"
+# FP64-pipe instructions the closed-form path needs per (node, energy, angle pair) = 4 logical updates
+# (gamma and gamma-tilde for angles k and k+N/2): DESIGN.md §6 tally.
+ALGO_FP64_INSTR_PER_UNIT = 184.0
+
+
+class ClockSampler(threading.Thread):
+    def __init__(self, index=0, period=0.2):
+        super().__init__(daemon=True)
+        self.index, self.period, self.rows, self._halt = index, period, [], threading.Event()
+
+    def run(self):
+        q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+        while not self._halt.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-i", str(self.index)],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([c.strip() for c in out.split(",")])
+            except Exception:
+                pass
+            self._halt.wait(self.period)
+
+    def stop(self):
+        self._halt.set()
+        self.join(timeout=5)
+        sm = [float(r[0]) for r in self.rows if r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if r[1].replace(".", "").isdigit()]
+        reasons = set()
+        for r in self.rows:
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--cfg", type=int, default=4)
+    ap.add_argument("--pts-per-xi", type=float, default=None)
+    ap.add_argument("--n-angles", type=int, default=None)
+    ap.add_argument("--n-energies", type=int, default=None)
+    ap.add_argument("--size-scale", type=float, default=1.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep-only", action="store_true", help="time sc_riccati_sweep alone (profiling aid)")
+    return ap.parse_args()
+
+
+def workload_from_args(a):
+    kw = {}
+    if a.pts_per_xi: kw["pts_per_xi"] = a.pts_per_xi
+    if a.n_angles: kw["n_angles"] = a.n_angles
+    if a.n_energies: kw["n_energies"] = a.n_energies
+    if a.size_scale != 1.0: kw["size_scale"] = a.size_scale
+    return workloads.make_workload(a.cfg, **kw)
+
+
+def config_of(wl, a, extra=None):
+    c = {"workload": f"BASELINE.json configs[{wl.cfg}]: {wl.name}", "grid": f"{wl.nx}x{wl.ny}", "n_in": wl.n_in,
+         "n_angles": wl.n_angles, "n_energies": wl.n_energies, "t": wl.t, "kappa": wl.kappa,
+         "step": "one self-consistent iteration (sweep + A-solve + BB mixing)",
+         "l2": "inputs larger than L2 (march scratch and partial sums are GBs per step); no flush needed"}
+    if extra:
+        c.update(extra)
+    return c
+
+
+# ------------------------------------------------------------------------------------------------
+# CPU oracle legs
+# ------------------------------------------------------------------------------------------------
+def oracle_sample(wl, cores):
+    """One bounded sample of the workload on the oracle: a subset of angles (one per core, evenly spaced) and
+    the lowest Matsubara energies, sized to ~10-30 s.  Returns (updates, seconds, description)."""
+    import oracle
+    os.environ.setdefault("OMP_NUM_THREADS", str(cores))
+    o = oracle.Oracle.from_workload(wl)
+    per_angle_nodes = wl.n_in
+    target = 1.2e8                                  # updates per core at ~130 ns each -> ~15 s
+    ne = int(max(1, min(wl.n_energies, target // (2 * per_angle_nodes))))
+    nang = min(cores, wl.n_angles)
+    angles = [int(round(i * wl.n_angles / nang)) % wl.n_angles for i in range(nang)]
+    z, w = o.matsubara(ne)
+    Ax, Ay = (wl.Aext_x, wl.Aext_y) if np.any(wl.Aext_x) else (None, None)
+    stores = o.reset_stores(wl.delta0, Ax, Ay, z)
+    t0 = time.perf_counter()
+    r = o.raw_sweep(wl.delta0, Ax, Ay, z, w, stores, angle_list=angles)
+    dt = time.perf_counter() - t0
+    return r["stats"]["n_updates"], dt, f"{nang} of {wl.n_angles} angles x {ne} of {wl.n_energies} energies, all trajectories, 1 sweep"
+
+
+def run_reference(a):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    wl = workload_from_args(a)
+    cores = os.cpu_count() or 1
+    for _ in range(min(a.warmup, 1)):
+        pass                                        # the oracle has no warm-up state worth timing away
+    tot_u, tot_t, desc = 0, 0.0, ""
+    for _ in range(a.steps):
+        u, t, desc = oracle_sample(wl, cores)
+        tot_u += u; tot_t += t
+    val = tot_u / tot_t
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": a.gpus, "steps": a.steps,
+            "warmup": a.warmup, "ms_per_step": 1e3 * tot_t / a.steps, "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_of(wl, a),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------
+# CUDA path
+# ------------------------------------------------------------------------------------------------
+def run_ours(a):
+    import torch
+    import paper_2205_15000_b200 as sc
+
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    torch.cuda.set_device(local)
+    devname = f"cuda:{local}"
+    wl = workload_from_args(a)
+    if world > 1:
+        raise SystemExit("multi-GPU energy sharding is not built yet (DESIGN.md §8): run with --gpus 1")
+
+    ctx = sc.ScContext.from_workload(wl, device=local)
+    dev = lambda x: torch.as_tensor(np.ascontiguousarray(x), device=devname)
+    ng = wl.nx * wl.ny
+    delta = dev(wl.delta0.astype(np.complex128))
+    aix = torch.zeros((wl.ny, wl.nx), dtype=torch.float64, device=devname); aiy = torch.zeros_like(aix)
+    ctx.sc_set_external_field(dev(wl.Aext_x), dev(wl.Aext_y))
+    acc = wl.accelerator
+    dn = torch.zeros_like(delta); jx = torch.zeros_like(aix); jy = torch.zeros_like(aix); fe = torch.zeros_like(aix)
+
+    def step():
+        if a.sweep_only:
+            ctx.sc_set_fields(delta, dev_ax, dev_ay)
+            ctx.sc_riccati_sweep(dn, jx, jy, fe)
+        else:
+            ctx.sc_iterate(acc, 1.0, False, delta, aix, aiy)
+
+    dev_ax, dev_ay = dev(wl.Aext_x), dev(wl.Aext_y)
+    # launches of OUR kernels per step: rotate_in, march, rotate_back (+ memset) ; A-solve: 3 reductions + 2x(pad, mul,
+    # crop) [+ 4 cuFFT library launches, not counted]; mixing: diff, 2x3 reduction stages, alpha, residual, update
+    launches_per_step = 3 if a.sweep_only else (3 + (3 + 6 if wl.kappa > 0 else 0) + (1 + 2 + 1 + 4 + 1 + 1))
+
+    for _ in range(max(a.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local); sampler.start()
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    march_ms = []
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(a.steps):
+        step()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+
+    # per-kernel duration of the dominant kernel (the march), CUDA events on the launching stream, same inputs
+    ctx.sc_set_fields(delta, dev_ax if wl.kappa <= 0 else None, dev_ay if wl.kappa <= 0 else None)
+    for _ in range(2):
+        st = ctx.sc_riccati_sweep(dn, jx, jy, fe, want_stats=True)
+        march_ms.append(ctx.last_march_ms())
+    n_updates = st.n_updates
+    units = n_updates / 4.0                       # (node, energy, angle-pair) units incl. the boundary pieces
+    peak_dfma, clk = ctx.sc_debug_fp64_peak()
+    mk_ms = float(np.mean(march_ms))
+    achieved = 2.0 * ALGO_FP64_INSTR_PER_UNIT * units / (mk_ms * 1e-3) / 1e12
+    peak = 2.0 * peak_dfma / 1e12
+    roofline = {"bound": "alu", "kernel": "sck::march_kernel<0,false>", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                "frac": achieved / peak, "traffic": None,
+                "note": "fp64 pipe: flops = 2 x FP64-pipe instructions; achieved = algorithmic count (DESIGN.md §6) x units / "
+                        "march duration (CUDA events); peak = measured register-resident DFMA rate on this GPU",
+                "march_ms": mk_ms, "march_share_of_step": mk_ms / (ms / a.steps), "algo_fp64_instr_per_unit": ALGO_FP64_INSTR_PER_UNIT,
+                "units_per_launch": units, "hbm_bytes_per_unit_algorithmic": 64.0,
+                "hbm_gbs_algorithmic": 64.0 * units / (mk_ms * 1e-3) / 1e9}
+
+    # end to end through the C ABI with HOST buffers: H2D of Delta, A_ind; iterate; D2H of Delta, A_ind + stats
+    hd = torch.empty((wl.ny, wl.nx), dtype=torch.complex128).pin_memory(); hd.copy_(delta)
+    hax = torch.zeros((wl.ny, wl.nx), dtype=torch.float64).pin_memory(); hay = torch.zeros_like(hax).pin_memory()
+    hax.copy_(aix); hay.copy_(aiy)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(a.steps):
+        delta.copy_(hd, non_blocking=True); aix.copy_(hax, non_blocking=True); aiy.copy_(hay, non_blocking=True)
+        st2 = ctx.sc_iterate(acc, 1.0, False, delta, aix, aiy, want_stats=True)
+        hd.copy_(delta, non_blocking=True); hax.copy_(aix, non_blocking=True); hay.copy_(aiy, non_blocking=True)
+        torch.cuda.synchronize()
+    e2e_s = (time.perf_counter() - t0) / a.steps
+    bytes_io = ng * 16 + 2 * ng * 8
+
+    value = n_updates * a.steps / (ms * 1e-3)
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": max(a.warmup, 3),
+            "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": config_of(wl, a, {"seconds_per_self_consistent_iteration": ms / a.steps / 1e3,
+                                                             "updates_per_step": n_updates, "updates_executed_per_step": st.n_updates_executed}),
+            "clocks": clocks,
+            "e2e": {"value": n_updates / e2e_s, "unit": UNIT, "h2d_bytes_per_step": bytes_io, "d2h_bytes_per_step": bytes_io + 64,
+                    "res_delta_last": st2.res_delta},
+            "gpu_launches": launches_per_step * a.steps, "roofline": roofline}
+    if not a.no_cpu_baseline and rank == 0:
+        cores = os.cpu_count() or 1
+        u, t, desc = oracle_sample(wl, cores)
+        line["cpu_baseline"] = {"value": u / t, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+    if rank == 0:
+        print(json.dumps(line))
+
+
+if __name__ == "__main__":
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)

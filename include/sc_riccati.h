@@ -137,6 +137,10 @@ sc_status sc_debug_math(sc_ctx* ctx, int n, double* max_rel_err);
  * roofline denominator of the march kernel). */
 sc_status sc_debug_fp64_peak(sc_ctx* ctx, double* dfma_per_s, double* sm_clock_mhz);
 
+/* Device time of the most recent march kernel launch (CUDA events recorded on the stream around that launch
+ * alone); synchronises.  Used by bench.py for the roofline of the dominant kernel. */
+sc_status sc_debug_last_march_ms(sc_ctx* ctx, float* ms);
+
 const char* sc_last_error(const sc_ctx* ctx);
 const char* sc_version(void);
 

@@ -101,6 +101,7 @@ def load_library():
     L.sc_debug_partial.argtypes = [vp, i, vp, vp, vp]
     L.sc_debug_math.argtypes = [vp, i, vp]
     L.sc_debug_fp64_peak.argtypes = [vp, C.POINTER(d), C.POINTER(d)]
+    L.sc_debug_last_march_ms.argtypes = [vp, C.POINTER(C.c_float)]
     _lib = L
     return L
 
@@ -258,6 +259,13 @@ class ScContext:
         out = np.zeros(6)
         self._check(self._L.sc_debug_math(self._h, n, out.ctypes.data_as(C.c_void_p)))
         return dict(zip(["rcp", "rsqrt", "exp", "expm1", "sin", "cosm1"], out))
+
+    def sc_debug_last_march_ms(self):
+        ms = C.c_float()
+        self._check(self._L.sc_debug_last_march_ms(self._h, C.byref(ms)))
+        return ms.value
+
+    last_march_ms = sc_debug_last_march_ms
 
     def sc_debug_fp64_peak(self):
         a, b = C.c_double(), C.c_double()

@@ -78,7 +78,7 @@ struct sc_ctx {
     // scratch
     DevBuf<double2> d_scrT, d_scrG; long long scr_stride = 0; int n_slots = 0;
     DevBuf<double> d_part; DevBuf<int> d_counter; DevBuf<int> d_nbad; DevBuf<double> d_statmax;
-    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr, evm0 = nullptr, evm1 = nullptr;
     // vector potential / driver state
     scf::FieldState fs;
 };
@@ -137,8 +137,10 @@ template <int MODE>
 sc_status launch_march(sc_ctx* ctx, const sck::MarchArgs& A, bool stats) {
     CU(cudaMemsetAsync(ctx->d_counter.p, 0, sizeof(int), ctx->stream));
     const int blocks = ctx->n_slots / sck::MARCH_WARPS;
+    CU(cudaEventRecord(ctx->evm0, ctx->stream));
     if (stats) sck::march_kernel<MODE, true><<<blocks, sck::MARCH_WARPS * 32, 0, ctx->stream>>>(A);
     else sck::march_kernel<MODE, false><<<blocks, sck::MARCH_WARPS * 32, 0, ctx->stream>>>(A);
+    CU(cudaEventRecord(ctx->evm1, ctx->stream));
     CU(cudaGetLastError());
     return SC_OK;
 }
@@ -272,7 +274,7 @@ sc_status sc_create(const sc_grid* grid, const unsigned char* mask, const sc_sha
     cudaDeviceProp prop; CU(cudaGetDeviceProperties(&prop, opts->device));
     ctx->n_sm = prop.multiProcessorCount;
     ctx->stream = (cudaStream_t)opts->cuda_stream;
-    CU(cudaEventCreate(&ctx->ev0)); CU(cudaEventCreate(&ctx->ev1));
+    CU(cudaEventCreate(&ctx->ev0)); CU(cudaEventCreate(&ctx->ev1)); CU(cudaEventCreate(&ctx->evm0)); CU(cudaEventCreate(&ctx->evm1));
 
     // ---- upload ----
     cudaStream_t s = ctx->stream;
@@ -315,6 +317,8 @@ sc_status sc_destroy(sc_ctx* ctx) {
     if (!ctx) return SC_ERR_ARG;
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
+    if (ctx->evm0) cudaEventDestroy(ctx->evm0);
+    if (ctx->evm1) cudaEventDestroy(ctx->evm1);
     scf::release(ctx->fs);
     delete ctx;
     return SC_OK;
@@ -552,6 +556,13 @@ sc_status sc_debug_math(sc_ctx* ctx, int n, double* max_rel_err) {
     CU(cudaGetLastError());
     CU(cudaMemcpyAsync(max_rel_err, d.p, 6 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
+    return SC_OK;
+}
+
+sc_status sc_debug_last_march_ms(sc_ctx* ctx, float* ms) {
+    if (!ctx || !ms) return SC_ERR_ARG;
+    CU(cudaEventSynchronize(ctx->evm1));
+    CU(cudaEventElapsedTime(ms, ctx->evm0, ctx->evm1));
     return SC_OK;
 }
 
