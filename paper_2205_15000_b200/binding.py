@@ -59,7 +59,8 @@ class SweepStats:
 
 
 def lib_path() -> str:
-    return os.path.join(_HERE, "libsc_riccati.so")
+    """In-tree library; SC_RICCATI_LIB overrides it (build-variant experiments)."""
+    return os.environ.get("SC_RICCATI_LIB") or os.path.join(_HERE, "libsc_riccati.so")
 
 
 def declared_symbols() -> list:

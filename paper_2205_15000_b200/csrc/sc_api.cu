@@ -71,12 +71,12 @@ struct sc_ctx {
     // fields
     DevBuf<double2> d_delta; DevBuf<double> d_Ax, d_Ay; bool have_A = false, have_fields = false;
     DevBuf<double> d_Aext_x, d_Aext_y; bool have_Aext = false;
-    DevBuf<double2> d_ndD; DevBuf<double> d_nda; bool nodes_fresh = false;
+    DevBuf<double2> d_ndD; DevBuf<double> d_nda; DevBuf<double4> d_pc; bool nodes_fresh = false;
     // energies and stores
     EnergySet mats;
     DevBuf<double2> d_store[2]; int cur = 0; bool stores_valid = false;
     // scratch
-    DevBuf<double2> d_scrT, d_scrG; long long scr_stride = 0; int n_slots = 0;
+    DevBuf<double4> d_scr; long long scr_stride = 0; int n_slots = 0;
     DevBuf<double> d_part; DevBuf<int> d_counter; DevBuf<int> d_nbad; DevBuf<double> d_statmax;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr, evm0 = nullptr, evm1 = nullptr;
     // vector potential / driver state
@@ -110,7 +110,7 @@ sc_status ensure_nodes(sc_ctx* ctx) {
     const int wpb = 8;
     sck::rotate_in_kernel<<<(ctx->G + wpb - 1) / wpb, wpb * 32, 0, ctx->stream>>>(
         grid_dev(ctx), traj_dev(ctx), ctx->d_vx.p, ctx->d_vy.p, ctx->d_eta.p, ctx->geo.c, ctx->opt.charge_sign,
-        ctx->d_ndD.p, ctx->d_nda.p, ctx->d_nbad.p);
+        ctx->d_ndD.p, ctx->d_nda.p, ctx->d_pc.p, ctx->d_nbad.p);
     if (!ctx->fb_rows.empty()) {
         const int n = (int)ctx->fb_rows.size();
         sck::fallback_kernel<<<(n + 127) / 128, 128, 0, ctx->stream>>>(grid_dev(ctx), n, ctx->d_fb_rows.p, ctx->d_fb_px.p,
@@ -123,12 +123,12 @@ sc_status ensure_nodes(sc_ctx* ctx) {
 
 sck::MarchArgs march_args(sc_ctx* ctx, const EnergySet& E, const double2* store_old, double2* store_new) {
     sck::MarchArgs A{};
-    A.T = traj_dev(ctx); A.E = E.dev(); A.order = ctx->d_order.p; A.n_items = ctx->G; A.h = ctx->grid.h;
-    A.nd_D = ctx->d_ndD.p; A.nd_a = ctx->d_nda.p; A.bc_mode = ctx->opt.bc_mode;
+    A.T = traj_dev(ctx); A.E = E.dev(); A.order = ctx->d_order.p; A.n_items = ctx->G;
+    A.nd_D = ctx->d_ndD.p; A.pc = ctx->d_pc.p; A.bc_mode = ctx->opt.bc_mode;
     A.ga_idx = ctx->d_ga_idx.p; A.ga_w = ctx->d_ga_w.p; A.ga_n = ctx->d_ga_n.p;
     A.fb_D = ctx->d_fb_D.p; A.fb_a = ctx->d_fb_a.p;
     A.store_old = store_old; A.store_new = store_new;
-    A.scr_T = ctx->d_scrT.p; A.scr_G = ctx->d_scrG.p; A.scr_stride = ctx->scr_stride;
+    A.scr = ctx->d_scr.p; A.scr_stride = ctx->scr_stride;
     A.part = ctx->d_part.p; A.ldos = nullptr; A.counter = ctx->d_counter.p; A.stat_max2 = ctx->d_statmax.p;
     return A;
 }
@@ -137,9 +137,16 @@ template <int MODE>
 sc_status launch_march(sc_ctx* ctx, const sck::MarchArgs& A, bool stats) {
     CU(cudaMemsetAsync(ctx->d_counter.p, 0, sizeof(int), ctx->stream));
     const int blocks = ctx->n_slots / sck::MARCH_WARPS;
+    const int smem = MODE == 0 ? sck::MARCH_SMEM : 0;
+    static bool attr_set = false;
+    if (MODE == 0 && !attr_set) {
+        CU(cudaFuncSetAttribute(sck::march_kernel<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        CU(cudaFuncSetAttribute(sck::march_kernel<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        attr_set = true;
+    }
     CU(cudaEventRecord(ctx->evm0, ctx->stream));
-    if (stats) sck::march_kernel<MODE, true><<<blocks, sck::MARCH_WARPS * 32, 0, ctx->stream>>>(A);
-    else sck::march_kernel<MODE, false><<<blocks, sck::MARCH_WARPS * 32, 0, ctx->stream>>>(A);
+    if (stats) sck::march_kernel<MODE, true><<<blocks, sck::MARCH_WARPS * 32, smem, ctx->stream>>>(A);
+    else sck::march_kernel<MODE, false><<<blocks, sck::MARCH_WARPS * 32, smem, ctx->stream>>>(A);
     CU(cudaEventRecord(ctx->evm1, ctx->stream));
     CU(cudaGetLastError());
     return SC_OK;
@@ -147,7 +154,7 @@ sc_status launch_march(sc_ctx* ctx, const sck::MarchArgs& A, bool stats) {
 
 sc_status reset_stores(sc_ctx* ctx, const EnergySet& E, double2* store) {
     const long long total = (long long)ctx->G * E.ne;
-    sck::reset_store_kernel<<<(unsigned)((total + 255) / 256), 256, 0, ctx->stream>>>(traj_dev(ctx), E.dev(), ctx->d_ndD.p, ctx->d_nda.p, store);
+    sck::reset_store_kernel<<<(unsigned)((total + 255) / 256), 256, 0, ctx->stream>>>(traj_dev(ctx), E.dev(), ctx->d_pc.p, store);
     CU(cudaGetLastError());
     return SC_OK;
 }
@@ -292,7 +299,7 @@ sc_status sc_create(const sc_grid* grid, const unsigned char* mask, const sc_sha
 
     const size_t ng = (size_t)grid->nx * grid->ny;
     CU(ctx->d_delta.alloc(ng)); CU(ctx->d_Ax.alloc(ng)); CU(ctx->d_Ay.alloc(ng));
-    CU(ctx->d_ndD.alloc(nodes)); CU(ctx->d_nda.alloc(nodes));
+    CU(ctx->d_ndD.alloc(nodes)); CU(ctx->d_nda.alloc(nodes)); CU(ctx->d_pc.alloc(nodes + G));
     CU(ctx->d_part.alloc((size_t)nodes * sck::RED_VALS));
     CU(ctx->d_counter.alloc(1)); CU(ctx->d_nbad.alloc(1));
     CU(cudaMemsetAsync(ctx->d_nbad.p, 0, sizeof(int), s));
@@ -303,10 +310,10 @@ sc_status sc_create(const sc_grid* grid, const unsigned char* mask, const sc_sha
     if (sc_status st = upload_energies(ctx, E)) return st;
     CU(ctx->d_store[0].alloc((size_t)ND * E.ne)); CU(ctx->d_store[1].alloc((size_t)ND * E.ne));
 
-    // persistent march grid: 2 CTAs of 8 warps per SM; per-warp scratch of (smax+1) pieces x 32 lanes
-    ctx->n_slots = ctx->n_sm * 2 * sck::MARCH_WARPS;
+    // persistent march grid: MARCH_MIN_CTAS CTAs of 8 warps per SM; per-warp scratch of (smax+1) pieces x 32 lanes
+    ctx->n_slots = ctx->n_sm * sck::MARCH_MIN_CTAS * sck::MARCH_WARPS;
     ctx->scr_stride = (long long)(smax + 2) * 32;
-    CU(ctx->d_scrT.alloc((size_t)ctx->n_slots * ctx->scr_stride)); CU(ctx->d_scrG.alloc((size_t)ctx->n_slots * ctx->scr_stride));
+    CU(ctx->d_scr.alloc((size_t)ctx->n_slots * ctx->scr_stride));
     CU(ctx->d_statmax.alloc(ctx->n_slots));
     CU(cudaMemsetAsync(ctx->d_statmax.p, 0, ctx->n_slots * sizeof(double), s));
     CU(cudaStreamSynchronize(s));

@@ -82,9 +82,12 @@ __device__ __forceinline__ double interp_plain(const GridDev& G, const double* F
     return acc;
 }
 
-// a2: one warp per trajectory, lanes over nodes (coalesced along the trajectory).
+// a2: one warp per trajectory, lanes over nodes (coalesced along the trajectory).  Also writes the PIECE
+// coefficients the march consumes: piece p of a trajectory with nn nodes (p = 0..nn) is {Re De, Im De, a, length}
+// with De, a the half-step values by linear interpolation and nearest-neighbour extrapolation at both ends
+// (reading R4).  Piece records of trajectory g start at noff[g] + g.
 __global__ void rotate_in_kernel(GridDev G, TrajDev T, const double* vx, const double* vy, const double* eta,
-                                 double c, int sigma, double2* nd_D, double* nd_a, int* n_bad) {
+                                 double c, int sigma, double2* nd_D, double* nd_a, double4* pc, int* n_bad) {
     const int g = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (g >= T.n) return;
     const int lane = threadIdx.x & 31;
@@ -99,6 +102,16 @@ __global__ void rotate_in_kernel(GridDev G, TrajDev T, const double* vx, const d
         if (!interp_delta(G, x, y, dr, di)) atomicAdd(n_bad, 1);
         nd_D[off + m] = make_double2(e * dr, e * di);
         nd_a[off + m] = sigma * (cx * interp_plain(G, G.Ax, x, y) + cy * interp_plain(G, G.Ay, x, y));
+    }
+    __syncwarp();
+    double4* P = pc + off + g;
+    for (int p = lane; p <= nn; p += 32) {
+        const int lo = p > 0 ? p - 1 : 0, hi = p < nn ? p : nn - 1;
+        const double2 Dl = nd_D[off + lo], Dh = nd_D[off + hi];
+        const double al = nd_a[off + lo], ah = nd_a[off + hi];
+        const double len = p == 0 ? T.l0[g] : (p == nn ? T.l1[g] : G.h);
+        P[p] = lo == hi ? make_double4(Dl.x, Dl.y, al, len)
+                        : make_double4(0.5 * (Dl.x + Dh.x), 0.5 * (Dl.y + Dh.y), 0.5 * (al + ah), len);
     }
 }
 
@@ -116,16 +129,15 @@ __global__ void fallback_kernel(GridDev G, int nfb, const int* rows, const doubl
 }
 
 // R8: store[dF][n] = gamma_h(last piece); store[dB][partner n] = conj(gamma-tilde_h(first piece)).
-__global__ void reset_store_kernel(TrajDev T, EnergyDev E, const double2* nd_D, const double* nd_a, double2* store) {
+__global__ void reset_store_kernel(TrajDev T, EnergyDev E, const double4* pc, double2* store) {
     const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= (long long)T.n * E.ne) return;
     const int g = (int)(idx / E.ne), n = (int)(idx % E.ne);
-    const long long off = T.noff[g];
-    const int nn = T.nn[g];
-    const double2 Dl = nd_D[off + nn - 1], D0 = nd_D[off];
-    const cplx ge = scm::gamma_hom(Dl.x, Dl.y, E.zr[n] + nd_a[off + nn - 1], E.zi[n]);
+    const double4* P = pc + T.noff[g] + g;
+    const double4 cl = P[T.nn[g]], c0 = P[0];
+    const cplx ge = scm::gamma_hom(cl.x, cl.y, E.zr[n] + cl.z, E.zi[n]);
     store[(size_t)T.dF[g] * E.ne + n] = make_double2(ge.re, ge.im);
-    const cplx gt = scm::gamma_hom(-D0.x, D0.y, E.zr[n] + nd_a[off], E.zi[n]);
+    const cplx gt = scm::gamma_hom(-c0.x, c0.y, E.zr[n] + c0.z, E.zi[n]);
     store[(size_t)T.dB[g] * E.ne + E.partner[n]] = make_double2(gt.re, -gt.im);
 }
 
@@ -136,22 +148,45 @@ struct MarchArgs {
     TrajDev T;
     EnergyDev E;
     const int* order; int n_items;          // longest-first work list
-    double h;
-    const double2* nd_D; const double* nd_a;
+    const double2* nd_D;                    // node coefficients Delta_j eta_k           [node]
+    const double4* pc;                      // piece coefficients {Re De, Im De, a, len} [node + g]
     int bc_mode;
     const int* ga_idx; const double* ga_w; const unsigned char* ga_n;   // entry gathers per store row [row][4]
     const double2* fb_D; const double* fb_a;
     const double2* store_old; double2* store_new;
-    double2* scr_T; double2* scr_G; long long scr_stride;   // per warp slot: (smax+1)*32 double2 each
-    double* part;                            // MODE 0: [node][6] = SF.re, SF.im, X2.re, X2.im, SG, SI
-    double* ldos;                            // MODE 1: [node][ne] = Re g_n
+    double4* scr; long long scr_stride;     // per warp slot: (smax+2)*32 entries {T.re, T.im, gt.re, gt.im}
+    double* part;                           // MODE 0: [node][6] = SF.re, SF.im, X2.re, X2.im, SG, SI
+    double* ldos;                           // MODE 1: [node][ne] = Re g_n
     int* counter;
-    double* stat_max2;                       // per warp slot: max |gamma|^2 seen (optional)
+    double* stat_max2;                      // per warp slot: max |gamma|^2 seen (optional)
 };
 
 constexpr int MARCH_WARPS = 8;               // warps per CTA
+#ifndef SC_MARCH_MIN_CTAS
+#define SC_MARCH_MIN_CTAS 2
+#endif
+constexpr int MARCH_MIN_CTAS = SC_MARCH_MIN_CTAS;   // resident CTAs per SM the register budget is sized for
+constexpr int PF_DIST = 12;                  // pass 2: scratch lines are pulled into L2 this many nodes ahead
 constexpr int RED_NODES = 4;                 // nodes per shared-memory reduction batch
 constexpr int RED_VALS = 6;
+constexpr int STAGE_LD = 33;                 // padded row of the transpose stage: conflict-free rows AND columns
+constexpr int MARCH_SMEM = MARCH_WARPS * RED_NODES * RED_VALS * STAGE_LD * (int)sizeof(double);   // 50688 B (> 48 KB: opt-in)
+
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+// 256-bit global accesses (LDG.E.ENL2.256 / STG.E.ENL2.256 on sm_100a): one scratch entry per lane per instruction
+__device__ __forceinline__ double4 ld256(const double4* p) {
+    double4 v;
+    asm volatile("ld.global.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v.x), "=d"(v.y), "=d"(v.z), "=d"(v.w) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ void st256(double4* p, double a, double b, double c, double d) {
+    asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
+}
+__device__ __forceinline__ double4 ldu256(const double4* p) {      // warp-uniform coefficient record (read-only path)
+    double4 v;
+    asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v.x), "=d"(v.y), "=d"(v.z), "=d"(v.w) : "l"(p));
+    return v;
+}
 
 __device__ __forceinline__ cplx gather_start(const MarchArgs& A, int row, int n) {
     const int cnt = A.ga_n[row];
@@ -164,15 +199,44 @@ __device__ __forceinline__ cplx gather_start(const MarchArgs& A, int row, int n)
     return mk(sr, si);
 }
 
+// products at one node (Eq. 24 :165): P = gamma gamma~, 1/(1+P); writes the six weighted terms of the
+// energy sums into rows r..r+5 of the warp's transpose stage (MODE 0), or returns Re g (MODE 1)
+template <int MODE, bool STATS>
+__device__ __forceinline__ double node_products(cplx gm, double gtr, double gti, double2 Dn, double wn, double* st, double& max2) {
+    const double Pr = fma(gm.re, gtr, -gm.im * gti), Pi = fma(gm.re, gti, gm.im * gtr);
+    const double qr = 1.0 + Pr;
+    const double rq = scm::rcp_nr(fma(qr, qr, Pi * Pi));
+    const double ir = qr * rq, ii = -Pi * rq;               // 1/(1+P)
+    if (STATS) max2 = fmax(max2, fmax(fma(gm.re, gm.re, gm.im * gm.im), fma(gtr, gtr, gti * gti)));
+    if (MODE == 0) {
+        const double wr = wn * ir, wi = wn * ii;
+        st[0 * STAGE_LD] = fma(gm.re, wr, -gm.im * wi);      // SF  = w gamma/(1+P)
+        st[1 * STAGE_LD] = fma(gm.re, wi, gm.im * wr);
+        st[2 * STAGE_LD] = fma(gtr, wr, -gti * wi);          // X2  = w gamma~/(1+P)  (SF of k+N/2 = conj)
+        st[3 * STAGE_LD] = fma(gtr, wi, gti * wr);
+        st[4 * STAGE_LD] = 2.0 * wi;                         // SG  = w Im g = 2 w Im 1/(1+P)
+        st[5 * STAGE_LD] = wn * fma(Dn.x, gm.im - gti, -Dn.y * (gm.re + gtr));   // SI (Eq. 19 :128 numerator)
+    }
+    return fma(2.0, ir, -1.0);                               // Re g = 2 Re 1/(1+P) - 1
+}
+
+// column sums of the stage: lane c < cnt sums row c over the 32 lanes (4 partial sums, fixed order)
+__device__ __forceinline__ double stage_colsum(const double* stage, int lane) {
+    const double* col = stage + lane * STAGE_LD;
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+#pragma unroll
+    for (int i = 0; i < 32; i += 4) { s0 += col[i]; s1 += col[i + 1]; s2 += col[i + 2]; s3 += col[i + 3]; }
+    return (s0 + s1) + (s2 + s3);
+}
+
 // MODE 0: Matsubara sums; 1: per-energy Re g (LDOS); 2: boundary values only.
 template <int MODE, bool STATS>
-__global__ void __launch_bounds__(MARCH_WARPS * 32, 2) march_kernel(MarchArgs A) {
-    __shared__ double stage_all[MARCH_WARPS][RED_NODES * RED_VALS][32];
+__global__ void __launch_bounds__(MARCH_WARPS * 32, MARCH_MIN_CTAS) march_kernel(MarchArgs A) {
+    extern __shared__ double stage_all[];        // MODE 0: MARCH_WARPS x (24 rows x STAGE_LD) doubles (MARCH_SMEM bytes)
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const int slot = blockIdx.x * MARCH_WARPS + wib;
-    double (*stage)[32] = stage_all[wib];
-    double2* __restrict__ sT = A.scr_T + (size_t)slot * A.scr_stride;
-    double2* __restrict__ sG = A.scr_G + (size_t)slot * A.scr_stride;
+    double* const stage = stage_all + wib * (RED_NODES * RED_VALS * STAGE_LD);
+    double4* const scr = A.scr + (size_t)slot * A.scr_stride + lane;     // entry e of this lane: scr[e*32]
     const int ne = A.E.ne;
     double max2 = 0.0;
 
@@ -184,10 +248,9 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32, 2) march_kernel(MarchArgs A)
         const int g = A.order[item];
         const int nn = A.T.nn[g];
         const long long noff = A.T.noff[g];
-        const double l0 = A.T.l0[g], l1 = A.T.l1[g];
         const int dF = A.T.dF[g], dB = A.T.dB[g];
         const double2* __restrict__ ND = A.nd_D + noff;
-        const double* __restrict__ NA = A.nd_a + noff;
+        const double4* __restrict__ PC = A.pc + noff + g;
 
         for (int n0 = 0; n0 < ne; n0 += 32) {
             const bool act = n0 + lane < ne;
@@ -196,11 +259,11 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32, 2) march_kernel(MarchArgs A)
             const double wn = act ? A.E.w[n] : 0.0;
             const int nb = A.E.partner[n];
 
-            // ---------------- pass 1: gamma-tilde from u_out down to u_in; record T and gamma-tilde ----------
-            double2 Dhi = ND[nn - 1]; double ahi = NA[nn - 1];
+            // ---------------- pass 1: gamma-tilde from u_out down to u_in; entry p = {T_p, gamma~(node p-1)} ----------
+            double4 c4 = ldu256(PC + nn);
             cplx gt;
             if (A.bc_mode == 1) {
-                gt = scm::gamma_hom(-Dhi.x, Dhi.y, zr0 + ahi, zi0);
+                gt = scm::gamma_hom(-c4.x, c4.y, zr0 + c4.z, zi0);
             } else if (A.ga_n[dB]) {
                 const cplx s = gather_start(A, dB, nb);            // gamma of the mirrored trajectory at its entry
                 gt = mk(s.re, -s.im);
@@ -209,93 +272,88 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32, 2) march_kernel(MarchArgs A)
                 gt = mk(s.re, -s.im);
             }
             {
-                // piece nn: [u_jl, u_out], coefficients of node nn-1 (nearest-neighbour extrapolation, :1003)
-                const double zr = zr0 + ahi;
-                const cplx T = scm::coef_T(fma(Dhi.x, Dhi.x, Dhi.y * Dhi.y), zr, zi0, l1);
-                gt = scm::step_T(gt, -Dhi.x, Dhi.y, zr, zi0, T);
-                sT[(size_t)nn * 32 + lane] = make_double2(T.re, T.im);
-                sG[(size_t)(nn - 1) * 32 + lane] = make_double2(gt.re, gt.im);
-            }
-            double2 Dnx = nn >= 2 ? ND[nn - 2] : Dhi; double anx = nn >= 2 ? NA[nn - 2] : ahi;
-            for (int m = nn - 1; m >= 1; --m) {
-                // piece m: [u_{m-1}, u_m], half-step coefficients by linear interpolation (:1003)
-                const double2 Dlo = Dnx; const double alo = anx;
-                if (m >= 2) { Dnx = ND[m - 2]; anx = NA[m - 2]; }          // prefetch for the next iteration
-                const double Dr = 0.5 * (Dlo.x + Dhi.x), Di = 0.5 * (Dlo.y + Dhi.y);
-                const double zr = zr0 + 0.5 * (alo + ahi);
-                const cplx T = scm::coef_T(fma(Dr, Dr, Di * Di), zr, zi0, A.h);
-                gt = scm::step_T(gt, -Dr, Di, zr, zi0, T);
-                sT[(size_t)m * 32 + lane] = make_double2(T.re, T.im);
-                sG[(size_t)(m - 1) * 32 + lane] = make_double2(gt.re, gt.im);
-                Dhi = Dlo; ahi = alo;
-            }
-            {
-                // piece 0: [u_in, u_jf], coefficients of node 0
-                const double zr = zr0 + ahi;
-                const cplx T = scm::coef_T(fma(Dhi.x, Dhi.x, Dhi.y * Dhi.y), zr, zi0, l0);
-                gt = scm::step_T(gt, -Dhi.x, Dhi.y, zr, zi0, T);
-                sT[lane] = make_double2(T.re, T.im);
+                double4* e = scr + (size_t)nn * 32;
+                double4 cn = ldu256(PC + (nn >= 1 ? nn - 1 : 0));
+#pragma unroll 2
+                for (int p = nn; p >= 0; --p) {
+                    const double4 cc = c4;
+                    c4 = cn;
+                    if (p >= 2) cn = ldu256(PC + p - 2);                       // coefficient record two pieces ahead
+                    const double zr = zr0 + cc.z;
+                    const cplx T = scm::coef_T(fma(cc.x, cc.x, cc.y * cc.y), zr, zi0, cc.w);
+                    gt = scm::step_T(gt, -cc.x, cc.y, zr, zi0, T);
+                    st256(e, T.re, T.im, gt.re, gt.im);
+                    e -= 32;
+                }
                 if (act) A.store_new[(size_t)dB * ne + nb] = make_double2(gt.re, -gt.im);
             }
 
             // ---------------- pass 2: gamma from u_in up to u_out; products and energy reduction ------------
             cplx gm;
-            double2 Dlo = Dhi; double alo = ahi;        // node 0
-            if (A.bc_mode == 1) gm = scm::gamma_hom(Dlo.x, Dlo.y, zr0 + alo, zi0);
-            else if (A.ga_n[dF]) gm = gather_start(A, dF, n);
-            else gm = scm::gamma_hom(A.fb_D[dF].x, A.fb_D[dF].y, zr0 + A.fb_a[dF], zi0);
             {
-                const double2 t = sT[lane];
-                gm = scm::step_T(gm, Dlo.x, Dlo.y, zr0 + alo, zi0, mk(t.x, t.y));
+                const double4 c0 = ldu256(PC);
+                if (A.bc_mode == 1) gm = scm::gamma_hom(c0.x, c0.y, zr0 + c0.z, zi0);
+                else if (A.ga_n[dF]) gm = gather_start(A, dF, n);
+                else gm = scm::gamma_hom(A.fb_D[dF].x, A.fb_D[dF].y, zr0 + A.fb_a[dF], zi0);
+                const double4 e0 = ld256(scr);
+                gm = scm::step_T(gm, c0.x, c0.y, zr0 + c0.z, zi0, mk(e0.x, e0.y));
             }
-            double2 Tn = sT[(size_t)1 * 32 + lane];
-            double2 Gn = sG[lane];
-            double2 Dn2 = nn >= 2 ? ND[1] : Dlo; double an2 = nn >= 2 ? NA[1] : alo;
-            for (int m = 0; m < nn; ++m) {
-                // node m: gm = gamma(u_m), Gn = gamma-tilde(u_m), (Dlo, alo) = node coefficients
-                const double2 Tc = Tn; const double2 Gc = Gn;
-                if (m + 1 < nn) { Tn = sT[(size_t)(m + 2) * 32 + lane]; Gn = sG[(size_t)(m + 1) * 32 + lane]; }
-                if (MODE != 2) {
-                    const double Pr = fma(gm.re, Gc.x, -gm.im * Gc.y), Pi = fma(gm.re, Gc.y, gm.im * Gc.x);
-                    const double qr = 1.0 + Pr;
-                    const double rq = scm::rcp_nr(fma(qr, qr, Pi * Pi));
-                    const double ir = qr * rq, ii = -Pi * rq;               // 1/(1+P)
-                    if (STATS) max2 = fmax(max2, fmax(fma(gm.re, gm.re, gm.im * gm.im), fma(Gc.x, Gc.x, Gc.y * Gc.y)));
-                    if (MODE == 0) {
-                        const double wr = wn * ir, wi = wn * ii;
-                        const int r = (m & (RED_NODES - 1)) * RED_VALS;
-                        stage[r + 0][lane] = fma(gm.re, wr, -gm.im * wi);    // SF  = w gamma/(1+P)
-                        stage[r + 1][lane] = fma(gm.re, wi, gm.im * wr);
-                        stage[r + 2][lane] = fma(Gc.x, wr, -Gc.y * wi);      // X2  = w gamma~/(1+P)  (SF of k+N/2 = conj)
-                        stage[r + 3][lane] = fma(Gc.x, wi, Gc.y * wr);
-                        stage[r + 4][lane] = 2.0 * wi;                       // SG  = w Im g = 2 w Im 1/(1+P)
-                        stage[r + 5][lane] = wn * fma(Dlo.x, gm.im - Gc.y, -Dlo.y * (gm.re + Gc.x));   // SI
-                        if ((m & (RED_NODES - 1)) == RED_NODES - 1 || m == nn - 1) {
-                            __syncwarp();
-                            const int cnt = ((m & (RED_NODES - 1)) + 1) * RED_VALS;
-                            if (lane < cnt) {
-                                double s = 0.0;
-#pragma unroll 8
-                                for (int i = 0; i < 32; ++i) s += stage[lane][(i + lane) & 31];
-                                double* dst = A.part + (size_t)(noff + (m & ~(RED_NODES - 1))) * RED_VALS + lane;
-                                if (n0) s += *dst;
-                                *dst = s;
-                            }
-                            __syncwarp();
-                        }
-                    } else if (act) {
-                        A.ldos[(size_t)(noff + m) * ne + n] = fma(2.0, ir, -1.0);   // Re g = 2 Re 1/(1+P) - 1
+            const double4* e = scr + 32;                 // entry of node 0
+            for (int q = 4; q < PF_DIST && q < nn; q += 4) prefetch_l2((const char*)(e - lane) + (size_t)q * 1024 + lane * 128);
+            double4 En = ld256(e);
+            double4 cN = ldu256(PC + 1);
+            double2 dN = ND[0];
+            int m = 0;
+            for (; m + RED_NODES <= nn; m += RED_NODES) {
+                if (m + PF_DIST < nn) prefetch_l2((const char*)(e - lane) + (size_t)PF_DIST * 1024 + lane * 128);
+                double part_old = 0.0;
+                if (MODE == 0 && n0 && lane < RED_NODES * RED_VALS) part_old = A.part[(size_t)(noff + m) * RED_VALS + lane];
+#pragma unroll
+                for (int b = 0; b < RED_NODES; ++b) {
+                    const double4 Ec = En; const double4 cc = cN; const double2 dc = dN;
+                    En = ld256(e + (b + 1) * 32);                // one node ahead (scratch has 2 spare entries)
+                    cN = ldu256(PC + m + b + 2 <= PC + nn ? PC + m + b + 2 : PC + nn);
+                    dN = ND[m + b + 1 < nn ? m + b + 1 : nn - 1];
+                    if (MODE != 2) {
+                        const double rg = node_products<MODE, STATS>(gm, Ec.z, Ec.w, dc, wn, stage + b * RED_VALS * STAGE_LD + lane, max2);
+                        if (MODE == 1 && act) A.ldos[(size_t)(noff + m + b) * ne + n] = rg;
                     }
+                    gm = scm::step_T(gm, cc.x, cc.y, zr0 + cc.z, zi0, mk(Ec.x, Ec.y));
                 }
-                // step to node m+1 (or to u_out)
-                if (m + 1 < nn) {
-                    const double2 Dhi2 = Dn2; const double ahi2 = an2;
-                    if (m + 2 < nn) { Dn2 = ND[m + 2]; an2 = NA[m + 2]; }
-                    const double Dr = 0.5 * (Dlo.x + Dhi2.x), Di = 0.5 * (Dlo.y + Dhi2.y);
-                    gm = scm::step_T(gm, Dr, Di, zr0 + 0.5 * (alo + ahi2), zi0, mk(Tc.x, Tc.y));
-                    Dlo = Dhi2; alo = ahi2;
-                } else {
-                    gm = scm::step_T(gm, Dlo.x, Dlo.y, zr0 + alo, zi0, mk(Tc.x, Tc.y));
+                e += RED_NODES * 32;
+                if (MODE == 0) {
+                    __syncwarp();
+                    if (lane < RED_NODES * RED_VALS) {
+                        double s = stage_colsum(stage, lane);
+                        if (n0) s += part_old;
+                        A.part[(size_t)(noff + m) * RED_VALS + lane] = s;
+                    }
+                    __syncwarp();
+                }
+            }
+            if (m < nn) {                                        // ragged tail: 1..3 nodes
+                const int rem = nn - m;
+                double part_old = 0.0;
+                if (MODE == 0 && n0 && lane < rem * RED_VALS) part_old = A.part[(size_t)(noff + m) * RED_VALS + lane];
+                for (int b = 0; b < rem; ++b) {
+                    const double4 Ec = En; const double4 cc = cN; const double2 dc = dN;
+                    En = ld256(e + (b + 1) * 32);
+                    cN = ldu256(PC + m + b + 2 <= PC + nn ? PC + m + b + 2 : PC + nn);
+                    dN = ND[m + b + 1 < nn ? m + b + 1 : nn - 1];
+                    if (MODE != 2) {
+                        const double rg = node_products<MODE, STATS>(gm, Ec.z, Ec.w, dc, wn, stage + b * RED_VALS * STAGE_LD + lane, max2);
+                        if (MODE == 1 && act) A.ldos[(size_t)(noff + m + b) * ne + n] = rg;
+                    }
+                    gm = scm::step_T(gm, cc.x, cc.y, zr0 + cc.z, zi0, mk(Ec.x, Ec.y));
+                }
+                if (MODE == 0) {
+                    __syncwarp();
+                    if (lane < rem * RED_VALS) {
+                        double s = stage_colsum(stage, lane);
+                        if (n0) s += part_old;
+                        A.part[(size_t)(noff + m) * RED_VALS + lane] = s;
+                    }
+                    __syncwarp();
                 }
             }
             if (act) A.store_new[(size_t)dF * ne + n] = make_double2(gm.re, gm.im);
@@ -444,34 +502,30 @@ __global__ void rotate_back_ldos_kernel(BackLdosArgs L) {
 // re-march one trajectory for one energy with the same device functions; writes gamma, gamma-tilde per node
 __global__ void debug_traj_kernel(MarchArgs A, int g, int n, double2* outG, double2* outGT) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
-    const int nn = A.T.nn[g]; const long long noff = A.T.noff[g];
-    const double2* ND = A.nd_D + noff; const double* NA = A.nd_a + noff;
+    const int nn = A.T.nn[g];
+    const double4* PC = A.pc + A.T.noff[g] + g;
     const int nb = A.E.partner[n];
     const double zr0 = A.E.zr[n], zi0 = A.E.zi[n];
     const int dF = A.T.dF[g], dB = A.T.dB[g];
     cplx gt;
-    if (A.bc_mode == 1) gt = scm::gamma_hom(-ND[nn - 1].x, ND[nn - 1].y, zr0 + NA[nn - 1], zi0);
+    if (A.bc_mode == 1) gt = scm::gamma_hom(-PC[nn].x, PC[nn].y, zr0 + PC[nn].z, zi0);
     else if (A.ga_n[dB]) { cplx s = gather_start(A, dB, nb); gt = mk(s.re, -s.im); }
     else { cplx s = scm::gamma_hom(A.fb_D[dB].x, A.fb_D[dB].y, A.E.zr[nb] + A.fb_a[dB], A.E.zi[nb]); gt = mk(s.re, -s.im); }
-    for (int m = nn; m >= 1; --m) {
-        double Dr, Di, a, len;
-        if (m == nn) { Dr = ND[nn - 1].x; Di = ND[nn - 1].y; a = NA[nn - 1]; len = A.T.l1[g]; }
-        else { Dr = 0.5 * (ND[m - 1].x + ND[m].x); Di = 0.5 * (ND[m - 1].y + ND[m].y); a = 0.5 * (NA[m - 1] + NA[m]); len = A.h; }
-        const cplx T = scm::coef_T(Dr * Dr + Di * Di, zr0 + a, zi0, len);
-        gt = scm::step_T(gt, -Dr, Di, zr0 + a, zi0, T);
-        outGT[m - 1] = make_double2(gt.re, gt.im);
+    for (int p = nn; p >= 1; --p) {
+        const double4 c = PC[p];
+        const cplx T = scm::coef_T(c.x * c.x + c.y * c.y, zr0 + c.z, zi0, c.w);
+        gt = scm::step_T(gt, -c.x, c.y, zr0 + c.z, zi0, T);
+        outGT[p - 1] = make_double2(gt.re, gt.im);
     }
     cplx gm;
-    if (A.bc_mode == 1) gm = scm::gamma_hom(ND[0].x, ND[0].y, zr0 + NA[0], zi0);
+    if (A.bc_mode == 1) gm = scm::gamma_hom(PC[0].x, PC[0].y, zr0 + PC[0].z, zi0);
     else if (A.ga_n[dF]) gm = gather_start(A, dF, n);
     else gm = scm::gamma_hom(A.fb_D[dF].x, A.fb_D[dF].y, zr0 + A.fb_a[dF], zi0);
-    for (int m = 0; m < nn; ++m) {
-        double Dr, Di, a, len;
-        if (m == 0) { Dr = ND[0].x; Di = ND[0].y; a = NA[0]; len = A.T.l0[g]; }
-        else { Dr = 0.5 * (ND[m - 1].x + ND[m].x); Di = 0.5 * (ND[m - 1].y + ND[m].y); a = 0.5 * (NA[m - 1] + NA[m]); len = A.h; }
-        const cplx T = scm::coef_T(Dr * Dr + Di * Di, zr0 + a, zi0, len);
-        gm = scm::step_T(gm, Dr, Di, zr0 + a, zi0, T);
-        outG[m] = make_double2(gm.re, gm.im);
+    for (int p = 0; p < nn; ++p) {
+        const double4 c = PC[p];
+        const cplx T = scm::coef_T(c.x * c.x + c.y * c.y, zr0 + c.z, zi0, c.w);
+        gm = scm::step_T(gm, c.x, c.y, zr0 + c.z, zi0, T);
+        outG[p] = make_double2(gm.re, gm.im);
     }
 }
 

@@ -14,6 +14,17 @@
 
 namespace scm {
 
+// polynomial coefficients live in constant memory so that the DFMAs take them as c[bank][offset] operands
+// instead of re-materialising 64-bit immediates with two UMOVs each
+__constant__ double kExp[12] = {1.6059043836821613e-10, 2.08767569878681e-09, 2.505210838544172e-08, 2.755731922398589e-07,
+                                2.7557319223985893e-06, 2.48015873015873e-05, 1.984126984126984e-04, 1.388888888888889e-03,
+                                8.333333333333333e-03, 4.1666666666666664e-02, 1.6666666666666666e-01, 0.5};   // 1/13! .. 1/2!
+__constant__ double kSin[6] = {1.58969099521155010221e-10, -2.50507602534068634195e-08, 2.75573137070700676789e-06,
+                               -1.98412698298579493134e-04, 8.33333333332248946124e-03, -1.66666666666666324348e-01};
+__constant__ double kCos[6] = {-1.13596475577881948265e-11, 2.08757232129817482790e-09, -2.75573143513906633035e-07,
+                               2.48015872894767294178e-05, -1.38888888888741095749e-03, 4.16666666666666019037e-02};
+__constant__ double kRed[4] = {1.4426950408889634074, 6.93147180369123816490e-01, 1.90821492927058770002e-10, 6755399441055744.0};
+
 struct cplx { double re, im; };
 
 __device__ __forceinline__ cplx mk(double a, double b) { cplx r; r.re = a; r.im = b; return r; }
@@ -49,9 +60,7 @@ __device__ __forceinline__ double rsqrt_nr(double x) {
 
 // ex = exp(x), xm1 = exp(x) - 1 without cancellation, for x <= ~0 (any x > -700 works; x <= -700 -> 0, -1)
 __device__ __forceinline__ void exp_pair(double x, double& ex, double& xm1) {
-    const double L2E = 1.4426950408889634074;
-    const double LN2_HI = 6.93147180369123816490e-01, LN2_LO = 1.90821492927058770002e-10;
-    const double MAGIC = 6755399441055744.0;   // 1.5 * 2^52: adds round the product to an integer
+    const double L2E = kRed[0], LN2_HI = kRed[1], LN2_LO = kRed[2], MAGIC = kRed[3];   // MAGIC = 1.5 * 2^52
     x = fmax(x, -700.0);
     double kf = fma(x, L2E, MAGIC);
     const int k = __double2loint(kf);
@@ -59,18 +68,9 @@ __device__ __forceinline__ void exp_pair(double x, double& ex, double& xm1) {
     double r = fma(-kf, LN2_HI, x);
     r = fma(-kf, LN2_LO, r);
     // expm1(r) = r + r^2 (1/2 + r/6 + ... + r^11/13!), |r| <= ln2/2: truncation < 5e-18
-    double p = 1.6059043836821613e-10;                  // 1/13!
-    p = fma(p, r, 2.08767569878681e-09);                // 1/12!
-    p = fma(p, r, 2.505210838544172e-08);               // 1/11!
-    p = fma(p, r, 2.755731922398589e-07);               // 1/10!
-    p = fma(p, r, 2.7557319223985893e-06);              // 1/9!
-    p = fma(p, r, 2.48015873015873e-05);                // 1/8!
-    p = fma(p, r, 1.984126984126984e-04);               // 1/7!
-    p = fma(p, r, 1.388888888888889e-03);               // 1/6!
-    p = fma(p, r, 8.333333333333333e-03);               // 1/5!
-    p = fma(p, r, 4.1666666666666664e-02);              // 1/4!
-    p = fma(p, r, 1.6666666666666666e-01);              // 1/3!
-    p = fma(p, r, 0.5);
+    double p = kExp[0];
+#pragma unroll
+    for (int i = 1; i < 12; ++i) p = fma(p, r, kExp[i]);
     const double r2 = r * r;
     p = fma(p, r2, r);                                  // expm1(r)
     const double s = __hiloint2double((k + 1023) << 20, 0);   // 2^k, k in [-1010, 0]
@@ -81,19 +81,10 @@ __device__ __forceinline__ void exp_pair(double x, double& ex, double& xm1) {
 // s = sin(y), cm1 = cos(y) - 1 for |y| <= pi/4 (minimax kernels of the classic fdlibm k_sin/k_cos)
 __device__ __forceinline__ void sincos_small(double y, double& s, double& cm1) {
     const double z = y * y;
-    double ps = 1.58969099521155010221e-10;
-    ps = fma(ps, z, -2.50507602534068634195e-08);
-    ps = fma(ps, z, 2.75573137070700676789e-06);
-    ps = fma(ps, z, -1.98412698298579493134e-04);
-    ps = fma(ps, z, 8.33333333332248946124e-03);
-    ps = fma(ps, z, -1.66666666666666324348e-01);
+    double ps = kSin[0], pc = kCos[0];
+#pragma unroll
+    for (int i = 1; i < 6; ++i) { ps = fma(ps, z, kSin[i]); pc = fma(pc, z, kCos[i]); }
     s = fma(y * z, ps, y);
-    double pc = -1.13596475577881948265e-11;
-    pc = fma(pc, z, 2.08757232129817482790e-09);
-    pc = fma(pc, z, -2.75573143513906633035e-07);
-    pc = fma(pc, z, 2.48015872894767294178e-05);
-    pc = fma(pc, z, -1.38888888888741095749e-03);
-    pc = fma(pc, z, 4.16666666666666019037e-02);
     cm1 = fma(z * z, pc, -0.5 * z);
 }
 
