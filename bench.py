@@ -83,6 +83,7 @@ def parse():
     ap.add_argument("--size-scale", type=float, default=1.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep-only", action="store_true", help="time sc_riccati_sweep alone (profiling aid)")
+    ap.add_argument("--stepper", type=int, default=0, help="0 closed-form step (north_star), 1 the paper's implicit mid-point rule")
     return ap.parse_args()
 
 
@@ -158,16 +159,18 @@ def run_ours(a):
 
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    import torch.distributed as dist
     if world > 1:
-        import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     torch.cuda.set_device(local)
     devname = f"cuda:{local}"
     wl = workload_from_args(a)
+    ctx = sc.ScContext.from_workload(wl, device=local, stepper=a.stepper)
     if world > 1:
-        raise SystemExit("multi-GPU energy sharding is not built yet (DESIGN.md §8): run with --gpus 1")
-
-    ctx = sc.ScContext.from_workload(wl, device=local)
+        # energy sharding: this rank marches its slice of the Matsubara table; one NCCL all-reduce of the
+        # five accumulator fields per sweep; A-solve and mixing are replicated (deterministic, identical on all ranks)
+        from paper_2205_15000_b200 import sharding
+        sharding.attach(ctx, wl.t, wl.n_energies)
     dev = lambda x: torch.as_tensor(np.ascontiguousarray(x), device=devname)
     ng = wl.nx * wl.ny
     delta = dev(wl.delta0.astype(np.complex128))
@@ -194,22 +197,34 @@ def run_ours(a):
     sampler = ClockSampler(local); sampler.start()
     e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
     march_ms = []
+    if world > 1:
+        dist.barrier()
     torch.cuda.synchronize()
     e0.record()
     for _ in range(a.steps):
         step()
     e1.record()
     torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
     ms = e0.elapsed_time(e1)
     clocks = sampler.stop()
+    if world > 1:                                   # device time of the slowest rank
+        tmax = torch.tensor([ms], dtype=torch.float64, device=devname)
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        ms = float(tmax.item())
 
     # per-kernel duration of the dominant kernel (the march), CUDA events on the launching stream, same inputs
     ctx.sc_set_fields(delta, dev_ax if wl.kappa <= 0 else None, dev_ay if wl.kappa <= 0 else None)
     for _ in range(2):
         st = ctx.sc_riccati_sweep(dn, jx, jy, fe, want_stats=True)
         march_ms.append(ctx.last_march_ms())
-    n_updates = st.n_updates
-    units = n_updates / 4.0                       # (node, energy, angle-pair) units incl. the boundary pieces
+    units = st.n_updates / 4.0                    # this rank's (node, energy, angle-pair) units incl. the boundary pieces
+    n_updates, n_exec = st.n_updates, st.n_updates_executed
+    if world > 1:                                 # whole-job updates = sum over the energy shards
+        tot = torch.tensor([n_updates, n_exec], dtype=torch.float64, device=devname)
+        dist.all_reduce(tot)
+        n_updates, n_exec = int(tot[0].item()), int(tot[1].item())
     peak_dfma, clk = ctx.sc_debug_fp64_peak()
     mk_ms = float(np.mean(march_ms))
     achieved = 2.0 * ALGO_FP64_INSTR_PER_UNIT * units / (mk_ms * 1e-3) / 1e12
@@ -234,13 +249,19 @@ def run_ours(a):
         hd.copy_(delta, non_blocking=True); hax.copy_(aix, non_blocking=True); hay.copy_(aiy, non_blocking=True)
         torch.cuda.synchronize()
     e2e_s = (time.perf_counter() - t0) / a.steps
+    if world > 1:
+        tmax = torch.tensor([e2e_s], dtype=torch.float64, device=devname)
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        e2e_s = float(tmax.item())
     bytes_io = ng * 16 + 2 * ng * 8
 
     value = n_updates * a.steps / (ms * 1e-3)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": max(a.warmup, 3),
             "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic", "config": config_of(wl, a, {"seconds_per_self_consistent_iteration": ms / a.steps / 1e3,
-                                                             "updates_per_step": n_updates, "updates_executed_per_step": st.n_updates_executed}),
+                                                             "updates_per_step": n_updates, "updates_executed_per_step": n_exec,
+                                                             "stepper": "closed-form" if a.stepper == 0 else "implicit mid-point",
+                                                             "parallelism": f"energy-sharded x{world}, 1 all-reduce/sweep" if world > 1 else "single GPU"}),
             "clocks": clocks,
             "e2e": {"value": n_updates / e2e_s, "unit": UNIT, "h2d_bytes_per_step": bytes_io, "d2h_bytes_per_step": bytes_io + 64,
                     "res_delta_last": st2.res_delta},
@@ -251,6 +272,9 @@ def run_ours(a):
         line["cpu_baseline"] = {"value": u / t, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
     if rank == 0:
         print(json.dumps(line))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
 
 
 if __name__ == "__main__":

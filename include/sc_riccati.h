@@ -54,7 +54,7 @@ typedef struct {
     int n_angles;        /* N_phi, even; phi_k = 2 pi k / N_phi (:189) */
     int n_matsubara;     /* N_eps; eps_n = t (n + 1/2), n = 0..N_eps-1 (:98) */
     int precision;       /* 64 (default) or 32: arithmetic of the march; ABI buffers stay fp64 */
-    int stepper;         /* 0 = closed-form step (:982); 1 = implicit mid-point C4-C9 (:984-1001) (not yet built) */
+    int stepper;         /* 0 = closed-form step (:982); 1 = implicit mid-point C4-C9 (:984-1001) */
     int quadrature;      /* 0 = paper's rule: Boole / Simpson 3/8 / Simpson 1/3 / trapezoid by N_phi mod 4,3,2 (:189); 1 = trapezoid */
     int charge_sign;     /* sigma_e = -1 for electrons (:43, :890) */
     int bc_mode;         /* 0 = specular (:155); 1 = bulk: every start value is the local homogeneous solution */
@@ -82,6 +82,22 @@ sc_status sc_destroy(sc_ctx* ctx);
 /* Set Delta(R) (dev, complex fp64 [ny][nx]) and the TOTAL vector potential A = A_ext + A_ind (dev fp64
  * [ny][nx] each; NULL = 0).  Copies into context-owned buffers; does not touch the boundary stores. */
 sc_status sc_set_fields(sc_ctx* ctx, const void* delta, const double* Ax, const double* Ay);
+
+/* Replace the Matsubara table by any energies z_n = z_re + i z_im (Im z > 0) with weights w_n (host, n values):
+ * Ozaki poles (:207, reading R-A4), or ONE SHARD of the Matsubara energies when the sweep is split by energy across
+ * GPUs.  The table must be closed under z -> -conj(z) (Eq. 13 :95; energies on the imaginary axis
+ * are).  denominator_sum = sum over the WHOLE job's table of w_n t / Im z_n, the second term of the denominator of
+ * Eq. 22 (:144); NaN = compute it from this table.  Re-sizes and invalidates the boundary stores. */
+sc_status sc_set_energies(sc_ctx* ctx, const double* z_re, const double* z_im, const double* w, int n,
+                          double denominator_sum);
+
+/* Energy-sharded sweeps: with a hook set, sc_riccati_sweep (and sc_iterate) write the five un-finalised
+ * accumulators sum_k W_k {Re, Im conj(eta_k) SF_k, v_kx SG_k, v_ky SG_k, SI_k} of this context's energies into
+ * acc (dev fp64 [5][ny][nx], caller-owned), call fn(user) on the host — which must enqueue, on the context's
+ * stream, the sum of acc over all shards (one all-reduce) — and then apply Eq. 22 / Eq. 8 / Eq. 19 to the summed
+ * accumulators.  fn = NULL, acc = NULL removes the hook. */
+typedef void (*sc_allreduce_fn)(void* user);
+sc_status sc_set_allreduce_hook(sc_ctx* ctx, double* acc, sc_allreduce_fn fn, void* user);
 
 /* Boundary stores := local homogeneous solution at each trajectory end (Algorithm 1 "Initialize
  * gamma_dD", :205; reading R8).  Needs fields.  Called implicitly by the first sweep. */

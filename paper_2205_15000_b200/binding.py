@@ -70,6 +70,8 @@ def declared_symbols() -> list:
     return sorted(set(re.findall(r"\b(sc_[a-z0-9_]+)\s*\(", src)))
 
 
+ALLREDUCE_FN = C.CFUNCTYPE(None, C.c_void_p)
+
 _lib = None
 
 
@@ -91,6 +93,8 @@ def load_library():
     L.sc_destroy.argtypes = [vp]
     L.sc_set_fields.argtypes = [vp, vp, vp, vp]
     L.sc_reset_boundary.argtypes = [vp]
+    L.sc_set_energies.argtypes = [vp, vp, vp, vp, i, d]
+    L.sc_set_allreduce_hook.argtypes = [vp, vp, ALLREDUCE_FN, vp]
     L.sc_riccati_sweep.argtypes = [vp, vp, vp, vp, vp, C.POINTER(_Stats)]
     L.sc_ldos.argtypes = [vp, vp, i, d, i, vp, C.POINTER(_Stats)]
     L.sc_update_vector_potential.argtypes = [vp, vp, vp, vp, vp, C.POINTER(d)]
@@ -193,6 +197,21 @@ class ScContext:
     def sc_set_fields(self, delta, Ax=None, Ay=None):
         n = self.nx * self.ny
         self._check(self._L.sc_set_fields(self._h, _dev_ptr(delta, "c128", n), _dev_ptr(Ax, "f64", n), _dev_ptr(Ay, "f64", n)))
+
+    def sc_set_energies(self, z, w, denominator_sum=float("nan")):
+        z = np.ascontiguousarray(z, np.complex128)
+        zr = np.ascontiguousarray(z.real); zi = np.ascontiguousarray(z.imag); w = np.ascontiguousarray(w, np.float64)
+        self._check(self._L.sc_set_energies(self._h, zr.ctypes.data_as(C.c_void_p), zi.ctypes.data_as(C.c_void_p),
+                                            w.ctypes.data_as(C.c_void_p), len(zr), float(denominator_sum)))
+
+    def sc_set_allreduce_hook(self, acc, fn):
+        """acc: CUDA fp64 tensor [5][ny][nx]; fn(): enqueues the all-reduce of acc on the context's stream."""
+        if fn is None:
+            self._hook = None
+            self._check(self._L.sc_set_allreduce_hook(self._h, None, ALLREDUCE_FN(), None))
+            return
+        self._hook = (ALLREDUCE_FN(lambda user: fn()), acc)          # keep the callback and the buffer alive
+        self._check(self._L.sc_set_allreduce_hook(self._h, _dev_ptr(acc, "f64", 5 * self.nx * self.ny), self._hook[0], None))
 
     def sc_reset_boundary(self):
         self._check(self._L.sc_reset_boundary(self._h))

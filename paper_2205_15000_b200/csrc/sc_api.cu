@@ -79,6 +79,9 @@ struct sc_ctx {
     DevBuf<double4> d_scr; long long scr_stride = 0; int n_slots = 0;
     DevBuf<double> d_part; DevBuf<int> d_counter; DevBuf<int> d_nbad; DevBuf<double> d_statmax;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr, evm0 = nullptr, evm1 = nullptr;
+    // Eq. 22 denominator sum (sum_n w_n t / eps_n over the WHOLE job's energy table) and the energy-shard hook
+    double denom_sum = 0.0;
+    double* hook_acc = nullptr; sc_allreduce_fn hook_fn = nullptr; void* hook_user = nullptr;
     // vector potential / driver state
     scf::FieldState fs;
 };
@@ -108,9 +111,9 @@ sc_status ensure_nodes(sc_ctx* ctx) {
     if (ctx->nodes_fresh) return SC_OK;
     if (!ctx->have_fields) return fail(ctx, SC_ERR_STATE, "sc_set_fields has not been called");
     const int wpb = 8;
-    sck::rotate_in_kernel<<<(ctx->G + wpb - 1) / wpb, wpb * 32, 0, ctx->stream>>>(
+    sck::rotate_in_kernel<double><<<(ctx->G + wpb - 1) / wpb, wpb * 32, 0, ctx->stream>>>(
         grid_dev(ctx), traj_dev(ctx), ctx->d_vx.p, ctx->d_vy.p, ctx->d_eta.p, ctx->geo.c, ctx->opt.charge_sign,
-        ctx->d_ndD.p, ctx->d_nda.p, ctx->d_pc.p, ctx->d_nbad.p);
+        ctx->d_ndD.p, ctx->d_nda.p, nullptr, ctx->d_pc.p, ctx->d_nbad.p);
     if (!ctx->fb_rows.empty()) {
         const int n = (int)ctx->fb_rows.size();
         sck::fallback_kernel<<<(n + 127) / 128, 128, 0, ctx->stream>>>(grid_dev(ctx), n, ctx->d_fb_rows.p, ctx->d_fb_px.p,
@@ -133,41 +136,44 @@ sck::MarchArgs march_args(sc_ctx* ctx, const EnergySet& E, const double2* store_
     return A;
 }
 
-template <int MODE>
-sc_status launch_march(sc_ctx* ctx, const sck::MarchArgs& A, bool stats) {
-    CU(cudaMemsetAsync(ctx->d_counter.p, 0, sizeof(int), ctx->stream));
+template <int MODE, bool STATS, int STEP>
+sc_status launch_march_t(sc_ctx* ctx, const sck::MarchArgs& A) {
     const int blocks = ctx->n_slots / sck::MARCH_WARPS;
     const int smem = MODE == 0 ? sck::MARCH_SMEM : 0;
     static bool attr_set = false;
     if (MODE == 0 && !attr_set) {
-        CU(cudaFuncSetAttribute(sck::march_kernel<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        CU(cudaFuncSetAttribute(sck::march_kernel<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        CU(cudaFuncSetAttribute(sck::march_kernel<MODE, STATS, STEP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         attr_set = true;
     }
     CU(cudaEventRecord(ctx->evm0, ctx->stream));
-    if (stats) sck::march_kernel<MODE, true><<<blocks, sck::MARCH_WARPS * 32, smem, ctx->stream>>>(A);
-    else sck::march_kernel<MODE, false><<<blocks, sck::MARCH_WARPS * 32, smem, ctx->stream>>>(A);
+    sck::march_kernel<MODE, STATS, STEP><<<blocks, sck::MARCH_WARPS * 32, smem, ctx->stream>>>(A);
     CU(cudaEventRecord(ctx->evm1, ctx->stream));
     CU(cudaGetLastError());
     return SC_OK;
 }
 
+template <int MODE>
+sc_status launch_march(sc_ctx* ctx, const sck::MarchArgs& A, bool stats) {
+    CU(cudaMemsetAsync(ctx->d_counter.p, 0, sizeof(int), ctx->stream));
+    const bool st = stats && MODE == 0;
+    if (ctx->opt.stepper == 1) return st ? launch_march_t<MODE, MODE == 0, 1>(ctx, A) : launch_march_t<MODE, false, 1>(ctx, A);
+    return st ? launch_march_t<MODE, MODE == 0, 0>(ctx, A) : launch_march_t<MODE, false, 0>(ctx, A);
+}
+
 sc_status reset_stores(sc_ctx* ctx, const EnergySet& E, double2* store) {
     const long long total = (long long)ctx->G * E.ne;
-    sck::reset_store_kernel<<<(unsigned)((total + 255) / 256), 256, 0, ctx->stream>>>(traj_dev(ctx), E.dev(), ctx->d_pc.p, store);
+    sck::reset_store_kernel<double><<<(unsigned)((total + 255) / 256), 256, 0, ctx->stream>>>(traj_dev(ctx), E.dev(), ctx->d_pc.p, store);
     CU(cudaGetLastError());
     return SC_OK;
 }
 
-sck::BackArgs back_args(sc_ctx* ctx, void* delta_new, double* jx, double* jy, double* feI, int ne_mats) {
+sck::BackArgs back_args(sc_ctx* ctx, void* delta_new, double* jx, double* jy, double* feI) {
     sck::BackArgs B{};
     B.G = grid_dev(ctx); B.nphi = ctx->geo.nphi; B.nrot = ctx->geo.nrot; B.c = ctx->geo.c;
     B.vx = ctx->d_vx.p; B.vy = ctx->d_vy.p; B.eta = ctx->d_eta.p; B.W = ctx->d_W.p;
     B.line_g = ctx->d_line_g.p; B.T = traj_dev(ctx); B.part = ctx->d_part.p;
     B.t = ctx->t; B.sigma = ctx->opt.charge_sign;
-    double D = std::log(ctx->t);
-    for (int n = 0; n < ne_mats; ++n) D += 1.0 / (n + 0.5);
-    B.D = D;
+    B.D = std::log(ctx->t) + ctx->denom_sum;
     B.delta_new = (double2*)delta_new; B.jx = jx; B.jy = jy; B.feI = feI; B.n_bad = ctx->d_nbad.p;
     return B;
 }
@@ -209,7 +215,7 @@ sc_status sc_create(const sc_grid* grid, const unsigned char* mask, const sc_sha
     if (!(T_over_Tc > 0)) return fail(ctx, SC_ERR_ARG, "T/Tc must be positive");
     if (opts->n_matsubara < 1) return fail(ctx, SC_ERR_ARG, "n_matsubara < 1");
     if (opts->precision != 64 && opts->precision != 0) return fail(ctx, SC_ERR_ARG, "only precision=64 is built in this version");
-    if (opts->stepper != 0) return fail(ctx, SC_ERR_ARG, "only the closed-form stepper is built in this version");
+    if (opts->stepper != 0 && opts->stepper != 1) return fail(ctx, SC_ERR_ARG, "stepper must be 0 (closed form) or 1 (implicit mid-point)");
     ctx->opt = *opts; ctx->grid = *grid; ctx->t = T_over_Tc; ctx->kappa = kappa; ctx->sym = (int)symmetry;
     if (ctx->opt.charge_sign == 0) ctx->opt.charge_sign = -1;
     // ---- geometry (host) ----
@@ -308,12 +314,13 @@ sc_status sc_create(const sc_grid* grid, const unsigned char* mask, const sc_sha
     EnergySet& E = ctx->mats;
     for (int n = 0; n < opts->n_matsubara; ++n) { E.zr.push_back(0.0); E.zi.push_back(T_over_Tc * (n + 0.5)); E.w.push_back(1.0); E.partner.push_back(n); }
     if (sc_status st = upload_energies(ctx, E)) return st;
+    for (int n = 0; n < opts->n_matsubara; ++n) ctx->denom_sum += 1.0 / (n + 0.5);
     CU(ctx->d_store[0].alloc((size_t)ND * E.ne)); CU(ctx->d_store[1].alloc((size_t)ND * E.ne));
 
     // persistent march grid: MARCH_MIN_CTAS CTAs of 8 warps per SM; per-warp scratch of (smax+1) pieces x 32 lanes
     ctx->n_slots = ctx->n_sm * sck::MARCH_MIN_CTAS * sck::MARCH_WARPS;
     ctx->scr_stride = (long long)(smax + 2) * 32;
-    CU(ctx->d_scr.alloc((size_t)ctx->n_slots * ctx->scr_stride));
+    CU(ctx->d_scr.alloc((size_t)ctx->n_slots * ctx->scr_stride + 512));   // + 16 KB: the L2 prefetch of the last slot may run past its end
     CU(ctx->d_statmax.alloc(ctx->n_slots));
     CU(cudaMemsetAsync(ctx->d_statmax.p, 0, ctx->n_slots * sizeof(double), s));
     CU(cudaStreamSynchronize(s));
@@ -344,6 +351,33 @@ sc_status sc_set_fields(sc_ctx* ctx, const void* delta, const double* Ax, const 
     return SC_OK;
 }
 
+sc_status sc_set_energies(sc_ctx* ctx, const double* z_re, const double* z_im, const double* w, int n, double denominator_sum) {
+    if (!ctx || !z_re || !z_im || !w || n < 1) return fail(ctx, SC_ERR_ARG, "bad argument");
+    EnergySet& E = ctx->mats;
+    E.zr.assign(z_re, z_re + n); E.zi.assign(z_im, z_im + n); E.w.assign(w, w + n); E.partner.assign(n, -1);
+    double ds = 0.0;
+    for (int m = 0; m < n; ++m) {
+        if (!(z_im[m] > 0)) return fail(ctx, SC_ERR_ARG, "energies must lie in the upper half plane");
+        ds += w[m] * ctx->t / z_im[m];
+        // partner: -conj(z) (Eq. 13 :95); Matsubara / Ozaki energies on the imaginary axis are their own partner
+        for (int q = 0; q < n; ++q)
+            if (std::fabs(z_re[q] + z_re[m]) <= 1e-12 * (1.0 + std::fabs(z_re[m])) && std::fabs(z_im[q] - z_im[m]) <= 1e-12 * z_im[m]) { E.partner[m] = q; break; }
+        if (E.partner[m] < 0) return fail(ctx, SC_ERR_ARG, "energy table is not closed under z -> -conj(z)");
+    }
+    ctx->denom_sum = std::isnan(denominator_sum) ? ds : denominator_sum;
+    if (sc_status st = upload_energies(ctx, E)) return st;
+    const size_t ND = ctx->geo.dt.size();
+    CU(ctx->d_store[0].alloc(ND * E.ne)); CU(ctx->d_store[1].alloc(ND * E.ne));
+    ctx->stores_valid = false; ctx->cur = 0;
+    return SC_OK;
+}
+
+sc_status sc_set_allreduce_hook(sc_ctx* ctx, double* acc, sc_allreduce_fn fn, void* user) {
+    if (!ctx || ((fn != nullptr) != (acc != nullptr))) return fail(ctx, SC_ERR_ARG, "hook and accumulator buffer must be given together");
+    ctx->hook_acc = acc; ctx->hook_fn = fn; ctx->hook_user = user;
+    return SC_OK;
+}
+
 sc_status sc_reset_boundary(sc_ctx* ctx) {
     if (!ctx) return SC_ERR_ARG;
     if (sc_status st = ensure_nodes(ctx)) return st;
@@ -361,10 +395,19 @@ sc_status sc_riccati_sweep(sc_ctx* ctx, void* delta_new, double* jx, double* jy,
     sck::MarchArgs A = march_args(ctx, ctx->mats, ctx->d_store[ctx->cur].p, ctx->d_store[ctx->cur ^ 1].p);
     if (sc_status st = launch_march<0>(ctx, A, stats != nullptr)) return st;
     ctx->cur ^= 1;
-    sck::BackArgs B = back_args(ctx, delta_new, jx, jy, fe_I, ctx->mats.ne);
+    sck::BackArgs B = back_args(ctx, delta_new, jx, jy, fe_I);
+    B.raw = ctx->hook_fn ? ctx->hook_acc : nullptr;
     dim3 grd((ctx->grid.nx + 127) / 128, ctx->grid.ny);
     sck::rotate_back_kernel<<<grd, 128, 0, ctx->stream>>>(B);
     CU(cudaGetLastError());
+    if (ctx->hook_fn) {
+        // energy-sharded sweep: the caller sums the raw accumulators of all shards on this stream, then a7 runs
+        ctx->hook_fn(ctx->hook_user);
+        const size_t ng = (size_t)ctx->grid.nx * ctx->grid.ny;
+        sck::finalise_kernel<<<(unsigned)((ng + 255) / 256), 256, 0, ctx->stream>>>(ng, ctx->hook_acc, ctx->t, B.D, ctx->opt.charge_sign,
+                                                                                  (double2*)delta_new, jx, jy, fe_I);
+        CU(cudaGetLastError());
+    }
     return fill_stats(ctx, stats, ctx->mats.ne, true);
 }
 
@@ -425,7 +468,7 @@ sc_status sc_ldos(sc_ctx* ctx, const double* energies, int n_e, double broadenin
         A.ldos = d_ldn.p - (size_t)pair_nodes[p0] * E.ne;       // node offsets are global
         if (sc_status st = launch_march<1>(ctx, A, false)) return st;
         sck::BackLdosArgs L{};
-        L.B = back_args(ctx, nullptr, nullptr, nullptr, nullptr, 1);
+        L.B = back_args(ctx, nullptr, nullptr, nullptr, nullptr);
         L.ne_out = n_e; L.out_idx = d_out_idx.p; L.partner = E.d_partner.p; L.ne = E.ne;
         L.ldos_nodes = A.ldos; L.out = ldos; L.p0 = p0; L.p1 = p1; L.accumulate = first ? 0 : 1;
         dim3 grd((n_e + 63) / 64, ctx->grid.nx, ctx->grid.ny);
@@ -526,7 +569,7 @@ sc_status sc_debug_trajectory(sc_ctx* ctx, int k, int local, int n_energy, int* 
     DevBuf<double2> dG, dGT; CU(dG.alloc(nn)); CU(dGT.alloc(nn));
     // the last sweep read store[cur^1] (now the "new" side) and wrote store[cur]
     sck::MarchArgs A = march_args(ctx, ctx->mats, ctx->d_store[ctx->cur ^ 1].p, nullptr);
-    sck::debug_traj_kernel<<<1, 32, 0, ctx->stream>>>(A, g, n_energy, dG.p, dGT.p);
+    sck::debug_traj_kernel<<<1, 32, 0, ctx->stream>>>(A, ctx->opt.stepper, g, n_energy, dG.p, dGT.p);
     CU(cudaGetLastError());
     CU(cudaMemcpyAsync(gamma, dG.p, nn * sizeof(double2), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaMemcpyAsync(gamma_tilde, dGT.p, nn * sizeof(double2), cudaMemcpyDeviceToHost, ctx->stream));

@@ -17,7 +17,17 @@
 
 namespace sck {
 using scm::cplx;
+using scm::cplx_t;
 using scm::mk;
+
+// vector types of the march's working precision R (opts.precision: 64 -> double, 32 -> float)
+template <typename R> struct VT;
+template <> struct VT<double> { using V2 = double2; using V4 = double4; };
+template <> struct VT<float> { using V2 = float2; using V4 = float4; };
+__device__ __forceinline__ double2 mk2(double a, double b) { return make_double2(a, b); }
+__device__ __forceinline__ float2 mk2(float a, float b) { return make_float2(a, b); }
+__device__ __forceinline__ double4 mk4(double a, double b, double c, double d) { return make_double4(a, b, c, d); }
+__device__ __forceinline__ float4 mk4(float a, float b, float c, float d) { return make_float4(a, b, c, d); }
 
 struct GridDev {
     int nx, ny; double h;
@@ -86,8 +96,10 @@ __device__ __forceinline__ double interp_plain(const GridDev& G, const double* F
 // coefficients the march consumes: piece p of a trajectory with nn nodes (p = 0..nn) is {Re De, Im De, a, length}
 // with De, a the half-step values by linear interpolation and nearest-neighbour extrapolation at both ends
 // (reading R4).  Piece records of trajectory g start at noff[g] + g.
+template <typename R>
 __global__ void rotate_in_kernel(GridDev G, TrajDev T, const double* vx, const double* vy, const double* eta,
-                                 double c, int sigma, double2* nd_D, double* nd_a, double4* pc, int* n_bad) {
+                                 double c, int sigma, double2* nd_D, double* nd_a, typename VT<R>::V2* nd_Dr,
+                                 typename VT<R>::V4* pc, int* n_bad) {
     const int g = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (g >= T.n) return;
     const int lane = threadIdx.x & 31;
@@ -101,17 +113,18 @@ __global__ void rotate_in_kernel(GridDev G, TrajDev T, const double* vx, const d
         double dr, di;
         if (!interp_delta(G, x, y, dr, di)) atomicAdd(n_bad, 1);
         nd_D[off + m] = make_double2(e * dr, e * di);
+        if (sizeof(R) == 4) nd_Dr[off + m] = mk2((R)(e * dr), (R)(e * di));      // fp32 mode: the march reads a float copy
         nd_a[off + m] = sigma * (cx * interp_plain(G, G.Ax, x, y) + cy * interp_plain(G, G.Ay, x, y));
     }
     __syncwarp();
-    double4* P = pc + off + g;
+    typename VT<R>::V4* P = pc + off + g;
     for (int p = lane; p <= nn; p += 32) {
         const int lo = p > 0 ? p - 1 : 0, hi = p < nn ? p : nn - 1;
         const double2 Dl = nd_D[off + lo], Dh = nd_D[off + hi];
         const double al = nd_a[off + lo], ah = nd_a[off + hi];
         const double len = p == 0 ? T.l0[g] : (p == nn ? T.l1[g] : G.h);
-        P[p] = lo == hi ? make_double4(Dl.x, Dl.y, al, len)
-                        : make_double4(0.5 * (Dl.x + Dh.x), 0.5 * (Dl.y + Dh.y), 0.5 * (al + ah), len);
+        P[p] = lo == hi ? mk4((R)Dl.x, (R)Dl.y, (R)al, (R)len)
+                        : mk4((R)(0.5 * (Dl.x + Dh.x)), (R)(0.5 * (Dl.y + Dh.y)), (R)(0.5 * (al + ah)), (R)len);
     }
 }
 
@@ -129,16 +142,17 @@ __global__ void fallback_kernel(GridDev G, int nfb, const int* rows, const doubl
 }
 
 // R8: store[dF][n] = gamma_h(last piece); store[dB][partner n] = conj(gamma-tilde_h(first piece)).
-__global__ void reset_store_kernel(TrajDev T, EnergyDev E, const double4* pc, double2* store) {
+template <typename R>
+__global__ void reset_store_kernel(TrajDev T, EnergyDev E, const typename VT<R>::V4* pc, typename VT<R>::V2* store) {
     const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= (long long)T.n * E.ne) return;
     const int g = (int)(idx / E.ne), n = (int)(idx % E.ne);
-    const double4* P = pc + T.noff[g] + g;
-    const double4 cl = P[T.nn[g]], c0 = P[0];
+    const typename VT<R>::V4* P = pc + T.noff[g] + g;
+    const typename VT<R>::V4 cl = P[T.nn[g]], c0 = P[0];
     const cplx ge = scm::gamma_hom(cl.x, cl.y, E.zr[n] + cl.z, E.zi[n]);
-    store[(size_t)T.dF[g] * E.ne + n] = make_double2(ge.re, ge.im);
-    const cplx gt = scm::gamma_hom(-c0.x, c0.y, E.zr[n] + c0.z, E.zi[n]);
-    store[(size_t)T.dB[g] * E.ne + E.partner[n]] = make_double2(gt.re, -gt.im);
+    store[(size_t)T.dF[g] * E.ne + n] = mk2((R)ge.re, (R)ge.im);
+    const cplx gt = scm::gamma_hom(-(double)c0.x, c0.y, E.zr[n] + c0.z, E.zi[n]);
+    store[(size_t)T.dB[g] * E.ne + E.partner[n]] = mk2((R)gt.re, (R)-gt.im);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -229,14 +243,42 @@ __device__ __forceinline__ double stage_colsum(const double* stage, int lane) {
     return (s0 + s1) + (s2 + s3);
 }
 
+// Scratch entry of one (piece, lane): STEP 0 (closed form) {T.re, T.im, gt.re, gt.im} = 32 B, one 256-bit access;
+// STEP 1 (mid-point) {gt.re, gt.im} = 16 B, one 128-bit access.  A warp's 32 entries of a piece are contiguous.
+struct Ent { double tr, ti, gr, gi; };
+template <int STEP> struct ScrT { static constexpr int BYTES = STEP == 0 ? 32 : 16; static constexpr int ROW = 32 * BYTES; };
+template <int STEP>
+__device__ __forceinline__ Ent ld_ent(const char* p) {
+    Ent e;
+    if (STEP == 0) { const double4 v = ld256((const double4*)p); e.tr = v.x; e.ti = v.y; e.gr = v.z; e.gi = v.w; }
+    else {
+        asm volatile("ld.global.v2.f64 {%0,%1}, [%2];" : "=d"(e.gr), "=d"(e.gi) : "l"(p));
+        e.tr = e.ti = 0.0;
+    }
+    return e;
+}
+template <int STEP>
+__device__ __forceinline__ void st_ent(char* p, cplx T, cplx gt) {
+    if (STEP == 0) st256((double4*)p, T.re, T.im, gt.re, gt.im);
+    else asm volatile("st.global.v2.f64 [%0], {%1,%2};" ::"l"(p), "d"(gt.re), "d"(gt.im) : "memory");
+}
+// one step of gamma with piece record cc; STEP 0 re-uses the stored T of the piece
+template <int STEP>
+__device__ __forceinline__ cplx step_up(cplx g, const double4& cc, double zr0, double zi0, const Ent& E) {
+    if (STEP == 0) return scm::step_T(g, cc.x, cc.y, zr0 + cc.z, zi0, mk(E.tr, E.ti));
+    return scm::step_mid(g, cc.x, cc.y, zr0 + cc.z, zi0, cc.w);
+}
+
 // MODE 0: Matsubara sums; 1: per-energy Re g (LDOS); 2: boundary values only.
-template <int MODE, bool STATS>
+// STEP 0: closed-form step; 1: implicit mid-point rule (C4-C9 :984-1001).
+template <int MODE, bool STATS, int STEP>
 __global__ void __launch_bounds__(MARCH_WARPS * 32, MARCH_MIN_CTAS) march_kernel(MarchArgs A) {
     extern __shared__ double stage_all[];        // MODE 0: MARCH_WARPS x (24 rows x STAGE_LD) doubles (MARCH_SMEM bytes)
+    constexpr int ROW = ScrT<STEP>::ROW;
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const int slot = blockIdx.x * MARCH_WARPS + wib;
     double* const stage = stage_all + wib * (RED_NODES * RED_VALS * STAGE_LD);
-    double4* const scr = A.scr + (size_t)slot * A.scr_stride + lane;     // entry e of this lane: scr[e*32]
+    char* const scr = (char*)(A.scr + (size_t)slot * A.scr_stride) + lane * ScrT<STEP>::BYTES;   // entry e of this lane: scr + e*ROW
     const int ne = A.E.ne;
     double max2 = 0.0;
 
@@ -272,7 +314,7 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32, MARCH_MIN_CTAS) march_kernel
                 gt = mk(s.re, -s.im);
             }
             {
-                double4* e = scr + (size_t)nn * 32;
+                char* e = scr + (size_t)nn * ROW;
                 double4 cn = ldu256(PC + (nn >= 1 ? nn - 1 : 0));
 #pragma unroll 2
                 for (int p = nn; p >= 0; --p) {
@@ -280,10 +322,15 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32, MARCH_MIN_CTAS) march_kernel
                     c4 = cn;
                     if (p >= 2) cn = ldu256(PC + p - 2);                       // coefficient record two pieces ahead
                     const double zr = zr0 + cc.z;
-                    const cplx T = scm::coef_T(fma(cc.x, cc.x, cc.y * cc.y), zr, zi0, cc.w);
-                    gt = scm::step_T(gt, -cc.x, cc.y, zr, zi0, T);
-                    st256(e, T.re, T.im, gt.re, gt.im);
-                    e -= 32;
+                    cplx T = mk(0.0, 0.0);
+                    if (STEP == 0) {
+                        T = scm::coef_T(fma(cc.x, cc.x, cc.y * cc.y), zr, zi0, cc.w);
+                        gt = scm::step_T(gt, -cc.x, cc.y, zr, zi0, T);
+                    } else {
+                        gt = scm::step_mid(gt, -cc.x, cc.y, zr, zi0, cc.w);
+                    }
+                    st_ent<STEP>(e, T, gt);
+                    e -= ROW;
                 }
                 if (act) A.store_new[(size_t)dB * ne + nb] = make_double2(gt.re, -gt.im);
             }
@@ -295,32 +342,32 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32, MARCH_MIN_CTAS) march_kernel
                 if (A.bc_mode == 1) gm = scm::gamma_hom(c0.x, c0.y, zr0 + c0.z, zi0);
                 else if (A.ga_n[dF]) gm = gather_start(A, dF, n);
                 else gm = scm::gamma_hom(A.fb_D[dF].x, A.fb_D[dF].y, zr0 + A.fb_a[dF], zi0);
-                const double4 e0 = ld256(scr);
-                gm = scm::step_T(gm, c0.x, c0.y, zr0 + c0.z, zi0, mk(e0.x, e0.y));
+                const Ent e0 = ld_ent<STEP>(scr);
+                gm = step_up<STEP>(gm, c0, zr0, zi0, e0);
             }
-            const double4* e = scr + 32;                 // entry of node 0
-            for (int q = 4; q < PF_DIST && q < nn; q += 4) prefetch_l2((const char*)(e - lane) + (size_t)q * 1024 + lane * 128);
-            double4 En = ld256(e);
+            const char* e = scr + ROW;                  // entry of node 0
+            for (int q = 4; q < PF_DIST && q < nn; q += 4) prefetch_l2(e - lane * ScrT<STEP>::BYTES + (size_t)q * ROW + lane * 128);
+            Ent En = ld_ent<STEP>(e);
             double4 cN = ldu256(PC + 1);
             double2 dN = ND[0];
             int m = 0;
             for (; m + RED_NODES <= nn; m += RED_NODES) {
-                if (m + PF_DIST < nn) prefetch_l2((const char*)(e - lane) + (size_t)PF_DIST * 1024 + lane * 128);
+                if (m + PF_DIST < nn) prefetch_l2(e - lane * ScrT<STEP>::BYTES + (size_t)PF_DIST * ROW + lane * 128);
                 double part_old = 0.0;
                 if (MODE == 0 && n0 && lane < RED_NODES * RED_VALS) part_old = A.part[(size_t)(noff + m) * RED_VALS + lane];
 #pragma unroll
                 for (int b = 0; b < RED_NODES; ++b) {
-                    const double4 Ec = En; const double4 cc = cN; const double2 dc = dN;
-                    En = ld256(e + (b + 1) * 32);                // one node ahead (scratch has 2 spare entries)
+                    const Ent Ec = En; const double4 cc = cN; const double2 dc = dN;
+                    En = ld_ent<STEP>(e + (b + 1) * ROW);                // one node ahead (scratch has 2 spare entries)
                     cN = ldu256(PC + m + b + 2 <= PC + nn ? PC + m + b + 2 : PC + nn);
                     dN = ND[m + b + 1 < nn ? m + b + 1 : nn - 1];
                     if (MODE != 2) {
-                        const double rg = node_products<MODE, STATS>(gm, Ec.z, Ec.w, dc, wn, stage + b * RED_VALS * STAGE_LD + lane, max2);
+                        const double rg = node_products<MODE, STATS>(gm, Ec.gr, Ec.gi, dc, wn, stage + b * RED_VALS * STAGE_LD + lane, max2);
                         if (MODE == 1 && act) A.ldos[(size_t)(noff + m + b) * ne + n] = rg;
                     }
-                    gm = scm::step_T(gm, cc.x, cc.y, zr0 + cc.z, zi0, mk(Ec.x, Ec.y));
+                    gm = step_up<STEP>(gm, cc, zr0, zi0, Ec);
                 }
-                e += RED_NODES * 32;
+                e += RED_NODES * ROW;
                 if (MODE == 0) {
                     __syncwarp();
                     if (lane < RED_NODES * RED_VALS) {
@@ -336,15 +383,15 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32, MARCH_MIN_CTAS) march_kernel
                 double part_old = 0.0;
                 if (MODE == 0 && n0 && lane < rem * RED_VALS) part_old = A.part[(size_t)(noff + m) * RED_VALS + lane];
                 for (int b = 0; b < rem; ++b) {
-                    const double4 Ec = En; const double4 cc = cN; const double2 dc = dN;
-                    En = ld256(e + (b + 1) * 32);
+                    const Ent Ec = En; const double4 cc = cN; const double2 dc = dN;
+                    En = ld_ent<STEP>(e + (b + 1) * ROW);
                     cN = ldu256(PC + m + b + 2 <= PC + nn ? PC + m + b + 2 : PC + nn);
                     dN = ND[m + b + 1 < nn ? m + b + 1 : nn - 1];
                     if (MODE != 2) {
-                        const double rg = node_products<MODE, STATS>(gm, Ec.z, Ec.w, dc, wn, stage + b * RED_VALS * STAGE_LD + lane, max2);
+                        const double rg = node_products<MODE, STATS>(gm, Ec.gr, Ec.gi, dc, wn, stage + b * RED_VALS * STAGE_LD + lane, max2);
                         if (MODE == 1 && act) A.ldos[(size_t)(noff + m + b) * ne + n] = rg;
                     }
-                    gm = scm::step_T(gm, cc.x, cc.y, zr0 + cc.z, zi0, mk(Ec.x, Ec.y));
+                    gm = step_up<STEP>(gm, cc, zr0, zi0, Ec);
                 }
                 if (MODE == 0) {
                     __syncwarp();
@@ -379,6 +426,7 @@ struct BackArgs {
     double t, D; int sigma;
     double2* delta_new; double* jx; double* jy; double* feI;
     int* n_bad;
+    double* raw;                 // non-null: write the 5 un-finalised accumulators [5][ny][nx] instead (energy-sharded sweep)
 };
 
 // weights of the (up to 4) valid lattice nodes around a grid point for pair p; returns count
@@ -449,12 +497,29 @@ __global__ void rotate_back_kernel(BackArgs B) {
             sI += (Wk + Wk2) * f5;
         }
     }
+    if (B.raw) {
+        const size_t ng = (size_t)B.G.nx * B.G.ny;
+        B.raw[q] = nr; B.raw[ng + q] = ni; B.raw[2 * ng + q] = sjx; B.raw[3 * ng + q] = sjy; B.raw[4 * ng + q] = sI;
+        return;
+    }
     // Delta_new = -2 i t Num / D (Eq. 22 with f = -2 pi i gamma/(1+P)); j = 2 sigma t J (Eq. 8); I = t I (Eq. 19)
     const double s = 2.0 * B.t / B.D;
     if (B.delta_new) B.delta_new[q] = make_double2(s * ni, -s * nr);
     if (B.jx) B.jx[q] = 2.0 * B.sigma * B.t * sjx;
     if (B.jy) B.jy[q] = 2.0 * B.sigma * B.t * sjy;
     if (B.feI) B.feI[q] = B.t * sI;
+}
+
+// a7 alone, after the accumulators of all energy shards have been summed
+__global__ void finalise_kernel(size_t ng, const double* raw, double t, double D, int sigma,
+                                double2* delta_new, double* jx, double* jy, double* feI) {
+    const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= ng) return;
+    const double s = 2.0 * t / D;
+    if (delta_new) delta_new[q] = make_double2(s * raw[ng + q], -s * raw[q]);
+    if (jx) jx[q] = 2.0 * sigma * t * raw[2 * ng + q];
+    if (jy) jy[q] = 2.0 * sigma * t * raw[3 * ng + q];
+    if (feI) feI[q] = t * raw[4 * ng + q];
 }
 
 // LDOS rotate-back: thread per (grid point, energy); energies fastest so the gathers coalesce.
@@ -500,7 +565,7 @@ __global__ void rotate_back_ldos_kernel(BackLdosArgs L) {
 // debug / measurement kernels
 // ------------------------------------------------------------------------------------------------
 // re-march one trajectory for one energy with the same device functions; writes gamma, gamma-tilde per node
-__global__ void debug_traj_kernel(MarchArgs A, int g, int n, double2* outG, double2* outGT) {
+__global__ void debug_traj_kernel(MarchArgs A, int stepper, int g, int n, double2* outG, double2* outGT) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     const int nn = A.T.nn[g];
     const double4* PC = A.pc + A.T.noff[g] + g;
@@ -513,8 +578,8 @@ __global__ void debug_traj_kernel(MarchArgs A, int g, int n, double2* outG, doub
     else { cplx s = scm::gamma_hom(A.fb_D[dB].x, A.fb_D[dB].y, A.E.zr[nb] + A.fb_a[dB], A.E.zi[nb]); gt = mk(s.re, -s.im); }
     for (int p = nn; p >= 1; --p) {
         const double4 c = PC[p];
-        const cplx T = scm::coef_T(c.x * c.x + c.y * c.y, zr0 + c.z, zi0, c.w);
-        gt = scm::step_T(gt, -c.x, c.y, zr0 + c.z, zi0, T);
+        if (stepper == 1) gt = scm::step_mid(gt, -c.x, c.y, zr0 + c.z, zi0, c.w);
+        else { const cplx T = scm::coef_T(c.x * c.x + c.y * c.y, zr0 + c.z, zi0, c.w); gt = scm::step_T(gt, -c.x, c.y, zr0 + c.z, zi0, T); }
         outGT[p - 1] = make_double2(gt.re, gt.im);
     }
     cplx gm;
@@ -523,8 +588,8 @@ __global__ void debug_traj_kernel(MarchArgs A, int g, int n, double2* outG, doub
     else gm = scm::gamma_hom(A.fb_D[dF].x, A.fb_D[dF].y, zr0 + A.fb_a[dF], zi0);
     for (int p = 0; p < nn; ++p) {
         const double4 c = PC[p];
-        const cplx T = scm::coef_T(c.x * c.x + c.y * c.y, zr0 + c.z, zi0, c.w);
-        gm = scm::step_T(gm, c.x, c.y, zr0 + c.z, zi0, T);
+        if (stepper == 1) gm = scm::step_mid(gm, c.x, c.y, zr0 + c.z, zi0, c.w);
+        else { const cplx T = scm::coef_T(c.x * c.x + c.y * c.y, zr0 + c.z, zi0, c.w); gm = scm::step_T(gm, c.x, c.y, zr0 + c.z, zi0, T); }
         outG[p] = make_double2(gm.re, gm.im);
     }
 }

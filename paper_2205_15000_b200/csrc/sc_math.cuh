@@ -1,4 +1,4 @@
-// sc_math.cuh — fp64 building blocks of the march kernel (sm_100a).
+// sc_math.cuh — arithmetic building blocks of the march kernel (sm_100a), fp64 and fp32.
 //
 // The march is bound by the FP64 pipe, so every transcendental is written out as a short
 // DFMA sequence seeded by the MUFU approximations (MUFU.RCP64H / MUFU.RSQ64H, reached through
@@ -9,6 +9,8 @@
 //   sin / cos         |y| <= pi/4 polynomial kernels (the arguments are 2*l*Im(Omega) << 1); library
 //                     sincos on the rare warp that exceeds it
 // Accuracy (measured by sc_debug_math, tests/test_gpu_parity.py): <= 4 ulp each.
+// The optional FP32 mode (opts.precision = 32) uses the same formulas on float: MUFU.RCP / MUFU.RSQ directly
+// (1-2 ulp), degree-7 expm1 and degree-4 sin/cos kernels.  Everything above the primitives is one template.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -25,10 +27,23 @@ __constant__ double kCos[6] = {-1.13596475577881948265e-11, 2.087572321298174827
                                2.48015872894767294178e-05, -1.38888888888741095749e-03, 4.16666666666666019037e-02};
 __constant__ double kRed[4] = {1.4426950408889634074, 6.93147180369123816490e-01, 1.90821492927058770002e-10, 6755399441055744.0};
 
-struct cplx { double re, im; };
+template <typename R> struct cplx_t { R re, im; };
+using cplx = cplx_t<double>;
+using cplxf = cplx_t<float>;
 
-__device__ __forceinline__ cplx mk(double a, double b) { cplx r; r.re = a; r.im = b; return r; }
+template <typename R>
+__device__ __forceinline__ cplx_t<R> mk(R a, R b) { cplx_t<R> r; r.re = a; r.im = b; return r; }
 
+__device__ __forceinline__ double mad(double a, double b, double c) { return fma(a, b, c); }
+__device__ __forceinline__ float mad(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ double absr(double a) { return fabs(a); }
+__device__ __forceinline__ float absr(float a) { return fabsf(a); }
+__device__ __forceinline__ double cpsign(double a, double b) { return copysign(a, b); }
+__device__ __forceinline__ float cpsign(float a, float b) { return copysignf(a, b); }
+__device__ __forceinline__ double maxr(double a, double b) { return fmax(a, b); }
+__device__ __forceinline__ float maxr(float a, float b) { return fmaxf(a, b); }
+
+// ---------------------------------------------------------------------------------------------- fp64 primitives
 __device__ __forceinline__ double rcp_nr(double x) {
     double y;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
@@ -87,66 +102,123 @@ __device__ __forceinline__ void sincos_small(double y, double& s, double& cm1) {
     s = fma(y * z, ps, y);
     cm1 = fma(z * z, pc, -0.5 * z);
 }
+__device__ __forceinline__ void sincos_lib(double y, double& s, double& cm1) { double c; sincos(y, &s, &c); cm1 = c - 1.0; }
 
+// ---------------------------------------------------------------------------------------------- fp32 primitives
+__device__ __forceinline__ float rcp_nr(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float rsqrt_nr(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
+__device__ __forceinline__ void exp_pair(float x, float& ex, float& xm1) {
+    x = fmaxf(x, -80.0f);
+    float kf = fmaf(x, 1.4426950408889634f, 12582912.0f);            // 1.5 * 2^23
+    const int k = __float_as_int(kf) - 0x4B400000;
+    kf -= 12582912.0f;
+    float r = fmaf(-kf, 0.693145751953125f, x);
+    r = fmaf(-kf, 1.42860682030941723212e-6f, r);
+    // expm1(r) = r + r^2 (1/2 + r/6 + ... + r^5/7!), |r| <= ln2/2: truncation < 2e-8 relative
+    float p = 1.9841270e-4f;
+    p = fmaf(p, r, 1.3888889e-3f); p = fmaf(p, r, 8.3333333e-3f); p = fmaf(p, r, 4.1666667e-2f);
+    p = fmaf(p, r, 1.6666667e-1f); p = fmaf(p, r, 0.5f);
+    p = fmaf(p, r * r, r);
+    const float s = __int_as_float((k + 127) << 23);                  // 2^k, k in [-116, 0]
+    xm1 = fmaf(s, p, s - 1.0f);
+    ex = fmaf(s, p, s);
+}
+
+__device__ __forceinline__ void sincos_small(float y, float& s, float& cm1) {
+    const float z = y * y;
+    float ps = 2.7183114939898219064e-6f, pc = 2.43904487962774090654e-5f;
+    ps = fmaf(ps, z, -1.98393348360966317347e-4f); ps = fmaf(ps, z, 8.3333293858894631756e-3f); ps = fmaf(ps, z, -1.66666666416265235595e-1f);
+    pc = fmaf(pc, z, -1.38867637746099294692e-3f); pc = fmaf(pc, z, 4.16666233237390631894e-2f);
+    s = fmaf(y * z, ps, y);
+    cm1 = fmaf(z * z, pc, -0.5f * z);
+}
+__device__ __forceinline__ void sincos_lib(float y, float& s, float& cm1) { float c; sincosf(y, &s, &c); cm1 = c - 1.0f; }
+
+// ---------------------------------------------------------------------------------------------- the step
 // Principal square root Omega of w (Re Omega >= 0) and rq = 1/|Omega|^2 (so that 1/Omega = conj(Omega) rq).
-__device__ __forceinline__ void csqrt_inv(double wr, double wi, double& sr, double& si, double& rq) {
-    const double q = fma(wr, wr, wi * wi);
+template <typename R>
+__device__ __forceinline__ void csqrt_inv(R wr, R wi, R& sr, R& si, R& rq) {
+    const R q = mad(wr, wr, wi * wi);
     rq = rsqrt_nr(q);                  // 1/|w| = 1/|Omega|^2
-    const double m = q * rq;           // |w|
-    const double p = 0.5 * (m + fabs(wr));
-    const double rp = rsqrt_nr(p);
-    const double a = p * rp;           // sqrt(p)
-    const double b = 0.5 * fabs(wi) * rp;
-    sr = wr >= 0.0 ? a : b;
-    si = copysign(wr >= 0.0 ? b : a, wi);
+    const R m = q * rq;                // |w|
+    const R p = R(0.5) * (m + absr(wr));
+    const R rp = rsqrt_nr(p);
+    const R a = p * rp;                // sqrt(p)
+    const R b = R(0.5) * absr(wi) * rp;
+    sr = wr >= R(0) ? a : b;
+    si = cpsign(wr >= R(0) ? b : a, wi);
 }
 
 // Step coefficient T = tanh(Omega l)/Omega, Omega = sqrt(|De|^2 - z^2): the closed-form step
 // of PAPER.md:982 is the Moebius map gamma' = [gamma + iT(z gamma + De)] / [1 - iT(z + conj(De) gamma)].
 // T depends on De only through |De|^2, so gamma (De) and gamma-tilde (-conj De) share it.
-__device__ __forceinline__ cplx coef_T(double d2, double zr, double zi, double len) {
-    const double wr = fma(zi, zi, fma(-zr, zr, d2));
-    const double wi = -2.0 * zr * zi;
-    double sr, si, rq;
+template <typename R>
+__device__ __forceinline__ cplx_t<R> coef_T(R d2, R zr, R zi, R len) {
+    const R wr = mad(zi, zi, mad(-zr, zr, d2));
+    const R wi = R(-2) * zr * zi;
+    R sr, si, rq;
     csqrt_inv(wr, wi, sr, si, rq);
-    const double m2l = -2.0 * len;
-    const double x = m2l * sr, y = m2l * si;
-    double ex, xm1, s, cm1;
+    const R m2l = R(-2) * len;
+    const R x = m2l * sr, y = m2l * si;
+    R ex, xm1, s, cm1;
     exp_pair(x, ex, xm1);
-    if (__any_sync(0xffffffffu, fabs(y) > 0.78539816339744830962)) {
-        double cc;
-        sincos(y, &s, &cc);
-        cm1 = cc - 1.0;
-    } else {
-        sincos_small(y, s, cm1);
-    }
+    if (__any_sync(0xffffffffu, absr(y) > R(0.78539816339744830962))) sincos_lib(y, s, cm1);
+    else sincos_small(y, s, cm1);
     // E - 1 = (e^x - 1) cos y + (cos y - 1) + i e^x sin y
-    const double er = fma(xm1, cm1, xm1) + cm1;
-    const double ei = ex * s;
-    const double fr = 2.0 + er;                         // 1 + E
-    const double rf = rcp_nr(fma(fr, fr, ei * ei));
+    const R er = mad(xm1, cm1, xm1) + cm1;
+    const R ei = ex * s;
+    const R fr = R(2) + er;                             // 1 + E
+    const R rf = rcp_nr(mad(fr, fr, ei * ei));
     // tanh(Omega l) = -(E-1)/(E+1) = -(E-1) conj(E+1) / |E+1|^2
-    const double tr = -fma(er, fr, ei * ei) * rf;
-    const double ti = fma(er, ei, -ei * fr) * rf;
-    const double ir = sr * rq, ii = -si * rq;           // 1/Omega
-    return mk(fma(tr, ir, -ti * ii), fma(tr, ii, ti * ir));
+    const R tr = -mad(er, fr, ei * ei) * rf;
+    const R ti = mad(er, ei, -ei * fr) * rf;
+    const R ir = sr * rq, ii = -si * rq;                // 1/Omega
+    return mk(mad(tr, ir, -ti * ii), mad(tr, ii, ti * ir));
 }
 
-// One closed-form step given T: 27 fp64 instructions + 1 MUFU.
-__device__ __forceinline__ cplx step_T(cplx g, double Dr, double Di, double zr, double zi, cplx T) {
-    const double ur = fma(zr, g.re, fma(-zi, g.im, Dr));        // u = z g + De
-    const double ui = fma(zr, g.im, fma(zi, g.re, Di));
-    const double Nr = fma(-T.re, ui, fma(-T.im, ur, g.re));     // N = g + i T u
-    const double Ni = fma(T.re, ur, fma(-T.im, ui, g.im));
-    const double vr = fma(Dr, g.re, fma(Di, g.im, zr));         // v = z + conj(De) g
-    const double vi = fma(Dr, g.im, fma(-Di, g.re, zi));
-    const double Qr = fma(T.re, vi, fma(T.im, vr, 1.0));        // Q = 1 - i T v
-    const double Qi = fma(-T.re, vr, T.im * vi);
-    const double rq = rcp_nr(fma(Qr, Qr, Qi * Qi));
-    return mk(fma(Nr, Qr, Ni * Qi) * rq, fma(Ni, Qr, -Nr * Qi) * rq);
+// One closed-form step given T: 27 arithmetic instructions + 1 MUFU.
+template <typename R>
+__device__ __forceinline__ cplx_t<R> step_T(cplx_t<R> g, R Dr, R Di, R zr, R zi, cplx_t<R> T) {
+    const R ur = mad(zr, g.re, mad(-zi, g.im, Dr));        // u = z g + De
+    const R ui = mad(zr, g.im, mad(zi, g.re, Di));
+    const R Nr = mad(-T.re, ui, mad(-T.im, ur, g.re));     // N = g + i T u
+    const R Ni = mad(T.re, ur, mad(-T.im, ui, g.im));
+    const R vr = mad(Dr, g.re, mad(Di, g.im, zr));         // v = z + conj(De) g
+    const R vi = mad(Dr, g.im, mad(-Di, g.re, zi));
+    const R Qr = mad(T.re, vi, mad(T.im, vr, R(1)));       // Q = 1 - i T v
+    const R Qi = mad(-T.re, vr, T.im * vi);
+    const R rq = rcp_nr(mad(Qr, Qr, Qi * Qi));
+    return mk(mad(Nr, Qr, Ni * Qi) * rq, mad(Ni, Qr, -Nr * Qi) * rq);
 }
 
-// Local homogeneous solution gamma_h = -De/(z + i Omega) (start values, boundary reset): rare, library math.
+// Implicit mid-point step (PAPER.md C4-C9 :984-1001, v_F = 1): gamma' = gamma + l f((gamma + gamma')/2) with
+// f = i[conj(De) g^2 + 2 z g + De] is the quadratic c2 g'^2 + c1 g' + c0 = 0; the root that tends to gamma as
+// l -> 0 is g' = 2 c0 / (-c1 + sqrt(c1^2 - 4 c2 c0)) with the principal square root (-c1 ~ 1, sqrt ~ 1: the
+// denominator never cancels).  No exponential, no T to share: ~63 arithmetic instructions + 3 MUFU per step.
+template <typename R>
+__device__ __forceinline__ cplx_t<R> step_mid(cplx_t<R> g, R Dr, R Di, R zr, R zi, R len) {
+    const R q = R(0.25) * len;
+    const R c2r = q * Di, c2i = q * Dr;                      // c2 = i (l/4) conj(De)
+    const R pr = mad(c2r, g.re, -c2i * g.im);                // c2 g
+    const R pi = mad(c2r, g.im, c2i * g.re);
+    const R lr = -len * zi, li = len * zr;                   // i l z
+    const R c1r = mad(R(2), pr, lr) - R(1), c1i = mad(R(2), pi, li);
+    const R ar = pr + lr + R(1), ai = pi + li;               // c1 - c2 g + 2
+    const R c0r = mad(ar, g.re, mad(-ai, g.im, R(-4) * c2r)); // (c1 - c2 g + 2) g - 4 conj(c2)
+    const R c0i = mad(ar, g.im, mad(ai, g.re, R(4) * c2i));
+    const R mr = mad(c2r, c0r, -c2i * c0i), mi = mad(c2r, c0i, c2i * c0r);      // c2 c0
+    const R dr = mad(c1r, c1r, mad(-c1i, c1i, R(-4) * mr));  // c1^2 - 4 c2 c0
+    const R di = mad(R(2) * c1r, c1i, R(-4) * mi);
+    R sr, si, rq;
+    csqrt_inv(dr, di, sr, si, rq);
+    const R er = sr - c1r, ei = si - c1i;                    // -c1 + sqrt(.)
+    const R rd = R(2) * rcp_nr(mad(er, er, ei * ei));
+    return mk(mad(c0r, er, c0i * ei) * rd, mad(c0i, er, -c0r * ei) * rd);
+}
+
+// Local homogeneous solution gamma_h = -De/(z + i Omega) (start values, boundary reset): rare, library math,
+// always evaluated in fp64.
 __device__ __forceinline__ cplx gamma_hom(double Dr, double Di, double zr, double zi) {
     const double wr = Dr * Dr + Di * Di - (zr * zr - zi * zi), wi = -2.0 * zr * zi;
     const double m = hypot(wr, wi);

@@ -53,7 +53,7 @@ class GpuRun:
 
 
 def compare_sweeps(sc, wl, n_sweeps=2, **kw):
-    o = oracle.Oracle.from_workload(wl, **{k: v for k, v in kw.items() if k in ("bc_mode",)})
+    o = oracle.Oracle.from_workload(wl, **{k: v for k, v in kw.items() if k in ("bc_mode", "stepper")})
     g = GpuRun(sc, wl, **kw)
     Ax = wl.Aext_x if np.any(wl.Aext_x) else None
     Ay = wl.Aext_y if np.any(wl.Aext_x) else None
@@ -120,6 +120,72 @@ def test_reduced_configs(sc, cfg, kw, ns):
 def test_bulk_boundary_mode(sc):
     wl = wlmod.make_workload(1, pts_per_xi=5, n_angles=8, n_energies=8)
     compare_sweeps(sc, wl, n_sweeps=1, bc_mode=1)
+
+
+@pytest.mark.parametrize("cfg,kw", [
+    (1, dict(pts_per_xi=6, n_angles=16, n_energies=40)),
+    (2, dict(pts_per_xi=5, n_angles=32, n_energies=33, size_scale=0.5)),
+])
+def test_midpoint_stepper_parity(sc, cfg, kw):
+    """stepper = 1: the paper's own implicit mid-point rule (C4-C9 :984-1001) on both sides."""
+    wl = wlmod.make_workload(cfg, **kw)
+    o, g, stores, worst = compare_sweeps(sc, wl, n_sweeps=2, stepper=1)
+    # and it is a different discretisation from the closed form (O(h^2) apart), so the switch is live
+    g0 = GpuRun(sc, wl)
+    g0.set_fields(wl.delta0, wl.Aext_x if np.any(wl.Aext_x) else None, wl.Aext_y if np.any(wl.Aext_x) else None)
+    r0 = g0.sweep(); 
+    g1 = GpuRun(sc, wl, stepper=1)
+    g1.set_fields(wl.delta0, wl.Aext_x if np.any(wl.Aext_x) else None, wl.Aext_y if np.any(wl.Aext_x) else None)
+    r1 = g1.sweep()
+    d = relerr(r1["delta_new"], r0["delta_new"])
+    assert 1e-8 < d < 5e-2, d
+
+
+def test_energy_sharded_sweep_equals_full_sweep(sc):
+    """two energy shards (two contexts on one GPU, run one after the other), raw accumulators summed
+    in the all-reduce hook, then finalised == the oracle's full sweep.  No kernel waits on another."""
+    from paper_2205_15000_b200 import sharding
+    wl = wlmod.make_workload(1, pts_per_xi=6, n_angles=16, n_energies=40)
+    o = oracle.Oracle.from_workload(wl)
+    runs, accs = [], []
+    for r in range(2):
+        g = GpuRun(sc, wl)
+        z, w, dsum = sharding.matsubara_shard(wl.t, wl.n_energies, 2, r)
+        g.ctx.sc_set_energies(z, w, dsum)
+        acc = torch.zeros((5, wl.ny, wl.nx), dtype=torch.float64, device="cuda")
+        runs.append(g); accs.append(acc)
+    runs[0].ctx.sc_set_allreduce_hook(accs[0], lambda: None)
+    runs[1].ctx.sc_set_allreduce_hook(accs[1], lambda: accs[1].add_(accs[0]))
+    stores = None
+    n_upd = 0
+    for it in range(2):
+        ro = o.sweep(wl.delta0, wl.Aext_x, wl.Aext_y, wl.n_energies, stores)
+        stores = ro["stores"]
+        for g in runs:
+            g.set_fields(wl.delta0, wl.Aext_x, wl.Aext_y)
+        r0 = runs[0].sweep(); r1 = runs[1].sweep()
+        for key in ("delta_new", "jx", "jy", "fe_I"):
+            assert relerr(r1[key], ro[key]) < TOL, (it, key)
+        assert r0["stats"].n_updates + r1["stats"].n_updates == ro["stats"]["n_updates"]
+
+
+def test_custom_energy_table_with_weights(sc):
+    """sc_set_energies with non-uniform weights on the imaginary axis (the shape of an Ozaki pole table, :207)."""
+    wl = wlmod.make_workload(0)
+    o = oracle.Oracle.from_workload(wl)
+    rng = np.random.default_rng(3)
+    z = 1j * np.sort(rng.uniform(0.05, 6.0, 21)); w = rng.uniform(0.2, 1.5, 21)
+    g = GpuRun(sc, wl)
+    g.ctx.sc_set_energies(z, w)
+    g.set_fields(wl.delta0, None, None)
+    rg = g.sweep()
+    st = o.reset_stores(wl.delta0, None, None, z)
+    ro = o.raw_sweep(wl.delta0, None, None, z, w, st)
+    D = np.log(wl.t) + float(np.sum(w * wl.t / z.imag))
+    assert relerr(rg["delta_new"], -2j * wl.t * ro["num"] / D * wl.mask) < TOL
+    assert relerr(rg["jx"], 2.0 * wl.charge_sign * wl.t * ro["Jx"] * wl.mask) < TOL
+    with pytest.raises(sc.ScError):
+        g.ctx.sc_set_energies(np.array([0.3 + 0.1j]), np.ones(1))       # not closed under z -> -conj z
 
 
 def test_tiny_and_thin_grains(sc):
