@@ -84,6 +84,8 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep-only", action="store_true", help="time sc_riccati_sweep alone (profiling aid)")
     ap.add_argument("--stepper", type=int, default=0, help="0 closed-form step (north_star), 1 the paper's implicit mid-point rule")
+    ap.add_argument("--precision", type=int, default=64, choices=[64, 32], help="arithmetic of the march (ABI buffers stay fp64)")
+    ap.add_argument("--no-fp32-leg", action="store_true", help="skip the extra FP32-mode timing that configs[4] asks for")
     return ap.parse_args()
 
 
@@ -165,7 +167,7 @@ def run_ours(a):
     torch.cuda.set_device(local)
     devname = f"cuda:{local}"
     wl = workload_from_args(a)
-    ctx = sc.ScContext.from_workload(wl, device=local, stepper=a.stepper)
+    ctx = sc.ScContext.from_workload(wl, device=local, stepper=a.stepper, precision=a.precision)
     if world > 1:
         # energy sharding: this rank marches its slice of the Matsubara table; one NCCL all-reduce of the
         # five accumulator fields per sweep; A-solve and mixing are replicated (deterministic, identical on all ranks)
@@ -255,9 +257,41 @@ def run_ours(a):
         e2e_s = float(tmax.item())
     bytes_io = ng * 16 + 2 * ng * 8
 
+    # configs[4]: "... FP64, with an FP32 mode also timed": the same step with opts.precision = 32 (same inputs, same
+    # warm-up and step counts), reported beside the FP64 headline, never instead of it
+    fp32_leg = None
+    if a.precision == 64 and wl.cfg == 4 and not a.no_fp32_leg and not a.sweep_only:
+        ctx.close(); del ctx
+        torch.cuda.empty_cache()
+        c32 = sc.ScContext.from_workload(wl, device=local, stepper=a.stepper, precision=32)
+        if world > 1:
+            from paper_2205_15000_b200 import sharding
+            sharding.attach(c32, wl.t, wl.n_energies)
+        c32.sc_set_external_field(dev_ax, dev_ay)
+        d32 = dev(wl.delta0.astype(np.complex128)); ax32 = torch.zeros_like(aix); ay32 = torch.zeros_like(aix)
+        for _ in range(max(a.warmup, 3)):
+            c32.sc_iterate(acc, 1.0, False, d32, ax32, ay32)
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        f0 = torch.cuda.Event(enable_timing=True); f1 = torch.cuda.Event(enable_timing=True)
+        f0.record()
+        for _ in range(a.steps):
+            c32.sc_iterate(acc, 1.0, False, d32, ax32, ay32)
+        f1.record(); torch.cuda.synchronize()
+        ms32 = f0.elapsed_time(f1)
+        if world > 1:
+            tmax = torch.tensor([ms32], dtype=torch.float64, device=devname)
+            dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+            ms32 = float(tmax.item())
+        fp32_leg = {"dtype": "f32", "value": n_updates * a.steps / (ms32 * 1e-3), "unit": UNIT, "ms_per_step": ms32 / a.steps,
+                    "march_ms": c32.last_march_ms(), "hbm_bytes_per_unit_algorithmic": 32.0}
+        c32.close()
+
     value = n_updates * a.steps / (ms * 1e-3)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": max(a.warmup, 3),
-            "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
+            "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+            "dtype": "f64" if a.precision == 64 else "f32",
             "data": "synthetic", "config": config_of(wl, a, {"seconds_per_self_consistent_iteration": ms / a.steps / 1e3,
                                                              "updates_per_step": n_updates, "updates_executed_per_step": n_exec,
                                                              "stepper": "closed-form" if a.stepper == 0 else "implicit mid-point",
@@ -266,6 +300,8 @@ def run_ours(a):
             "e2e": {"value": n_updates / e2e_s, "unit": UNIT, "h2d_bytes_per_step": bytes_io, "d2h_bytes_per_step": bytes_io + 64,
                     "res_delta_last": st2.res_delta},
             "gpu_launches": launches_per_step * a.steps, "roofline": roofline}
+    if fp32_leg:
+        line["config"]["fp32_mode"] = fp32_leg
     if not a.no_cpu_baseline and rank == 0:
         cores = os.cpu_count() or 1
         u, t, desc = oracle_sample(wl, cores)

@@ -71,12 +71,14 @@ struct sc_ctx {
     // fields
     DevBuf<double2> d_delta; DevBuf<double> d_Ax, d_Ay; bool have_A = false, have_fields = false;
     DevBuf<double> d_Aext_x, d_Aext_y; bool have_Aext = false;
-    DevBuf<double2> d_ndD; DevBuf<double> d_nda; DevBuf<double4> d_pc; bool nodes_fresh = false;
+    DevBuf<double2> d_ndD; DevBuf<double> d_nda; DevBuf<float2> d_ndDr; DevBuf<char> d_pc; bool nodes_fresh = false;
+    bool f32 = false;            // opts.precision == 32: pc, stores, scratch hold float; ABI buffers stay fp64
+    size_t rsz() const { return f32 ? sizeof(float) : sizeof(double); }
     // energies and stores
     EnergySet mats;
-    DevBuf<double2> d_store[2]; int cur = 0; bool stores_valid = false;
+    DevBuf<char> d_store[2]; int cur = 0; bool stores_valid = false;      // V2 of R [directed trajectory][energy]
     // scratch
-    DevBuf<double4> d_scr; long long scr_stride = 0; int n_slots = 0;
+    DevBuf<char> d_scr; long long scr_stride = 0; int n_slots = 0;       // scr_stride in bytes
     DevBuf<double> d_part; DevBuf<int> d_counter; DevBuf<int> d_nbad; DevBuf<double> d_statmax;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr, evm0 = nullptr, evm1 = nullptr;
     // Eq. 22 denominator sum (sum_n w_n t / eps_n over the WHOLE job's energy table) and the energy-shard hook
@@ -111,9 +113,14 @@ sc_status ensure_nodes(sc_ctx* ctx) {
     if (ctx->nodes_fresh) return SC_OK;
     if (!ctx->have_fields) return fail(ctx, SC_ERR_STATE, "sc_set_fields has not been called");
     const int wpb = 8;
-    sck::rotate_in_kernel<double><<<(ctx->G + wpb - 1) / wpb, wpb * 32, 0, ctx->stream>>>(
-        grid_dev(ctx), traj_dev(ctx), ctx->d_vx.p, ctx->d_vy.p, ctx->d_eta.p, ctx->geo.c, ctx->opt.charge_sign,
-        ctx->d_ndD.p, ctx->d_nda.p, nullptr, ctx->d_pc.p, ctx->d_nbad.p);
+    if (ctx->f32)
+        sck::rotate_in_kernel<float><<<(ctx->G + wpb - 1) / wpb, wpb * 32, 0, ctx->stream>>>(
+            grid_dev(ctx), traj_dev(ctx), ctx->d_vx.p, ctx->d_vy.p, ctx->d_eta.p, ctx->geo.c, ctx->opt.charge_sign,
+            ctx->d_ndD.p, ctx->d_nda.p, ctx->d_ndDr.p, (float4*)ctx->d_pc.p, ctx->d_nbad.p);
+    else
+        sck::rotate_in_kernel<double><<<(ctx->G + wpb - 1) / wpb, wpb * 32, 0, ctx->stream>>>(
+            grid_dev(ctx), traj_dev(ctx), ctx->d_vx.p, ctx->d_vy.p, ctx->d_eta.p, ctx->geo.c, ctx->opt.charge_sign,
+            ctx->d_ndD.p, ctx->d_nda.p, nullptr, (double4*)ctx->d_pc.p, ctx->d_nbad.p);
     if (!ctx->fb_rows.empty()) {
         const int n = (int)ctx->fb_rows.size();
         sck::fallback_kernel<<<(n + 127) / 128, 128, 0, ctx->stream>>>(grid_dev(ctx), n, ctx->d_fb_rows.p, ctx->d_fb_px.p,
@@ -124,10 +131,17 @@ sc_status ensure_nodes(sc_ctx* ctx) {
     return SC_OK;
 }
 
-sck::MarchArgs march_args(sc_ctx* ctx, const EnergySet& E, const double2* store_old, double2* store_new) {
-    sck::MarchArgs A{};
+template <typename R> const typename sck::VT<R>::V2* node_D(const sc_ctx* ctx);
+template <> const double2* node_D<double>(const sc_ctx* ctx) { return ctx->d_ndD.p; }
+template <> const float2* node_D<float>(const sc_ctx* ctx) { return ctx->d_ndDr.p; }
+
+template <typename R>
+sck::MarchArgsT<R> march_args(sc_ctx* ctx, const EnergySet& E, const char* store_old_raw, char* store_new_raw) {
+    using V2 = typename sck::VT<R>::V2; using V4 = typename sck::VT<R>::V4;
+    const V2* store_old = (const V2*)store_old_raw; V2* store_new = (V2*)store_new_raw;
+    sck::MarchArgsT<R> A{};
     A.T = traj_dev(ctx); A.E = E.dev(); A.order = ctx->d_order.p; A.n_items = ctx->G;
-    A.nd_D = ctx->d_ndD.p; A.pc = ctx->d_pc.p; A.bc_mode = ctx->opt.bc_mode;
+    A.nd_D = node_D<R>(ctx); A.pc = (const V4*)ctx->d_pc.p; A.bc_mode = ctx->opt.bc_mode;
     A.ga_idx = ctx->d_ga_idx.p; A.ga_w = ctx->d_ga_w.p; A.ga_n = ctx->d_ga_n.p;
     A.fb_D = ctx->d_fb_D.p; A.fb_a = ctx->d_fb_a.p;
     A.store_old = store_old; A.store_new = store_new;
@@ -136,33 +150,47 @@ sck::MarchArgs march_args(sc_ctx* ctx, const EnergySet& E, const double2* store_
     return A;
 }
 
-template <int MODE, bool STATS, int STEP>
-sc_status launch_march_t(sc_ctx* ctx, const sck::MarchArgs& A) {
+template <int MODE, bool STATS, int STEP, typename R>
+sc_status launch_march_t(sc_ctx* ctx, const sck::MarchArgsT<R>& A) {
     const int blocks = ctx->n_slots / sck::MARCH_WARPS;
-    const int smem = MODE == 0 ? sck::MARCH_SMEM : 0;
+    const int smem = MODE == 0 ? sck::march_smem<R>() : 0;
     static bool attr_set = false;
     if (MODE == 0 && !attr_set) {
-        CU(cudaFuncSetAttribute(sck::march_kernel<MODE, STATS, STEP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        CU(cudaFuncSetAttribute(sck::march_kernel<MODE, STATS, STEP, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         attr_set = true;
     }
     CU(cudaEventRecord(ctx->evm0, ctx->stream));
-    sck::march_kernel<MODE, STATS, STEP><<<blocks, sck::MARCH_WARPS * 32, smem, ctx->stream>>>(A);
+    sck::march_kernel<MODE, STATS, STEP, R><<<blocks, sck::MARCH_WARPS * 32, smem, ctx->stream>>>(A);
     CU(cudaEventRecord(ctx->evm1, ctx->stream));
     CU(cudaGetLastError());
     return SC_OK;
 }
 
-template <int MODE>
-sc_status launch_march(sc_ctx* ctx, const sck::MarchArgs& A, bool stats) {
-    CU(cudaMemsetAsync(ctx->d_counter.p, 0, sizeof(int), ctx->stream));
+template <int MODE, typename R>
+sc_status launch_march_r(sc_ctx* ctx, const EnergySet& E, const char* so, char* sn, bool stats,
+                         const int* items, int n_items, double* ldos) {
+    sck::MarchArgsT<R> A = march_args<R>(ctx, E, so, sn);
+    if (items) { A.order = items; A.n_items = n_items; }
+    A.ldos = ldos;
     const bool st = stats && MODE == 0;
-    if (ctx->opt.stepper == 1) return st ? launch_march_t<MODE, MODE == 0, 1>(ctx, A) : launch_march_t<MODE, false, 1>(ctx, A);
-    return st ? launch_march_t<MODE, MODE == 0, 0>(ctx, A) : launch_march_t<MODE, false, 0>(ctx, A);
+    if (ctx->opt.stepper == 1) return st ? launch_march_t<MODE, MODE == 0, 1, R>(ctx, A) : launch_march_t<MODE, false, 1, R>(ctx, A);
+    return st ? launch_march_t<MODE, MODE == 0, 0, R>(ctx, A) : launch_march_t<MODE, false, 0, R>(ctx, A);
 }
 
-sc_status reset_stores(sc_ctx* ctx, const EnergySet& E, double2* store) {
+// one march launch over the work list (default: all physical trajectories, longest first)
+template <int MODE>
+sc_status launch_march(sc_ctx* ctx, const EnergySet& E, const char* so, char* sn, bool stats,
+                       const int* items = nullptr, int n_items = 0, double* ldos = nullptr) {
+    CU(cudaMemsetAsync(ctx->d_counter.p, 0, sizeof(int), ctx->stream));
+    return ctx->f32 ? launch_march_r<MODE, float>(ctx, E, so, sn, stats, items, n_items, ldos)
+                    : launch_march_r<MODE, double>(ctx, E, so, sn, stats, items, n_items, ldos);
+}
+
+sc_status reset_stores(sc_ctx* ctx, const EnergySet& E, char* store) {
     const long long total = (long long)ctx->G * E.ne;
-    sck::reset_store_kernel<double><<<(unsigned)((total + 255) / 256), 256, 0, ctx->stream>>>(traj_dev(ctx), E.dev(), ctx->d_pc.p, store);
+    const unsigned nb = (unsigned)((total + 255) / 256);
+    if (ctx->f32) sck::reset_store_kernel<float><<<nb, 256, 0, ctx->stream>>>(traj_dev(ctx), E.dev(), (const float4*)ctx->d_pc.p, (float2*)store);
+    else sck::reset_store_kernel<double><<<nb, 256, 0, ctx->stream>>>(traj_dev(ctx), E.dev(), (const double4*)ctx->d_pc.p, (double2*)store);
     CU(cudaGetLastError());
     return SC_OK;
 }
@@ -214,9 +242,10 @@ sc_status sc_create(const sc_grid* grid, const unsigned char* mask, const sc_sha
     if (grid->nx < 2 || grid->ny < 2 || !(grid->h > 0)) return fail(ctx, SC_ERR_ARG, "bad grid");
     if (!(T_over_Tc > 0)) return fail(ctx, SC_ERR_ARG, "T/Tc must be positive");
     if (opts->n_matsubara < 1) return fail(ctx, SC_ERR_ARG, "n_matsubara < 1");
-    if (opts->precision != 64 && opts->precision != 0) return fail(ctx, SC_ERR_ARG, "only precision=64 is built in this version");
+    if (opts->precision != 64 && opts->precision != 32 && opts->precision != 0) return fail(ctx, SC_ERR_ARG, "precision must be 64 or 32");
     if (opts->stepper != 0 && opts->stepper != 1) return fail(ctx, SC_ERR_ARG, "stepper must be 0 (closed form) or 1 (implicit mid-point)");
     ctx->opt = *opts; ctx->grid = *grid; ctx->t = T_over_Tc; ctx->kappa = kappa; ctx->sym = (int)symmetry;
+    ctx->f32 = opts->precision == 32;
     if (ctx->opt.charge_sign == 0) ctx->opt.charge_sign = -1;
     // ---- geometry (host) ----
     scgeo::Geometry& Gm = ctx->geo;
@@ -305,7 +334,8 @@ sc_status sc_create(const sc_grid* grid, const unsigned char* mask, const sc_sha
 
     const size_t ng = (size_t)grid->nx * grid->ny;
     CU(ctx->d_delta.alloc(ng)); CU(ctx->d_Ax.alloc(ng)); CU(ctx->d_Ay.alloc(ng));
-    CU(ctx->d_ndD.alloc(nodes)); CU(ctx->d_nda.alloc(nodes)); CU(ctx->d_pc.alloc(nodes + G));
+    CU(ctx->d_ndD.alloc(nodes)); CU(ctx->d_nda.alloc(nodes)); CU(ctx->d_pc.alloc((size_t)(nodes + G) * 4 * ctx->rsz()));
+    if (ctx->f32) CU(ctx->d_ndDr.alloc(nodes));
     CU(ctx->d_part.alloc((size_t)nodes * sck::RED_VALS));
     CU(ctx->d_counter.alloc(1)); CU(ctx->d_nbad.alloc(1));
     CU(cudaMemsetAsync(ctx->d_nbad.p, 0, sizeof(int), s));
@@ -315,12 +345,12 @@ sc_status sc_create(const sc_grid* grid, const unsigned char* mask, const sc_sha
     for (int n = 0; n < opts->n_matsubara; ++n) { E.zr.push_back(0.0); E.zi.push_back(T_over_Tc * (n + 0.5)); E.w.push_back(1.0); E.partner.push_back(n); }
     if (sc_status st = upload_energies(ctx, E)) return st;
     for (int n = 0; n < opts->n_matsubara; ++n) ctx->denom_sum += 1.0 / (n + 0.5);
-    CU(ctx->d_store[0].alloc((size_t)ND * E.ne)); CU(ctx->d_store[1].alloc((size_t)ND * E.ne));
+    CU(ctx->d_store[0].alloc((size_t)ND * E.ne * 2 * ctx->rsz())); CU(ctx->d_store[1].alloc((size_t)ND * E.ne * 2 * ctx->rsz()));
 
     // persistent march grid: MARCH_MIN_CTAS CTAs of 8 warps per SM; per-warp scratch of (smax+1) pieces x 32 lanes
     ctx->n_slots = ctx->n_sm * sck::MARCH_MIN_CTAS * sck::MARCH_WARPS;
-    ctx->scr_stride = (long long)(smax + 2) * 32;
-    CU(ctx->d_scr.alloc((size_t)ctx->n_slots * ctx->scr_stride + 512));   // + 16 KB: the L2 prefetch of the last slot may run past its end
+    ctx->scr_stride = (long long)(smax + 2) * 32 * (opts->stepper == 1 ? 2 : 4) * (long long)ctx->rsz();
+    CU(ctx->d_scr.alloc((size_t)ctx->n_slots * ctx->scr_stride + 16384));   // + 16 KB: the L2 prefetch of the last slot may run past its end
     CU(ctx->d_statmax.alloc(ctx->n_slots));
     CU(cudaMemsetAsync(ctx->d_statmax.p, 0, ctx->n_slots * sizeof(double), s));
     CU(cudaStreamSynchronize(s));
@@ -367,7 +397,7 @@ sc_status sc_set_energies(sc_ctx* ctx, const double* z_re, const double* z_im, c
     ctx->denom_sum = std::isnan(denominator_sum) ? ds : denominator_sum;
     if (sc_status st = upload_energies(ctx, E)) return st;
     const size_t ND = ctx->geo.dt.size();
-    CU(ctx->d_store[0].alloc(ND * E.ne)); CU(ctx->d_store[1].alloc(ND * E.ne));
+    CU(ctx->d_store[0].alloc(ND * E.ne * 2 * ctx->rsz())); CU(ctx->d_store[1].alloc(ND * E.ne * 2 * ctx->rsz()));
     ctx->stores_valid = false; ctx->cur = 0;
     return SC_OK;
 }
@@ -392,8 +422,7 @@ sc_status sc_riccati_sweep(sc_ctx* ctx, void* delta_new, double* jx, double* jy,
     if (stats) { CU(cudaEventRecord(ctx->ev0, ctx->stream)); CU(cudaMemsetAsync(ctx->d_nbad.p, 0, sizeof(int), ctx->stream)); }
     if (sc_status st = ensure_nodes(ctx)) return st;
     if (!ctx->stores_valid) { if (sc_status st = sc_reset_boundary(ctx)) return st; }
-    sck::MarchArgs A = march_args(ctx, ctx->mats, ctx->d_store[ctx->cur].p, ctx->d_store[ctx->cur ^ 1].p);
-    if (sc_status st = launch_march<0>(ctx, A, stats != nullptr)) return st;
+    if (sc_status st = launch_march<0>(ctx, ctx->mats, ctx->d_store[ctx->cur].p, ctx->d_store[ctx->cur ^ 1].p, stats != nullptr)) return st;
     ctx->cur ^= 1;
     sck::BackArgs B = back_args(ctx, delta_new, jx, jy, fe_I);
     B.raw = ctx->hook_fn ? ctx->hook_acc : nullptr;
@@ -433,13 +462,12 @@ sc_status sc_ldos(sc_ctx* ctx, const double* energies, int n_e, double broadenin
     }
     if (sc_status st = upload_energies(ctx, E)) return st;
     const int ND = (int)ctx->geo.dt.size();
-    DevBuf<double2> st0, st1;
-    CU(st0.alloc((size_t)ND * E.ne)); CU(st1.alloc((size_t)ND * E.ne));
+    DevBuf<char> st0, st1;
+    CU(st0.alloc((size_t)ND * E.ne * 2 * ctx->rsz())); CU(st1.alloc((size_t)ND * E.ne * 2 * ctx->rsz()));
     if (sc_status st = reset_stores(ctx, E, st0.p)) return st;
-    double2* so = st0.p; double2* sn = st1.p;
+    char* so = st0.p; char* sn = st1.p;
     for (int it = 0; it + 1 < n_boundary_iters; ++it) {
-        sck::MarchArgs A = march_args(ctx, E, so, sn);
-        if (sc_status st = launch_march<2>(ctx, A, false)) return st;
+        if (sc_status st = launch_march<2>(ctx, E, so, sn, false)) return st;
         std::swap(so, sn);
     }
     // last sweep: per-energy Re g at every node, in batches of angle pairs sized to the free memory
@@ -463,14 +491,12 @@ sc_status sc_ldos(sc_ctx* ctx, const double* energies, int n_e, double broadenin
         std::vector<int> items;
         for (int g : ctx->h_order) if (ctx->h_k[g] >= p0 && ctx->h_k[g] < p1) items.push_back(g);
         CU(d_items.upload(items, ctx->stream));
-        sck::MarchArgs A = march_args(ctx, E, so, sn);
-        A.order = d_items.p; A.n_items = (int)items.size();
-        A.ldos = d_ldn.p - (size_t)pair_nodes[p0] * E.ne;       // node offsets are global
-        if (sc_status st = launch_march<1>(ctx, A, false)) return st;
+        double* const ldn = d_ldn.p - (size_t)pair_nodes[p0] * E.ne;       // node offsets are global
+        if (sc_status st = launch_march<1>(ctx, E, so, sn, false, d_items.p, (int)items.size(), ldn)) return st;
         sck::BackLdosArgs L{};
         L.B = back_args(ctx, nullptr, nullptr, nullptr, nullptr);
         L.ne_out = n_e; L.out_idx = d_out_idx.p; L.partner = E.d_partner.p; L.ne = E.ne;
-        L.ldos_nodes = A.ldos; L.out = ldos; L.p0 = p0; L.p1 = p1; L.accumulate = first ? 0 : 1;
+        L.ldos_nodes = ldn; L.out = ldos; L.p0 = p0; L.p1 = p1; L.accumulate = first ? 0 : 1;
         dim3 grd((n_e + 63) / 64, ctx->grid.nx, ctx->grid.ny);
         sck::rotate_back_ldos_kernel<<<grd, 64, 0, ctx->stream>>>(L);
         CU(cudaGetLastError());
@@ -568,8 +594,8 @@ sc_status sc_debug_trajectory(sc_ctx* ctx, int k, int local, int n_energy, int* 
     const int nn = ctx->h_nn[g];
     DevBuf<double2> dG, dGT; CU(dG.alloc(nn)); CU(dGT.alloc(nn));
     // the last sweep read store[cur^1] (now the "new" side) and wrote store[cur]
-    sck::MarchArgs A = march_args(ctx, ctx->mats, ctx->d_store[ctx->cur ^ 1].p, nullptr);
-    sck::debug_traj_kernel<<<1, 32, 0, ctx->stream>>>(A, ctx->opt.stepper, g, n_energy, dG.p, dGT.p);
+    if (ctx->f32) sck::debug_traj_kernel<float><<<1, 32, 0, ctx->stream>>>(march_args<float>(ctx, ctx->mats, ctx->d_store[ctx->cur ^ 1].p, nullptr), ctx->opt.stepper, g, n_energy, dG.p, dGT.p);
+    else sck::debug_traj_kernel<double><<<1, 32, 0, ctx->stream>>>(march_args<double>(ctx, ctx->mats, ctx->d_store[ctx->cur ^ 1].p, nullptr), ctx->opt.stepper, g, n_energy, dG.p, dGT.p);
     CU(cudaGetLastError());
     CU(cudaMemcpyAsync(gamma, dG.p, nn * sizeof(double2), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaMemcpyAsync(gamma_tilde, dGT.p, nn * sizeof(double2), cudaMemcpyDeviceToHost, ctx->stream));

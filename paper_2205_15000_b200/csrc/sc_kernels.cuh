@@ -17,6 +17,7 @@
 
 namespace sck {
 using scm::cplx;
+using scm::cplxf;
 using scm::cplx_t;
 using scm::mk;
 
@@ -156,38 +157,41 @@ __global__ void reset_store_kernel(TrajDev T, EnergyDev E, const typename VT<R>:
 }
 
 // ------------------------------------------------------------------------------------------------
-// the march
+// the march (working precision R = double, or float with opts.precision = 32)
 // ------------------------------------------------------------------------------------------------
-struct MarchArgs {
+template <typename R>
+struct MarchArgsT {
+    using V2 = typename VT<R>::V2; using V4 = typename VT<R>::V4;
     TrajDev T;
     EnergyDev E;
     const int* order; int n_items;          // longest-first work list
-    const double2* nd_D;                    // node coefficients Delta_j eta_k           [node]
-    const double4* pc;                      // piece coefficients {Re De, Im De, a, len} [node + g]
+    const V2* nd_D;                         // node coefficients Delta_j eta_k           [node]
+    const V4* pc;                           // piece coefficients {Re De, Im De, a, len} [node + g]
     int bc_mode;
     const int* ga_idx; const double* ga_w; const unsigned char* ga_n;   // entry gathers per store row [row][4]
     const double2* fb_D; const double* fb_a;
-    const double2* store_old; double2* store_new;
-    double4* scr; long long scr_stride;     // per warp slot: (smax+2)*32 entries {T.re, T.im, gt.re, gt.im}
+    const V2* store_old; V2* store_new;
+    char* scr; long long scr_stride;        // per warp slot: scr_stride bytes = (smax+2) rows of 32 entries
     double* part;                           // MODE 0: [node][6] = SF.re, SF.im, X2.re, X2.im, SG, SI
     double* ldos;                           // MODE 1: [node][ne] = Re g_n
     int* counter;
     double* stat_max2;                      // per warp slot: max |gamma|^2 seen (optional)
 };
+using MarchArgs = MarchArgsT<double>;
 
 constexpr int MARCH_WARPS = 8;               // warps per CTA
 #ifndef SC_MARCH_MIN_CTAS
 #define SC_MARCH_MIN_CTAS 2
 #endif
-constexpr int MARCH_MIN_CTAS = SC_MARCH_MIN_CTAS;   // resident CTAs per SM the register budget is sized for
+constexpr int MARCH_MIN_CTAS = SC_MARCH_MIN_CTAS;   // resident CTAs per SM the fp64 register budget is sized for
 constexpr int PF_DIST = 12;                  // pass 2: scratch lines are pulled into L2 this many nodes ahead
 constexpr int RED_NODES = 4;                 // nodes per shared-memory reduction batch
 constexpr int RED_VALS = 6;
 constexpr int STAGE_LD = 33;                 // padded row of the transpose stage: conflict-free rows AND columns
-constexpr int MARCH_SMEM = MARCH_WARPS * RED_NODES * RED_VALS * STAGE_LD * (int)sizeof(double);   // 50688 B (> 48 KB: opt-in)
+template <typename R> constexpr int march_smem() { return MARCH_WARPS * RED_NODES * RED_VALS * STAGE_LD * (int)sizeof(R); }   // fp64: 50688 B (> 48 KB: opt-in)
 
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
-// 256-bit global accesses (LDG.E.ENL2.256 / STG.E.ENL2.256 on sm_100a): one scratch entry per lane per instruction
+// 256-bit global accesses (LDG.E.ENL2.256 / STG.E.ENL2.256 on sm_100a): one fp64 scratch entry per lane per instruction
 __device__ __forceinline__ double4 ld256(const double4* p) {
     double4 v;
     asm volatile("ld.global.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v.x), "=d"(v.y), "=d"(v.z), "=d"(v.w) : "l"(p));
@@ -196,60 +200,72 @@ __device__ __forceinline__ double4 ld256(const double4* p) {
 __device__ __forceinline__ void st256(double4* p, double a, double b, double c, double d) {
     asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
 }
-__device__ __forceinline__ double4 ldu256(const double4* p) {      // warp-uniform coefficient record (read-only path)
+// warp-uniform coefficient record (read-only path)
+__device__ __forceinline__ double4 ldu(const double4* p) {
     double4 v;
     asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v.x), "=d"(v.y), "=d"(v.z), "=d"(v.w) : "l"(p));
     return v;
 }
+__device__ __forceinline__ float4 ldu(const float4* p) { return __ldg(p); }
 
-__device__ __forceinline__ cplx gather_start(const MarchArgs& A, int row, int n) {
+template <typename R>
+__device__ __forceinline__ cplx_t<R> gather_start(const MarchArgsT<R>& A, int row, int n) {
     const int cnt = A.ga_n[row];
-    double sr = 0.0, si = 0.0;
+    R sr = R(0), si = R(0);
     for (int i = 0; i < cnt; ++i) {
-        const double w = A.ga_w[4 * row + i];
-        const double2 v = A.store_old[(size_t)A.ga_idx[4 * row + i] * A.E.ne + n];
-        sr = fma(w, v.x, sr); si = fma(w, v.y, si);
+        const R w = (R)A.ga_w[4 * row + i];
+        const typename VT<R>::V2 v = A.store_old[(size_t)A.ga_idx[4 * row + i] * A.E.ne + n];
+        sr = scm::mad(w, v.x, sr); si = scm::mad(w, v.y, si);
     }
     return mk(sr, si);
+}
+template <typename R>
+__device__ __forceinline__ cplx_t<R> hom_start(double Dr, double Di, double zr, double zi) {   // rare: fp64 library math
+    const cplx s = scm::gamma_hom(Dr, Di, zr, zi);
+    return mk((R)s.re, (R)s.im);
 }
 
 // products at one node (Eq. 24 :165): P = gamma gamma~, 1/(1+P); writes the six weighted terms of the
 // energy sums into rows r..r+5 of the warp's transpose stage (MODE 0), or returns Re g (MODE 1)
-template <int MODE, bool STATS>
-__device__ __forceinline__ double node_products(cplx gm, double gtr, double gti, double2 Dn, double wn, double* st, double& max2) {
-    const double Pr = fma(gm.re, gtr, -gm.im * gti), Pi = fma(gm.re, gti, gm.im * gtr);
-    const double qr = 1.0 + Pr;
-    const double rq = scm::rcp_nr(fma(qr, qr, Pi * Pi));
-    const double ir = qr * rq, ii = -Pi * rq;               // 1/(1+P)
-    if (STATS) max2 = fmax(max2, fmax(fma(gm.re, gm.re, gm.im * gm.im), fma(gtr, gtr, gti * gti)));
+template <int MODE, bool STATS, typename R>
+__device__ __forceinline__ R node_products(cplx_t<R> gm, R gtr, R gti, typename VT<R>::V2 Dn, R wn, R* st, R& max2) {
+    using scm::mad;
+    const R Pr = mad(gm.re, gtr, -gm.im * gti), Pi = mad(gm.re, gti, gm.im * gtr);
+    const R qr = R(1) + Pr;
+    const R rq = scm::rcp_nr(mad(qr, qr, Pi * Pi));
+    const R ir = qr * rq, ii = -Pi * rq;               // 1/(1+P)
+    if (STATS) max2 = scm::maxr(max2, scm::maxr(mad(gm.re, gm.re, gm.im * gm.im), mad(gtr, gtr, gti * gti)));
     if (MODE == 0) {
-        const double wr = wn * ir, wi = wn * ii;
-        st[0 * STAGE_LD] = fma(gm.re, wr, -gm.im * wi);      // SF  = w gamma/(1+P)
-        st[1 * STAGE_LD] = fma(gm.re, wi, gm.im * wr);
-        st[2 * STAGE_LD] = fma(gtr, wr, -gti * wi);          // X2  = w gamma~/(1+P)  (SF of k+N/2 = conj)
-        st[3 * STAGE_LD] = fma(gtr, wi, gti * wr);
-        st[4 * STAGE_LD] = 2.0 * wi;                         // SG  = w Im g = 2 w Im 1/(1+P)
-        st[5 * STAGE_LD] = wn * fma(Dn.x, gm.im - gti, -Dn.y * (gm.re + gtr));   // SI (Eq. 19 :128 numerator)
+        const R wr = wn * ir, wi = wn * ii;
+        st[0 * STAGE_LD] = mad(gm.re, wr, -gm.im * wi);      // SF  = w gamma/(1+P)
+        st[1 * STAGE_LD] = mad(gm.re, wi, gm.im * wr);
+        st[2 * STAGE_LD] = mad(gtr, wr, -gti * wi);          // X2  = w gamma~/(1+P)  (SF of k+N/2 = conj)
+        st[3 * STAGE_LD] = mad(gtr, wi, gti * wr);
+        st[4 * STAGE_LD] = R(2) * wi;                        // SG  = w Im g = 2 w Im 1/(1+P)
+        st[5 * STAGE_LD] = wn * mad(Dn.x, gm.im - gti, -Dn.y * (gm.re + gtr));   // SI (Eq. 19 :128 numerator)
     }
-    return fma(2.0, ir, -1.0);                               // Re g = 2 Re 1/(1+P) - 1
+    return mad(R(2), ir, R(-1));                             // Re g = 2 Re 1/(1+P) - 1
 }
 
 // column sums of the stage: lane c < cnt sums row c over the 32 lanes (4 partial sums, fixed order)
-__device__ __forceinline__ double stage_colsum(const double* stage, int lane) {
-    const double* col = stage + lane * STAGE_LD;
-    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+template <typename R>
+__device__ __forceinline__ double stage_colsum(const R* stage, int lane) {
+    const R* col = stage + lane * STAGE_LD;
+    R s0 = R(0), s1 = R(0), s2 = R(0), s3 = R(0);
 #pragma unroll
     for (int i = 0; i < 32; i += 4) { s0 += col[i]; s1 += col[i + 1]; s2 += col[i + 2]; s3 += col[i + 3]; }
-    return (s0 + s1) + (s2 + s3);
+    return (double)((s0 + s1) + (s2 + s3));
 }
 
-// Scratch entry of one (piece, lane): STEP 0 (closed form) {T.re, T.im, gt.re, gt.im} = 32 B, one 256-bit access;
-// STEP 1 (mid-point) {gt.re, gt.im} = 16 B, one 128-bit access.  A warp's 32 entries of a piece are contiguous.
-struct Ent { double tr, ti, gr, gi; };
-template <int STEP> struct ScrT { static constexpr int BYTES = STEP == 0 ? 32 : 16; static constexpr int ROW = 32 * BYTES; };
+// Scratch entry of one (piece, lane): STEP 0 (closed form) {T.re, T.im, gt.re, gt.im} = 4 R, one 256-bit (fp64) or
+// 128-bit (fp32) access; STEP 1 (mid-point) {gt.re, gt.im} = 2 R.  A warp's 32 entries of a piece are contiguous.
+template <typename R> struct Ent { R tr, ti, gr, gi; };
+template <typename R, int STEP> struct ScrT {
+    static constexpr int BYTES = (STEP == 0 ? 4 : 2) * (int)sizeof(R); static constexpr int ROW = 32 * BYTES;
+};
 template <int STEP>
-__device__ __forceinline__ Ent ld_ent(const char* p) {
-    Ent e;
+__device__ __forceinline__ Ent<double> ld_ent(const char* p, double) {
+    Ent<double> e;
     if (STEP == 0) { const double4 v = ld256((const double4*)p); e.tr = v.x; e.ti = v.y; e.gr = v.z; e.gi = v.w; }
     else {
         asm volatile("ld.global.v2.f64 {%0,%1}, [%2];" : "=d"(e.gr), "=d"(e.gi) : "l"(p));
@@ -258,29 +274,45 @@ __device__ __forceinline__ Ent ld_ent(const char* p) {
     return e;
 }
 template <int STEP>
+__device__ __forceinline__ Ent<float> ld_ent(const char* p, float) {
+    Ent<float> e;
+    if (STEP == 0) asm volatile("ld.global.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(e.tr), "=f"(e.ti), "=f"(e.gr), "=f"(e.gi) : "l"(p));
+    else {
+        asm volatile("ld.global.v2.f32 {%0,%1}, [%2];" : "=f"(e.gr), "=f"(e.gi) : "l"(p));
+        e.tr = e.ti = 0.f;
+    }
+    return e;
+}
+template <int STEP>
 __device__ __forceinline__ void st_ent(char* p, cplx T, cplx gt) {
     if (STEP == 0) st256((double4*)p, T.re, T.im, gt.re, gt.im);
     else asm volatile("st.global.v2.f64 [%0], {%1,%2};" ::"l"(p), "d"(gt.re), "d"(gt.im) : "memory");
 }
-// one step of gamma with piece record cc; STEP 0 re-uses the stored T of the piece
 template <int STEP>
-__device__ __forceinline__ cplx step_up(cplx g, const double4& cc, double zr0, double zi0, const Ent& E) {
+__device__ __forceinline__ void st_ent(char* p, cplxf T, cplxf gt) {
+    if (STEP == 0) asm volatile("st.global.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(p), "f"(T.re), "f"(T.im), "f"(gt.re), "f"(gt.im) : "memory");
+    else asm volatile("st.global.v2.f32 [%0], {%1,%2};" ::"l"(p), "f"(gt.re), "f"(gt.im) : "memory");
+}
+// one step of gamma with piece record cc; STEP 0 re-uses the stored T of the piece
+template <int STEP, typename R>
+__device__ __forceinline__ cplx_t<R> step_up(cplx_t<R> g, const typename VT<R>::V4& cc, R zr0, R zi0, const Ent<R>& E) {
     if (STEP == 0) return scm::step_T(g, cc.x, cc.y, zr0 + cc.z, zi0, mk(E.tr, E.ti));
     return scm::step_mid(g, cc.x, cc.y, zr0 + cc.z, zi0, cc.w);
 }
 
 // MODE 0: Matsubara sums; 1: per-energy Re g (LDOS); 2: boundary values only.
 // STEP 0: closed-form step; 1: implicit mid-point rule (C4-C9 :984-1001).
-template <int MODE, bool STATS, int STEP>
-__global__ void __launch_bounds__(MARCH_WARPS * 32, MARCH_MIN_CTAS) march_kernel(MarchArgs A) {
-    extern __shared__ double stage_all[];        // MODE 0: MARCH_WARPS x (24 rows x STAGE_LD) doubles (MARCH_SMEM bytes)
-    constexpr int ROW = ScrT<STEP>::ROW;
+template <int MODE, bool STATS, int STEP, typename R>
+__global__ void __launch_bounds__(MARCH_WARPS * 32, MARCH_MIN_CTAS) march_kernel(MarchArgsT<R> A) {
+    using V2 = typename VT<R>::V2; using V4 = typename VT<R>::V4;
+    extern __shared__ double stage_raw[];        // MODE 0: MARCH_WARPS x (24 rows x STAGE_LD) values of R
+    constexpr int ROW = ScrT<R, STEP>::ROW, BYTES = ScrT<R, STEP>::BYTES;
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const int slot = blockIdx.x * MARCH_WARPS + wib;
-    double* const stage = stage_all + wib * (RED_NODES * RED_VALS * STAGE_LD);
-    char* const scr = (char*)(A.scr + (size_t)slot * A.scr_stride) + lane * ScrT<STEP>::BYTES;   // entry e of this lane: scr + e*ROW
+    R* const stage = reinterpret_cast<R*>(stage_raw) + wib * (RED_NODES * RED_VALS * STAGE_LD);
+    char* const scr = A.scr + (size_t)slot * A.scr_stride + lane * BYTES;   // entry e of this lane: scr + e*ROW
     const int ne = A.E.ne;
-    double max2 = 0.0;
+    R max2 = R(0);
 
     for (;;) {
         int item = 0;
@@ -291,40 +323,40 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32, MARCH_MIN_CTAS) march_kernel
         const int nn = A.T.nn[g];
         const long long noff = A.T.noff[g];
         const int dF = A.T.dF[g], dB = A.T.dB[g];
-        const double2* __restrict__ ND = A.nd_D + noff;
-        const double4* __restrict__ PC = A.pc + noff + g;
+        const V2* __restrict__ ND = A.nd_D + noff;
+        const V4* __restrict__ PC = A.pc + noff + g;
 
         for (int n0 = 0; n0 < ne; n0 += 32) {
             const bool act = n0 + lane < ne;
             const int n = act ? n0 + lane : ne - 1;
-            const double zr0 = A.E.zr[n], zi0 = A.E.zi[n];
-            const double wn = act ? A.E.w[n] : 0.0;
+            const R zr0 = (R)A.E.zr[n], zi0 = (R)A.E.zi[n];
+            const R wn = act ? (R)A.E.w[n] : R(0);
             const int nb = A.E.partner[n];
 
             // ---------------- pass 1: gamma-tilde from u_out down to u_in; entry p = {T_p, gamma~(node p-1)} ----------
-            double4 c4 = ldu256(PC + nn);
-            cplx gt;
+            V4 c4 = ldu(PC + nn);
+            cplx_t<R> gt;
             if (A.bc_mode == 1) {
-                gt = scm::gamma_hom(-c4.x, c4.y, zr0 + c4.z, zi0);
+                gt = hom_start<R>(-(double)c4.x, c4.y, A.E.zr[n] + c4.z, A.E.zi[n]);
             } else if (A.ga_n[dB]) {
-                const cplx s = gather_start(A, dB, nb);            // gamma of the mirrored trajectory at its entry
+                const cplx_t<R> s = gather_start(A, dB, nb);            // gamma of the mirrored trajectory at its entry
                 gt = mk(s.re, -s.im);
             } else {
-                const cplx s = scm::gamma_hom(A.fb_D[dB].x, A.fb_D[dB].y, A.E.zr[nb] + A.fb_a[dB], A.E.zi[nb]);
+                const cplx_t<R> s = hom_start<R>(A.fb_D[dB].x, A.fb_D[dB].y, A.E.zr[nb] + A.fb_a[dB], A.E.zi[nb]);
                 gt = mk(s.re, -s.im);
             }
             {
                 char* e = scr + (size_t)nn * ROW;
-                double4 cn = ldu256(PC + (nn >= 1 ? nn - 1 : 0));
+                V4 cn = ldu(PC + (nn >= 1 ? nn - 1 : 0));
 #pragma unroll 2
                 for (int p = nn; p >= 0; --p) {
-                    const double4 cc = c4;
+                    const V4 cc = c4;
                     c4 = cn;
-                    if (p >= 2) cn = ldu256(PC + p - 2);                       // coefficient record two pieces ahead
-                    const double zr = zr0 + cc.z;
-                    cplx T = mk(0.0, 0.0);
+                    if (p >= 2) cn = ldu(PC + p - 2);                          // coefficient record two pieces ahead
+                    const R zr = zr0 + cc.z;
+                    cplx_t<R> T = mk(R(0), R(0));
                     if (STEP == 0) {
-                        T = scm::coef_T(fma(cc.x, cc.x, cc.y * cc.y), zr, zi0, cc.w);
+                        T = scm::coef_T(scm::mad(cc.x, cc.x, cc.y * cc.y), zr, zi0, cc.w);
                         gt = scm::step_T(gt, -cc.x, cc.y, zr, zi0, T);
                     } else {
                         gt = scm::step_mid(gt, -cc.x, cc.y, zr, zi0, cc.w);
@@ -332,40 +364,40 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32, MARCH_MIN_CTAS) march_kernel
                     st_ent<STEP>(e, T, gt);
                     e -= ROW;
                 }
-                if (act) A.store_new[(size_t)dB * ne + nb] = make_double2(gt.re, -gt.im);
+                if (act) A.store_new[(size_t)dB * ne + nb] = mk2(gt.re, -gt.im);
             }
 
             // ---------------- pass 2: gamma from u_in up to u_out; products and energy reduction ------------
-            cplx gm;
+            cplx_t<R> gm;
             {
-                const double4 c0 = ldu256(PC);
-                if (A.bc_mode == 1) gm = scm::gamma_hom(c0.x, c0.y, zr0 + c0.z, zi0);
+                const V4 c0 = ldu(PC);
+                if (A.bc_mode == 1) gm = hom_start<R>(c0.x, c0.y, A.E.zr[n] + c0.z, A.E.zi[n]);
                 else if (A.ga_n[dF]) gm = gather_start(A, dF, n);
-                else gm = scm::gamma_hom(A.fb_D[dF].x, A.fb_D[dF].y, zr0 + A.fb_a[dF], zi0);
-                const Ent e0 = ld_ent<STEP>(scr);
-                gm = step_up<STEP>(gm, c0, zr0, zi0, e0);
+                else gm = hom_start<R>(A.fb_D[dF].x, A.fb_D[dF].y, A.E.zr[n] + A.fb_a[dF], A.E.zi[n]);
+                const Ent<R> e0 = ld_ent<STEP>(scr, R(0));
+                gm = step_up<STEP, R>(gm, c0, zr0, zi0, e0);
             }
             const char* e = scr + ROW;                  // entry of node 0
-            for (int q = 4; q < PF_DIST && q < nn; q += 4) prefetch_l2(e - lane * ScrT<STEP>::BYTES + (size_t)q * ROW + lane * 128);
-            Ent En = ld_ent<STEP>(e);
-            double4 cN = ldu256(PC + 1);
-            double2 dN = ND[0];
+            for (int q = 4; q < PF_DIST && q < nn; q += 4) prefetch_l2(e - lane * BYTES + (size_t)q * ROW + lane * 128);
+            Ent<R> En = ld_ent<STEP>(e, R(0));
+            V4 cN = ldu(PC + 1);
+            V2 dN = ND[0];
             int m = 0;
             for (; m + RED_NODES <= nn; m += RED_NODES) {
-                if (m + PF_DIST < nn) prefetch_l2(e - lane * ScrT<STEP>::BYTES + (size_t)PF_DIST * ROW + lane * 128);
+                if (m + PF_DIST < nn) prefetch_l2(e - lane * BYTES + (size_t)PF_DIST * ROW + lane * 128);
                 double part_old = 0.0;
                 if (MODE == 0 && n0 && lane < RED_NODES * RED_VALS) part_old = A.part[(size_t)(noff + m) * RED_VALS + lane];
 #pragma unroll
                 for (int b = 0; b < RED_NODES; ++b) {
-                    const Ent Ec = En; const double4 cc = cN; const double2 dc = dN;
-                    En = ld_ent<STEP>(e + (b + 1) * ROW);                // one node ahead (scratch has 2 spare entries)
-                    cN = ldu256(PC + m + b + 2 <= PC + nn ? PC + m + b + 2 : PC + nn);
+                    const Ent<R> Ec = En; const V4 cc = cN; const V2 dc = dN;
+                    En = ld_ent<STEP>(e + (b + 1) * ROW, R(0));          // one node ahead (scratch has 2 spare entries)
+                    cN = ldu(PC + m + b + 2 <= PC + nn ? PC + m + b + 2 : PC + nn);
                     dN = ND[m + b + 1 < nn ? m + b + 1 : nn - 1];
                     if (MODE != 2) {
-                        const double rg = node_products<MODE, STATS>(gm, Ec.gr, Ec.gi, dc, wn, stage + b * RED_VALS * STAGE_LD + lane, max2);
-                        if (MODE == 1 && act) A.ldos[(size_t)(noff + m + b) * ne + n] = rg;
+                        const R rg = node_products<MODE, STATS, R>(gm, Ec.gr, Ec.gi, dc, wn, stage + b * RED_VALS * STAGE_LD + lane, max2);
+                        if (MODE == 1 && act) A.ldos[(size_t)(noff + m + b) * ne + n] = (double)rg;
                     }
-                    gm = step_up<STEP>(gm, cc, zr0, zi0, Ec);
+                    gm = step_up<STEP, R>(gm, cc, zr0, zi0, Ec);
                 }
                 e += RED_NODES * ROW;
                 if (MODE == 0) {
@@ -383,15 +415,15 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32, MARCH_MIN_CTAS) march_kernel
                 double part_old = 0.0;
                 if (MODE == 0 && n0 && lane < rem * RED_VALS) part_old = A.part[(size_t)(noff + m) * RED_VALS + lane];
                 for (int b = 0; b < rem; ++b) {
-                    const Ent Ec = En; const double4 cc = cN; const double2 dc = dN;
-                    En = ld_ent<STEP>(e + (b + 1) * ROW);
-                    cN = ldu256(PC + m + b + 2 <= PC + nn ? PC + m + b + 2 : PC + nn);
+                    const Ent<R> Ec = En; const V4 cc = cN; const V2 dc = dN;
+                    En = ld_ent<STEP>(e + (b + 1) * ROW, R(0));
+                    cN = ldu(PC + m + b + 2 <= PC + nn ? PC + m + b + 2 : PC + nn);
                     dN = ND[m + b + 1 < nn ? m + b + 1 : nn - 1];
                     if (MODE != 2) {
-                        const double rg = node_products<MODE, STATS>(gm, Ec.gr, Ec.gi, dc, wn, stage + b * RED_VALS * STAGE_LD + lane, max2);
-                        if (MODE == 1 && act) A.ldos[(size_t)(noff + m + b) * ne + n] = rg;
+                        const R rg = node_products<MODE, STATS, R>(gm, Ec.gr, Ec.gi, dc, wn, stage + b * RED_VALS * STAGE_LD + lane, max2);
+                        if (MODE == 1 && act) A.ldos[(size_t)(noff + m + b) * ne + n] = (double)rg;
                     }
-                    gm = step_up<STEP>(gm, cc, zr0, zi0, Ec);
+                    gm = step_up<STEP, R>(gm, cc, zr0, zi0, Ec);
                 }
                 if (MODE == 0) {
                     __syncwarp();
@@ -403,13 +435,14 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32, MARCH_MIN_CTAS) march_kernel
                     __syncwarp();
                 }
             }
-            if (act) A.store_new[(size_t)dF * ne + n] = make_double2(gm.re, gm.im);
+            if (act) A.store_new[(size_t)dF * ne + n] = mk2(gm.re, gm.im);
         }
     }
     if (STATS) {
+        double mx = (double)max2;
 #pragma unroll
-        for (int o = 16; o; o >>= 1) max2 = fmax(max2, __shfl_xor_sync(0xffffffffu, max2, o));
-        if (lane == 0) A.stat_max2[slot] = max2;
+        for (int o = 16; o; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+        if (lane == 0) A.stat_max2[slot] = mx;
     }
 }
 
@@ -565,31 +598,33 @@ __global__ void rotate_back_ldos_kernel(BackLdosArgs L) {
 // debug / measurement kernels
 // ------------------------------------------------------------------------------------------------
 // re-march one trajectory for one energy with the same device functions; writes gamma, gamma-tilde per node
-__global__ void debug_traj_kernel(MarchArgs A, int stepper, int g, int n, double2* outG, double2* outGT) {
+template <typename R>
+__global__ void debug_traj_kernel(MarchArgsT<R> A, int stepper, int g, int n, double2* outG, double2* outGT) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    using V4 = typename VT<R>::V4;
     const int nn = A.T.nn[g];
-    const double4* PC = A.pc + A.T.noff[g] + g;
+    const V4* PC = A.pc + A.T.noff[g] + g;
     const int nb = A.E.partner[n];
-    const double zr0 = A.E.zr[n], zi0 = A.E.zi[n];
+    const R zr0 = (R)A.E.zr[n], zi0 = (R)A.E.zi[n];
     const int dF = A.T.dF[g], dB = A.T.dB[g];
-    cplx gt;
-    if (A.bc_mode == 1) gt = scm::gamma_hom(-PC[nn].x, PC[nn].y, zr0 + PC[nn].z, zi0);
-    else if (A.ga_n[dB]) { cplx s = gather_start(A, dB, nb); gt = mk(s.re, -s.im); }
-    else { cplx s = scm::gamma_hom(A.fb_D[dB].x, A.fb_D[dB].y, A.E.zr[nb] + A.fb_a[dB], A.E.zi[nb]); gt = mk(s.re, -s.im); }
+    cplx_t<R> gt;
+    if (A.bc_mode == 1) gt = hom_start<R>(-(double)PC[nn].x, PC[nn].y, A.E.zr[n] + PC[nn].z, A.E.zi[n]);
+    else if (A.ga_n[dB]) { cplx_t<R> s = gather_start(A, dB, nb); gt = mk(s.re, -s.im); }
+    else { cplx_t<R> s = hom_start<R>(A.fb_D[dB].x, A.fb_D[dB].y, A.E.zr[nb] + A.fb_a[dB], A.E.zi[nb]); gt = mk(s.re, -s.im); }
     for (int p = nn; p >= 1; --p) {
-        const double4 c = PC[p];
+        const V4 c = PC[p];
         if (stepper == 1) gt = scm::step_mid(gt, -c.x, c.y, zr0 + c.z, zi0, c.w);
-        else { const cplx T = scm::coef_T(c.x * c.x + c.y * c.y, zr0 + c.z, zi0, c.w); gt = scm::step_T(gt, -c.x, c.y, zr0 + c.z, zi0, T); }
+        else { const cplx_t<R> T = scm::coef_T(scm::mad(c.x, c.x, c.y * c.y), zr0 + c.z, zi0, c.w); gt = scm::step_T(gt, -c.x, c.y, zr0 + c.z, zi0, T); }
         outGT[p - 1] = make_double2(gt.re, gt.im);
     }
-    cplx gm;
-    if (A.bc_mode == 1) gm = scm::gamma_hom(PC[0].x, PC[0].y, zr0 + PC[0].z, zi0);
+    cplx_t<R> gm;
+    if (A.bc_mode == 1) gm = hom_start<R>(PC[0].x, PC[0].y, A.E.zr[n] + PC[0].z, A.E.zi[n]);
     else if (A.ga_n[dF]) gm = gather_start(A, dF, n);
-    else gm = scm::gamma_hom(A.fb_D[dF].x, A.fb_D[dF].y, zr0 + A.fb_a[dF], zi0);
+    else gm = hom_start<R>(A.fb_D[dF].x, A.fb_D[dF].y, A.E.zr[n] + A.fb_a[dF], A.E.zi[n]);
     for (int p = 0; p < nn; ++p) {
-        const double4 c = PC[p];
+        const V4 c = PC[p];
         if (stepper == 1) gm = scm::step_mid(gm, c.x, c.y, zr0 + c.z, zi0, c.w);
-        else { const cplx T = scm::coef_T(c.x * c.x + c.y * c.y, zr0 + c.z, zi0, c.w); gm = scm::step_T(gm, c.x, c.y, zr0 + c.z, zi0, T); }
+        else { const cplx_t<R> T = scm::coef_T(scm::mad(c.x, c.x, c.y * c.y), zr0 + c.z, zi0, c.w); gm = scm::step_T(gm, c.x, c.y, zr0 + c.z, zi0, T); }
         outG[p] = make_double2(gm.re, gm.im);
     }
 }

@@ -13,6 +13,7 @@ torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
 
 TOL = 1e-9
+TOL32 = 2e-4          # north_star: "to 2e-4 in the optional FP32 mode"
 
 
 def relerr(a, b):
@@ -52,7 +53,7 @@ class GpuRun:
                     fe_I=self.fe.cpu().numpy(), stats=st)
 
 
-def compare_sweeps(sc, wl, n_sweeps=2, **kw):
+def compare_sweeps(sc, wl, n_sweeps=2, tol=TOL, **kw):
     o = oracle.Oracle.from_workload(wl, **{k: v for k, v in kw.items() if k in ("bc_mode", "stepper")})
     g = GpuRun(sc, wl, **kw)
     Ax = wl.Aext_x if np.any(wl.Aext_x) else None
@@ -66,11 +67,11 @@ def compare_sweeps(sc, wl, n_sweeps=2, **kw):
         rg = g.sweep()
         for key in ("delta_new", "jx", "jy", "fe_I"):
             e = relerr(rg[key], ro[key])
-            assert e < TOL, (it, key, e)
+            assert e < tol, (it, key, e)
             worst = max(worst, e)
         assert rg["stats"].n_bad == 0 and ro["stats"]["n_bad"] == 0
         assert rg["stats"].n_updates == ro["stats"]["n_updates"]
-        assert abs(rg["stats"].min_one_minus_abs_gamma - ro["stats"]["min_one_minus_abs_gamma"]) < 1e-9
+        assert abs(rg["stats"].min_one_minus_abs_gamma - ro["stats"]["min_one_minus_abs_gamma"]) < max(1e-9, tol)
         assert np.all(rg["delta_new"][wl.mask == 0] == 0)
     return o, g, stores, worst
 
@@ -139,6 +140,34 @@ def test_midpoint_stepper_parity(sc, cfg, kw):
     r1 = g1.sweep()
     d = relerr(r1["delta_new"], r0["delta_new"])
     assert 1e-8 < d < 5e-2, d
+
+
+@pytest.mark.parametrize("cfg,kw,ns", [
+    (0, {}, 3),
+    (1, dict(pts_per_xi=6, n_angles=16, n_energies=40), 2),          # A != 0, ragged energy tail
+    (2, dict(pts_per_xi=5, n_angles=32, n_energies=33, size_scale=0.5), 2),
+    (4, dict(pts_per_xi=5, n_angles=16, n_energies=64, size_scale=0.2), 2),
+])
+@pytest.mark.parametrize("stepper", [0, 1])
+def test_fp32_mode_parity(sc, cfg, kw, ns, stepper):
+    """opts.precision = 32: the march in float (pieces, scratch, boundary stores), fp64 ABI and fp64 oracle; 2e-4."""
+    wl = wlmod.make_workload(cfg, **kw)
+    o, g, stores, worst = compare_sweeps(sc, wl, n_sweeps=ns, tol=TOL32, precision=32, stepper=stepper)
+    assert worst > 1e-12          # it really is a float path
+    # per-trajectory tap in the same precision
+    z, _ = o.matsubara(wl.n_energies)
+    Ax = wl.Aext_x if np.any(wl.Aext_x) else None
+    Ay = wl.Aext_y if np.any(wl.Aext_x) else None
+    st = None
+    for _ in range(ns - 1):
+        st = o.sweep(wl.delta0, Ax, Ay, wl.n_energies, st)["stores"]
+    if st is None:
+        st = o.reset_stores(wl.delta0, Ax, Ay, z)
+    for k in (0, wl.n_angles // 2 - 1):
+        for n in (0, wl.n_energies - 1):
+            Go, GTo, _ = o.debug_trajectory(wl.delta0, Ax, Ay, k, o.ntraj_angle(k) // 2, z, n, st)
+            Gg, GTg = g.ctx.sc_debug_trajectory(k, o.ntraj_angle(k) // 2, n)
+            assert np.max(np.abs(Gg - Go)) < TOL32 and np.max(np.abs(GTg - GTo)) < TOL32
 
 
 def test_energy_sharded_sweep_equals_full_sweep(sc):
