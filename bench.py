@@ -198,10 +198,10 @@ def run_ours(a):
     torch.cuda.synchronize()
     sampler = ClockSampler(local); sampler.start()
     e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
-    march_ms = []
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
+    ctx.sc_debug_march_time()                       # reset: count only the march launches of the timed steps
     e0.record()
     for _ in range(a.steps):
         step()
@@ -211,16 +211,15 @@ def run_ours(a):
         dist.barrier()
     ms = e0.elapsed_time(e1)
     clocks = sampler.stop()
+    march_total_ms, march_launches = ctx.sc_debug_march_time()      # CUDA events around each march launch of the timed region
     if world > 1:                                   # device time of the slowest rank
         tmax = torch.tensor([ms], dtype=torch.float64, device=devname)
         dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
         ms = float(tmax.item())
 
-    # per-kernel duration of the dominant kernel (the march), CUDA events on the launching stream, same inputs
-    ctx.sc_set_fields(delta, dev_ax if wl.kappa <= 0 else None, dev_ay if wl.kappa <= 0 else None)
-    for _ in range(2):
-        st = ctx.sc_riccati_sweep(dn, jx, jy, fe, want_stats=True)
-        march_ms.append(ctx.last_march_ms())
+    # unit counts of one sweep (one extra sweep with stats, outside the timed region)
+    ctx.sc_set_fields(delta, dev_ax + aix, dev_ay + aiy)
+    st = ctx.sc_riccati_sweep(dn, jx, jy, fe, want_stats=True)
     units = st.n_updates / 4.0                    # this rank's (node, energy, angle-pair) units incl. the boundary pieces
     n_updates, n_exec = st.n_updates, st.n_updates_executed
     if world > 1:                                 # whole-job updates = sum over the energy shards
@@ -228,10 +227,10 @@ def run_ours(a):
         dist.all_reduce(tot)
         n_updates, n_exec = int(tot[0].item()), int(tot[1].item())
     peak_dfma, clk = ctx.sc_debug_fp64_peak()
-    mk_ms = float(np.mean(march_ms))
+    mk_ms = march_total_ms / max(march_launches, 1)
     achieved = 2.0 * ALGO_FP64_INSTR_PER_UNIT * units / (mk_ms * 1e-3) / 1e12
     peak = 2.0 * peak_dfma / 1e12
-    roofline = {"bound": "alu", "kernel": "sck::march_kernel<0,false>", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+    roofline = {"bound": "alu", "kernel": "sck::march_kernel<0,false,%d,%s>" % (a.stepper, "double" if a.precision == 64 else "float"), "launches_timed": march_launches, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                 "frac": achieved / peak, "traffic": None,
                 "note": "fp64 pipe: flops = 2 x FP64-pipe instructions; achieved = algorithmic count (DESIGN.md §6) x units / "
                         "march duration (CUDA events); peak = measured register-resident DFMA rate on this GPU",
@@ -275,6 +274,7 @@ def run_ours(a):
         if world > 1:
             dist.barrier()
         f0 = torch.cuda.Event(enable_timing=True); f1 = torch.cuda.Event(enable_timing=True)
+        c32.sc_debug_march_time()
         f0.record()
         for _ in range(a.steps):
             c32.sc_iterate(acc, 1.0, False, d32, ax32, ay32)
@@ -285,7 +285,7 @@ def run_ours(a):
             dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
             ms32 = float(tmax.item())
         fp32_leg = {"dtype": "f32", "value": n_updates * a.steps / (ms32 * 1e-3), "unit": UNIT, "ms_per_step": ms32 / a.steps,
-                    "march_ms": c32.last_march_ms(), "hbm_bytes_per_unit_algorithmic": 32.0}
+                    "march_ms": c32.sc_debug_march_time()[0] / a.steps, "hbm_bytes_per_unit_algorithmic": 32.0}
         c32.close()
 
     value = n_updates * a.steps / (ms * 1e-3)

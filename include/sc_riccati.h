@@ -156,6 +156,11 @@ sc_status sc_debug_fp64_peak(sc_ctx* ctx, double* dfma_per_s, double* sm_clock_m
 /* Device time of the most recent march kernel launch (CUDA events recorded on the stream around that launch
  * alone); synchronises.  Used by bench.py for the roofline of the dominant kernel. */
 sc_status sc_debug_last_march_ms(sc_ctx* ctx, float* ms);
+/* Sum of the device times of the march launches since the previous call of this function (at most the last 64),
+ * each bracketed by its own CUDA events on the stream, and their count; synchronises, then resets the count.
+ * bench.py calls it around the timed region: the roofline of the dominant kernel comes from the launches that
+ * the timed steps themselves made.  Either output may be NULL (reset only). */
+sc_status sc_debug_march_time(sc_ctx* ctx, float* total_ms, int* n_launches);
 
 const char* sc_last_error(const sc_ctx* ctx);
 const char* sc_version(void);

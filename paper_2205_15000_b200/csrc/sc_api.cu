@@ -5,6 +5,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <complex>
 #include <cstdio>
 #include <cstring>
 #include <numeric>
@@ -40,9 +41,49 @@ struct DevBuf {
 struct EnergySet {
     std::vector<double> zr, zi, w; std::vector<int> partner;
     DevBuf<double> d_zr, d_zi, d_w; DevBuf<int> d_partner;
+    std::vector<double> tc; DevBuf<double> d_tc;      // Taylor table of T (empty: not on the imaginary axis)
     int ne = 0;
-    sck::EnergyDev dev() const { return sck::EnergyDev{ne, d_zr.p, d_zi.p, d_w.p, d_partner.p}; }
+    sck::EnergyDev dev() const { return sck::EnergyDev{ne, d_zr.p, d_zi.p, d_w.p, d_partner.p, tc.empty() ? nullptr : d_tc.p}; }
 };
+
+// T(w) = tanh(h sqrt w)/sqrt w for complex w (even in sqrt w: no branch issue); series near w = 0
+std::complex<double> T_of_w(std::complex<double> w, double h) {
+    const std::complex<double> u = h * h * w;
+    if (std::abs(u) < 1e-4) return h * (1.0 - u / 3.0 + 2.0 * u * u / 15.0 - 17.0 * u * u * u / 315.0);
+    const std::complex<double> x = std::sqrt(w);
+    return std::tanh(h * x) / x;
+}
+
+// Table behind sc_math.cuh taylor_T for every energy i*zi on the imaginary axis: with the nearest pole of
+// T(w) = sum_k (2/h)/(w + (2k+1)^2 wp) removed, R(w) = T(w) - (2/h)/(w + wp) is analytic for |w - w0| < w0 + 9 wp,
+// w0 = zi^2; its Taylor coefficients r_k = R^(k)(w0)/k! come from the trapezoid rule on a circle of half that radius
+// (geometric convergence; R is real on the real axis, so the r_k are real).
+// Row = r_0..r_8, (w0 + 9 wp)^2, w0 + wp, 2/h.
+void taylor_table(EnergySet& E, double h) {
+    E.tc.clear();
+    for (double v : E.zr) if (v != 0.0) return;
+    const double PI = 3.14159265358979323846, wp = (PI / (2.0 * h)) * (PI / (2.0 * h));
+    const int M = 128;
+    E.tc.assign((size_t)E.zr.size() * sck::TC_LD, 0.0);
+    std::vector<std::complex<double>> f(M);
+    for (size_t n = 0; n < E.zi.size(); ++n) {
+        const double w0 = E.zi[n] * E.zi[n], rad = w0 + 9.0 * wp, rho = 0.5 * rad;
+        for (int j = 0; j < M; ++j) {
+            const std::complex<double> w = w0 + std::polar(rho, 2.0 * PI * j / M);
+            f[j] = T_of_w(w, h) - (2.0 / h) / (w + wp);
+        }
+        double rk = 1.0;
+        for (int k = 0; k <= 8; ++k) {
+            std::complex<double> acc = 0.0;
+            for (int j = 0; j < M; ++j) acc += f[j] * std::polar(1.0, -2.0 * PI * ((j * k) % M) / M);
+            E.tc[n * sck::TC_LD + k] = acc.real() / M / rk;
+            rk *= rho;
+        }
+        E.tc[n * sck::TC_LD + 9] = rad * rad;
+        E.tc[n * sck::TC_LD + 10] = w0 + wp;
+        E.tc[n * sck::TC_LD + 11] = 2.0 / h;
+    }
+}
 
 }  // namespace
 
@@ -80,7 +121,9 @@ struct sc_ctx {
     // scratch
     DevBuf<char> d_scr; long long scr_stride = 0; int n_slots = 0;       // scr_stride in bytes
     DevBuf<double> d_part; DevBuf<int> d_counter; DevBuf<int> d_nbad; DevBuf<double> d_statmax;
-    cudaEvent_t ev0 = nullptr, ev1 = nullptr, evm0 = nullptr, evm1 = nullptr;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    static constexpr int MEV = 64;                 // ring of event pairs around the march launches (sc_debug_march_time)
+    cudaEvent_t mev[MEV][2] = {}; int mev_n = 0;
     // Eq. 22 denominator sum (sum_n w_n t / eps_n over the WHOLE job's energy table) and the energy-shard hook
     double denom_sum = 0.0;
     double* hook_acc = nullptr; sc_allreduce_fn hook_fn = nullptr; void* hook_user = nullptr;
@@ -103,6 +146,8 @@ sck::TrajDev traj_dev(const sc_ctx* c) {
 
 sc_status upload_energies(sc_ctx* ctx, EnergySet& E) {
     E.ne = (int)E.zr.size();
+    taylor_table(E, ctx->grid.h);
+    CU(E.d_tc.upload(E.tc, ctx->stream));
     CU(E.d_zr.upload(E.zr, ctx->stream)); CU(E.d_zi.upload(E.zi, ctx->stream));
     CU(E.d_w.upload(E.w, ctx->stream)); CU(E.d_partner.upload(E.partner, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
@@ -153,15 +198,17 @@ sck::MarchArgsT<R> march_args(sc_ctx* ctx, const EnergySet& E, const char* store
 template <int MODE, bool STATS, int STEP, typename R>
 sc_status launch_march_t(sc_ctx* ctx, const sck::MarchArgsT<R>& A) {
     const int blocks = ctx->n_slots / sck::MARCH_WARPS;
-    const int smem = MODE == 0 ? sck::march_smem<R>() : 0;
+    const int smem = sck::march_smem<R>();
     static bool attr_set = false;
-    if (MODE == 0 && !attr_set) {
+    if (!attr_set) {
         CU(cudaFuncSetAttribute(sck::march_kernel<MODE, STATS, STEP, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         attr_set = true;
     }
-    CU(cudaEventRecord(ctx->evm0, ctx->stream));
+    cudaEvent_t* ev = ctx->mev[ctx->mev_n % sc_ctx::MEV];
+    CU(cudaEventRecord(ev[0], ctx->stream));
     sck::march_kernel<MODE, STATS, STEP, R><<<blocks, sck::MARCH_WARPS * 32, smem, ctx->stream>>>(A);
-    CU(cudaEventRecord(ctx->evm1, ctx->stream));
+    CU(cudaEventRecord(ev[1], ctx->stream));
+    ++ctx->mev_n;
     CU(cudaGetLastError());
     return SC_OK;
 }
@@ -316,7 +363,8 @@ sc_status sc_create(const sc_grid* grid, const unsigned char* mask, const sc_sha
     cudaDeviceProp prop; CU(cudaGetDeviceProperties(&prop, opts->device));
     ctx->n_sm = prop.multiProcessorCount;
     ctx->stream = (cudaStream_t)opts->cuda_stream;
-    CU(cudaEventCreate(&ctx->ev0)); CU(cudaEventCreate(&ctx->ev1)); CU(cudaEventCreate(&ctx->evm0)); CU(cudaEventCreate(&ctx->evm1));
+    CU(cudaEventCreate(&ctx->ev0)); CU(cudaEventCreate(&ctx->ev1));
+    for (auto& e : ctx->mev) { CU(cudaEventCreate(&e[0])); CU(cudaEventCreate(&e[1])); }
 
     // ---- upload ----
     cudaStream_t s = ctx->stream;
@@ -361,8 +409,7 @@ sc_status sc_destroy(sc_ctx* ctx) {
     if (!ctx) return SC_ERR_ARG;
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
-    if (ctx->evm0) cudaEventDestroy(ctx->evm0);
-    if (ctx->evm1) cudaEventDestroy(ctx->evm1);
+    for (auto& e : ctx->mev) { if (e[0]) cudaEventDestroy(e[0]); if (e[1]) cudaEventDestroy(e[1]); }
     scf::release(ctx->fs);
     delete ctx;
     return SC_OK;
@@ -637,8 +684,26 @@ sc_status sc_debug_math(sc_ctx* ctx, int n, double* max_rel_err) {
 
 sc_status sc_debug_last_march_ms(sc_ctx* ctx, float* ms) {
     if (!ctx || !ms) return SC_ERR_ARG;
-    CU(cudaEventSynchronize(ctx->evm1));
-    CU(cudaEventElapsedTime(ms, ctx->evm0, ctx->evm1));
+    if (ctx->mev_n == 0) return fail(ctx, SC_ERR_STATE, "no march kernel has been launched");
+    cudaEvent_t* ev = ctx->mev[(ctx->mev_n - 1) % sc_ctx::MEV];
+    CU(cudaEventSynchronize(ev[1]));
+    CU(cudaEventElapsedTime(ms, ev[0], ev[1]));
+    return SC_OK;
+}
+
+sc_status sc_debug_march_time(sc_ctx* ctx, float* total_ms, int* n_launches) {
+    if (!ctx) return SC_ERR_ARG;
+    const int n = std::min(ctx->mev_n, (int)sc_ctx::MEV);
+    float tot = 0.f;
+    for (int i = 0; i < n; ++i) {
+        cudaEvent_t* ev = ctx->mev[(ctx->mev_n - 1 - i) % sc_ctx::MEV];
+        CU(cudaEventSynchronize(ev[1]));
+        float ms = 0.f; CU(cudaEventElapsedTime(&ms, ev[0], ev[1]));
+        tot += ms;
+    }
+    if (total_ms) *total_ms = tot;
+    if (n_launches) *n_launches = n;
+    ctx->mev_n = 0;
     return SC_OK;
 }
 

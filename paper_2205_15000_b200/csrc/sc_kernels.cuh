@@ -44,7 +44,10 @@ struct TrajDev {                 // physical trajectories (angles k < N/2), stru
     const int* dF; const int* dB;   // store rows: (k,t) and its mirror (k+N/2, N_rot-1-t)
 };
 
-struct EnergyDev { int ne; const double* zr; const double* zi; const double* w; const int* partner; };
+// tc: per-energy table of the step coefficient T (sc_math.cuh taylor_T), [ne][TC_LD] = r_0..r_8, (w0 + 9 wp)^2,
+// w0 + wp, 2/h; null when the energy table is not on the imaginary axis (then every piece takes the exp-based evaluation)
+constexpr int TC_LD = 12;
+struct EnergyDev { int ne; const double* zr; const double* zi; const double* w; const int* partner; const double* tc; };
 
 // ------------------------------------------------------------------------------------------------
 // masked bilinear interpolation of Delta (R5) and plain bilinear of A at a point
@@ -188,7 +191,6 @@ constexpr int PF_DIST = 12;                  // pass 2: scratch lines are pulled
 constexpr int RED_NODES = 4;                 // nodes per shared-memory reduction batch
 constexpr int RED_VALS = 6;
 constexpr int STAGE_LD = 33;                 // padded row of the transpose stage: conflict-free rows AND columns
-template <typename R> constexpr int march_smem() { return MARCH_WARPS * RED_NODES * RED_VALS * STAGE_LD * (int)sizeof(R); }   // fp64: 50688 B (> 48 KB: opt-in)
 
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 // 256-bit global accesses (LDG.E.ENL2.256 / STG.E.ENL2.256 on sm_100a): one fp64 scratch entry per lane per instruction
@@ -300,16 +302,42 @@ __device__ __forceinline__ cplx_t<R> step_up(cplx_t<R> g, const typename VT<R>::
     return scm::step_mid(g, cc.x, cc.y, zr0 + cc.z, zi0, cc.w);
 }
 
+// ---- coefficient staging: the warp-uniform piece / node records of a trajectory are streamed through shared
+// memory in chunks of 32 (one record per lane, coalesced cp.async, double-buffered one chunk ahead), so that no
+// step ever waits on a global load of its coefficients; the step loop reads them with broadcast LDS.
+constexpr int CHUNK = 32;
+template <typename R> __host__ __device__ constexpr int march_stage_bytes() { return RED_NODES * RED_VALS * STAGE_LD * (int)sizeof(R); }   // per warp
+template <typename R> __host__ __device__ constexpr int march_coef_bytes() { return 2 * CHUNK * 6 * (int)sizeof(R); }                      // per warp: pc[2][32] V4 + nd[2][32] V2
+template <typename R> __host__ __device__ constexpr int march_smem() { return MARCH_WARPS * (march_stage_bytes<R>() + march_coef_bytes<R>()); }   // fp64: 75264 B (opt-in)
+
+template <int BYTES>
+__device__ __forceinline__ void cp_async(void* smem, const void* gmem) {
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+    if (BYTES == 32) {
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gmem) : "memory");
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa + 16), "l"((const char*)gmem + 16) : "memory");
+    } else if (BYTES == 16) {
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gmem) : "memory");
+    } else {
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sa), "l"(gmem) : "memory");
+    }
+}
+__device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
 // MODE 0: Matsubara sums; 1: per-energy Re g (LDOS); 2: boundary values only.
 // STEP 0: closed-form step; 1: implicit mid-point rule (C4-C9 :984-1001).
 template <int MODE, bool STATS, int STEP, typename R>
 __global__ void __launch_bounds__(MARCH_WARPS * 32, MARCH_MIN_CTAS) march_kernel(MarchArgsT<R> A) {
     using V2 = typename VT<R>::V2; using V4 = typename VT<R>::V4;
-    extern __shared__ double stage_raw[];        // MODE 0: MARCH_WARPS x (24 rows x STAGE_LD) values of R
+    extern __shared__ double4 smem_raw[];
     constexpr int ROW = ScrT<R, STEP>::ROW, BYTES = ScrT<R, STEP>::BYTES;
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const int slot = blockIdx.x * MARCH_WARPS + wib;
-    R* const stage = reinterpret_cast<R*>(stage_raw) + wib * (RED_NODES * RED_VALS * STAGE_LD);
+    char* const smem_w = reinterpret_cast<char*>(smem_raw) + wib * (march_stage_bytes<R>() + march_coef_bytes<R>());
+    R* const stage = reinterpret_cast<R*>(smem_w);                                        // [4 nodes][6 values][33]
+    V4* const pcb = reinterpret_cast<V4*>(smem_w + march_stage_bytes<R>());               // [2][CHUNK] piece records
+    V2* const ndb = reinterpret_cast<V2*>(pcb + 2 * CHUNK);                               // [2][CHUNK] node Delta
     char* const scr = A.scr + (size_t)slot * A.scr_stride + lane * BYTES;   // entry e of this lane: scr + e*ROW
     const int ne = A.E.ne;
     R max2 = R(0);
@@ -325,6 +353,8 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32, MARCH_MIN_CTAS) march_kernel
         const int dF = A.T.dF[g], dB = A.T.dB[g];
         const V2* __restrict__ ND = A.nd_D + noff;
         const V4* __restrict__ PC = A.pc + noff + g;
+        double* __restrict__ const PART = A.part + (size_t)noff * RED_VALS;
+        const int npart = nn * RED_VALS;
 
         for (int n0 = 0; n0 < ne; n0 += 32) {
             const bool act = n0 + lane < ne;
@@ -332,11 +362,25 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32, MARCH_MIN_CTAS) march_kernel
             const R zr0 = (R)A.E.zr[n], zi0 = (R)A.E.zi[n];
             const R wn = act ? (R)A.E.w[n] : R(0);
             const int nb = A.E.partner[n];
+            // Taylor table of T about this lane's energy (interior pieces all have length h)
+            constexpr int KT = scm::TaylorK<R>::K;
+            const bool tay = STEP == 0 && A.E.tc != nullptr;
+            R tcf[KT + 1]; R thr2 = R(-1), pole_a = R(1), pole_res = R(0);
+            if (tay) {
+#pragma unroll
+                for (int k = 0; k <= KT; ++k) tcf[k] = (R)A.E.tc[(size_t)n * TC_LD + k];
+                thr2 = (R)(A.E.tc[(size_t)n * TC_LD + 9] * scm::TaylorK<R>::RMAX2);
+                pole_a = (R)A.E.tc[(size_t)n * TC_LD + 10]; pole_res = (R)A.E.tc[(size_t)n * TC_LD + 11];
+            }
+            const R m2zi = R(-2) * zi0;
 
             // ---------------- pass 1: gamma-tilde from u_out down to u_in; entry p = {T_p, gamma~(node p-1)} ----------
-            V4 c4 = ldu(PC + nn);
+            const int ctop = nn >> 5;                                  // chunk c holds pieces 32c .. 32c+31
+            if (ctop * CHUNK + lane <= nn) cp_async<sizeof(V4)>(pcb + (ctop & 1) * CHUNK + lane, PC + ctop * CHUNK + lane);
+            cp_commit();
             cplx_t<R> gt;
             if (A.bc_mode == 1) {
+                const V4 c4 = ldu(PC + nn);
                 gt = hom_start<R>(-(double)c4.x, c4.y, A.E.zr[n] + c4.z, A.E.zi[n]);
             } else if (A.ga_n[dB]) {
                 const cplx_t<R> s = gather_start(A, dB, nb);            // gamma of the mirrored trajectory at its entry
@@ -347,30 +391,55 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32, MARCH_MIN_CTAS) march_kernel
             }
             {
                 char* e = scr + (size_t)nn * ROW;
-                V4 cn = ldu(PC + (nn >= 1 ? nn - 1 : 0));
-#pragma unroll 2
-                for (int p = nn; p >= 0; --p) {
-                    const V4 cc = c4;
-                    c4 = cn;
-                    if (p >= 2) cn = ldu(PC + p - 2);                          // coefficient record two pieces ahead
-                    const R zr = zr0 + cc.z;
-                    cplx_t<R> T = mk(R(0), R(0));
-                    if (STEP == 0) {
-                        T = scm::coef_T(scm::mad(cc.x, cc.x, cc.y * cc.y), zr, zi0, cc.w);
-                        gt = scm::step_T(gt, -cc.x, cc.y, zr, zi0, T);
+                int p = nn;
+                for (int c = ctop; c >= 0; --c) {
+                    if (c > 0) {
+                        cp_async<sizeof(V4)>(pcb + ((c - 1) & 1) * CHUNK + lane, PC + (c - 1) * CHUNK + lane);
+                        cp_commit();
+                        cp_wait<1>();
                     } else {
-                        gt = scm::step_mid(gt, -cc.x, cc.y, zr, zi0, cc.w);
+                        cp_wait<0>();
                     }
-                    st_ent<STEP>(e, T, gt);
-                    e -= ROW;
+                    __syncwarp();
+                    const V4* __restrict__ buf = pcb + (c & 1) * CHUNK;
+                    const int plo = c * CHUNK;
+#pragma unroll 2
+                    for (; p >= plo; --p) {
+                        const V4 cc = buf[p & (CHUNK - 1)];
+                        const R zr = zr0 + cc.z;
+                        cplx_t<R> T = mk(R(0), R(0));
+                        if (STEP == 0) {
+                            const R d2 = scm::mad(cc.x, cc.x, cc.y * cc.y);
+                            // w = |De|^2 - z^2 = zi0^2 + dw,  dw = (|De|^2 - a^2) - 2 i zi0 a   (z = i zi0 + a)
+                            const R dwr = scm::mad(-cc.z, cc.z, d2), dwi = m2zi * cc.z;
+                            const R s2 = scm::mad(dwr, dwr, dwi * dwi);
+                            const bool interior = p > 0 && p < nn;
+                            if (interior && !__any_sync(0xffffffffu, !(s2 <= thr2))) T = scm::taylor_T<R, KT>(tcf, pole_a, pole_res, dwr, dwi, s2);
+                            else T = scm::coef_T_slow(d2, zr, zi0, cc.w);
+                            gt = scm::step_T(gt, -cc.x, cc.y, zr, zi0, T);
+                        } else {
+                            gt = scm::step_mid(gt, -cc.x, cc.y, zr, zi0, cc.w);
+                        }
+                        st_ent<STEP>(e, T, gt);
+                        e -= ROW;
+                    }
+                    __syncwarp();                                       // chunk c is free for the load issued next round
                 }
                 if (act) A.store_new[(size_t)dB * ne + nb] = mk2(gt.re, -gt.im);
             }
 
             // ---------------- pass 2: gamma from u_in up to u_out; products and energy reduction ------------
+            // chunk c of pass 2 holds, for nodes m = 32c .. 32c+31, the piece m+1 (the step that leaves the node) and Delta_m
+            const int nchunk = (nn + CHUNK - 1) >> 5;
             cplx_t<R> gm;
             {
-                const V4 c0 = ldu(PC);
+                const V4 c0 = pcb[0];                                   // piece 0 is still in buffer 0 (last chunk of pass 1)
+                __syncwarp();
+                if (lane < nn) {
+                    cp_async<sizeof(V4)>(pcb + CHUNK + lane, PC + 1 + lane);      // pass-2 chunk 0 goes to buffer 1
+                    cp_async<sizeof(V2)>(ndb + CHUNK + lane, ND + lane);
+                }
+                cp_commit();
                 if (A.bc_mode == 1) gm = hom_start<R>(c0.x, c0.y, A.E.zr[n] + c0.z, A.E.zi[n]);
                 else if (A.ga_n[dF]) gm = gather_start(A, dF, n);
                 else gm = hom_start<R>(A.fb_D[dF].x, A.fb_D[dF].y, A.E.zr[n] + A.fb_a[dF], A.E.zi[n]);
@@ -380,60 +449,78 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32, MARCH_MIN_CTAS) march_kernel
             const char* e = scr + ROW;                  // entry of node 0
             for (int q = 4; q < PF_DIST && q < nn; q += 4) prefetch_l2(e - lane * BYTES + (size_t)q * ROW + lane * 128);
             Ent<R> En = ld_ent<STEP>(e, R(0));
-            V4 cN = ldu(PC + 1);
-            V2 dN = ND[0];
+            double part_nxt = 0.0;                       // running sums of the earlier energy rounds, fetched one batch ahead
+            if (MODE == 0 && n0 && lane < RED_NODES * RED_VALS && lane < npart) part_nxt = PART[lane];
             int m = 0;
-            for (; m + RED_NODES <= nn; m += RED_NODES) {
-                if (m + PF_DIST < nn) prefetch_l2(e - lane * BYTES + (size_t)PF_DIST * ROW + lane * 128);
-                double part_old = 0.0;
-                if (MODE == 0 && n0 && lane < RED_NODES * RED_VALS) part_old = A.part[(size_t)(noff + m) * RED_VALS + lane];
+            for (int c = 0; c < nchunk; ++c) {
+                const int bsel = (c + 1) & 1;                           // chunk c lives in buffer (c+1)&1
+                if (c + 1 < nchunk) {
+                    const int q = (c + 1) * CHUNK + lane;
+                    if (q < nn) {
+                        cp_async<sizeof(V4)>(pcb + (bsel ^ 1) * CHUNK + lane, PC + 1 + q);
+                        cp_async<sizeof(V2)>(ndb + (bsel ^ 1) * CHUNK + lane, ND + q);
+                    }
+                    cp_commit();
+                    cp_wait<1>();
+                } else {
+                    cp_wait<0>();
+                }
+                __syncwarp();
+                const V4* __restrict__ pbuf = pcb + bsel * CHUNK;
+                const V2* __restrict__ dbuf = ndb + bsel * CHUNK;
+                const int mhi = min(nn, (c + 1) * CHUNK);
+                for (; m + RED_NODES <= mhi; m += RED_NODES) {
+                    if (m + PF_DIST < nn) prefetch_l2(e - lane * BYTES + (size_t)PF_DIST * ROW + lane * 128);
+                    const double part_old = part_nxt;
+                    if (MODE == 0 && n0 && lane < RED_NODES * RED_VALS && (m + RED_NODES) * RED_VALS + lane < npart)
+                        part_nxt = PART[(m + RED_NODES) * RED_VALS + lane];
 #pragma unroll
-                for (int b = 0; b < RED_NODES; ++b) {
-                    const Ent<R> Ec = En; const V4 cc = cN; const V2 dc = dN;
-                    En = ld_ent<STEP>(e + (b + 1) * ROW, R(0));          // one node ahead (scratch has 2 spare entries)
-                    cN = ldu(PC + m + b + 2 <= PC + nn ? PC + m + b + 2 : PC + nn);
-                    dN = ND[m + b + 1 < nn ? m + b + 1 : nn - 1];
-                    if (MODE != 2) {
-                        const R rg = node_products<MODE, STATS, R>(gm, Ec.gr, Ec.gi, dc, wn, stage + b * RED_VALS * STAGE_LD + lane, max2);
-                        if (MODE == 1 && act) A.ldos[(size_t)(noff + m + b) * ne + n] = (double)rg;
+                    for (int b = 0; b < RED_NODES; ++b) {
+                        const Ent<R> Ec = En;
+                        const V4 cc = pbuf[(m + b) & (CHUNK - 1)]; const V2 dc = dbuf[(m + b) & (CHUNK - 1)];
+                        En = ld_ent<STEP>(e + (b + 1) * ROW, R(0));          // one node ahead (scratch has 2 spare entries)
+                        if (MODE != 2) {
+                            const R rg = node_products<MODE, STATS, R>(gm, Ec.gr, Ec.gi, dc, wn, stage + b * RED_VALS * STAGE_LD + lane, max2);
+                            if (MODE == 1 && act) A.ldos[(size_t)(noff + m + b) * ne + n] = (double)rg;
+                        }
+                        gm = step_up<STEP, R>(gm, cc, zr0, zi0, Ec);
                     }
-                    gm = step_up<STEP, R>(gm, cc, zr0, zi0, Ec);
-                }
-                e += RED_NODES * ROW;
-                if (MODE == 0) {
-                    __syncwarp();
-                    if (lane < RED_NODES * RED_VALS) {
-                        double s = stage_colsum(stage, lane);
-                        if (n0) s += part_old;
-                        A.part[(size_t)(noff + m) * RED_VALS + lane] = s;
+                    e += RED_NODES * ROW;
+                    if (MODE == 0) {
+                        __syncwarp();
+                        if (lane < RED_NODES * RED_VALS) {
+                            double s = stage_colsum(stage, lane);
+                            if (n0) s += part_old;
+                            PART[m * RED_VALS + lane] = s;
+                        }
+                        __syncwarp();
                     }
-                    __syncwarp();
                 }
-            }
-            if (m < nn) {                                        // ragged tail: 1..3 nodes
-                const int rem = nn - m;
-                double part_old = 0.0;
-                if (MODE == 0 && n0 && lane < rem * RED_VALS) part_old = A.part[(size_t)(noff + m) * RED_VALS + lane];
-                for (int b = 0; b < rem; ++b) {
-                    const Ent<R> Ec = En; const V4 cc = cN; const V2 dc = dN;
-                    En = ld_ent<STEP>(e + (b + 1) * ROW, R(0));
-                    cN = ldu(PC + m + b + 2 <= PC + nn ? PC + m + b + 2 : PC + nn);
-                    dN = ND[m + b + 1 < nn ? m + b + 1 : nn - 1];
-                    if (MODE != 2) {
-                        const R rg = node_products<MODE, STATS, R>(gm, Ec.gr, Ec.gi, dc, wn, stage + b * RED_VALS * STAGE_LD + lane, max2);
-                        if (MODE == 1 && act) A.ldos[(size_t)(noff + m + b) * ne + n] = (double)rg;
+                if (m < mhi) {                                       // ragged tail: 1..3 nodes (last chunk only)
+                    const int rem = mhi - m;
+                    const double part_old = part_nxt;
+                    for (int b = 0; b < rem; ++b) {
+                        const Ent<R> Ec = En;
+                        const V4 cc = pbuf[(m + b) & (CHUNK - 1)]; const V2 dc = dbuf[(m + b) & (CHUNK - 1)];
+                        En = ld_ent<STEP>(e + (b + 1) * ROW, R(0));
+                        if (MODE != 2) {
+                            const R rg = node_products<MODE, STATS, R>(gm, Ec.gr, Ec.gi, dc, wn, stage + b * RED_VALS * STAGE_LD + lane, max2);
+                            if (MODE == 1 && act) A.ldos[(size_t)(noff + m + b) * ne + n] = (double)rg;
+                        }
+                        gm = step_up<STEP, R>(gm, cc, zr0, zi0, Ec);
                     }
-                    gm = step_up<STEP, R>(gm, cc, zr0, zi0, Ec);
-                }
-                if (MODE == 0) {
-                    __syncwarp();
-                    if (lane < rem * RED_VALS) {
-                        double s = stage_colsum(stage, lane);
-                        if (n0) s += part_old;
-                        A.part[(size_t)(noff + m) * RED_VALS + lane] = s;
+                    if (MODE == 0) {
+                        __syncwarp();
+                        if (lane < rem * RED_VALS) {
+                            double s = stage_colsum(stage, lane);
+                            if (n0) s += part_old;
+                            PART[m * RED_VALS + lane] = s;
+                        }
+                        __syncwarp();
                     }
-                    __syncwarp();
+                    m = mhi;
                 }
+                __syncwarp();                                           // this chunk's buffer is free for the next load
             }
             if (act) A.store_new[(size_t)dF * ne + n] = mk2(gm.re, gm.im);
         }
@@ -611,10 +698,25 @@ __global__ void debug_traj_kernel(MarchArgsT<R> A, int stepper, int g, int n, do
     if (A.bc_mode == 1) gt = hom_start<R>(-(double)PC[nn].x, PC[nn].y, A.E.zr[n] + PC[nn].z, A.E.zi[n]);
     else if (A.ga_n[dB]) { cplx_t<R> s = gather_start(A, dB, nb); gt = mk(s.re, -s.im); }
     else { cplx_t<R> s = hom_start<R>(A.fb_D[dB].x, A.fb_D[dB].y, A.E.zr[nb] + A.fb_a[dB], A.E.zi[nb]); gt = mk(s.re, -s.im); }
+    // the same evaluation of T as the march: Taylor table for interior pieces inside its radius, exp-based otherwise
+    constexpr int KT = scm::TaylorK<R>::K;
+    R tcf[KT + 1]; R thr2 = R(-1), pole_a = R(1), pole_res = R(0);
+    if (A.E.tc) {
+        for (int k = 0; k <= KT; ++k) tcf[k] = (R)A.E.tc[(size_t)n * TC_LD + k];
+        thr2 = (R)(A.E.tc[(size_t)n * TC_LD + 9] * scm::TaylorK<R>::RMAX2);
+        pole_a = (R)A.E.tc[(size_t)n * TC_LD + 10]; pole_res = (R)A.E.tc[(size_t)n * TC_LD + 11];
+    }
+    auto coefT = [&](const V4& c, int p) {
+        const R d2 = scm::mad(c.x, c.x, c.y * c.y);
+        const R dwr = scm::mad(-c.z, c.z, d2), dwi = R(-2) * zi0 * c.z;
+        const R s2 = scm::mad(dwr, dwr, dwi * dwi);
+        if (p > 0 && p < nn && s2 <= thr2) return scm::taylor_T<R, KT>(tcf, pole_a, pole_res, dwr, dwi, s2);
+        return scm::coef_T(d2, zr0 + c.z, zi0, c.w);
+    };
     for (int p = nn; p >= 1; --p) {
         const V4 c = PC[p];
         if (stepper == 1) gt = scm::step_mid(gt, -c.x, c.y, zr0 + c.z, zi0, c.w);
-        else { const cplx_t<R> T = scm::coef_T(scm::mad(c.x, c.x, c.y * c.y), zr0 + c.z, zi0, c.w); gt = scm::step_T(gt, -c.x, c.y, zr0 + c.z, zi0, T); }
+        else { const cplx_t<R> T = coefT(c, p); gt = scm::step_T(gt, -c.x, c.y, zr0 + c.z, zi0, T); }
         outGT[p - 1] = make_double2(gt.re, gt.im);
     }
     cplx_t<R> gm;
@@ -624,7 +726,7 @@ __global__ void debug_traj_kernel(MarchArgsT<R> A, int stepper, int g, int n, do
     for (int p = 0; p < nn; ++p) {
         const V4 c = PC[p];
         if (stepper == 1) gm = scm::step_mid(gm, c.x, c.y, zr0 + c.z, zi0, c.w);
-        else { const cplx_t<R> T = scm::coef_T(scm::mad(c.x, c.x, c.y * c.y), zr0 + c.z, zi0, c.w); gm = scm::step_T(gm, c.x, c.y, zr0 + c.z, zi0, T); }
+        else { const cplx_t<R> T = coefT(c, p); gm = scm::step_T(gm, c.x, c.y, zr0 + c.z, zi0, T); }
         outG[p] = make_double2(gm.re, gm.im);
     }
 }

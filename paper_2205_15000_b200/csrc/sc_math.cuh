@@ -177,6 +177,39 @@ __device__ __forceinline__ cplx_t<R> coef_T(R d2, R zr, R zi, R len) {
     return mk(mad(tr, ir, -ti * ii), mad(tr, ii, ti * ir));
 }
 
+// Out-of-line copy of the exp-based evaluation: the march's hot loop evaluates T by taylor_T below and only calls
+// this for the two end pieces of a trajectory and for pieces outside the table's radius.
+template <typename R>
+__device__ __noinline__ cplx_t<R> coef_T_slow(R d2, R zr, R zi, R len) { return coef_T(d2, zr, zi, len); }
+
+// T as a function of w = Omega^2 is meromorphic: T(w) = tanh(l sqrt w)/sqrt w = sum_k (2/l)/(w + (2k+1)^2 wp),
+// wp = (pi/2l)^2.  For an energy i*zi on the imaginary axis and a piece of the common length l = h,
+// w = zi^2 + dw with dw = |De|^2 - a^2 - 2 i zi a.  The nearest pole is taken out in closed form and the rest,
+// R(w) = T(w) - (2/h)/(w + wp), is expanded about w0 = zi^2: its radius of convergence is w0 + 9 wp (the second
+// pole), against which dw is small for any |a| up to a few units:
+//     T = (2/h)/(w0 + wp + dw) + sum_k r_k(zi) dw^k,   r_k REAL (R is real on the real axis),
+// the r_k tabulated per energy by the host (sc_api.cu taylor_table).  A real-coefficient polynomial at a complex
+// point costs 2 FMAs per term: divide by the real quadratic (x - dw)(x - conj dw) = x^2 - r x + s; the remainder
+// b1 x + (b0 - r b1) at x = dw is (b0 - b1 Re dw) + i b1 Im dw.
+template <typename R> struct TaylorK;
+template <> struct TaylorK<double> { static constexpr int K = 8; static constexpr double RMAX2 = 0.012 * 0.012; };   // 0.012^9 = 5e-18
+template <> struct TaylorK<float> { static constexpr int K = 4; static constexpr double RMAX2 = 0.03 * 0.03; };      // 0.03^5  = 2e-8
+template <typename R, int K>
+__device__ __forceinline__ cplx_t<R> taylor_T(const R (&c)[K + 1], R pole_a, R pole_res, R dwr, R dwi, R s) {
+    const R r = dwr + dwr;
+    R b2 = c[K];
+    R b1 = mad(r, b2, c[K - 1]);
+#pragma unroll
+    for (int k = K - 2; k >= 0; --k) {
+        const R b0 = mad(r, b1, mad(-s, b2, c[k]));
+        b2 = b1; b1 = b0;
+    }
+    // here b1 holds b_0 and b2 holds b_1;  pole term: res / (A + dw) = res conj(A + dw) / |A + dw|^2
+    const R pr = pole_a + dwr;
+    const R q = pole_res * rcp_nr(mad(pr, pr, dwi * dwi));
+    return mk(mad(pr, q, mad(-b2, dwr, b1)), mad(-dwi, q, b2 * dwi));
+}
+
 // One closed-form step given T: 27 arithmetic instructions + 1 MUFU.
 template <typename R>
 __device__ __forceinline__ cplx_t<R> step_T(cplx_t<R> g, R Dr, R Di, R zr, R zi, cplx_t<R> T) {
