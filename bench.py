@@ -35,8 +35,16 @@ import workloads  # noqa: E402
 METRIC = "riccati_trajectory_step_updates_per_s"
 UNIT = "updates/s"
 # FP64-pipe instructions the closed-form path needs per (node, energy, angle pair) = 4 logical updates
-# (gamma and gamma-tilde for angles k and k+N/2): DESIGN.md §6 tally.
-ALGO_FP64_INSTR_PER_UNIT = 184.0
+# (gamma and gamma-tilde for angles k and k+N/2): DESIGN.md §6 tally of the kernel's own algorithm (step coefficient
+# T from the per-energy table 36, two Moebius steps 54, node products 28, energy reduction 8); ncu counts 126.1
+# executed.  Evaluating T from its definition (sqrt, exp, sin/cos) instead would be 184 — reported as context only.
+ALGO_FP64_INSTR_PER_UNIT = 126.0
+TEXTBOOK_FP64_INSTR_PER_UNIT = 184.0
+ALGO_FP64_INSTR_PER_UNIT_MIDPOINT = 2 * 66.0 + 28.0 + 8.0
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE march launch at configs[4], fp64, closed-form stepper, from the
+# `ncu --set full` capture summarised in profiles/r1_march_fp64_cfg4_ncu_full.md (4.922 TB read + 4.421 TB written)
+NCU_TRAFFIC_BYTES = {(4, 64, 0): 9.343071e12}
+NCU_PIPE_FP64_ACTIVE_PCT = {(4, 64, 0): 68.0}
 
 
 class ClockSampler(threading.Thread):
@@ -228,13 +236,25 @@ def run_ours(a):
         n_updates, n_exec = int(tot[0].item()), int(tot[1].item())
     peak_dfma, clk = ctx.sc_debug_fp64_peak()
     mk_ms = march_total_ms / max(march_launches, 1)
-    achieved = 2.0 * ALGO_FP64_INSTR_PER_UNIT * units / (mk_ms * 1e-3) / 1e12
+    full_size = world == 1 and not (a.pts_per_xi or a.n_angles or a.n_energies or a.size_scale != 1.0)
+    algo = ALGO_FP64_INSTR_PER_UNIT if a.stepper == 0 else ALGO_FP64_INSTR_PER_UNIT_MIDPOINT
+    achieved = 2.0 * algo * units / (mk_ms * 1e-3) / 1e12
     peak = 2.0 * peak_dfma / 1e12
+    peak_sustained = 2.0 * ctx.sc_debug_fp64_peak_sustained(2.0) / 1e12
     roofline = {"bound": "alu", "kernel": "sck::march_kernel<0,false,%d,%s>" % (a.stepper, "double" if a.precision == 64 else "float"), "launches_timed": march_launches, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                "frac": achieved / peak, "traffic": None,
+                "frac": achieved / peak,
+                "traffic": NCU_TRAFFIC_BYTES.get((wl.cfg, a.precision, a.stepper)) if full_size else None,
+                "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/)",
+                "algorithmic_bytes_per_launch": 64.0 * units,
+                "ncu_pipe_fp64_cycles_active_pct": NCU_PIPE_FP64_ACTIVE_PCT.get((wl.cfg, a.precision, a.stepper)) if full_size else None,
                 "note": "fp64 pipe: flops = 2 x FP64-pipe instructions; achieved = algorithmic count (DESIGN.md §6) x units / "
-                        "march duration (CUDA events); peak = measured register-resident DFMA rate on this GPU",
-                "march_ms": mk_ms, "march_share_of_step": mk_ms / (ms / a.steps), "algo_fp64_instr_per_unit": ALGO_FP64_INSTR_PER_UNIT,
+                        "march duration (CUDA events around the march launches of the timed steps); peak = register-resident "
+                        "DFMA rate measured in this process, best of 3 short runs (burst clock); peak_sustained = the same "
+                        "loop held for 2 s (power-limited clock, what a 1.8 s march launch can draw on)",
+                "peak_sustained": peak_sustained, "frac_of_sustained": achieved / peak_sustained,
+                "textbook_count_context": {"fp64_instr_per_unit": TEXTBOOK_FP64_INSTR_PER_UNIT,
+                                           "tflops": 2.0 * TEXTBOOK_FP64_INSTR_PER_UNIT * units / (mk_ms * 1e-3) / 1e12},
+                "march_ms": mk_ms, "march_share_of_step": mk_ms / (ms / a.steps), "algo_fp64_instr_per_unit": algo,
                 "units_per_launch": units, "hbm_bytes_per_unit_algorithmic": 64.0,
                 "hbm_gbs_algorithmic": 64.0 * units / (mk_ms * 1e-3) / 1e9}
 

@@ -152,6 +152,9 @@ sc_status sc_debug_math(sc_ctx* ctx, int n, double* max_rel_err);
 /* Register-resident DFMA microbenchmark: measured fp64 FMA instructions per second of the device (the
  * roofline denominator of the march kernel). */
 sc_status sc_debug_fp64_peak(sc_ctx* ctx, double* dfma_per_s, double* sm_clock_mhz);
+/* The same microbenchmark launched back to back for `seconds` (<= 30), rate of the second half: what the FP64 pipe
+ * sustains once the part sits at its power limit (the march runs for seconds at a time). */
+sc_status sc_debug_fp64_peak_sustained(sc_ctx* ctx, double seconds, double* dfma_per_s);
 
 /* Device time of the most recent march kernel launch (CUDA events recorded on the stream around that launch
  * alone); synchronises.  Used by bench.py for the roofline of the dominant kernel. */

@@ -107,6 +107,7 @@ def load_library():
     L.sc_debug_math.argtypes = [vp, i, vp]
     L.sc_debug_fp64_peak.argtypes = [vp, C.POINTER(d), C.POINTER(d)]
     L.sc_debug_last_march_ms.argtypes = [vp, C.POINTER(C.c_float)]
+    L.sc_debug_fp64_peak_sustained.argtypes = [vp, d, C.POINTER(d)]
     L.sc_debug_march_time.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(i)]
     _lib = L
     return L
@@ -293,6 +294,11 @@ class ScContext:
         ms, n = C.c_float(), C.c_int()
         self._check(self._L.sc_debug_march_time(self._h, C.byref(ms), C.byref(n)))
         return ms.value, n.value
+
+    def sc_debug_fp64_peak_sustained(self, seconds=2.0):
+        a = C.c_double()
+        self._check(self._L.sc_debug_fp64_peak_sustained(self._h, float(seconds), C.byref(a)))
+        return a.value
 
     def sc_debug_fp64_peak(self):
         a, b = C.c_double(), C.c_double()

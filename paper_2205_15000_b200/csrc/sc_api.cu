@@ -726,4 +726,26 @@ sc_status sc_debug_fp64_peak(sc_ctx* ctx, double* dfma_per_s, double* sm_clock_m
     return SC_OK;
 }
 
+sc_status sc_debug_fp64_peak_sustained(sc_ctx* ctx, double seconds, double* dfma_per_s) {
+    if (!ctx || !dfma_per_s || !(seconds > 0) || seconds > 30) return fail(ctx, SC_ERR_ARG, "bad argument");
+    DevBuf<double> d; CU(d.alloc(1));
+    const int iters = 20000, blocks = ctx->n_sm * 4, threads = 256;
+    // back-to-back launches for `seconds`: the rate the part holds once it sits at its power limit
+    sck::fp64_peak_kernel<<<blocks, threads, 0, ctx->stream>>>(iters, d.p);
+    CU(cudaEventRecord(ctx->ev0, ctx->stream));
+    sck::fp64_peak_kernel<<<blocks, threads, 0, ctx->stream>>>(iters, d.p);
+    CU(cudaEventRecord(ctx->ev1, ctx->stream));
+    CU(cudaEventSynchronize(ctx->ev1));
+    float one = 0; CU(cudaEventElapsedTime(&one, ctx->ev0, ctx->ev1));
+    const int n = std::max(4, (int)(seconds * 1e3 / std::max(one, 1e-3f)));
+    for (int i = 0; i < n / 2; ++i) sck::fp64_peak_kernel<<<blocks, threads, 0, ctx->stream>>>(iters, d.p);   // reach the steady clock
+    CU(cudaEventRecord(ctx->ev0, ctx->stream));
+    for (int i = 0; i < n - n / 2; ++i) sck::fp64_peak_kernel<<<blocks, threads, 0, ctx->stream>>>(iters, d.p);
+    CU(cudaEventRecord(ctx->ev1, ctx->stream));
+    CU(cudaEventSynchronize(ctx->ev1));
+    float ms = 0; CU(cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1));
+    *dfma_per_s = (double)(n - n / 2) * blocks * threads * (double)iters * 64.0 / (ms * 1e-3);
+    return SC_OK;
+}
+
 }  // extern "C"

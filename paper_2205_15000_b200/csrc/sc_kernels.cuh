@@ -188,11 +188,16 @@ constexpr int MARCH_WARPS = 8;               // warps per CTA
 #endif
 constexpr int MARCH_MIN_CTAS = SC_MARCH_MIN_CTAS;   // resident CTAs per SM the fp64 register budget is sized for
 constexpr int PF_DIST = 12;                  // pass 2: scratch lines are pulled into L2 this many nodes ahead
+#ifndef SC_PF1_DIST
+#define SC_PF1_DIST 0
+#endif
+constexpr int PF1_DIST = SC_PF1_DIST;        // ... and into L1 this many nodes ahead (0: off); the register look-ahead is one node
 constexpr int RED_NODES = 4;                 // nodes per shared-memory reduction batch
 constexpr int RED_VALS = 6;
 constexpr int STAGE_LD = 33;                 // padded row of the transpose stage: conflict-free rows AND columns
 
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 // 256-bit global accesses (LDG.E.ENL2.256 / STG.E.ENL2.256 on sm_100a): one fp64 scratch entry per lane per instruction
 __device__ __forceinline__ double4 ld256(const double4* p) {
     double4 v;
@@ -471,6 +476,7 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32, MARCH_MIN_CTAS) march_kernel
                 const int mhi = min(nn, (c + 1) * CHUNK);
                 for (; m + RED_NODES <= mhi; m += RED_NODES) {
                     if (m + PF_DIST < nn) prefetch_l2(e - lane * BYTES + (size_t)PF_DIST * ROW + lane * 128);
+                    if (PF1_DIST && m + PF1_DIST < nn) prefetch_l1(e - lane * BYTES + (size_t)PF1_DIST * ROW + lane * 128);
                     const double part_old = part_nxt;
                     if (MODE == 0 && n0 && lane < RED_NODES * RED_VALS && (m + RED_NODES) * RED_VALS + lane < npart)
                         part_nxt = PART[(m + RED_NODES) * RED_VALS + lane];

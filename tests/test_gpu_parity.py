@@ -170,6 +170,35 @@ def test_fp32_mode_parity(sc, cfg, kw, ns, stepper):
             assert np.max(np.abs(Gg - Go)) < TOL32 and np.max(np.abs(GTg - GTo)) < TOL32
 
 
+@pytest.mark.parametrize("amp", [0.3, 2.0, 12.0])
+def test_step_coefficient_table_and_fallback(sc, amp):
+    """The march evaluates T = tanh(Omega l)/Omega from a per-energy table where |De|^2 - a^2 - 2 i eps a is small
+    against the distance to the table's second pole, and from exp/sqrt elsewhere (trajectory ends, strong A, high
+    energies on coarse grids).  Vector potentials of 0.3 (inside the radius everywhere), 2 (mixed: the high-energy
+    lanes of a warp leave it) and 12 (outside everywhere) must all match the oracle, which knows neither path."""
+    wl = wlmod.make_workload(1, pts_per_xi=6, n_angles=16, n_energies=96)
+    rng = np.random.default_rng(17)
+    y, x = np.meshgrid((np.arange(wl.ny) - 0.5 * (wl.ny - 1)) * wl.h, (np.arange(wl.nx) - 0.5 * (wl.nx - 1)) * wl.h, indexing="ij")
+    r = max(float(np.max(np.hypot(x, y))), 1.0)
+    Ax = amp * (-y / r + 0.1 * rng.uniform(-1, 1, x.shape)); Ay = amp * (x / r + 0.1 * rng.uniform(-1, 1, x.shape))
+    o = oracle.Oracle.from_workload(wl)
+    g = GpuRun(sc, wl)
+    g.set_fields(wl.delta0, Ax, Ay)
+    stores = None
+    for it in range(2):
+        ro = o.sweep(wl.delta0, Ax, Ay, wl.n_energies, stores)
+        stores = ro["stores"]
+        rg = g.sweep()
+        for key in ("delta_new", "jx", "jy", "fe_I"):
+            assert relerr(rg[key], ro[key]) < TOL, (amp, it, key, relerr(rg[key], ro[key]))
+
+
+def test_coarse_grid_high_energies_leave_the_table(sc):
+    """h = 0.5 xi0 and eps up to 19: h^2 w reaches ~90, far outside anything a series in w could cover."""
+    wl = wlmod.make_workload(0, pts_per_xi=2, n_energies=38)
+    compare_sweeps(sc, wl, n_sweeps=2)
+
+
 def test_energy_sharded_sweep_equals_full_sweep(sc):
     """two energy shards (two contexts on one GPU, run one after the other), raw accumulators summed
     in the all-reduce hook, then finalised == the oracle's full sweep.  No kernel waits on another."""
