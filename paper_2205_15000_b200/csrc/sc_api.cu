@@ -97,9 +97,9 @@ struct sc_ctx {
     scgeo::Geometry geo;
     // physical trajectories (k < N/2)
     int G = 0; int smax = 0; long long n_nodes = 0; long long n_pieces_logical = 0;
-    std::vector<int> h_k, h_t, h_jf, h_nn, h_dF, h_dB, h_order, h_line_g;
+    std::vector<int> h_k, h_t, h_jf, h_nn, h_dF, h_dB, h_order, h_line_g, h_line_n;
     std::vector<long long> h_noff;
-    DevBuf<int> d_k, d_t, d_jf, d_nn, d_dF, d_dB, d_order, d_line_g;
+    DevBuf<int> d_k, d_t, d_jf, d_nn, d_dF, d_dB, d_order, d_line_g, d_line_n;
     DevBuf<double> d_l0, d_l1;
     DevBuf<long long> d_noff;
     DevBuf<double> d_vx, d_vy, d_eta, d_W;
@@ -246,7 +246,7 @@ sck::BackArgs back_args(sc_ctx* ctx, void* delta_new, double* jx, double* jy, do
     sck::BackArgs B{};
     B.G = grid_dev(ctx); B.nphi = ctx->geo.nphi; B.nrot = ctx->geo.nrot; B.c = ctx->geo.c;
     B.vx = ctx->d_vx.p; B.vy = ctx->d_vy.p; B.eta = ctx->d_eta.p; B.W = ctx->d_W.p;
-    B.line_g = ctx->d_line_g.p; B.T = traj_dev(ctx); B.part = ctx->d_part.p;
+    B.line_g = ctx->d_line_g.p; B.line_n = ctx->d_line_n.p; B.T = traj_dev(ctx); B.part = ctx->d_part.p;
     B.t = ctx->t; B.sigma = ctx->opt.charge_sign;
     B.D = std::log(ctx->t) + ctx->denom_sum;
     B.delta_new = (double2*)delta_new; B.jx = jx; B.jy = jy; B.feI = feI; B.n_bad = ctx->d_nbad.p;
@@ -313,15 +313,13 @@ sc_status sc_create(const sc_grid* grid, const unsigned char* mask, const sc_sha
         }
     if (scgeo::build(Gm, ctx->sym, opts->crystal_rotation, opts->quadrature)) return fail(ctx, SC_ERR_GEOMETRY, Gm.err);
     const int N = Gm.nphi, H = N / 2, NR = Gm.nrot;
-    for (size_t li = 0; li < Gm.line_count.size(); ++li)
-        if (Gm.line_count[li] > 1) return fail(ctx, SC_ERR_GEOMETRY, "lines crossing the grain more than once (holes, concave unions) are not built yet");
 
     // ---- physical trajectories = directed trajectories of the first half of the angles ----
     ctx->G = Gm.aoff[H];
     if (ctx->G == 0) return fail(ctx, SC_ERR_GEOMETRY, "grain contains no lattice node");
     const int G = ctx->G;
     ctx->h_k.resize(G); ctx->h_t.resize(G); ctx->h_jf.resize(G); ctx->h_nn.resize(G); ctx->h_dF.resize(G); ctx->h_dB.resize(G);
-    ctx->h_noff.resize(G); ctx->h_line_g.assign((size_t)H * NR, -1);
+    ctx->h_noff.resize(G); ctx->h_line_g.assign((size_t)H * NR, -1); ctx->h_line_n.assign((size_t)H * NR, 0);
     std::vector<double> l0(G), l1(G);
     long long nodes = 0, pieces = 0; int smax = 0;
     for (int g = 0; g < G; ++g) {
@@ -330,10 +328,13 @@ sc_status sc_create(const sc_grid* grid, const unsigned char* mask, const sc_sha
         l0[g] = (d.jf - Gm.c) * Gm.h - d.u_in; l1[g] = d.u_out - (d.jl - Gm.c) * Gm.h;
         ctx->h_noff[g] = nodes; nodes += ctx->h_nn[g]; pieces += ctx->h_nn[g] + 1; smax = std::max(smax, ctx->h_nn[g]);
         ctx->h_dF[g] = g;
-        const int mir = Gm.line_first[(size_t)(d.k + H) * NR + (NR - 1 - d.t)];
-        if (mir < 0) return fail(ctx, SC_ERR_GEOMETRY, "internal: mirror trajectory missing");
-        ctx->h_dB[g] = mir;
-        ctx->h_line_g[(size_t)d.k * NR + d.t] = g;
+        // mirror image on angle k+H: line N_rot-1-t, and (holes, concave unions) the intervals of a line in reverse order
+        const size_t li = (size_t)d.k * NR + d.t, lm = (size_t)(d.k + H) * NR + (NR - 1 - d.t);
+        const int c = g - Gm.line_first[li], cnt = Gm.line_count[li];
+        if (Gm.line_first[lm] < 0 || Gm.line_count[lm] != cnt) return fail(ctx, SC_ERR_GEOMETRY, "internal: mirror trajectory missing");
+        ctx->h_dB[g] = Gm.line_first[lm] + (cnt - 1 - c);
+        if (c == 0) ctx->h_line_g[li] = g;
+        ctx->h_line_n[li] = cnt;
     }
     ctx->n_nodes = nodes; ctx->n_pieces_logical = pieces; ctx->smax = smax;
     ctx->h_order.resize(G);
@@ -372,7 +373,7 @@ sc_status sc_create(const sc_grid* grid, const unsigned char* mask, const sc_sha
     CU(ctx->d_mask.upload(hm, s));
     CU(ctx->d_k.upload(ctx->h_k, s)); CU(ctx->d_t.upload(ctx->h_t, s)); CU(ctx->d_jf.upload(ctx->h_jf, s)); CU(ctx->d_nn.upload(ctx->h_nn, s));
     CU(ctx->d_dF.upload(ctx->h_dF, s)); CU(ctx->d_dB.upload(ctx->h_dB, s)); CU(ctx->d_order.upload(ctx->h_order, s));
-    CU(ctx->d_line_g.upload(ctx->h_line_g, s)); CU(ctx->d_l0.upload(l0, s)); CU(ctx->d_l1.upload(l1, s)); CU(ctx->d_noff.upload(ctx->h_noff, s));
+    CU(ctx->d_line_g.upload(ctx->h_line_g, s)); CU(ctx->d_line_n.upload(ctx->h_line_n, s)); CU(ctx->d_l0.upload(l0, s)); CU(ctx->d_l1.upload(l1, s)); CU(ctx->d_noff.upload(ctx->h_noff, s));
     CU(ctx->d_vx.upload(Gm.vx, s)); CU(ctx->d_vy.upload(Gm.vy, s)); CU(ctx->d_eta.upload(Gm.eta, s)); CU(ctx->d_W.upload(Gm.W, s));
     CU(ctx->d_ga_idx.upload(ga_idx, s)); CU(ctx->d_ga_w.upload(ga_w, s)); CU(ctx->d_ga_n.upload(ga_n, s));
     CU(ctx->d_fb_rows.upload(ctx->fb_rows, s)); CU(ctx->d_fb_px.upload(fpx, s)); CU(ctx->d_fb_py.upload(fpy, s));

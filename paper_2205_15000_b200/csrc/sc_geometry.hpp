@@ -127,8 +127,10 @@ inline std::vector<Seg> clip(const std::vector<ShapeH>& S, double vx, double vy,
     std::vector<Seg> out;
     for (size_t i = 0; i + 1 < ev.size(); ++i) {
         if (!(ev[i + 1].u - ev[i].u > 0.0)) continue;
-        const double um = 0.5 * (ev[i].u + ev[i + 1].u);
-        if (!in_grain(S, um * vx - w * vy, um * vy + w * vx)) continue;
+        // between two consecutive crossings the line is either inside or outside, except at a point where it only
+        // touches a boundary (a lattice line tangent to a hole): sample two points, neither the midpoint
+        const double u1 = ev[i].u + 0.37 * (ev[i + 1].u - ev[i].u), u2 = ev[i].u + 0.71 * (ev[i + 1].u - ev[i].u);
+        if (!in_grain(S, u1 * vx - w * vy, u1 * vy + w * vx) && !in_grain(S, u2 * vx - w * vy, u2 * vy + w * vx)) continue;
         if (!out.empty() && out.back().b.u == ev[i].u) out.back().b = ev[i + 1];   // fuse through an interior crossing
         else out.push_back(Seg{ev[i], ev[i + 1]});
     }

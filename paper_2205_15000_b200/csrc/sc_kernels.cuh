@@ -546,7 +546,8 @@ struct BackArgs {
     GridDev G;
     int nphi, nrot; double c;
     const double* vx; const double* vy; const double* eta; const double* W;
-    const int* line_g;           // [pair][t] -> physical trajectory or -1
+    const int* line_g;           // [pair][t] -> first physical trajectory on that lattice line, or -1
+    const int* line_n;           // [pair][t] -> number of trajectories (inside intervals) on that line
     TrajDev T;
     const double* part;          // [node][6]
     double t, D; int sigma;
@@ -562,33 +563,38 @@ __device__ __forceinline__ int back_weights(const BackArgs& B, int p, double x, 
     const int j0 = (int)floor(uu), t0 = (int)floor(ww);
     const double fu = uu - j0, fw = ww - t0;
     const int* lg = B.line_g + (size_t)p * B.nrot;
+    const int* ln = B.line_n + (size_t)p * B.nrot;
     int n = 0; double sw = 0.0;
 #pragma unroll
     for (int b = 0; b < 2; ++b) {
         const int tt = t0 + b;
         if (tt < 0 || tt >= B.nrot) continue;
-        const int g = lg[tt];
-        if (g < 0) continue;
-        const int jf = B.T.jf[g], nn = B.T.nn[g];
+        const int g0 = lg[tt];
+        if (g0 < 0) continue;
+        for (int g = g0; g < g0 + ln[tt]; ++g) {               // one interval unless the grain has holes / is concave
+            const int jf = B.T.jf[g], nn = B.T.nn[g];
 #pragma unroll
-        for (int a = 0; a < 2; ++a) {
-            const int jj = j0 + a;
-            if (jj < jf || jj >= jf + nn) continue;
-            const double wt = (a ? fu : 1.0 - fu) * (b ? fw : 1.0 - fw);
-            node[n] = B.T.noff[g] + (jj - jf); w[n] = wt; sw += wt; ++n;
+            for (int a = 0; a < 2; ++a) {
+                const int jj = j0 + a;
+                if (jj < jf || jj >= jf + nn) continue;
+                const double wt = (a ? fu : 1.0 - fu) * (b ? fw : 1.0 - fw);
+                node[n] = B.T.noff[g] + (jj - jf); w[n] = wt; sw += wt; ++n;
+            }
         }
     }
     if (sw > 1e-12) { const double r = 1.0 / sw; for (int i = 0; i < n; ++i) w[i] *= r; return n; }
     double bd = 1e300; long long best = -1;
     for (int tt = t0 - 2; tt <= t0 + 3; ++tt) {
         if (tt < 0 || tt >= B.nrot) continue;
-        const int g = lg[tt];
-        if (g < 0) continue;
-        const int jf = B.T.jf[g], nn = B.T.nn[g];
-        for (int jj = j0 - 2; jj <= j0 + 3; ++jj) {
-            if (jj < jf || jj >= jf + nn) continue;
-            const double d = (uu - jj) * (uu - jj) + (ww - tt) * (ww - tt);
-            if (d < bd) { bd = d; best = B.T.noff[g] + (jj - jf); }
+        const int g0 = lg[tt];
+        if (g0 < 0) continue;
+        for (int g = g0; g < g0 + ln[tt]; ++g) {
+            const int jf = B.T.jf[g], nn = B.T.nn[g];
+            for (int jj = j0 - 2; jj <= j0 + 3; ++jj) {
+                if (jj < jf || jj >= jf + nn) continue;
+                const double d = (uu - jj) * (uu - jj) + (ww - tt) * (ww - tt);
+                if (d < bd) { bd = d; best = B.T.noff[g] + (jj - jf); }
+            }
         }
     }
     if (best < 0) return 0;

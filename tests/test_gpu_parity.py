@@ -199,6 +199,21 @@ def test_coarse_grid_high_energies_leave_the_table(sc):
     compare_sweeps(sc, wl, n_sweeps=2)
 
 
+@pytest.mark.parametrize("kw", [dict(), dict(hole_offset=0.9, n_angles=12, pts_per_xi=4.0, n_energies=33)])
+def test_annulus_two_trajectories_per_line(sc, kw):
+    """Multiply-connected grain (disc minus disc, solenoid-gauge flux through the hole): lattice lines through the
+    hole carry two trajectories; specular reflection off the inner (concave) wall; rotate-back picks the interval."""
+    wl = wlmod.make_annulus_workload(**kw)
+    o, g, stores, worst = compare_sweeps(sc, wl, n_sweeps=3)
+    assert max(o.tables(0)["t"].tolist().count(t) for t in set(o.tables(0)["t"].tolist())) == 2
+    # LDOS through the same geometry (per-energy rotate-back)
+    e = np.array([-0.3, 0.0, 0.1, 0.3])
+    out = torch.zeros((len(e), wl.ny, wl.nx), dtype=torch.float64, device="cuda")
+    g.ctx.sc_ldos(e, 0.02, 2, out)
+    torch.cuda.synchronize()
+    assert relerr(out.cpu().numpy(), o.ldos(wl.delta0, wl.Aext_x, wl.Aext_y, e, 0.02, 2)) < TOL
+
+
 def test_energy_sharded_sweep_equals_full_sweep(sc):
     """two energy shards (two contexts on one GPU, run one after the other), raw accumulators summed
     in the all-reduce hook, then finalised == the oracle's full sweep.  No kernel waits on another."""

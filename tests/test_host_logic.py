@@ -59,9 +59,16 @@ CASES = [
 ]
 
 
+def _workload(cfg, kw):
+    return wlmod.make_annulus_workload(**kw) if cfg == "annulus" else wlmod.make_workload(cfg, **kw)
+
+
+CASES += [("annulus", {}), ("annulus", dict(hole_offset=0.9, n_angles=12, pts_per_xi=4.0))]   # two trajectories per line
+
+
 @pytest.mark.parametrize("cfg,kw", CASES)
 def test_trajectory_tables_match_oracle(lib, cfg, kw):
-    wl = wlmod.make_workload(cfg, **kw)
+    wl = _workload(cfg, kw)
     o = oracle.Oracle.from_workload(wl)
     c = sc.ScContext.from_workload(wl, tables_only=True)
     assert c.n_rot == o.nrot and c.n_traj == o.ntraj
@@ -79,10 +86,11 @@ def test_trajectory_tables_match_oracle(lib, cfg, kw):
     c.close()
 
 
-def test_mirror_structure_of_tables(lib):
+@pytest.mark.parametrize("annulus", [False, True])
+def test_mirror_structure_of_tables(lib, annulus):
     """angle k+N/2 is the exact mirror (j,t)->(N_rot-1-j, N_rot-1-t) of angle k — what lets the kernel take
-    gamma-tilde_k from gamma_{k+N/2} (Eq. 13 :95)."""
-    wl = wlmod.make_workload(1, pts_per_xi=5, n_angles=16, n_energies=4)
+    gamma-tilde_k from gamma_{k+N/2} (Eq. 13 :95); with a hole, the intervals of a line come in reverse order."""
+    wl = wlmod.make_annulus_workload(hole_offset=0.7) if annulus else wlmod.make_workload(1, pts_per_xi=5, n_angles=16, n_energies=4)
     c = sc.ScContext.from_workload(wl, tables_only=True)
     H = wl.n_angles // 2
     for k in range(H):

@@ -261,3 +261,27 @@ def matsubara(t: float, n: int):
     """eps_n = t (n + 1/2), n = 0..n-1, unit weights (PAPER.md:98 in units of 2 pi kB Tc)."""
     nn = np.arange(n, dtype=np.float64)
     return np.zeros(n), t * (nn + 0.5), np.ones(n)
+
+
+def make_annulus_workload(r_in: float = 1.53, r_out: float = 4.0, pts_per_xi: float = 5.0, n_angles: int = 16,
+                          n_energies: int = 24, t: float = 0.3, kappa: float = 3.0, flux_in_hole: float = 1.0,
+                          hole_offset: float = 0.0, seed: int = 7) -> Workload:
+    """Multiply-connected grain: a disc with a disc removed ("remove"), threaded
+    by `flux_in_hole` flux quanta in the solenoid gauge A = Phi/(2 r) phi-hat (units A0 = Phi0/(pi xi0); the
+    paper's annulus benchmarks :563-569), order parameter with the matching winding plus seeded noise.  Lattice
+    lines through the hole cross the grain twice: two trajectories per line."""
+    rng = np.random.Generator(np.random.PCG64(SEED_BASE + 100 + seed))
+    h = 1.0 / pts_per_xi
+    n = _even_grid(2 * r_out, h)
+    shapes = [disc(r_out), disc(r_in, cx=hole_offset, cy=0.0, add=False)]
+    mask = make_mask(shapes, n, n, h)
+    X, Y = grid_xy(n, n, h)
+    Xc = X - hole_offset
+    r2 = np.maximum(Xc * Xc + Y * Y, (0.5 * h) ** 2)
+    Ax = -0.5 * flux_in_hole * Y / r2; Ay = 0.5 * flux_in_hole * Xc / r2
+    gap = 0.25
+    delta0 = gap * (1.0 + 0.05 * rng.uniform(-1, 1, (n, n))) * np.exp(-1j * round(flux_in_hole) * np.arctan2(Y, Xc)
+                                                                      + 0.05j * rng.uniform(-1, 1, (n, n)))
+    return Workload("annulus_swave_solenoid", -2, n, n, h, shapes, mask, SYM_S, 0.0, n_angles, n_energies, t, kappa, -1,
+                    delta0 * mask, Ax, Ay, gap, accelerator=1, n_iterations=5)
+
