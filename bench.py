@@ -34,17 +34,20 @@ import workloads  # noqa: E402
 
 METRIC = "riccati_trajectory_step_updates_per_s"
 UNIT = "updates/s"
-# FP64-pipe instructions the closed-form path needs per (node, energy, angle pair) = 4 logical updates
-# (gamma and gamma-tilde for angles k and k+N/2): DESIGN.md §6 tally of the kernel's own algorithm (step coefficient
-# T from the per-energy table 36, two Moebius steps 54, node products 28, energy reduction 8); ncu counts 126.1
-# executed.  Evaluating T from its definition (sqrt, exp, sin/cos) instead would be 184 — reported as context only.
-ALGO_FP64_INSTR_PER_UNIT = 126.0
+# FP64-pipe instructions the closed-form path needs per unit = (piece, energy, angle pair) = 4 logical updates
+# (gamma and gamma-tilde for angles k and k+N/2): DESIGN.md §6 tally of the kernel's own algorithm.
+#   "recompute" rounds (every piece inside the radius of the per-energy Taylor table of T): T twice 2 x 17, two Moebius
+#       steps 54, node products 27, energy reduction 8 = 123; scratch traffic 16 B written + 16 B read = 32 B per unit
+#   "stored-T" rounds (strong vector potential): T once from the pole-subtracted table 36, 54, 27, 8 = 125; 64 B per unit
+# Evaluating T from its definition (sqrt, exp, sin/cos) would be 86 per evaluation — reported as context only.
+ALGO_FP64_INSTR_PER_UNIT = {"recompute": 123.0, "stored": 125.0}
+ALGO_HBM_BYTES_PER_UNIT = {"recompute": 32.0, "stored": 64.0}
 TEXTBOOK_FP64_INSTR_PER_UNIT = 184.0
-ALGO_FP64_INSTR_PER_UNIT_MIDPOINT = 2 * 66.0 + 28.0 + 8.0
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE march launch at configs[4], fp64, closed-form stepper, from the
-# `ncu --set full` capture summarised in profiles/r1_march_fp64_cfg4_ncu_full.md (4.922 TB read + 4.421 TB written)
-NCU_TRAFFIC_BYTES = {(4, 64, 0): 9.343071e12}
-NCU_PIPE_FP64_ACTIVE_PCT = {(4, 64, 0): 68.0}
+ALGO_FP64_INSTR_PER_UNIT_MIDPOINT = 2 * 66.0 + 27.0 + 8.0
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE march launch at configs[4], fp64, closed-form stepper, all rounds in
+# "recompute" mode (--sweep-only: A = A_ext), from the `ncu --set full` capture summarised in profiles/
+NCU_TRAFFIC_BYTES = {}
+NCU_PIPE_FP64_ACTIVE_PCT = {}
 
 
 class ClockSampler(threading.Thread):
@@ -210,6 +213,7 @@ def run_ours(a):
         dist.barrier()
     torch.cuda.synchronize()
     ctx.sc_debug_march_time()                       # reset: count only the march launches of the timed steps
+    ctx.sc_debug_march_units()
     e0.record()
     for _ in range(a.steps):
         step()
@@ -220,6 +224,7 @@ def run_ours(a):
     ms = e0.elapsed_time(e1)
     clocks = sampler.stop()
     march_total_ms, march_launches = ctx.sc_debug_march_time()      # CUDA events around each march launch of the timed region
+    units_timed, units_timed_stored = ctx.sc_debug_march_units()     # units of those launches, and how many spilled T
     if world > 1:                                   # device time of the slowest rank
         tmax = torch.tensor([ms], dtype=torch.float64, device=devname)
         dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
@@ -237,26 +242,40 @@ def run_ours(a):
     peak_dfma, clk = ctx.sc_debug_fp64_peak()
     mk_ms = march_total_ms / max(march_launches, 1)
     full_size = world == 1 and not (a.pts_per_xi or a.n_angles or a.n_energies or a.size_scale != 1.0)
-    algo = ALGO_FP64_INSTR_PER_UNIT if a.stepper == 0 else ALGO_FP64_INSTR_PER_UNIT_MIDPOINT
-    achieved = 2.0 * algo * units / (mk_ms * 1e-3) / 1e12
-    peak = 2.0 * peak_dfma / 1e12
+    # algorithmic work of ONE average march launch of the timed region (units counted by the library, by mode)
+    nl = max(march_launches, 1)
+    u_all = units_timed / nl; u_st = units_timed_stored / nl; u_rec = u_all - u_st
+    if a.stepper == 0:
+        instr = ALGO_FP64_INSTR_PER_UNIT["recompute"] * u_rec + ALGO_FP64_INSTR_PER_UNIT["stored"] * u_st
+        hbm = ALGO_HBM_BYTES_PER_UNIT["recompute"] * u_rec + ALGO_HBM_BYTES_PER_UNIT["stored"] * u_st
+    else:
+        instr = ALGO_FP64_INSTR_PER_UNIT_MIDPOINT * u_all
+        hbm = 32.0 * u_all
+    if a.precision == 32:
+        hbm *= 0.5
+    achieved = 2.0 * instr / (mk_ms * 1e-3) / 1e12
+    peak_burst = 2.0 * peak_dfma / 1e12
     peak_sustained = 2.0 * ctx.sc_debug_fp64_peak_sustained(2.0) / 1e12
-    roofline = {"bound": "alu", "kernel": "sck::march_kernel<0,false,%d,%s>" % (a.stepper, "double" if a.precision == 64 else "float"), "launches_timed": march_launches, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+    peak = max(peak_burst, peak_sustained)
+    key = (wl.cfg, a.precision, a.stepper)
+    roofline = {"bound": "alu", "kernel": "sck::march_kernel<0,false,%d,%s,1>" % (a.stepper, "double" if a.precision == 64 else "float"),
+                "launches_timed": march_launches, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                 "frac": achieved / peak,
-                "traffic": NCU_TRAFFIC_BYTES.get((wl.cfg, a.precision, a.stepper)) if full_size else None,
-                "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/)",
-                "algorithmic_bytes_per_launch": 64.0 * units,
-                "ncu_pipe_fp64_cycles_active_pct": NCU_PIPE_FP64_ACTIVE_PCT.get((wl.cfg, a.precision, a.stepper)) if full_size else None,
+                "traffic": NCU_TRAFFIC_BYTES.get(key) if full_size and u_st == 0 else None,
+                "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/; capture with all rounds in recompute mode)",
+                "algorithmic_bytes_per_launch": hbm,
+                "ncu_pipe_fp64_cycles_active_pct": NCU_PIPE_FP64_ACTIVE_PCT.get(key) if full_size else None,
                 "note": "fp64 pipe: flops = 2 x FP64-pipe instructions; achieved = algorithmic count (DESIGN.md §6) x units / "
                         "march duration (CUDA events around the march launches of the timed steps); peak = register-resident "
-                        "DFMA rate measured in this process, best of 3 short runs (burst clock); peak_sustained = the same "
-                        "loop held for 2 s (power-limited clock, what a 1.8 s march launch can draw on)",
-                "peak_sustained": peak_sustained, "frac_of_sustained": achieved / peak_sustained,
+                        "DFMA rate measured in this process: the larger of a best-of-3 burst (11 ms) and a 2 s sustained run",
+                "peak_burst": peak_burst, "peak_sustained": peak_sustained,
                 "textbook_count_context": {"fp64_instr_per_unit": TEXTBOOK_FP64_INSTR_PER_UNIT,
-                                           "tflops": 2.0 * TEXTBOOK_FP64_INSTR_PER_UNIT * units / (mk_ms * 1e-3) / 1e12},
-                "march_ms": mk_ms, "march_share_of_step": mk_ms / (ms / a.steps), "algo_fp64_instr_per_unit": algo,
-                "units_per_launch": units, "hbm_bytes_per_unit_algorithmic": 64.0,
-                "hbm_gbs_algorithmic": 64.0 * units / (mk_ms * 1e-3) / 1e9}
+                                           "tflops": 2.0 * TEXTBOOK_FP64_INSTR_PER_UNIT * u_all / (mk_ms * 1e-3) / 1e12},
+                "march_ms": mk_ms, "march_share_of_step": mk_ms / (ms / a.steps),
+                "algo_fp64_instr_per_unit": instr / max(u_all, 1.0), "units_per_launch": u_all,
+                "units_share_stored_T": u_st / max(u_all, 1.0),
+                "hbm_bytes_per_unit_algorithmic": hbm / max(u_all, 1.0),
+                "hbm_gbs_algorithmic": hbm / (mk_ms * 1e-3) / 1e9}
 
     # end to end through the C ABI with HOST buffers: H2D of Delta, A_ind; iterate; D2H of Delta, A_ind + stats
     hd = torch.empty((wl.ny, wl.nx), dtype=torch.complex128).pin_memory(); hd.copy_(delta)
@@ -305,7 +324,7 @@ def run_ours(a):
             dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
             ms32 = float(tmax.item())
         fp32_leg = {"dtype": "f32", "value": n_updates * a.steps / (ms32 * 1e-3), "unit": UNIT, "ms_per_step": ms32 / a.steps,
-                    "march_ms": c32.sc_debug_march_time()[0] / a.steps, "hbm_bytes_per_unit_algorithmic": 32.0}
+                    "march_ms": c32.sc_debug_march_time()[0] / a.steps}
         c32.close()
 
     value = n_updates * a.steps / (ms * 1e-3)

@@ -109,6 +109,7 @@ def load_library():
     L.sc_debug_last_march_ms.argtypes = [vp, C.POINTER(C.c_float)]
     L.sc_debug_fp64_peak_sustained.argtypes = [vp, d, C.POINTER(d)]
     L.sc_debug_march_time.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(i)]
+    L.sc_debug_march_units.argtypes = [vp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
     _lib = L
     return L
 
@@ -294,6 +295,12 @@ class ScContext:
         ms, n = C.c_float(), C.c_int()
         self._check(self._L.sc_debug_march_time(self._h, C.byref(ms), C.byref(n)))
         return ms.value, n.value
+
+    def sc_debug_march_units(self):
+        """(units marched, units in rounds that spilled T) since the previous call; resets."""
+        a, b = C.c_longlong(), C.c_longlong()
+        self._check(self._L.sc_debug_march_units(self._h, C.byref(a), C.byref(b)))
+        return a.value, b.value
 
     def sc_debug_fp64_peak_sustained(self, seconds=2.0):
         a = C.c_double()

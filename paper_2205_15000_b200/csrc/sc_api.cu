@@ -41,9 +41,10 @@ struct DevBuf {
 struct EnergySet {
     std::vector<double> zr, zi, w; std::vector<int> partner;
     DevBuf<double> d_zr, d_zi, d_w; DevBuf<int> d_partner;
-    std::vector<double> tc; DevBuf<double> d_tc;      // Taylor table of T (empty: not on the imaginary axis)
+    std::vector<double> tc; DevBuf<double> d_tc; int tmode = 1;     // Taylor table of T; 1: real coefficients, 2: complex
+    std::vector<double> tcp; DevBuf<double> d_tcp;                  // tmode 1: pole-subtracted table
     int ne = 0;
-    sck::EnergyDev dev() const { return sck::EnergyDev{ne, d_zr.p, d_zi.p, d_w.p, d_partner.p, tc.empty() ? nullptr : d_tc.p}; }
+    sck::EnergyDev dev() const { return sck::EnergyDev{ne, d_zr.p, d_zi.p, d_w.p, d_partner.p, d_tc.p, d_tcp.p, tmode}; }
 };
 
 // T(w) = tanh(h sqrt w)/sqrt w for complex w (even in sqrt w: no branch issue); series near w = 0
@@ -54,18 +55,39 @@ std::complex<double> T_of_w(std::complex<double> w, double h) {
     return std::tanh(h * x) / x;
 }
 
-// Table behind sc_math.cuh taylor_T for every energy i*zi on the imaginary axis: with the nearest pole of
-// T(w) = sum_k (2/h)/(w + (2k+1)^2 wp) removed, R(w) = T(w) - (2/h)/(w + wp) is analytic for |w - w0| < w0 + 9 wp,
-// w0 = zi^2; its Taylor coefficients r_k = R^(k)(w0)/k! come from the trapezoid rule on a circle of half that radius
-// (geometric convergence; R is real on the real axis, so the r_k are real).
-// Row = r_0..r_8, (w0 + 9 wp)^2, w0 + wp, 2/h.
+// Table behind sc_math.cuh taylor_real / taylor_cplx: for every energy z0, the Taylor coefficients
+// c_k = T^(k)(w0)/k! of T(w) about w0 = -z0^2, k = 0..TC_KMAX.  T(w) = sum_j (2/h)/(w + (2j+1)^2 wp), wp = (pi/2h)^2,
+// is analytic inside the circle through the nearest pole; the c_k come from the trapezoid rule on a circle of
+// half that radius (geometric convergence).  On the imaginary axis w0 is real and so are the c_k.
+// Row = Re c_0..c_8, Im c_0..c_8, (distance to the nearest pole)^2.
 void taylor_table(EnergySet& E, double h) {
-    E.tc.clear();
-    for (double v : E.zr) if (v != 0.0) return;
     const double PI = 3.14159265358979323846, wp = (PI / (2.0 * h)) * (PI / (2.0 * h));
-    const int M = 128;
+    const int M = 128, K = sck::TC_KMAX;
+    E.tmode = 1;
+    for (double v : E.zr) if (v != 0.0) E.tmode = 2;
     E.tc.assign((size_t)E.zr.size() * sck::TC_LD, 0.0);
     std::vector<std::complex<double>> f(M);
+    for (size_t n = 0; n < E.zi.size(); ++n) {
+        const std::complex<double> z0(E.zr[n], E.zi[n]), w0 = -z0 * z0;
+        double rad = 1e300;
+        for (int j = 0; j < 64; ++j) rad = std::min(rad, std::abs(w0 + (2.0 * j + 1.0) * (2.0 * j + 1.0) * wp));
+        const double rho = 0.5 * rad;
+        for (int j = 0; j < M; ++j) f[j] = T_of_w(w0 + std::polar(rho, 2.0 * PI * j / M), h);
+        double rk = 1.0;
+        for (int k = 0; k <= K; ++k) {
+            std::complex<double> acc = 0.0;
+            for (int j = 0; j < M; ++j) acc += f[j] * std::polar(1.0, -2.0 * PI * ((j * k) % M) / M);
+            E.tc[n * sck::TC_LD + k] = acc.real() / M / rk;
+            E.tc[n * sck::TC_LD + K + 1 + k] = E.tmode == 2 ? acc.imag() / M / rk : 0.0;
+            rk *= rho;
+        }
+        E.tc[n * sck::TC_LD + 2 * (K + 1)] = rad * rad;
+    }
+    // Imaginary axis: second table with the nearest pole removed, R(w) = T(w) - (2/h)/(w + wp), analytic out to the
+    // second pole: |w - w0| < w0 + 9 wp.  Row = r_0..r_8, (w0 + 9 wp)^2, w0 + wp, 2/h.
+    E.tcp.clear();
+    if (E.tmode != 1) return;
+    E.tcp.assign((size_t)E.zr.size() * sck::TCP_LD, 0.0);
     for (size_t n = 0; n < E.zi.size(); ++n) {
         const double w0 = E.zi[n] * E.zi[n], rad = w0 + 9.0 * wp, rho = 0.5 * rad;
         for (int j = 0; j < M; ++j) {
@@ -76,12 +98,12 @@ void taylor_table(EnergySet& E, double h) {
         for (int k = 0; k <= 8; ++k) {
             std::complex<double> acc = 0.0;
             for (int j = 0; j < M; ++j) acc += f[j] * std::polar(1.0, -2.0 * PI * ((j * k) % M) / M);
-            E.tc[n * sck::TC_LD + k] = acc.real() / M / rk;
+            E.tcp[n * sck::TCP_LD + k] = acc.real() / M / rk;
             rk *= rho;
         }
-        E.tc[n * sck::TC_LD + 9] = rad * rad;
-        E.tc[n * sck::TC_LD + 10] = w0 + wp;
-        E.tc[n * sck::TC_LD + 11] = 2.0 / h;
+        E.tcp[n * sck::TCP_LD + 9] = rad * rad;
+        E.tcp[n * sck::TCP_LD + 10] = w0 + wp;
+        E.tcp[n * sck::TCP_LD + 11] = 2.0 / h;
     }
 }
 
@@ -112,7 +134,7 @@ struct sc_ctx {
     // fields
     DevBuf<double2> d_delta; DevBuf<double> d_Ax, d_Ay; bool have_A = false, have_fields = false;
     DevBuf<double> d_Aext_x, d_Aext_y; bool have_Aext = false;
-    DevBuf<double2> d_ndD; DevBuf<double> d_nda; DevBuf<float2> d_ndDr; DevBuf<char> d_pc; bool nodes_fresh = false;
+    DevBuf<double2> d_ndD; DevBuf<double> d_nda; DevBuf<float2> d_ndDr; DevBuf<char> d_pc; DevBuf<float2> d_pmax; bool nodes_fresh = false;
     bool f32 = false;            // opts.precision == 32: pc, stores, scratch hold float; ABI buffers stay fp64
     size_t rsz() const { return f32 ? sizeof(float) : sizeof(double); }
     // energies and stores
@@ -120,10 +142,11 @@ struct sc_ctx {
     DevBuf<char> d_store[2]; int cur = 0; bool stores_valid = false;      // V2 of R [directed trajectory][energy]
     // scratch
     DevBuf<char> d_scr; long long scr_stride = 0; int n_slots = 0;       // scr_stride in bytes
-    DevBuf<double> d_part; DevBuf<int> d_counter; DevBuf<int> d_nbad; DevBuf<double> d_statmax;
+    DevBuf<double> d_part; DevBuf<int> d_counter; DevBuf<int> d_nbad; DevBuf<double> d_statmax; DevBuf<unsigned long long> d_nstored;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     static constexpr int MEV = 64;                 // ring of event pairs around the march launches (sc_debug_march_time)
     cudaEvent_t mev[MEV][2] = {}; int mev_n = 0;
+    long long march_units = 0;                    // (piece, energy) units of the march launches since the last sc_debug_march_units
     // Eq. 22 denominator sum (sum_n w_n t / eps_n over the WHOLE job's energy table) and the energy-shard hook
     double denom_sum = 0.0;
     double* hook_acc = nullptr; sc_allreduce_fn hook_fn = nullptr; void* hook_user = nullptr;
@@ -147,7 +170,7 @@ sck::TrajDev traj_dev(const sc_ctx* c) {
 sc_status upload_energies(sc_ctx* ctx, EnergySet& E) {
     E.ne = (int)E.zr.size();
     taylor_table(E, ctx->grid.h);
-    CU(E.d_tc.upload(E.tc, ctx->stream));
+    CU(E.d_tc.upload(E.tc, ctx->stream)); CU(E.d_tcp.upload(E.tcp, ctx->stream));
     CU(E.d_zr.upload(E.zr, ctx->stream)); CU(E.d_zi.upload(E.zi, ctx->stream));
     CU(E.d_w.upload(E.w, ctx->stream)); CU(E.d_partner.upload(E.partner, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
@@ -161,11 +184,11 @@ sc_status ensure_nodes(sc_ctx* ctx) {
     if (ctx->f32)
         sck::rotate_in_kernel<float><<<(ctx->G + wpb - 1) / wpb, wpb * 32, 0, ctx->stream>>>(
             grid_dev(ctx), traj_dev(ctx), ctx->d_vx.p, ctx->d_vy.p, ctx->d_eta.p, ctx->geo.c, ctx->opt.charge_sign,
-            ctx->d_ndD.p, ctx->d_nda.p, ctx->d_ndDr.p, (float4*)ctx->d_pc.p, ctx->d_nbad.p);
+            ctx->d_ndD.p, ctx->d_nda.p, ctx->d_ndDr.p, (float4*)ctx->d_pc.p, ctx->d_pmax.p, ctx->d_nbad.p);
     else
         sck::rotate_in_kernel<double><<<(ctx->G + wpb - 1) / wpb, wpb * 32, 0, ctx->stream>>>(
             grid_dev(ctx), traj_dev(ctx), ctx->d_vx.p, ctx->d_vy.p, ctx->d_eta.p, ctx->geo.c, ctx->opt.charge_sign,
-            ctx->d_ndD.p, ctx->d_nda.p, nullptr, (double4*)ctx->d_pc.p, ctx->d_nbad.p);
+            ctx->d_ndD.p, ctx->d_nda.p, nullptr, (double4*)ctx->d_pc.p, ctx->d_pmax.p, ctx->d_nbad.p);
     if (!ctx->fb_rows.empty()) {
         const int n = (int)ctx->fb_rows.size();
         sck::fallback_kernel<<<(n + 127) / 128, 128, 0, ctx->stream>>>(grid_dev(ctx), n, ctx->d_fb_rows.p, ctx->d_fb_px.p,
@@ -186,27 +209,27 @@ sck::MarchArgsT<R> march_args(sc_ctx* ctx, const EnergySet& E, const char* store
     const V2* store_old = (const V2*)store_old_raw; V2* store_new = (V2*)store_new_raw;
     sck::MarchArgsT<R> A{};
     A.T = traj_dev(ctx); A.E = E.dev(); A.order = ctx->d_order.p; A.n_items = ctx->G;
-    A.nd_D = node_D<R>(ctx); A.pc = (const V4*)ctx->d_pc.p; A.bc_mode = ctx->opt.bc_mode;
+    A.nd_D = node_D<R>(ctx); A.pc = (const V4*)ctx->d_pc.p; A.pmax = ctx->d_pmax.p; A.h = ctx->grid.h; A.bc_mode = ctx->opt.bc_mode;
     A.ga_idx = ctx->d_ga_idx.p; A.ga_w = ctx->d_ga_w.p; A.ga_n = ctx->d_ga_n.p;
     A.fb_D = ctx->d_fb_D.p; A.fb_a = ctx->d_fb_a.p;
     A.store_old = store_old; A.store_new = store_new;
     A.scr = ctx->d_scr.p; A.scr_stride = ctx->scr_stride;
-    A.part = ctx->d_part.p; A.ldos = nullptr; A.counter = ctx->d_counter.p; A.stat_max2 = ctx->d_statmax.p;
+    A.part = ctx->d_part.p; A.ldos = nullptr; A.counter = ctx->d_counter.p; A.stat_max2 = ctx->d_statmax.p; A.n_stored = ctx->d_nstored.p;
     return A;
 }
 
-template <int MODE, bool STATS, int STEP, typename R>
+template <int MODE, bool STATS, int STEP, typename R, int TM>
 sc_status launch_march_t(sc_ctx* ctx, const sck::MarchArgsT<R>& A) {
     const int blocks = ctx->n_slots / sck::MARCH_WARPS;
     const int smem = sck::march_smem<R>();
     static bool attr_set = false;
     if (!attr_set) {
-        CU(cudaFuncSetAttribute(sck::march_kernel<MODE, STATS, STEP, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        CU(cudaFuncSetAttribute(sck::march_kernel<MODE, STATS, STEP, R, TM>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         attr_set = true;
     }
     cudaEvent_t* ev = ctx->mev[ctx->mev_n % sc_ctx::MEV];
     CU(cudaEventRecord(ev[0], ctx->stream));
-    sck::march_kernel<MODE, STATS, STEP, R><<<blocks, sck::MARCH_WARPS * 32, smem, ctx->stream>>>(A);
+    sck::march_kernel<MODE, STATS, STEP, R, TM><<<blocks, sck::MARCH_WARPS * 32, smem, ctx->stream>>>(A);
     CU(cudaEventRecord(ev[1], ctx->stream));
     ++ctx->mev_n;
     CU(cudaGetLastError());
@@ -218,10 +241,12 @@ sc_status launch_march_r(sc_ctx* ctx, const EnergySet& E, const char* so, char* 
                          const int* items, int n_items, double* ldos) {
     sck::MarchArgsT<R> A = march_args<R>(ctx, E, so, sn);
     if (items) { A.order = items; A.n_items = n_items; }
+    else ctx->march_units += ctx->n_pieces_logical * E.ne;
     A.ldos = ldos;
     const bool st = stats && MODE == 0;
-    if (ctx->opt.stepper == 1) return st ? launch_march_t<MODE, MODE == 0, 1, R>(ctx, A) : launch_march_t<MODE, false, 1, R>(ctx, A);
-    return st ? launch_march_t<MODE, MODE == 0, 0, R>(ctx, A) : launch_march_t<MODE, false, 0, R>(ctx, A);
+    if (ctx->opt.stepper == 1) return st ? launch_march_t<MODE, MODE == 0, 1, R, 1>(ctx, A) : launch_march_t<MODE, false, 1, R, 1>(ctx, A);
+    if (E.tmode == 2) return st ? launch_march_t<MODE, MODE == 0, 0, R, 2>(ctx, A) : launch_march_t<MODE, false, 0, R, 2>(ctx, A);
+    return st ? launch_march_t<MODE, MODE == 0, 0, R, 1>(ctx, A) : launch_march_t<MODE, false, 0, R, 1>(ctx, A);
 }
 
 // one march launch over the work list (default: all physical trajectories, longest first)
@@ -383,11 +408,11 @@ sc_status sc_create(const sc_grid* grid, const unsigned char* mask, const sc_sha
 
     const size_t ng = (size_t)grid->nx * grid->ny;
     CU(ctx->d_delta.alloc(ng)); CU(ctx->d_Ax.alloc(ng)); CU(ctx->d_Ay.alloc(ng));
-    CU(ctx->d_ndD.alloc(nodes)); CU(ctx->d_nda.alloc(nodes)); CU(ctx->d_pc.alloc((size_t)(nodes + G) * 4 * ctx->rsz()));
+    CU(ctx->d_ndD.alloc(nodes)); CU(ctx->d_nda.alloc(nodes)); CU(ctx->d_pc.alloc((size_t)(nodes + G) * 4 * ctx->rsz())); CU(ctx->d_pmax.alloc(G));
     if (ctx->f32) CU(ctx->d_ndDr.alloc(nodes));
     CU(ctx->d_part.alloc((size_t)nodes * sck::RED_VALS));
-    CU(ctx->d_counter.alloc(1)); CU(ctx->d_nbad.alloc(1));
-    CU(cudaMemsetAsync(ctx->d_nbad.p, 0, sizeof(int), s));
+    CU(ctx->d_counter.alloc(1)); CU(ctx->d_nbad.alloc(1)); CU(ctx->d_nstored.alloc(1));
+    CU(cudaMemsetAsync(ctx->d_nbad.p, 0, sizeof(int), s)); CU(cudaMemsetAsync(ctx->d_nstored.p, 0, sizeof(unsigned long long), s));
 
     // Matsubara energies eps_n = t(n+1/2) (:98), unit weights, self-partnered (z = i eps -> -conj z = z)
     EnergySet& E = ctx->mats;
@@ -396,9 +421,10 @@ sc_status sc_create(const sc_grid* grid, const unsigned char* mask, const sc_sha
     for (int n = 0; n < opts->n_matsubara; ++n) ctx->denom_sum += 1.0 / (n + 0.5);
     CU(ctx->d_store[0].alloc((size_t)ND * E.ne * 2 * ctx->rsz())); CU(ctx->d_store[1].alloc((size_t)ND * E.ne * 2 * ctx->rsz()));
 
-    // persistent march grid: MARCH_MIN_CTAS CTAs of 8 warps per SM; per-warp scratch of (smax+1) pieces x 32 lanes
+    // persistent march grid: MARCH_MIN_CTAS CTAs of 8 warps per SM; per-warp scratch of smax + 1 (+2 spare) entries x 32 lanes
+    // x {T, gamma~} (rounds that recompute T in pass 2 use half of each row's bytes)
     ctx->n_slots = ctx->n_sm * sck::MARCH_MIN_CTAS * sck::MARCH_WARPS;
-    ctx->scr_stride = (long long)(smax + 2) * 32 * (opts->stepper == 1 ? 2 : 4) * (long long)ctx->rsz();
+    ctx->scr_stride = (long long)(smax + 3) * 32 * 4 * (long long)ctx->rsz();
     CU(ctx->d_scr.alloc((size_t)ctx->n_slots * ctx->scr_stride + 16384));   // + 16 KB: the L2 prefetch of the last slot may run past its end
     CU(ctx->d_statmax.alloc(ctx->n_slots));
     CU(cudaMemsetAsync(ctx->d_statmax.p, 0, ctx->n_slots * sizeof(double), s));
@@ -705,6 +731,17 @@ sc_status sc_debug_march_time(sc_ctx* ctx, float* total_ms, int* n_launches) {
     if (total_ms) *total_ms = tot;
     if (n_launches) *n_launches = n;
     ctx->mev_n = 0;
+    return SC_OK;
+}
+
+sc_status sc_debug_march_units(sc_ctx* ctx, long long* units_total, long long* units_stored_T) {
+    if (!ctx) return SC_ERR_ARG;
+    CU(cudaStreamSynchronize(ctx->stream));
+    unsigned long long ns = 0; CU(cudaMemcpy(&ns, ctx->d_nstored.p, sizeof(ns), cudaMemcpyDeviceToHost));
+    CU(cudaMemset(ctx->d_nstored.p, 0, sizeof(ns)));
+    if (units_stored_T) *units_stored_T = (long long)ns;
+    if (units_total) *units_total = ctx->march_units;
+    ctx->march_units = 0;
     return SC_OK;
 }
 

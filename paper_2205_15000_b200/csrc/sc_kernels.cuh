@@ -2,8 +2,8 @@
 //
 //   rotate_in_kernel     a2: Delta, A on the reference grid -> node coefficients on every trajectory
 //   reset_store_kernel   R8: boundary stores := local homogeneous solution
-//   march_kernel         a3+a4+a5: boundary gather, gamma-tilde down (stores T and gamma-tilde per node),
-//                        gamma up (re-uses T), node products, reduction over energies
+//   march_kernel         a3+a4+a5: boundary gather, gamma-tilde down (stores gamma-tilde per node), gamma up,
+//                        node products, reduction over energies
 //   rotate_back_kernel   a6+a7: masked-bilinear gather of the per-angle sums to the grid, angle sum, finalise
 //
 // One warp owns one trajectory of one angle pair (k, k+N/2); its 32 lanes are 32 energies.  Delta and A
@@ -44,10 +44,14 @@ struct TrajDev {                 // physical trajectories (angles k < N/2), stru
     const int* dF; const int* dB;   // store rows: (k,t) and its mirror (k+N/2, N_rot-1-t)
 };
 
-// tc: per-energy table of the step coefficient T (sc_math.cuh taylor_T), [ne][TC_LD] = r_0..r_8, (w0 + 9 wp)^2,
-// w0 + wp, 2/h; null when the energy table is not on the imaginary axis (then every piece takes the exp-based evaluation)
-constexpr int TC_LD = 12;
-struct EnergyDev { int ne; const double* zr; const double* zi; const double* w; const int* partner; const double* tc; };
+// tc: per-energy Taylor table of the step coefficient T (sc_math.cuh), [ne][TC_LD] = Re c_0..c_8, Im c_0..c_8,
+// (distance from w0 = -z0^2 to the nearest pole of T)^2.  tmode 1: every energy on the imaginary axis (real c_k);
+// 2: general energies in the upper half plane (complex c_k).
+// tcp (tmode 1 only): the pole-subtracted table, [ne][TCP_LD] = r_0..r_8, (distance to the second pole)^2, w0 + wp, 2/h.
+constexpr int TC_KMAX = 8;
+constexpr int TC_LD = 2 * (TC_KMAX + 1) + 2;
+constexpr int TCP_LD = 12;
+struct EnergyDev { int ne; const double* zr; const double* zi; const double* w; const int* partner; const double* tc; const double* tcp; int tmode; };
 
 // ------------------------------------------------------------------------------------------------
 // masked bilinear interpolation of Delta (R5) and plain bilinear of A at a point
@@ -97,13 +101,14 @@ __device__ __forceinline__ double interp_plain(const GridDev& G, const double* F
 }
 
 // a2: one warp per trajectory, lanes over nodes (coalesced along the trajectory).  Also writes the PIECE
-// coefficients the march consumes: piece p of a trajectory with nn nodes (p = 0..nn) is {Re De, Im De, a, length}
+// coefficients the march consumes: piece p of a trajectory with nn nodes (p = 0..nn) is {Re De, Im De, a, |De|^2 - a^2}
 // with De, a the half-step values by linear interpolation and nearest-neighbour extrapolation at both ends
-// (reading R4).  Piece records of trajectory g start at noff[g] + g.
+// (reading R4); its length is l0 (p = 0), l1 (p = nn) or h.  Piece records of trajectory g start at
+// noff[g] + g.  The fourth entry is the energy-independent part of the argument of the T table (sc_math.cuh).
 template <typename R>
 __global__ void rotate_in_kernel(GridDev G, TrajDev T, const double* vx, const double* vy, const double* eta,
                                  double c, int sigma, double2* nd_D, double* nd_a, typename VT<R>::V2* nd_Dr,
-                                 typename VT<R>::V4* pc, int* n_bad) {
+                                 typename VT<R>::V4* pc, float2* pmax, int* n_bad) {
     const int g = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (g >= T.n) return;
     const int lane = threadIdx.x & 31;
@@ -122,14 +127,20 @@ __global__ void rotate_in_kernel(GridDev G, TrajDev T, const double* vx, const d
     }
     __syncwarp();
     typename VT<R>::V4* P = pc + off + g;
+    float wmax = 0.f, amax = 0.f;        // bounds on | |De|^2 - a^2 | and |a| over the trajectory's pieces (rounded up)
     for (int p = lane; p <= nn; p += 32) {
         const int lo = p > 0 ? p - 1 : 0, hi = p < nn ? p : nn - 1;
         const double2 Dl = nd_D[off + lo], Dh = nd_D[off + hi];
         const double al = nd_a[off + lo], ah = nd_a[off + hi];
-        const double len = p == 0 ? T.l0[g] : (p == nn ? T.l1[g] : G.h);
-        P[p] = lo == hi ? mk4((R)Dl.x, (R)Dl.y, (R)al, (R)len)
-                        : mk4((R)(0.5 * (Dl.x + Dh.x)), (R)(0.5 * (Dl.y + Dh.y)), (R)(0.5 * (al + ah)), (R)len);
+        const double dx = lo == hi ? Dl.x : 0.5 * (Dl.x + Dh.x), dy = lo == hi ? Dl.y : 0.5 * (Dl.y + Dh.y);
+        const double am = lo == hi ? al : 0.5 * (al + ah);
+        const typename VT<R>::V4 rec = mk4((R)dx, (R)dy, (R)am, (R)(dx * dx + dy * dy - am * am));
+        P[p] = rec;
+        wmax = fmaxf(wmax, __double2float_ru(fabs((double)rec.w))); amax = fmaxf(amax, __double2float_ru(fabs((double)rec.z)));
     }
+#pragma unroll
+    for (int o = 16; o; o >>= 1) { wmax = fmaxf(wmax, __shfl_xor_sync(0xffffffffu, wmax, o)); amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o)); }
+    if (lane == 0) pmax[g] = make_float2(wmax, amax);
 }
 
 // fallback coefficients for boundary points that have no valid specular partner (R6 fallback):
@@ -169,16 +180,19 @@ struct MarchArgsT {
     EnergyDev E;
     const int* order; int n_items;          // longest-first work list
     const V2* nd_D;                         // node coefficients Delta_j eta_k           [node]
-    const V4* pc;                           // piece coefficients {Re De, Im De, a, len} [node + g]
+    const V4* pc;                           // piece coefficients {Re De, Im De, a, |De|^2 - a^2} [node + g]
+    const float2* pmax;                     // per trajectory: max | |De|^2 - a^2 |, max |a| over its pieces
+    double h;                               // length of every interior piece
     int bc_mode;
     const int* ga_idx; const double* ga_w; const unsigned char* ga_n;   // entry gathers per store row [row][4]
     const double2* fb_D; const double* fb_a;
     const V2* store_old; V2* store_new;
-    char* scr; long long scr_stride;        // per warp slot: scr_stride bytes = (smax+2) rows of 32 entries
+    char* scr; long long scr_stride;        // per warp slot: scr_stride bytes = (smax+2) rows of 32 entries of 4 R
     double* part;                           // MODE 0: [node][6] = SF.re, SF.im, X2.re, X2.im, SG, SI
     double* ldos;                           // MODE 1: [node][ne] = Re g_n
     int* counter;
     double* stat_max2;                      // per warp slot: max |gamma|^2 seen (optional)
+    unsigned long long* n_stored;           // running count of (piece, energy) units marched by rounds that spilled T
 };
 using MarchArgs = MarchArgsT<double>;
 
@@ -187,26 +201,15 @@ constexpr int MARCH_WARPS = 8;               // warps per CTA
 #define SC_MARCH_MIN_CTAS 2
 #endif
 constexpr int MARCH_MIN_CTAS = SC_MARCH_MIN_CTAS;   // resident CTAs per SM the fp64 register budget is sized for
-constexpr int PF_DIST = 12;                  // pass 2: scratch lines are pulled into L2 this many nodes ahead
-#ifndef SC_PF1_DIST
-#define SC_PF1_DIST 0
+#ifndef SC_PF_DIST
+#define SC_PF_DIST 16
 #endif
-constexpr int PF1_DIST = SC_PF1_DIST;        // ... and into L1 this many nodes ahead (0: off); the register look-ahead is one node
+constexpr int PF_DIST = SC_PF_DIST;          // pass 2: scratch lines are pulled into L2 this many nodes ahead
 constexpr int RED_NODES = 4;                 // nodes per shared-memory reduction batch
 constexpr int RED_VALS = 6;
 constexpr int STAGE_LD = 33;                 // padded row of the transpose stage: conflict-free rows AND columns
 
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
-__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
-// 256-bit global accesses (LDG.E.ENL2.256 / STG.E.ENL2.256 on sm_100a): one fp64 scratch entry per lane per instruction
-__device__ __forceinline__ double4 ld256(const double4* p) {
-    double4 v;
-    asm volatile("ld.global.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v.x), "=d"(v.y), "=d"(v.z), "=d"(v.w) : "l"(p));
-    return v;
-}
-__device__ __forceinline__ void st256(double4* p, double a, double b, double c, double d) {
-    asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
-}
 // warp-uniform coefficient record (read-only path)
 __device__ __forceinline__ double4 ldu(const double4* p) {
     double4 v;
@@ -240,18 +243,18 @@ __device__ __forceinline__ R node_products(cplx_t<R> gm, R gtr, R gti, typename 
     const R Pr = mad(gm.re, gtr, -gm.im * gti), Pi = mad(gm.re, gti, gm.im * gtr);
     const R qr = R(1) + Pr;
     const R rq = scm::rcp_nr(mad(qr, qr, Pi * Pi));
-    const R ir = qr * rq, ii = -Pi * rq;               // 1/(1+P)
     if (STATS) max2 = scm::maxr(max2, scm::maxr(mad(gm.re, gm.re, gm.im * gm.im), mad(gtr, gtr, gti * gti)));
     if (MODE == 0) {
-        const R wr = wn * ir, wi = wn * ii;
+        const R wq = wn * rq;
+        const R wr = qr * wq, wi = -Pi * wq;                 // w/(1+P)
         st[0 * STAGE_LD] = mad(gm.re, wr, -gm.im * wi);      // SF  = w gamma/(1+P)
         st[1 * STAGE_LD] = mad(gm.re, wi, gm.im * wr);
         st[2 * STAGE_LD] = mad(gtr, wr, -gti * wi);          // X2  = w gamma~/(1+P)  (SF of k+N/2 = conj)
         st[3 * STAGE_LD] = mad(gtr, wi, gti * wr);
-        st[4 * STAGE_LD] = R(2) * wi;                        // SG  = w Im g = 2 w Im 1/(1+P)
+        st[4 * STAGE_LD] = wi + wi;                          // SG  = w Im g = 2 w Im 1/(1+P)
         st[5 * STAGE_LD] = wn * mad(Dn.x, gm.im - gti, -Dn.y * (gm.re + gtr));   // SI (Eq. 19 :128 numerator)
     }
-    return mad(R(2), ir, R(-1));                             // Re g = 2 Re 1/(1+P) - 1
+    return mad(R(2) * qr, rq, R(-1));                        // Re g = 2 Re 1/(1+P) - 1
 }
 
 // column sums of the stage: lane c < cnt sums row c over the 32 lanes (4 partial sums, fixed order)
@@ -264,47 +267,103 @@ __device__ __forceinline__ double stage_colsum(const R* stage, int lane) {
     return (double)((s0 + s1) + (s2 + s3));
 }
 
-// Scratch entry of one (piece, lane): STEP 0 (closed form) {T.re, T.im, gt.re, gt.im} = 4 R, one 256-bit (fp64) or
-// 128-bit (fp32) access; STEP 1 (mid-point) {gt.re, gt.im} = 2 R.  A warp's 32 entries of a piece are contiguous.
+// Scratch between the two passes, one entry per (piece or node, lane), a warp's 32 entries contiguous.
+//   ST = false ("recompute"): entry m = gamma~(node m) = 2 R.  T is NOT spilled: re-evaluating it from the table in
+//        pass 2 costs 18 FP64 instructions against 32 B of HBM traffic (~70 instruction slots at the machine balance).
+//        Chosen per (trajectory, 32-energy round) when every piece is inside the table's radius (bound from pmax).
+//   ST = true  ("stored"):    entry p = {T_p, gamma~(node p-1)} = 4 R, one 256-bit (fp64) / 128-bit (fp32) access:
+//        T is evaluated once per piece, from the table where a warp vote allows, from exp/sqrt elsewhere.
+//   STEP 1 (mid-point) has no T: always the 2 R layout.
 template <typename R> struct Ent { R tr, ti, gr, gi; };
-template <typename R, int STEP> struct ScrT {
-    static constexpr int BYTES = (STEP == 0 ? 4 : 2) * (int)sizeof(R); static constexpr int ROW = 32 * BYTES;
-};
-template <int STEP>
+template <typename R, bool ST> struct ScrT { static constexpr int BYTES = (ST ? 4 : 2) * (int)sizeof(R); static constexpr int ROW = 32 * BYTES; };
+template <bool ST>
 __device__ __forceinline__ Ent<double> ld_ent(const char* p, double) {
     Ent<double> e;
-    if (STEP == 0) { const double4 v = ld256((const double4*)p); e.tr = v.x; e.ti = v.y; e.gr = v.z; e.gi = v.w; }
-    else {
-        asm volatile("ld.global.v2.f64 {%0,%1}, [%2];" : "=d"(e.gr), "=d"(e.gi) : "l"(p));
-        e.tr = e.ti = 0.0;
-    }
+    if (ST) asm volatile("ld.global.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(e.tr), "=d"(e.ti), "=d"(e.gr), "=d"(e.gi) : "l"(p));
+    else { asm volatile("ld.global.v2.f64 {%0,%1}, [%2];" : "=d"(e.gr), "=d"(e.gi) : "l"(p)); e.tr = e.ti = 0.0; }
     return e;
 }
-template <int STEP>
+template <bool ST>
 __device__ __forceinline__ Ent<float> ld_ent(const char* p, float) {
     Ent<float> e;
-    if (STEP == 0) asm volatile("ld.global.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(e.tr), "=f"(e.ti), "=f"(e.gr), "=f"(e.gi) : "l"(p));
-    else {
-        asm volatile("ld.global.v2.f32 {%0,%1}, [%2];" : "=f"(e.gr), "=f"(e.gi) : "l"(p));
-        e.tr = e.ti = 0.f;
-    }
+    if (ST) asm volatile("ld.global.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(e.tr), "=f"(e.ti), "=f"(e.gr), "=f"(e.gi) : "l"(p));
+    else { asm volatile("ld.global.v2.f32 {%0,%1}, [%2];" : "=f"(e.gr), "=f"(e.gi) : "l"(p)); e.tr = e.ti = 0.f; }
     return e;
 }
-template <int STEP>
+template <bool ST>
 __device__ __forceinline__ void st_ent(char* p, cplx T, cplx gt) {
-    if (STEP == 0) st256((double4*)p, T.re, T.im, gt.re, gt.im);
+    if (ST) asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(T.re), "d"(T.im), "d"(gt.re), "d"(gt.im) : "memory");
     else asm volatile("st.global.v2.f64 [%0], {%1,%2};" ::"l"(p), "d"(gt.re), "d"(gt.im) : "memory");
 }
-template <int STEP>
+template <bool ST>
 __device__ __forceinline__ void st_ent(char* p, cplxf T, cplxf gt) {
-    if (STEP == 0) asm volatile("st.global.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(p), "f"(T.re), "f"(T.im), "f"(gt.re), "f"(gt.im) : "memory");
+    if (ST) asm volatile("st.global.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(p), "f"(T.re), "f"(T.im), "f"(gt.re), "f"(gt.im) : "memory");
     else asm volatile("st.global.v2.f32 [%0], {%1,%2};" ::"l"(p), "f"(gt.re), "f"(gt.im) : "memory");
 }
-// one step of gamma with piece record cc; STEP 0 re-uses the stored T of the piece
-template <int STEP, typename R>
-__device__ __forceinline__ cplx_t<R> step_up(cplx_t<R> g, const typename VT<R>::V4& cc, R zr0, R zi0, const Ent<R>& E) {
-    if (STEP == 0) return scm::step_T(g, cc.x, cc.y, zr0 + cc.z, zi0, mk(E.tr, E.ti));
-    return scm::step_mid(g, cc.x, cc.y, zr0 + cc.z, zi0, cc.w);
+
+// Per-lane Taylor table of T about this lane's energy (TM 1: real coefficients, 2: complex) and its evaluation for
+// one piece record.
+template <typename R, int TM>
+struct TTab {
+    static constexpr int K = scm::TaylorK<R>::K;
+    R cr[K + 1]; R ci[TM == 2 ? K + 1 : 1];
+    R thr2, m2zr, m2zi;
+    __device__ __forceinline__ void load(const EnergyDev& E, int n) {
+        const double* row = E.tc + (size_t)n * TC_LD;
+#pragma unroll
+        for (int k = 0; k <= K; ++k) { cr[k] = (R)row[k]; if (TM == 2) ci[k] = (R)row[TC_KMAX + 1 + k]; }
+        if (TM != 2) ci[0] = R(0);
+        thr2 = (R)(row[2 * (TC_KMAX + 1)] * (scm::TaylorK<R>::RMAX * scm::TaylorK<R>::RMAX));
+        m2zr = (R)(-2.0 * E.zr[n]); m2zi = (R)(-2.0 * E.zi[n]);
+    }
+    // every piece of a trajectory with the bounds pm is inside the radius of energy n (conservative; 1e-3 covers rounding)
+    static __device__ __forceinline__ bool covers(const EnergyDev& E, int n, float2 pm) {
+        const R thr = (R)(E.tc[(size_t)n * TC_LD + 2 * (TC_KMAX + 1)] * (scm::TaylorK<R>::RMAX * scm::TaylorK<R>::RMAX));
+        const R br = (R)pm.x + (R)(2.0 * fabs(E.zr[n])) * (R)pm.y, bi = (R)(2.0 * E.zi[n]) * (R)pm.y;
+        return scm::mad(br, br, bi * bi) * R(1.001) <= thr;
+    }
+    // dw = (|De|^2 - a^2) - 2 z0 a
+    __device__ __forceinline__ cplx_t<R> taylor(const typename VT<R>::V4& cc, R dwr, R dwi, R s2) const {
+        if constexpr (TM == 2) return scm::taylor_cplx<R, K>(cr, ci, dwr, dwi);
+        else return scm::taylor_real<R, K>(cr, dwr, dwi, s2);
+    }
+    // known to be inside the radius
+    __device__ __forceinline__ cplx_t<R> fast(const typename VT<R>::V4& cc) const {
+        const R dwr = TM == 2 ? scm::mad(m2zr, cc.z, cc.w) : cc.w, dwi = m2zi * cc.z;
+        return taylor(cc, dwr, dwi, scm::mad(dwr, dwr, dwi * dwi));
+    }
+    // one warp vote per piece: table inside the radius, exp-based evaluation outside
+    __device__ __forceinline__ cplx_t<R> voted(const typename VT<R>::V4& cc, R zr0, R zi0, R len) const {
+        const R dwr = TM == 2 ? scm::mad(m2zr, cc.z, cc.w) : cc.w, dwi = m2zi * cc.z;
+        const R s2 = scm::mad(dwr, dwr, dwi * dwi);
+        if (!__any_sync(0xffffffffu, !(s2 <= thr2))) return taylor(cc, dwr, dwi, s2);
+        return scm::coef_T_slow(scm::mad(cc.x, cc.x, cc.y * cc.y), zr0 + cc.z, zi0, len);
+    }
+};
+// Pole-subtracted table (energies on the imaginary axis), for the rounds that spill T: three times the radius.
+template <typename R>
+struct TTabPole {
+    static constexpr int K = scm::TaylorPoleK<R>::K;
+    R c[K + 1]; R thr2, pole_a, pole_res, m2zi;
+    __device__ __forceinline__ void load(const EnergyDev& E, int n) {
+        const double* row = E.tcp + (size_t)n * TCP_LD;
+#pragma unroll
+        for (int k = 0; k <= K; ++k) c[k] = (R)row[k];
+        thr2 = (R)(row[9] * (scm::TaylorPoleK<R>::RMAX * scm::TaylorPoleK<R>::RMAX));
+        pole_a = (R)row[10]; pole_res = (R)row[11]; m2zi = (R)(-2.0 * E.zi[n]);
+    }
+    __device__ __forceinline__ cplx_t<R> fast(const typename VT<R>::V4& cc) const { return mk(R(0), R(0)); }   // unused
+    __device__ __forceinline__ cplx_t<R> voted(const typename VT<R>::V4& cc, R zr0, R zi0, R len) const {
+        const R dwr = cc.w, dwi = m2zi * cc.z;
+        const R s2 = scm::mad(dwr, dwr, dwi * dwi);
+        if (!__any_sync(0xffffffffu, !(s2 <= thr2))) return scm::taylor_pole<R, K>(c, pole_a, pole_res, dwr, dwi, s2);
+        return scm::coef_T_slow(scm::mad(cc.x, cc.x, cc.y * cc.y), zr0 + cc.z, zi0, len);
+    }
+};
+// T of an end piece (length != h): exp-based
+template <typename R>
+__device__ __forceinline__ cplx_t<R> end_T(const typename VT<R>::V4& cc, R zr0, R zi0, R len) {
+    return scm::coef_T_slow(scm::mad(cc.x, cc.x, cc.y * cc.y), zr0 + cc.z, zi0, len);
 }
 
 // ---- coefficient staging: the warp-uniform piece / node records of a trajectory are streamed through shared
@@ -330,213 +389,263 @@ __device__ __forceinline__ void cp_async(void* smem, const void* gmem) {
 __device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
+// state of one warp while it works on one trajectory
+template <typename R>
+struct WarpJob {
+    using V2 = typename VT<R>::V2; using V4 = typename VT<R>::V4;
+    int lane, nn, dF, dB, ne; long long noff;
+    R len0, len1, hlen;
+    const V2* ND; const V4* PC; double* PART;
+    R* stage; V4* pcb; V2* ndb;
+    char* scr_w;                             // this warp slot's scratch
+};
+
+// One 32-energy round of one trajectory: pass 1 (gamma-tilde from u_out down to u_in, spilled per node), pass 2
+// (gamma from u_in up to u_out, node products, reduction over the 32 energies).
 // MODE 0: Matsubara sums; 1: per-energy Re g (LDOS); 2: boundary values only.
 // STEP 0: closed-form step; 1: implicit mid-point rule (C4-C9 :984-1001).
-template <int MODE, bool STATS, int STEP, typename R>
+// ST: T spilled with gamma-tilde (see ScrT).  TM: layout of the T table.
+template <int MODE, bool STATS, int STEP, typename R, bool ST, typename TAB>
+__device__ __forceinline__ void march_round(const MarchArgsT<R>& A, const WarpJob<R>& J, const TAB& tab, int n0, R& max2) {
+    using V2 = typename VT<R>::V2; using V4 = typename VT<R>::V4;
+    constexpr int ROW = ScrT<R, ST>::ROW, BYTES = ScrT<R, ST>::BYTES;
+    constexpr int NB = ST ? 1 : 0;                          // ST: node m lives in entry m+1 (entry p = piece p)
+    const int lane = J.lane, nn = J.nn, ne = J.ne;
+    char* const scr = J.scr_w + lane * BYTES;               // entry e of this lane: scr + e*ROW
+    const bool pf_lane = lane * 128 < RED_NODES * ROW;      // lanes that cover 4 rows in 128-byte lines
+    const bool act = n0 + lane < ne;
+    const int n = act ? n0 + lane : ne - 1;
+    const R zr0 = (R)A.E.zr[n], zi0 = (R)A.E.zi[n];
+    const R wn = act ? (R)A.E.w[n] : R(0);
+    const int nb = A.E.partner[n];
+    const V4* __restrict__ PC = J.PC; const V2* __restrict__ ND = J.ND;
+    V4* const pcb = J.pcb; V2* const ndb = J.ndb;
+    const int npart = nn * RED_VALS;
+
+    // T of piece cc and the step across it
+    auto coefT = [&](const V4& cc, bool interior, R len) -> cplx_t<R> {
+        if (STEP != 0) return mk(R(0), R(0));
+        if (!interior) return end_T<R>(cc, zr0, zi0, len);
+        if (ST) return tab.voted(cc, zr0, zi0, len);
+        return tab.fast(cc);
+    };
+    auto stepT = [&](cplx_t<R> g, R sgn, const V4& cc, cplx_t<R> T, R len) -> cplx_t<R> {
+        if (STEP == 0) return scm::step_T(g, sgn * cc.x, cc.y, zr0 + cc.z, zi0, T);
+        return scm::step_mid(g, sgn * cc.x, cc.y, zr0 + cc.z, zi0, len);
+    };
+
+    // ---------------- pass 1: gamma-tilde from u_out down to u_in ----------------
+    const int ctop = nn >> 5;                                  // chunk c holds pieces 32c .. 32c+31
+    if (ctop * CHUNK + lane <= nn) cp_async<sizeof(V4)>(pcb + (ctop & 1) * CHUNK + lane, PC + ctop * CHUNK + lane);
+    cp_commit();
+    cplx_t<R> gt;
+    if (A.bc_mode == 1) {
+        const V4 c4 = ldu(PC + nn);
+        gt = hom_start<R>(-(double)c4.x, c4.y, A.E.zr[n] + c4.z, A.E.zi[n]);
+    } else if (A.ga_n[J.dB]) {
+        const cplx_t<R> s = gather_start(A, J.dB, nb);            // gamma of the mirrored trajectory at its entry
+        gt = mk(s.re, -s.im);
+    } else {
+        const cplx_t<R> s = hom_start<R>(A.fb_D[J.dB].x, A.fb_D[J.dB].y, A.E.zr[nb] + A.fb_a[J.dB], A.E.zi[nb]);
+        gt = mk(s.re, -s.im);
+    }
+    cplx_t<R> T0 = mk(R(0), R(0));                             // T of the entry piece, kept for pass 2 when not spilled
+    {
+        // the step across piece p lands on node p-1: entry p (ST) or entry p-1 (gamma~ only)
+        char* e = scr + (size_t)(nn - 1 + NB) * ROW;
+        int p = nn;
+        for (int c = ctop; c >= 0; --c) {
+            if (c > 0) {
+                cp_async<sizeof(V4)>(pcb + ((c - 1) & 1) * CHUNK + lane, PC + (c - 1) * CHUNK + lane);
+                cp_commit();
+                cp_wait<1>();
+            } else {
+                cp_wait<0>();
+            }
+            __syncwarp();
+            const V4* __restrict__ buf = pcb + (c & 1) * CHUNK;
+            const int plo = max(c * CHUNK, 1);
+            if (p == nn) {                                      // exit piece (length l1)
+                const V4 cc = buf[p & (CHUNK - 1)];
+                const cplx_t<R> T = coefT(cc, false, J.len1);
+                gt = stepT(gt, R(-1), cc, T, J.len1);
+                if (MODE != 2 || ST) st_ent<ST>(e, T, gt);
+                e -= ROW; --p;
+            }
+#pragma unroll 2
+            for (; p >= plo; --p) {
+                const V4 cc = buf[p & (CHUNK - 1)];
+                const cplx_t<R> T = coefT(cc, true, J.hlen);
+                gt = stepT(gt, R(-1), cc, T, J.hlen);
+                if (MODE != 2 || ST) st_ent<ST>(e, T, gt);
+                e -= ROW;
+            }
+            if (c == 0) {                                       // entry piece (length l0); its gamma~ is the end value
+                const V4 cc = buf[0];
+                T0 = coefT(cc, false, J.len0);
+                gt = stepT(gt, R(-1), cc, T0, J.len0);
+            }
+            __syncwarp();                                       // chunk c is free for the load issued next round
+        }
+        if (act) A.store_new[(size_t)J.dB * ne + nb] = mk2(gt.re, -gt.im);
+    }
+
+    // ---------------- pass 2: gamma from u_in up to u_out; products and energy reduction ------------
+    // chunk c of pass 2 holds, for nodes m = 32c .. 32c+31, the piece m+1 (the step that leaves the node) and Delta_m
+    const int nchunk = (nn + CHUNK - 1) >> 5;
+    cplx_t<R> gm;
+    {
+        const V4 c0 = pcb[0];                                   // piece 0 is still in buffer 0 (last chunk of pass 1)
+        __syncwarp();
+        if (lane < nn) {
+            cp_async<sizeof(V4)>(pcb + CHUNK + lane, PC + 1 + lane);      // pass-2 chunk 0 goes to buffer 1
+            cp_async<sizeof(V2)>(ndb + CHUNK + lane, ND + lane);
+        }
+        cp_commit();
+        if (A.bc_mode == 1) gm = hom_start<R>(c0.x, c0.y, A.E.zr[n] + c0.z, A.E.zi[n]);
+        else if (A.ga_n[J.dF]) gm = gather_start(A, J.dF, n);
+        else gm = hom_start<R>(A.fb_D[J.dF].x, A.fb_D[J.dF].y, A.E.zr[n] + A.fb_a[J.dF], A.E.zi[n]);
+        gm = stepT(gm, R(1), c0, T0, J.len0);
+    }
+    constexpr bool LD = ST || MODE != 2;        // pass 2 reads the scratch (burn-in sweeps without spilled T do not)
+    const char* e = scr + NB * ROW;             // entry of node 0
+    if (LD)
+        for (int q = RED_NODES; q < PF_DIST && q < nn; q += RED_NODES)
+            if (pf_lane) prefetch_l2(J.scr_w + (size_t)(q + NB) * ROW + lane * 128);
+    Ent<R> En{};
+    if (LD) En = ld_ent<ST>(e, R(0));
+    double part_nxt = 0.0;                       // running sums of the earlier energy rounds, fetched one batch ahead
+    if (MODE == 0 && n0 && lane < RED_NODES * RED_VALS && lane < npart) part_nxt = J.PART[lane];
+    int m = 0;
+    // node m: products with gamma~(m) from its entry, then the step across piece m+1 (T from entry m+1 when spilled)
+    auto node = [&](int b, const V4* pbuf, const V2* dbuf, bool exitp) {
+        const Ent<R> Ec = En;
+        const V4 cc = pbuf[(m + b) & (CHUNK - 1)]; const V2 dc = dbuf[(m + b) & (CHUNK - 1)];
+        if (LD) En = ld_ent<ST>(e + (b + 1) * ROW, R(0));          // one entry ahead (the scratch has 2 spare rows)
+        if (MODE != 2) {
+            const R rg = node_products<MODE, STATS, R>(gm, Ec.gr, Ec.gi, dc, wn, J.stage + b * RED_VALS * STAGE_LD + lane, max2);
+            if (MODE == 1 && act) A.ldos[(size_t)(J.noff + m + b) * ne + n] = (double)rg;
+        }
+        const R len = exitp ? J.len1 : J.hlen;
+        // ST: the entry of node m+b is the entry of piece m+b+1, the step that leaves the node: it holds that T
+        const cplx_t<R> T = ST ? mk(Ec.tr, Ec.ti) : coefT(cc, !exitp, len);
+        gm = stepT(gm, R(1), cc, T, len);
+    };
+    for (int c = 0; c < nchunk; ++c) {
+        const int bsel = (c + 1) & 1;                           // chunk c lives in buffer (c+1)&1
+        if (c + 1 < nchunk) {
+            const int q = (c + 1) * CHUNK + lane;
+            if (q < nn) {
+                cp_async<sizeof(V4)>(pcb + (bsel ^ 1) * CHUNK + lane, PC + 1 + q);
+                cp_async<sizeof(V2)>(ndb + (bsel ^ 1) * CHUNK + lane, ND + q);
+            }
+            cp_commit();
+            cp_wait<1>();
+        } else {
+            cp_wait<0>();
+        }
+        __syncwarp();
+        const V4* __restrict__ pbuf = pcb + bsel * CHUNK;
+        const V2* __restrict__ dbuf = ndb + bsel * CHUNK;
+        const int mhi = min(nn, (c + 1) * CHUNK);
+        for (; m + RED_NODES <= mhi; m += RED_NODES) {
+            if (LD && pf_lane && m + PF_DIST < nn) prefetch_l2(J.scr_w + (size_t)(m + PF_DIST + NB) * ROW + lane * 128);
+            const double part_old = part_nxt;
+            if (MODE == 0 && n0 && lane < RED_NODES * RED_VALS && (m + RED_NODES) * RED_VALS + lane < npart)
+                part_nxt = J.PART[(m + RED_NODES) * RED_VALS + lane];
+            if (m + RED_NODES < nn) {
+#pragma unroll
+                for (int b = 0; b < RED_NODES; ++b) node(b, pbuf, dbuf, false);
+            } else {                                             // the batch ends on the trajectory's last node
+#pragma unroll
+                for (int b = 0; b < RED_NODES; ++b) node(b, pbuf, dbuf, b == RED_NODES - 1);
+            }
+            e += RED_NODES * ROW;
+            if (MODE == 0) {
+                __syncwarp();
+                if (lane < RED_NODES * RED_VALS) {
+                    double s = stage_colsum(J.stage, lane);
+                    if (n0) s += part_old;
+                    J.PART[m * RED_VALS + lane] = s;
+                }
+                __syncwarp();
+            }
+        }
+        if (m < mhi) {                                       // ragged tail: 1..3 nodes (last chunk only)
+            const int rem = mhi - m;
+            const double part_old = part_nxt;
+            for (int b = 0; b < rem; ++b) node(b, pbuf, dbuf, m + b + 1 == nn);
+            if (MODE == 0) {
+                __syncwarp();
+                if (lane < rem * RED_VALS) {
+                    double s = stage_colsum(J.stage, lane);
+                    if (n0) s += part_old;
+                    J.PART[m * RED_VALS + lane] = s;
+                }
+                __syncwarp();
+            }
+            m = mhi;
+        }
+        __syncwarp();                                           // this chunk's buffer is free for the next load
+    }
+    if (act) A.store_new[(size_t)J.dF * ne + n] = mk2(gm.re, gm.im);
+}
+
+template <int MODE, bool STATS, int STEP, typename R, int TM>
 __global__ void __launch_bounds__(MARCH_WARPS * 32, MARCH_MIN_CTAS) march_kernel(MarchArgsT<R> A) {
     using V2 = typename VT<R>::V2; using V4 = typename VT<R>::V4;
     extern __shared__ double4 smem_raw[];
-    constexpr int ROW = ScrT<R, STEP>::ROW, BYTES = ScrT<R, STEP>::BYTES;
-    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-    const int slot = blockIdx.x * MARCH_WARPS + wib;
+    WarpJob<R> J;
+    J.lane = threadIdx.x & 31;
+    const int wib = threadIdx.x >> 5, slot = blockIdx.x * MARCH_WARPS + wib;
     char* const smem_w = reinterpret_cast<char*>(smem_raw) + wib * (march_stage_bytes<R>() + march_coef_bytes<R>());
-    R* const stage = reinterpret_cast<R*>(smem_w);                                        // [4 nodes][6 values][33]
-    V4* const pcb = reinterpret_cast<V4*>(smem_w + march_stage_bytes<R>());               // [2][CHUNK] piece records
-    V2* const ndb = reinterpret_cast<V2*>(pcb + 2 * CHUNK);                               // [2][CHUNK] node Delta
-    char* const scr = A.scr + (size_t)slot * A.scr_stride + lane * BYTES;   // entry e of this lane: scr + e*ROW
-    const int ne = A.E.ne;
+    J.stage = reinterpret_cast<R*>(smem_w);                                        // [4 nodes][6 values][33]
+    J.pcb = reinterpret_cast<V4*>(smem_w + march_stage_bytes<R>());               // [2][CHUNK] piece records
+    J.ndb = reinterpret_cast<V2*>(J.pcb + 2 * CHUNK);                             // [2][CHUNK] node Delta
+    J.scr_w = A.scr + (size_t)slot * A.scr_stride;
+    J.ne = A.E.ne; J.hlen = (R)A.h;
     R max2 = R(0);
+    unsigned long long nst = 0;
 
     for (;;) {
         int item = 0;
-        if (lane == 0) item = atomicAdd(A.counter, 1);
+        if (J.lane == 0) item = atomicAdd(A.counter, 1);
         item = __shfl_sync(0xffffffffu, item, 0);
         if (item >= A.n_items) break;
         const int g = A.order[item];
-        const int nn = A.T.nn[g];
-        const long long noff = A.T.noff[g];
-        const int dF = A.T.dF[g], dB = A.T.dB[g];
-        const V2* __restrict__ ND = A.nd_D + noff;
-        const V4* __restrict__ PC = A.pc + noff + g;
-        double* __restrict__ const PART = A.part + (size_t)noff * RED_VALS;
-        const int npart = nn * RED_VALS;
+        J.nn = A.T.nn[g]; J.noff = A.T.noff[g];
+        J.dF = A.T.dF[g]; J.dB = A.T.dB[g];
+        J.len0 = (R)A.T.l0[g]; J.len1 = (R)A.T.l1[g];
+        J.ND = A.nd_D + J.noff; J.PC = A.pc + J.noff + g;
+        J.PART = A.part + (size_t)J.noff * RED_VALS;
+        const float2 pm = A.pmax[g];
 
-        for (int n0 = 0; n0 < ne; n0 += 32) {
-            const bool act = n0 + lane < ne;
-            const int n = act ? n0 + lane : ne - 1;
-            const R zr0 = (R)A.E.zr[n], zi0 = (R)A.E.zi[n];
-            const R wn = act ? (R)A.E.w[n] : R(0);
-            const int nb = A.E.partner[n];
-            // Taylor table of T about this lane's energy (interior pieces all have length h)
-            constexpr int KT = scm::TaylorK<R>::K;
-            const bool tay = STEP == 0 && A.E.tc != nullptr;
-            R tcf[KT + 1]; R thr2 = R(-1), pole_a = R(1), pole_res = R(0);
-            if (tay) {
-#pragma unroll
-                for (int k = 0; k <= KT; ++k) tcf[k] = (R)A.E.tc[(size_t)n * TC_LD + k];
-                thr2 = (R)(A.E.tc[(size_t)n * TC_LD + 9] * scm::TaylorK<R>::RMAX2);
-                pole_a = (R)A.E.tc[(size_t)n * TC_LD + 10]; pole_res = (R)A.E.tc[(size_t)n * TC_LD + 11];
-            }
-            const R m2zi = R(-2) * zi0;
-
-            // ---------------- pass 1: gamma-tilde from u_out down to u_in; entry p = {T_p, gamma~(node p-1)} ----------
-            const int ctop = nn >> 5;                                  // chunk c holds pieces 32c .. 32c+31
-            if (ctop * CHUNK + lane <= nn) cp_async<sizeof(V4)>(pcb + (ctop & 1) * CHUNK + lane, PC + ctop * CHUNK + lane);
-            cp_commit();
-            cplx_t<R> gt;
-            if (A.bc_mode == 1) {
-                const V4 c4 = ldu(PC + nn);
-                gt = hom_start<R>(-(double)c4.x, c4.y, A.E.zr[n] + c4.z, A.E.zi[n]);
-            } else if (A.ga_n[dB]) {
-                const cplx_t<R> s = gather_start(A, dB, nb);            // gamma of the mirrored trajectory at its entry
-                gt = mk(s.re, -s.im);
-            } else {
-                const cplx_t<R> s = hom_start<R>(A.fb_D[dB].x, A.fb_D[dB].y, A.E.zr[nb] + A.fb_a[dB], A.E.zi[nb]);
-                gt = mk(s.re, -s.im);
-            }
-            {
-                char* e = scr + (size_t)nn * ROW;
-                int p = nn;
-                for (int c = ctop; c >= 0; --c) {
-                    if (c > 0) {
-                        cp_async<sizeof(V4)>(pcb + ((c - 1) & 1) * CHUNK + lane, PC + (c - 1) * CHUNK + lane);
-                        cp_commit();
-                        cp_wait<1>();
-                    } else {
-                        cp_wait<0>();
-                    }
-                    __syncwarp();
-                    const V4* __restrict__ buf = pcb + (c & 1) * CHUNK;
-                    const int plo = c * CHUNK;
-#pragma unroll 2
-                    for (; p >= plo; --p) {
-                        const V4 cc = buf[p & (CHUNK - 1)];
-                        const R zr = zr0 + cc.z;
-                        cplx_t<R> T = mk(R(0), R(0));
-                        if (STEP == 0) {
-                            const R d2 = scm::mad(cc.x, cc.x, cc.y * cc.y);
-                            // w = |De|^2 - z^2 = zi0^2 + dw,  dw = (|De|^2 - a^2) - 2 i zi0 a   (z = i zi0 + a)
-                            const R dwr = scm::mad(-cc.z, cc.z, d2), dwi = m2zi * cc.z;
-                            const R s2 = scm::mad(dwr, dwr, dwi * dwi);
-                            const bool interior = p > 0 && p < nn;
-                            if (interior && !__any_sync(0xffffffffu, !(s2 <= thr2))) T = scm::taylor_T<R, KT>(tcf, pole_a, pole_res, dwr, dwi, s2);
-                            else T = scm::coef_T_slow(d2, zr, zi0, cc.w);
-                            gt = scm::step_T(gt, -cc.x, cc.y, zr, zi0, T);
-                        } else {
-                            gt = scm::step_mid(gt, -cc.x, cc.y, zr, zi0, cc.w);
-                        }
-                        st_ent<STEP>(e, T, gt);
-                        e -= ROW;
-                    }
-                    __syncwarp();                                       // chunk c is free for the load issued next round
-                }
-                if (act) A.store_new[(size_t)dB * ne + nb] = mk2(gt.re, -gt.im);
-            }
-
-            // ---------------- pass 2: gamma from u_in up to u_out; products and energy reduction ------------
-            // chunk c of pass 2 holds, for nodes m = 32c .. 32c+31, the piece m+1 (the step that leaves the node) and Delta_m
-            const int nchunk = (nn + CHUNK - 1) >> 5;
-            cplx_t<R> gm;
-            {
-                const V4 c0 = pcb[0];                                   // piece 0 is still in buffer 0 (last chunk of pass 1)
-                __syncwarp();
-                if (lane < nn) {
-                    cp_async<sizeof(V4)>(pcb + CHUNK + lane, PC + 1 + lane);      // pass-2 chunk 0 goes to buffer 1
-                    cp_async<sizeof(V2)>(ndb + CHUNK + lane, ND + lane);
-                }
-                cp_commit();
-                if (A.bc_mode == 1) gm = hom_start<R>(c0.x, c0.y, A.E.zr[n] + c0.z, A.E.zi[n]);
-                else if (A.ga_n[dF]) gm = gather_start(A, dF, n);
-                else gm = hom_start<R>(A.fb_D[dF].x, A.fb_D[dF].y, A.E.zr[n] + A.fb_a[dF], A.E.zi[n]);
-                const Ent<R> e0 = ld_ent<STEP>(scr, R(0));
-                gm = step_up<STEP, R>(gm, c0, zr0, zi0, e0);
-            }
-            const char* e = scr + ROW;                  // entry of node 0
-            for (int q = 4; q < PF_DIST && q < nn; q += 4) prefetch_l2(e - lane * BYTES + (size_t)q * ROW + lane * 128);
-            Ent<R> En = ld_ent<STEP>(e, R(0));
-            double part_nxt = 0.0;                       // running sums of the earlier energy rounds, fetched one batch ahead
-            if (MODE == 0 && n0 && lane < RED_NODES * RED_VALS && lane < npart) part_nxt = PART[lane];
-            int m = 0;
-            for (int c = 0; c < nchunk; ++c) {
-                const int bsel = (c + 1) & 1;                           // chunk c lives in buffer (c+1)&1
-                if (c + 1 < nchunk) {
-                    const int q = (c + 1) * CHUNK + lane;
-                    if (q < nn) {
-                        cp_async<sizeof(V4)>(pcb + (bsel ^ 1) * CHUNK + lane, PC + 1 + q);
-                        cp_async<sizeof(V2)>(ndb + (bsel ^ 1) * CHUNK + lane, ND + q);
-                    }
-                    cp_commit();
-                    cp_wait<1>();
+        for (int n0 = 0; n0 < J.ne; n0 += 32) {
+            const int n = min(n0 + J.lane, J.ne - 1);
+            // STEP 0: T is re-evaluated in pass 2 if every piece is inside the table's radius for all 32 lanes, else spilled
+            if (STEP == 0 && __any_sync(0xffffffffu, !TTab<R, TM>::covers(A.E, n, pm))) {
+                if constexpr (TM == 1) {
+                    TTabPole<R> tab; tab.load(A.E, n);
+                    march_round<MODE, STATS, STEP, R, true>(A, J, tab, n0, max2);
                 } else {
-                    cp_wait<0>();
+                    TTab<R, TM> tab; tab.load(A.E, n);
+                    march_round<MODE, STATS, STEP, R, true>(A, J, tab, n0, max2);
                 }
-                __syncwarp();
-                const V4* __restrict__ pbuf = pcb + bsel * CHUNK;
-                const V2* __restrict__ dbuf = ndb + bsel * CHUNK;
-                const int mhi = min(nn, (c + 1) * CHUNK);
-                for (; m + RED_NODES <= mhi; m += RED_NODES) {
-                    if (m + PF_DIST < nn) prefetch_l2(e - lane * BYTES + (size_t)PF_DIST * ROW + lane * 128);
-                    if (PF1_DIST && m + PF1_DIST < nn) prefetch_l1(e - lane * BYTES + (size_t)PF1_DIST * ROW + lane * 128);
-                    const double part_old = part_nxt;
-                    if (MODE == 0 && n0 && lane < RED_NODES * RED_VALS && (m + RED_NODES) * RED_VALS + lane < npart)
-                        part_nxt = PART[(m + RED_NODES) * RED_VALS + lane];
-#pragma unroll
-                    for (int b = 0; b < RED_NODES; ++b) {
-                        const Ent<R> Ec = En;
-                        const V4 cc = pbuf[(m + b) & (CHUNK - 1)]; const V2 dc = dbuf[(m + b) & (CHUNK - 1)];
-                        En = ld_ent<STEP>(e + (b + 1) * ROW, R(0));          // one node ahead (scratch has 2 spare entries)
-                        if (MODE != 2) {
-                            const R rg = node_products<MODE, STATS, R>(gm, Ec.gr, Ec.gi, dc, wn, stage + b * RED_VALS * STAGE_LD + lane, max2);
-                            if (MODE == 1 && act) A.ldos[(size_t)(noff + m + b) * ne + n] = (double)rg;
-                        }
-                        gm = step_up<STEP, R>(gm, cc, zr0, zi0, Ec);
-                    }
-                    e += RED_NODES * ROW;
-                    if (MODE == 0) {
-                        __syncwarp();
-                        if (lane < RED_NODES * RED_VALS) {
-                            double s = stage_colsum(stage, lane);
-                            if (n0) s += part_old;
-                            PART[m * RED_VALS + lane] = s;
-                        }
-                        __syncwarp();
-                    }
-                }
-                if (m < mhi) {                                       // ragged tail: 1..3 nodes (last chunk only)
-                    const int rem = mhi - m;
-                    const double part_old = part_nxt;
-                    for (int b = 0; b < rem; ++b) {
-                        const Ent<R> Ec = En;
-                        const V4 cc = pbuf[(m + b) & (CHUNK - 1)]; const V2 dc = dbuf[(m + b) & (CHUNK - 1)];
-                        En = ld_ent<STEP>(e + (b + 1) * ROW, R(0));
-                        if (MODE != 2) {
-                            const R rg = node_products<MODE, STATS, R>(gm, Ec.gr, Ec.gi, dc, wn, stage + b * RED_VALS * STAGE_LD + lane, max2);
-                            if (MODE == 1 && act) A.ldos[(size_t)(noff + m + b) * ne + n] = (double)rg;
-                        }
-                        gm = step_up<STEP, R>(gm, cc, zr0, zi0, Ec);
-                    }
-                    if (MODE == 0) {
-                        __syncwarp();
-                        if (lane < rem * RED_VALS) {
-                            double s = stage_colsum(stage, lane);
-                            if (n0) s += part_old;
-                            PART[m * RED_VALS + lane] = s;
-                        }
-                        __syncwarp();
-                    }
-                    m = mhi;
-                }
-                __syncwarp();                                           // this chunk's buffer is free for the next load
+                nst += (unsigned long long)(J.nn + 1) * min(32, J.ne - n0);
+            } else {
+                TTab<R, TM> tab;
+                if (STEP == 0) tab.load(A.E, n);
+                march_round<MODE, STATS, STEP, R, false>(A, J, tab, n0, max2);
             }
-            if (act) A.store_new[(size_t)dF * ne + n] = mk2(gm.re, gm.im);
         }
     }
     if (STATS) {
         double mx = (double)max2;
 #pragma unroll
         for (int o = 16; o; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-        if (lane == 0) A.stat_max2[slot] = mx;
+        if (J.lane == 0) A.stat_max2[slot] = mx;
     }
+    if (J.lane == 0 && nst) atomicAdd(A.n_stored, nst);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -697,50 +806,42 @@ __global__ void rotate_back_ldos_kernel(BackLdosArgs L) {
 // debug / measurement kernels
 // ------------------------------------------------------------------------------------------------
 // re-march one trajectory for one energy with the same device functions; writes gamma, gamma-tilde per node
-template <typename R>
-__global__ void debug_traj_kernel(MarchArgsT<R> A, int stepper, int g, int n, double2* outG, double2* outGT) {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+template <typename R, int TM>
+__device__ void debug_traj_body(const MarchArgsT<R>& A, int stepper, int g, int n, double2* outG, double2* outGT) {
     using V4 = typename VT<R>::V4;
     const int nn = A.T.nn[g];
     const V4* PC = A.pc + A.T.noff[g] + g;
     const int nb = A.E.partner[n];
     const R zr0 = (R)A.E.zr[n], zi0 = (R)A.E.zi[n];
     const int dF = A.T.dF[g], dB = A.T.dB[g];
+    const R hlen = (R)A.h, len0 = (R)A.T.l0[g], len1 = (R)A.T.l1[g];
     cplx_t<R> gt;
     if (A.bc_mode == 1) gt = hom_start<R>(-(double)PC[nn].x, PC[nn].y, A.E.zr[n] + PC[nn].z, A.E.zi[n]);
     else if (A.ga_n[dB]) { cplx_t<R> s = gather_start(A, dB, nb); gt = mk(s.re, -s.im); }
     else { cplx_t<R> s = hom_start<R>(A.fb_D[dB].x, A.fb_D[dB].y, A.E.zr[nb] + A.fb_a[dB], A.E.zi[nb]); gt = mk(s.re, -s.im); }
-    // the same evaluation of T as the march: Taylor table for interior pieces inside its radius, exp-based otherwise
-    constexpr int KT = scm::TaylorK<R>::K;
-    R tcf[KT + 1]; R thr2 = R(-1), pole_a = R(1), pole_res = R(0);
-    if (A.E.tc) {
-        for (int k = 0; k <= KT; ++k) tcf[k] = (R)A.E.tc[(size_t)n * TC_LD + k];
-        thr2 = (R)(A.E.tc[(size_t)n * TC_LD + 9] * scm::TaylorK<R>::RMAX2);
-        pole_a = (R)A.E.tc[(size_t)n * TC_LD + 10]; pole_res = (R)A.E.tc[(size_t)n * TC_LD + 11];
-    }
-    auto coefT = [&](const V4& c, int p) {
-        const R d2 = scm::mad(c.x, c.x, c.y * c.y);
-        const R dwr = scm::mad(-c.z, c.z, d2), dwi = R(-2) * zi0 * c.z;
-        const R s2 = scm::mad(dwr, dwr, dwi * dwi);
-        if (p > 0 && p < nn && s2 <= thr2) return scm::taylor_T<R, KT>(tcf, pole_a, pole_res, dwr, dwi, s2);
-        return scm::coef_T(d2, zr0 + c.z, zi0, c.w);
+    // a table evaluation of T as in the march (per-piece vote; the march's choice between the two tables of an
+    // imaginary-axis energy depends on the other 31 lanes of its round, so this tap may take the other one: both are
+    // accurate to rounding)
+    TTab<R, TM> tab; tab.load(A.E, n);
+    auto step = [&](cplx_t<R> x, R sgn, int p) {
+        const R len = p == 0 ? len0 : (p == nn ? len1 : hlen);
+        if (stepper == 1) return scm::step_mid(x, sgn * PC[p].x, PC[p].y, zr0 + PC[p].z, zi0, len);
+        const cplx_t<R> T = p > 0 && p < nn ? tab.voted(PC[p], zr0, zi0, len) : end_T<R>(PC[p], zr0, zi0, len);
+        return scm::step_T(x, sgn * PC[p].x, PC[p].y, zr0 + PC[p].z, zi0, T);
     };
-    for (int p = nn; p >= 1; --p) {
-        const V4 c = PC[p];
-        if (stepper == 1) gt = scm::step_mid(gt, -c.x, c.y, zr0 + c.z, zi0, c.w);
-        else { const cplx_t<R> T = coefT(c, p); gt = scm::step_T(gt, -c.x, c.y, zr0 + c.z, zi0, T); }
-        outGT[p - 1] = make_double2(gt.re, gt.im);
-    }
+    for (int p = nn; p >= 1; --p) { gt = step(gt, R(-1), p); outGT[p - 1] = make_double2(gt.re, gt.im); }
     cplx_t<R> gm;
     if (A.bc_mode == 1) gm = hom_start<R>(PC[0].x, PC[0].y, A.E.zr[n] + PC[0].z, A.E.zi[n]);
     else if (A.ga_n[dF]) gm = gather_start(A, dF, n);
     else gm = hom_start<R>(A.fb_D[dF].x, A.fb_D[dF].y, A.E.zr[n] + A.fb_a[dF], A.E.zi[n]);
-    for (int p = 0; p < nn; ++p) {
-        const V4 c = PC[p];
-        if (stepper == 1) gm = scm::step_mid(gm, c.x, c.y, zr0 + c.z, zi0, c.w);
-        else { const cplx_t<R> T = coefT(c, p); gm = scm::step_T(gm, c.x, c.y, zr0 + c.z, zi0, T); }
-        outG[p] = make_double2(gm.re, gm.im);
-    }
+    for (int p = 0; p < nn; ++p) { gm = step(gm, R(1), p); outG[p] = make_double2(gm.re, gm.im); }
+}
+template <typename R>
+__global__ void debug_traj_kernel(MarchArgsT<R> A, int stepper, int g, int n, double2* outG, double2* outGT) {
+    // a full warp runs the same trajectory and energy (the table evaluation votes across the warp); lane 0 writes
+    if (blockIdx.x != 0 || threadIdx.x >= 32) return;
+    if (A.E.tmode == 2) debug_traj_body<R, 2>(A, stepper, g, n, outG, outGT);
+    else debug_traj_body<R, 1>(A, stepper, g, n, outG, outGT);
 }
 
 // max relative error of the math building blocks vs the CUDA library on pseudo-random arguments

@@ -177,25 +177,49 @@ __device__ __forceinline__ cplx_t<R> coef_T(R d2, R zr, R zi, R len) {
     return mk(mad(tr, ir, -ti * ii), mad(tr, ii, ti * ir));
 }
 
-// Out-of-line copy of the exp-based evaluation: the march's hot loop evaluates T by taylor_T below and only calls
-// this for the two end pieces of a trajectory and for pieces outside the table's radius.
+// Out-of-line copy of the exp-based evaluation: the march's hot loop evaluates T by the Taylor table below and only
+// calls this for the two end pieces of a trajectory and for pieces outside the table's radius.
 template <typename R>
 __device__ __noinline__ cplx_t<R> coef_T_slow(R d2, R zr, R zi, R len) { return coef_T(d2, zr, zi, len); }
 
 // T as a function of w = Omega^2 is meromorphic: T(w) = tanh(l sqrt w)/sqrt w = sum_k (2/l)/(w + (2k+1)^2 wp),
-// wp = (pi/2l)^2.  For an energy i*zi on the imaginary axis and a piece of the common length l = h,
-// w = zi^2 + dw with dw = |De|^2 - a^2 - 2 i zi a.  The nearest pole is taken out in closed form and the rest,
-// R(w) = T(w) - (2/h)/(w + wp), is expanded about w0 = zi^2: its radius of convergence is w0 + 9 wp (the second
-// pole), against which dw is small for any |a| up to a few units:
-//     T = (2/h)/(w0 + wp + dw) + sum_k r_k(zi) dw^k,   r_k REAL (R is real on the real axis),
-// the r_k tabulated per energy by the host (sc_api.cu taylor_table).  A real-coefficient polynomial at a complex
-// point costs 2 FMAs per term: divide by the real quadratic (x - dw)(x - conj dw) = x^2 - r x + s; the remainder
-// b1 x + (b0 - r b1) at x = dw is (b0 - b1 Re dw) + i b1 Im dw.
+// wp = (pi/2l)^2, poles on the negative real axis only.  For an energy z0 (Matsubara i*eps, or eps + i*delta) and a
+// piece of the common length l = h with Doppler shift a,
+//     w = |De|^2 - (z0 + a)^2 = w0 + dw,   w0 = -z0^2,   dw = (|De|^2 - a^2) - 2 z0 a,
+// and |dw| is small against the distance from w0 to the nearest pole (eps^2 + wp on the imaginary axis; the ratio
+// is at most |a| 2h/pi + |De|^2/wp at ANY Matsubara energy), so T is a short Taylor polynomial in dw whose
+// coefficients c_k(z0) = T^(k)(w0)/k! the host tabulates per energy (sc_api.cu taylor_table).  On the imaginary
+// axis w0 is real and the c_k are REAL (T is real on the real axis): a real-coefficient polynomial at a complex point
+// costs 2 FMAs per term — divide by the real quadratic (x - dw)(x - conj dw) = x^2 - r x + s; the remainder
+// b1 x + (b0 - r b1) at x = dw is (b0 - b1 Re dw) + i b1 Im dw.  Off the axis (sc_ldos) the c_k are complex: Horner.
+// K and the radius fraction: truncation <= RMAX^(K+1) relative.
+#ifndef SC_TK
+#define SC_TK 6
+#endif
 template <typename R> struct TaylorK;
-template <> struct TaylorK<double> { static constexpr int K = 8; static constexpr double RMAX2 = 0.012 * 0.012; };   // 0.012^9 = 5e-18
-template <> struct TaylorK<float> { static constexpr int K = 4; static constexpr double RMAX2 = 0.03 * 0.03; };      // 0.03^5  = 2e-8
+template <> struct TaylorK<double> { static constexpr int K = SC_TK; static constexpr double RMAX = SC_TK >= 8 ? 0.024 : 0.01; };   // 0.01^7 = 1e-14, 0.024^9 = 3e-15
+template <> struct TaylorK<float> { static constexpr int K = 3; static constexpr double RMAX = 0.012; };                                // 0.012^4 = 2e-8
 template <typename R, int K>
-__device__ __forceinline__ cplx_t<R> taylor_T(const R (&c)[K + 1], R pole_a, R pole_res, R dwr, R dwi, R s) {
+__device__ __forceinline__ cplx_t<R> taylor_real(const R (&c)[K + 1], R dwr, R dwi, R s) {
+    const R r = dwr + dwr;
+    R b2 = c[K];
+    R b1 = mad(r, b2, c[K - 1]);
+#pragma unroll
+    for (int k = K - 2; k >= 0; --k) {
+        const R b0 = mad(r, b1, mad(-s, b2, c[k]));
+        b2 = b1; b1 = b0;
+    }
+    return mk(mad(-b2, dwr, b1), b2 * dwi);              // here b1 holds b_0 and b2 holds b_1
+}
+// The same with the nearest pole taken out in closed form (energies on the imaginary axis only): the rest,
+// R(w) = T(w) - (2/h)/(w + wp), converges out to the SECOND pole, |dw| < w0 + 9 wp — three times the reach in |a|:
+//     T = (2/h)/(w0 + wp + dw) + sum_k r_k dw^k,   r_k real.
+// Used by the rounds that spill T (strong vector potentials), where T is evaluated once per piece.
+template <typename R> struct TaylorPoleK;
+template <> struct TaylorPoleK<double> { static constexpr int K = 8; static constexpr double RMAX = 0.012; };   // 0.012^9 = 5e-18
+template <> struct TaylorPoleK<float> { static constexpr int K = 4; static constexpr double RMAX = 0.03; };      // 0.03^5  = 2e-8
+template <typename R, int K>
+__device__ __forceinline__ cplx_t<R> taylor_pole(const R (&c)[K + 1], R pole_a, R pole_res, R dwr, R dwi, R s) {
     const R r = dwr + dwr;
     R b2 = c[K];
     R b1 = mad(r, b2, c[K - 1]);
@@ -208,6 +232,17 @@ __device__ __forceinline__ cplx_t<R> taylor_T(const R (&c)[K + 1], R pole_a, R p
     const R pr = pole_a + dwr;
     const R q = pole_res * rcp_nr(mad(pr, pr, dwi * dwi));
     return mk(mad(pr, q, mad(-b2, dwr, b1)), mad(-dwi, q, b2 * dwi));
+}
+template <typename R, int K>
+__device__ __forceinline__ cplx_t<R> taylor_cplx(const R (&cr)[K + 1], const R (&ci)[K + 1], R dwr, R dwi) {
+    R pr = cr[K], pi = ci[K];
+#pragma unroll
+    for (int k = K - 1; k >= 0; --k) {
+        const R qr = mad(pr, dwr, mad(-pi, dwi, cr[k]));
+        pi = mad(pr, dwi, mad(pi, dwr, ci[k]));
+        pr = qr;
+    }
+    return mk(pr, pi);
 }
 
 // One closed-form step given T: 27 arithmetic instructions + 1 MUFU.
