@@ -37,7 +37,7 @@ UNIT = "updates/s"
 # FP64-pipe instructions the closed-form path needs per unit = (piece, energy, angle pair) = 4 logical updates
 # (gamma and gamma-tilde for angles k and k+N/2): DESIGN.md §6 tally of the kernel's own algorithm.
 #   "recompute" rounds (every piece inside the radius of the per-energy Taylor table of T): T twice 2 x 17, two Moebius
-#       steps 54, node products 27, energy reduction 8 = 123; scratch traffic 16 B written + 16 B read = 32 B per unit
+#       steps 2 x 27, node products 27, energy reduction 8 = 123; scratch traffic 16 B written + 16 B read = 32 B per unit
 #   "stored-T" rounds (strong vector potential): T once from the pole-subtracted table 36, 54, 27, 8 = 125; 64 B per unit
 # Evaluating T from its definition (sqrt, exp, sin/cos) would be 86 per evaluation — reported as context only.
 ALGO_FP64_INSTR_PER_UNIT = {"recompute": 123.0, "stored": 125.0}

@@ -207,7 +207,7 @@ constexpr int MARCH_MIN_CTAS = SC_MARCH_MIN_CTAS;   // resident CTAs per SM the 
 constexpr int PF_DIST = SC_PF_DIST;          // pass 2: scratch lines are pulled into L2 this many nodes ahead
 constexpr int RED_NODES = 4;                 // nodes per shared-memory reduction batch
 constexpr int RED_VALS = 6;
-constexpr int STAGE_LD = 33;                 // padded row of the transpose stage: conflict-free rows AND columns
+constexpr int STAGE_LD = 34;                 // padded row of the transpose stage: 16-byte aligned rows, conflict-free 128-bit column reads
 
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 // warp-uniform coefficient record (read-only path)
@@ -260,10 +260,11 @@ __device__ __forceinline__ R node_products(cplx_t<R> gm, R gtr, R gti, typename 
 // column sums of the stage: lane c < cnt sums row c over the 32 lanes (4 partial sums, fixed order)
 template <typename R>
 __device__ __forceinline__ double stage_colsum(const R* stage, int lane) {
-    const R* col = stage + lane * STAGE_LD;
+    using V2 = typename VT<R>::V2;
+    const V2* col = reinterpret_cast<const V2*>(stage + lane * STAGE_LD);
     R s0 = R(0), s1 = R(0), s2 = R(0), s3 = R(0);
 #pragma unroll
-    for (int i = 0; i < 32; i += 4) { s0 += col[i]; s1 += col[i + 1]; s2 += col[i + 2]; s3 += col[i + 3]; }
+    for (int i = 0; i < 16; i += 2) { const V2 a = col[i], b = col[i + 1]; s0 += a.x; s1 += a.y; s2 += b.x; s3 += b.y; }
     return (double)((s0 + s1) + (s2 + s3));
 }
 
@@ -306,6 +307,7 @@ __device__ __forceinline__ void st_ent(char* p, cplxf T, cplxf gt) {
 template <typename R, int TM>
 struct TTab {
     static constexpr int K = scm::TaylorK<R>::K;
+    static constexpr bool IMAG = TM == 1;       // every energy on the imaginary axis: Re z = a exactly
     R cr[K + 1]; R ci[TM == 2 ? K + 1 : 1];
     R thr2, m2zr, m2zi;
     __device__ __forceinline__ void load(const EnergyDev& E, int n) {
@@ -344,6 +346,7 @@ struct TTab {
 template <typename R>
 struct TTabPole {
     static constexpr int K = scm::TaylorPoleK<R>::K;
+    static constexpr bool IMAG = true;
     R c[K + 1]; R thr2, pole_a, pole_res, m2zi;
     __device__ __forceinline__ void load(const EnergyDev& E, int n) {
         const double* row = E.tcp + (size_t)n * TCP_LD;
@@ -430,7 +433,7 @@ __device__ __forceinline__ void march_round(const MarchArgsT<R>& A, const WarpJo
         return tab.fast(cc);
     };
     auto stepT = [&](cplx_t<R> g, R sgn, const V4& cc, cplx_t<R> T, R len) -> cplx_t<R> {
-        if (STEP == 0) return scm::step_T(g, sgn * cc.x, cc.y, zr0 + cc.z, zi0, T);
+        if (STEP == 0) return scm::step_T(g, sgn * cc.x, cc.y, TAB::IMAG ? cc.z : zr0 + cc.z, zi0, T);
         return scm::step_mid(g, sgn * cc.x, cc.y, zr0 + cc.z, zi0, len);
     };
 
