@@ -37,17 +37,19 @@ UNIT = "updates/s"
 # FP64-pipe instructions the closed-form path needs per unit = (piece, energy, angle pair) = 4 logical updates
 # (gamma and gamma-tilde for angles k and k+N/2): DESIGN.md §6 tally of the kernel's own algorithm.
 #   "recompute" rounds (every piece inside the radius of the per-energy Taylor table of T): T twice 2 x 17, two Moebius
-#       steps 2 x 27, node products 27, energy reduction 8 = 123; scratch traffic 16 B written + 16 B read = 32 B per unit
-#   "stored-T" rounds (strong vector potential): T once from the pole-subtracted table 36, 54, 27, 8 = 125; 64 B per unit
+#       steps 2 x 27, node products 28, energy reduction 8 = 124 (ncu source page: 124.2 executed); scratch traffic
+#       16 B written + 16 B read = 32 B per unit
+#   "stored-T" rounds (strong vector potential): T once from the pole-subtracted table 36, 54, 28, 8 = 126; 64 B per unit
 # Evaluating T from its definition (sqrt, exp, sin/cos) would be 86 per evaluation — reported as context only.
-ALGO_FP64_INSTR_PER_UNIT = {"recompute": 123.0, "stored": 125.0}
+ALGO_FP64_INSTR_PER_UNIT = {"recompute": 124.0, "stored": 126.0}
 ALGO_HBM_BYTES_PER_UNIT = {"recompute": 32.0, "stored": 64.0}
 TEXTBOOK_FP64_INSTR_PER_UNIT = 184.0
-ALGO_FP64_INSTR_PER_UNIT_MIDPOINT = 2 * 66.0 + 27.0 + 8.0
+ALGO_FP64_INSTR_PER_UNIT_MIDPOINT = 2 * 66.0 + 28.0 + 8.0
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE march launch at configs[4], fp64, closed-form stepper, all rounds in
 # "recompute" mode (--sweep-only: A = A_ext), from the `ncu --set full` capture summarised in profiles/
-NCU_TRAFFIC_BYTES = {}
-NCU_PIPE_FP64_ACTIVE_PCT = {}
+# (profiles/r1_march_fp64_cfg4_ncu_full.md: 2.636 TB read + 2.309 TB written)
+NCU_TRAFFIC_BYTES = {(4, 64, 0): 4.945456e12}
+NCU_PIPE_FP64_ACTIVE_PCT = {(4, 64, 0): 74.6}
 
 
 class ClockSampler(threading.Thread):
@@ -261,8 +263,8 @@ def run_ours(a):
     roofline = {"bound": "alu", "kernel": "sck::march_kernel<0,false,%d,%s,1>" % (a.stepper, "double" if a.precision == 64 else "float"),
                 "launches_timed": march_launches, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                 "frac": achieved / peak,
-                "traffic": NCU_TRAFFIC_BYTES.get(key) if full_size and u_st == 0 else None,
-                "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/; capture with all rounds in recompute mode)",
+                "traffic": NCU_TRAFFIC_BYTES.get(key) if full_size else None,
+                "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/) of a launch with ALL rounds in recompute mode (32 B algorithmic per unit = 4.22e12); stored-T rounds move 64 B per unit",
                 "algorithmic_bytes_per_launch": hbm,
                 "ncu_pipe_fp64_cycles_active_pct": NCU_PIPE_FP64_ACTIVE_PCT.get(key) if full_size else None,
                 "note": "fp64 pipe: flops = 2 x FP64-pipe instructions; achieved = algorithmic count (DESIGN.md §6) x units / "

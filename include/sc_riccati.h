@@ -127,11 +127,22 @@ sc_status sc_update_vector_potential(sc_ctx* ctx, const double* jx, const double
 sc_status sc_set_external_field(sc_ctx* ctx, const double* Aext_x, const double* Aext_y);
 
 /* One self-consistency iteration (Algorithm 1 :203-205): fields := (delta, A_ext + A_ind); sweep; A-solve;
- * x = (Re D, Im D, kappa^2 A_ind) <- x + alpha (g(x) - x) with accelerator 0 = Picard (E5 :1070, alpha =
- * step) or 1 = Barzilai-Borwein (E8-E11 :1107-1115, first alpha = step, clipped to [1e-3, 100]).  burnin != 0
- * keeps delta, A_ind fixed (:962).  delta_inout / Aind_*_inout: dev, updated in place. */
+ * x = (Re D, Im D, kappa^2 A_ind) (E3 :1053), d = g(x) - x (E4), then by accelerator
+ *   0 Picard           x += step d                                                        (E5 :1070)
+ *   1 Barzilai-Borwein x += alpha d, alpha_0 = step, alternating BB1/BB2 scaling, clipped   (E8-E11 :1107-1115)
+ *   2 Polyak           v <- (1 - drag) v + step d, x += v, v_0 = 0                          (E6-E7 :1087-1089)
+ *   3 CongAcc          per component of x: cosine-similarity-adapted step and moving average (E12-E17 :1134-1151)
+ * Changing the accelerator between calls restarts it.  burnin != 0 keeps delta, A_ind fixed (:962).
+ * delta_inout / Aind_*_inout: dev, updated in place. */
 sc_status sc_iterate(sc_ctx* ctx, int accelerator, double step, int burnin, void* delta_inout,
                      double* Aind_x_inout, double* Aind_y_inout, sc_sweep_stats* stats);
+
+/* Parameters of the accelerators (PAPER.md Listings 14-16 :1093, :1121, :1157); an argument <= 0 keeps its
+ * current value.  Defaults: drag 0.5 (Polyak beta in (0,1]); step_factor k = 1.234 and cos_similarity_min
+ * s_min = 0.7 (CongAcc E13-E14); step sizes of Barzilai-Borwein and CongAcc clipped to [step_min, step_max] =
+ * [1e-3, 100].  SC_ERR_ARG if a value is out of range. */
+sc_status sc_set_accelerator_params(sc_ctx* ctx, double drag, double step_factor, double cos_similarity_min,
+                                    double step_min, double step_max);
 
 /* ---- parity / debug taps (synchronise) -------------------------------------------------------- */
 /* Geometry: lattice size N_rot, number of trajectories of angle k (all N_phi angles are addressable). */

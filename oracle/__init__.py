@@ -285,18 +285,93 @@ def residual(new, old, p=2):
     return float(na / nb) if nb > 0 else float(na)
 
 
-class Driver:
-    """x = (Re Delta, Im Delta, kappa^2 A_x^ind, kappa^2 A_y^ind) (E3 :1053); d = g(x) - x (E4);
-    Picard x += alpha d (E5) or Barzilai-Borwein with alternating BB1/BB2 scaling (E8-E11),
-    alpha clipped to [1e-3, 100] (Listing 15 :1121-1127).  Reading R-BB: iteration index i starts at 0;
-    the first update uses alpha = step; for i >= 1 alpha_{i+1} = alpha_i * (s^BB1 if i odd else s^BB2)."""
+class Accelerator:
+    """Fixed-point accelerators of App. E (:1044-1151) acting on the concatenated iterate x with d = g(x) - x (E4):
+    update(d) returns the increment x_{i+1} - x_i.  `ncomp` equal slices of x are the "components" of CongAcc.
+      0  Picard: alpha d (E5 :1070);
+      1  Barzilai-Borwein with alternating BB1/BB2 scaling (E8-E11 :1107-1115), alpha clipped to [1e-3, 100]
+         (Listing 15 :1121-1127).  Reading R-BB: iteration index i starts at 0; the first update uses alpha = step;
+         for i >= 1 alpha_{i+1} = alpha_i * (s^BB1 if i odd else s^BB2);
+      2  Polyak "small heavy sphere" (E6-E7 :1087-1089): v <- (1 - drag) v + alpha d, increment v, v_0 = 0
+         (Listing 14 :1093: step 2.0, drag 0.5);
+      3  CongAcc (E12-E17 :1134-1151), per component c: s = cos(m_c, d_c) (taken as 0 while m_c = 0);
+         alpha_c <- clip(alpha_c k^s); w_c <- w_c if s >= s_min else the root w* of E17 (bisection on [0, 1],
+         60 halvings); m_c <- w_c m_c + (1 - w_c) d_c; increment alpha_c m_c; w_{0,c} = 0, m_{0,c} = 0
+         (Listing 16 :1157: step 0.5, k = 1.234, s_min = 0.7, alpha in [1e-3, 100])."""
 
-    def __init__(self, orc: Oracle, Aext_x, Aext_y, ne, accelerator=0, step=1.0):
-        self.o, self.ne, self.acc, self.alpha = orc, ne, accelerator, step
-        self.Aext = (np.asarray(Aext_x, np.float64), np.asarray(Aext_y, np.float64))
-        self.stores = None
+    def __init__(self, kind=0, step=1.0, drag=0.5, step_factor=1.234, cos_min=0.7, step_min=1e-3, step_max=100.0, ncomp=4):
+        self.kind, self.alpha = kind, step
+        self.drag, self.kfac, self.smin, self.amin, self.amax, self.ncomp = drag, step_factor, cos_min, step_min, step_max, ncomp
         self.i = 0
         self.d_prev = None
+        self.vel = None
+        self.m = None
+        self.alpha_c = [step] * ncomp
+        self.w_c = [0.0] * ncomp
+
+    @staticmethod
+    def cos_mix(w, mm, md, dd):
+        """cos(w m + (1-w) d, d) from the three dot products m.m, m.d, d.d."""
+        num = w * md + (1.0 - w) * dd
+        n2 = w * w * mm + 2.0 * w * (1.0 - w) * md + (1.0 - w) * (1.0 - w) * dd
+        return num / np.sqrt(n2 * dd) if n2 > 0 and dd > 0 else 1.0
+
+    def update(self, d):
+        d = np.asarray(d, np.float64)
+        if self.kind == 1 and self.d_prev is not None:
+            dd = d - self.d_prev
+            dot = abs(float(np.dot(self.d_prev, dd)))
+            if self.i % 2 == 1:
+                s = float(np.dot(self.d_prev, self.d_prev)) / dot if dot > 0 else 1.0
+            else:
+                nd = float(np.dot(dd, dd))
+                s = dot / nd if nd > 0 else 1.0
+            self.alpha = min(max(self.alpha * s, self.amin), self.amax)
+        if self.kind == 2:
+            if self.vel is None:
+                self.vel = np.zeros_like(d)
+            self.vel = (1.0 - self.drag) * self.vel + self.alpha * d
+            upd = self.vel.copy()
+        elif self.kind == 3:
+            if self.m is None:
+                self.m = np.zeros_like(d)
+            n = d.size // self.ncomp
+            upd = np.zeros_like(d)
+            for c in range(self.ncomp):
+                sl = slice(c * n, (c + 1) * n)
+                mc, dc = self.m[sl], d[sl]
+                mm, md, dd_ = float(np.dot(mc, mc)), float(np.dot(mc, dc)), float(np.dot(dc, dc))
+                s = md / np.sqrt(mm * dd_) if mm > 0 and dd_ > 0 else 0.0
+                self.alpha_c[c] = min(max(self.alpha_c[c] * self.kfac ** s, self.amin), self.amax)
+                if self.i == 0:
+                    self.w_c[c] = 0.0
+                elif s < self.smin:
+                    lo, hi = 0.0, 1.0                      # cos = 1 at w = 0 and = s < s_min at w = 1
+                    for _ in range(60):
+                        mid = 0.5 * (lo + hi)
+                        if self.cos_mix(mid, mm, md, dd_) >= self.smin:
+                            lo = mid
+                        else:
+                            hi = mid
+                    self.w_c[c] = 0.5 * (lo + hi)
+                self.m[sl] = self.w_c[c] * mc + (1.0 - self.w_c[c]) * dc
+                upd[sl] = self.alpha_c[c] * self.m[sl]
+        else:
+            upd = self.alpha * d
+        self.d_prev = d.copy()
+        self.i += 1
+        return upd
+
+
+class Driver:
+    """Algorithm 1 (:203-205): sweep -> A-solve -> accelerator on x = (Re Delta, Im Delta, kappa^2 A_x^ind,
+    kappa^2 A_y^ind) (E3 :1053) -> residual (Eq. 27 :201).  `accelerator` and the keyword parameters are Accelerator's."""
+
+    def __init__(self, orc: Oracle, Aext_x, Aext_y, ne, accelerator=0, step=1.0, **kw):
+        self.o, self.ne = orc, ne
+        self.accel = Accelerator(accelerator, step, ncomp=4, **kw)
+        self.Aext = (np.asarray(Aext_x, np.float64), np.asarray(Aext_y, np.float64))
+        self.stores = None
 
     def iterate(self, delta, Aind_x, Aind_y, burnin=False):
         o = self.o
@@ -316,19 +391,7 @@ class Driver:
             gAx, gAy = np.zeros_like(Aind_x), np.zeros_like(Aind_y)
         x = np.concatenate([delta.real.ravel(), delta.imag.ravel(), k2 * Aind_x.ravel(), k2 * Aind_y.ravel()])
         gx = np.concatenate([r["delta_new"].real.ravel(), r["delta_new"].imag.ravel(), k2 * gAx.ravel(), k2 * gAy.ravel()])
-        d = gx - x
-        if self.acc == 1 and self.d_prev is not None:
-            dd = d - self.d_prev
-            dot = abs(float(np.dot(self.d_prev, dd)))
-            if self.i % 2 == 1:
-                s = float(np.dot(self.d_prev, self.d_prev)) / dot if dot > 0 else 1.0
-            else:
-                nd = float(np.dot(dd, dd))
-                s = dot / nd if nd > 0 else 1.0
-            self.alpha = min(max(self.alpha * s, 1e-3), 100.0)
-        xn = x + self.alpha * d
-        self.d_prev = d
-        self.i += 1
+        xn = x + self.accel.update(gx - x)
         n = o.nx * o.ny
         shp = (o.ny, o.nx)
         out["delta"] = (xn[:n] + 1j * xn[n:2 * n]).reshape(shp) * o.mask
@@ -337,5 +400,6 @@ class Driver:
         else:
             out["Aind_x"], out["Aind_y"] = Aind_x, Aind_y
         out["res_delta"] = residual(out["delta"], delta)
-        out["alpha"] = self.alpha
+        out["alpha"] = self.accel.alpha if self.accel.kind != 3 else list(self.accel.alpha_c)
+        out["w"] = list(self.accel.w_c)
         return out

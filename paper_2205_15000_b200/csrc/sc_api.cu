@@ -604,7 +604,7 @@ sc_status sc_update_vector_potential(sc_ctx* ctx, const double* jx, const double
 
 sc_status sc_iterate(sc_ctx* ctx, int accelerator, double step, int burnin, void* delta_inout, double* Aix, double* Aiy, sc_sweep_stats* stats) {
     if (!ctx || !delta_inout) return fail(ctx, SC_ERR_ARG, "null argument");
-    if (accelerator != 0 && accelerator != 1) return fail(ctx, SC_ERR_ARG, "accelerator must be 0 (Picard) or 1 (Barzilai-Borwein)");
+    if (accelerator < 0 || accelerator > 3) return fail(ctx, SC_ERR_ARG, "accelerator must be 0 (Picard), 1 (Barzilai-Borwein), 2 (Polyak) or 3 (CongAcc)");
     const int nx = ctx->grid.nx, ny = ctx->grid.ny; const size_t ng = (size_t)nx * ny;
     const bool withA = ctx->kappa > 0 && Aix && Aiy;
     std::string e;
@@ -634,6 +634,20 @@ sc_status sc_iterate(sc_ctx* ctx, int accelerator, double step, int burnin, void
         stats->res_delta = r[0]; stats->res_A = r[1]; stats->res_j = r[2]; stats->res_fe = r[3];
         stats->min_one_minus_abs_gamma = 0.0;
     }
+    return SC_OK;
+}
+
+sc_status sc_set_accelerator_params(sc_ctx* ctx, double drag, double step_factor, double cos_similarity_min,
+                                    double step_min, double step_max) {
+    if (!ctx) return SC_ERR_ARG;
+    scf::AccelParams P = ctx->fs.par;
+    if (drag > 0) { if (drag > 1) return fail(ctx, SC_ERR_ARG, "drag must lie in (0, 1]"); P.drag = drag; }
+    if (step_factor > 0) { if (step_factor < 1) return fail(ctx, SC_ERR_ARG, "step_factor must be >= 1"); P.kfac = step_factor; }
+    if (cos_similarity_min > 0) { if (cos_similarity_min >= 1) return fail(ctx, SC_ERR_ARG, "cos_similarity_min must be < 1"); P.smin = cos_similarity_min; }
+    if (step_min > 0) P.amin = step_min;
+    if (step_max > 0) P.amax = step_max;
+    if (!(P.amin <= P.amax)) return fail(ctx, SC_ERR_ARG, "step_min > step_max");
+    ctx->fs.par = P;
     return SC_OK;
 }
 

@@ -6,8 +6,8 @@
 // D3-D6 (:1014-1021).  The paper truncates an eigen-decomposition of G "to increase performance" (:1033);
 // here the cross-correlation is done exactly as a zero-padded (2nx x 2ny) FFT convolution (cuFFT D2Z/Z2D —
 // a library FFT, off the roofline-judged path): O(N^2 log N) instead of O(N^4).
-// a9: x = (Re D, Im D, kappa^2 A_x, kappa^2 A_y) (E3 :1053), d = g(x) - x (E4), Picard (E5) or
-// Barzilai-Borwein (E8-E11) with the step size kept on the device.
+// a9: x = (Re D, Im D, kappa^2 A_x, kappa^2 A_y) (E3 :1053), d = g(x) - x (E4), Picard (E5), Barzilai-Borwein
+// (E8-E11), Polyak (E6-E7) or CongAcc (E12-E17), with step sizes, weights and the bisection of E17 kept on the device.
 #pragma once
 #include <cuda_runtime.h>
 #include <cufft.h>
@@ -20,13 +20,18 @@ namespace scf {
 
 constexpr int RED_BLOCKS = 296;
 constexpr int RED_THREADS = 256;
+constexpr int RED_MAXOUT = 12;      // outputs of one reduction (CongAcc: 3 dot products x 4 components)
+constexpr int RED_RES = RED_BLOCKS * RED_MAXOUT;   // offset of the results behind the partials
+
+// parameters of the accelerators (PAPER.md Listings 14-16 :1093, :1121, :1157)
+struct AccelParams { double drag = 0.5, kfac = 1.234, smin = 0.7, amin = 1e-3, amax = 100.0; };
 
 struct FieldState {
     // vector potential
     int nx = 0, ny = 0; double h = 0;
     cufftHandle plan_f = 0, plan_b = 0; bool plans = false;
     cufftDoubleComplex* Ghat = nullptr; double* pad = nullptr; cufftDoubleComplex* spec = nullptr;
-    double* red = nullptr;          // RED_BLOCKS * 8 partials + 16 results
+    double* red = nullptr;          // RED_BLOCKS * RED_MAXOUT partials + 32 results
     // driver
     size_t ng = 0;
     double *Atot_x = nullptr, *Atot_y = nullptr, *jx = nullptr, *jy = nullptr, *feI = nullptr, *gAx = nullptr, *gAy = nullptr;
@@ -34,14 +39,17 @@ struct FieldState {
     double* d_prev = nullptr;       // 4*ng
     double* d_cur = nullptr;        // 4*ng
     double *prev_jx = nullptr, *prev_jy = nullptr, *prev_fe = nullptr;
-    double* state = nullptr;        // [0] alpha, [1] iteration index, [2..5] residuals (delta, A, j, fe)
-    bool driver = false, first = true;
+    double* upd = nullptr;          // 4*ng: x_{i+1} - x_i
+    double* aux = nullptr;          // 4*ng: Polyak velocity v / CongAcc moving average m (allocated on first use)
+    double* state = nullptr;        // [0] alpha, [1] iteration index, [2..5] residuals (delta, A, j, fe), [6..9] alpha_c, [10..13] w_c
+    AccelParams par;
+    bool driver = false, first = true; int last_kind = -1;
 };
 
 inline void release(FieldState& F) {
     if (F.plans) { cufftDestroy(F.plan_f); cufftDestroy(F.plan_b); }
     void* ptrs[] = {F.Ghat, F.pad, F.spec, F.red, F.Atot_x, F.Atot_y, F.jx, F.jy, F.feI, F.gAx, F.gAy, F.dnew,
-                    F.d_prev, F.d_cur, F.prev_jx, F.prev_jy, F.prev_fe, F.state};
+                    F.d_prev, F.d_cur, F.prev_jx, F.prev_jy, F.prev_fe, F.state, F.upd, F.aux};
     for (void* p : ptrs) if (p) cudaFree(p);
     F = FieldState();
 }
@@ -125,7 +133,7 @@ inline int ensure_vp(FieldState& F, int nx, int ny, double h, cudaStream_t s, st
     SCF_CU(cudaMalloc((void**)&F.pad, (size_t)px * py * sizeof(double)));
     SCF_CU(cudaMalloc((void**)&F.spec, nspec * sizeof(cufftDoubleComplex)));
     SCF_CU(cudaMalloc((void**)&F.Ghat, nspec * sizeof(cufftDoubleComplex)));
-    if (!F.red) SCF_CU(cudaMalloc((void**)&F.red, (RED_BLOCKS * 8 + 16) * sizeof(double)));
+    if (!F.red) SCF_CU(cudaMalloc((void**)&F.red, (RED_RES + 32) * sizeof(double)));
     SCF_FFT(cufftPlan2d(&F.plan_f, py, px, CUFFT_D2Z));
     SCF_FFT(cufftPlan2d(&F.plan_b, py, px, CUFFT_Z2D));
     SCF_FFT(cufftSetStream(F.plan_f, s)); SCF_FFT(cufftSetStream(F.plan_b, s));
@@ -153,7 +161,7 @@ inline int vector_potential(FieldState& F, int nx, int ny, double h, const unsig
     }
     if (int rc = ensure_vp(F, nx, ny, h, s, err)) return rc;
     const int px = 2 * nx, py = 2 * ny; const size_t nspec = (size_t)py * (px / 2 + 1);
-    double* res = F.red + RED_BLOCKS * 8;
+    double* res = F.red + RED_RES;
     reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, MeanOp{mask, jx, jy}, F.red, 3);
     reduce_stage2<<<1, 32, 0, s>>>(F.red, 3, res);
     mean_finish_kernel<<<1, 1, 0, s>>>(res);
@@ -186,8 +194,9 @@ inline int ensure_driver(FieldState& F, size_t ng, std::string& err) {
     for (double** b : bufs) { SCF_CU(cudaMalloc((void**)b, ng * sizeof(double))); SCF_CU(cudaMemset(*b, 0, ng * sizeof(double))); }
     SCF_CU(cudaMalloc((void**)&F.dnew, ng * sizeof(double2)));
     SCF_CU(cudaMalloc((void**)&F.d_prev, 4 * ng * sizeof(double))); SCF_CU(cudaMalloc((void**)&F.d_cur, 4 * ng * sizeof(double)));
+    SCF_CU(cudaMalloc((void**)&F.upd, 4 * ng * sizeof(double)));
     SCF_CU(cudaMalloc((void**)&F.state, 16 * sizeof(double))); SCF_CU(cudaMemset(F.state, 0, 16 * sizeof(double)));
-    if (!F.red) SCF_CU(cudaMalloc((void**)&F.red, (RED_BLOCKS * 8 + 16) * sizeof(double)));
+    if (!F.red) SCF_CU(cudaMalloc((void**)&F.red, (RED_RES + 32) * sizeof(double)));
     F.driver = true; F.first = true;
     return 0;
 }
@@ -219,25 +228,69 @@ struct DotOp {     // c = 0: dp.dd, 1: dp.dp, 2: dd.dd, with dd = d - dp
     }
 };
 // state[0] = alpha, state[1] = iteration index i (reading R-BB: i starts at 0, first update uses alpha = step)
-__global__ void alpha_kernel(double* state, const double* dots, int accelerator, double step, int first) {
-    if (first) { state[0] = step; state[1] = 0.0; }
+__global__ void alpha_kernel(double* state, const double* dots, int accelerator, double step, int first, AccelParams P) {
+    if (first) { state[0] = step; state[1] = 0.0; for (int c = 0; c < 4; ++c) { state[6 + c] = step; state[10 + c] = 0.0; } }
     const int i = (int)state[1];
     if (accelerator == 1 && i >= 1) {
         const double dot = fabs(dots[0]);
         double s = 1.0;
         if (i & 1) { if (dot > 0) s = dots[1] / dot; } else { if (dots[2] > 0) s = dot / dots[2]; }
-        state[0] = fmin(fmax(state[0] * s, 1e-3), 100.0);
-    } else if (accelerator == 0) state[0] = step;
+        state[0] = fmin(fmax(state[0] * s, P.amin), P.amax);
+    } else if (accelerator != 1) state[0] = step;
     state[1] = i + 1;
 }
-struct NormOp {    // c: 0 |dx_delta|^2, 1 |x_delta|^2, 2 |dx_A|^2, 3 |x_A|^2 (before the update)
-    size_t ng; const double2* delta; const double* aix; const double* aiy; const double* d; const double* state; double k2; int withA;
+// CongAcc (E12-E17 :1134-1151): dots of component c = {m.m, m.d, d.d}[c]; one thread per component
+struct CongDotOp {   // output c = 3 * component + {0: m.m, 1: m.d, 2: d.d}; i runs over one component (ng values)
+    size_t ng; const double* m; const double* d;
     __device__ double operator()(size_t i, int c) const {
-        const double al = state[0];
-        if (c == 0) return al * al * (d[i] * d[i] + d[ng + i] * d[ng + i]);
+        const size_t q = (size_t)(c / 3) * ng + i;
+        const int w = c % 3;
+        return w == 0 ? m[q] * m[q] : w == 1 ? m[q] * d[q] : d[q] * d[q];
+    }
+};
+__device__ inline double cong_cos_mix(double w, double mm, double md, double dd) {
+    const double num = w * md + (1.0 - w) * dd;
+    const double n2 = w * w * mm + 2.0 * w * (1.0 - w) * md + (1.0 - w) * (1.0 - w) * dd;
+    return (n2 > 0 && dd > 0) ? num / sqrt(n2 * dd) : 1.0;
+}
+// runs after alpha_kernel (state[1] already holds i + 1)
+__global__ void congacc_kernel(double* state, const double* dots, AccelParams P) {
+    const int c = threadIdx.x;
+    if (c >= 4) return;
+    const int i = (int)state[1] - 1;
+    const double mm = dots[3 * c], md = dots[3 * c + 1], dd = dots[3 * c + 2];
+    const double s = (mm > 0 && dd > 0) ? md / sqrt(mm * dd) : 0.0;            // E12
+    state[6 + c] = fmin(fmax(state[6 + c] * pow(P.kfac, s), P.amin), P.amax);   // E13
+    if (i == 0) state[10 + c] = 0.0;                                            // w_0 = 0 (:1151)
+    else if (s < P.smin) {                                                      // E14, E17 by bisection
+        double lo = 0.0, hi = 1.0;
+        for (int it = 0; it < 60; ++it) {
+            const double mid = 0.5 * (lo + hi);
+            if (cong_cos_mix(mid, mm, md, dd) >= P.smin) lo = mid; else hi = mid;
+        }
+        state[10 + c] = 0.5 * (lo + hi);
+    }
+}
+// the increment x_{i+1} - x_i: alpha d (Picard E5, BB E11); v <- (1 - drag) v + alpha d (Polyak E6-E7);
+// m_c <- w_c m_c + (1 - w_c) d_c, alpha_c m_c (CongAcc E15-E16)
+__global__ void step_kernel(size_t ng, int accelerator, const double* d, double* aux, const double* state, double drag, double* upd) {
+    const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= 4 * ng) return;
+    if (accelerator == 2) { const double v = (1.0 - drag) * aux[q] + state[0] * d[q]; aux[q] = v; upd[q] = v; }
+    else if (accelerator == 3) {
+        const int c = (int)(q / ng);
+        const double w = state[10 + c];
+        const double m = w * aux[q] + (1.0 - w) * d[q];
+        aux[q] = m; upd[q] = state[6 + c] * m;
+    } else upd[q] = state[0] * d[q];
+}
+struct NormOp {    // c: 0 |dx_delta|^2, 1 |x_delta|^2, 2 |dx_A|^2, 3 |x_A|^2 (before the update)
+    size_t ng; const double2* delta; const double* aix; const double* aiy; const double* u; double k2; int withA;
+    __device__ double operator()(size_t i, int c) const {
+        if (c == 0) return u[i] * u[i] + u[ng + i] * u[ng + i];
         if (c == 1) return delta[i].x * delta[i].x + delta[i].y * delta[i].y;
         if (!withA) return 0.0;
-        if (c == 2) return al * al * (d[2 * ng + i] * d[2 * ng + i] + d[3 * ng + i] * d[3 * ng + i]) / (k2 * k2);
+        if (c == 2) return (u[2 * ng + i] * u[2 * ng + i] + u[3 * ng + i] * u[3 * ng + i]) / (k2 * k2);
         return aix[i] * aix[i] + aiy[i] * aiy[i];
     }
 };
@@ -256,38 +309,48 @@ __global__ void residual_kernel(double* state, const double* n1, const double* n
     state[4] = n2[1] > 0 ? sqrt(n2[0] / n2[1]) : sqrt(n2[0]);
     state[5] = n2[3] > 0 ? sqrt(n2[2] / n2[3]) : sqrt(n2[2]);
 }
-__global__ void update_kernel(size_t ng, double2* delta, double* aix, double* aiy, const double* d, const double* state,
+__global__ void update_kernel(size_t ng, double2* delta, double* aix, double* aiy, const double* u,
                               const unsigned char* mask, double k2, int withA) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= ng) return;
-    const double al = state[0];
     const double m = mask[i] ? 1.0 : 0.0;
-    delta[i] = make_double2(m * (delta[i].x + al * d[i]), m * (delta[i].y + al * d[ng + i]));
-    if (withA) { aix[i] += al * d[2 * ng + i] / k2; aiy[i] += al * d[3 * ng + i] / k2; }
+    delta[i] = make_double2(m * (delta[i].x + u[i]), m * (delta[i].y + u[ng + i]));
+    if (withA) { aix[i] += u[2 * ng + i] / k2; aiy[i] += u[3 * ng + i] / k2; }
 }
 
 inline int mix(FieldState& F, int accelerator, double step, double kappa, bool withA, double2* delta, double* aix, double* aiy,
                const unsigned char* mask, size_t ng, cudaStream_t s, std::string& err) {
     const double k2 = withA ? kappa * kappa : 0.0;
-    const unsigned nb = (unsigned)((ng + 255) / 256);
-    double* res = F.red + RED_BLOCKS * 8;
+    const unsigned nb = (unsigned)((ng + 255) / 256), nb4 = (unsigned)((4 * ng + 255) / 256);
+    double* res = F.red + RED_RES;
+    if (accelerator != F.last_kind) F.first = true;         // a change of method restarts it (v_0 = 0, w_0 = 0, m_0 = 0)
+    if (accelerator >= 2) {
+        if (!F.aux) SCF_CU(cudaMalloc((void**)&F.aux, 4 * ng * sizeof(double)));
+        if (F.first) SCF_CU(cudaMemsetAsync(F.aux, 0, 4 * ng * sizeof(double), s));
+    }
     diff_kernel<<<nb, 256, 0, s>>>(ng, delta, F.dnew, aix, aiy, F.gAx, F.gAy, k2, withA ? 1 : 0, F.d_cur);
     if (!F.first && accelerator == 1) {
         reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(4 * ng, DotOp{F.d_cur, F.d_prev}, F.red, 3);
         reduce_stage2<<<1, 32, 0, s>>>(F.red, 3, res);
     }
-    alpha_kernel<<<1, 1, 0, s>>>(F.state, res, accelerator, step, F.first ? 1 : 0);
-    reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, NormOp{ng, delta, aix, aiy, F.d_cur, F.state, k2, withA ? 1 : 0}, F.red, 4);
+    alpha_kernel<<<1, 1, 0, s>>>(F.state, res, accelerator, step, F.first ? 1 : 0, F.par);
+    if (accelerator == 3) {
+        reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, CongDotOp{ng, F.aux, F.d_cur}, F.red, 12);
+        reduce_stage2<<<1, 32, 0, s>>>(F.red, 12, res + 16);
+        congacc_kernel<<<1, 4, 0, s>>>(F.state, res + 16, F.par);
+    }
+    step_kernel<<<nb4, 256, 0, s>>>(ng, accelerator, F.d_cur, F.aux, F.state, F.par.drag, F.upd);
+    reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, NormOp{ng, delta, aix, aiy, F.upd, k2, withA ? 1 : 0}, F.red, 4);
     reduce_stage2<<<1, 32, 0, s>>>(F.red, 4, res + 4);
     reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, ObsNormOp{F.jx, F.jy, F.feI, F.prev_jx, F.prev_jy, F.prev_fe}, F.red, 4);
     reduce_stage2<<<1, 32, 0, s>>>(F.red, 4, res + 8);
     residual_kernel<<<1, 1, 0, s>>>(F.state, res + 4, res + 8);
-    update_kernel<<<nb, 256, 0, s>>>(ng, delta, aix, aiy, F.d_cur, F.state, mask, k2 > 0 ? k2 : 1.0, withA ? 1 : 0);
+    update_kernel<<<nb, 256, 0, s>>>(ng, delta, aix, aiy, F.upd, mask, k2 > 0 ? k2 : 1.0, withA ? 1 : 0);
     SCF_CU(cudaMemcpyAsync(F.prev_jx, F.jx, ng * sizeof(double), cudaMemcpyDeviceToDevice, s));
     SCF_CU(cudaMemcpyAsync(F.prev_jy, F.jy, ng * sizeof(double), cudaMemcpyDeviceToDevice, s));
     SCF_CU(cudaMemcpyAsync(F.prev_fe, F.feI, ng * sizeof(double), cudaMemcpyDeviceToDevice, s));
     std::swap(F.d_cur, F.d_prev);
-    F.first = false;
+    F.first = false; F.last_kind = accelerator;
     SCF_CU(cudaGetLastError());
     return 0;
 }

@@ -515,8 +515,8 @@ __device__ __forceinline__ void march_round(const MarchArgsT<R>& A, const WarpJo
     if (LD)
         for (int q = RED_NODES; q < PF_DIST && q < nn; q += RED_NODES)
             if (pf_lane) prefetch_l2(J.scr_w + (size_t)(q + NB) * ROW + lane * 128);
-    Ent<R> En{};
-    if (LD) En = ld_ent<ST>(e, R(0));
+    Ent<R> En{}, En2{};                          // entries of the next two nodes (register look-ahead over the HBM latency)
+    if (LD) { En = ld_ent<ST>(e, R(0)); En2 = ld_ent<ST>(e + ROW, R(0)); }
     double part_nxt = 0.0;                       // running sums of the earlier energy rounds, fetched one batch ahead
     if (MODE == 0 && n0 && lane < RED_NODES * RED_VALS && lane < npart) part_nxt = J.PART[lane];
     int m = 0;
@@ -524,7 +524,7 @@ __device__ __forceinline__ void march_round(const MarchArgsT<R>& A, const WarpJo
     auto node = [&](int b, const V4* pbuf, const V2* dbuf, bool exitp) {
         const Ent<R> Ec = En;
         const V4 cc = pbuf[(m + b) & (CHUNK - 1)]; const V2 dc = dbuf[(m + b) & (CHUNK - 1)];
-        if (LD) En = ld_ent<ST>(e + (b + 1) * ROW, R(0));          // one entry ahead (the scratch has 2 spare rows)
+        if (LD) { En = En2; En2 = ld_ent<ST>(e + (b + 2) * ROW, R(0)); }   // two entries ahead (the scratch has spare rows)
         if (MODE != 2) {
             const R rg = node_products<MODE, STATS, R>(gm, Ec.gr, Ec.gi, dc, wn, J.stage + b * RED_VALS * STAGE_LD + lane, max2);
             if (MODE == 1 && act) A.ldos[(size_t)(J.noff + m + b) * ne + n] = (double)rg;

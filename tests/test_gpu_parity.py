@@ -346,3 +346,56 @@ def test_self_consistent_iterations_match(sc, cfg, kw, acc, niter):
             assert relerr(ax_g.cpu().numpy(), ax_o) < tol * 10, it
         assert abs(st.res_delta - r["res_delta"]) < 1e-7 * max(r["res_delta"], 1e-3)
     assert r["res_delta"] < 0.2
+
+
+@pytest.mark.parametrize("cfg,kw,acc,step,niter", [
+    (0, {}, 2, 2.0, 12),                                                   # Polyak, Listing 14 defaults, kappa = inf
+    (1, dict(pts_per_xi=5, n_angles=16, n_energies=24), 2, 0.3, 6),       # Polyak with induced A (small step: kappa = 2)
+    (1, dict(pts_per_xi=5, n_angles=16, n_energies=24), 3, 0.5, 8),       # CongAcc, Listing 16 defaults, induced A
+    (0, {}, 3, 0.5, 10),
+])
+def test_polyak_and_congacc_iterations_match(sc, cfg, kw, acc, step, niter):
+    """NEXT-2 accelerators (PAPER.md E6-E7 :1087-1089, E12-E17 :1134-1151) against the oracle's Accelerator."""
+    wl = wlmod.make_workload(cfg, **kw)
+    o = oracle.Oracle.from_workload(wl)
+    drv = oracle.Driver(o, wl.Aext_x, wl.Aext_y, wl.n_energies, accelerator=acc, step=step)
+    ctx = sc.ScContext.from_workload(wl)
+    ctx.sc_set_external_field(dev(wl.Aext_x), dev(wl.Aext_y))
+    d_g = dev(wl.delta0.astype(np.complex128)).clone()
+    ax_g = torch.zeros((wl.ny, wl.nx), dtype=torch.float64, device="cuda"); ay_g = torch.zeros_like(ax_g)
+    d_o = wl.delta0.copy(); ax_o = np.zeros((wl.ny, wl.nx)); ay_o = np.zeros((wl.ny, wl.nx))
+    wmax = 0.0
+    for it in range(niter):
+        r = drv.iterate(d_o, ax_o, ay_o)
+        d_o, ax_o, ay_o = r["delta"], r["Aind_x"], r["Aind_y"]
+        wmax = max(wmax, max(r["w"]))
+        st = ctx.sc_iterate(acc, step, False, d_g, ax_g, ay_g, want_stats=True)
+        torch.cuda.synchronize()
+        tol = TOL * max(1.0, 3.0 ** min(it, 6))        # rounding differences are amplified by the iteration map
+        assert relerr(d_g.cpu().numpy(), d_o) < tol, it
+        if wl.kappa > 0:
+            assert relerr(ax_g.cpu().numpy(), ax_o) < tol * 10, it
+        assert abs(st.res_delta - r["res_delta"]) < 1e-7 * max(r["res_delta"], 1e-3)
+    assert np.all(np.isfinite(d_o))
+    if acc == 3 and wl.kappa > 0:
+        assert wmax > 0.0                               # the E17 bisection was exercised (oscillating A component)
+
+
+def test_accelerator_argument_checks(sc):
+    wl = wlmod.make_workload(0)
+    ctx = sc.ScContext.from_workload(wl)
+    d = dev(wl.delta0.astype(np.complex128)).clone()
+    with pytest.raises(sc.ScError):
+        ctx.sc_iterate(4, 1.0, False, d)
+    with pytest.raises(sc.ScError):
+        ctx.sc_set_accelerator_params(drag=1.5)
+    with pytest.raises(sc.ScError):
+        ctx.sc_set_accelerator_params(step_min=10.0, step_max=1.0)
+    ctx.sc_set_accelerator_params(drag=1.0)             # drag = 1: Polyak forgets its velocity = Picard
+    d2 = d.clone()
+    c2 = sc.ScContext.from_workload(wl)
+    for _ in range(3):
+        ctx.sc_iterate(2, 0.7, False, d)
+        c2.sc_iterate(0, 0.7, False, d2)
+    torch.cuda.synchronize()
+    assert relerr(d.cpu().numpy(), d2.cpu().numpy()) < 1e-13

@@ -454,3 +454,93 @@ def test_abs_peak_at_110_wall_in_closed_grain():
     assert wl.mask[j, i]
     assert ld[j, i] > 5.0 * ld[c, c] and ld[c, c] < 1.0
     assert np.all(ld[wl.mask > 0] > 0)
+
+
+# ---- accelerators of App. E on fixed-point problems with known answers ---------------------------------
+def _run_linear(acc, lam, x0, xstar, n):
+    """iterate x <- x + acc.update(g(x) - x) for the linear map g(x) = x - lam (x - x*) (lam: per-element)."""
+    x = np.array(x0, float)
+    hist = [x.copy()]
+    for _ in range(n):
+        x = x + acc.update(-lam * (x - xstar))
+        hist.append(x.copy())
+    return np.array(hist)
+
+
+def test_accelerator_picard_geometric_rate():
+    # E5 (:1070): e_n = (1 - alpha lam)^n e_0
+    lam, xs = np.array([0.3, 0.9, 1.4]), np.array([1.0, -2.0, 0.5])
+    h = _run_linear(oracle.Accelerator(0, step=0.8), lam, [0, 0, 0], xs, 7)
+    assert np.allclose(h[7] - xs, (1 - 0.8 * lam) ** 7 * (0 - xs), rtol=1e-12, atol=1e-14)
+
+
+def test_accelerator_bb_is_the_secant_step_on_an_isotropic_problem():
+    # E8-E11 (:1107-1115): for g(x) = x - lam (x - x*) with one scalar lam, d_i - d_{i-1} = -lam alpha_i d_{i-1},
+    # so s^BB1 = s^BB2 = 1/(lam alpha_i) and alpha_{i+1} = 1/lam: the second update lands on x* exactly
+    xs = np.array([1.0, -2.0, 0.5, 3.0])
+    acc = oracle.Accelerator(1, step=1.0)
+    h = _run_linear(acc, 0.37, [0.2, 0.1, -1.0, 4.0], xs, 2)
+    assert abs(acc.alpha - 1 / 0.37) < 1e-12
+    assert np.max(np.abs(h[2] - xs)) < 1e-13
+    # the step size is clipped to [1e-3, 100] (Listing 15 :1121-1127)
+    acc = oracle.Accelerator(1, step=1.0)
+    _run_linear(acc, 1e-4, [0.2, 0.1], xs[:2], 2)
+    assert acc.alpha == 100.0
+
+
+def test_accelerator_polyak_two_term_recurrence():
+    # E6-E7 (:1087-1089) with v_0 = 0 on a scalar linear problem: eliminating v gives
+    # e_{n+1} = (2 - beta - alpha lam) e_n - (1 - beta) e_{n-1},  e_1 = (1 - alpha lam) e_0
+    al, be, lam = 2.0, 0.5, 0.21
+    h = _run_linear(oracle.Accelerator(2, step=al, drag=be), lam, [1.0], np.array([0.0]), 12)[:, 0]
+    e = [1.0, 1.0 - al * lam]
+    for n in range(1, 12):
+        e.append((2 - be - al * lam) * e[n] - (1 - be) * e[n - 1])
+    assert np.allclose(h, e, rtol=1e-12, atol=1e-15)
+    # closed form through the roots of r^2 - (2 - beta - alpha lam) r + (1 - beta) = 0
+    r = np.roots([1.0, -(2 - be - al * lam), 1 - be])
+    c = np.linalg.solve(np.array([[1, 1], [r[0], r[1]]]), np.array([e[0], e[1]], complex))
+    assert abs((c[0] * r[0] ** 12 + c[1] * r[1] ** 12).real - h[12]) < 1e-12
+    # drag = 1 forgets the velocity: Picard
+    hp = _run_linear(oracle.Accelerator(2, step=0.7, drag=1.0), lam, [1.0], np.array([0.0]), 5)[:, 0]
+    assert np.allclose(hp, (1 - 0.7 * lam) ** np.arange(6), rtol=1e-13)
+
+
+def test_accelerator_congacc_step_growth_and_clip():
+    # E12-E16 (:1134-1146) with a CONSTANT difference d (cos = 1 from the second iteration on, 0 at the first where
+    # m = 0): alpha_1 = alpha_0, alpha_{i+1} = alpha_i k, m = d  =>  x_n = x_0 + d alpha_0 (1 + k + ... + k^{n-1})
+    d = np.array([0.3, -0.2, 0.0, 1.0, 0.5, 0.5, -1.0, 2.0])
+    acc = oracle.Accelerator(3, step=0.5, step_factor=1.234, ncomp=4)
+    x = np.zeros(8)
+    for _ in range(6):
+        x = x + acc.update(d)
+    assert np.allclose(x, d * 0.5 * sum(1.234 ** i for i in range(6)), rtol=1e-13)
+    assert np.allclose(acc.alpha_c, 0.5 * 1.234 ** 5, rtol=1e-13) and acc.w_c == [0.0] * 4
+    for _ in range(40):
+        acc.update(d)
+    assert acc.alpha_c == [100.0] * 4                      # step_size_max (Listing 16 :1157)
+    # opposite direction: cos = -1, alpha shrinks by k per iteration (E13), down to step_size_min
+    acc = oracle.Accelerator(3, step=0.5, ncomp=1)
+    acc.update(np.array([1.0, 0.0])); a1 = acc.alpha_c[0]
+    acc.update(np.array([-1.0, 0.0]))
+    assert abs(acc.alpha_c[0] - a1 / 1.234) < 1e-15
+
+
+def test_accelerator_congacc_weight_solves_E17():
+    # E14, E17 (:1138-1149): m = (1,0), d = (0,1): cos(w m + (1-w) d, d) = (1-w)/sqrt(w^2 + (1-w)^2) = s_min
+    # => w* = 1/(1 + s_min/sqrt(1 - s_min^2))
+    for smin in (0.7, 0.3, 0.95):
+        acc = oracle.Accelerator(3, step=0.5, cos_min=smin, ncomp=1)
+        acc.update(np.array([1.0, 0.0]))                    # m_1 = d_0 = (1, 0), w_1 = 0
+        upd = acc.update(np.array([0.0, 1.0]))              # cos(m, d) = 0 < s_min -> w* from E17
+        wstar = 1.0 / (1.0 + smin / math.sqrt(1.0 - smin * smin))
+        assert abs(acc.w_c[0] - wstar) < 1e-14
+        m = np.array([wstar, 1.0 - wstar])
+        assert abs(m[1] / np.linalg.norm(m) - smin) < 1e-14     # the mixed direction has exactly the tolerated similarity
+        assert np.allclose(upd, acc.alpha_c[0] * m, rtol=1e-13)
+        assert abs(acc.alpha_c[0] - 0.5) < 1e-15            # k^0: cos(m, d) = 0 leaves the step size
+    # components are treated independently (E12 "component index c")
+    acc = oracle.Accelerator(3, step=0.5, ncomp=2)
+    acc.update(np.array([1.0, 0.0, 1.0, 0.0]))
+    acc.update(np.array([1.0, 0.0, 0.0, 1.0]))
+    assert acc.w_c[0] == 0.0 and acc.w_c[1] > 0.4 and abs(acc.alpha_c[0] - 0.5 * 1.234) < 1e-15
