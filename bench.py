@@ -203,8 +203,8 @@ def run_ours(a):
 
     dev_ax, dev_ay = dev(wl.Aext_x), dev(wl.Aext_y)
     # launches of OUR kernels per step: rotate_in, march, rotate_back (+ memset) ; A-solve: 3 reductions + 2x(pad, mul,
-    # crop) [+ 4 cuFFT library launches, not counted]; mixing: diff, 2x3 reduction stages, alpha, residual, update
-    launches_per_step = 3 if a.sweep_only else (3 + (3 + 6 if wl.kappa > 0 else 0) + (1 + 2 + 1 + 4 + 1 + 1))
+    # crop) [+ 4 cuFFT library launches, not counted]; mixing: diff, 2x3 reduction stages, alpha, increment, residual, update
+    launches_per_step = 3 if a.sweep_only else (3 + (3 + 6 if wl.kappa > 0 else 0) + (1 + 2 + 1 + 1 + 4 + 1 + 1))
 
     for _ in range(max(a.warmup, 3)):
         step()
