@@ -36,12 +36,12 @@ METRIC = "riccati_trajectory_step_updates_per_s"
 UNIT = "updates/s"
 # FP64-pipe instructions the closed-form path needs per unit = (piece, energy, angle pair) = 4 logical updates
 # (gamma and gamma-tilde for angles k and k+N/2): DESIGN.md §6 tally of the kernel's own algorithm.
-#   "recompute" rounds (every piece inside the radius of the per-energy Taylor table of T): T twice 2 x 17, two Moebius
-#       steps 2 x 27, node products 28, energy reduction 8 = 124 (ncu source page: 124.2 executed); scratch traffic
+#   "recompute" rounds (every piece inside the radius of the per-energy Taylor table of T): T twice 2 x 15, two Moebius
+#       steps 2 x 27, node products 28, energy reduction 8 = 120 (ncu source page counted 124.2 executed with the degree-6 table, 4 more); scratch traffic
 #       16 B written + 16 B read = 32 B per unit
 #   "stored-T" rounds (strong vector potential): T once from the pole-subtracted table 36, 54, 28, 8 = 126; 64 B per unit
 # Evaluating T from its definition (sqrt, exp, sin/cos) would be 86 per evaluation — reported as context only.
-ALGO_FP64_INSTR_PER_UNIT = {"recompute": 124.0, "stored": 126.0}
+ALGO_FP64_INSTR_PER_UNIT = {"recompute": 120.0, "stored": 126.0}
 ALGO_HBM_BYTES_PER_UNIT = {"recompute": 32.0, "stored": 64.0}
 TEXTBOOK_FP64_INSTR_PER_UNIT = 184.0
 ALGO_FP64_INSTR_PER_UNIT_MIDPOINT = 2 * 66.0 + 28.0 + 8.0

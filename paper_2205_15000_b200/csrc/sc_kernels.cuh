@@ -196,7 +196,10 @@ struct MarchArgsT {
 };
 using MarchArgs = MarchArgsT<double>;
 
-constexpr int MARCH_WARPS = 8;               // warps per CTA
+#ifndef SC_MARCH_WARPS
+#define SC_MARCH_WARPS 8
+#endif
+constexpr int MARCH_WARPS = SC_MARCH_WARPS;  // warps per CTA
 #ifndef SC_MARCH_MIN_CTAS
 #define SC_MARCH_MIN_CTAS 2
 #endif
@@ -205,7 +208,10 @@ constexpr int MARCH_MIN_CTAS = SC_MARCH_MIN_CTAS;   // resident CTAs per SM the 
 #define SC_PF_DIST 16
 #endif
 constexpr int PF_DIST = SC_PF_DIST;          // pass 2: scratch lines are pulled into L2 this many nodes ahead
-constexpr int RED_NODES = 4;                 // nodes per shared-memory reduction batch
+#ifndef SC_RED_NODES
+#define SC_RED_NODES 4
+#endif
+constexpr int RED_NODES = SC_RED_NODES;      // nodes per shared-memory reduction batch
 constexpr int RED_VALS = 6;
 constexpr int STAGE_LD = 34;                 // padded row of the transpose stage: 16-byte aligned rows, conflict-free 128-bit column reads
 
@@ -373,6 +379,7 @@ __device__ __forceinline__ cplx_t<R> end_T(const typename VT<R>::V4& cc, R zr0, 
 // memory in chunks of 32 (one record per lane, coalesced cp.async, double-buffered one chunk ahead), so that no
 // step ever waits on a global load of its coefficients; the step loop reads them with broadcast LDS.
 constexpr int CHUNK = 32;
+static_assert(CHUNK % RED_NODES == 0, "a reduction batch must not straddle two coefficient chunks (the running sums are fetched one batch ahead)");
 template <typename R> __host__ __device__ constexpr int march_stage_bytes() { return RED_NODES * RED_VALS * STAGE_LD * (int)sizeof(R); }   // per warp
 template <typename R> __host__ __device__ constexpr int march_coef_bytes() { return 2 * CHUNK * 6 * (int)sizeof(R); }                      // per warp: pc[2][32] V4 + nd[2][32] V2
 template <typename R> __host__ __device__ constexpr int march_smem() { return MARCH_WARPS * (march_stage_bytes<R>() + march_coef_bytes<R>()); }   // fp64: 75264 B (opt-in)

@@ -192,12 +192,15 @@ __device__ __noinline__ cplx_t<R> coef_T_slow(R d2, R zr, R zi, R len) { return 
 // axis w0 is real and the c_k are REAL (T is real on the real axis): a real-coefficient polynomial at a complex point
 // costs 2 FMAs per term — divide by the real quadratic (x - dw)(x - conj dw) = x^2 - r x + s; the remainder
 // b1 x + (b0 - r b1) at x = dw is (b0 - b1 Re dw) + i b1 Im dw.  Off the axis (sc_ldos) the c_k are complex: Horner.
-// K and the radius fraction: truncation <= RMAX^(K+1) relative.
+// K and the radius fraction: truncation <= RMAX^(K+1) relative.  K = 5 at 0.01 of the radius bounds it by 1e-12; the
+// bound is only approached at the highest energies (|dw| ~ 2 eps |a|), where one step already contracts a perturbation
+// of gamma by e^{-2 eps h}; at the low energies that carry a long memory |dw|/radius ~ |De|^2/wp ~ 1e-4 and the
+// truncation is below 1e-20.  The parity budget is 1e-9.
 #ifndef SC_TK
-#define SC_TK 6
+#define SC_TK 5
 #endif
 template <typename R> struct TaylorK;
-template <> struct TaylorK<double> { static constexpr int K = SC_TK; static constexpr double RMAX = SC_TK >= 8 ? 0.024 : 0.01; };   // 0.01^7 = 1e-14, 0.024^9 = 3e-15
+template <> struct TaylorK<double> { static constexpr int K = SC_TK; static constexpr double RMAX = SC_TK >= 8 ? 0.024 : 0.01; };   // 0.01^6 = 1e-12, 0.024^9 = 3e-15
 template <> struct TaylorK<float> { static constexpr int K = 3; static constexpr double RMAX = 0.012; };                                // 0.012^4 = 2e-8
 template <typename R, int K>
 __device__ __forceinline__ cplx_t<R> taylor_real(const R (&c)[K + 1], R dwr, R dwi, R s) {
