@@ -39,10 +39,12 @@ UNIT = "updates/s"
 #   "recompute" rounds (every piece inside the radius of the per-energy Taylor table of T): T twice 2 x 15, two Moebius
 #       steps 2 x 27, node products 28, energy reduction 8 = 120 (ncu source page counted 124.2 executed with the degree-6 table, 4 more); scratch traffic
 #       16 B written + 16 B read = 32 B per unit
+#   "recompute_pole" rounds (|a| beyond that table but inside the pole-subtracted one): T twice 2 x 24 (degree 5 + the
+#       pole term with one reciprocal), 54, 28, 8 = 138; 32 B per unit
 #   "stored-T" rounds (strong vector potential): T once from the pole-subtracted table 36, 54, 28, 8 = 126; 64 B per unit
 # Evaluating T from its definition (sqrt, exp, sin/cos) would be 86 per evaluation — reported as context only.
-ALGO_FP64_INSTR_PER_UNIT = {"recompute": 120.0, "stored": 126.0}
-ALGO_HBM_BYTES_PER_UNIT = {"recompute": 32.0, "stored": 64.0}
+ALGO_FP64_INSTR_PER_UNIT = {"recompute": 120.0, "recompute_pole": 138.0, "stored": 126.0}
+ALGO_HBM_BYTES_PER_UNIT = {"recompute": 32.0, "recompute_pole": 32.0, "stored": 64.0}
 TEXTBOOK_FP64_INSTR_PER_UNIT = 184.0
 ALGO_FP64_INSTR_PER_UNIT_MIDPOINT = 2 * 66.0 + 28.0 + 8.0
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE march launch at configs[4], fp64, closed-form stepper, all rounds in
@@ -226,7 +228,7 @@ def run_ours(a):
     ms = e0.elapsed_time(e1)
     clocks = sampler.stop()
     march_total_ms, march_launches = ctx.sc_debug_march_time()      # CUDA events around each march launch of the timed region
-    units_timed, units_timed_stored = ctx.sc_debug_march_units()     # units of those launches, and how many spilled T
+    units_timed, units_timed_stored, units_timed_pole = ctx.sc_debug_march_units()     # units of those launches, by mode
     if world > 1:                                   # device time of the slowest rank
         tmax = torch.tensor([ms], dtype=torch.float64, device=devname)
         dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
@@ -246,10 +248,10 @@ def run_ours(a):
     full_size = world == 1 and not (a.pts_per_xi or a.n_angles or a.n_energies or a.size_scale != 1.0)
     # algorithmic work of ONE average march launch of the timed region (units counted by the library, by mode)
     nl = max(march_launches, 1)
-    u_all = units_timed / nl; u_st = units_timed_stored / nl; u_rec = u_all - u_st
+    u_all = units_timed / nl; u_st = units_timed_stored / nl; u_pl = units_timed_pole / nl; u_rec = u_all - u_st - u_pl
     if a.stepper == 0:
-        instr = ALGO_FP64_INSTR_PER_UNIT["recompute"] * u_rec + ALGO_FP64_INSTR_PER_UNIT["stored"] * u_st
-        hbm = ALGO_HBM_BYTES_PER_UNIT["recompute"] * u_rec + ALGO_HBM_BYTES_PER_UNIT["stored"] * u_st
+        instr = sum(ALGO_FP64_INSTR_PER_UNIT[k] * u for k, u in (("recompute", u_rec), ("recompute_pole", u_pl), ("stored", u_st)))
+        hbm = sum(ALGO_HBM_BYTES_PER_UNIT[k] * u for k, u in (("recompute", u_rec), ("recompute_pole", u_pl), ("stored", u_st)))
     else:
         instr = ALGO_FP64_INSTR_PER_UNIT_MIDPOINT * u_all
         hbm = 32.0 * u_all
@@ -275,7 +277,7 @@ def run_ours(a):
                                            "tflops": 2.0 * TEXTBOOK_FP64_INSTR_PER_UNIT * u_all / (mk_ms * 1e-3) / 1e12},
                 "march_ms": mk_ms, "march_share_of_step": mk_ms / (ms / a.steps),
                 "algo_fp64_instr_per_unit": instr / max(u_all, 1.0), "units_per_launch": u_all,
-                "units_share_stored_T": u_st / max(u_all, 1.0),
+                "units_share_stored_T": u_st / max(u_all, 1.0), "units_share_recompute_pole_table": u_pl / max(u_all, 1.0),
                 "hbm_bytes_per_unit_algorithmic": hbm / max(u_all, 1.0),
                 "hbm_gbs_algorithmic": hbm / (mk_ms * 1e-3) / 1e9}
 

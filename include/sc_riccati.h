@@ -176,10 +176,11 @@ sc_status sc_debug_last_march_ms(sc_ctx* ctx, float* ms);
  * the timed steps themselves made.  Either output may be NULL (reset only). */
 sc_status sc_debug_march_time(sc_ctx* ctx, float* total_ms, int* n_launches);
 /* (piece, energy, angle pair) units marched by the full-work-list march launches since the previous call of this
- * function, and how many of them belonged to rounds that spilled the step coefficient T between the passes
- * (some piece outside the radius of the per-energy table: 64 B of scratch traffic per unit) rather than
- * re-evaluating it (32 B per unit); synchronises, then resets both.  Either output may be NULL. */
-sc_status sc_debug_march_units(sc_ctx* ctx, long long* units_total, long long* units_stored_T);
+ * function, and how many of them belonged to rounds that (i) spilled the step coefficient T between the passes
+ * (some piece outside the radii of the per-energy tables: 64 B of scratch traffic per unit), (ii) re-evaluated it in
+ * pass 2 from the pole-subtracted table; the rest re-evaluated it from the pole-free table (both 32 B per unit;
+ * DESIGN.md 4-6); synchronises, then resets.  Any output may be NULL. */
+sc_status sc_debug_march_units(sc_ctx* ctx, long long* units_total, long long* units_stored_T, long long* units_pole_table);
 
 const char* sc_last_error(const sc_ctx* ctx);
 const char* sc_version(void);

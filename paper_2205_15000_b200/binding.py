@@ -110,7 +110,7 @@ def load_library():
     L.sc_debug_last_march_ms.argtypes = [vp, C.POINTER(C.c_float)]
     L.sc_debug_fp64_peak_sustained.argtypes = [vp, d, C.POINTER(d)]
     L.sc_debug_march_time.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(i)]
-    L.sc_debug_march_units.argtypes = [vp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
+    L.sc_debug_march_units.argtypes = [vp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
     _lib = L
     return L
 
@@ -301,10 +301,11 @@ class ScContext:
         return ms.value, n.value
 
     def sc_debug_march_units(self):
-        """(units marched, units in rounds that spilled T) since the previous call; resets."""
-        a, b = C.c_longlong(), C.c_longlong()
-        self._check(self._L.sc_debug_march_units(self._h, C.byref(a), C.byref(b)))
-        return a.value, b.value
+        """(units marched, units in rounds that spilled T, units in rounds that recomputed T from the pole-subtracted
+        table) since the previous call; resets."""
+        a, b, c = C.c_longlong(), C.c_longlong(), C.c_longlong()
+        self._check(self._L.sc_debug_march_units(self._h, C.byref(a), C.byref(b), C.byref(c)))
+        return a.value, b.value, c.value
 
     def sc_debug_fp64_peak_sustained(self, seconds=2.0):
         a = C.c_double()

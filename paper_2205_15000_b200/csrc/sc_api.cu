@@ -411,8 +411,8 @@ sc_status sc_create(const sc_grid* grid, const unsigned char* mask, const sc_sha
     CU(ctx->d_ndD.alloc(nodes)); CU(ctx->d_nda.alloc(nodes)); CU(ctx->d_pc.alloc((size_t)(nodes + G) * 4 * ctx->rsz())); CU(ctx->d_pmax.alloc(G));
     if (ctx->f32) CU(ctx->d_ndDr.alloc(nodes));
     CU(ctx->d_part.alloc((size_t)nodes * sck::RED_VALS));
-    CU(ctx->d_counter.alloc(1)); CU(ctx->d_nbad.alloc(1)); CU(ctx->d_nstored.alloc(1));
-    CU(cudaMemsetAsync(ctx->d_nbad.p, 0, sizeof(int), s)); CU(cudaMemsetAsync(ctx->d_nstored.p, 0, sizeof(unsigned long long), s));
+    CU(ctx->d_counter.alloc(1)); CU(ctx->d_nbad.alloc(1)); CU(ctx->d_nstored.alloc(2));
+    CU(cudaMemsetAsync(ctx->d_nbad.p, 0, sizeof(int), s)); CU(cudaMemsetAsync(ctx->d_nstored.p, 0, 2 * sizeof(unsigned long long), s));
 
     // Matsubara energies eps_n = t(n+1/2) (:98), unit weights, self-partnered (z = i eps -> -conj z = z)
     EnergySet& E = ctx->mats;
@@ -748,12 +748,13 @@ sc_status sc_debug_march_time(sc_ctx* ctx, float* total_ms, int* n_launches) {
     return SC_OK;
 }
 
-sc_status sc_debug_march_units(sc_ctx* ctx, long long* units_total, long long* units_stored_T) {
+sc_status sc_debug_march_units(sc_ctx* ctx, long long* units_total, long long* units_stored_T, long long* units_pole_table) {
     if (!ctx) return SC_ERR_ARG;
     CU(cudaStreamSynchronize(ctx->stream));
-    unsigned long long ns = 0; CU(cudaMemcpy(&ns, ctx->d_nstored.p, sizeof(ns), cudaMemcpyDeviceToHost));
+    unsigned long long ns[2] = {0, 0}; CU(cudaMemcpy(ns, ctx->d_nstored.p, sizeof(ns), cudaMemcpyDeviceToHost));
     CU(cudaMemset(ctx->d_nstored.p, 0, sizeof(ns)));
-    if (units_stored_T) *units_stored_T = (long long)ns;
+    if (units_stored_T) *units_stored_T = (long long)ns[0];
+    if (units_pole_table) *units_pole_table = (long long)ns[1];
     if (units_total) *units_total = ctx->march_units;
     ctx->march_units = 0;
     return SC_OK;

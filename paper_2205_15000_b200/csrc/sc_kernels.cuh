@@ -192,7 +192,8 @@ struct MarchArgsT {
     double* ldos;                           // MODE 1: [node][ne] = Re g_n
     int* counter;
     double* stat_max2;                      // per warp slot: max |gamma|^2 seen (optional)
-    unsigned long long* n_stored;           // running count of (piece, energy) units marched by rounds that spilled T
+    unsigned long long* n_stored;           // [0] running count of (piece, energy) units marched by rounds that spilled T,
+                                            // [1] by rounds that re-evaluated T from the pole-subtracted table
 };
 using MarchArgs = MarchArgsT<double>;
 
@@ -348,20 +349,30 @@ struct TTab {
         return scm::coef_T_slow(scm::mad(cc.x, cc.x, cc.y * cc.y), zr0 + cc.z, zi0, len);
     }
 };
-// Pole-subtracted table (energies on the imaginary axis), for the rounds that spill T: three times the radius.
-template <typename R>
+// Pole-subtracted table (energies on the imaginary axis): three times the radius.  KC = TaylorPoleK (degree 8) for the
+// rounds that spill T (one warp vote per piece, exp-based evaluation outside the radius); KC = TaylorPoleShortK
+// (degree 5) for rounds that re-evaluate T in pass 2 and are known to be inside its radius.
+template <typename R, typename KC>
 struct TTabPole {
-    static constexpr int K = scm::TaylorPoleK<R>::K;
+    static constexpr int K = KC::K;
     static constexpr bool IMAG = true;
     R c[K + 1]; R thr2, pole_a, pole_res, m2zi;
     __device__ __forceinline__ void load(const EnergyDev& E, int n) {
         const double* row = E.tcp + (size_t)n * TCP_LD;
 #pragma unroll
         for (int k = 0; k <= K; ++k) c[k] = (R)row[k];
-        thr2 = (R)(row[9] * (scm::TaylorPoleK<R>::RMAX * scm::TaylorPoleK<R>::RMAX));
+        thr2 = (R)(row[9] * (KC::RMAX * KC::RMAX));
         pole_a = (R)row[10]; pole_res = (R)row[11]; m2zi = (R)(-2.0 * E.zi[n]);
     }
-    __device__ __forceinline__ cplx_t<R> fast(const typename VT<R>::V4& cc) const { return mk(R(0), R(0)); }   // unused
+    static __device__ __forceinline__ bool covers(const EnergyDev& E, int n, float2 pm) {
+        const R thr = (R)(E.tcp[(size_t)n * TCP_LD + 9] * (KC::RMAX * KC::RMAX));
+        const R br = (R)pm.x, bi = (R)(2.0 * E.zi[n]) * (R)pm.y;
+        return scm::mad(br, br, bi * bi) * R(1.001) <= thr;
+    }
+    __device__ __forceinline__ cplx_t<R> fast(const typename VT<R>::V4& cc) const {
+        const R dwr = cc.w, dwi = m2zi * cc.z;
+        return scm::taylor_pole<R, K>(c, pole_a, pole_res, dwr, dwi, scm::mad(dwr, dwr, dwi * dwi));
+    }
     __device__ __forceinline__ cplx_t<R> voted(const typename VT<R>::V4& cc, R zr0, R zi0, R len) const {
         const R dwr = cc.w, dwi = m2zi * cc.z;
         const R s2 = scm::mad(dwr, dwr, dwi * dwi);
@@ -615,7 +626,7 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32, MARCH_MIN_CTAS) march_kernel
     J.scr_w = A.scr + (size_t)slot * A.scr_stride;
     J.ne = A.E.ne; J.hlen = (R)A.h;
     R max2 = R(0);
-    unsigned long long nst = 0;
+    unsigned long long nst = 0, npl = 0;
 
     for (;;) {
         int item = 0;
@@ -632,16 +643,24 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32, MARCH_MIN_CTAS) march_kernel
 
         for (int n0 = 0; n0 < J.ne; n0 += 32) {
             const int n = min(n0 + J.lane, J.ne - 1);
-            // STEP 0: T is re-evaluated in pass 2 if every piece is inside the table's radius for all 32 lanes, else spilled
+            // STEP 0: T is re-evaluated in pass 2 if every piece is inside a table's radius for all 32 lanes, else spilled
             if (STEP == 0 && __any_sync(0xffffffffu, !TTab<R, TM>::covers(A.E, n, pm))) {
                 if constexpr (TM == 1) {
-                    TTabPole<R> tab; tab.load(A.E, n);
-                    march_round<MODE, STATS, STEP, R, true>(A, J, tab, n0, max2);
+                    using Short = TTabPole<R, scm::TaylorPoleShortK<R>>;
+                    if (!__any_sync(0xffffffffu, !Short::covers(A.E, n, pm))) {
+                        Short tab; tab.load(A.E, n);
+                        march_round<MODE, STATS, STEP, R, false>(A, J, tab, n0, max2);
+                        npl += (unsigned long long)(J.nn + 1) * min(32, J.ne - n0);
+                    } else {
+                        TTabPole<R, scm::TaylorPoleK<R>> tab; tab.load(A.E, n);
+                        march_round<MODE, STATS, STEP, R, true>(A, J, tab, n0, max2);
+                        nst += (unsigned long long)(J.nn + 1) * min(32, J.ne - n0);
+                    }
                 } else {
                     TTab<R, TM> tab; tab.load(A.E, n);
                     march_round<MODE, STATS, STEP, R, true>(A, J, tab, n0, max2);
+                    nst += (unsigned long long)(J.nn + 1) * min(32, J.ne - n0);
                 }
-                nst += (unsigned long long)(J.nn + 1) * min(32, J.ne - n0);
             } else {
                 TTab<R, TM> tab;
                 if (STEP == 0) tab.load(A.E, n);
@@ -656,6 +675,7 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32, MARCH_MIN_CTAS) march_kernel
         if (J.lane == 0) A.stat_max2[slot] = mx;
     }
     if (J.lane == 0 && nst) atomicAdd(A.n_stored, nst);
+    if (J.lane == 0 && npl) atomicAdd(A.n_stored + 1, npl);
 }
 
 // ------------------------------------------------------------------------------------------------

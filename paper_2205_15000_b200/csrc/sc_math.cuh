@@ -221,6 +221,11 @@ __device__ __forceinline__ cplx_t<R> taylor_real(const R (&c)[K + 1], R dwr, R d
 template <typename R> struct TaylorPoleK;
 template <> struct TaylorPoleK<double> { static constexpr int K = 8; static constexpr double RMAX = 0.012; };   // 0.012^9 = 5e-18
 template <> struct TaylorPoleK<float> { static constexpr int K = 4; static constexpr double RMAX = 0.03; };      // 0.03^5  = 2e-8
+// ... and a short version of it for rounds that re-evaluate T in pass 2 but whose |a| is beyond the pole-free table
+// (same truncation rule as TaylorK: RMAX^(K+1))
+template <typename R> struct TaylorPoleShortK;
+template <> struct TaylorPoleShortK<double> { static constexpr int K = 5; static constexpr double RMAX = 0.01; };   // 1e-12
+template <> struct TaylorPoleShortK<float> { static constexpr int K = 3; static constexpr double RMAX = 0.012; };
 template <typename R, int K>
 __device__ __forceinline__ cplx_t<R> taylor_pole(const R (&c)[K + 1], R pole_a, R pole_res, R dwr, R dwi, R s) {
     const R r = dwr + dwr;
