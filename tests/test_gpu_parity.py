@@ -170,12 +170,14 @@ def test_fp32_mode_parity(sc, cfg, kw, ns, stepper):
             assert np.max(np.abs(Gg - Go)) < TOL32 and np.max(np.abs(GTg - GTo)) < TOL32
 
 
-@pytest.mark.parametrize("amp", [0.3, 2.0, 12.0])
+@pytest.mark.parametrize("amp", [0.02, 0.3, 2.0, 12.0])
 def test_step_coefficient_table_and_fallback(sc, amp):
-    """The march evaluates T = tanh(Omega l)/Omega from a per-energy table where |De|^2 - a^2 - 2 i eps a is small
-    against the distance to the table's second pole, and from exp/sqrt elsewhere (trajectory ends, strong A, high
-    energies on coarse grids).  Vector potentials of 0.3 (inside the radius everywhere), 2 (mixed: the high-energy
-    lanes of a warp leave it) and 12 (outside everywhere) must all match the oracle, which knows neither path."""
+    """The march evaluates T = tanh(Omega l)/Omega from per-energy tables where |De|^2 - a^2 - 2 i eps a is small
+    against the distance to the table's nearest (or second) pole, and from exp/sqrt elsewhere (trajectory ends, strong
+    A, high energies on coarse grids); rounds inside a radius re-evaluate T in pass 2, the others spill it (DESIGN.md
+    §4).  Vector potentials of 0.02 (pole-free table), 0.3 (pole-subtracted table, still re-evaluated), 2 (spilled;
+    mixed: the high-energy lanes of a warp leave the radius) and 12 (outside everywhere) must all match the oracle,
+    which knows none of these paths."""
     wl = wlmod.make_workload(1, pts_per_xi=6, n_angles=16, n_energies=96)
     rng = np.random.default_rng(17)
     y, x = np.meshgrid((np.arange(wl.ny) - 0.5 * (wl.ny - 1)) * wl.h, (np.arange(wl.nx) - 0.5 * (wl.nx - 1)) * wl.h, indexing="ij")
@@ -184,6 +186,7 @@ def test_step_coefficient_table_and_fallback(sc, amp):
     o = oracle.Oracle.from_workload(wl)
     g = GpuRun(sc, wl)
     g.set_fields(wl.delta0, Ax, Ay)
+    g.ctx.sc_debug_march_units()
     stores = None
     for it in range(2):
         ro = o.sweep(wl.delta0, Ax, Ay, wl.n_energies, stores)
@@ -191,6 +194,12 @@ def test_step_coefficient_table_and_fallback(sc, amp):
         rg = g.sweep()
         for key in ("delta_new", "jx", "jy", "fe_I"):
             assert relerr(rg[key], ro[key]) < TOL, (amp, it, key, relerr(rg[key], ro[key]))
+    total, stored, pole = g.ctx.sc_debug_march_units()
+    assert total == 2 * (g.ctx.n_pieces // 2) * wl.n_energies and 0 <= stored + pole <= total
+    # which path the rounds took: pole-free table / pole-subtracted table (both recompute T) / spilled T
+    share = {0.02: (stored == 0 and pole < 0.2 * total), 0.3: (pole > 0.3 * total and stored < 0.2 * total),
+             2.0: (stored > 0.3 * total and pole > 0), 12.0: (stored > 0.8 * total)}[amp]
+    assert share, (amp, total, stored, pole)
 
 
 def test_coarse_grid_high_energies_leave_the_table(sc):
