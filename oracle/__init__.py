@@ -46,6 +46,7 @@ def lib():
         L.orc_create.argtypes = [C.c_int, C.c_int, C.c_double, C.c_void_p, C.POINTER(_Shape), C.c_int, C.c_double,
                                  C.c_int, C.c_double, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int]
         L.orc_destroy.argtypes = [C.c_void_p]
+        L.orc_set_components.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
         L.orc_error.restype = C.c_char_p
         L.orc_error.argtypes = [C.c_void_p]
         for f in ("orc_nrot", "orc_ntraj", "orc_n_gather_fallback"):
@@ -153,6 +154,24 @@ class Oracle:
         self.nrot = L.orc_nrot(self._h)
         self.ntraj = L.orc_ntraj(self._h)
         self.n_gather_fallback = L.orc_n_gather_fallback(self._h)
+        self.symmetries = [int(symmetry)]
+        self.tc_ratio = [1.0]
+        self.crystal_rotation = crystal_rotation
+
+    def set_components(self, symmetries, tc_ratio):
+        """Several order-parameter components (Eq. 1 :37, Listing 11 :909-926): Delta(p_F,R) = sum_G
+        Delta_G(R) eta_G(p_F), each with its own T_c^G = tc_ratio[G] * T_c in the gap equation (Eq. 20-22 :135-144;
+        T_c, the energy unit, is the largest).  Afterwards every Delta argument / Delta_new result is
+        [ncomp][ny][nx]."""
+        syms = np.ascontiguousarray(symmetries, np.int32)
+        assert len(syms) == len(tc_ratio) >= 1
+        lib().orc_set_components(self._h, len(syms), _p(syms))
+        self.symmetries = [int(v) for v in syms]
+        self.tc_ratio = [float(v) for v in tc_ratio]
+
+    @property
+    def ncomp(self):
+        return len(self.symmetries)
 
     @classmethod
     def from_workload(cls, wl, **kw):
@@ -199,7 +218,8 @@ class Oracle:
         g_old, gt_old = stores
         g_new = np.array(g_old, copy=True); gt_new = np.array(gt_old, copy=True)
         ny, nx = self.ny, self.nx
-        num = np.zeros((ny, nx), np.complex128)
+        assert delta.size == self.ncomp * ny * nx
+        num = np.zeros((ny, nx) if self.ncomp == 1 else (self.ncomp, ny, nx), np.complex128)
         Jx = np.zeros((ny, nx)); Jy = np.zeros((ny, nx)); Ia = np.zeros((ny, nx)); Ra = np.zeros((ny, nx))
         al = None if angle_list is None else np.ascontiguousarray(angle_list, np.int32)
         dbg = None
@@ -229,9 +249,13 @@ class Oracle:
             stores = self.reset_stores(delta, Ax, Ay, z)
         r = self.raw_sweep(delta, Ax, Ay, z, w, stores, angle_list, dbg_angle)
         t = self.t
-        D = matsubara_denominator(t, ne)
         m = self.mask.astype(bool)
-        r["delta_new"] = np.where(m, -2j * t * r["num"] / D, 0.0)
+        # Eq. 22 (:144): each component divides by its own ln(T/T_c^G) + sum 1/(n+1/2)
+        D = np.array([math.log(t / tc) + float(np.sum(1.0 / (np.arange(ne) + 0.5))) for tc in self.tc_ratio])
+        if self.ncomp == 1:
+            r["delta_new"] = np.where(m, -2j * t * r["num"] / D[0], 0.0)
+        else:
+            r["delta_new"] = np.where(m[None], -2j * t * r["num"] / D[:, None, None], 0.0)
         r["jx"] = np.where(m, 2.0 * self.sigma * t * r["Jx"], 0.0)
         r["jy"] = np.where(m, 2.0 * self.sigma * t * r["Jy"], 0.0)
         r["fe_I"] = np.where(m, t * r["I"], 0.0)
@@ -254,9 +278,25 @@ class Oracle:
     def free_energy_density(self, delta, ne, fe_I):
         """omega(R) of PAPER.md Eq. 17 (:120) without the magnetic term, Eilenberger form Eq. 19;
         |Delta(R)|^2 = <|Delta(p_F,R)|^2>_pF (:122) with the same Fermi-surface quadrature as the sweep."""
-        eta2 = sum(self.angle_info(k)[2] * self.angle_info(k)[1] ** 2 for k in range(self.n_angles))
-        d2 = eta2 * np.abs(delta) ** 2
-        return d2 * math.log(self.t) + d2 * float(np.sum(1.0 / (np.arange(ne) + 0.5))) - fe_I
+        if self.ncomp == 1:
+            eta2 = sum(self.angle_info(k)[2] * self.angle_info(k)[1] ** 2 for k in range(self.n_angles))
+            d2 = eta2 * np.abs(delta) ** 2
+            return d2 * math.log(self.t) + d2 * float(np.sum(1.0 / (np.arange(ne) + 0.5))) - fe_I
+        # Eq. 17 (:120): sum_G |Delta_G|^2 ln(T/T_c^G) + <|Delta(p_F,R)|^2> sum 1/(n+1/2) - I
+        delta = np.asarray(delta).reshape(self.ncomp, self.ny, self.nx)
+        d2 = np.zeros((self.ny, self.nx))
+        for k in range(self.n_angles):
+            W = self.angle_info(k)[2]
+            tot = sum(self.basis(s, k) * delta[c] for c, s in enumerate(self.symmetries))
+            d2 += W * np.abs(tot) ** 2
+        logs = sum(np.abs(delta[c]) ** 2 * math.log(self.t / tc) for c, tc in enumerate(self.tc_ratio))
+        return logs + d2 * float(np.sum(1.0 / (np.arange(ne) + 0.5))) - fe_I
+
+    def basis(self, sym, k):
+        """eta_G(phi_k) of Table III (:1238-1246) with the crystal-axes rotation (:890)."""
+        phi = 2.0 * math.pi * k / self.n_angles - 2.0 * math.pi * self.crystal_rotation
+        return {0: 1.0, 1: math.sqrt(2.0) * math.cos(2 * phi), 2: math.sqrt(2.0) * math.sin(2 * phi),
+                3: math.sqrt(2.0) * math.sin(4 * phi)}[sym]
 
     def debug_trajectory(self, delta, Ax, Ay, k, local, z, n, stores):
         z = _c128(z); ne = len(z)
@@ -389,14 +429,23 @@ class Driver:
             gAx, gAy = vector_potential(o.mask, o.h, o.kappa, r["jx"], r["jy"])
         else:
             gAx, gAy = np.zeros_like(Aind_x), np.zeros_like(Aind_y)
-        x = np.concatenate([delta.real.ravel(), delta.imag.ravel(), k2 * Aind_x.ravel(), k2 * Aind_y.ravel()])
-        gx = np.concatenate([r["delta_new"].real.ravel(), r["delta_new"].imag.ravel(), k2 * gAx.ravel(), k2 * gAy.ravel()])
-        xn = x + self.accel.update(gx - x)
+        # E3 (:1053): x = (Re Delta_G, Im Delta_G for every component G, kappa^2 A_x, kappa^2 A_y)
+        nc = o.ncomp
         n = o.nx * o.ny
+        dl = np.asarray(delta).reshape(nc, o.ny, o.nx); dn = np.asarray(r["delta_new"]).reshape(nc, o.ny, o.nx)
+        parts = lambda d_, ax_, ay_: np.concatenate([v for c in range(nc) for v in (d_[c].real.ravel(), d_[c].imag.ravel())] +
+                                                    [k2 * ax_.ravel(), k2 * ay_.ravel()])
+        x = parts(dl, Aind_x, Aind_y)
+        gx = parts(dn, gAx, gAy)
+        if self.accel.ncomp != 2 * nc + 2:
+            self.accel.ncomp = 2 * nc + 2
+            self.accel.alpha_c = [self.accel.alpha] * (2 * nc + 2); self.accel.w_c = [0.0] * (2 * nc + 2)
+        xn = x + self.accel.update(gx - x)
         shp = (o.ny, o.nx)
-        out["delta"] = (xn[:n] + 1j * xn[n:2 * n]).reshape(shp) * o.mask
+        dout = np.stack([(xn[2 * c * n:(2 * c + 1) * n] + 1j * xn[(2 * c + 1) * n:(2 * c + 2) * n]).reshape(shp) * o.mask for c in range(nc)])
+        out["delta"] = dout[0] if nc == 1 else dout
         if o.kappa > 0:
-            out["Aind_x"] = (xn[2 * n:3 * n] / k2).reshape(shp); out["Aind_y"] = (xn[3 * n:] / k2).reshape(shp)
+            out["Aind_x"] = (xn[2 * nc * n:(2 * nc + 1) * n] / k2).reshape(shp); out["Aind_y"] = (xn[(2 * nc + 1) * n:] / k2).reshape(shp)
         else:
             out["Aind_x"], out["Aind_y"] = Aind_x, Aind_y
         out["res_delta"] = residual(out["delta"], delta)

@@ -71,6 +71,9 @@ struct Ctx {
     int nrot; double c;
     std::vector<double> vx, vy, W;   // v_k = (vx,vy); n_k = (-vy, vx); quadrature weight
     std::vector<double> eta;         // eta_k (real for all Table III functions)
+    // several order-parameter components (Eq. 1 :37): Delta(p_F,R) = sum_G Delta_G(R) eta_G(p_F); syms.size() >= 1,
+    // syms[0] == sym.  The fields handed to the sweep are then [ncomp][ny][nx].
+    std::vector<int> syms;
     std::vector<std::vector<Traj>> traj;               // [k][local]
     std::vector<int> off;                              // global trajectory id offset per angle
     std::vector<std::vector<std::vector<int>>> line;   // [k][t] -> local trajectory indices
@@ -350,6 +353,16 @@ static double interp_plain(const Ctx& C, const double* F, double x, double y) {
 // ---------------------------------------------------------------------------------------------------
 // Homogeneous solution: Omega = sqrt(|De|^2 - z^2) principal branch (Re >= 0),
 // gamma_h = -De / (z + i Omega).
+// Delta(p_F, R) of Eq. 1 (:37) for the direction phi at the point (x, y): sum over the components of
+// eta_G(phi) times the masked-bilinear interpolant of Delta_G.  `bad` counts the point once.
+static cd gap_at(const Ctx& C, const cd* D, double phi, double x, double y, int* bad) {
+    const size_t ng = (size_t)C.nx * C.ny;
+    cd s = 0.0;
+    for (size_t c = 0; c < C.syms.size(); ++c)
+        s += basis(C.syms[c], phi, C.rot) * interp_delta(C, D + c * ng, x, y, c == 0 ? bad : nullptr);
+    return s;
+}
+
 static inline cd omega_of(cd De, cd z) { return std::sqrt(cd(std::norm(De), 0.0) - z * z); }
 static inline cd gamma_h(cd De, cd z) { return -De / (z + I_ * omega_of(De, z)); }
 
@@ -411,7 +424,7 @@ static void make_pieces(const Ctx& C, const Traj& T, const cd* D, const double* 
     for (int m = 0; m < nn; ++m) {
         double u = lattice_u(C, T.jf + m);
         double x = u * C.vx[k] + w * nx, y = u * C.vy[k] + w * ny;
-        P.Dn[m] = C.eta[k] * interp_delta(C, D, x, y, bad);
+        P.Dn[m] = gap_at(C, D, 2.0 * PI * k / C.nphi, x, y, bad);
         P.an[m] = C.sigma * (C.vx[k] * interp_plain(C, Ax, x, y) + C.vy[k] * interp_plain(C, Ay, x, y));
     }
     P.M = nn + 1; P.len.resize(P.M); P.a.resize(P.M); P.De.resize(P.M);
@@ -433,7 +446,7 @@ static cd start_gamma(const Ctx& C, const Traj& T, const Pieces& P, const cd* D,
     int k = T.k; double w = lattice_u(C, T.t);
     double x = T.u_in * C.vx[k] - w * C.vy[k], y = T.u_in * C.vy[k] + w * C.vx[k];
     double phi = std::atan2(g.diry, g.dirx);
-    cd De = basis(C.sym, phi, C.rot) * interp_delta(C, D, x, y, nullptr);
+    cd De = gap_at(C, D, phi, x, y, nullptr);
     double a = C.sigma * (g.dirx * interp_plain(C, Ax, x, y) + g.diry * interp_plain(C, Ay, x, y));
     return gamma_h(De, z0 + a);
 }
@@ -446,7 +459,7 @@ static cd start_gammat(const Ctx& C, const Traj& T, const Pieces& P, const cd* D
     int k = T.k; double w = lattice_u(C, T.t);
     double x = T.u_out * C.vx[k] - w * C.vy[k], y = T.u_out * C.vy[k] + w * C.vx[k];
     double phi = std::atan2(g.diry, g.dirx);
-    cd De = basis(C.sym, phi, C.rot) * interp_delta(C, D, x, y, nullptr);
+    cd De = gap_at(C, D, phi, x, y, nullptr);
     double a = C.sigma * (g.dirx * interp_plain(C, Ax, x, y) + g.diry * interp_plain(C, Ay, x, y));
     return gamma_h(-std::conj(De), z0 + a);
 }
@@ -474,9 +487,14 @@ void* orc_create(int nx, int ny, double h, const unsigned char* mask, const orc_
         double x = (i - 0.5 * (nx - 1)) * h, y = (j - 0.5 * (ny - 1)) * h;
         if ((bool)mask[(size_t)j * nx + i] != inside_csg(C->shapes, x, y)) { C->err = "mask disagrees with shapes"; return C; }
     }
+    C->syms.assign(1, symmetry);
     build_tables(*C);
     return C;
 }
+// Several order-parameter components (Eq. 1 :37, Listing 11 :909-926): syms[0..n-1]; afterwards every Delta
+// argument is [n][ny][nx] and orc_sweep's num is [n][ny][nx] (num_G = sum_k W_k conj(eta_G,k) SF_k, Eq. 22 :144).
+void orc_set_components(void* p, int n, const int* syms) { ((Ctx*)p)->syms.assign(syms, syms + n); }
+int orc_ncomp(void* p) { return (int)((Ctx*)p)->syms.size(); }
 void orc_destroy(void* p) { delete (Ctx*)p; }
 const char* orc_error(void* p) { return ((Ctx*)p)->err.c_str(); }
 int orc_nrot(void* p) { return ((Ctx*)p)->nrot; }
@@ -579,7 +597,9 @@ int orc_sweep(void* p, const double* delta, const double* Ax, const double* Ay,
     std::vector<int> angles;
     if (angle_list) angles.assign(angle_list, angle_list + n_angle_list);
     else for (int k = 0; k < C->nphi; ++k) angles.push_back(k);
-    for (size_t q = 0; q < ng; ++q) { num[2 * q] = num[2 * q + 1] = 0.0; Jx[q] = Jy[q] = Iacc[q] = Racc[q] = 0.0; }
+    const size_t ncomp = C->syms.size();
+    for (size_t q = 0; q < 2 * ng * ncomp; ++q) num[q] = 0.0;
+    for (size_t q = 0; q < ng; ++q) { Jx[q] = Jy[q] = Iacc[q] = Racc[q] = 0.0; }
     double gmin = 1e300; long long nupd = 0; int bad = 0;
 #pragma omp parallel for ordered schedule(dynamic, 1) reduction(min : gmin) reduction(+ : nupd, bad)
     for (int ia = 0; ia < (int)angles.size(); ++ia) {
@@ -627,8 +647,10 @@ int orc_sweep(void* p, const double* delta, const double* Ax, const double* Ay,
                 if (!rotate_back_weights(*C, valid, k, x, y, idx, w, &n)) { ++bad; continue; }
                 cd F = 0.0; double Gv = 0.0, Iv = 0.0, Rv = 0.0;
                 for (int s = 0; s < n; ++s) { F += w[s] * SF[idx[s]]; Gv += w[s] * SG[idx[s]]; Iv += w[s] * SI[idx[s]]; Rv += w[s] * SR[idx[s]]; }
-                cd c = C->W[k] * C->eta[k] * F;           // eta real: conj(eta_k) = eta_k
-                num[2 * q] += c.real(); num[2 * q + 1] += c.imag();
+                for (size_t cc = 0; cc < ncomp; ++cc) {      // eta real: conj(eta_G,k) = eta_G,k
+                    cd c = C->W[k] * basis(C->syms[cc], 2.0 * PI * k / C->nphi, C->rot) * F;
+                    num[2 * (cc * ng + q)] += c.real(); num[2 * (cc * ng + q) + 1] += c.imag();
+                }
                 Jx[q] += C->W[k] * C->vx[k] * Gv; Jy[q] += C->W[k] * C->vy[k] * Gv;
                 Iacc[q] += C->W[k] * Iv; Racc[q] += C->W[k] * Rv;
             }

@@ -544,3 +544,58 @@ def test_accelerator_congacc_weight_solves_E17():
     acc.update(np.array([1.0, 0.0, 1.0, 0.0]))
     acc.update(np.array([1.0, 0.0, 0.0, 1.0]))
     assert acc.w_c[0] == 0.0 and acc.w_c[1] > 0.4 and abs(acc.alpha_c[0] - 0.5 * 1.234) < 1e-15
+
+
+# ---- several order-parameter components (Eq. 1 :37, Eq. 20-22 :135-144, Listing 11 :909-926) --------------------
+@pytest.mark.parametrize("Ds,Dd,tc_s", [(0.05, 0.20, 0.6), (0.05j, 0.20, 0.6), (0.18 * np.exp(0.4j), 0.07 * np.exp(-1.1j), 1.0)])
+def test_two_component_uniform_gap_closed_form(Ds, Dd, tc_s):
+    """Uniform Delta_s + Delta_d eta_d in an axis-aligned square ([100] walls: eta_s and eta_{dx2-y2} are both invariant
+    under the specular reflections, so every start value stays the homogeneous solution): f/pi = Delta(phi)/Lambda_n(phi)
+    with Delta(phi) = Delta_s + Delta_d sqrt2 cos 2phi, hence Delta_new,G = t sum_n <eta_G Delta/Lambda_n> / (ln(T/T_c^G)
+    + sum 1/(n+1/2)) exactly on the discrete angle set — pins the sum over components at the nodes, the projection
+    on each eta_G and each component's own T_c in the denominator.  d + s, d + is, and a general relative phase."""
+    n, h, t, ne, nphi = 12, 0.1, 0.3, 24, 32
+    shapes = [square(n * h)]
+    mask = make_mask(shapes, n, n, h)
+    tc = [tc_s, 1.0] if tc_s < 1.0 else [1.0, 0.5]
+    o = oracle.Oracle(n, n, h, mask, shapes, t, 0, nphi)
+    o.set_components([0, 1], tc)
+    delta = np.stack([np.full((n, n), Ds, complex), np.full((n, n), Dd, complex)])
+    r = o.sweep(delta, None, None, ne)
+    eps = t * (np.arange(ne) + 0.5)
+    num = np.zeros(2, complex)
+    for k in range(nphi):
+        phi = 2 * np.pi * k / nphi
+        W = o.angle_info(k)[2]
+        eta = np.array([1.0, np.sqrt(2.0) * np.cos(2 * phi)])
+        Dphi = Ds * eta[0] + Dd * eta[1]
+        num += W * eta * Dphi * t * np.sum(1.0 / np.sqrt(eps ** 2 + abs(Dphi) ** 2))
+    for c in range(2):
+        expect = num[c] / (np.log(t / tc[c]) + np.sum(1.0 / (np.arange(ne) + 0.5)))
+        assert np.max(np.abs(r["delta_new"][c] - expect)) < 1e-13, c
+    assert np.max(np.abs(r["jx"])) < 1e-14 and np.max(np.abs(r["jy"])) < 1e-14
+    # free energy (Eq. 17 :120 with Eq. 19): sum_G |D_G|^2 ln(T/T_c^G) + <|Delta(phi)|^2> sum 1/(n+1/2) - I, and
+    # I = t sum_n <2 |Delta(phi)|^2/(eps_n + Lambda_n)> for the homogeneous solution (Eq. 38's integrand)
+    fe = o.free_energy_density(delta, ne, r["fe_I"])
+    ref = abs(Ds) ** 2 * np.log(t / tc[0]) + abs(Dd) ** 2 * np.log(t / tc[1])
+    for k in range(nphi):
+        phi = 2 * np.pi * k / nphi
+        W = o.angle_info(k)[2]
+        d2 = abs(Ds + Dd * np.sqrt(2.0) * np.cos(2 * phi)) ** 2
+        L = np.sqrt(eps ** 2 + d2)
+        ref += W * (d2 * np.sum(1.0 / (np.arange(ne) + 0.5)) - t * np.sum(2.0 * d2 / (eps + L)))
+    assert np.max(np.abs(fe[mask > 0] - ref)) < 1e-13
+
+
+def test_second_component_with_zero_amplitude_changes_nothing():
+    """Delta_2 = 0: the first component's Delta_new, j, I equal the one-component sweep bit for bit (the node gap is
+    the same sum), and the projection on the second basis function is what a one-component run cannot see."""
+    wl = wlmod.make_workload(1, pts_per_xi=4, n_angles=16, n_energies=12)
+    o1 = oracle.Oracle.from_workload(wl)
+    r1 = o1.sweep(wl.delta0, wl.Aext_x, wl.Aext_y, wl.n_energies)
+    o2 = oracle.Oracle.from_workload(wl)
+    o2.set_components([wl.symmetry, 2], [1.0, 0.3])
+    d2 = np.stack([wl.delta0, np.zeros_like(wl.delta0)])
+    r2 = o2.sweep(d2, wl.Aext_x, wl.Aext_y, wl.n_energies)
+    assert np.array_equal(r2["delta_new"][0], r1["delta_new"]) and np.array_equal(r2["jx"], r1["jx"]) and np.array_equal(r2["fe_I"], r1["fe_I"])
+    assert np.max(np.abs(r2["delta_new"][1])) > 1e-6        # a vortex + walls do induce a d_xy admixture
