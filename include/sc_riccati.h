@@ -79,9 +79,19 @@ sc_status sc_create(const sc_grid* grid, const unsigned char* mask, const sc_sha
                     double T_over_Tc, double kappa, sc_symmetry symmetry, const sc_opts* opts, sc_ctx** out);
 sc_status sc_destroy(sc_ctx* ctx);
 
-/* Set Delta(R) (dev, complex fp64 [ny][nx]) and the TOTAL vector potential A = A_ext + A_ind (dev fp64
+/* Set Delta(R) (dev, complex fp64 [ny][nx]; [n][ny][nx] after sc_set_components) and the TOTAL vector potential A = A_ext + A_ind (dev fp64
  * [ny][nx] each; NULL = 0).  Copies into context-owned buffers; does not touch the boundary stores. */
 sc_status sc_set_fields(sc_ctx* ctx, const void* delta, const double* Ax, const double* Ay);
+
+/* Several order-parameter components (Eq. 1 :37, Listing 11 :909-926): Delta(p_F,R) = sum_G Delta_G(R) eta_G(p_F)
+ * with basis functions symmetries[0..n-1] (Table III :1238) and critical temperatures T_c^G = tc_ratio[G] * T_c
+ * (host arrays; T_c, the energy unit, is the largest: 0 < tc_ratio <= 1), 1 <= n <= 4.  Each component obeys its own gap
+ * equation (Eq. 22 :144 with ln(T/T_c^G)).  Afterwards EVERY order-parameter buffer of the ABI (sc_set_fields' delta,
+ * sc_riccati_sweep's delta_new, sc_iterate's delta_inout) is complex fp64 [n][ny][nx], and sc_iterate mixes
+ * x = (Re D_0, Im D_0, ..., kappa^2 A_x, kappa^2 A_y) (E3 :1053; 2n + 2 CongAcc components).  Call it after sc_create
+ * and before sc_set_fields: it invalidates the fields, the boundary stores and the driver state.  sc_create's single
+ * symmetry is the n = 1 case.  SC_ERR_ARG if n, a symmetry or a ratio is out of range. */
+sc_status sc_set_components(sc_ctx* ctx, int n, const sc_symmetry* symmetries, const double* tc_ratio);
 
 /* Replace the Matsubara table by any energies z_n = z_re + i z_im (Im z > 0) with weights w_n (host, n values):
  * Ozaki poles (:207, reading R-A4), or ONE SHARD of the Matsubara energies when the sweep is split by energy across
@@ -93,7 +103,8 @@ sc_status sc_set_energies(sc_ctx* ctx, const double* z_re, const double* z_im, c
 
 /* Energy-sharded sweeps: with a hook set, sc_riccati_sweep (and sc_iterate) write the five un-finalised
  * accumulators sum_k W_k {Re, Im conj(eta_k) SF_k, v_kx SG_k, v_ky SG_k, SI_k} of this context's energies into
- * acc (dev fp64 [5][ny][nx], caller-owned), call fn(user) on the host — which must enqueue, on the context's
+ * acc (dev fp64 [5][ny][nx], caller-owned; with n order-parameter components [2n+3][ny][nx]: Re, Im per component,
+ * then the current and I terms), call fn(user) on the host — which must enqueue, on the context's
  * stream, the sum of acc over all shards (one all-reduce) — and then apply Eq. 22 / Eq. 8 / Eq. 19 to the summed
  * accumulators.  fn = NULL, acc = NULL removes the hook. */
 typedef void (*sc_allreduce_fn)(void* user);

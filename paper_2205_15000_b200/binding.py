@@ -94,6 +94,7 @@ def load_library():
     L.sc_set_fields.argtypes = [vp, vp, vp, vp]
     L.sc_reset_boundary.argtypes = [vp]
     L.sc_set_energies.argtypes = [vp, vp, vp, vp, i, d]
+    L.sc_set_components.argtypes = [vp, i, vp, vp]
     L.sc_set_allreduce_hook.argtypes = [vp, vp, ALLREDUCE_FN, vp]
     L.sc_riccati_sweep.argtypes = [vp, vp, vp, vp, vp, C.POINTER(_Stats)]
     L.sc_ldos.argtypes = [vp, vp, i, d, i, vp, C.POINTER(_Stats)]
@@ -147,6 +148,7 @@ class ScContext:
         self._L = L
         self.nx, self.ny, self.h, self.t, self.kappa = nx, ny, h, t, kappa
         self.n_angles, self.n_matsubara = n_angles, n_matsubara
+        self.n_components = 1
         self.device = torch.device("cuda", device)
         mask = np.ascontiguousarray(mask, np.uint8)
         arr = (_Shape * len(shapes))()
@@ -198,9 +200,16 @@ class ScContext:
             raise ScError(rc, self._L.sc_last_error(self._h).decode())
 
     # ---- the calls of include/sc_riccati.h -------------------------------------------------------
+    def sc_set_components(self, symmetries, tc_ratio):
+        sy = np.ascontiguousarray(symmetries, np.int32); tc = np.ascontiguousarray(tc_ratio, np.float64)
+        if len(sy) != len(tc):
+            raise ScError(1, "symmetries and tc_ratio differ in length")
+        self._check(self._L.sc_set_components(self._h, len(sy), sy.ctypes.data_as(C.c_void_p), tc.ctypes.data_as(C.c_void_p)))
+        self.n_components = len(sy)
+
     def sc_set_fields(self, delta, Ax=None, Ay=None):
         n = self.nx * self.ny
-        self._check(self._L.sc_set_fields(self._h, _dev_ptr(delta, "c128", n), _dev_ptr(Ax, "f64", n), _dev_ptr(Ay, "f64", n)))
+        self._check(self._L.sc_set_fields(self._h, _dev_ptr(delta, "c128", self.n_components * n), _dev_ptr(Ax, "f64", n), _dev_ptr(Ay, "f64", n)))
 
     def sc_set_energies(self, z, w, denominator_sum=float("nan")):
         z = np.ascontiguousarray(z, np.complex128)
@@ -209,13 +218,13 @@ class ScContext:
                                             w.ctypes.data_as(C.c_void_p), len(zr), float(denominator_sum)))
 
     def sc_set_allreduce_hook(self, acc, fn):
-        """acc: CUDA fp64 tensor [5][ny][nx]; fn(): enqueues the all-reduce of acc on the context's stream."""
+        """acc: CUDA fp64 tensor [2 n_components + 3][ny][nx]; fn(): enqueues the all-reduce of acc on the context's stream."""
         if fn is None:
             self._hook = None
             self._check(self._L.sc_set_allreduce_hook(self._h, None, ALLREDUCE_FN(), None))
             return
         self._hook = (ALLREDUCE_FN(lambda user: fn()), acc)          # keep the callback and the buffer alive
-        self._check(self._L.sc_set_allreduce_hook(self._h, _dev_ptr(acc, "f64", 5 * self.nx * self.ny), self._hook[0], None))
+        self._check(self._L.sc_set_allreduce_hook(self._h, _dev_ptr(acc, "f64", (2 * self.n_components + 3) * self.nx * self.ny), self._hook[0], None))
 
     def sc_reset_boundary(self):
         self._check(self._L.sc_reset_boundary(self._h))
@@ -223,7 +232,7 @@ class ScContext:
     def sc_riccati_sweep(self, delta_new=None, jx=None, jy=None, fe_I=None, want_stats=False):
         n = self.nx * self.ny
         st = _Stats()
-        self._check(self._L.sc_riccati_sweep(self._h, _dev_ptr(delta_new, "c128", n), _dev_ptr(jx, "f64", n),
+        self._check(self._L.sc_riccati_sweep(self._h, _dev_ptr(delta_new, "c128", self.n_components * n), _dev_ptr(jx, "f64", n),
                                              _dev_ptr(jy, "f64", n), _dev_ptr(fe_I, "f64", n),
                                              C.byref(st) if want_stats else None))
         return _stats(st) if want_stats else None
@@ -250,7 +259,7 @@ class ScContext:
     def sc_iterate(self, accelerator, step, burnin, delta, Aind_x=None, Aind_y=None, want_stats=False):
         n = self.nx * self.ny
         st = _Stats()
-        self._check(self._L.sc_iterate(self._h, accelerator, step, int(burnin), _dev_ptr(delta, "c128", n),
+        self._check(self._L.sc_iterate(self._h, accelerator, step, int(burnin), _dev_ptr(delta, "c128", self.n_components * n),
                                        _dev_ptr(Aind_x, "f64", n), _dev_ptr(Aind_y, "f64", n),
                                        C.byref(st) if want_stats else None))
         return _stats(st) if want_stats else None

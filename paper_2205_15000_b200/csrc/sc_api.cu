@@ -114,6 +114,7 @@ struct sc_ctx {
     sc_opts opt{};
     sc_grid grid{};
     double t = 0, kappa = -1; int sym = 0;
+    int ncomp = 1; int syms[sck::MAX_COMP] = {0, 0, 0, 0}; double tc_ratio[sck::MAX_COMP] = {1, 1, 1, 1};   // Eq. 1 :37 components
     cudaStream_t stream = nullptr;
     int n_sm = 148;
     scgeo::Geometry geo;
@@ -128,7 +129,7 @@ struct sc_ctx {
     DevBuf<unsigned char> d_mask, d_ga_n;
     DevBuf<int> d_ga_idx; DevBuf<double> d_ga_w;
     // fallback rows
-    std::vector<int> fb_rows;
+    std::vector<int> fb_rows; std::vector<double> fb_phi;      // mirrored direction of every fallback row
     DevBuf<int> d_fb_rows; DevBuf<double> d_fb_px, d_fb_py, d_fb_dx, d_fb_dy, d_fb_eta;
     DevBuf<double2> d_fb_D; DevBuf<double> d_fb_a;
     // fields
@@ -161,7 +162,7 @@ sc_status fail(sc_ctx* c, sc_status s, const std::string& m) { if (c) c->err = m
 
 sck::GridDev grid_dev(const sc_ctx* c) {
     return sck::GridDev{c->grid.nx, c->grid.ny, c->grid.h, c->d_mask.p, c->d_delta.p,
-                        c->have_A ? c->d_Ax.p : nullptr, c->have_A ? c->d_Ay.p : nullptr};
+                        c->have_A ? c->d_Ax.p : nullptr, c->have_A ? c->d_Ay.p : nullptr, c->ncomp};
 }
 sck::TrajDev traj_dev(const sc_ctx* c) {
     return sck::TrajDev{c->G, c->d_k.p, c->d_t.p, c->d_jf.p, c->d_nn.p, c->d_l0.p, c->d_l1.p, c->d_noff.p, c->d_dF.p, c->d_dB.p};
@@ -183,11 +184,11 @@ sc_status ensure_nodes(sc_ctx* ctx) {
     const int wpb = 8;
     if (ctx->f32)
         sck::rotate_in_kernel<float><<<(ctx->G + wpb - 1) / wpb, wpb * 32, 0, ctx->stream>>>(
-            grid_dev(ctx), traj_dev(ctx), ctx->d_vx.p, ctx->d_vy.p, ctx->d_eta.p, ctx->geo.c, ctx->opt.charge_sign,
+            grid_dev(ctx), traj_dev(ctx), ctx->d_vx.p, ctx->d_vy.p, ctx->d_eta.p, ctx->geo.nphi, ctx->geo.c, ctx->opt.charge_sign,
             ctx->d_ndD.p, ctx->d_nda.p, ctx->d_ndDr.p, (float4*)ctx->d_pc.p, ctx->d_pmax.p, ctx->d_nbad.p);
     else
         sck::rotate_in_kernel<double><<<(ctx->G + wpb - 1) / wpb, wpb * 32, 0, ctx->stream>>>(
-            grid_dev(ctx), traj_dev(ctx), ctx->d_vx.p, ctx->d_vy.p, ctx->d_eta.p, ctx->geo.c, ctx->opt.charge_sign,
+            grid_dev(ctx), traj_dev(ctx), ctx->d_vx.p, ctx->d_vy.p, ctx->d_eta.p, ctx->geo.nphi, ctx->geo.c, ctx->opt.charge_sign,
             ctx->d_ndD.p, ctx->d_nda.p, nullptr, (double4*)ctx->d_pc.p, ctx->d_pmax.p, ctx->d_nbad.p);
     if (!ctx->fb_rows.empty()) {
         const int n = (int)ctx->fb_rows.size();
@@ -273,7 +274,7 @@ sck::BackArgs back_args(sc_ctx* ctx, void* delta_new, double* jx, double* jy, do
     B.vx = ctx->d_vx.p; B.vy = ctx->d_vy.p; B.eta = ctx->d_eta.p; B.W = ctx->d_W.p;
     B.line_g = ctx->d_line_g.p; B.line_n = ctx->d_line_n.p; B.T = traj_dev(ctx); B.part = ctx->d_part.p;
     B.t = ctx->t; B.sigma = ctx->opt.charge_sign;
-    B.D = std::log(ctx->t) + ctx->denom_sum;
+    for (int c = 0; c < sck::MAX_COMP; ++c) B.D[c] = std::log(ctx->t / ctx->tc_ratio[c]) + ctx->denom_sum;
     B.delta_new = (double2*)delta_new; B.jx = jx; B.jy = jy; B.feI = feI; B.n_bad = ctx->d_nbad.p;
     return B;
 }
@@ -317,6 +318,7 @@ sc_status sc_create(const sc_grid* grid, const unsigned char* mask, const sc_sha
     if (opts->precision != 64 && opts->precision != 32 && opts->precision != 0) return fail(ctx, SC_ERR_ARG, "precision must be 64 or 32");
     if (opts->stepper != 0 && opts->stepper != 1) return fail(ctx, SC_ERR_ARG, "stepper must be 0 (closed form) or 1 (implicit mid-point)");
     ctx->opt = *opts; ctx->grid = *grid; ctx->t = T_over_Tc; ctx->kappa = kappa; ctx->sym = (int)symmetry;
+    ctx->ncomp = 1; ctx->syms[0] = (int)symmetry; ctx->tc_ratio[0] = 1.0;
     ctx->f32 = opts->precision == 32;
     if (ctx->opt.charge_sign == 0) ctx->opt.charge_sign = -1;
     // ---- geometry (host) ----
@@ -378,7 +380,8 @@ sc_status sc_create(const sc_grid* grid, const unsigned char* mask, const sc_sha
             ctx->fb_rows.push_back(d);
             fpx.push_back(D.u_in * Gm.vx[D.k] - w * Gm.vy[D.k]); fpy.push_back(D.u_in * Gm.vy[D.k] + w * Gm.vx[D.k]);
             fdx.push_back(D.mdir[0]); fdy.push_back(D.mdir[1]);
-            feta.push_back(scgeo::eta_of(ctx->sym, std::atan2(D.mdir[1], D.mdir[0]), opts->crystal_rotation));
+            ctx->fb_phi.push_back(std::atan2(D.mdir[1], D.mdir[0]));
+            feta.push_back(scgeo::eta_of(ctx->sym, ctx->fb_phi.back(), opts->crystal_rotation));
         }
     }
 
@@ -445,13 +448,36 @@ sc_status sc_destroy(sc_ctx* ctx) {
 sc_status sc_set_fields(sc_ctx* ctx, const void* delta, const double* Ax, const double* Ay) {
     if (!ctx || !delta) return fail(ctx, SC_ERR_ARG, "null argument");
     const size_t ng = (size_t)ctx->grid.nx * ctx->grid.ny;
-    CU(cudaMemcpyAsync(ctx->d_delta.p, delta, ng * sizeof(double2), cudaMemcpyDeviceToDevice, ctx->stream));
+    CU(cudaMemcpyAsync(ctx->d_delta.p, delta, ctx->ncomp * ng * sizeof(double2), cudaMemcpyDeviceToDevice, ctx->stream));
     ctx->have_A = Ax && Ay;
     if (ctx->have_A) {
         CU(cudaMemcpyAsync(ctx->d_Ax.p, Ax, ng * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
         CU(cudaMemcpyAsync(ctx->d_Ay.p, Ay, ng * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
     }
     ctx->have_fields = true; ctx->nodes_fresh = false;
+    return SC_OK;
+}
+
+sc_status sc_set_components(sc_ctx* ctx, int n, const sc_symmetry* symmetries, const double* tc_ratio) {
+    if (!ctx || !symmetries || !tc_ratio) return fail(ctx, SC_ERR_ARG, "null argument");
+    if (n < 1 || n > sck::MAX_COMP) return fail(ctx, SC_ERR_ARG, "1 <= n_components <= 4");
+    const int N = ctx->geo.nphi; const size_t ng = (size_t)ctx->grid.nx * ctx->grid.ny, nfb = ctx->fb_rows.size();
+    std::vector<double> eta((size_t)n * N), feta((size_t)n * nfb);
+    for (int c = 0; c < n; ++c) {
+        if ((int)symmetries[c] < 0 || (int)symmetries[c] > 3) return fail(ctx, SC_ERR_ARG, "unknown symmetry");
+        if (!(tc_ratio[c] > 0) || tc_ratio[c] > 1.0) return fail(ctx, SC_ERR_ARG, "tc_ratio must lie in (0, 1]: T_c is the largest T_c^G");
+        for (int k = 0; k < N; ++k) eta[(size_t)c * N + k] = scgeo::eta_of((int)symmetries[c], 2.0 * scgeo::kPi * k / N, ctx->opt.crystal_rotation);
+        for (size_t i = 0; i < nfb; ++i) feta[c * nfb + i] = scgeo::eta_of((int)symmetries[c], ctx->fb_phi[i], ctx->opt.crystal_rotation);
+    }
+    CU(cudaStreamSynchronize(ctx->stream));
+    ctx->ncomp = n;
+    for (int c = 0; c < sck::MAX_COMP; ++c) { ctx->syms[c] = c < n ? (int)symmetries[c] : 0; ctx->tc_ratio[c] = c < n ? tc_ratio[c] : 1.0; }
+    ctx->sym = ctx->syms[0];
+    CU(ctx->d_eta.upload(eta, ctx->stream)); CU(ctx->d_fb_eta.upload(feta, ctx->stream));
+    CU(ctx->d_delta.alloc(n * ng));
+    CU(cudaStreamSynchronize(ctx->stream));
+    ctx->have_fields = false; ctx->nodes_fresh = false; ctx->stores_valid = false;
+    scf::release_driver(ctx->fs);                      // the iterate's length changes with the number of components
     return SC_OK;
 }
 
@@ -507,7 +533,8 @@ sc_status sc_riccati_sweep(sc_ctx* ctx, void* delta_new, double* jx, double* jy,
         // energy-sharded sweep: the caller sums the raw accumulators of all shards on this stream, then a7 runs
         ctx->hook_fn(ctx->hook_user);
         const size_t ng = (size_t)ctx->grid.nx * ctx->grid.ny;
-        sck::finalise_kernel<<<(unsigned)((ng + 255) / 256), 256, 0, ctx->stream>>>(ng, ctx->hook_acc, ctx->t, B.D, ctx->opt.charge_sign,
+        sck::FinArgs FA; for (int c = 0; c < sck::MAX_COMP; ++c) FA.D[c] = B.D[c];
+        sck::finalise_kernel<<<(unsigned)((ng + 255) / 256), 256, 0, ctx->stream>>>(ng, ctx->ncomp, ctx->hook_acc, ctx->t, FA, ctx->opt.charge_sign,
                                                                                   (double2*)delta_new, jx, jy, fe_I);
         CU(cudaGetLastError());
     }
@@ -608,7 +635,7 @@ sc_status sc_iterate(sc_ctx* ctx, int accelerator, double step, int burnin, void
     const int nx = ctx->grid.nx, ny = ctx->grid.ny; const size_t ng = (size_t)nx * ny;
     const bool withA = ctx->kappa > 0 && Aix && Aiy;
     std::string e;
-    if (int rc = scf::ensure_driver(ctx->fs, ng, e)) return fail(ctx, rc == 2 ? SC_ERR_NOMEM : SC_ERR_CUDA, e);
+    if (int rc = scf::ensure_driver(ctx->fs, ng, ctx->ncomp, e)) return fail(ctx, rc == 2 ? SC_ERR_NOMEM : SC_ERR_CUDA, e);
     if (stats) CU(cudaEventRecord(ctx->ev0, ctx->stream));
     // total A = A_ext + A_ind
     scf::FieldState& F = ctx->fs;

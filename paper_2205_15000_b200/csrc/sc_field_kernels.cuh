@@ -20,7 +20,9 @@ namespace scf {
 
 constexpr int RED_BLOCKS = 296;
 constexpr int RED_THREADS = 256;
-constexpr int RED_MAXOUT = 12;      // outputs of one reduction (CongAcc: 3 dot products x 4 components)
+constexpr int NX_MAX = 10;          // slices of the iterate x: (Re, Im) of up to 4 order-parameter components + kappa^2 A_x, A_y
+constexpr int RED_MAXOUT = 3 * NX_MAX;   // outputs of one reduction (CongAcc: 3 dot products per slice)
+constexpr int ST_ALPHA = 8, ST_W = 24;   // offsets of alpha_c and w_c in the device state array
 constexpr int RED_RES = RED_BLOCKS * RED_MAXOUT;   // offset of the results behind the partials
 
 // parameters of the accelerators (PAPER.md Listings 14-16 :1093, :1121, :1157)
@@ -33,19 +35,27 @@ struct FieldState {
     cufftDoubleComplex* Ghat = nullptr; double* pad = nullptr; cufftDoubleComplex* spec = nullptr;
     double* red = nullptr;          // RED_BLOCKS * RED_MAXOUT partials + 32 results
     // driver
-    size_t ng = 0;
+    size_t ng = 0; int nc = 1;      // grid points, order-parameter components (x has 2 nc + 2 slices of ng)
     double *Atot_x = nullptr, *Atot_y = nullptr, *jx = nullptr, *jy = nullptr, *feI = nullptr, *gAx = nullptr, *gAy = nullptr;
     double2* dnew = nullptr;
-    double* d_prev = nullptr;       // 4*ng
-    double* d_cur = nullptr;        // 4*ng
+    double* d_prev = nullptr;       // (2 nc + 2) * ng
+    double* d_cur = nullptr;        // (2 nc + 2) * ng
     double *prev_jx = nullptr, *prev_jy = nullptr, *prev_fe = nullptr;
-    double* upd = nullptr;          // 4*ng: x_{i+1} - x_i
-    double* aux = nullptr;          // 4*ng: Polyak velocity v / CongAcc moving average m (allocated on first use)
-    double* state = nullptr;        // [0] alpha, [1] iteration index, [2..5] residuals (delta, A, j, fe), [6..9] alpha_c, [10..13] w_c
+    double* upd = nullptr;          // (2 nc + 2) * ng: x_{i+1} - x_i
+    double* aux = nullptr;          // same size: Polyak velocity v / CongAcc moving average m (allocated on first use)
+    double* state = nullptr;        // [0] alpha, [1] iteration index, [2..5] residuals (delta, A, j, fe), [ST_ALPHA..] alpha_c, [ST_W..] w_c
     AccelParams par;
     bool driver = false, first = true; int last_kind = -1;
 };
 
+// driver buffers only (the number of order-parameter components changed); keeps the FFT plans and the G table
+inline void release_driver(FieldState& F) {
+    void** ptrs[] = {(void**)&F.Atot_x, (void**)&F.Atot_y, (void**)&F.jx, (void**)&F.jy, (void**)&F.feI, (void**)&F.gAx, (void**)&F.gAy,
+                     (void**)&F.dnew, (void**)&F.d_prev, (void**)&F.d_cur, (void**)&F.prev_jx, (void**)&F.prev_jy, (void**)&F.prev_fe,
+                     (void**)&F.state, (void**)&F.upd, (void**)&F.aux};
+    for (void** p : ptrs) { if (*p) cudaFree(*p); *p = nullptr; }
+    F.driver = false; F.first = true; F.last_kind = -1;
+}
 inline void release(FieldState& F) {
     if (F.plans) { cufftDestroy(F.plan_f); cufftDestroy(F.plan_b); }
     void* ptrs[] = {F.Ghat, F.pad, F.spec, F.red, F.Atot_x, F.Atot_y, F.jx, F.jy, F.feI, F.gAx, F.gAy, F.dnew,
@@ -133,7 +143,7 @@ inline int ensure_vp(FieldState& F, int nx, int ny, double h, cudaStream_t s, st
     SCF_CU(cudaMalloc((void**)&F.pad, (size_t)px * py * sizeof(double)));
     SCF_CU(cudaMalloc((void**)&F.spec, nspec * sizeof(cufftDoubleComplex)));
     SCF_CU(cudaMalloc((void**)&F.Ghat, nspec * sizeof(cufftDoubleComplex)));
-    if (!F.red) SCF_CU(cudaMalloc((void**)&F.red, (RED_RES + 32) * sizeof(double)));
+    if (!F.red) SCF_CU(cudaMalloc((void**)&F.red, (RED_RES + 64) * sizeof(double)));
     SCF_FFT(cufftPlan2d(&F.plan_f, py, px, CUFFT_D2Z));
     SCF_FFT(cufftPlan2d(&F.plan_b, py, px, CUFFT_Z2D));
     SCF_FFT(cufftSetStream(F.plan_f, s)); SCF_FFT(cufftSetStream(F.plan_b, s));
@@ -187,16 +197,17 @@ inline int vector_potential(FieldState& F, int nx, int ny, double h, const unsig
 }
 
 // ---- driver ---------------------------------------------------------------------------------------
-inline int ensure_driver(FieldState& F, size_t ng, std::string& err) {
+inline int ensure_driver(FieldState& F, size_t ng, int nc, std::string& err) {
     if (F.driver) return 0;
-    F.ng = ng;
+    F.ng = ng; F.nc = nc;
+    const size_t nx = (size_t)(2 * nc + 2) * ng;
     double** bufs[] = {&F.Atot_x, &F.Atot_y, &F.jx, &F.jy, &F.feI, &F.gAx, &F.gAy, &F.prev_jx, &F.prev_jy, &F.prev_fe};
     for (double** b : bufs) { SCF_CU(cudaMalloc((void**)b, ng * sizeof(double))); SCF_CU(cudaMemset(*b, 0, ng * sizeof(double))); }
-    SCF_CU(cudaMalloc((void**)&F.dnew, ng * sizeof(double2)));
-    SCF_CU(cudaMalloc((void**)&F.d_prev, 4 * ng * sizeof(double))); SCF_CU(cudaMalloc((void**)&F.d_cur, 4 * ng * sizeof(double)));
-    SCF_CU(cudaMalloc((void**)&F.upd, 4 * ng * sizeof(double)));
-    SCF_CU(cudaMalloc((void**)&F.state, 16 * sizeof(double))); SCF_CU(cudaMemset(F.state, 0, 16 * sizeof(double)));
-    if (!F.red) SCF_CU(cudaMalloc((void**)&F.red, (RED_RES + 32) * sizeof(double)));
+    SCF_CU(cudaMalloc((void**)&F.dnew, nc * ng * sizeof(double2)));
+    SCF_CU(cudaMalloc((void**)&F.d_prev, nx * sizeof(double))); SCF_CU(cudaMalloc((void**)&F.d_cur, nx * sizeof(double)));
+    SCF_CU(cudaMalloc((void**)&F.upd, nx * sizeof(double)));
+    SCF_CU(cudaMalloc((void**)&F.state, 64 * sizeof(double))); SCF_CU(cudaMemset(F.state, 0, 64 * sizeof(double)));
+    if (!F.red) SCF_CU(cudaMalloc((void**)&F.red, (RED_RES + 64) * sizeof(double)));
     F.driver = true; F.first = true;
     return 0;
 }
@@ -211,14 +222,17 @@ inline void add_fields(double* ox, double* oy, const double* ax, const double* a
     add_fields_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(n, ox, oy, ax, ay, bx, by);
 }
 
-// d = g(x) - x for the concatenated iterate
-__global__ void diff_kernel(size_t ng, const double2* delta, const double2* dnew, const double* aix, const double* aiy,
+// d = g(x) - x for the concatenated iterate x = (Re D_0, Im D_0, ..., Re D_{nc-1}, Im D_{nc-1}, kappa^2 A_x, kappa^2 A_y) (E3 :1053)
+__global__ void diff_kernel(size_t ng, int nc, const double2* delta, const double2* dnew, const double* aix, const double* aiy,
                             const double* gax, const double* gay, double k2, int withA, double* d) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= ng) return;
-    d[i] = dnew[i].x - delta[i].x; d[ng + i] = dnew[i].y - delta[i].y;
-    d[2 * ng + i] = withA ? k2 * (gax[i] - aix[i]) : 0.0;
-    d[3 * ng + i] = withA ? k2 * (gay[i] - aiy[i]) : 0.0;
+    for (int c = 0; c < nc; ++c) {
+        d[(2 * c) * ng + i] = dnew[c * ng + i].x - delta[c * ng + i].x;
+        d[(2 * c + 1) * ng + i] = dnew[c * ng + i].y - delta[c * ng + i].y;
+    }
+    d[(2 * nc) * ng + i] = withA ? k2 * (gax[i] - aix[i]) : 0.0;
+    d[(2 * nc + 1) * ng + i] = withA ? k2 * (gay[i] - aiy[i]) : 0.0;
 }
 struct DotOp {     // c = 0: dp.dd, 1: dp.dp, 2: dd.dd, with dd = d - dp
     const double* d; const double* dp;
@@ -229,7 +243,7 @@ struct DotOp {     // c = 0: dp.dd, 1: dp.dp, 2: dd.dd, with dd = d - dp
 };
 // state[0] = alpha, state[1] = iteration index i (reading R-BB: i starts at 0, first update uses alpha = step)
 __global__ void alpha_kernel(double* state, const double* dots, int accelerator, double step, int first, AccelParams P) {
-    if (first) { state[0] = step; state[1] = 0.0; for (int c = 0; c < 4; ++c) { state[6 + c] = step; state[10 + c] = 0.0; } }
+    if (first) { state[0] = step; state[1] = 0.0; for (int c = 0; c < NX_MAX; ++c) { state[ST_ALPHA + c] = step; state[ST_W + c] = 0.0; } }
     const int i = (int)state[1];
     if (accelerator == 1 && i >= 1) {
         const double dot = fabs(dots[0]);
@@ -239,8 +253,8 @@ __global__ void alpha_kernel(double* state, const double* dots, int accelerator,
     } else if (accelerator != 1) state[0] = step;
     state[1] = i + 1;
 }
-// CongAcc (E12-E17 :1134-1151): dots of component c = {m.m, m.d, d.d}[c]; one thread per component
-struct CongDotOp {   // output c = 3 * component + {0: m.m, 1: m.d, 2: d.d}; i runs over one component (ng values)
+// CongAcc (E12-E17 :1134-1151): dots of slice c = {m.m, m.d, d.d}[c]; one thread per slice
+struct CongDotOp {   // output c = 3 * slice + {0: m.m, 1: m.d, 2: d.d}; i runs over one slice (ng values)
     size_t ng; const double* m; const double* d;
     __device__ double operator()(size_t i, int c) const {
         const size_t q = (size_t)(c / 3) * ng + i;
@@ -253,44 +267,44 @@ __device__ inline double cong_cos_mix(double w, double mm, double md, double dd)
     const double n2 = w * w * mm + 2.0 * w * (1.0 - w) * md + (1.0 - w) * (1.0 - w) * dd;
     return (n2 > 0 && dd > 0) ? num / sqrt(n2 * dd) : 1.0;
 }
-// runs after alpha_kernel (state[1] already holds i + 1)
-__global__ void congacc_kernel(double* state, const double* dots, AccelParams P) {
+// runs after alpha_kernel (state[1] already holds i + 1); one thread per slice of x
+__global__ void congacc_kernel(double* state, const double* dots, int nslice, AccelParams P) {
     const int c = threadIdx.x;
-    if (c >= 4) return;
+    if (c >= nslice) return;
     const int i = (int)state[1] - 1;
     const double mm = dots[3 * c], md = dots[3 * c + 1], dd = dots[3 * c + 2];
     const double s = (mm > 0 && dd > 0) ? md / sqrt(mm * dd) : 0.0;            // E12
-    state[6 + c] = fmin(fmax(state[6 + c] * pow(P.kfac, s), P.amin), P.amax);   // E13
-    if (i == 0) state[10 + c] = 0.0;                                            // w_0 = 0 (:1151)
+    state[ST_ALPHA + c] = fmin(fmax(state[ST_ALPHA + c] * pow(P.kfac, s), P.amin), P.amax);   // E13
+    if (i == 0) state[ST_W + c] = 0.0;                                          // w_0 = 0 (:1151)
     else if (s < P.smin) {                                                      // E14, E17 by bisection
         double lo = 0.0, hi = 1.0;
         for (int it = 0; it < 60; ++it) {
             const double mid = 0.5 * (lo + hi);
             if (cong_cos_mix(mid, mm, md, dd) >= P.smin) lo = mid; else hi = mid;
         }
-        state[10 + c] = 0.5 * (lo + hi);
+        state[ST_W + c] = 0.5 * (lo + hi);
     }
 }
 // the increment x_{i+1} - x_i: alpha d (Picard E5, BB E11); v <- (1 - drag) v + alpha d (Polyak E6-E7);
 // m_c <- w_c m_c + (1 - w_c) d_c, alpha_c m_c (CongAcc E15-E16)
-__global__ void step_kernel(size_t ng, int accelerator, const double* d, double* aux, const double* state, double drag, double* upd) {
+__global__ void step_kernel(size_t ng, int nslice, int accelerator, const double* d, double* aux, const double* state, double drag, double* upd) {
     const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (q >= 4 * ng) return;
+    if (q >= nslice * ng) return;
     if (accelerator == 2) { const double v = (1.0 - drag) * aux[q] + state[0] * d[q]; aux[q] = v; upd[q] = v; }
     else if (accelerator == 3) {
         const int c = (int)(q / ng);
-        const double w = state[10 + c];
+        const double w = state[ST_W + c];
         const double m = w * aux[q] + (1.0 - w) * d[q];
-        aux[q] = m; upd[q] = state[6 + c] * m;
+        aux[q] = m; upd[q] = state[ST_ALPHA + c] * m;
     } else upd[q] = state[0] * d[q];
 }
-struct NormOp {    // c: 0 |dx_delta|^2, 1 |x_delta|^2, 2 |dx_A|^2, 3 |x_A|^2 (before the update)
-    size_t ng; const double2* delta; const double* aix; const double* aiy; const double* u; double k2; int withA;
+struct NormOp {    // c: 0 |dx_delta|^2, 1 |x_delta|^2, 2 |dx_A|^2, 3 |x_A|^2 (before the update); delta = all components
+    size_t ng; int nc; const double2* delta; const double* aix; const double* aiy; const double* u; double k2; int withA;
     __device__ double operator()(size_t i, int c) const {
-        if (c == 0) return u[i] * u[i] + u[ng + i] * u[ng + i];
-        if (c == 1) return delta[i].x * delta[i].x + delta[i].y * delta[i].y;
+        if (c == 0) { double s = 0.0; for (int g = 0; g < 2 * nc; ++g) s += u[g * ng + i] * u[g * ng + i]; return s; }
+        if (c == 1) { double s = 0.0; for (int g = 0; g < nc; ++g) s += delta[g * ng + i].x * delta[g * ng + i].x + delta[g * ng + i].y * delta[g * ng + i].y; return s; }
         if (!withA) return 0.0;
-        if (c == 2) return (u[2 * ng + i] * u[2 * ng + i] + u[3 * ng + i] * u[3 * ng + i]) / (k2 * k2);
+        if (c == 2) return (u[(2 * nc) * ng + i] * u[(2 * nc) * ng + i] + u[(2 * nc + 1) * ng + i] * u[(2 * nc + 1) * ng + i]) / (k2 * k2);
         return aix[i] * aix[i] + aiy[i] * aiy[i];
     }
 };
@@ -309,43 +323,46 @@ __global__ void residual_kernel(double* state, const double* n1, const double* n
     state[4] = n2[1] > 0 ? sqrt(n2[0] / n2[1]) : sqrt(n2[0]);
     state[5] = n2[3] > 0 ? sqrt(n2[2] / n2[3]) : sqrt(n2[2]);
 }
-__global__ void update_kernel(size_t ng, double2* delta, double* aix, double* aiy, const double* u,
+__global__ void update_kernel(size_t ng, int nc, double2* delta, double* aix, double* aiy, const double* u,
                               const unsigned char* mask, double k2, int withA) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= ng) return;
     const double m = mask[i] ? 1.0 : 0.0;
-    delta[i] = make_double2(m * (delta[i].x + u[i]), m * (delta[i].y + u[ng + i]));
-    if (withA) { aix[i] += u[2 * ng + i] / k2; aiy[i] += u[3 * ng + i] / k2; }
+    for (int c = 0; c < nc; ++c)
+        delta[c * ng + i] = make_double2(m * (delta[c * ng + i].x + u[(2 * c) * ng + i]), m * (delta[c * ng + i].y + u[(2 * c + 1) * ng + i]));
+    if (withA) { aix[i] += u[(2 * nc) * ng + i] / k2; aiy[i] += u[(2 * nc + 1) * ng + i] / k2; }
 }
 
 inline int mix(FieldState& F, int accelerator, double step, double kappa, bool withA, double2* delta, double* aix, double* aiy,
                const unsigned char* mask, size_t ng, cudaStream_t s, std::string& err) {
     const double k2 = withA ? kappa * kappa : 0.0;
-    const unsigned nb = (unsigned)((ng + 255) / 256), nb4 = (unsigned)((4 * ng + 255) / 256);
+    const int nc = F.nc, nslice = 2 * nc + 2;
+    const size_t nxl = (size_t)nslice * ng;
+    const unsigned nb = (unsigned)((ng + 255) / 256), nbx = (unsigned)((nxl + 255) / 256);
     double* res = F.red + RED_RES;
     if (accelerator != F.last_kind) F.first = true;         // a change of method restarts it (v_0 = 0, w_0 = 0, m_0 = 0)
     if (accelerator >= 2) {
-        if (!F.aux) SCF_CU(cudaMalloc((void**)&F.aux, 4 * ng * sizeof(double)));
-        if (F.first) SCF_CU(cudaMemsetAsync(F.aux, 0, 4 * ng * sizeof(double), s));
+        if (!F.aux) SCF_CU(cudaMalloc((void**)&F.aux, nxl * sizeof(double)));
+        if (F.first) SCF_CU(cudaMemsetAsync(F.aux, 0, nxl * sizeof(double), s));
     }
-    diff_kernel<<<nb, 256, 0, s>>>(ng, delta, F.dnew, aix, aiy, F.gAx, F.gAy, k2, withA ? 1 : 0, F.d_cur);
+    diff_kernel<<<nb, 256, 0, s>>>(ng, nc, delta, F.dnew, aix, aiy, F.gAx, F.gAy, k2, withA ? 1 : 0, F.d_cur);
     if (!F.first && accelerator == 1) {
-        reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(4 * ng, DotOp{F.d_cur, F.d_prev}, F.red, 3);
+        reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(nxl, DotOp{F.d_cur, F.d_prev}, F.red, 3);
         reduce_stage2<<<1, 32, 0, s>>>(F.red, 3, res);
     }
     alpha_kernel<<<1, 1, 0, s>>>(F.state, res, accelerator, step, F.first ? 1 : 0, F.par);
     if (accelerator == 3) {
-        reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, CongDotOp{ng, F.aux, F.d_cur}, F.red, 12);
-        reduce_stage2<<<1, 32, 0, s>>>(F.red, 12, res + 16);
-        congacc_kernel<<<1, 4, 0, s>>>(F.state, res + 16, F.par);
+        reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, CongDotOp{ng, F.aux, F.d_cur}, F.red, 3 * nslice);
+        reduce_stage2<<<1, 32, 0, s>>>(F.red, 3 * nslice, res + 16);
+        congacc_kernel<<<1, 32, 0, s>>>(F.state, res + 16, nslice, F.par);
     }
-    step_kernel<<<nb4, 256, 0, s>>>(ng, accelerator, F.d_cur, F.aux, F.state, F.par.drag, F.upd);
-    reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, NormOp{ng, delta, aix, aiy, F.upd, k2, withA ? 1 : 0}, F.red, 4);
+    step_kernel<<<nbx, 256, 0, s>>>(ng, nslice, accelerator, F.d_cur, F.aux, F.state, F.par.drag, F.upd);
+    reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, NormOp{ng, nc, delta, aix, aiy, F.upd, k2, withA ? 1 : 0}, F.red, 4);
     reduce_stage2<<<1, 32, 0, s>>>(F.red, 4, res + 4);
     reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, ObsNormOp{F.jx, F.jy, F.feI, F.prev_jx, F.prev_jy, F.prev_fe}, F.red, 4);
     reduce_stage2<<<1, 32, 0, s>>>(F.red, 4, res + 8);
     residual_kernel<<<1, 1, 0, s>>>(F.state, res + 4, res + 8);
-    update_kernel<<<nb, 256, 0, s>>>(ng, delta, aix, aiy, F.upd, mask, k2 > 0 ? k2 : 1.0, withA ? 1 : 0);
+    update_kernel<<<nb, 256, 0, s>>>(ng, nc, delta, aix, aiy, F.upd, mask, k2 > 0 ? k2 : 1.0, withA ? 1 : 0);
     SCF_CU(cudaMemcpyAsync(F.prev_jx, F.jx, ng * sizeof(double), cudaMemcpyDeviceToDevice, s));
     SCF_CU(cudaMemcpyAsync(F.prev_jy, F.jy, ng * sizeof(double), cudaMemcpyDeviceToDevice, s));
     SCF_CU(cudaMemcpyAsync(F.prev_fe, F.feI, ng * sizeof(double), cudaMemcpyDeviceToDevice, s));

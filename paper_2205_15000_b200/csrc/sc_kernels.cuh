@@ -30,10 +30,12 @@ __device__ __forceinline__ float2 mk2(float a, float b) { return make_float2(a, 
 __device__ __forceinline__ double4 mk4(double a, double b, double c, double d) { return make_double4(a, b, c, d); }
 __device__ __forceinline__ float4 mk4(float a, float b, float c, float d) { return make_float4(a, b, c, d); }
 
+constexpr int MAX_COMP = 4;        // order-parameter components Delta_G (Eq. 1 :37)
 struct GridDev {
     int nx, ny; double h;
     const unsigned char* mask;
-    const double2* delta; const double* Ax; const double* Ay;   // Ax/Ay may be null
+    const double2* delta; const double* Ax; const double* Ay;   // delta: [ncomp][ny][nx]; Ax/Ay may be null
+    int ncomp;
 };
 
 struct TrajDev {                 // physical trajectories (angles k < N/2), struct of arrays
@@ -56,7 +58,7 @@ struct EnergyDev { int ne; const double* zr; const double* zi; const double* w; 
 // ------------------------------------------------------------------------------------------------
 // masked bilinear interpolation of Delta (R5) and plain bilinear of A at a point
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ bool interp_delta(const GridDev& G, double x, double y, double& dr, double& di) {
+__device__ __forceinline__ bool interp_delta(const GridDev& G, const double2* __restrict__ F, double x, double y, double& dr, double& di) {
     const double gx = x / G.h + 0.5 * (G.nx - 1), gy = y / G.h + 0.5 * (G.ny - 1);
     const int i0 = (int)floor(gx), j0 = (int)floor(gy);
     const double fx = gx - i0, fy = gy - j0;
@@ -68,7 +70,7 @@ __device__ __forceinline__ bool interp_delta(const GridDev& G, double x, double 
             const int ii = min(max(i0 + a, 0), G.nx - 1), jj = min(max(j0 + b, 0), G.ny - 1);
             const double w = (a ? fx : 1.0 - fx) * (b ? fy : 1.0 - fy);
             const size_t q = (size_t)jj * G.nx + ii;
-            if (G.mask[q]) { const double2 d = G.delta[q]; sw += w; ar += w * d.x; ai += w * d.y; }
+            if (G.mask[q]) { const double2 d = F[q]; sw += w; ar += w * d.x; ai += w * d.y; }
         }
     if (sw > 1e-12) { dr = ar / sw; di = ai / sw; return true; }
     double bd = 1e300; int bi = -1, bj = -1;
@@ -79,9 +81,23 @@ __device__ __forceinline__ bool interp_delta(const GridDev& G, double x, double 
             if (d < bd) { bd = d; bi = ii; bj = jj; }
         }
     if (bi < 0) { dr = di = 0.0; return false; }
-    const double2 d = G.delta[(size_t)bj * G.nx + bi];
+    const double2 d = F[(size_t)bj * G.nx + bi];
     dr = d.x; di = d.y;
     return true;
+}
+// Delta(p_F, R) = sum_G eta_G Delta_G(R) (Eq. 1 :37) at a point; eta: the ncomp basis-function values of the direction,
+// `stride` apart
+__device__ __forceinline__ bool interp_gap(const GridDev& G, const double* eta, int stride, double x, double y, double& dr, double& di) {
+    const size_t ng = (size_t)G.nx * G.ny;
+    bool ok = true;
+    dr = di = 0.0;
+    for (int c = 0; c < G.ncomp; ++c) {
+        double r, i;
+        ok = interp_delta(G, G.delta + c * ng, x, y, r, i) && ok;
+        const double e = eta[(size_t)c * stride];
+        dr = fma(e, r, dr); di = fma(e, i, di);
+    }
+    return ok;
 }
 
 __device__ __forceinline__ double interp_plain(const GridDev& G, const double* F, double x, double y) {
@@ -106,23 +122,23 @@ __device__ __forceinline__ double interp_plain(const GridDev& G, const double* F
 // (reading R4); its length is l0 (p = 0), l1 (p = nn) or h.  Piece records of trajectory g start at
 // noff[g] + g.  The fourth entry is the energy-independent part of the argument of the T table (sc_math.cuh).
 template <typename R>
-__global__ void rotate_in_kernel(GridDev G, TrajDev T, const double* vx, const double* vy, const double* eta,
-                                 double c, int sigma, double2* nd_D, double* nd_a, typename VT<R>::V2* nd_Dr,
+__global__ void rotate_in_kernel(GridDev G, TrajDev T, const double* vx, const double* vy, const double* eta /*[ncomp][nphi]*/,
+                                 int nphi, double c, int sigma, double2* nd_D, double* nd_a, typename VT<R>::V2* nd_Dr,
                                  typename VT<R>::V4* pc, float2* pmax, int* n_bad) {
     const int g = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (g >= T.n) return;
     const int lane = threadIdx.x & 31;
     const int k = T.k[g];
-    const double cx = vx[k], cy = vy[k], e = eta[k], w = (T.t[g] - c) * G.h;
+    const double cx = vx[k], cy = vy[k], w = (T.t[g] - c) * G.h;
     const int jf = T.jf[g], nn = T.nn[g];
     const long long off = T.noff[g];
     for (int m = lane; m < nn; m += 32) {
         const double u = (jf + m - c) * G.h;
         const double x = u * cx - w * cy, y = u * cy + w * cx;
         double dr, di;
-        if (!interp_delta(G, x, y, dr, di)) atomicAdd(n_bad, 1);
-        nd_D[off + m] = make_double2(e * dr, e * di);
-        if (sizeof(R) == 4) nd_Dr[off + m] = mk2((R)(e * dr), (R)(e * di));      // fp32 mode: the march reads a float copy
+        if (!interp_gap(G, eta + k, nphi, x, y, dr, di)) atomicAdd(n_bad, 1);
+        nd_D[off + m] = make_double2(dr, di);
+        if (sizeof(R) == 4) nd_Dr[off + m] = mk2((R)dr, (R)di);                  // fp32 mode: the march reads a float copy
         nd_a[off + m] = sigma * (cx * interp_plain(G, G.Ax, x, y) + cy * interp_plain(G, G.Ay, x, y));
     }
     __syncwarp();
@@ -146,13 +162,13 @@ __global__ void rotate_in_kernel(GridDev G, TrajDev T, const double* vx, const d
 // fallback coefficients for boundary points that have no valid specular partner (R6 fallback):
 // Delta(R_min) eta(mirrored direction) and sigma v_in . A(R_min)
 __global__ void fallback_kernel(GridDev G, int nfb, const int* rows, const double* px, const double* py,
-                                const double* dx, const double* dy, const double* eta_m, int sigma,
+                                const double* dx, const double* dy, const double* eta_m /*[ncomp][nfb]*/, int sigma,
                                 double2* fb_D, double* fb_a) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= nfb) return;
     double dr, di;
-    interp_delta(G, px[i], py[i], dr, di);
-    fb_D[rows[i]] = make_double2(eta_m[i] * dr, eta_m[i] * di);
+    interp_gap(G, eta_m + i, nfb, px[i], py[i], dr, di);
+    fb_D[rows[i]] = make_double2(dr, di);
     fb_a[rows[i]] = sigma * (dx[i] * interp_plain(G, G.Ax, px[i], py[i]) + dy[i] * interp_plain(G, G.Ay, px[i], py[i]));
 }
 
@@ -684,15 +700,17 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32, MARCH_MIN_CTAS) march_kernel
 struct BackArgs {
     GridDev G;
     int nphi, nrot; double c;
-    const double* vx; const double* vy; const double* eta; const double* W;
+    const double* vx; const double* vy; const double* eta /*[ncomp][nphi]*/; const double* W;
     const int* line_g;           // [pair][t] -> first physical trajectory on that lattice line, or -1
     const int* line_n;           // [pair][t] -> number of trajectories (inside intervals) on that line
     TrajDev T;
     const double* part;          // [node][6]
-    double t, D; int sigma;
-    double2* delta_new; double* jx; double* jy; double* feI;
+    double t; double D[MAX_COMP]; int sigma;      // D_G = ln(T/T_c^G) + sum_n w_n t/eps_n (Eq. 22 :144)
+    double2* delta_new;          // [ncomp][ny][nx]
+    double* jx; double* jy; double* feI;
     int* n_bad;
-    double* raw;                 // non-null: write the 5 un-finalised accumulators [5][ny][nx] instead (energy-sharded sweep)
+    double* raw;                 // non-null: write the 2 ncomp + 3 un-finalised accumulators [..][ny][nx] instead (energy-sharded
+                                 // sweep): Re, Im of every component's numerator, then Jx, Jy, I
 };
 
 // weights of the (up to 4) valid lattice nodes around a grid point for pair p; returns count
@@ -745,7 +763,10 @@ __global__ void rotate_back_kernel(BackArgs B) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
     if (i >= B.G.nx) return;
     const size_t q = (size_t)j * B.G.nx + i;
-    double nr = 0.0, ni = 0.0, sjx = 0.0, sjy = 0.0, sI = 0.0;
+    const int nc = B.G.ncomp;
+    double nr[MAX_COMP], ni[MAX_COMP], sjx = 0.0, sjy = 0.0, sI = 0.0;
+#pragma unroll
+    for (int c = 0; c < MAX_COMP; ++c) nr[c] = ni[c] = 0.0;
     if (B.G.mask[q]) {
         const double x = (i - 0.5 * (B.G.nx - 1)) * B.G.h, y = (j - 0.5 * (B.G.ny - 1)) * B.G.h;
         const int H = B.nphi / 2;
@@ -760,37 +781,47 @@ __global__ void rotate_back_kernel(BackArgs B) {
                 f3 = fma(w[s], v[3], f3); f4 = fma(w[s], v[4], f4); f5 = fma(w[s], v[5], f5);
             }
             // angle k = p: SF = (f0,f1), SG = f4, SI = f5;  angle k+H: SF = conj(X2) = (f2,-f3), SG' v' = SG v, SI' = SI
-            const double Wk = B.W[p], Wk2 = B.W[p + H], ek = B.eta[p], ek2 = B.eta[p + H];
-            nr += Wk * ek * f0 + Wk2 * ek2 * f2;
-            ni += Wk * ek * f1 - Wk2 * ek2 * f3;
+            const double Wk = B.W[p], Wk2 = B.W[p + H];
+#pragma unroll
+            for (int c = 0; c < MAX_COMP; ++c)
+                if (c < nc) {                                 // projection on eta_G (real): Eq. 22 numerator of component G
+                    const double ek = B.eta[(size_t)c * B.nphi + p], ek2 = B.eta[(size_t)c * B.nphi + p + H];
+                    nr[c] += Wk * ek * f0 + Wk2 * ek2 * f2;
+                    ni[c] += Wk * ek * f1 - Wk2 * ek2 * f3;
+                }
             const double wj = (Wk + Wk2) * f4;
             sjx = fma(wj, B.vx[p], sjx); sjy = fma(wj, B.vy[p], sjy);
             sI += (Wk + Wk2) * f5;
         }
     }
+    const size_t ng = (size_t)B.G.nx * B.G.ny;
     if (B.raw) {
-        const size_t ng = (size_t)B.G.nx * B.G.ny;
-        B.raw[q] = nr; B.raw[ng + q] = ni; B.raw[2 * ng + q] = sjx; B.raw[3 * ng + q] = sjy; B.raw[4 * ng + q] = sI;
+#pragma unroll
+        for (int c = 0; c < MAX_COMP; ++c) if (c < nc) { B.raw[(2 * c) * ng + q] = nr[c]; B.raw[(2 * c + 1) * ng + q] = ni[c]; }
+        B.raw[(2 * nc) * ng + q] = sjx; B.raw[(2 * nc + 1) * ng + q] = sjy; B.raw[(2 * nc + 2) * ng + q] = sI;
         return;
     }
     // Delta_new = -2 i t Num / D (Eq. 22 with f = -2 pi i gamma/(1+P)); j = 2 sigma t J (Eq. 8); I = t I (Eq. 19)
-    const double s = 2.0 * B.t / B.D;
-    if (B.delta_new) B.delta_new[q] = make_double2(s * ni, -s * nr);
+    if (B.delta_new) {
+#pragma unroll
+        for (int c = 0; c < MAX_COMP; ++c) if (c < nc) { const double s = 2.0 * B.t / B.D[c]; B.delta_new[c * ng + q] = make_double2(s * ni[c], -s * nr[c]); }
+    }
     if (B.jx) B.jx[q] = 2.0 * B.sigma * B.t * sjx;
     if (B.jy) B.jy[q] = 2.0 * B.sigma * B.t * sjy;
     if (B.feI) B.feI[q] = B.t * sI;
 }
 
 // a7 alone, after the accumulators of all energy shards have been summed
-__global__ void finalise_kernel(size_t ng, const double* raw, double t, double D, int sigma,
+struct FinArgs { double D[MAX_COMP]; };
+__global__ void finalise_kernel(size_t ng, int nc, const double* raw, double t, FinArgs F, int sigma,
                                 double2* delta_new, double* jx, double* jy, double* feI) {
     const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (q >= ng) return;
-    const double s = 2.0 * t / D;
-    if (delta_new) delta_new[q] = make_double2(s * raw[ng + q], -s * raw[q]);
-    if (jx) jx[q] = 2.0 * sigma * t * raw[2 * ng + q];
-    if (jy) jy[q] = 2.0 * sigma * t * raw[3 * ng + q];
-    if (feI) feI[q] = t * raw[4 * ng + q];
+    if (delta_new)
+        for (int c = 0; c < nc; ++c) { const double s = 2.0 * t / F.D[c]; delta_new[c * ng + q] = make_double2(s * raw[(2 * c + 1) * ng + q], -s * raw[(2 * c) * ng + q]); }
+    if (jx) jx[q] = 2.0 * sigma * t * raw[(2 * nc) * ng + q];
+    if (jy) jy[q] = 2.0 * sigma * t * raw[(2 * nc + 1) * ng + q];
+    if (feI) feI[q] = t * raw[(2 * nc + 2) * ng + q];
 }
 
 // LDOS rotate-back: thread per (grid point, energy); energies fastest so the gathers coalesce.

@@ -1,8 +1,8 @@
 """Energy sharding of the sweep across GPUs — host logic only.
 
 The march, the specular boundary condition and the boundary stores never couple different energies, so rank r
-of W owns a contiguous slice of the Matsubara table for all angles and trajectories; the five un-finalised
-accumulator fields are summed with ONE all-reduce per sweep (`sc_set_allreduce_hook`), after which every rank
+of W owns a contiguous slice of the Matsubara table for all angles and trajectories; the un-finalised accumulator
+fields (Re, Im of every order-parameter component's numerator, Jx, Jy, I: five for one component) are summed with ONE all-reduce per sweep (`sc_set_allreduce_hook`), after which every rank
 applies Eq. 22 / Eq. 8 / Eq. 19 to the same summed accumulators.  The denominator of
 Eq. 22 is a property of the whole table, so it is passed to every shard explicitly.
 """
@@ -42,6 +42,6 @@ def attach(ctx, t: float, n_energies: int, group=None):
     if len(z) == 0:
         raise ValueError("more ranks than energies")
     ctx.sc_set_energies(z, w, dsum)
-    acc = torch.zeros((5, ctx.ny, ctx.nx), dtype=torch.float64, device=ctx.device)
+    acc = torch.zeros((2 * ctx.n_components + 3, ctx.ny, ctx.nx), dtype=torch.float64, device=ctx.device)
     ctx.sc_set_allreduce_hook(acc, lambda: dist.all_reduce(acc, group=group))
     return acc

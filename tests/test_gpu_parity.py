@@ -408,3 +408,103 @@ def test_accelerator_argument_checks(sc):
         c2.sc_iterate(0, 0.7, False, d2)
     torch.cuda.synchronize()
     assert relerr(d.cpu().numpy(), d2.cpu().numpy()) < 1e-13
+
+
+# ---- several order-parameter components (NEXT-4: PAPER.md Eq. 1 :37, Eq. 22 :144, Listing 11 :909-926) -------------
+def _two_component_case(name):
+    rng = np.random.default_rng(41)
+    if name == "d+is rotated square":          # [110] walls suppress the d-wave and let a sub-dominant s admixture grow
+        wl = wlmod.make_workload(2, pts_per_xi=4, n_angles=16, n_energies=20, size_scale=0.4)
+        syms, tc = [wl.symmetry, 0], [1.0, 0.4]
+        d2 = 0.3j * wl.bulk_gap * (1 + 0.1 * rng.uniform(-1, 1, wl.delta0.shape)) * wl.mask
+    else:                                       # s-wave vortex disc in a field with a d_xy admixture
+        wl = wlmod.make_workload(1, pts_per_xi=5, n_angles=16, n_energies=24)
+        syms, tc = [wl.symmetry, 2], [1.0, 0.6]
+        d2 = 0.2 * wl.delta0 * np.exp(0.7j) * (1 + 0.2 * rng.uniform(-1, 1, wl.delta0.shape))
+    return wl, syms, tc, np.stack([wl.delta0, d2]).astype(np.complex128)
+
+
+@pytest.mark.parametrize("name", ["d+is rotated square", "s+dxy vortex disc"])
+def test_two_component_sweeps_match(sc, name):
+    wl, syms, tc, delta = _two_component_case(name)
+    Ax = wl.Aext_x if np.any(wl.Aext_x) else None
+    Ay = wl.Aext_y if np.any(wl.Aext_x) else None
+    o = oracle.Oracle.from_workload(wl); o.set_components(syms, tc)
+    ctx = sc.ScContext.from_workload(wl); ctx.sc_set_components(syms, tc)
+    ctx.sc_set_fields(dev(delta), dev(Ax), dev(Ay))
+    dn = torch.zeros((2, wl.ny, wl.nx), dtype=torch.complex128, device="cuda")
+    jx = torch.zeros((wl.ny, wl.nx), dtype=torch.float64, device="cuda"); jy = torch.zeros_like(jx); fe = torch.zeros_like(jx)
+    stores = None
+    for it in range(3):
+        ro = o.sweep(delta, Ax, Ay, wl.n_energies, stores); stores = ro["stores"]
+        st = ctx.sc_riccati_sweep(dn, jx, jy, fe, want_stats=True)
+        torch.cuda.synchronize()
+        g = dn.cpu().numpy()
+        for c in range(2):
+            assert relerr(g[c], ro["delta_new"][c]) < TOL, (it, c)
+        assert relerr(jx.cpu().numpy(), ro["jx"]) < TOL and relerr(jy.cpu().numpy(), ro["jy"]) < TOL
+        assert relerr(fe.cpu().numpy(), ro["fe_I"]) < TOL
+        assert st.n_bad == 0 and np.all(g[:, wl.mask == 0] == 0)
+    assert np.max(np.abs(ro["delta_new"][1])) > 1e-3     # the second component's gap equation is really exercised
+
+
+@pytest.mark.parametrize("acc,step", [(1, 1.0), (3, 0.5)])
+def test_two_component_iterations_match(sc, acc, step):
+    """Driver over x = (Re D_0, Im D_0, Re D_1, Im D_1, kappa^2 A_x, kappa^2 A_y): six slices, six CongAcc components."""
+    wl, syms, tc, delta = _two_component_case("s+dxy vortex disc")
+    o = oracle.Oracle.from_workload(wl); o.set_components(syms, tc)
+    drv = oracle.Driver(o, wl.Aext_x, wl.Aext_y, wl.n_energies, accelerator=acc, step=step)
+    ctx = sc.ScContext.from_workload(wl); ctx.sc_set_components(syms, tc)
+    ctx.sc_set_external_field(dev(wl.Aext_x), dev(wl.Aext_y))
+    d_g = dev(delta).clone()
+    ax_g = torch.zeros((wl.ny, wl.nx), dtype=torch.float64, device="cuda"); ay_g = torch.zeros_like(ax_g)
+    d_o = delta.copy(); ax_o = np.zeros((wl.ny, wl.nx)); ay_o = np.zeros((wl.ny, wl.nx))
+    for it in range(5):
+        r = drv.iterate(d_o, ax_o, ay_o)
+        d_o, ax_o, ay_o = r["delta"], r["Aind_x"], r["Aind_y"]
+        st = ctx.sc_iterate(acc, step, False, d_g, ax_g, ay_g, want_stats=True)
+        torch.cuda.synchronize()
+        tol = TOL * max(1.0, 3.0 ** min(it, 6))
+        assert relerr(d_g.cpu().numpy(), d_o) < tol, it
+        assert relerr(ax_g.cpu().numpy(), ax_o) < tol * 10, it
+        assert abs(st.res_delta - r["res_delta"]) < 1e-7 * max(r["res_delta"], 1e-3)
+
+
+def test_components_argument_checks_and_single_component_identity(sc):
+    wl = wlmod.make_workload(1, pts_per_xi=4, n_angles=16, n_energies=12)
+    a = GpuRun(sc, wl); a.set_fields(wl.delta0, wl.Aext_x, wl.Aext_y); ra = a.sweep()
+    b = GpuRun(sc, wl); b.ctx.sc_set_components([wl.symmetry], [1.0]); b.set_fields(wl.delta0, wl.Aext_x, wl.Aext_y); rb = b.sweep()
+    for key in ("delta_new", "jx", "jy", "fe_I"):
+        assert np.array_equal(ra[key], rb[key])
+    for bad in (([0] * 5, [1.0] * 5), ([0, 7], [1.0, 1.0]), ([0, 1], [1.0, 1.5]), ([0, 1], [1.0, 0.0])):
+        with pytest.raises(sc.ScError):
+            b.ctx.sc_set_components(*bad)
+    b.ctx.sc_set_components([0, 1], [1.0, 0.5])
+    with pytest.raises(sc.ScError):                       # the fields were invalidated, and buffers are now [2][ny][nx]
+        b.ctx.sc_riccati_sweep(b.dn, b.jx, b.jy, b.fe)
+
+
+def test_two_component_energy_sharded_sweep(sc):
+    """Energy shards with two components: 2 n + 3 = 7 raw accumulator fields through the all-reduce hook, finalised
+    with each component's own denominator."""
+    from paper_2205_15000_b200 import sharding
+    wl, syms, tc, delta = _two_component_case("s+dxy vortex disc")
+    o = oracle.Oracle.from_workload(wl); o.set_components(syms, tc)
+    ro = o.sweep(delta, wl.Aext_x, wl.Aext_y, wl.n_energies)
+    ctxs, accs = [], []
+    for r in range(2):
+        c = sc.ScContext.from_workload(wl); c.sc_set_components(syms, tc)
+        z, w, dsum = sharding.matsubara_shard(wl.t, wl.n_energies, 2, r)
+        c.sc_set_energies(z, w, dsum)
+        c.sc_set_fields(dev(delta), dev(wl.Aext_x), dev(wl.Aext_y))
+        ctxs.append(c); accs.append(torch.zeros((7, wl.ny, wl.nx), dtype=torch.float64, device="cuda"))
+    ctxs[0].sc_set_allreduce_hook(accs[0], lambda: None)
+    ctxs[1].sc_set_allreduce_hook(accs[1], lambda: accs[1].add_(accs[0]))
+    dn = torch.zeros((2, wl.ny, wl.nx), dtype=torch.complex128, device="cuda")
+    jx = torch.zeros((wl.ny, wl.nx), dtype=torch.float64, device="cuda"); jy = torch.zeros_like(jx); fe = torch.zeros_like(jx)
+    ctxs[0].sc_riccati_sweep(dn, jx, jy, fe)
+    ctxs[1].sc_riccati_sweep(dn, jx, jy, fe)
+    torch.cuda.synchronize()
+    for c in range(2):
+        assert relerr(dn.cpu().numpy()[c], ro["delta_new"][c]) < TOL
+    assert relerr(jx.cpu().numpy(), ro["jx"]) < TOL and relerr(fe.cpu().numpy(), ro["fe_I"]) < TOL
