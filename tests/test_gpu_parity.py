@@ -446,6 +446,12 @@ def test_two_component_sweeps_match(sc, name):
         assert relerr(fe.cpu().numpy(), ro["fe_I"]) < TOL
         assert st.n_bad == 0 and np.all(g[:, wl.mask == 0] == 0)
     assert np.max(np.abs(ro["delta_new"][1])) > 1e-3     # the second component's gap equation is really exercised
+    # LDOS through the same two-component gap (the d+is admixture splits the zero-energy surface states)
+    e = np.array([-0.12, 0.0, 0.05, 0.12])
+    out = torch.zeros((len(e), wl.ny, wl.nx), dtype=torch.float64, device="cuda")
+    ctx.sc_ldos(e, 0.02, 2, out)
+    torch.cuda.synchronize()
+    assert relerr(out.cpu().numpy(), o.ldos(delta, Ax, Ay, e, 0.02, 2)) < TOL
 
 
 @pytest.mark.parametrize("acc,step", [(1, 1.0), (3, 0.5)])
