@@ -10,3 +10,4 @@ from .binding import (ScError, ScContext, SweepStats, lib_path, load_library, de
 
 __all__ = ["ScError", "ScContext", "SweepStats", "lib_path", "load_library", "declared_symbols",
            "SYM_S", "SYM_DX2Y2", "SYM_DXY", "SYM_G"]
+from .ozaki import ozaki_poles, ozaki_energy_table  # noqa: F401,E402

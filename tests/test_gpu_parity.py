@@ -514,3 +514,30 @@ def test_two_component_energy_sharded_sweep(sc):
     for c in range(2):
         assert relerr(dn.cpu().numpy()[c], ro["delta_new"][c]) < TOL
     assert relerr(jx.cpu().numpy(), ro["jx"]) < TOL and relerr(fe.cpu().numpy(), ro["fe_I"]) < TOL
+
+
+def test_ozaki_energy_table_sweep_matches(sc):
+    """the paper sums over Ozaki's poles instead of Matsubara frequencies.  20 poles (the last ones at
+    eps ~ 25-75 x 2 pi k_B T_c with weights ~8-25) through sc_set_energies against the oracle's raw sweep on the same
+    table, in a field (the high poles leave the T tables' radius: exp-based evaluation)."""
+    from paper_2205_15000_b200.ozaki import ozaki_energy_table
+    wl = wlmod.make_workload(1, pts_per_xi=5, n_angles=16, n_energies=20)
+    z, w = ozaki_energy_table(wl.t, 20)
+    o = oracle.Oracle.from_workload(wl)
+    g = GpuRun(sc, wl)
+    g.ctx.sc_set_energies(z, w)
+    g.set_fields(wl.delta0, wl.Aext_x, wl.Aext_y)
+    st = o.reset_stores(wl.delta0, wl.Aext_x, wl.Aext_y, z)
+    D = np.log(wl.t) + float(np.sum(w * wl.t / z.imag))
+    for it in range(2):
+        ro = o.raw_sweep(wl.delta0, wl.Aext_x, wl.Aext_y, z, w, st); st = ro["stores"]
+        rg = g.sweep()
+        assert relerr(rg["delta_new"], -2j * wl.t * ro["num"] / D * wl.mask) < TOL
+        assert relerr(rg["jx"], 2.0 * wl.charge_sign * wl.t * ro["Jx"] * wl.mask) < TOL
+        assert relerr(rg["fe_I"], wl.t * ro["I"] * wl.mask) < TOL
+    # and the physics: 20 Ozaki poles reproduce the 400-term Matsubara gap-equation output to ~1e-4, 20 Matsubara terms do not
+    g2 = GpuRun(sc, wl, ); g2.set_fields(wl.delta0, wl.Aext_x, wl.Aext_y); r20 = g2.sweep()["delta_new"]
+    wl4 = wlmod.make_workload(1, pts_per_xi=5, n_angles=16, n_energies=400)
+    g4 = GpuRun(sc, wl4); g4.set_fields(wl.delta0, wl.Aext_x, wl.Aext_y); r400 = g4.sweep()["delta_new"]
+    g.ctx.sc_reset_boundary(); roz = g.sweep()["delta_new"]
+    assert relerr(roz, r400) < 0.1 * relerr(r20, r400)
