@@ -58,6 +58,17 @@ struct EnergyDev { int ne; const double* zr; const double* zi; const double* w; 
 // ------------------------------------------------------------------------------------------------
 // masked bilinear interpolation of Delta (R5) and plain bilinear of A at a point
 // ------------------------------------------------------------------------------------------------
+// R5 fallback (rare, out of line): no corner in the mask -> nearest mask point within 2 cells
+__device__ __noinline__ int nearest_mask_point(const unsigned char* mask, int nx, int ny, double gx, double gy, int i0, int j0) {
+    double bd = 1e300; int best = -1;
+    for (int jj = j0 - 2; jj <= j0 + 3; ++jj)
+        for (int ii = i0 - 2; ii <= i0 + 3; ++ii) {
+            if (ii < 0 || ii >= nx || jj < 0 || jj >= ny || !mask[(size_t)jj * nx + ii]) continue;
+            const double d = (gx - ii) * (gx - ii) + (gy - jj) * (gy - jj);
+            if (d < bd) { bd = d; best = jj * nx + ii; }
+        }
+    return best;
+}
 __device__ __forceinline__ bool interp_delta(const GridDev& G, const double2* __restrict__ F, double x, double y, double& dr, double& di) {
     const double gx = x / G.h + 0.5 * (G.nx - 1), gy = y / G.h + 0.5 * (G.ny - 1);
     const int i0 = (int)floor(gx), j0 = (int)floor(gy);
@@ -73,15 +84,9 @@ __device__ __forceinline__ bool interp_delta(const GridDev& G, const double2* __
             if (G.mask[q]) { const double2 d = F[q]; sw += w; ar += w * d.x; ai += w * d.y; }
         }
     if (sw > 1e-12) { dr = ar / sw; di = ai / sw; return true; }
-    double bd = 1e300; int bi = -1, bj = -1;
-    for (int jj = j0 - 2; jj <= j0 + 3; ++jj)
-        for (int ii = i0 - 2; ii <= i0 + 3; ++ii) {
-            if (ii < 0 || ii >= G.nx || jj < 0 || jj >= G.ny || !G.mask[(size_t)jj * G.nx + ii]) continue;
-            const double d = (gx - ii) * (gx - ii) + (gy - jj) * (gy - jj);
-            if (d < bd) { bd = d; bi = ii; bj = jj; }
-        }
-    if (bi < 0) { dr = di = 0.0; return false; }
-    const double2 d = F[(size_t)bj * G.nx + bi];
+    const int best = nearest_mask_point(G.mask, G.nx, G.ny, gx, gy, i0, j0);
+    if (best < 0) { dr = di = 0.0; return false; }
+    const double2 d = F[best];
     dr = d.x; di = d.y;
     return true;
 }
@@ -122,7 +127,7 @@ __device__ __forceinline__ double interp_plain(const GridDev& G, const double* F
 // (reading R4); its length is l0 (p = 0), l1 (p = nn) or h.  Piece records of trajectory g start at
 // noff[g] + g.  The fourth entry is the energy-independent part of the argument of the T table (sc_math.cuh).
 template <typename R>
-__global__ void rotate_in_kernel(GridDev G, TrajDev T, const double* vx, const double* vy, const double* eta /*[ncomp][nphi]*/,
+__global__ void __launch_bounds__(256, 3) rotate_in_kernel(GridDev G, TrajDev T, const double* vx, const double* vy, const double* eta /*[ncomp][nphi]*/,
                                  int nphi, double c, int sigma, double2* nd_D, double* nd_a, typename VT<R>::V2* nd_Dr,
                                  typename VT<R>::V4* pc, float2* pmax, int* n_bad) {
     const int g = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
@@ -132,6 +137,7 @@ __global__ void rotate_in_kernel(GridDev G, TrajDev T, const double* vx, const d
     const double cx = vx[k], cy = vy[k], w = (T.t[g] - c) * G.h;
     const int jf = T.jf[g], nn = T.nn[g];
     const long long off = T.noff[g];
+#pragma unroll 1
     for (int m = lane; m < nn; m += 32) {
         const double u = (jf + m - c) * G.h;
         const double x = u * cx - w * cy, y = u * cy + w * cx;
