@@ -95,8 +95,9 @@ sc_status sc_set_components(sc_ctx* ctx, int n, const sc_symmetry* symmetries, c
 
 /* Replace the Matsubara table by any energies z_n = z_re + i z_im (Im z > 0) with weights w_n (host, n values):
  * Ozaki poles (:207, reading R-A4), or ONE SHARD of the Matsubara energies when the sweep is split by energy across
- * GPUs.  The table must be closed under z -> -conj(z) (Eq. 13 :95; energies on the imaginary axis
- * are).  denominator_sum = sum over the WHOLE job's table of w_n t / Im z_n, the second term of the denominator of
+ * GPUs.  The table must be closed under z -> -conj(z) with equal weights for the two partners (Eq. 13 :95:
+ * the sums of angle k + N/2 are taken from the partner energies of angle k; energies on the imaginary axis are their own
+ * partners).  denominator_sum = sum over the WHOLE job's table of w_n t / Im z_n, the second term of the denominator of
  * Eq. 22 (:144); NaN = compute it from this table.  Re-sizes and invalidates the boundary stores. */
 sc_status sc_set_energies(sc_ctx* ctx, const double* z_re, const double* z_im, const double* w, int n,
                           double denominator_sum);

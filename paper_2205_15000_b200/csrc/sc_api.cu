@@ -493,6 +493,8 @@ sc_status sc_set_energies(sc_ctx* ctx, const double* z_re, const double* z_im, c
         for (int q = 0; q < n; ++q)
             if (std::fabs(z_re[q] + z_re[m]) <= 1e-12 * (1.0 + std::fabs(z_re[m])) && std::fabs(z_im[q] - z_im[m]) <= 1e-12 * z_im[m]) { E.partner[m] = q; break; }
         if (E.partner[m] < 0) return fail(ctx, SC_ERR_ARG, "energy table is not closed under z -> -conj(z)");
+        // the sums of angle k + N/2 are taken from the partner energies of angle k (Eq. 13): partners must weigh the same
+        if (std::fabs(w[E.partner[m]] - w[m]) > 1e-12 * std::fabs(w[m])) return fail(ctx, SC_ERR_ARG, "partner energies z and -conj(z) must have equal weights");
     }
     ctx->denom_sum = std::isnan(denominator_sum) ? ds : denominator_sum;
     if (sc_status st = upload_energies(ctx, E)) return st;

@@ -541,3 +541,25 @@ def test_ozaki_energy_table_sweep_matches(sc):
     g4 = GpuRun(sc, wl4); g4.set_fields(wl.delta0, wl.Aext_x, wl.Aext_y); r400 = g4.sweep()["delta_new"]
     g.ctx.sc_reset_boundary(); roz = g.sweep()["delta_new"]
     assert relerr(roz, r400) < 0.1 * relerr(r20, r400)
+
+
+def test_sweep_with_energies_off_the_imaginary_axis(sc):
+    """sc_set_energies accepts any table closed under z -> -conj(z) (Eq. 13 :95): a Matsubara-type sweep (energy sums,
+    Delta_new, j, I) over complex energies exercises the complex-coefficient T table outside sc_ldos."""
+    wl = wlmod.make_workload(1, pts_per_xi=5, n_angles=16, n_energies=8)
+    z = np.array([0.3 + 0.2j, -0.3 + 0.2j, 0.1 + 0.5j, -0.1 + 0.5j, 0.9j, 1.7 + 0.05j, -1.7 + 0.05j])
+    w = np.array([1.0, 1.0, 0.7, 0.7, 1.3, 0.4, 0.4])
+    o = oracle.Oracle.from_workload(wl)
+    g = GpuRun(sc, wl)
+    g.ctx.sc_set_energies(z, w)
+    g.set_fields(wl.delta0, wl.Aext_x, wl.Aext_y)
+    st = o.reset_stores(wl.delta0, wl.Aext_x, wl.Aext_y, z)
+    D = np.log(wl.t) + float(np.sum(w * wl.t / z.imag))
+    for it in range(2):
+        ro = o.raw_sweep(wl.delta0, wl.Aext_x, wl.Aext_y, z, w, st); st = ro["stores"]
+        rg = g.sweep()
+        assert relerr(rg["delta_new"], -2j * wl.t * ro["num"] / D * wl.mask) < TOL, it
+        assert relerr(rg["jx"], 2.0 * wl.charge_sign * wl.t * ro["Jx"] * wl.mask) < TOL, it
+        assert relerr(rg["fe_I"], wl.t * ro["I"] * wl.mask) < TOL, it
+    with pytest.raises(sc.ScError):                       # partners must carry the same weight
+        g.ctx.sc_set_energies(np.array([0.3 + 0.2j, -0.3 + 0.2j]), np.array([1.0, 0.5]))
