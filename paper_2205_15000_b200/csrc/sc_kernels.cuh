@@ -227,6 +227,9 @@ constexpr int MARCH_WARPS = SC_MARCH_WARPS;  // warps per CTA
 #define SC_MARCH_MIN_CTAS 2
 #endif
 constexpr int MARCH_MIN_CTAS = SC_MARCH_MIN_CTAS;   // resident CTAs per SM the fp64 register budget is sized for
+#ifndef SC_HALF_SPILL
+#define SC_HALF_SPILL 1
+#endif
 #ifndef SC_PF_DIST
 #define SC_PF_DIST 16
 #endif
@@ -453,9 +456,15 @@ __device__ __forceinline__ void march_round(const MarchArgsT<R>& A, const WarpJo
     using V2 = typename VT<R>::V2; using V4 = typename VT<R>::V4;
     constexpr int ROW = ScrT<R, ST>::ROW, BYTES = ScrT<R, ST>::BYTES;
     constexpr int NB = ST ? 1 : 0;                          // ST: node m lives in entry m+1 (entry p = piece p)
+    // HALF: only every second gamma~ is spilled (odd nodes, and the last node); pass 2 steps the stored value of node
+    // m+1 down across piece m+1 — with the T it evaluates anyway for gamma's step up across the same piece — to get
+    // gamma~ at the even node m: one more Moebius step per two units (13.5 FP64 instructions per unit) for half the
+    // scratch traffic (16 instead of 32 B per unit).  Entry m>>1 holds node m+1 (m even, m+1 < nn) or the last node.
+    constexpr bool HALF = !ST && STEP == 0 && SC_HALF_SPILL != 0;
+    constexpr int PFROWS = HALF ? RED_NODES / 2 : RED_NODES;   // scratch rows one reduction batch consumes
     const int lane = J.lane, nn = J.nn, ne = J.ne;
     char* const scr = J.scr_w + lane * BYTES;               // entry e of this lane: scr + e*ROW
-    const bool pf_lane = lane * 128 < RED_NODES * ROW;      // lanes that cover 4 rows in 128-byte lines
+    const bool pf_lane = lane * 128 < PFROWS * ROW;         // lanes that cover a batch's rows in 128-byte lines
     const bool act = n0 + lane < ne;
     const int n = act ? n0 + lane : ne - 1;
     const R zr0 = (R)A.E.zr[n], zi0 = (R)A.E.zi[n];
@@ -512,7 +521,8 @@ __device__ __forceinline__ void march_round(const MarchArgsT<R>& A, const WarpJo
                 const V4 cc = buf[p & (CHUNK - 1)];
                 const cplx_t<R> T = coefT(cc, false, J.len1);
                 gt = stepT(gt, R(-1), cc, T, J.len1);
-                if (MODE != 2 || ST) st_ent<ST>(e, T, gt);
+                if (HALF) { if (MODE != 2) st_ent<ST>(scr + (size_t)((nn - 1) >> 1) * ROW, T, gt); }   // the last node is always spilled
+                else if (MODE != 2 || ST) st_ent<ST>(e, T, gt);
                 e -= ROW; --p;
             }
 #pragma unroll 2
@@ -520,7 +530,8 @@ __device__ __forceinline__ void march_round(const MarchArgsT<R>& A, const WarpJo
                 const V4 cc = buf[p & (CHUNK - 1)];
                 const cplx_t<R> T = coefT(cc, true, J.hlen);
                 gt = stepT(gt, R(-1), cc, T, J.hlen);
-                if (MODE != 2 || ST) st_ent<ST>(e, T, gt);
+                if (HALF) { if (MODE != 2 && !(p & 1)) st_ent<ST>(scr + (size_t)((p - 1) >> 1) * ROW, T, gt); }   // landed on the odd node p-1
+                else if (MODE != 2 || ST) st_ent<ST>(e, T, gt);
                 e -= ROW;
             }
             if (c == 0) {                                       // entry piece (length l0); its gamma~ is the end value
@@ -554,22 +565,39 @@ __device__ __forceinline__ void march_round(const MarchArgsT<R>& A, const WarpJo
     const char* e = scr + NB * ROW;             // entry of node 0
     if (LD)
         for (int q = RED_NODES; q < PF_DIST && q < nn; q += RED_NODES)
-            if (pf_lane) prefetch_l2(J.scr_w + (size_t)(q + NB) * ROW + lane * 128);
-    Ent<R> En{}, En2{};                          // entries of the next two nodes (register look-ahead over the HBM latency)
+            if (pf_lane) prefetch_l2(J.scr_w + (size_t)(HALF ? q >> 1 : q + NB) * ROW + lane * 128);
+    Ent<R> En{}, En2{};                          // the next two entries (register look-ahead over the HBM latency)
     if (LD) { En = ld_ent<ST>(e, R(0)); En2 = ld_ent<ST>(e + ROW, R(0)); }
+    cplx_t<R> gt_odd = mk(R(0), R(0));           // HALF: gamma~ of the odd node, held from the even node before it
     double part_nxt = 0.0;                       // running sums of the earlier energy rounds, fetched one batch ahead
     if (MODE == 0 && n0 && lane < RED_NODES * RED_VALS && lane < npart) part_nxt = J.PART[lane];
     int m = 0;
     // node m: products with gamma~(m) from its entry, then the step across piece m+1 (T from entry m+1 when spilled)
     auto node = [&](int b, const V4* pbuf, const V2* dbuf, bool exitp) {
-        const Ent<R> Ec = En;
         const V4 cc = pbuf[(m + b) & (CHUNK - 1)]; const V2 dc = dbuf[(m + b) & (CHUNK - 1)];
+        const R len = exitp ? J.len1 : J.hlen;
+        if (HALF) {                                            // batches start on even nodes: the parity of m+b is that of b
+            const cplx_t<R> T = coefT(cc, !exitp, len);
+            cplx_t<R> gth = gt_odd;
+            if (!(b & 1)) {
+                const cplx_t<R> G = mk(En.gr, En.gi);          // entry (m+b)>>1: node m+b+1, or the last node itself
+                if (LD) { En = En2; En2 = ld_ent<ST>(e + ((b >> 1) + 2) * ROW, R(0)); }
+                gt_odd = G;
+                gth = exitp ? G : stepT(G, R(-1), cc, T, len);
+            }
+            if (MODE != 2) {
+                const R rg = node_products<MODE, STATS, R>(gm, gth.re, gth.im, dc, wn, J.stage + b * RED_VALS * STAGE_LD + lane, max2);
+                if (MODE == 1 && act) A.ldos[(size_t)(J.noff + m + b) * ne + n] = (double)rg;
+            }
+            gm = stepT(gm, R(1), cc, T, len);
+            return;
+        }
+        const Ent<R> Ec = En;
         if (LD) { En = En2; En2 = ld_ent<ST>(e + (b + 2) * ROW, R(0)); }   // two entries ahead (the scratch has spare rows)
         if (MODE != 2) {
             const R rg = node_products<MODE, STATS, R>(gm, Ec.gr, Ec.gi, dc, wn, J.stage + b * RED_VALS * STAGE_LD + lane, max2);
             if (MODE == 1 && act) A.ldos[(size_t)(J.noff + m + b) * ne + n] = (double)rg;
         }
-        const R len = exitp ? J.len1 : J.hlen;
         // ST: the entry of node m+b is the entry of piece m+b+1, the step that leaves the node: it holds that T
         const cplx_t<R> T = ST ? mk(Ec.tr, Ec.ti) : coefT(cc, !exitp, len);
         gm = stepT(gm, R(1), cc, T, len);
@@ -592,7 +620,7 @@ __device__ __forceinline__ void march_round(const MarchArgsT<R>& A, const WarpJo
         const V2* __restrict__ dbuf = ndb + bsel * CHUNK;
         const int mhi = min(nn, (c + 1) * CHUNK);
         for (; m + RED_NODES <= mhi; m += RED_NODES) {
-            if (LD && pf_lane && m + PF_DIST < nn) prefetch_l2(J.scr_w + (size_t)(m + PF_DIST + NB) * ROW + lane * 128);
+            if (LD && pf_lane && m + PF_DIST < nn) prefetch_l2(J.scr_w + (size_t)(HALF ? (m + PF_DIST) >> 1 : m + PF_DIST + NB) * ROW + lane * 128);
             const double part_old = part_nxt;
             if (MODE == 0 && n0 && lane < RED_NODES * RED_VALS && (m + RED_NODES) * RED_VALS + lane < npart)
                 part_nxt = J.PART[(m + RED_NODES) * RED_VALS + lane];
@@ -603,7 +631,7 @@ __device__ __forceinline__ void march_round(const MarchArgsT<R>& A, const WarpJo
 #pragma unroll
                 for (int b = 0; b < RED_NODES; ++b) node(b, pbuf, dbuf, b == RED_NODES - 1);
             }
-            e += RED_NODES * ROW;
+            e += PFROWS * ROW;
             if (MODE == 0) {
                 __syncwarp();
                 if (lane < RED_NODES * RED_VALS) {
