@@ -52,9 +52,9 @@ TEXTBOOK_FP64_INSTR_PER_UNIT = 184.0
 ALGO_FP64_INSTR_PER_UNIT_MIDPOINT = 2 * 66.0 + 28.0 + 8.0
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE march launch at configs[4], fp64, closed-form stepper, all rounds in
 # "recompute" mode (--sweep-only: A = A_ext), from the `ncu --set full` capture summarised in profiles/
-# (profiles/r1_march_fp64_cfg4_ncu_full.md: 2.645 TB read + 2.309 TB written)
-NCU_TRAFFIC_BYTES = {(4, 64, 0): 4.953921e12}
-NCU_PIPE_FP64_ACTIVE_PCT = {(4, 64, 0): 73.7}
+# (profiles/r1_march_fp64_cfg4_ncu_full.md: 1.519 TB read + 1.255 TB written)
+NCU_TRAFFIC_BYTES = {(4, 64, 0): 2.773693e12}
+NCU_PIPE_FP64_ACTIVE_PCT = {(4, 64, 0): 73.5}
 
 
 class ClockSampler(threading.Thread):
@@ -269,7 +269,7 @@ def run_ours(a):
                 "launches_timed": march_launches, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                 "frac": achieved / peak,
                 "traffic": NCU_TRAFFIC_BYTES.get(key) if full_size else None,
-                "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/) of a launch with ALL rounds in recompute mode (32 B algorithmic per unit = 4.22e12); stored-T rounds move 64 B per unit",
+                "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/) of a launch with ALL rounds in recompute mode (16 B algorithmic per unit = 2.11e12, + 0.39e12 running sums + 0.3e12 coefficient records); stored-T rounds move 64 B per unit",
                 "algorithmic_bytes_per_launch": hbm,
                 "ncu_pipe_fp64_cycles_active_pct": NCU_PIPE_FP64_ACTIVE_PCT.get(key) if full_size else None,
                 "note": "fp64 pipe: flops = 2 x FP64-pipe instructions; achieved = algorithmic count (DESIGN.md §6) x units / "
