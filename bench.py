@@ -349,7 +349,10 @@ def run_ours(a):
                                                              "parallelism": f"energy-sharded x{world}, 1 all-reduce/sweep" if world > 1 else "single GPU"}),
             "clocks": clocks,
             "e2e": {"value": n_updates / e2e_s, "unit": UNIT, "h2d_bytes_per_step": bytes_io, "d2h_bytes_per_step": bytes_io + 64,
-                    "res_delta_last": st2.res_delta},
+                    "res_delta_last": st2.res_delta,
+                    "note": "the e2e steps continue the same self-consistency run (iterations after the timed ones): as the "
+                            "Barzilai-Borwein transient of A_ind decays more rounds take the cheaper table tiers, so a step here "
+                            "can be faster than a timed one although it also pays the host copies"},
             "gpu_launches": launches_per_step * a.steps, "roofline": roofline}
     if fp32_leg:
         line["config"]["fp32_mode"] = fp32_leg
