@@ -227,6 +227,10 @@ constexpr int MARCH_WARPS = SC_MARCH_WARPS;  // warps per CTA
 #define SC_MARCH_MIN_CTAS 2
 #endif
 constexpr int MARCH_MIN_CTAS = SC_MARCH_MIN_CTAS;   // resident CTAs per SM the fp64 register budget is sized for
+#ifndef SC_P1_UNROLL
+#define SC_P1_UNROLL 2
+#endif
+constexpr int P1_UNROLL = SC_P1_UNROLL;      // pass 1: pieces per unrolled loop body
 #ifndef SC_HALF_SPILL
 #define SC_HALF_SPILL 1
 #endif
@@ -525,7 +529,7 @@ __device__ __forceinline__ void march_round(const MarchArgsT<R>& A, const WarpJo
                 else if (MODE != 2 || ST) st_ent<ST>(e, T, gt);
                 e -= ROW; --p;
             }
-#pragma unroll 2
+#pragma unroll P1_UNROLL
             for (; p >= plo; --p) {
                 const V4 cc = buf[p & (CHUNK - 1)];
                 const cplx_t<R> T = coefT(cc, true, J.hlen);
