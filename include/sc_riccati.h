@@ -135,6 +135,14 @@ sc_status sc_ldos(sc_ctx* ctx, const double* energies, int n_e, double broadenin
 sc_status sc_update_vector_potential(sc_ctx* ctx, const double* jx, const double* jy,
                                      double* Aind_x, double* Aind_y, double* fe_magnetic);
 
+/* Choose how sc_update_vector_potential / sc_iterate evaluate D1: eps = 0 (default) the exact cross-correlation with the
+ * full G table (zero-padded FFT); eps > 0 the paper's truncated eigen-decomposition G = sum_k lambda_k V^(k) V^(k)T
+ * (D7 :1027) keeping the N* eigenpairs of largest |lambda| with sqrt(1 - sum_{n<N*} lambda_n^2 / sum_n lambda_n^2) < eps
+ * (D9 :1036, the config key vector_potential_error) and N* pairs of separable 1-D cross-correlations (D8 :1031).
+ * n_kept (host, may be NULL): receives N* (0 for eps = 0); asking for it runs the eigen-decomposition now (synchronises).
+ * SC_ERR_ARG unless 0 <= eps < 1. */
+sc_status sc_set_vector_potential_error(sc_ctx* ctx, double eps, int* n_kept);
+
 /* Set the external vector potential used by sc_iterate (dev fp64 [ny][nx]; NULL = 0). */
 sc_status sc_set_external_field(sc_ctx* ctx, const double* Aext_x, const double* Aext_y);
 

@@ -122,6 +122,39 @@ def vector_potential(mask, h, kappa, jx, jy):
     return Ax, Ay
 
 
+def vector_potential_lowrank(mask, h, kappa, jx, jy, eps):
+    """The paper's own evaluation of D1 (App. D :1023-1038): eigendecompose the N x N table G_{m,n} (D7), keep the N*
+    eigenpairs of largest |lambda| with sqrt(1 - sum_{n<N*} lambda_n^2 / sum_n lambda_n^2) < eps (D9), and apply
+    A = -(1/kappa^2) sum_k lambda_k sum_{m'} sum_{n'} V_{|m'-m|} V_{|n'-n|} j_{m'n'} (D8) as two 1-D cross-correlations
+    per eigenpair; j has its mask-mean removed (:1040).  Returns (Ax, Ay, N*)."""
+    mask = np.ascontiguousarray(mask, np.uint8)
+    ny, nx = mask.shape
+    N = max(nx, ny)
+    G = np.array([[G_table_entry(m, n, h) for n in range(N)] for m in range(N)])
+    lam, V = np.linalg.eigh(G)
+    order = np.argsort(-np.abs(lam), kind="stable")
+    tot = float(np.sum(lam ** 2))
+    nstar = N
+    kept = 0.0
+    for c, k in enumerate(order):
+        kept += float(lam[k]) ** 2
+        if math.sqrt(max(0.0, 1.0 - kept / tot)) < eps:
+            nstar = c + 1
+            break
+    m = mask.astype(bool)
+    out = []
+    for j in (np.asarray(jx, np.float64), np.asarray(jy, np.float64)):
+        J = np.where(m, j - j[m].mean(), 0.0)                         # [n'][m']
+        A = np.zeros((ny, nx))
+        for k in order[:nstar]:
+            v = V[:, k]
+            Ty = v[np.abs(np.subtract.outer(np.arange(ny), np.arange(ny)))]   # (Ty)_{n,n'} = V_{|n'-n|}
+            Tx = v[np.abs(np.subtract.outer(np.arange(nx), np.arange(nx)))]
+            A += lam[k] * (Ty @ J @ Tx)
+        out.append(-A / (kappa * kappa))
+    return out[0], out[1], nstar
+
+
 def matsubara_denominator(t: float, ne: int) -> float:
     """D = ln t + sum_{n<ne} 1/(n + 1/2): denominator of PAPER.md Eq. 22 (:144), same cutoff as the
     numerator (reading R-A5)."""

@@ -102,6 +102,7 @@ def load_library():
     L.sc_set_external_field.argtypes = [vp, vp, vp]
     L.sc_iterate.argtypes = [vp, i, d, i, vp, vp, vp, C.POINTER(_Stats)]
     L.sc_set_accelerator_params.argtypes = [vp, d, d, d, d, d]
+    L.sc_set_vector_potential_error.argtypes = [vp, d, C.POINTER(i)]
     L.sc_debug_geometry.argtypes = [vp, C.POINTER(i), C.POINTER(i), C.POINTER(C.c_longlong)]
     L.sc_debug_tables.argtypes = [vp, i, C.POINTER(i), vp, vp, vp, vp]
     L.sc_debug_trajectory.argtypes = [vp, i, i, i, C.POINTER(i), vp, vp]
@@ -263,6 +264,12 @@ class ScContext:
                                        _dev_ptr(Aind_x, "f64", n), _dev_ptr(Aind_y, "f64", n),
                                        C.byref(st) if want_stats else None))
         return _stats(st) if want_stats else None
+
+    def sc_set_vector_potential_error(self, eps):
+        """Returns N*, the number of eigenpairs of G kept (0: exact FFT correlation)."""
+        n = C.c_int()
+        self._check(self._L.sc_set_vector_potential_error(self._h, float(eps), C.byref(n)))
+        return n.value
 
     def sc_set_accelerator_params(self, drag=0.0, step_factor=0.0, cos_similarity_min=0.0, step_min=0.0, step_max=0.0):
         self._check(self._L.sc_set_accelerator_params(self._h, drag, step_factor, cos_similarity_min, step_min, step_max))

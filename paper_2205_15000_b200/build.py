@@ -8,7 +8,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsc_riccati.so")
 SOURCES = ["sc_api.cu"]
-DEPS = ["sc_api.cu", "sc_kernels.cuh", "sc_math.cuh", "sc_geometry.hpp", "sc_field_kernels.cuh",
+DEPS = ["sc_api.cu", "sc_kernels.cuh", "sc_math.cuh", "sc_geometry.hpp", "sc_field_kernels.cuh", "sc_lowrank.cuh",
         os.path.join("..", "..", "include", "sc_riccati.h")]
 
 
@@ -16,7 +16,7 @@ def nvcc_command(extra=()):
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     return [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
             "-Xcompiler", "-fPIC", "-shared", *extra,
-            *[os.path.join(CSRC, s) for s in SOURCES], "-o", LIB, "-lcufft",
+            *[os.path.join(CSRC, s) for s in SOURCES], "-o", LIB, "-lcufft", "-lcusolver", "-lcublas",
             "-Xlinker", "-rpath=/usr/local/cuda/lib64"]
 
 

@@ -666,6 +666,22 @@ sc_status sc_iterate(sc_ctx* ctx, int accelerator, double step, int burnin, void
     return SC_OK;
 }
 
+sc_status sc_set_vector_potential_error(sc_ctx* ctx, double eps, int* n_kept) {
+    if (!ctx || !(eps >= 0.0) || eps >= 1.0) return fail(ctx, SC_ERR_ARG, "vector_potential_error must lie in [0, 1)");
+    ctx->fs.vp_eps = eps;
+    if (n_kept) {
+        *n_kept = 0;
+        if (eps > 0.0) {
+            std::string e;
+            if (!ctx->fs.lr) ctx->fs.lr = new scf::LowRank();
+            if (int rc = scf::ensure_lowrank(*ctx->fs.lr, ctx->grid.nx, ctx->grid.ny, ctx->grid.h, eps, ctx->stream, e))
+                return fail(ctx, rc == 2 ? SC_ERR_NOMEM : SC_ERR_CUDA, e);
+            *n_kept = ctx->fs.lr->nstar;
+        }
+    }
+    return SC_OK;
+}
+
 sc_status sc_set_accelerator_params(sc_ctx* ctx, double drag, double step_factor, double cos_similarity_min,
                                     double step_min, double step_max) {
     if (!ctx) return SC_ERR_ARG;

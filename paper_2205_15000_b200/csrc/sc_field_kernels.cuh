@@ -34,6 +34,8 @@ struct FieldState {
     cufftHandle plan_f = 0, plan_b = 0; bool plans = false;
     cufftDoubleComplex* Ghat = nullptr; double* pad = nullptr; cufftDoubleComplex* spec = nullptr;
     double* red = nullptr;          // RED_BLOCKS * RED_MAXOUT partials + 32 results
+    double vp_eps = 0.0;            // > 0: the paper's truncated eigen-decomposition of G (D7-D9) instead of the exact FFT correlation
+    struct LowRank* lr = nullptr;
     // driver
     size_t ng = 0; int nc = 1;      // grid points, order-parameter components (x has 2 nc + 2 slices of ng)
     double *Atot_x = nullptr, *Atot_y = nullptr, *jx = nullptr, *jy = nullptr, *feI = nullptr, *gAx = nullptr, *gAy = nullptr;
@@ -56,7 +58,9 @@ inline void release_driver(FieldState& F) {
     for (void** p : ptrs) { if (*p) cudaFree(*p); *p = nullptr; }
     F.driver = false; F.first = true; F.last_kind = -1;
 }
+inline void release_lowrank(FieldState& F);
 inline void release(FieldState& F) {
+    release_lowrank(F);
     if (F.plans) { cufftDestroy(F.plan_f); cufftDestroy(F.plan_b); }
     void* ptrs[] = {F.Ghat, F.pad, F.spec, F.red, F.Atot_x, F.Atot_y, F.jx, F.jy, F.feI, F.gAx, F.gAy, F.dnew,
                     F.d_prev, F.d_cur, F.prev_jx, F.prev_jy, F.prev_fe, F.state, F.upd, F.aux};
@@ -102,6 +106,11 @@ inline double G_closed(int m, int n, double h) {
     const double PI_ = 3.14159265358979323846;
     return h * h / (4.0 * PI_) * (2.0 * std::log(h) - std::log(2.0) - 3.0 + 0.25 * acc);
 }
+
+}  // namespace scf
+#include "sc_lowrank.cuh"
+namespace scf {
+inline void release_lowrank(FieldState& F) { if (F.lr) { release(*F.lr); delete F.lr; F.lr = nullptr; } }
 
 __global__ void pad_current_kernel(int nx, int ny, const unsigned char* mask, const double* j, const double* mean, int comp, double* pad) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x, jj = blockIdx.y;
@@ -175,8 +184,16 @@ inline int vector_potential(FieldState& F, int nx, int ny, double h, const unsig
     reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, MeanOp{mask, jx, jy}, F.red, 3);
     reduce_stage2<<<1, 32, 0, s>>>(F.red, 3, res);
     mean_finish_kernel<<<1, 1, 0, s>>>(res);
+    if (F.vp_eps > 0.0) {      // the paper's truncated eigen-decomposition (D7-D9) instead of the exact correlation
+        if (!F.lr) F.lr = new LowRank();
+        if (int rc = ensure_lowrank(*F.lr, nx, ny, h, F.vp_eps, s, err)) return rc;
+        for (int comp = 0; comp < 2; ++comp) {
+            masked_current_kernel<<<(unsigned)((ng + 255) / 256), 256, 0, s>>>(ng, mask, comp ? jy : jx, res, comp, F.lr->J);
+            if (int rc = lowrank_apply(*F.lr, -1.0 / (kappa * kappa), comp ? Ay : Ax, s, err)) return rc;
+        }
+    }
     const double scale = -1.0 / (kappa * kappa) / ((double)px * py);
-    for (int comp = 0; comp < 2; ++comp) {
+    for (int comp = 0; comp < 2 && !(F.vp_eps > 0.0); ++comp) {
         dim3 g1((px + 127) / 128, py);
         pad_current_kernel<<<g1, 128, 0, s>>>(nx, ny, mask, comp ? jy : jx, res, comp, F.pad);
         SCF_FFT(cufftExecD2Z(F.plan_f, F.pad, F.spec));

@@ -563,3 +563,28 @@ def test_sweep_with_energies_off_the_imaginary_axis(sc):
         assert relerr(rg["fe_I"], wl.t * ro["I"] * wl.mask) < TOL, it
     with pytest.raises(sc.ScError):                       # partners must carry the same weight
         g.ctx.sc_set_energies(np.array([0.3 + 0.2j, -0.3 + 0.2j]), np.array([1.0, 0.5]))
+
+
+@pytest.mark.parametrize("eps", [1e-2, 1e-5])
+def test_lowrank_vector_potential_matches(sc, eps):
+    """sc_set_vector_potential_error(eps > 0): the paper's truncated eigen-decomposition of G (D7-D9 :1023-1038) on the
+    device (cuSOLVER + cuBLAS) against the oracle's numpy restatement: same N*, same fields; and eps = 0 goes back to
+    the exact FFT correlation."""
+    wl = wlmod.make_workload(1, pts_per_xi=3, n_angles=8, n_energies=8)          # 60 x 60 grid
+    rng = np.random.default_rng(9)
+    jx = rng.normal(size=(wl.ny, wl.nx)) * wl.mask; jy = rng.normal(size=(wl.ny, wl.nx)) * wl.mask
+    ctx = sc.ScContext.from_workload(wl)
+    ox, oy, ns = oracle.vector_potential_lowrank(wl.mask, wl.h, wl.kappa, jx, jy, eps)
+    assert ctx.sc_set_vector_potential_error(eps) == ns and 1 <= ns < wl.nx
+    Ax = torch.zeros((wl.ny, wl.nx), dtype=torch.float64, device="cuda"); Ay = torch.zeros_like(Ax)
+    ctx.sc_update_vector_potential(dev(jx), dev(jy), Ax, Ay)
+    torch.cuda.synchronize()
+    assert relerr(Ax.cpu().numpy(), ox) < TOL and relerr(Ay.cpu().numpy(), oy) < TOL
+    ex, ey = oracle.vector_potential(wl.mask, wl.h, wl.kappa, jx, jy)
+    assert relerr(ox, ex) < 10 * eps                                              # the truncation is what eps says it is
+    assert ctx.sc_set_vector_potential_error(0.0) == 0
+    ctx.sc_update_vector_potential(dev(jx), dev(jy), Ax, Ay)
+    torch.cuda.synchronize()
+    assert relerr(Ax.cpu().numpy(), ex) < TOL
+    with pytest.raises(sc.ScError):
+        ctx.sc_set_vector_potential_error(1.5)

@@ -599,3 +599,33 @@ def test_second_component_with_zero_amplitude_changes_nothing():
     r2 = o2.sweep(d2, wl.Aext_x, wl.Aext_y, wl.n_energies)
     assert np.array_equal(r2["delta_new"][0], r1["delta_new"]) and np.array_equal(r2["jx"], r1["jx"]) and np.array_equal(r2["fe_I"], r1["fe_I"])
     assert np.max(np.abs(r2["delta_new"][1])) > 1e-6        # a vortex + walls do induce a d_xy admixture
+
+
+# ---- the paper's truncated eigen-decomposition of the vector-potential kernel (App. D, D7-D9 :1023-1038) -----------
+def test_lowrank_vector_potential_against_the_full_correlation():
+    """D8 with all N eigenpairs is D1 exactly (G = V Lambda V^T); with N* < N of them (D9) the error obeys the
+    Cauchy-Schwarz bound |dA| <= (2/kappa^2) ||G - G_N*||_F ||J||_F = (2/kappa^2) sqrt(sum_{n>=N*} lambda_n^2) ||J||_F
+    (each |m'-m|, |n'-n| entry of the table is visited at most four times), and N* grows as eps shrinks."""
+    n, h, kappa = 24, 0.25, 1.7
+    shapes = [Shape(kind=0, cx=0.0, cy=0.0, r=0.5 * n * h - 0.1)]
+    mask = make_mask(shapes, n, n, h)
+    rng = np.random.default_rng(5)
+    jx = rng.normal(size=(n, n)) * mask; jy = rng.normal(size=(n, n)) * mask
+    ex, ey = oracle.vector_potential(mask, h, kappa, jx, jy)
+    fx, fy, nfull = oracle.vector_potential_lowrank(mask, h, kappa, jx, jy, 0.0)      # eps = 0: D9 is never met, all N pairs
+    assert nfull == n
+    assert np.max(np.abs(fx - ex)) < 1e-12 * np.max(np.abs(ex)) and np.max(np.abs(fy - ey)) < 1e-12 * np.max(np.abs(ey))
+    G = np.array([[oracle.G_table_entry(a, b, h) for b in range(n)] for a in range(n)])
+    lam = np.sort(np.abs(np.linalg.eigvalsh(G)))[::-1]
+    last = n
+    for eps in (1e-1, 1e-2, 1e-4, 1e-6):
+        ax, ay, ns = oracle.vector_potential_lowrank(mask, h, kappa, jx, jy, eps)
+        assert 1 <= ns <= n
+        assert np.sqrt(1.0 - np.sum(lam[:ns] ** 2) / np.sum(lam ** 2)) < eps                       # D9 holds for N* ...
+        assert ns == 1 or not np.sqrt(1.0 - np.sum(lam[:ns - 1] ** 2) / np.sum(lam ** 2)) < eps     # ... and not for N* - 1
+        m = mask.astype(bool)
+        Jn = np.sqrt(np.sum((jx - jx[m].mean()) ** 2 * mask))
+        bound = 2.0 / kappa ** 2 * np.sqrt(np.sum(lam[ns:] ** 2)) * Jn
+        assert np.max(np.abs(ax - ex)) <= bound * (1 + 1e-9) + 1e-15
+        last = ns
+    assert last > 3                                                                            # eps = 1e-6 needs several pairs
