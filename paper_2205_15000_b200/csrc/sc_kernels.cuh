@@ -293,15 +293,20 @@ __device__ __forceinline__ R node_products(cplx_t<R> gm, R gtr, R gti, typename 
     return mad(R(2) * qr, rq, R(-1));                        // Re g = 2 Re 1/(1+P) - 1
 }
 
-// column sums of the stage: lane c < cnt sums row c over the 32 lanes (4 partial sums, fixed order)
+// column sums of the stage: lane c < cnt sums row c over the 32 lanes — 8 partial sums of 4 values each, then a
+// fixed tree (31 additions, dependency depth 6)
 template <typename R>
 __device__ __forceinline__ double stage_colsum(const R* stage, int lane) {
     using V2 = typename VT<R>::V2;
     const V2* col = reinterpret_cast<const V2*>(stage + lane * STAGE_LD);
-    R s0 = R(0), s1 = R(0), s2 = R(0), s3 = R(0);
+    R s[8];
 #pragma unroll
-    for (int i = 0; i < 16; i += 2) { const V2 a = col[i], b = col[i + 1]; s0 += a.x; s1 += a.y; s2 += b.x; s3 += b.y; }
-    return (double)((s0 + s1) + (s2 + s3));
+    for (int q = 0; q < 4; ++q) { const V2 a = col[q]; s[2 * q] = a.x; s[2 * q + 1] = a.y; }
+#pragma unroll
+    for (int i = 4; i < 16; i += 4)
+#pragma unroll
+        for (int q = 0; q < 4; ++q) { const V2 a = col[i + q]; s[2 * q] += a.x; s[2 * q + 1] += a.y; }
+    return (double)(((s[0] + s[1]) + (s[2] + s[3])) + ((s[4] + s[5]) + (s[6] + s[7])));
 }
 
 // Scratch between the two passes, one entry per (piece or node, lane), a warp's 32 entries contiguous.
@@ -508,7 +513,7 @@ __device__ __forceinline__ void march_round(const MarchArgsT<R>& A, const WarpJo
     cplx_t<R> T0 = mk(R(0), R(0));                             // T of the entry piece, kept for pass 2 when not spilled
     {
         // the step across piece p lands on node p-1: entry p (ST) or entry p-1 (gamma~ only)
-        char* e = scr + (size_t)(nn - 1 + NB) * ROW;
+        char* e = scr + (size_t)(HALF ? (nn - 1) >> 1 : nn - 1 + NB) * ROW;   // HALF: successive spills go to successive lower rows
         int p = nn;
         for (int c = ctop; c >= 0; --c) {
             if (c > 0) {
@@ -525,8 +530,7 @@ __device__ __forceinline__ void march_round(const MarchArgsT<R>& A, const WarpJo
                 const V4 cc = buf[p & (CHUNK - 1)];
                 const cplx_t<R> T = coefT(cc, false, J.len1);
                 gt = stepT(gt, R(-1), cc, T, J.len1);
-                if (HALF) { if (MODE != 2) st_ent<ST>(scr + (size_t)((nn - 1) >> 1) * ROW, T, gt); }   // the last node is always spilled
-                else if (MODE != 2 || ST) st_ent<ST>(e, T, gt);
+                if (MODE != 2 || ST) st_ent<ST>(e, T, gt);      // (HALF: the last node is always spilled)
                 e -= ROW; --p;
             }
 #pragma unroll P1_UNROLL
@@ -534,9 +538,8 @@ __device__ __forceinline__ void march_round(const MarchArgsT<R>& A, const WarpJo
                 const V4 cc = buf[p & (CHUNK - 1)];
                 const cplx_t<R> T = coefT(cc, true, J.hlen);
                 gt = stepT(gt, R(-1), cc, T, J.hlen);
-                if (HALF) { if (MODE != 2 && !(p & 1)) st_ent<ST>(scr + (size_t)((p - 1) >> 1) * ROW, T, gt); }   // landed on the odd node p-1
-                else if (MODE != 2 || ST) st_ent<ST>(e, T, gt);
-                e -= ROW;
+                if (HALF) { if (!(p & 1)) { if (MODE != 2) st_ent<ST>(e, T, gt); e -= ROW; } }   // landed on the odd node p-1: row (p-1)>>1
+                else { if (MODE != 2 || ST) st_ent<ST>(e, T, gt); e -= ROW; }
             }
             if (c == 0) {                                       // entry piece (length l0); its gamma~ is the end value
                 const V4 cc = buf[0];
