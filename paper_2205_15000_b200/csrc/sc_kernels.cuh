@@ -533,9 +533,10 @@ __device__ __forceinline__ void march_round(const MarchArgsT<R>& A, const WarpJo
                 if (MODE != 2 || ST) st_ent<ST>(e, T, gt);      // (HALF: the last node is always spilled)
                 e -= ROW; --p;
             }
+            const V4* __restrict__ bp = buf + (p & (CHUNK - 1));
 #pragma unroll P1_UNROLL
-            for (; p >= plo; --p) {
-                const V4 cc = buf[p & (CHUNK - 1)];
+            for (; p >= plo; --p, --bp) {
+                const V4 cc = *bp;
                 const cplx_t<R> T = coefT(cc, true, J.hlen);
                 gt = stepT(gt, R(-1), cc, T, J.hlen);
                 if (HALF) { if (!(p & 1)) { if (MODE != 2) st_ent<ST>(e, T, gt); e -= ROW; } }   // landed on the odd node p-1: row (p-1)>>1
@@ -581,7 +582,7 @@ __device__ __forceinline__ void march_round(const MarchArgsT<R>& A, const WarpJo
     int m = 0;
     // node m: products with gamma~(m) from its entry, then the step across piece m+1 (T from entry m+1 when spilled)
     auto node = [&](int b, const V4* pbuf, const V2* dbuf, bool exitp) {
-        const V4 cc = pbuf[(m + b) & (CHUNK - 1)]; const V2 dc = dbuf[(m + b) & (CHUNK - 1)];
+        const V4 cc = pbuf[b]; const V2 dc = dbuf[b];              // pbuf, dbuf: the batch's first records in the staged chunk
         const R len = exitp ? J.len1 : J.hlen;
         if (HALF) {                                            // batches start on even nodes: the parity of m+b is that of b
             const cplx_t<R> T = coefT(cc, !exitp, len);
@@ -631,12 +632,13 @@ __device__ __forceinline__ void march_round(const MarchArgsT<R>& A, const WarpJo
             const double part_old = part_nxt;
             if (MODE == 0 && n0 && lane < RED_NODES * RED_VALS && (m + RED_NODES) * RED_VALS + lane < npart)
                 part_nxt = J.PART[(m + RED_NODES) * RED_VALS + lane];
+            const V4* __restrict__ pb = pbuf + (m & (CHUNK - 1)); const V2* __restrict__ db = dbuf + (m & (CHUNK - 1));
             if (m + RED_NODES < nn) {
 #pragma unroll
-                for (int b = 0; b < RED_NODES; ++b) node(b, pbuf, dbuf, false);
+                for (int b = 0; b < RED_NODES; ++b) node(b, pb, db, false);
             } else {                                             // the batch ends on the trajectory's last node
 #pragma unroll
-                for (int b = 0; b < RED_NODES; ++b) node(b, pbuf, dbuf, b == RED_NODES - 1);
+                for (int b = 0; b < RED_NODES; ++b) node(b, pb, db, b == RED_NODES - 1);
             }
             e += PFROWS * ROW;
             if (MODE == 0) {
@@ -652,7 +654,7 @@ __device__ __forceinline__ void march_round(const MarchArgsT<R>& A, const WarpJo
         if (m < mhi) {                                       // ragged tail: 1..3 nodes (last chunk only)
             const int rem = mhi - m;
             const double part_old = part_nxt;
-            for (int b = 0; b < rem; ++b) node(b, pbuf, dbuf, m + b + 1 == nn);
+            for (int b = 0; b < rem; ++b) node(b, pbuf + (m & (CHUNK - 1)), dbuf + (m & (CHUNK - 1)), m + b + 1 == nn);
             if (MODE == 0) {
                 __syncwarp();
                 if (lane < rem * RED_VALS) {
