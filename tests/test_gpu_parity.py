@@ -588,3 +588,42 @@ def test_lowrank_vector_potential_matches(sc, eps):
     assert relerr(Ax.cpu().numpy(), ex) < TOL
     with pytest.raises(sc.ScError):
         ctx.sc_set_vector_potential_error(1.5)
+
+
+def test_restart_with_burnin_matches(sc):
+    """Restart from saved Delta, A (the boundary values are never saved, so a restart first iterates
+    them with Delta and A held fixed — `burnin`): 3 iterations, then a FRESH context and oracle driver continue from the
+    saved fields with 3 burn-in sweeps + 2 iterations.  The burn-in leaves Delta, A_ind untouched, the two sides agree,
+    and the burnt-in boundary values bring the restarted run closer to the uninterrupted one than a cold restart."""
+    wl = wlmod.make_workload(1, pts_per_xi=5, n_angles=16, n_energies=24)
+    def fresh():
+        o = oracle.Oracle.from_workload(wl)
+        drv = oracle.Driver(o, wl.Aext_x, wl.Aext_y, wl.n_energies, accelerator=0, step=0.3)
+        ctx = sc.ScContext.from_workload(wl); ctx.sc_set_external_field(dev(wl.Aext_x), dev(wl.Aext_y))
+        return drv, ctx
+    drv, ctx = fresh()
+    d_o = wl.delta0.copy(); ax_o = np.zeros((wl.ny, wl.nx)); ay_o = np.zeros_like(ax_o)
+    d_g = dev(wl.delta0.astype(np.complex128)).clone(); ax_g = torch.zeros((wl.ny, wl.nx), dtype=torch.float64, device="cuda"); ay_g = torch.zeros_like(ax_g)
+    for it in range(5):
+        if it == 3:
+            saved = (d_o.copy(), ax_o.copy(), ay_o.copy())
+        r = drv.iterate(d_o, ax_o, ay_o); d_o, ax_o, ay_o = r["delta"], r["Aind_x"], r["Aind_y"]
+        ctx.sc_iterate(0, 0.3, False, d_g, ax_g, ay_g)
+    uninterrupted = d_o.copy()
+    results = {}
+    for nburn in (3, 0):
+        drv, ctx = fresh()
+        d_o, ax_o, ay_o = (a.copy() for a in saved)
+        d_g = dev(d_o).clone(); ax_g = dev(ax_o).clone(); ay_g = dev(ay_o).clone()
+        for _ in range(nburn):
+            r = drv.iterate(d_o, ax_o, ay_o, burnin=True)
+            ctx.sc_iterate(0, 0.3, True, d_g, ax_g, ay_g)
+            torch.cuda.synchronize()
+            assert np.array_equal(d_g.cpu().numpy(), saved[0]) and np.array_equal(ax_g.cpu().numpy(), saved[1])
+        for _ in range(2):
+            r = drv.iterate(d_o, ax_o, ay_o); d_o, ax_o, ay_o = r["delta"], r["Aind_x"], r["Aind_y"]
+            ctx.sc_iterate(0, 0.3, False, d_g, ax_g, ay_g)
+        torch.cuda.synchronize()
+        assert relerr(d_g.cpu().numpy(), d_o) < 10 * TOL and relerr(ax_g.cpu().numpy(), ax_o) < 100 * TOL
+        results[nburn] = relerr(d_o, uninterrupted)
+    assert results[3] < 0.5 * results[0]
