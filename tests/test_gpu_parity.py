@@ -627,3 +627,30 @@ def test_restart_with_burnin_matches(sc):
         assert relerr(d_g.cpu().numpy(), d_o) < 10 * TOL and relerr(ax_g.cpu().numpy(), ax_o) < 100 * TOL
         results[nburn] = relerr(d_o, uninterrupted)
     assert results[3] < 0.5 * results[0]
+
+
+@pytest.mark.parametrize("sym,rot,nphi,quad,sigma", [
+    (wlmod.SYM_DXY, 0.07, 18, 0, -1),        # d_xy, rotated crystal axes, N % 4 != 0 but N % 3 == 0: Simpson 3/8 (:189)
+    (wlmod.SYM_G, 0.0, 10, 0, -1),           # g-wave (Table III :1238), N % 2 == 0 only: Simpson 1/3
+    (wlmod.SYM_DX2Y2, 0.125, 16, 1, -1),     # trapezoid rule selected explicitly; [110]-type walls by rotating the crystal
+    (wlmod.SYM_S, 0.0, 16, 0, +1),           # positive carriers: the Doppler shift and the current change sign (:43)
+])
+def test_options_symmetry_rotation_quadrature_charge(sc, sym, rot, nphi, quad, sigma):
+    import dataclasses
+    wl = wlmod.make_workload(1, pts_per_xi=4, n_angles=nphi, n_energies=12)
+    wl = dataclasses.replace(wl, symmetry=sym, crystal_rotation=rot, charge_sign=sigma)
+    o = oracle.Oracle.from_workload(wl, quadrature=quad)
+    ctx = sc.ScContext.from_workload(wl, quadrature=quad)
+    ctx.sc_set_fields(dev(wl.delta0.astype(np.complex128)), dev(wl.Aext_x), dev(wl.Aext_y))
+    dn = torch.zeros((wl.ny, wl.nx), dtype=torch.complex128, device="cuda")
+    jx = torch.zeros((wl.ny, wl.nx), dtype=torch.float64, device="cuda"); jy = torch.zeros_like(jx); fe = torch.zeros_like(jx)
+    stores = None
+    for it in range(2):
+        ro = o.sweep(wl.delta0, wl.Aext_x, wl.Aext_y, wl.n_energies, stores); stores = ro["stores"]
+        st = ctx.sc_riccati_sweep(dn, jx, jy, fe, want_stats=True)
+        torch.cuda.synchronize()
+        assert relerr(dn.cpu().numpy(), ro["delta_new"]) < TOL and relerr(jx.cpu().numpy(), ro["jx"]) < TOL
+        assert relerr(jy.cpu().numpy(), ro["jy"]) < TOL and relerr(fe.cpu().numpy(), ro["fe_I"]) < TOL
+        assert st.n_bad == 0
+    with pytest.raises(sc.ScError):          # odd angle counts have no k + N/2 partner (Eq. 13)
+        sc.ScContext.from_workload(dataclasses.replace(wl, n_angles=9))
