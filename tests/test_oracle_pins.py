@@ -629,3 +629,43 @@ def test_lowrank_vector_potential_against_the_full_correlation():
         assert np.max(np.abs(ax - ex)) <= bound * (1 + 1e-9) + 1e-15
         last = ns
     assert last > 3                                                                            # eps = 1e-6 needs several pairs
+
+
+# ---- Fermi-surface quadrature (:189) and basis functions (Table III :1238-1246) ---------------------------------------
+@pytest.mark.parametrize("nphi,order", [(64, 4), (20, 4), (18, 3), (10, 2), (7, 1)])
+def test_quadrature_weights_are_the_composite_newton_cotes_rules(nphi, order):
+    """:189 "Boole's rule, Simpson's 3/8 rule, Simpson's 1/3 rule or the trapezoidal rule depending on N_phi mod 4, 3, 2":
+    the periodic composite rule built from scipy's closed Newton-Cotes coefficients of that order."""
+    from scipy.integrate import newton_cotes
+    an, _ = newton_cotes(order, 1)                       # weights on 0..order for spacing 1
+    w = np.zeros(nphi)
+    for start in range(0, nphi, order):
+        for i, a in enumerate(an):
+            w[(start + i) % nphi] += a
+    w /= nphi                                            # spacing 1/N_phi of the unit circle average
+    sq = make_mask([square(0.4)], 4, 4, 0.1)
+    o = oracle.Oracle(4, 4, 0.1, sq, [square(0.4)], 0.5, 0, nphi)
+    W = np.array([o.angle_info(k)[2] for k in range(nphi)])
+    assert np.max(np.abs(W - w)) < 1e-15 and abs(W.sum() - 1.0) < 1e-14
+    if nphi % 2 == 0:
+        ot = oracle.Oracle(4, 4, 0.1, sq, [square(0.4)], 0.5, 0, nphi, quadrature=1)
+        assert np.allclose([ot.angle_info(k)[2] for k in range(nphi)], 1.0 / nphi, rtol=0, atol=1e-16)
+
+
+def test_basis_functions_are_orthonormal_on_the_angle_set():
+    """<eta_i eta_j> = delta_ij (:143, used to divide Eq. 20 down to Eq. 22) for s, d_x2-y2, d_xy, g (Table III) with the
+    paper's quadrature at N_phi = 64 (the products carry frequencies <= 8, none of which aliases with the period-4
+    weight pattern), with and without a crystal-axes rotation."""
+    sq = make_mask([square(0.4)], 4, 4, 0.1)
+    for rot in (0.0, 0.031):
+        eta = []
+        for sym in range(4):
+            o = oracle.Oracle(4, 4, 0.1, sq, [square(0.4)], 0.5, sym, 64, crystal_rotation=rot)
+            info = [o.angle_info(k) for k in range(64)]
+            eta.append(np.array([e for _, e, _ in info])); W = np.array([w for _, _, w in info])
+        gram = np.array([[np.sum(W * a * b) for b in eta] for a in eta])
+        assert np.max(np.abs(gram - np.eye(4))) < 1e-13
+    # d_x2-y2 -> d_xy under a rotation of the crystal axes by 1/8 turn (:890)
+    o1 = oracle.Oracle(4, 4, 0.1, sq, [square(0.4)], 0.5, 1, 64, crystal_rotation=0.125)
+    o2 = oracle.Oracle(4, 4, 0.1, sq, [square(0.4)], 0.5, 2, 64)
+    assert max(abs(o1.angle_info(k)[1] - o2.angle_info(k)[1]) for k in range(64)) < 1e-14
