@@ -38,6 +38,8 @@ typedef struct sc_ctx sc_ctx;
 
 typedef enum { SC_OK = 0, SC_ERR_ARG = 1, SC_ERR_GEOMETRY = 2, SC_ERR_STATE = 3,
                SC_ERR_CUDA = 4, SC_ERR_NOMEM = 5, SC_ERR_NUMERIC = 6 } sc_status;
+/* SC_ERR_NUMERIC: a reduced output field (sc_riccati_sweep) or a residual (sc_iterate) is not finite.  It is only
+ * detected by calls given a stats pointer — the calls that synchronise anyway; the outputs are still written. */
 
 /* Order-parameter basis functions eta(phi) on a circular Fermi surface, Table III (:1238-1246):
  * s: 1;  d_{x2-y2}: sqrt2 cos 2phi;  d_xy: sqrt2 sin 2phi;  g: sqrt2 sin 4phi. */

@@ -143,7 +143,7 @@ struct sc_ctx {
     DevBuf<char> d_store[2]; int cur = 0; bool stores_valid = false;      // V2 of R [directed trajectory][energy]
     // scratch
     DevBuf<char> d_scr; long long scr_stride = 0; int n_slots = 0;       // scr_stride in bytes
-    DevBuf<double> d_part; DevBuf<int> d_counter; DevBuf<int> d_nbad; DevBuf<double> d_statmax; DevBuf<unsigned long long> d_nstored;
+    DevBuf<double> d_part; DevBuf<int> d_counter; DevBuf<int> d_nbad; DevBuf<int> d_nonfinite; DevBuf<double> d_statmax; DevBuf<unsigned long long> d_nstored;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     static constexpr int MEV = 64;                 // ring of event pairs around the march launches (sc_debug_march_time)
     cudaEvent_t mev[MEV][2] = {}; int mev_n = 0;
@@ -414,7 +414,7 @@ sc_status sc_create(const sc_grid* grid, const unsigned char* mask, const sc_sha
     CU(ctx->d_ndD.alloc(nodes)); CU(ctx->d_nda.alloc(nodes)); CU(ctx->d_pc.alloc((size_t)(nodes + G) * 4 * ctx->rsz())); CU(ctx->d_pmax.alloc(G));
     if (ctx->f32) CU(ctx->d_ndDr.alloc(nodes));
     CU(ctx->d_part.alloc((size_t)nodes * sck::RED_VALS));
-    CU(ctx->d_counter.alloc(1)); CU(ctx->d_nbad.alloc(1)); CU(ctx->d_nstored.alloc(2));
+    CU(ctx->d_counter.alloc(1)); CU(ctx->d_nbad.alloc(1)); CU(ctx->d_nonfinite.alloc(1)); CU(ctx->d_nstored.alloc(2));
     CU(cudaMemsetAsync(ctx->d_nbad.p, 0, sizeof(int), s)); CU(cudaMemsetAsync(ctx->d_nstored.p, 0, 2 * sizeof(unsigned long long), s));
 
     // Matsubara energies eps_n = t(n+1/2) (:98), unit weights, self-partnered (z = i eps -> -conj z = z)
@@ -540,7 +540,20 @@ sc_status sc_riccati_sweep(sc_ctx* ctx, void* delta_new, double* jx, double* jy,
                                                                                   (double2*)delta_new, jx, jy, fe_I);
         CU(cudaGetLastError());
     }
-    return fill_stats(ctx, stats, ctx->mats.ne, true);
+    if (stats) {          // SC_ERR_NUMERIC: a reduced field is not finite (checked only where the call synchronises anyway)
+        const size_t ng = (size_t)ctx->grid.nx * ctx->grid.ny;
+        CU(cudaMemsetAsync(ctx->d_nonfinite.p, 0, sizeof(int), ctx->stream));
+        const double* fields[4] = {(const double*)delta_new, jx, jy, fe_I};
+        const size_t counts[4] = {2 * ng * ctx->ncomp, ng, ng, ng};
+        for (int f = 0; f < 4; ++f)
+            if (fields[f]) sck::nonfinite_kernel<<<(unsigned)((counts[f] + 255) / 256), 256, 0, ctx->stream>>>(counts[f], fields[f], ctx->d_nonfinite.p);
+        CU(cudaGetLastError());
+        if (sc_status st = fill_stats(ctx, stats, ctx->mats.ne, true)) return st;
+        int bad = 0; CU(cudaMemcpy(&bad, ctx->d_nonfinite.p, sizeof(int), cudaMemcpyDeviceToHost));
+        if (bad) return fail(ctx, SC_ERR_NUMERIC, std::to_string(bad) + " non-finite values in the sweep's output fields");
+        return SC_OK;
+    }
+    return SC_OK;
 }
 
 sc_status sc_ldos(sc_ctx* ctx, const double* energies, int n_e, double broadening, int n_boundary_iters,
@@ -662,6 +675,8 @@ sc_status sc_iterate(sc_ctx* ctx, int accelerator, double step, int burnin, void
         if (!burnin) { if (int rc = scf::read_residuals(F, r, ctx->stream, e)) return fail(ctx, SC_ERR_CUDA, e); }
         stats->res_delta = r[0]; stats->res_A = r[1]; stats->res_j = r[2]; stats->res_fe = r[3];
         stats->min_one_minus_abs_gamma = 0.0;
+        if (!std::isfinite(r[0]) || !std::isfinite(r[1]) || !std::isfinite(r[2]) || !std::isfinite(r[3]))
+            return fail(ctx, SC_ERR_NUMERIC, "non-finite residual: the iterate has diverged or an input field is not finite");
     }
     return SC_OK;
 }

@@ -867,6 +867,12 @@ __global__ void finalise_kernel(size_t ng, int nc, const double* raw, double t, 
     if (feI) feI[q] = t * raw[(2 * nc + 2) * ng + q];
 }
 
+// counts the non-finite values of a reduced field (SC_ERR_NUMERIC; only run when the caller asked for stats)
+__global__ void nonfinite_kernel(size_t n, const double* a, int* count) {
+    const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q < n && !isfinite(a[q])) atomicAdd(count, 1);
+}
+
 // LDOS rotate-back: thread per (grid point, energy); energies fastest so the gathers coalesce.
 struct BackLdosArgs {
     BackArgs B;

@@ -654,3 +654,22 @@ def test_options_symmetry_rotation_quadrature_charge(sc, sym, rot, nphi, quad, s
         assert st.n_bad == 0
     with pytest.raises(sc.ScError):          # odd angle counts have no k + N/2 partner (Eq. 13)
         sc.ScContext.from_workload(dataclasses.replace(wl, n_angles=9))
+
+
+def test_non_finite_fields_are_reported(sc):
+    """SC_ERR_NUMERIC (status 6) from the calls that synchronise: a NaN in Delta poisons the trajectories through it."""
+    wl = wlmod.make_workload(0)
+    g = GpuRun(sc, wl)
+    d = wl.delta0.astype(np.complex128).copy(); d[wl.ny // 2, wl.nx // 2] = np.nan
+    g.set_fields(d, None, None)
+    with pytest.raises(sc.ScError) as e:
+        g.sweep(stats=True)
+    assert e.value.status == 6
+    g.ctx.sc_riccati_sweep(g.dn, g.jx, g.jy, g.fe)          # without stats the call does not synchronise and cannot report
+    dd = dev(d).clone()
+    with pytest.raises(sc.ScError) as e:
+        g.ctx.sc_iterate(0, 1.0, False, dd, want_stats=True)
+    assert e.value.status == 6
+    g.set_fields(wl.delta0, None, None)                      # the context stays usable
+    g.ctx.sc_reset_boundary()
+    assert np.all(np.isfinite(g.sweep()["delta_new"]))
