@@ -528,8 +528,8 @@ sc_status sc_riccati_sweep(sc_ctx* ctx, void* delta_new, double* jx, double* jy,
     ctx->cur ^= 1;
     sck::BackArgs B = back_args(ctx, delta_new, jx, jy, fe_I);
     B.raw = ctx->hook_fn ? ctx->hook_acc : nullptr;
-    dim3 grd((ctx->grid.nx + 127) / 128, ctx->grid.ny);
-    sck::rotate_back_kernel<<<grd, 128, 0, ctx->stream>>>(B);
+    dim3 grd((ctx->grid.nx + sck::BACK_TX - 1) / sck::BACK_TX, (ctx->grid.ny + sck::BACK_TY - 1) / sck::BACK_TY);
+    sck::rotate_back_kernel<<<grd, dim3(sck::BACK_TX, sck::BACK_TY), 0, ctx->stream>>>(B);
     CU(cudaGetLastError());
     if (ctx->hook_fn) {
         // energy-sharded sweep: the caller sums the raw accumulators of all shards on this stream, then a7 runs

@@ -802,9 +802,15 @@ __device__ __forceinline__ int back_weights(const BackArgs& B, int p, double x, 
     return 1;
 }
 
-__global__ void rotate_back_kernel(BackArgs B) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
-    if (i >= B.G.nx) return;
+// 2-D thread tiles (BACK_TX x BACK_TY grid points): neighbouring points share lattice nodes, so a compact tile re-uses
+// the gathered `part` lines in L1 instead of fetching them again from L2
+#ifndef SC_BACK_TY
+#define SC_BACK_TY 8
+#endif
+constexpr int BACK_TX = 16, BACK_TY = SC_BACK_TY;
+__global__ void __launch_bounds__(BACK_TX * BACK_TY) rotate_back_kernel(BackArgs B) {
+    const int i = blockIdx.x * BACK_TX + threadIdx.x, j = blockIdx.y * BACK_TY + threadIdx.y;
+    if (i >= B.G.nx || j >= B.G.ny) return;
     const size_t q = (size_t)j * B.G.nx + i;
     const int nc = B.G.ncomp;
     double nr[MAX_COMP], ni[MAX_COMP], sjx = 0.0, sjy = 0.0, sI = 0.0;
