@@ -673,3 +673,21 @@ def test_non_finite_fields_are_reported(sc):
     g.set_fields(wl.delta0, None, None)                      # the context stays usable
     g.ctx.sc_reset_boundary()
     assert np.all(np.isfinite(g.sweep()["delta_new"]))
+
+
+@pytest.mark.parametrize("kw,tol", [(dict(precision=32), 2e-4), (dict(stepper=1), 1e-9)])
+def test_two_components_in_fp32_and_with_the_midpoint_stepper(sc, kw, tol):
+    wl, syms, tc, delta = _two_component_case("s+dxy vortex disc")
+    o = oracle.Oracle.from_workload(wl, **{k: v for k, v in kw.items() if k == "stepper"}); o.set_components(syms, tc)
+    ctx = sc.ScContext.from_workload(wl, **kw); ctx.sc_set_components(syms, tc)
+    ctx.sc_set_fields(dev(delta), dev(wl.Aext_x), dev(wl.Aext_y))
+    dn = torch.zeros((2, wl.ny, wl.nx), dtype=torch.complex128, device="cuda")
+    jx = torch.zeros((wl.ny, wl.nx), dtype=torch.float64, device="cuda"); jy = torch.zeros_like(jx); fe = torch.zeros_like(jx)
+    stores = None
+    for it in range(2):
+        ro = o.sweep(delta, wl.Aext_x, wl.Aext_y, wl.n_energies, stores); stores = ro["stores"]
+        ctx.sc_riccati_sweep(dn, jx, jy, fe)
+        torch.cuda.synchronize()
+        for c in range(2):
+            assert relerr(dn.cpu().numpy()[c], ro["delta_new"][c]) < tol, (it, c)
+        assert relerr(jx.cpu().numpy(), ro["jx"]) < tol and relerr(fe.cpu().numpy(), ro["fe_I"]) < tol
