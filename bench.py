@@ -37,19 +37,21 @@ UNIT = "updates/s"
 # FP64-pipe instructions the closed-form path needs per unit = (piece, energy, angle pair) = 4 logical updates
 # (gamma and gamma-tilde for angles k and k+N/2): DESIGN.md §6 tally of the kernel's own algorithm.
 #   "recompute" rounds (every piece inside the radius of the per-energy Taylor table of T): T twice 2 x 15, two Moebius
-#       steps 2 x 27, node products 28, energy reduction 8 = 120, + half a Moebius step 13.5 because only every second
-#       gamma-tilde is spilled and the other is re-stepped in pass 2 = 133.5; scratch traffic 8 B written + 8 B read = 16 B
+#       steps 2 x 27, node products 26 (28 with non-unit weights; the bench's Matsubara table has unit weights and the
+#       kernel variant with the weights compiled out runs), energy reduction 8 = 118, + half a Moebius step 13.5 because
+#       only every second gamma-tilde is spilled and the other is re-stepped in pass 2 = 131.5; scratch traffic 8 B
+#       written + 8 B read = 16 B
 #   "recompute_pole" rounds (|a| beyond that table but inside the pole-subtracted one): T twice 2 x 24 (degree 5 + the
-#       pole term with one reciprocal), 54, 28, 8, 13.5 = 151.5; 16 B per unit
-#   "stored-T" rounds (strong vector potential): T once from the pole-subtracted table 36, 54, 28, 8 = 126; 64 B per unit
+#       pole term with one reciprocal), 54, 26, 8, 13.5 = 149.5; 16 B per unit
+#   "stored-T" rounds (strong vector potential): T once from the pole-subtracted table 36, 54, 26, 8 = 124; 64 B per unit
 # Evaluating T from its definition (sqrt, exp, sin/cos) would be 86 per evaluation — reported as context only.
-ALGO_FP64_INSTR_PER_UNIT = {"recompute": 133.5, "recompute_pole": 151.5, "stored": 126.0}
+ALGO_FP64_INSTR_PER_UNIT = {"recompute": 131.5, "recompute_pole": 149.5, "stored": 124.0}
 # the least FP64 work any of these layouts could do per unit if nothing were evaluated twice: T once 15, two steps 54,
-# node products 28, reduction 8 — reported beside the roofline so that recomputation is not mistaken for useful work
-MIN_WORK_FP64_INSTR_PER_UNIT = 105.0
+# node products 26, reduction 8 — reported beside the roofline so that recomputation is not mistaken for useful work
+MIN_WORK_FP64_INSTR_PER_UNIT = 103.0
 ALGO_HBM_BYTES_PER_UNIT = {"recompute": 16.0, "recompute_pole": 16.0, "stored": 64.0}
 TEXTBOOK_FP64_INSTR_PER_UNIT = 184.0
-ALGO_FP64_INSTR_PER_UNIT_MIDPOINT = 2 * 66.0 + 28.0 + 8.0
+ALGO_FP64_INSTR_PER_UNIT_MIDPOINT = 2 * 66.0 + 28.0 + 8.0     # the mid-point kernels keep the weights
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE march launch at configs[4], fp64, closed-form stepper, all rounds in
 # "recompute" mode (--sweep-only: A = A_ext), from the `ncu --set full` capture summarised in profiles/
 # (profiles/r1_march_fp64_cfg4_ncu_full.md: 1.512 TB read + 1.255 TB written)

@@ -273,7 +273,9 @@ __device__ __forceinline__ cplx_t<R> hom_start(double Dr, double Di, double zr, 
 
 // products at one node (Eq. 24 :165): P = gamma gamma~, 1/(1+P); writes the six weighted terms of the
 // energy sums into rows r..r+5 of the warp's transpose stage (MODE 0), or returns Re g (MODE 1)
-template <int MODE, bool STATS, typename R>
+// UW: every weight of the energy table is 1 and every lane is active (plain Matsubara sums over a multiple of 32 energies):
+// the two multiplications by w_n are compiled out (bitwise the same result)
+template <int MODE, bool STATS, typename R, bool UW>
 __device__ __forceinline__ R node_products(cplx_t<R> gm, R gtr, R gti, typename VT<R>::V2 Dn, R wn, R* st, R& max2) {
     using scm::mad;
     const R Pr = mad(gm.re, gtr, -gm.im * gti), Pi = mad(gm.re, gti, gm.im * gtr);
@@ -281,14 +283,15 @@ __device__ __forceinline__ R node_products(cplx_t<R> gm, R gtr, R gti, typename 
     const R rq = scm::rcp_nr(mad(qr, qr, Pi * Pi));
     if (STATS) max2 = scm::maxr(max2, scm::maxr(mad(gm.re, gm.re, gm.im * gm.im), mad(gtr, gtr, gti * gti)));
     if (MODE == 0) {
-        const R wq = wn * rq;
+        const R wq = UW ? rq : wn * rq;
         const R wr = qr * wq, wi = -Pi * wq;                 // w/(1+P)
         st[0 * STAGE_LD] = mad(gm.re, wr, -gm.im * wi);      // SF  = w gamma/(1+P)
         st[1 * STAGE_LD] = mad(gm.re, wi, gm.im * wr);
         st[2 * STAGE_LD] = mad(gtr, wr, -gti * wi);          // X2  = w gamma~/(1+P)  (SF of k+N/2 = conj)
         st[3 * STAGE_LD] = mad(gtr, wi, gti * wr);
         st[4 * STAGE_LD] = wi + wi;                          // SG  = w Im g = 2 w Im 1/(1+P)
-        st[5 * STAGE_LD] = wn * mad(Dn.x, gm.im - gti, -Dn.y * (gm.re + gtr));   // SI (Eq. 19 :128 numerator)
+        const R si = mad(Dn.x, gm.im - gti, -Dn.y * (gm.re + gtr));
+        st[5 * STAGE_LD] = UW ? si : wn * si;   // SI (Eq. 19 :128 numerator)
     }
     return mad(R(2) * qr, rq, R(-1));                        // Re g = 2 Re 1/(1+P) - 1
 }
@@ -460,7 +463,7 @@ struct WarpJob {
 // MODE 0: Matsubara sums; 1: per-energy Re g (LDOS); 2: boundary values only.
 // STEP 0: closed-form step; 1: implicit mid-point rule (C4-C9 :984-1001).
 // ST: T spilled with gamma-tilde (see ScrT).  TM: layout of the T table.
-template <int MODE, bool STATS, int STEP, typename R, bool ST, typename TAB>
+template <int MODE, bool STATS, int STEP, typename R, bool ST, bool UW, typename TAB>
 __device__ __forceinline__ void march_round(const MarchArgsT<R>& A, const WarpJob<R>& J, const TAB& tab, int n0, R& max2) {
     using V2 = typename VT<R>::V2; using V4 = typename VT<R>::V4;
     constexpr int ROW = ScrT<R, ST>::ROW, BYTES = ScrT<R, ST>::BYTES;
@@ -594,7 +597,7 @@ __device__ __forceinline__ void march_round(const MarchArgsT<R>& A, const WarpJo
                 gth = exitp ? G : stepT(G, R(-1), cc, T, len);
             }
             if (MODE != 2) {
-                const R rg = node_products<MODE, STATS, R>(gm, gth.re, gth.im, dc, wn, J.stage + b * RED_VALS * STAGE_LD + lane, max2);
+                const R rg = node_products<MODE, STATS, R, UW>(gm, gth.re, gth.im, dc, wn, J.stage + b * RED_VALS * STAGE_LD + lane, max2);
                 if (MODE == 1 && act) A.ldos[(size_t)(J.noff + m + b) * ne + n] = (double)rg;
             }
             gm = stepT(gm, R(1), cc, T, len);
@@ -603,7 +606,7 @@ __device__ __forceinline__ void march_round(const MarchArgsT<R>& A, const WarpJo
         const Ent<R> Ec = En;
         if (LD) { En = En2; En2 = ld_ent<ST>(e + (b + 2) * ROW, R(0)); }   // two entries ahead (the scratch has spare rows)
         if (MODE != 2) {
-            const R rg = node_products<MODE, STATS, R>(gm, Ec.gr, Ec.gi, dc, wn, J.stage + b * RED_VALS * STAGE_LD + lane, max2);
+            const R rg = node_products<MODE, STATS, R, UW>(gm, Ec.gr, Ec.gi, dc, wn, J.stage + b * RED_VALS * STAGE_LD + lane, max2);
             if (MODE == 1 && act) A.ldos[(size_t)(J.noff + m + b) * ne + n] = (double)rg;
         }
         // ST: the entry of node m+b is the entry of piece m+b+1, the step that leaves the node: it holds that T
@@ -671,7 +674,7 @@ __device__ __forceinline__ void march_round(const MarchArgsT<R>& A, const WarpJo
     if (act) A.store_new[(size_t)J.dF * ne + n] = mk2(gm.re, gm.im);
 }
 
-template <int MODE, bool STATS, int STEP, typename R, int TM>
+template <int MODE, bool STATS, int STEP, typename R, int TM, bool UW = false>
 __global__ void __launch_bounds__(MARCH_WARPS * 32, MARCH_MIN_CTAS) march_kernel(MarchArgsT<R> A) {
     using V2 = typename VT<R>::V2; using V4 = typename VT<R>::V4;
     extern __shared__ double4 smem_raw[];
@@ -708,22 +711,22 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32, MARCH_MIN_CTAS) march_kernel
                     using Short = TTabPole<R, scm::TaylorPoleShortK<R>>;
                     if (!__any_sync(0xffffffffu, !Short::covers(A.E, n, pm))) {
                         Short tab; tab.load(A.E, n);
-                        march_round<MODE, STATS, STEP, R, false>(A, J, tab, n0, max2);
+                        march_round<MODE, STATS, STEP, R, false, UW>(A, J, tab, n0, max2);
                         npl += (unsigned long long)(J.nn + 1) * min(32, J.ne - n0);
                     } else {
                         TTabPole<R, scm::TaylorPoleK<R>> tab; tab.load(A.E, n);
-                        march_round<MODE, STATS, STEP, R, true>(A, J, tab, n0, max2);
+                        march_round<MODE, STATS, STEP, R, true, UW>(A, J, tab, n0, max2);
                         nst += (unsigned long long)(J.nn + 1) * min(32, J.ne - n0);
                     }
                 } else {
                     TTab<R, TM> tab; tab.load(A.E, n);
-                    march_round<MODE, STATS, STEP, R, true>(A, J, tab, n0, max2);
+                    march_round<MODE, STATS, STEP, R, true, UW>(A, J, tab, n0, max2);
                     nst += (unsigned long long)(J.nn + 1) * min(32, J.ne - n0);
                 }
             } else {
                 TTab<R, TM> tab;
                 if (STEP == 0) tab.load(A.E, n);
-                march_round<MODE, STATS, STEP, R, false>(A, J, tab, n0, max2);
+                march_round<MODE, STATS, STEP, R, false, UW>(A, J, tab, n0, max2);
             }
         }
     }
