@@ -273,7 +273,7 @@ def run_ours(a):
         peak = 2.0 * 148 * 128 * (clocks.get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
         peak_kind = "nominal fp32 pipe: 148 SMs x 128 FMA lanes x max SM clock"
     key = (wl.cfg, a.precision, a.stepper)
-    roofline = {"bound": "alu", "kernel": "sck::march_kernel<0,false,%d,%s,1>" % (a.stepper, "double" if a.precision == 64 else "float"),
+    roofline = {"bound": "alu", "kernel": "sck::march_kernel<0,false,%d,%s,1,%s>" % (a.stepper, "double" if a.precision == 64 else "float", "true" if a.stepper == 0 else "false"),
                 "launches_timed": march_launches, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                 "frac": achieved / peak,
                 "traffic": NCU_TRAFFIC_BYTES.get(key) if full_size else None,
