@@ -54,9 +54,9 @@ TEXTBOOK_FP64_INSTR_PER_UNIT = 184.0
 ALGO_FP64_INSTR_PER_UNIT_MIDPOINT = 2 * 66.0 + 28.0 + 8.0     # the mid-point kernels keep the weights
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE march launch at configs[4], fp64, closed-form stepper, all rounds in
 # "recompute" mode (--sweep-only: A = A_ext), from the `ncu --set full` capture summarised in profiles/
-# (profiles/r1_march_fp64_cfg4_ncu_full.md: 1.512 TB read + 1.255 TB written)
-NCU_TRAFFIC_BYTES = {(4, 64, 0): 2.766660e12}
-NCU_PIPE_FP64_ACTIVE_PCT = {(4, 64, 0): 74.1}
+# (profiles/r1_march_fp64_cfg4_ncu_full.md: 1.518 TB read + 1.255 TB written)
+NCU_TRAFFIC_BYTES = {(4, 64, 0): 2.773331e12}
+NCU_PIPE_FP64_ACTIVE_PCT = {(4, 64, 0): 74.3}
 
 
 class ClockSampler(threading.Thread):
