@@ -209,9 +209,6 @@ def run_ours(a):
             ctx.sc_iterate(acc, 1.0, False, delta, aix, aiy)
 
     dev_ax, dev_ay = dev(wl.Aext_x), dev(wl.Aext_y)
-    # launches of OUR kernels per step: rotate_in, march, rotate_back (+ memset) ; A-solve: 3 reductions + 2x(pad, mul,
-    # crop) [+ 4 cuFFT library launches, not counted]; mixing: diff, 2x3 reduction stages, alpha, increment, residual, update
-    launches_per_step = 3 if a.sweep_only else (3 + (3 + 6 if wl.kappa > 0 else 0) + (1 + 2 + 1 + 1 + 4 + 1 + 1))
 
     for _ in range(max(a.warmup, 3)):
         step()
@@ -223,6 +220,7 @@ def run_ours(a):
     torch.cuda.synchronize()
     ctx.sc_debug_march_time()                       # reset: count only the march launches of the timed steps
     ctx.sc_debug_march_units()
+    ctx.sc_debug_launch_count()
     e0.record()
     for _ in range(a.steps):
         step()
@@ -232,6 +230,8 @@ def run_ours(a):
         dist.barrier()
     ms = e0.elapsed_time(e1)
     clocks = sampler.stop()
+    gpu_launches = ctx.sc_debug_launch_count()      # kernels of the library launched by the timed steps (counted at the launch sites)
+    timed_kernel = ctx.sc_debug_last_march_variant()
     march_total_ms, march_launches = ctx.sc_debug_march_time()      # CUDA events around each march launch of the timed region
     units_timed, units_timed_stored, units_timed_pole = ctx.sc_debug_march_units()     # units of those launches, by mode
     if world > 1:                                   # device time of the slowest rank
@@ -273,7 +273,7 @@ def run_ours(a):
         peak = 2.0 * 148 * 128 * (clocks.get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
         peak_kind = "nominal fp32 pipe: 148 SMs x 128 FMA lanes x max SM clock"
     key = (wl.cfg, a.precision, a.stepper)
-    roofline = {"bound": "alu", "kernel": "sck::march_kernel<0,false,%d,%s,1,%s>" % (a.stepper, "double" if a.precision == 64 else "float", "true" if a.stepper == 0 else "false"),
+    roofline = {"bound": "alu", "kernel": "sck::" + timed_kernel,
                 "launches_timed": march_launches, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                 "frac": achieved / peak,
                 "traffic": NCU_TRAFFIC_BYTES.get(key) if full_size else None,
@@ -361,7 +361,7 @@ def run_ours(a):
                     "note": "the e2e steps continue the same self-consistency run (iterations after the timed ones): as the "
                             "Barzilai-Borwein transient of A_ind decays more rounds take the cheaper table tiers, so a step here "
                             "can be faster than a timed one although it also pays the host copies"},
-            "gpu_launches": launches_per_step * a.steps, "roofline": roofline}
+            "gpu_launches": gpu_launches, "roofline": roofline}
     if fp32_leg:
         line["config"]["fp32_mode"] = fp32_leg
     if not a.no_cpu_baseline and rank == 0:

@@ -179,6 +179,12 @@ sc_status sc_debug_trajectory(sc_ctx* ctx, int k, int local, int n_energy, int* 
 /* Per-angle energy-summed node sums of the last sweep for angle k on the rotated lattice [t][j] (host out,
  * N_rot*N_rot each; SF complex): SF = sum gamma/(1+P), SG = sum Im g, SI (Eq. 19 numerator). */
 sc_status sc_debug_partial(sc_ctx* ctx, int k, void* SF, double* SG, double* SI);
+/* The boundary values the LAST sweep's march launch wrote (the production launch itself, not a re-march): for every
+ * trajectory of angle k (all N_phi angles are addressable, in the order of sc_debug_tables) and every energy of the
+ * table, gamma at the exit point and gamma-tilde at the entry point (host out, complex fp64 [n_traj(k)][n_energies] each).
+ * The library stores gamma_end for all directed trajectories only; gamma-tilde_end of (k, t) is returned as the conjugate
+ * of gamma_end of the mirror trajectory on angle k + N/2 at the partner energy (Eq. 13 :95). */
+sc_status sc_debug_stores(sc_ctx* ctx, int k, void* gamma_end, void* gamma_tilde_end);
 /* Device-math self test: max relative error of the fp64 reciprocal / rsqrt / exp / sincos building blocks
  * against the CUDA math library on n random arguments (host out, 6 values). */
 sc_status sc_debug_math(sc_ctx* ctx, int n, double* max_rel_err);
@@ -203,6 +209,15 @@ sc_status sc_debug_march_time(sc_ctx* ctx, float* total_ms, int* n_launches);
  * pass 2 from the pole-subtracted table; the rest re-evaluated it from the pole-free table (both 32 B per unit;
  * DESIGN.md 4-6); synchronises, then resets.  Any output may be NULL. */
 sc_status sc_debug_march_units(sc_ctx* ctx, long long* units_total, long long* units_stored_T, long long* units_pole_table);
+
+/* Template arguments of the most recent march launch, e.g. "march_kernel<0,false,0,double,1,true>" =
+ * <MODE 0 sums / 1 LDOS / 2 boundary only, STATS, STEPPER, working precision, T-table layout 1 imaginary axis / 2 general,
+ * unit weights compiled out> (name: host out, len bytes).  The parity tests assert with it that the instantiation
+ * bench.py times is the one they compared with the oracle.  SC_ERR_STATE before the first sweep. */
+sc_status sc_debug_last_march_variant(sc_ctx* ctx, char* name, int len);
+/* Kernels of this library launched by the calling host thread since the previous call of this function (counted at the
+ * launch sites; cuFFT / cuBLAS / cuSOLVER launches, memsets and copies are not included); resets.  n_kernels may be NULL. */
+sc_status sc_debug_launch_count(sc_ctx* ctx, long long* n_kernels);
 
 const char* sc_last_error(const sc_ctx* ctx);
 const char* sc_version(void);

@@ -256,9 +256,9 @@ class Oracle:
         Jx = np.zeros((ny, nx)); Jy = np.zeros((ny, nx)); Ia = np.zeros((ny, nx)); Ra = np.zeros((ny, nx))
         al = None if angle_list is None else np.ascontiguousarray(angle_list, np.int32)
         dbg = None
-        if dbg_angle >= 0:
-            dbg = dict(SF=np.zeros((self.nrot, self.nrot), np.complex128), SG=np.zeros((self.nrot, self.nrot)),
-                       SI=np.zeros((self.nrot, self.nrot)), SR=np.zeros((self.nrot, self.nrot)))
+        if dbg_angle >= 0 or dbg_angle == -2:        # -2: the node sums of every angle of angle_list, [len(angle_list)][nrot][nrot]
+            shp = (self.nrot, self.nrot) if dbg_angle >= 0 else (len(al), self.nrot, self.nrot)
+            dbg = dict(SF=np.zeros(shp, np.complex128), SG=np.zeros(shp), SI=np.zeros(shp), SR=np.zeros(shp))
         gmin = np.zeros(1); nupd = np.zeros(1, np.int64); bad = np.zeros(1, np.int32)
         lib().orc_sweep(self._h, _p(delta), _p(Ax), _p(Ay), ne, _p(_f64(z.real)), _p(_f64(z.imag)), _p(w),
                         _p(g_old), _p(gt_old), _p(g_new), _p(gt_new), _p(num), _p(Jx), _p(Jy), _p(Ia), _p(Ra),

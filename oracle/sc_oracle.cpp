@@ -539,6 +539,7 @@ int orc_reset_stores(void* p, const double* delta, const double* Ax, const doubl
                      const double* zre, const double* zim, double* g_store, double* gt_store) {
     Ctx* C = (Ctx*)p; const cd* D = (const cd*)delta; cd* gs = (cd*)g_store; cd* gts = (cd*)gt_store;
     int bad = 0;
+#pragma omp parallel for schedule(dynamic, 1) reduction(+ : bad)
     for (int k = 0; k < C->nphi; ++k)
         for (size_t i = 0; i < C->traj[k].size(); ++i) {
             Pieces P; make_pieces(*C, C->traj[k][i], D, Ax, Ay, P, &bad);
@@ -633,9 +634,12 @@ int orc_sweep(void* p, const double* delta, const double* Ax, const double* Ay,
             }
             for (int m = 0; m < nn; ++m) valid[(size_t)T.t * C->nrot + (T.jf + m)] = 1;
         }
-        if (k == dbg_angle && dbg_SF) {
-            std::memcpy(dbg_SF, SF.data(), nl * sizeof(cd)); std::memcpy(dbg_SG, SG.data(), nl * sizeof(double));
-            std::memcpy(dbg_SI, SI.data(), nl * sizeof(double)); std::memcpy(dbg_SR, SR.data(), nl * sizeof(double));
+        // parity tap: the per-angle node sums of angle dbg_angle, or (dbg_angle == -2) of every angle of angle_list,
+        // [position in angle_list][N_rot][N_rot]
+        if ((k == dbg_angle || dbg_angle == -2) && dbg_SF) {
+            size_t o = dbg_angle == -2 ? (size_t)ia * nl : 0;
+            std::memcpy(dbg_SF + 2 * o, SF.data(), nl * sizeof(cd)); std::memcpy(dbg_SG + o, SG.data(), nl * sizeof(double));
+            std::memcpy(dbg_SI + o, SI.data(), nl * sizeof(double)); std::memcpy(dbg_SR + o, SR.data(), nl * sizeof(double));
         }
 #pragma omp ordered
         {

@@ -59,8 +59,8 @@ class SweepStats:
 
 
 def lib_path() -> str:
-    """In-tree library; SC_RICCATI_LIB overrides it (build-variant experiments)."""
-    return os.environ.get("SC_RICCATI_LIB") or os.path.join(_HERE, "libsc_riccati.so")
+    """The in-tree library built by `paper_2205_15000_b200.build`."""
+    return os.path.join(_HERE, "libsc_riccati.so")
 
 
 def declared_symbols() -> list:
@@ -107,12 +107,15 @@ def load_library():
     L.sc_debug_tables.argtypes = [vp, i, C.POINTER(i), vp, vp, vp, vp]
     L.sc_debug_trajectory.argtypes = [vp, i, i, i, C.POINTER(i), vp, vp]
     L.sc_debug_partial.argtypes = [vp, i, vp, vp, vp]
+    L.sc_debug_stores.argtypes = [vp, i, vp, vp]
     L.sc_debug_math.argtypes = [vp, i, vp]
     L.sc_debug_fp64_peak.argtypes = [vp, C.POINTER(d), C.POINTER(d)]
     L.sc_debug_last_march_ms.argtypes = [vp, C.POINTER(C.c_float)]
     L.sc_debug_fp64_peak_sustained.argtypes = [vp, d, C.POINTER(d)]
     L.sc_debug_march_time.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(i)]
     L.sc_debug_march_units.argtypes = [vp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
+    L.sc_debug_last_march_variant.argtypes = [vp, C.c_char_p, i]
+    L.sc_debug_launch_count.argtypes = [vp, C.POINTER(C.c_longlong)]
     _lib = L
     return L
 
@@ -217,6 +220,7 @@ class ScContext:
         zr = np.ascontiguousarray(z.real); zi = np.ascontiguousarray(z.imag); w = np.ascontiguousarray(w, np.float64)
         self._check(self._L.sc_set_energies(self._h, zr.ctypes.data_as(C.c_void_p), zi.ctypes.data_as(C.c_void_p),
                                             w.ctypes.data_as(C.c_void_p), len(zr), float(denominator_sum)))
+        self.n_matsubara = len(zr)
 
     def sc_set_allreduce_hook(self, acc, fn):
         """acc: CUDA fp64 tensor [2 n_components + 3][ny][nx]; fn(): enqueues the all-reduce of acc on the context's stream."""
@@ -298,6 +302,15 @@ class ScContext:
                                              SI.ctypes.data_as(C.c_void_p)))
         return SF, SG, SI
 
+    def sc_debug_stores(self, k, n_energies=None):
+        """(gamma_end, gamma_tilde_end) [n_traj(k)][n_energies] written by the last sweep's march launch."""
+        n = C.c_int()
+        self._check(self._L.sc_debug_tables(self._h, k, C.byref(n), None, None, None, None))
+        ne = n_energies or self.n_matsubara
+        G = np.zeros((n.value, ne), np.complex128); GT = np.zeros((n.value, ne), np.complex128)
+        self._check(self._L.sc_debug_stores(self._h, k, G.ctypes.data_as(C.c_void_p), GT.ctypes.data_as(C.c_void_p)))
+        return G, GT
+
     def sc_debug_math(self, n=2000):
         out = np.zeros(6)
         self._check(self._L.sc_debug_math(self._h, n, out.ctypes.data_as(C.c_void_p)))
@@ -322,6 +335,17 @@ class ScContext:
         a, b, c = C.c_longlong(), C.c_longlong(), C.c_longlong()
         self._check(self._L.sc_debug_march_units(self._h, C.byref(a), C.byref(b), C.byref(c)))
         return a.value, b.value, c.value
+
+    def sc_debug_last_march_variant(self):
+        buf = C.create_string_buffer(128)
+        self._check(self._L.sc_debug_last_march_variant(self._h, buf, 128))
+        return buf.value.decode()
+
+    def sc_debug_launch_count(self):
+        """Kernels of the library launched by this thread since the previous call; resets."""
+        n = C.c_longlong()
+        self._check(self._L.sc_debug_launch_count(self._h, C.byref(n)))
+        return n.value
 
     def sc_debug_fp64_peak_sustained(self, seconds=2.0):
         a = C.c_double()

@@ -9,6 +9,7 @@
 #include <cstdio>
 #include <cstring>
 #include <numeric>
+#include <set>
 #include <string>
 #include <vector>
 
@@ -117,6 +118,7 @@ struct sc_ctx {
     double t = 0, kappa = -1; int sym = 0;
     int ncomp = 1; int syms[sck::MAX_COMP] = {0, 0, 0, 0}; double tc_ratio[sck::MAX_COMP] = {1, 1, 1, 1};   // Eq. 1 :37 components
     cudaStream_t stream = nullptr;
+    bool on_device = false;                       // sc_create reached the device part (false: tables only, every compute call fails)
     int n_sm = 148;
     scgeo::Geometry geo;
     // physical trajectories (k < N/2)
@@ -149,6 +151,8 @@ struct sc_ctx {
     static constexpr int MEV = 64;                 // ring of event pairs around the march launches (sc_debug_march_time)
     cudaEvent_t mev[MEV][2] = {}; int mev_n = 0;
     long long march_units = 0;                    // (piece, energy) units of the march launches since the last sc_debug_march_units
+    std::string last_variant;                     // template arguments of the most recent march launch (sc_debug_last_march_variant)
+    std::set<const void*> smem_opted;             // march instantiations whose dynamic shared memory was opted in on THIS context's device
     // Eq. 22 denominator sum (sum_n w_n t / eps_n over the WHOLE job's energy table) and the energy-shard hook
     double denom_sum = 0.0;
     double* hook_acc = nullptr; sc_allreduce_fn hook_fn = nullptr; void* hook_user = nullptr;
@@ -160,6 +164,9 @@ namespace {
 
 sc_status fail(sc_ctx* c, sc_status s, const std::string& m) { if (c) c->err = m; return s; }
 #define CU(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return fail(ctx, e_ == cudaErrorMemoryAllocation ? SC_ERR_NOMEM : SC_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); } while (0)
+
+// every ABI call that touches the device runs on the context's device, whatever the caller's current device is
+#define ON_DEVICE(ctx) do { if (!(ctx)->on_device) return fail(ctx, SC_ERR_CUDA, "context has no CUDA device (sc_create failed)"); CU(cudaSetDevice((ctx)->opt.device)); } while (0)
 
 sck::GridDev grid_dev(const sc_ctx* c) {
     return sck::GridDev{c->grid.nx, c->grid.ny, c->grid.h, c->d_mask.p, c->d_delta.p,
@@ -185,17 +192,20 @@ sc_status ensure_nodes(sc_ctx* ctx) {
     if (ctx->nodes_fresh) return SC_OK;
     if (!ctx->have_fields) return fail(ctx, SC_ERR_STATE, "sc_set_fields has not been called");
     const int wpb = 8;
+    // n_bad[0]: interpolation points without a valid neighbour found by rotate-in (cleared here, where it is produced);
+    // n_bad[1]: by the rotate-back of the current call (cleared by that call)
+    CU(cudaMemsetAsync(ctx->d_nbad.p, 0, sizeof(int), ctx->stream));
     if (ctx->f32)
-        sck::rotate_in_kernel<float><<<(ctx->G + wpb - 1) / wpb, wpb * 32, 0, ctx->stream>>>(
+        ++sck::g_launches, sck::rotate_in_kernel<float><<<(ctx->G + wpb - 1) / wpb, wpb * 32, 0, ctx->stream>>>(
             grid_dev(ctx), traj_dev(ctx), ctx->d_vx.p, ctx->d_vy.p, ctx->d_eta.p, ctx->geo.nphi, ctx->geo.c, ctx->opt.charge_sign,
             ctx->d_ndD.p, ctx->d_nda.p, ctx->d_ndDr.p, (float4*)ctx->d_pc.p, ctx->d_pmax.p, ctx->d_nbad.p);
     else
-        sck::rotate_in_kernel<double><<<(ctx->G + wpb - 1) / wpb, wpb * 32, 0, ctx->stream>>>(
+        ++sck::g_launches, sck::rotate_in_kernel<double><<<(ctx->G + wpb - 1) / wpb, wpb * 32, 0, ctx->stream>>>(
             grid_dev(ctx), traj_dev(ctx), ctx->d_vx.p, ctx->d_vy.p, ctx->d_eta.p, ctx->geo.nphi, ctx->geo.c, ctx->opt.charge_sign,
             ctx->d_ndD.p, ctx->d_nda.p, nullptr, (double4*)ctx->d_pc.p, ctx->d_pmax.p, ctx->d_nbad.p);
     if (!ctx->fb_rows.empty()) {
         const int n = (int)ctx->fb_rows.size();
-        sck::fallback_kernel<<<(n + 127) / 128, 128, 0, ctx->stream>>>(grid_dev(ctx), n, ctx->d_fb_rows.p, ctx->d_fb_px.p,
+        ++sck::g_launches, sck::fallback_kernel<<<(n + 127) / 128, 128, 0, ctx->stream>>>(grid_dev(ctx), n, ctx->d_fb_rows.p, ctx->d_fb_px.p,
             ctx->d_fb_py.p, ctx->d_fb_dx.p, ctx->d_fb_dy.p, ctx->d_fb_eta.p, ctx->opt.charge_sign, ctx->d_fb_D.p, ctx->d_fb_a.p);
     }
     CU(cudaGetLastError());
@@ -226,14 +236,19 @@ template <int MODE, bool STATS, int STEP, typename R, int TM, bool UW = false>
 sc_status launch_march_t(sc_ctx* ctx, const sck::MarchArgsT<R>& A) {
     const int blocks = ctx->n_slots / sck::MARCH_WARPS;
     const int smem = sck::march_smem<R>();
-    static bool attr_set = false;
-    if (!attr_set) {
-        CU(cudaFuncSetAttribute(sck::march_kernel<MODE, STATS, STEP, R, TM, UW>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        attr_set = true;
+    // the opt-in to > 48 KB of dynamic shared memory is a per-device attribute of the function: remember it per context
+    const void* fn = (const void*)sck::march_kernel<MODE, STATS, STEP, R, TM, UW>;
+    if (!ctx->smem_opted.count(fn)) {
+        CU(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        ctx->smem_opted.insert(fn);
     }
+    char name[96];
+    std::snprintf(name, sizeof(name), "march_kernel<%d,%s,%d,%s,%d,%s>", MODE, STATS ? "true" : "false", STEP,
+                  sizeof(R) == 8 ? "double" : "float", TM, UW ? "true" : "false");
+    ctx->last_variant = name;
     cudaEvent_t* ev = ctx->mev[ctx->mev_n % sc_ctx::MEV];
     CU(cudaEventRecord(ev[0], ctx->stream));
-    sck::march_kernel<MODE, STATS, STEP, R, TM, UW><<<blocks, sck::MARCH_WARPS * 32, smem, ctx->stream>>>(A);
+    ++sck::g_launches, sck::march_kernel<MODE, STATS, STEP, R, TM, UW><<<blocks, sck::MARCH_WARPS * 32, smem, ctx->stream>>>(A);
     CU(cudaEventRecord(ev[1], ctx->stream));
     ++ctx->mev_n;
     CU(cudaGetLastError());
@@ -267,8 +282,8 @@ sc_status launch_march(sc_ctx* ctx, const EnergySet& E, const char* so, char* sn
 sc_status reset_stores(sc_ctx* ctx, const EnergySet& E, char* store) {
     const long long total = (long long)ctx->G * E.ne;
     const unsigned nb = (unsigned)((total + 255) / 256);
-    if (ctx->f32) sck::reset_store_kernel<float><<<nb, 256, 0, ctx->stream>>>(traj_dev(ctx), E.dev(), (const float4*)ctx->d_pc.p, (float2*)store);
-    else sck::reset_store_kernel<double><<<nb, 256, 0, ctx->stream>>>(traj_dev(ctx), E.dev(), (const double4*)ctx->d_pc.p, (double2*)store);
+    if (ctx->f32) ++sck::g_launches, sck::reset_store_kernel<float><<<nb, 256, 0, ctx->stream>>>(traj_dev(ctx), E.dev(), (const float4*)ctx->d_pc.p, (float2*)store);
+    else ++sck::g_launches, sck::reset_store_kernel<double><<<nb, 256, 0, ctx->stream>>>(traj_dev(ctx), E.dev(), (const double4*)ctx->d_pc.p, (double2*)store);
     CU(cudaGetLastError());
     return SC_OK;
 }
@@ -280,7 +295,7 @@ sck::BackArgs back_args(sc_ctx* ctx, void* delta_new, double* jx, double* jy, do
     B.line_g = ctx->d_line_g.p; B.line_n = ctx->d_line_n.p; B.T = traj_dev(ctx); B.part = ctx->d_part.p;
     B.t = ctx->t; B.sigma = ctx->opt.charge_sign;
     for (int c = 0; c < sck::MAX_COMP; ++c) B.D[c] = std::log(ctx->t / ctx->tc_ratio[c]) + ctx->denom_sum;
-    B.delta_new = (double2*)delta_new; B.jx = jx; B.jy = jy; B.feI = feI; B.n_bad = ctx->d_nbad.p;
+    B.delta_new = (double2*)delta_new; B.jx = jx; B.jy = jy; B.feI = feI; B.n_bad = ctx->d_nbad.p + 1;
     return B;
 }
 
@@ -290,8 +305,8 @@ sc_status fill_stats(sc_ctx* ctx, sc_sweep_stats* st, int ne, bool had_stats) {
     CU(cudaEventSynchronize(ctx->ev1));
     float ms = 0; CU(cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1));
     st->ms = ms;
-    int nb = 0; CU(cudaMemcpy(&nb, ctx->d_nbad.p, sizeof(int), cudaMemcpyDeviceToHost));
-    st->n_bad = nb;
+    int nb[2] = {0, 0}; CU(cudaMemcpy(nb, ctx->d_nbad.p, 2 * sizeof(int), cudaMemcpyDeviceToHost));
+    st->n_bad = nb[0] + nb[1];
     st->n_updates = 2LL * 2LL * ctx->n_pieces_logical * ne;     // gamma and gamma-tilde, both angles of every pair
     st->n_updates_executed = 2LL * ctx->n_pieces_logical * ne;
     if (had_stats) {
@@ -394,6 +409,7 @@ sc_status sc_create(const sc_grid* grid, const unsigned char* mask, const sc_sha
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(ctx, SC_ERR_CUDA, "no CUDA device: this library has no CPU path");
     CU(cudaSetDevice(opts->device));
+    ctx->on_device = true;
     cudaDeviceProp prop; CU(cudaGetDeviceProperties(&prop, opts->device));
     ctx->n_sm = prop.multiProcessorCount;
     ctx->stream = (cudaStream_t)opts->cuda_stream;
@@ -419,8 +435,8 @@ sc_status sc_create(const sc_grid* grid, const unsigned char* mask, const sc_sha
     CU(ctx->d_ndD.alloc(nodes)); CU(ctx->d_nda.alloc(nodes)); CU(ctx->d_pc.alloc((size_t)(nodes + G) * 4 * ctx->rsz())); CU(ctx->d_pmax.alloc(G));
     if (ctx->f32) CU(ctx->d_ndDr.alloc(nodes));
     CU(ctx->d_part.alloc((size_t)nodes * sck::RED_VALS));
-    CU(ctx->d_counter.alloc(1)); CU(ctx->d_nbad.alloc(1)); CU(ctx->d_nonfinite.alloc(1)); CU(ctx->d_nstored.alloc(2));
-    CU(cudaMemsetAsync(ctx->d_nbad.p, 0, sizeof(int), s)); CU(cudaMemsetAsync(ctx->d_nstored.p, 0, 2 * sizeof(unsigned long long), s));
+    CU(ctx->d_counter.alloc(1)); CU(ctx->d_nbad.alloc(2)); CU(ctx->d_nonfinite.alloc(1)); CU(ctx->d_nstored.alloc(2));
+    CU(cudaMemsetAsync(ctx->d_nbad.p, 0, 2 * sizeof(int), s)); CU(cudaMemsetAsync(ctx->d_nstored.p, 0, 2 * sizeof(unsigned long long), s));
 
     // Matsubara energies eps_n = t(n+1/2) (:98), unit weights, self-partnered (z = i eps -> -conj z = z)
     EnergySet& E = ctx->mats;
@@ -452,6 +468,7 @@ sc_status sc_destroy(sc_ctx* ctx) {
 
 sc_status sc_set_fields(sc_ctx* ctx, const void* delta, const double* Ax, const double* Ay) {
     if (!ctx || !delta) return fail(ctx, SC_ERR_ARG, "null argument");
+    ON_DEVICE(ctx);
     const size_t ng = (size_t)ctx->grid.nx * ctx->grid.ny;
     CU(cudaMemcpyAsync(ctx->d_delta.p, delta, ctx->ncomp * ng * sizeof(double2), cudaMemcpyDeviceToDevice, ctx->stream));
     ctx->have_A = Ax && Ay;
@@ -466,6 +483,7 @@ sc_status sc_set_fields(sc_ctx* ctx, const void* delta, const double* Ax, const 
 sc_status sc_set_components(sc_ctx* ctx, int n, const sc_symmetry* symmetries, const double* tc_ratio) {
     if (!ctx || !symmetries || !tc_ratio) return fail(ctx, SC_ERR_ARG, "null argument");
     if (n < 1 || n > sck::MAX_COMP) return fail(ctx, SC_ERR_ARG, "1 <= n_components <= 4");
+    ON_DEVICE(ctx);
     const int N = ctx->geo.nphi; const size_t ng = (size_t)ctx->grid.nx * ctx->grid.ny, nfb = ctx->fb_rows.size();
     std::vector<double> eta((size_t)n * N), feta((size_t)n * nfb);
     for (int c = 0; c < n; ++c) {
@@ -488,19 +506,24 @@ sc_status sc_set_components(sc_ctx* ctx, int n, const sc_symmetry* symmetries, c
 
 sc_status sc_set_energies(sc_ctx* ctx, const double* z_re, const double* z_im, const double* w, int n, double denominator_sum) {
     if (!ctx || !z_re || !z_im || !w || n < 1) return fail(ctx, SC_ERR_ARG, "bad argument");
-    EnergySet& E = ctx->mats;
-    E.zr.assign(z_re, z_re + n); E.zi.assign(z_im, z_im + n); E.w.assign(w, w + n); E.partner.assign(n, -1);
+    ON_DEVICE(ctx);
+    // validate into locals: on SC_ERR_ARG the context keeps its previous table, untouched
+    std::vector<int> partner(n, -1);
     double ds = 0.0;
     for (int m = 0; m < n; ++m) {
         if (!(z_im[m] > 0)) return fail(ctx, SC_ERR_ARG, "energies must lie in the upper half plane");
         ds += w[m] * ctx->t / z_im[m];
         // partner: -conj(z) (Eq. 13 :95); Matsubara / Ozaki energies on the imaginary axis are their own partner
         for (int q = 0; q < n; ++q)
-            if (std::fabs(z_re[q] + z_re[m]) <= 1e-12 * (1.0 + std::fabs(z_re[m])) && std::fabs(z_im[q] - z_im[m]) <= 1e-12 * z_im[m]) { E.partner[m] = q; break; }
-        if (E.partner[m] < 0) return fail(ctx, SC_ERR_ARG, "energy table is not closed under z -> -conj(z)");
+            if (std::fabs(z_re[q] + z_re[m]) <= 1e-12 * (1.0 + std::fabs(z_re[m])) && std::fabs(z_im[q] - z_im[m]) <= 1e-12 * z_im[m]) { partner[m] = q; break; }
+        if (partner[m] < 0) return fail(ctx, SC_ERR_ARG, "energy table is not closed under z -> -conj(z)");
         // the sums of angle k + N/2 are taken from the partner energies of angle k (Eq. 13): partners must weigh the same
-        if (std::fabs(w[E.partner[m]] - w[m]) > 1e-12 * std::fabs(w[m])) return fail(ctx, SC_ERR_ARG, "partner energies z and -conj(z) must have equal weights");
+        if (std::fabs(w[partner[m]] - w[m]) > 1e-12 * std::fabs(w[m])) return fail(ctx, SC_ERR_ARG, "partner energies z and -conj(z) must have equal weights");
     }
+    for (int m = 0; m < n; ++m)
+        if (partner[partner[m]] != m) return fail(ctx, SC_ERR_ARG, "duplicate energies: z -> -conj(z) is not an involution on the table");
+    EnergySet& E = ctx->mats;
+    E.zr.assign(z_re, z_re + n); E.zi.assign(z_im, z_im + n); E.w.assign(w, w + n); E.partner = partner;
     ctx->denom_sum = std::isnan(denominator_sum) ? ds : denominator_sum;
     if (sc_status st = upload_energies(ctx, E)) return st;
     const size_t ND = ctx->geo.dt.size();
@@ -517,6 +540,7 @@ sc_status sc_set_allreduce_hook(sc_ctx* ctx, double* acc, sc_allreduce_fn fn, vo
 
 sc_status sc_reset_boundary(sc_ctx* ctx) {
     if (!ctx) return SC_ERR_ARG;
+    ON_DEVICE(ctx);
     if (sc_status st = ensure_nodes(ctx)) return st;
     if (sc_status st = reset_stores(ctx, ctx->mats, ctx->d_store[ctx->cur].p)) return st;
     ctx->stores_valid = true;
@@ -526,7 +550,9 @@ sc_status sc_reset_boundary(sc_ctx* ctx) {
 sc_status sc_riccati_sweep(sc_ctx* ctx, void* delta_new, double* jx, double* jy, double* fe_I, sc_sweep_stats* stats) {
     if (!ctx) return SC_ERR_ARG;
     if (!ctx->have_fields) return fail(ctx, SC_ERR_STATE, "sc_riccati_sweep before sc_set_fields");
-    if (stats) { CU(cudaEventRecord(ctx->ev0, ctx->stream)); CU(cudaMemsetAsync(ctx->d_nbad.p, 0, sizeof(int), ctx->stream)); }
+    ON_DEVICE(ctx);
+    if (stats) CU(cudaEventRecord(ctx->ev0, ctx->stream));
+    CU(cudaMemsetAsync(ctx->d_nbad.p + 1, 0, sizeof(int), ctx->stream));
     if (sc_status st = ensure_nodes(ctx)) return st;
     if (!ctx->stores_valid) { if (sc_status st = sc_reset_boundary(ctx)) return st; }
     if (sc_status st = launch_march<0>(ctx, ctx->mats, ctx->d_store[ctx->cur].p, ctx->d_store[ctx->cur ^ 1].p, stats != nullptr)) return st;
@@ -534,14 +560,14 @@ sc_status sc_riccati_sweep(sc_ctx* ctx, void* delta_new, double* jx, double* jy,
     sck::BackArgs B = back_args(ctx, delta_new, jx, jy, fe_I);
     B.raw = ctx->hook_fn ? ctx->hook_acc : nullptr;
     dim3 grd((ctx->grid.nx + sck::BACK_TX - 1) / sck::BACK_TX, (ctx->grid.ny + sck::BACK_TY - 1) / sck::BACK_TY);
-    sck::rotate_back_kernel<<<grd, dim3(sck::BACK_TX, sck::BACK_TY), 0, ctx->stream>>>(B);
+    ++sck::g_launches, sck::rotate_back_kernel<<<grd, dim3(sck::BACK_TX, sck::BACK_TY), 0, ctx->stream>>>(B);
     CU(cudaGetLastError());
     if (ctx->hook_fn) {
         // energy-sharded sweep: the caller sums the raw accumulators of all shards on this stream, then a7 runs
         ctx->hook_fn(ctx->hook_user);
         const size_t ng = (size_t)ctx->grid.nx * ctx->grid.ny;
         sck::FinArgs FA; for (int c = 0; c < sck::MAX_COMP; ++c) FA.D[c] = B.D[c];
-        sck::finalise_kernel<<<(unsigned)((ng + 255) / 256), 256, 0, ctx->stream>>>(ng, ctx->ncomp, ctx->hook_acc, ctx->t, FA, ctx->opt.charge_sign,
+        ++sck::g_launches, sck::finalise_kernel<<<(unsigned)((ng + 255) / 256), 256, 0, ctx->stream>>>(ng, ctx->ncomp, ctx->hook_acc, ctx->t, FA, ctx->opt.charge_sign,
                                                                                   (double2*)delta_new, jx, jy, fe_I);
         CU(cudaGetLastError());
     }
@@ -551,7 +577,7 @@ sc_status sc_riccati_sweep(sc_ctx* ctx, void* delta_new, double* jx, double* jy,
         const double* fields[4] = {(const double*)delta_new, jx, jy, fe_I};
         const size_t counts[4] = {2 * ng * ctx->ncomp, ng, ng, ng};
         for (int f = 0; f < 4; ++f)
-            if (fields[f]) sck::nonfinite_kernel<<<(unsigned)((counts[f] + 255) / 256), 256, 0, ctx->stream>>>(counts[f], fields[f], ctx->d_nonfinite.p);
+            if (fields[f]) ++sck::g_launches, sck::nonfinite_kernel<<<(unsigned)((counts[f] + 255) / 256), 256, 0, ctx->stream>>>(counts[f], fields[f], ctx->d_nonfinite.p);
         CU(cudaGetLastError());
         if (sc_status st = fill_stats(ctx, stats, ctx->mats.ne, true)) return st;
         int bad = 0; CU(cudaMemcpy(&bad, ctx->d_nonfinite.p, sizeof(int), cudaMemcpyDeviceToHost));
@@ -567,7 +593,9 @@ sc_status sc_ldos(sc_ctx* ctx, const double* energies, int n_e, double broadenin
     if (!(broadening > 0)) return fail(ctx, SC_ERR_ARG, "broadening must be positive");
     if (n_boundary_iters < 1) return fail(ctx, SC_ERR_ARG, "n_boundary_iters < 1");
     if (!ctx->have_fields) return fail(ctx, SC_ERR_STATE, "sc_ldos before sc_set_fields");
-    if (stats) { CU(cudaEventRecord(ctx->ev0, ctx->stream)); CU(cudaMemsetAsync(ctx->d_nbad.p, 0, sizeof(int), ctx->stream)); }
+    ON_DEVICE(ctx);
+    if (stats) CU(cudaEventRecord(ctx->ev0, ctx->stream));
+    CU(cudaMemsetAsync(ctx->d_nbad.p + 1, 0, sizeof(int), ctx->stream));
     if (sc_status st = ensure_nodes(ctx)) return st;
     // internal energy list closed under eps -> -eps (gamma-tilde_k(eps) = conj gamma_{k+N/2}(-eps), Eq. 13 :95)
     EnergySet E;
@@ -576,8 +604,10 @@ sc_status sc_ldos(sc_ctx* ctx, const double* energies, int n_e, double broadenin
     E.partner.assign(n_e, -1);
     for (int m = 0; m < n_e; ++m) {
         if (E.partner[m] >= 0) continue;
-        int best = -1; double bd = 1e-12 * (1.0 + std::fabs(energies[m]));
-        for (int q = 0; q < (int)E.zr.size(); ++q) if (std::fabs(E.zr[q] + energies[m]) <= bd) { best = q; break; }
+        // the first still unpaired energy equal to -eps_m (eps = 0 pairs with itself; repeated energies pair off one by one)
+        int best = -1; const double bd = 1e-12 * (1.0 + std::fabs(energies[m]));
+        for (int q = 0; q < (int)E.zr.size(); ++q) if (E.partner[q] < 0 && std::fabs(E.zr[q] + energies[m]) <= bd && (q != m || energies[m] == 0.0)) { best = q; break; }
+        if (best < 0 && std::fabs(energies[m]) <= bd) best = m;
         if (best < 0) { best = (int)E.zr.size(); E.zr.push_back(-energies[m]); E.zi.push_back(broadening); E.w.push_back(0.0); E.partner.push_back(m); }
         E.partner[m] = best; E.partner[best] = m;
     }
@@ -619,7 +649,7 @@ sc_status sc_ldos(sc_ctx* ctx, const double* energies, int n_e, double broadenin
         L.ne_out = n_e; L.out_idx = d_out_idx.p; L.partner = E.d_partner.p; L.ne = E.ne;
         L.ldos_nodes = ldn; L.out = ldos; L.p0 = p0; L.p1 = p1; L.accumulate = first ? 0 : 1;
         dim3 grd((n_e + 63) / 64, ctx->grid.nx, ctx->grid.ny);
-        sck::rotate_back_ldos_kernel<<<grd, 64, 0, ctx->stream>>>(L);
+        ++sck::g_launches, sck::rotate_back_ldos_kernel<<<grd, 64, 0, ctx->stream>>>(L);
         CU(cudaGetLastError());
         CU(cudaStreamSynchronize(ctx->stream));     // d_ldn / d_items are re-used by the next batch
         first = false; p0 = p1;
@@ -631,6 +661,7 @@ sc_status sc_ldos(sc_ctx* ctx, const double* energies, int n_e, double broadenin
 
 sc_status sc_set_external_field(sc_ctx* ctx, const double* Ax, const double* Ay) {
     if (!ctx) return SC_ERR_ARG;
+    ON_DEVICE(ctx);
     const size_t ng = (size_t)ctx->grid.nx * ctx->grid.ny;
     ctx->have_Aext = Ax && Ay;
     if (ctx->have_Aext) {
@@ -643,6 +674,7 @@ sc_status sc_set_external_field(sc_ctx* ctx, const double* Ax, const double* Ay)
 
 sc_status sc_update_vector_potential(sc_ctx* ctx, const double* jx, const double* jy, double* Ax, double* Ay, double* fe_mag) {
     if (!ctx || !jx || !jy || !Ax || !Ay) return fail(ctx, SC_ERR_ARG, "null argument");
+    ON_DEVICE(ctx);
     std::string e;
     int rc = scf::vector_potential(ctx->fs, ctx->grid.nx, ctx->grid.ny, ctx->grid.h, ctx->d_mask.p, ctx->kappa, jx, jy, Ax, Ay, fe_mag, ctx->stream, e);
     if (rc) return fail(ctx, rc == 2 ? SC_ERR_NOMEM : SC_ERR_CUDA, e);
@@ -652,6 +684,7 @@ sc_status sc_update_vector_potential(sc_ctx* ctx, const double* jx, const double
 sc_status sc_iterate(sc_ctx* ctx, int accelerator, double step, int burnin, void* delta_inout, double* Aix, double* Aiy, sc_sweep_stats* stats) {
     if (!ctx || !delta_inout) return fail(ctx, SC_ERR_ARG, "null argument");
     if (accelerator < 0 || accelerator > 3) return fail(ctx, SC_ERR_ARG, "accelerator must be 0 (Picard), 1 (Barzilai-Borwein), 2 (Polyak) or 3 (CongAcc)");
+    ON_DEVICE(ctx);
     const int nx = ctx->grid.nx, ny = ctx->grid.ny; const size_t ng = (size_t)nx * ny;
     const bool withA = ctx->kappa > 0 && Aix && Aiy;
     std::string e;
@@ -692,6 +725,7 @@ sc_status sc_set_vector_potential_error(sc_ctx* ctx, double eps, int* n_kept) {
     if (n_kept) {
         *n_kept = 0;
         if (eps > 0.0) {
+            ON_DEVICE(ctx);
             std::string e;
             if (!ctx->fs.lr) ctx->fs.lr = new scf::LowRank();
             if (int rc = scf::ensure_lowrank(*ctx->fs.lr, ctx->grid.nx, ctx->grid.ny, ctx->grid.h, eps, ctx->stream, e))
@@ -741,14 +775,15 @@ sc_status sc_debug_tables(sc_ctx* ctx, int k, int* n, int* it, double* dt, int* 
 
 sc_status sc_debug_trajectory(sc_ctx* ctx, int k, int local, int n_energy, int* n_nodes, void* gamma, void* gamma_tilde) {
     if (!ctx || k < 0 || k >= ctx->geo.nphi / 2) return fail(ctx, SC_ERR_ARG, "k must be < n_angles/2");
+    ON_DEVICE(ctx);
     const int g = ctx->geo.aoff[k] + local;
     if (local < 0 || g >= ctx->geo.aoff[k + 1] || n_energy < 0 || n_energy >= ctx->mats.ne) return fail(ctx, SC_ERR_ARG, "bad index");
     if (!ctx->stores_valid) return fail(ctx, SC_ERR_STATE, "no sweep has been run");
     const int nn = ctx->h_nn[g];
     DevBuf<double2> dG, dGT; CU(dG.alloc(nn)); CU(dGT.alloc(nn));
     // the last sweep read store[cur^1] (now the "new" side) and wrote store[cur]
-    if (ctx->f32) sck::debug_traj_kernel<float><<<1, 32, 0, ctx->stream>>>(march_args<float>(ctx, ctx->mats, ctx->d_store[ctx->cur ^ 1].p, nullptr), ctx->opt.stepper, g, n_energy, dG.p, dGT.p);
-    else sck::debug_traj_kernel<double><<<1, 32, 0, ctx->stream>>>(march_args<double>(ctx, ctx->mats, ctx->d_store[ctx->cur ^ 1].p, nullptr), ctx->opt.stepper, g, n_energy, dG.p, dGT.p);
+    if (ctx->f32) ++sck::g_launches, sck::debug_traj_kernel<float><<<1, 32, 0, ctx->stream>>>(march_args<float>(ctx, ctx->mats, ctx->d_store[ctx->cur ^ 1].p, nullptr), ctx->opt.stepper, g, n_energy, dG.p, dGT.p);
+    else ++sck::g_launches, sck::debug_traj_kernel<double><<<1, 32, 0, ctx->stream>>>(march_args<double>(ctx, ctx->mats, ctx->d_store[ctx->cur ^ 1].p, nullptr), ctx->opt.stepper, g, n_energy, dG.p, dGT.p);
     CU(cudaGetLastError());
     CU(cudaMemcpyAsync(gamma, dG.p, nn * sizeof(double2), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaMemcpyAsync(gamma_tilde, dGT.p, nn * sizeof(double2), cudaMemcpyDeviceToHost, ctx->stream));
@@ -759,6 +794,7 @@ sc_status sc_debug_trajectory(sc_ctx* ctx, int k, int local, int n_energy, int* 
 
 sc_status sc_debug_partial(sc_ctx* ctx, int k, void* SF, double* SG, double* SI) {
     if (!ctx || k < 0 || k >= ctx->geo.nphi || !SF || !SG || !SI) return fail(ctx, SC_ERR_ARG, "bad argument");
+    ON_DEVICE(ctx);
     const int H = ctx->geo.nphi / 2, NR = ctx->geo.nrot, p = k % H;
     const int g0 = ctx->geo.aoff[p], g1 = ctx->geo.aoff[p + 1];
     if (g1 == g0) return SC_OK;
@@ -778,10 +814,42 @@ sc_status sc_debug_partial(sc_ctx* ctx, int k, void* SF, double* SG, double* SI)
     return SC_OK;
 }
 
+sc_status sc_debug_stores(sc_ctx* ctx, int k, void* gamma_end, void* gamma_tilde_end) {
+    if (!ctx || k < 0 || k >= ctx->geo.nphi || !gamma_end || !gamma_tilde_end) return fail(ctx, SC_ERR_ARG, "bad argument");
+    ON_DEVICE(ctx);
+    if (!ctx->stores_valid) return fail(ctx, SC_ERR_STATE, "no sweep has been run");
+    const int H = ctx->geo.nphi / 2, ne = ctx->mats.ne, km = (k + H) % ctx->geo.nphi;
+    const int a0 = ctx->geo.aoff[k], a1 = ctx->geo.aoff[k + 1], m0 = ctx->geo.aoff[km], m1 = ctx->geo.aoff[km + 1];
+    if (a1 - a0 != m1 - m0) return fail(ctx, SC_ERR_GEOMETRY, "internal: mirror angle has a different trajectory count");
+    const size_t rowb = (size_t)ne * 2 * ctx->rsz();
+    std::vector<char> own((size_t)(a1 - a0) * rowb), mir((size_t)(m1 - m0) * rowb);
+    CU(cudaStreamSynchronize(ctx->stream));
+    CU(cudaMemcpy(own.data(), ctx->d_store[ctx->cur].p + (size_t)a0 * rowb, own.size(), cudaMemcpyDeviceToHost));
+    CU(cudaMemcpy(mir.data(), ctx->d_store[ctx->cur].p + (size_t)m0 * rowb, mir.size(), cudaMemcpyDeviceToHost));
+    auto at = [&](const std::vector<char>& b, size_t row, int n, double& re, double& im) {
+        if (ctx->f32) { const float* v = (const float*)(b.data() + row * rowb) + 2 * n; re = v[0]; im = v[1]; }
+        else { const double* v = (const double*)(b.data() + row * rowb) + 2 * n; re = v[0]; im = v[1]; }
+    };
+    // mirror of directed trajectory d: h_dB for the first half of the angles, its inverse for the second half
+    std::vector<int> mirror(a1 - a0);
+    if (k < H) for (int d = a0; d < a1; ++d) mirror[d - a0] = ctx->h_dB[d];
+    else for (int g = m0; g < m1; ++g) mirror[ctx->h_dB[g] - a0] = g;
+    double* G = (double*)gamma_end; double* GT = (double*)gamma_tilde_end;
+    for (int d = a0; d < a1; ++d)
+        for (int n = 0; n < ne; ++n) {
+            const size_t o = 2 * ((size_t)(d - a0) * ne + n);
+            at(own, d - a0, n, G[o], G[o + 1]);
+            double re, im; at(mir, mirror[d - a0] - m0, ctx->mats.partner[n], re, im);
+            GT[o] = re; GT[o + 1] = -im;                        // Eq. 13 (:95): gamma-tilde_k(eps) = conj gamma_{k+N/2}(-conj eps)
+        }
+    return SC_OK;
+}
+
 sc_status sc_debug_math(sc_ctx* ctx, int n, double* max_rel_err) {
     if (!ctx || !max_rel_err) return SC_ERR_ARG;
+    ON_DEVICE(ctx);
     DevBuf<double> d; CU(d.alloc(6)); CU(cudaMemsetAsync(d.p, 0, 6 * sizeof(double), ctx->stream));
-    sck::math_test_kernel<<<64, 128, 0, ctx->stream>>>(n, d.p);
+    ++sck::g_launches, sck::math_test_kernel<<<64, 128, 0, ctx->stream>>>(n, d.p);
     CU(cudaGetLastError());
     CU(cudaMemcpyAsync(max_rel_err, d.p, 6 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
@@ -790,6 +858,7 @@ sc_status sc_debug_math(sc_ctx* ctx, int n, double* max_rel_err) {
 
 sc_status sc_debug_last_march_ms(sc_ctx* ctx, float* ms) {
     if (!ctx || !ms) return SC_ERR_ARG;
+    ON_DEVICE(ctx);
     if (ctx->mev_n == 0) return fail(ctx, SC_ERR_STATE, "no march kernel has been launched");
     cudaEvent_t* ev = ctx->mev[(ctx->mev_n - 1) % sc_ctx::MEV];
     CU(cudaEventSynchronize(ev[1]));
@@ -799,6 +868,7 @@ sc_status sc_debug_last_march_ms(sc_ctx* ctx, float* ms) {
 
 sc_status sc_debug_march_time(sc_ctx* ctx, float* total_ms, int* n_launches) {
     if (!ctx) return SC_ERR_ARG;
+    ON_DEVICE(ctx);
     const int n = std::min(ctx->mev_n, (int)sc_ctx::MEV);
     float tot = 0.f;
     for (int i = 0; i < n; ++i) {
@@ -815,6 +885,7 @@ sc_status sc_debug_march_time(sc_ctx* ctx, float* total_ms, int* n_launches) {
 
 sc_status sc_debug_march_units(sc_ctx* ctx, long long* units_total, long long* units_stored_T, long long* units_pole_table) {
     if (!ctx) return SC_ERR_ARG;
+    ON_DEVICE(ctx);
     CU(cudaStreamSynchronize(ctx->stream));
     unsigned long long ns[2] = {0, 0}; CU(cudaMemcpy(ns, ctx->d_nstored.p, sizeof(ns), cudaMemcpyDeviceToHost));
     CU(cudaMemset(ctx->d_nstored.p, 0, sizeof(ns)));
@@ -825,15 +896,30 @@ sc_status sc_debug_march_units(sc_ctx* ctx, long long* units_total, long long* u
     return SC_OK;
 }
 
+sc_status sc_debug_last_march_variant(sc_ctx* ctx, char* name, int len) {
+    if (!ctx || !name || len < 1) return SC_ERR_ARG;
+    if (ctx->last_variant.empty()) return fail(ctx, SC_ERR_STATE, "no march kernel has been launched");
+    std::snprintf(name, (size_t)len, "%s", ctx->last_variant.c_str());
+    return SC_OK;
+}
+
+sc_status sc_debug_launch_count(sc_ctx* ctx, long long* n_kernels) {
+    if (!ctx) return SC_ERR_ARG;
+    if (n_kernels) *n_kernels = sck::g_launches;
+    sck::g_launches = 0;
+    return SC_OK;
+}
+
 sc_status sc_debug_fp64_peak(sc_ctx* ctx, double* dfma_per_s, double* sm_clock_mhz) {
     if (!ctx || !dfma_per_s) return SC_ERR_ARG;
+    ON_DEVICE(ctx);
     DevBuf<double> d; CU(d.alloc(1));
     const int iters = 20000, blocks = ctx->n_sm * 4, threads = 256;
-    sck::fp64_peak_kernel<<<blocks, threads, 0, ctx->stream>>>(iters / 10, d.p);    // warm-up
+    ++sck::g_launches, sck::fp64_peak_kernel<<<blocks, threads, 0, ctx->stream>>>(iters / 10, d.p);    // warm-up
     double best = 0;
     for (int rep = 0; rep < 3; ++rep) {
         CU(cudaEventRecord(ctx->ev0, ctx->stream));
-        sck::fp64_peak_kernel<<<blocks, threads, 0, ctx->stream>>>(iters, d.p);
+        ++sck::g_launches, sck::fp64_peak_kernel<<<blocks, threads, 0, ctx->stream>>>(iters, d.p);
         CU(cudaEventRecord(ctx->ev1, ctx->stream));
         CU(cudaEventSynchronize(ctx->ev1));
         float ms = 0; CU(cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1));
@@ -846,19 +932,20 @@ sc_status sc_debug_fp64_peak(sc_ctx* ctx, double* dfma_per_s, double* sm_clock_m
 
 sc_status sc_debug_fp64_peak_sustained(sc_ctx* ctx, double seconds, double* dfma_per_s) {
     if (!ctx || !dfma_per_s || !(seconds > 0) || seconds > 30) return fail(ctx, SC_ERR_ARG, "bad argument");
+    ON_DEVICE(ctx);
     DevBuf<double> d; CU(d.alloc(1));
     const int iters = 20000, blocks = ctx->n_sm * 4, threads = 256;
     // back-to-back launches for `seconds`: the rate the part holds once it sits at its power limit
-    sck::fp64_peak_kernel<<<blocks, threads, 0, ctx->stream>>>(iters, d.p);
+    ++sck::g_launches, sck::fp64_peak_kernel<<<blocks, threads, 0, ctx->stream>>>(iters, d.p);
     CU(cudaEventRecord(ctx->ev0, ctx->stream));
-    sck::fp64_peak_kernel<<<blocks, threads, 0, ctx->stream>>>(iters, d.p);
+    ++sck::g_launches, sck::fp64_peak_kernel<<<blocks, threads, 0, ctx->stream>>>(iters, d.p);
     CU(cudaEventRecord(ctx->ev1, ctx->stream));
     CU(cudaEventSynchronize(ctx->ev1));
     float one = 0; CU(cudaEventElapsedTime(&one, ctx->ev0, ctx->ev1));
     const int n = std::max(4, (int)(seconds * 1e3 / std::max(one, 1e-3f)));
-    for (int i = 0; i < n / 2; ++i) sck::fp64_peak_kernel<<<blocks, threads, 0, ctx->stream>>>(iters, d.p);   // reach the steady clock
+    for (int i = 0; i < n / 2; ++i) ++sck::g_launches, sck::fp64_peak_kernel<<<blocks, threads, 0, ctx->stream>>>(iters, d.p);   // reach the steady clock
     CU(cudaEventRecord(ctx->ev0, ctx->stream));
-    for (int i = 0; i < n - n / 2; ++i) sck::fp64_peak_kernel<<<blocks, threads, 0, ctx->stream>>>(iters, d.p);
+    for (int i = 0; i < n - n / 2; ++i) ++sck::g_launches, sck::fp64_peak_kernel<<<blocks, threads, 0, ctx->stream>>>(iters, d.p);
     CU(cudaEventRecord(ctx->ev1, ctx->stream));
     CU(cudaEventSynchronize(ctx->ev1));
     float ms = 0; CU(cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1));

@@ -181,31 +181,31 @@ inline int vector_potential(FieldState& F, int nx, int ny, double h, const unsig
     if (int rc = ensure_vp(F, nx, ny, h, s, err)) return rc;
     const int px = 2 * nx, py = 2 * ny; const size_t nspec = (size_t)py * (px / 2 + 1);
     double* res = F.red + RED_RES;
-    reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, MeanOp{mask, jx, jy}, F.red, 3);
-    reduce_stage2<<<1, 32, 0, s>>>(F.red, 3, res);
-    mean_finish_kernel<<<1, 1, 0, s>>>(res);
+    ++sck::g_launches, reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, MeanOp{mask, jx, jy}, F.red, 3);
+    ++sck::g_launches, reduce_stage2<<<1, 32, 0, s>>>(F.red, 3, res);
+    ++sck::g_launches, mean_finish_kernel<<<1, 1, 0, s>>>(res);
     if (F.vp_eps > 0.0) {      // the paper's truncated eigen-decomposition (D7-D9) instead of the exact correlation
         if (!F.lr) F.lr = new LowRank();
         if (int rc = ensure_lowrank(*F.lr, nx, ny, h, F.vp_eps, s, err)) return rc;
         for (int comp = 0; comp < 2; ++comp) {
-            masked_current_kernel<<<(unsigned)((ng + 255) / 256), 256, 0, s>>>(ng, mask, comp ? jy : jx, res, comp, F.lr->J);
+            ++sck::g_launches, masked_current_kernel<<<(unsigned)((ng + 255) / 256), 256, 0, s>>>(ng, mask, comp ? jy : jx, res, comp, F.lr->J);
             if (int rc = lowrank_apply(*F.lr, -1.0 / (kappa * kappa), comp ? Ay : Ax, s, err)) return rc;
         }
     }
     const double scale = -1.0 / (kappa * kappa) / ((double)px * py);
     for (int comp = 0; comp < 2 && !(F.vp_eps > 0.0); ++comp) {
         dim3 g1((px + 127) / 128, py);
-        pad_current_kernel<<<g1, 128, 0, s>>>(nx, ny, mask, comp ? jy : jx, res, comp, F.pad);
+        ++sck::g_launches, pad_current_kernel<<<g1, 128, 0, s>>>(nx, ny, mask, comp ? jy : jx, res, comp, F.pad);
         SCF_FFT(cufftExecD2Z(F.plan_f, F.pad, F.spec));
-        spec_mul_kernel<<<(unsigned)((nspec + 255) / 256), 256, 0, s>>>(nspec, F.spec, F.Ghat);
+        ++sck::g_launches, spec_mul_kernel<<<(unsigned)((nspec + 255) / 256), 256, 0, s>>>(nspec, F.spec, F.Ghat);
         SCF_FFT(cufftExecZ2D(F.plan_b, F.spec, F.pad));
         dim3 g2((nx + 127) / 128, ny);
-        crop_kernel<<<g2, 128, 0, s>>>(nx, ny, F.pad, scale, comp ? Ay : Ax);
+        ++sck::g_launches, crop_kernel<<<g2, 128, 0, s>>>(nx, ny, F.pad, scale, comp ? Ay : Ax);
     }
     SCF_CU(cudaGetLastError());
     if (fe_mag) {
-        reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, FemagOp{mask, jx, jy, Ax, Ay}, F.red, 1);
-        reduce_stage2<<<1, 32, 0, s>>>(F.red, 1, res + 4);
+        ++sck::g_launches, reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, FemagOp{mask, jx, jy, Ax, Ay}, F.red, 1);
+        ++sck::g_launches, reduce_stage2<<<1, 32, 0, s>>>(F.red, 1, res + 4);
         double v = 0; SCF_CU(cudaMemcpyAsync(&v, res + 4, sizeof(double), cudaMemcpyDeviceToHost, s));
         SCF_CU(cudaStreamSynchronize(s));
         *fe_mag = 0.5 * h * h * v;
@@ -236,7 +236,7 @@ __global__ void add_fields_kernel(size_t n, double* ox, double* oy, const double
     oy[i] = (ay ? ay[i] : 0.0) + (by ? by[i] : 0.0);
 }
 inline void add_fields(double* ox, double* oy, const double* ax, const double* ay, const double* bx, const double* by, size_t n, cudaStream_t s) {
-    add_fields_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(n, ox, oy, ax, ay, bx, by);
+    ++sck::g_launches, add_fields_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(n, ox, oy, ax, ay, bx, by);
 }
 
 // d = g(x) - x for the concatenated iterate x = (Re D_0, Im D_0, ..., Re D_{nc-1}, Im D_{nc-1}, kappa^2 A_x, kappa^2 A_y) (E3 :1053)
@@ -362,24 +362,24 @@ inline int mix(FieldState& F, int accelerator, double step, double kappa, bool w
         if (!F.aux) SCF_CU(cudaMalloc((void**)&F.aux, nxl * sizeof(double)));
         if (F.first) SCF_CU(cudaMemsetAsync(F.aux, 0, nxl * sizeof(double), s));
     }
-    diff_kernel<<<nb, 256, 0, s>>>(ng, nc, delta, F.dnew, aix, aiy, F.gAx, F.gAy, k2, withA ? 1 : 0, F.d_cur);
+    ++sck::g_launches, diff_kernel<<<nb, 256, 0, s>>>(ng, nc, delta, F.dnew, aix, aiy, F.gAx, F.gAy, k2, withA ? 1 : 0, F.d_cur);
     if (!F.first && accelerator == 1) {
-        reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(nxl, DotOp{F.d_cur, F.d_prev}, F.red, 3);
-        reduce_stage2<<<1, 32, 0, s>>>(F.red, 3, res);
+        ++sck::g_launches, reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(nxl, DotOp{F.d_cur, F.d_prev}, F.red, 3);
+        ++sck::g_launches, reduce_stage2<<<1, 32, 0, s>>>(F.red, 3, res);
     }
-    alpha_kernel<<<1, 1, 0, s>>>(F.state, res, accelerator, step, F.first ? 1 : 0, F.par);
+    ++sck::g_launches, alpha_kernel<<<1, 1, 0, s>>>(F.state, res, accelerator, step, F.first ? 1 : 0, F.par);
     if (accelerator == 3) {
-        reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, CongDotOp{ng, F.aux, F.d_cur}, F.red, 3 * nslice);
-        reduce_stage2<<<1, 32, 0, s>>>(F.red, 3 * nslice, res + 16);
-        congacc_kernel<<<1, 32, 0, s>>>(F.state, res + 16, nslice, F.par);
+        ++sck::g_launches, reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, CongDotOp{ng, F.aux, F.d_cur}, F.red, 3 * nslice);
+        ++sck::g_launches, reduce_stage2<<<1, 32, 0, s>>>(F.red, 3 * nslice, res + 16);
+        ++sck::g_launches, congacc_kernel<<<1, 32, 0, s>>>(F.state, res + 16, nslice, F.par);
     }
-    step_kernel<<<nbx, 256, 0, s>>>(ng, nslice, accelerator, F.d_cur, F.aux, F.state, F.par.drag, F.upd);
-    reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, NormOp{ng, nc, delta, aix, aiy, F.upd, k2, withA ? 1 : 0}, F.red, 4);
-    reduce_stage2<<<1, 32, 0, s>>>(F.red, 4, res + 4);
-    reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, ObsNormOp{F.jx, F.jy, F.feI, F.prev_jx, F.prev_jy, F.prev_fe}, F.red, 4);
-    reduce_stage2<<<1, 32, 0, s>>>(F.red, 4, res + 8);
-    residual_kernel<<<1, 1, 0, s>>>(F.state, res + 4, res + 8);
-    update_kernel<<<nb, 256, 0, s>>>(ng, nc, delta, aix, aiy, F.upd, mask, k2 > 0 ? k2 : 1.0, withA ? 1 : 0);
+    ++sck::g_launches, step_kernel<<<nbx, 256, 0, s>>>(ng, nslice, accelerator, F.d_cur, F.aux, F.state, F.par.drag, F.upd);
+    ++sck::g_launches, reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, NormOp{ng, nc, delta, aix, aiy, F.upd, k2, withA ? 1 : 0}, F.red, 4);
+    ++sck::g_launches, reduce_stage2<<<1, 32, 0, s>>>(F.red, 4, res + 4);
+    ++sck::g_launches, reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, ObsNormOp{F.jx, F.jy, F.feI, F.prev_jx, F.prev_jy, F.prev_fe}, F.red, 4);
+    ++sck::g_launches, reduce_stage2<<<1, 32, 0, s>>>(F.red, 4, res + 8);
+    ++sck::g_launches, residual_kernel<<<1, 1, 0, s>>>(F.state, res + 4, res + 8);
+    ++sck::g_launches, update_kernel<<<nb, 256, 0, s>>>(ng, nc, delta, aix, aiy, F.upd, mask, k2 > 0 ? k2 : 1.0, withA ? 1 : 0);
     SCF_CU(cudaMemcpyAsync(F.prev_jx, F.jx, ng * sizeof(double), cudaMemcpyDeviceToDevice, s));
     SCF_CU(cudaMemcpyAsync(F.prev_jy, F.jy, ng * sizeof(double), cudaMemcpyDeviceToDevice, s));
     SCF_CU(cudaMemcpyAsync(F.prev_fe, F.feI, ng * sizeof(double), cudaMemcpyDeviceToDevice, s));

@@ -30,6 +30,10 @@ __device__ __forceinline__ float2 mk2(float a, float b) { return make_float2(a, 
 __device__ __forceinline__ double4 mk4(double a, double b, double c, double d) { return make_double4(a, b, c, d); }
 __device__ __forceinline__ float4 mk4(float a, float b, float c, float d) { return make_float4(a, b, c, d); }
 
+// kernels of this library launched by the calling host thread (one context per host thread) since the last
+// sc_debug_launch_count; library routines (cuFFT, cuBLAS, cuSOLVER) and memsets / copies are not counted
+inline thread_local long long g_launches = 0;
+
 constexpr int MAX_COMP = 4;        // order-parameter components Delta_G (Eq. 1 :37)
 struct GridDev {
     int nx, ny; double h;

@@ -106,8 +106,8 @@ inline int lowrank_apply(LowRank& L, double scale, double* out, cudaStream_t s, 
     const double one = 1.0, zero = 0.0;
     SCL_CU(cudaMemsetAsync(out, 0, (size_t)nx * ny * sizeof(double), s));
     for (int k = 0; k < L.nstar; ++k) {
-        toeplitz_kernel<<<dim3((nx + 127) / 128, nx), 128, 0, s>>>(nx, L.V + (size_t)k * N, L.Tx);
-        toeplitz_kernel<<<dim3((ny + 127) / 128, ny), 128, 0, s>>>(ny, L.V + (size_t)k * N, L.Ty);
+        ++sck::g_launches, toeplitz_kernel<<<dim3((nx + 127) / 128, nx), 128, 0, s>>>(nx, L.V + (size_t)k * N, L.Tx);
+        ++sck::g_launches, toeplitz_kernel<<<dim3((ny + 127) / 128, ny), 128, 0, s>>>(ny, L.V + (size_t)k * N, L.Ty);
         const double a = scale * L.lam[k];
         SCL_LIB(cublasDgemm(L.blas, CUBLAS_OP_N, CUBLAS_OP_N, nx, ny, nx, &one, L.Tx, nx, L.J, nx, &zero, L.W, nx));
         SCL_LIB(cublasDgemm(L.blas, CUBLAS_OP_N, CUBLAS_OP_N, nx, ny, ny, &a, L.W, nx, L.Ty, ny, &one, out, nx));

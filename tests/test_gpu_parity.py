@@ -53,7 +53,21 @@ class GpuRun:
                     fe_I=self.fe.cpu().numpy(), stats=st)
 
 
-def compare_sweeps(sc, wl, n_sweeps=2, tol=TOL, **kw):
+def expected_variant(wl, stats, precision=64, stepper=0, mode=0):
+    """The march instantiation sc_api.cu's dispatch must pick for a plain Matsubara sweep of `wl`:
+    the unit-weight kernel (weights compiled out) iff no stats are requested, the closed-form stepper runs and the
+    energy count is a multiple of 32; it is the kernel bench.py times."""
+    r = "double" if precision == 64 else "float"
+    uw = (not stats) and stepper == 0 and wl.n_energies % 32 == 0
+    return "march_kernel<%d,%s,%d,%s,1,%s>" % (mode, "true" if stats else "false", stepper, r, "true" if uw else "false")
+
+
+BENCH_KERNEL = {64: "march_kernel<0,false,0,double,1,true>", 32: "march_kernel<0,false,0,float,1,true>"}   # what bench.py times
+
+
+def compare_sweeps(sc, wl, n_sweeps=2, tol=TOL, stats=True, **kw):
+    """Element-wise parity of Delta_new, j, I over the whole grid for n_sweeps Jacobi sweeps.  stats=False runs the
+    stats-free kernel instantiations (the ones sc_iterate and bench.py launch) and asserts which one ran."""
     o = oracle.Oracle.from_workload(wl, **{k: v for k, v in kw.items() if k in ("bc_mode", "stepper")})
     g = GpuRun(sc, wl, **kw)
     Ax = wl.Aext_x if np.any(wl.Aext_x) else None
@@ -64,14 +78,17 @@ def compare_sweeps(sc, wl, n_sweeps=2, tol=TOL, **kw):
     for it in range(n_sweeps):
         ro = o.sweep(wl.delta0, Ax, Ay, wl.n_energies, stores)
         stores = ro["stores"]
-        rg = g.sweep()
+        rg = g.sweep(stats=stats)
+        assert g.ctx.sc_debug_last_march_variant() == expected_variant(wl, stats, kw.get("precision", 64), kw.get("stepper", 0))
         for key in ("delta_new", "jx", "jy", "fe_I"):
             e = relerr(rg[key], ro[key])
             assert e < tol, (it, key, e)
             worst = max(worst, e)
-        assert rg["stats"].n_bad == 0 and ro["stats"]["n_bad"] == 0
-        assert rg["stats"].n_updates == ro["stats"]["n_updates"]
-        assert abs(rg["stats"].min_one_minus_abs_gamma - ro["stats"]["min_one_minus_abs_gamma"]) < max(1e-9, tol)
+        assert ro["stats"]["n_bad"] == 0
+        if stats:
+            assert rg["stats"].n_bad == 0
+            assert rg["stats"].n_updates == ro["stats"]["n_updates"]
+            assert abs(rg["stats"].min_one_minus_abs_gamma - ro["stats"]["min_one_minus_abs_gamma"]) < max(1e-9, tol)
         assert np.all(rg["delta_new"][wl.mask == 0] == 0)
     return o, g, stores, worst
 
@@ -113,9 +130,40 @@ def test_cfg0_full_sweeps_and_taps(sc):
     (2, dict(pts_per_xi=5, n_angles=32, n_energies=33, size_scale=0.5), 2),   # d-wave, [110] walls
     (4, dict(pts_per_xi=5, n_angles=16, n_energies=64, size_scale=0.2), 1),   # many vortices, 2 full rounds
 ])
-def test_reduced_configs(sc, cfg, kw, ns):
+@pytest.mark.parametrize("stats", [True, False])
+def test_reduced_configs(sc, cfg, kw, ns, stats):
     wl = wlmod.make_workload(cfg, **kw)
-    compare_sweeps(sc, wl, n_sweeps=ns)
+    o, g, _, _ = compare_sweeps(sc, wl, n_sweeps=ns, stats=stats)
+    if cfg == 4 and not stats:
+        assert g.ctx.sc_debug_last_march_variant() == BENCH_KERNEL[64]
+
+
+@pytest.mark.parametrize("precision,tol", [(64, TOL), (32, TOL32)])
+def test_bench_kernel_instantiation_parity_and_bitwise_claim(sc, precision, tol):
+    """The instantiation bench.py times — march_kernel<0,false,0,R,1,true>: no stats, closed-form stepper, plain Matsubara
+    table with every weight 1 compiled out, whole warps of energies (sc_api.cu launch_march_r) — element-wise against
+    the oracle over three Jacobi sweeps on a vortex disc in a field (2 full 32-energy rounds, all table tiers reached
+    by the rim's |A|), and bit for bit against the weighted / stats instantiation on the same inputs."""
+    wl = wlmod.make_workload(4, pts_per_xi=5, n_angles=16, n_energies=64, size_scale=0.2)
+    o, g, _, _ = compare_sweeps(sc, wl, n_sweeps=3, tol=tol, stats=False, precision=precision)
+    assert g.ctx.sc_debug_last_march_variant() == BENCH_KERNEL[precision]
+    a = GpuRun(sc, wl, precision=precision); b = GpuRun(sc, wl, precision=precision)
+    for r in (a, b):
+        r.set_fields(wl.delta0, wl.Aext_x, wl.Aext_y)
+    for it in range(2):
+        ra = a.sweep(stats=False); rb = b.sweep(stats=True)
+        assert a.ctx.sc_debug_last_march_variant() == BENCH_KERNEL[precision]
+        assert b.ctx.sc_debug_last_march_variant() == expected_variant(wl, True, precision)
+        for key in ("delta_new", "jx", "jy", "fe_I"):
+            assert np.array_equal(ra[key], rb[key]), (it, key)
+    # per-angle energy sums of the unit-weight launch, both halves of the angle set
+    st = None
+    for _ in range(1):
+        st = o.sweep(wl.delta0, wl.Aext_x, wl.Aext_y, wl.n_energies, st)["stores"]
+    for k in (2, 11):
+        ro = o.sweep(wl.delta0, wl.Aext_x, wl.Aext_y, wl.n_energies, st, dbg_angle=k)
+        SF, SG, SI = a.ctx.sc_debug_partial(k)
+        assert relerr(SF, ro["dbg"]["SF"]) < tol and relerr(SG, ro["dbg"]["SG"]) < tol and relerr(SI, ro["dbg"]["SI"]) < tol
 
 
 def test_bulk_boundary_mode(sc):
@@ -149,10 +197,11 @@ def test_midpoint_stepper_parity(sc, cfg, kw):
     (4, dict(pts_per_xi=5, n_angles=16, n_energies=64, size_scale=0.2), 2),
 ])
 @pytest.mark.parametrize("stepper", [0, 1])
-def test_fp32_mode_parity(sc, cfg, kw, ns, stepper):
+@pytest.mark.parametrize("stats", [True, False])
+def test_fp32_mode_parity(sc, cfg, kw, ns, stepper, stats):
     """opts.precision = 32: the march in float (pieces, scratch, boundary stores), fp64 ABI and fp64 oracle; 2e-4."""
     wl = wlmod.make_workload(cfg, **kw)
-    o, g, stores, worst = compare_sweeps(sc, wl, n_sweeps=ns, tol=TOL32, precision=32, stepper=stepper)
+    o, g, stores, worst = compare_sweeps(sc, wl, n_sweeps=ns, tol=TOL32, precision=32, stepper=stepper, stats=stats)
     assert worst > 1e-12          # it really is a float path
     # per-trajectory tap in the same precision
     z, _ = o.matsubara(wl.n_energies)
@@ -170,8 +219,9 @@ def test_fp32_mode_parity(sc, cfg, kw, ns, stepper):
             assert np.max(np.abs(Gg - Go)) < TOL32 and np.max(np.abs(GTg - GTo)) < TOL32
 
 
+@pytest.mark.parametrize("stats", [True, False])
 @pytest.mark.parametrize("amp", [0.02, 0.3, 2.0, 12.0])
-def test_step_coefficient_table_and_fallback(sc, amp):
+def test_step_coefficient_table_and_fallback(sc, amp, stats):
     """The march evaluates T = tanh(Omega l)/Omega from per-energy tables where |De|^2 - a^2 - 2 i eps a is small
     against the distance to the table's nearest (or second) pole, and from exp/sqrt elsewhere (trajectory ends, strong
     A, high energies on coarse grids); rounds inside a radius re-evaluate T in pass 2, the others spill it (DESIGN.md
@@ -191,7 +241,8 @@ def test_step_coefficient_table_and_fallback(sc, amp):
     for it in range(2):
         ro = o.sweep(wl.delta0, Ax, Ay, wl.n_energies, stores)
         stores = ro["stores"]
-        rg = g.sweep()
+        rg = g.sweep(stats=stats)
+        assert g.ctx.sc_debug_last_march_variant() == expected_variant(wl, stats)       # ne = 96: stats=False is the unit-weight kernel
         for key in ("delta_new", "jx", "jy", "fe_I"):
             assert relerr(rg[key], ro[key]) < TOL, (amp, it, key, relerr(rg[key], ro[key]))
     total, stored, pole = g.ctx.sc_debug_march_units()
@@ -333,6 +384,8 @@ def test_vector_potential_parity(sc):
 @pytest.mark.parametrize("cfg,kw,acc,niter", [
     (0, {}, 0, 20),                                                        # configs[0]: 20 Picard iterations
     (1, dict(pts_per_xi=5, n_angles=16, n_energies=24), 1, 6),            # kappa = 2, Barzilai-Borwein, induced A
+    (1, dict(pts_per_xi=5, n_angles=16, n_energies=32), 1, 6),            # whole warps of energies: sc_iterate launches the unit-weight kernel bench.py times
+    (4, dict(pts_per_xi=4, n_angles=16, n_energies=64, size_scale=0.15), 1, 4),   # the bench's workload shape (vortices, flux), reduced
 ])
 def test_self_consistent_iterations_match(sc, cfg, kw, acc, niter):
     wl = wlmod.make_workload(cfg, **kw)
@@ -348,6 +401,7 @@ def test_self_consistent_iterations_match(sc, cfg, kw, acc, niter):
         d_o, ax_o, ay_o = r["delta"], r["Aind_x"], r["Aind_y"]
         st = ctx.sc_iterate(acc, 1.0, False, d_g, ax_g, ay_g, want_stats=True)
         torch.cuda.synchronize()
+        assert ctx.sc_debug_last_march_variant() == expected_variant(wl, False)       # sc_iterate never asks the march for stats
         # the fixed-point map amplifies rounding differences by at most alpha per iteration
         tol = TOL * max(1.0, 3.0 ** min(it, 6)) if acc == 1 else TOL
         assert relerr(d_g.cpu().numpy(), d_o) < tol, it
