@@ -1,0 +1,254 @@
+"""Pins of the oracle's interpolation rules (VERDICT r1 "weak #2"): the specular-gather weights (PAPER.md:197
+"interpolate from neighboring incoming trajectories, in both angle and boundary coordinate"; R6/R7/R9),
+the rotate-in interpolation (:189) and the rotate-back weights (:189).
+
+None of them re-types an oracle expression.  The expected values are
+  * a prescribed function of (boundary point, direction) that a correct linear x linear interpolation reproduces
+    exactly on a flat wall (and to O(h^2/R^2) on a disc), evaluated at a reflected direction that the test derives
+    from the analytic wall normal of the shape — not from the oracle's tables;
+  * scipy's RegularGridInterpolator on random fields (a library bilinear routine);
+  * a slab clip of every lattice line in the square's own frame (a different algorithm from the oracle's
+    half-plane loop) for the end points.
+A swapped pair of weights (nu <-> 1 - nu, omega <-> 1 - omega, fx <-> 1 - fx), a transposed index, a wrong mirror
+formula or a wrong / transposed normal turns one of them red (sabotage list: DESIGN.md §7).
+"""
+import math
+
+import numpy as np
+import pytest
+from scipy.interpolate import RegularGridInterpolator
+
+import oracle
+import workloads as wlmod
+from workloads import make_mask, square
+
+
+def _lattice(o, h):
+    c = 0.5 * (o.nrot - 1)
+    return c, lambda j: (j - c) * h
+
+
+def _endpoints(o, h, nphi):
+    """entry / exit points, line offsets and directions of every trajectory, from the oracle's tables"""
+    c, lat = _lattice(o, h)
+    out = []
+    for k in range(nphi):
+        T = o.tables(k)
+        v = o.angle_info(k)[0]
+        w = lat(T["t"])
+        S = np.stack([T["u_in"] * v[0] - w * v[1], T["u_in"] * v[1] + w * v[0]], axis=1)
+        E = np.stack([T["u_out"] * v[0] - w * v[1], T["u_out"] * v[1] + w * v[0]], axis=1)
+        out.append(dict(T=T, v=v, w=w, S=S, E=E))
+    return out
+
+
+def _slab_clip_square(L, rot_turns, v, w):
+    """Independent clip of the line R(u) = u v + w n against a square of side L rotated by rot_turns: slab test in the
+    square's own frame.  Returns (u_in, u_out, normal_in, normal_out) with the analytic outward wall normals, or None."""
+    a = 2 * math.pi * rot_turns
+    ex = np.array([math.cos(a), math.sin(a)]); ey = np.array([-math.sin(a), math.cos(a)])
+    n = np.array([-v[1], v[0]])
+    lo, hi, nlo, nhi = -np.inf, np.inf, None, None
+    for e in (ex, ey):
+        p0, d = w * float(n @ e), float(v @ e)          # coordinate along e: p0 + u d, inside iff |.| < L/2
+        if abs(d) < 1e-14:
+            if abs(p0) >= L / 2:
+                return None
+            continue
+        u1, u2 = (-L / 2 - p0) / d, (L / 2 - p0) / d
+        n1, n2 = -e, e                                   # the wall at -L/2 has outward normal -e
+        if u1 > u2:
+            u1, u2, n1, n2 = u2, u1, n2, n1
+        if u1 > lo:
+            lo, nlo = u1, n1
+        if u2 < hi:
+            hi, nhi = u2, n2
+    return (lo, hi, nlo, nhi) if hi > lo else None
+
+
+def _mirror_angle(v, n):
+    m = v - 2.0 * float(v @ n) * n
+    return math.atan2(m[1], m[0]) % (2 * math.pi)
+
+
+def test_gather_weights_reproduce_a_linear_store_on_flat_walls():
+    """PAPER.md:197, R6/R7/R9.  Square rotated by 0.15 angle steps: every reflected direction falls 0.3 (or 0.7) of the
+    way between two lattice angles, and no reflected ray lands on a lattice line, so all four (angle x offset)
+    weights of a gather are in play.  Old stores := a function linear in (end point, lattice angle); the start values
+    of gamma (at u_in) and gamma-tilde (at u_out) must be that function at (boundary point, reflected angle)."""
+    nphi, h, L = 16, 0.1, 2.3
+    dphi = 2 * math.pi / nphi
+    rot = 0.15 * dphi / (2 * math.pi)
+    shapes = [square(L, rot)]
+    n = 34
+    mask = make_mask(shapes, n, n, h)
+    o = oracle.Oracle(n, n, h, mask, shapes, 0.4, wlmod.SYM_S, nphi)
+    ep = _endpoints(o, h, nphi)
+    lin_g = lambda P, phi: (0.3 - 0.2j) + (0.11 + 0.05j) * P[..., 0] + (-0.07 + 0.13j) * P[..., 1] + (0.09 - 0.04j) * phi
+    lin_t = lambda P, phi: (-0.1 + 0.25j) + (0.06 - 0.02j) * P[..., 0] + (0.03 + 0.08j) * P[..., 1] + (-0.05 + 0.07j) * phi
+    g = np.zeros((o.ntraj, 1), complex); gt = np.zeros((o.ntraj, 1), complex)
+    for k in range(nphi):
+        off = o.traj_offset(k)
+        g[off:off + len(ep[k]["w"]), 0] = lin_g(ep[k]["E"], k * dphi)      # gamma_end lives at the exit point
+        gt[off:off + len(ep[k]["w"]), 0] = lin_t(ep[k]["S"], k * dphi)     # gamma-tilde_end at the entry point
+    z = np.array([0.3j])
+    zero = np.zeros((n, n), complex)
+    tested = total = 0
+    worst_clip = 0.0
+    for k in range(nphi):
+        e = ep[k]
+        for i in range(len(e["w"])):
+            clip = _slab_clip_square(L, rot, e["v"], e["w"][i])
+            assert clip is not None
+            worst_clip = max(worst_clip, abs(clip[0] - e["T"]["u_in"][i]), abs(clip[1] - e["T"]["u_out"][i]))
+            ends = o.debug_trajectory(zero, None, None, k, i, z, 0, (g, gt))[2]
+            for which, P, nrm, f, got in (("in", e["S"][i], clip[2], lin_g, complex(ends[4], ends[5])),
+                                          ("out", e["E"][i], clip[3], lin_t, complex(ends[6], ends[7]))):
+                total += 1
+                phi_m = _mirror_angle(e["v"], nrm)
+                if e["T"]["g_idx"][i, 0 if which == "in" else 1].min() < 0 or phi_m > (nphi - 1) * dphi:
+                    continue          # a candidate fell on another wall (corner) / the angle pair wraps through 2 pi
+                tested += 1
+                assert abs(got - f(P, phi_m)) < 1e-13, (k, i, which)
+    assert worst_clip < 1e-12
+    assert tested > 0.6 * total
+
+
+def test_gather_on_a_disc_uses_the_radial_normal():
+    """Same construction on a disc: the store is a smooth function of (polar angle of the end point, lattice angle),
+    the expected start value is that function at (polar angle of the boundary point, direction mirrored at the RADIAL
+    normal).  A curved wall makes the offset interpolation second order, O((h / cos)^2) — so the error must fall by ~4
+    when h and dphi are halved, and a transposed or tangential normal (error O(1)) cannot pass."""
+    errs = []
+    for nphi, h in ((16, 0.1), (32, 0.05)):
+        R = 1.5
+        dphi = 2 * math.pi / nphi
+        shapes = [wlmod.disc(R)]
+        n = int(round(2 * R / h)) + 2
+        mask = make_mask(shapes, n, n, h)
+        o = oracle.Oracle(n, n, h, mask, shapes, 0.4, wlmod.SYM_S, nphi)
+        ep = _endpoints(o, h, nphi)
+        f = lambda P, phi: 0.3 * np.sin(np.arctan2(P[..., 1], P[..., 0]) - 0.4) + 0.2j * np.cos(phi + 0.3) + 0.1 * np.cos(phi) * P[..., 0]
+        g = np.zeros((o.ntraj, 1), complex); gt = np.zeros((o.ntraj, 1), complex)
+        for k in range(nphi):
+            off = o.traj_offset(k)
+            g[off:off + len(ep[k]["w"]), 0] = f(ep[k]["E"], k * dphi)
+            gt[off:off + len(ep[k]["w"]), 0] = f(ep[k]["S"], k * dphi)
+        z = np.array([0.3j]); zero = np.zeros((n, n), complex)
+        worst = 0.0; cnt = 0
+        for k in range(nphi):
+            e = ep[k]
+            for i in range(len(e["w"])):
+                if abs(e["w"][i]) > 0.6 * R:       # incidence within 37 deg of the normal: cos > 0.8
+                    continue
+                # the end points are on the circle (pins the quadratic clip) ...
+                assert abs(np.hypot(*e["S"][i]) - R) < 1e-12 and abs(np.hypot(*e["E"][i]) - R) < 1e-12
+                ends = o.debug_trajectory(zero, None, None, k, i, z, 0, (g, gt))[2]
+                for P, got in ((e["S"][i], complex(ends[4], ends[5])), (e["E"][i], complex(ends[6], ends[7]))):
+                    phi_m = _mirror_angle(e["v"], P / R)           # ... and the wall normal there is radial
+                    if phi_m > (nphi - 1) * dphi:
+                        # the bracketing angles are N-1 and 0: the store's cos/sin in phi are periodic, so this is fine
+                        pass
+                    worst = max(worst, abs(got - f(P, phi_m))); cnt += 1
+        errs.append(worst)
+        assert cnt > 100
+    assert errs[0] < 0.02 and 3.0 < errs[0] / errs[1] < 5.5, errs
+
+
+# ---- rotate-in: Delta (masked bilinear) and A (plain bilinear) at the lattice nodes (R5) ----------------
+def test_rotate_in_interpolation_is_bilinear_and_exact_for_linear_fields():
+    nphi, h, R = 12, 0.1, 1.45
+    shapes = [wlmod.disc(R)]
+    n = 32
+    mask = make_mask(shapes, n, n, h)
+    X, Y = wlmod.grid_xy(n, n, h)
+    x = X[0]; y = Y[:, 0]
+    o = oracle.Oracle(n, n, h, mask, shapes, 0.4, wlmod.SYM_DX2Y2, nphi, charge_sign=-1)
+    rng = np.random.default_rng(11)
+    lin = (0.2 + 0.1j) + (0.05 - 0.02j) * X + (-0.03 + 0.04j) * Y
+    rnd = rng.normal(size=(n, n)) + 1j * rng.normal(size=(n, n))
+    Ax_l, Ay_l = 0.3 * X - 0.1 * Y + 0.02, 0.07 * X + 0.2 * Y - 0.01
+    Ax_r, Ay_r = rng.normal(size=(n, n)), rng.normal(size=(n, n))
+    interp = lambda F: RegularGridInterpolator((y, x), F, method="linear")        # library bilinear on the [y][x] grid
+    c, lat = _lattice(o, h)
+    n_int = n_edge = 0
+    for k in range(nphi):
+        T = o.tables(k); v, eta, _ = o.angle_info(k)
+        for i in range(0, len(T["t"]), 2):
+            jj = np.arange(T["jf"][i], T["jl"][i] + 1)
+            w = lat(T["t"][i]); u = lat(jj)
+            P = np.stack([u * v[1] + w * v[0], u * v[0] - w * v[1]], axis=1)       # (y, x) of the nodes
+            gx = P[:, 1] / h + 0.5 * (n - 1); gy = P[:, 0] / h + 0.5 * (n - 1)
+            i0 = np.floor(gx).astype(int); j0 = np.floor(gy).astype(int)
+            interior = mask[j0, i0] & mask[j0, i0 + 1] & mask[j0 + 1, i0] & mask[j0 + 1, i0 + 1] > 0
+            for D, Axx, Ayy, exact in ((lin, Ax_l, Ay_l, True), (rnd, Ax_r, Ay_r, False)):
+                Dn, an = o.debug_nodes(D * mask, Axx, Ayy, k, i)
+                assert len(Dn) == len(jj)
+                ref_a = -1 * (v[0] * interp(Axx)(P) + v[1] * interp(Ayy)(P))       # sigma_e v.A, A is not masked
+                assert np.max(np.abs(an - ref_a)) < 1e-13
+                ref_D = eta * interp(D)(P)
+                assert np.max(np.abs(Dn - ref_D)[interior], initial=0.0) < 1e-13
+                if exact:   # a linear field is reproduced exactly wherever all four corners are inside the grain
+                    lin_at = eta * ((0.2 + 0.1j) + (0.05 - 0.02j) * P[:, 1] + (-0.03 + 0.04j) * P[:, 0])
+                    assert np.max(np.abs(Dn - lin_at)[interior], initial=0.0) < 1e-13
+                    assert np.max(np.abs(an + (v[0] * (0.3 * P[:, 1] - 0.1 * P[:, 0] + 0.02) + v[1] * (0.07 * P[:, 1] + 0.2 * P[:, 0] - 0.01)))) < 1e-13
+                    # rim nodes: a renormalised average of the corners inside the grain stays within their hull: O(h)
+                    assert np.max(np.abs(Dn - lin_at)) < abs(eta) * 0.08 * h * 1.5 + 1e-15
+            n_int += int(interior.sum()); n_edge += int((~interior).sum())
+    assert n_int > 1000 and n_edge > 50
+
+
+def test_rotate_in_rim_nodes_use_only_corners_inside_the_grain():
+    """R5: Delta outside the mask must never leak into a node value: poisoning it changes nothing."""
+    nphi, h = 8, 0.1
+    shapes = [wlmod.disc(0.95)]
+    n = 22
+    mask = make_mask(shapes, n, n, h)
+    rng = np.random.default_rng(5)
+    D = rng.normal(size=(n, n)) + 1j * rng.normal(size=(n, n))
+    o = oracle.Oracle(n, n, h, mask, shapes, 0.4, wlmod.SYM_S, nphi)
+    for k in range(nphi):
+        for i in range(o.ntraj_angle(k)):
+            a = o.debug_nodes(D * mask, None, None, k, i)[0]
+            b = o.debug_nodes(np.where(mask > 0, D, 1e6), None, None, k, i)[0]
+            assert np.array_equal(a, b)
+
+
+# ---- rotate-back: masked bilinear gather of the per-angle node sums to the grid -------------------------
+def test_rotate_back_is_the_bilinear_interpolant_of_the_lattice_sums():
+    """With a one-angle angle_list the accumulators are W_k (eta_k, v_k, 1) x [the per-angle lattice sums interpolated to
+    the grid points].  The lattice sums themselves come out of the dbg tap; interpolating them with scipy's bilinear
+    routine in the rotated frame must give the grid fields wherever the four surrounding lattice nodes are all inside."""
+    wl = wlmod.make_workload(1, pts_per_xi=4, n_angles=12, n_energies=5)
+    o = oracle.Oracle.from_workload(wl)
+    h, n = wl.h, wl.nx
+    z, w = o.matsubara(5)
+    st = o.reset_stores(wl.delta0, wl.Aext_x, wl.Aext_y, z)
+    c, lat = _lattice(o, h)
+    axis = lat(np.arange(o.nrot))
+    X, Y = wlmod.grid_xy(n, n, h)
+    checked = 0
+    for k in (0, 1, 5, 7, 10):
+        r = o.raw_sweep(wl.delta0, wl.Aext_x, wl.Aext_y, z, w, st, angle_list=[k], dbg_angle=k)
+        v, eta, W = o.angle_info(k)
+        T = o.tables(k)
+        valid = np.zeros((o.nrot, o.nrot), bool)                      # [t][j]
+        for t, jf, jl in zip(T["t"], T["jf"], T["jl"]):
+            valid[t, jf:jl + 1] = True
+        U = X * v[0] + Y * v[1]; Wc = -X * v[1] + Y * v[0]            # lattice coordinates of the grid points
+        j0 = np.floor(U / h + c).astype(int); t0 = np.floor(Wc / h + c).astype(int)
+        inb = (j0 >= 0) & (t0 >= 0) & (j0 + 1 < o.nrot) & (t0 + 1 < o.nrot)
+        j0 = np.clip(j0, 0, o.nrot - 2); t0 = np.clip(t0, 0, o.nrot - 2)
+        ok = (wl.mask > 0) & inb & valid[t0, j0] & valid[t0, j0 + 1] & valid[t0 + 1, j0] & valid[t0 + 1, j0 + 1]
+        pts = np.stack([Wc[ok], U[ok]], axis=1)
+        for name, acc, fac in (("SF", r["num"], W * eta), ("SG", r["Jx"], W * v[0]), ("SG", r["Jy"], W * v[1]),
+                               ("SI", r["I"], W), ("SR", r["R"], W)):
+            ref = RegularGridInterpolator((axis, axis), r["dbg"][name], method="linear")(pts)
+            assert np.max(np.abs(acc[ok] - fac * ref)) < 1e-13 * max(1.0, float(np.max(np.abs(ref)))), (k, name)
+        # rim points (a neighbour outside): the value is still a convex combination of recorded nodes
+        rim = (wl.mask > 0) & ~ok
+        SR = r["dbg"]["SR"]
+        assert np.all(r["R"][rim] >= W * SR[valid].min() - 1e-14) and np.all(r["R"][rim] <= W * SR[valid].max() + 1e-14)
+        checked += int(ok.sum())
+        assert rim.sum() > 0
+    assert checked > 2000
