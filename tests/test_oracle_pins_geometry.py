@@ -114,16 +114,19 @@ def test_gather_weights_reproduce_a_linear_store_on_flat_walls():
     assert tested > 0.6 * total
 
 
-def test_gather_on_a_disc_uses_the_radial_normal():
-    """Same construction on a disc: the store is a smooth function of (polar angle of the end point, lattice angle),
-    the expected start value is that function at (polar angle of the boundary point, direction mirrored at the RADIAL
-    normal).  A curved wall makes the offset interpolation second order, O((h / cos)^2) — so the error must fall by ~4
-    when h and dphi are halved, and a transposed or tangential normal (error O(1)) cannot pass."""
+@pytest.mark.parametrize("hole", [0.0, 0.7])
+def test_gather_on_a_disc_uses_the_radial_normal(hole):
+    """Same construction on a disc, and on an annulus (a disc removed from a disc: PAPER.md:448, :545; DESIGN.md R-MC —
+    every lattice line through the hole carries two trajectories, and the hole's rim is a wall whose grain-outward normal
+    points at the centre): the store is a smooth function of (end point, lattice angle), the expected start value is that
+    function at (boundary point, direction mirrored at the RADIAL normal).  A curved wall makes the offset interpolation
+    second order, O((h / cos)^2) — so the error must fall by ~4 when h and dphi are halved, and a transposed or tangential
+    normal, or a trajectory matched to the wrong rim (errors O(1)), cannot pass."""
     errs = []
+    R = 1.5
     for nphi, h in ((16, 0.1), (32, 0.05)):
-        R = 1.5
         dphi = 2 * math.pi / nphi
-        shapes = [wlmod.disc(R)]
+        shapes = [wlmod.disc(R)] + ([wlmod.disc(hole, add=False)] if hole else [])
         n = int(round(2 * R / h)) + 2
         mask = make_mask(shapes, n, n, h)
         o = oracle.Oracle(n, n, h, mask, shapes, 0.4, wlmod.SYM_S, nphi)
@@ -135,24 +138,31 @@ def test_gather_on_a_disc_uses_the_radial_normal():
             g[off:off + len(ep[k]["w"]), 0] = f(ep[k]["E"], k * dphi)
             gt[off:off + len(ep[k]["w"]), 0] = f(ep[k]["S"], k * dphi)
         z = np.array([0.3j]); zero = np.zeros((n, n), complex)
-        worst = 0.0; cnt = 0
+        worst = 0.0; cnt = {"outer": 0, "inner": 0}
         for k in range(nphi):
             e = ep[k]
+            if hole:      # the independent clip: chord of the outer circle minus the chord of the inner one
+                for wv in np.unique(e["w"]):
+                    sel = np.where(e["w"] == wv)[0]
+                    a = math.sqrt(R * R - wv * wv)
+                    want = [(-a, a)] if abs(wv) >= hole else [(-a, -math.sqrt(hole * hole - wv * wv)), (math.sqrt(hole * hole - wv * wv), a)]
+                    c, lat = _lattice(o, h)
+                    want = [iv for iv in want if np.any((lat(np.arange(o.nrot)) > iv[0]) & (lat(np.arange(o.nrot)) < iv[1]))]
+                    got = sorted(zip(e["T"]["u_in"][sel], e["T"]["u_out"][sel]))
+                    assert len(got) == len(want) and np.allclose(got, want, rtol=0, atol=1e-12)
             for i in range(len(e["w"])):
-                if abs(e["w"][i]) > 0.6 * R:       # incidence within 37 deg of the normal: cos > 0.8
-                    continue
-                # the end points are on the circle (pins the quadratic clip) ...
-                assert abs(np.hypot(*e["S"][i]) - R) < 1e-12 and abs(np.hypot(*e["E"][i]) - R) < 1e-12
                 ends = o.debug_trajectory(zero, None, None, k, i, z, 0, (g, gt))[2]
                 for P, got in ((e["S"][i], complex(ends[4], ends[5])), (e["E"][i], complex(ends[6], ends[7]))):
-                    phi_m = _mirror_angle(e["v"], P / R)           # ... and the wall normal there is radial
-                    if phi_m > (nphi - 1) * dphi:
-                        # the bracketing angles are N-1 and 0: the store's cos/sin in phi are periodic, so this is fine
-                        pass
-                    worst = max(worst, abs(got - f(P, phi_m))); cnt += 1
+                    r = float(np.hypot(*P))
+                    rim = "outer" if abs(r - R) < 1e-12 else "inner"
+                    assert rim == "outer" or abs(r - hole) < 1e-12                 # every end point is on one of the circles
+                    if abs(float(e["v"] @ P)) / r < 0.8:                           # incidence within 37 deg of the normal only
+                        continue
+                    phi_m = _mirror_angle(e["v"], P / r)                           # the wall normal is radial (its sign drops out)
+                    worst = max(worst, abs(got - f(P, phi_m))); cnt[rim] += 1
         errs.append(worst)
-        assert cnt > 100
-    assert errs[0] < 0.02 and 3.0 < errs[0] / errs[1] < 5.5, errs
+        assert cnt["outer"] > 100 and (not hole or cnt["inner"] > 50)
+    assert errs[0] < 0.03 and 3.0 < errs[0] / errs[1] < 5.5, errs
 
 
 # ---- rotate-in: Delta (masked bilinear) and A (plain bilinear) at the lattice nodes (R5) ----------------
