@@ -57,6 +57,7 @@ def lib():
         L.orc_tables.argtypes = [C.c_void_p, C.c_int] + [C.c_void_p] * 4
         L.orc_step.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p]
         L.orc_gamma_h.argtypes = [C.c_void_p] * 3
+        L.orc_opcount.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p]
         L.orc_march.argtypes = [C.c_int, C.c_int] + [C.c_void_p] * 9
         L.orc_reset_stores.argtypes = [C.c_void_p] * 4 + [C.c_int] + [C.c_void_p] * 4
         L.orc_sweep.argtypes = ([C.c_void_p] * 4 + [C.c_int] + [C.c_void_p] * 12 + [C.c_void_p, C.c_int] +
@@ -89,6 +90,17 @@ def step(g: complex, De: complex, z: complex, l: float, stepper: int = 0) -> com
     lib().orc_step(stepper, _p(np.array([g.real, g.imag])), _p(np.array([De.real, De.imag])),
                    _p(np.array([z.real, z.imag])), l, _p(out))
     return complex(out[0], out[1])
+
+
+def step_opcount(stepper: int = 0, g: complex = 0.2 - 0.3j, De: complex = 0.3 + 0.1j, z: complex = 0.04 + 0.25j, l: float = 0.05):
+    """Real floating-point operations of one step as the oracle states it (textbook complex arithmetic), counted by
+    running the same C++ statements on an operation-counting scalar: dict(mul, add, div, sqrt, exp, sincos, value)."""
+    cnt = np.zeros(6, np.int64); out = np.zeros(2)
+    lib().orc_opcount(stepper, _p(np.array([g.real, g.imag])), _p(np.array([De.real, De.imag])),
+                      _p(np.array([z.real, z.imag])), l, _p(cnt), _p(out))
+    d = dict(zip(("mul", "add", "div", "sqrt", "exp", "sincos"), (int(v) for v in cnt)))
+    d["value"] = complex(out[0], out[1])
+    return d
 
 
 def gamma_h(De: complex, z: complex) -> complex:

@@ -351,8 +351,6 @@ static double interp_plain(const Ctx& C, const double* F, double x, double y) {
 // Riccati steps (Eq. 25 :169, App. C :968-1003)
 //   d gamma / ds = i [ conj(De) gamma^2 + 2 z gamma + De ]            (C1-C2 with v_F = 1)
 // ---------------------------------------------------------------------------------------------------
-// Homogeneous solution (SURVEY §8c-2): Omega = sqrt(|De|^2 - z^2) principal branch (Re >= 0),
-// gamma_h = -De / (z + i Omega).
 // Delta(p_F, R) of Eq. 1 (:37) for the direction phi at the point (x, y): sum over the components of
 // eta_G(phi) times the masked-bilinear interpolant of Delta_G.  `bad` counts the point once.
 static cd gap_at(const Ctx& C, const cd* D, double phi, double x, double y, int* bad) {
@@ -363,25 +361,33 @@ static cd gap_at(const Ctx& C, const cd* D, double phi, double x, double y, int*
     return s;
 }
 
-static inline cd omega_of(cd De, cd z) { return std::sqrt(cd(std::norm(De), 0.0) - z * z); }
-static inline cd gamma_h(cd De, cd z) { return -De / (z + I_ * omega_of(De, z)); }
+// Homogeneous solution (SURVEY §8c-2): Omega = sqrt(|De|^2 - z^2) principal branch (Re >= 0),
+// gamma_h = -De / (z + i Omega).
+// The four functions below are templates on the complex type only so that `orc_opcount` can run the very same
+// statements on an operation-counting scalar (bench.py's "textbook" flop count); every caller uses C = cd.
+template <class C> static inline C omega_of(C De, C z) { using std::sqrt; using std::norm; return sqrt(C(norm(De), 0.0) - z * z); }
+template <class C> static inline C gamma_h(C De, C z) { return -De / (z + C(0.0, 1.0) * omega_of(De, z)); }
 
 // Closed-form ("stepping method") step of length l with constant De, z:
 // delta = gamma - gamma_h obeys the Bernoulli equation delta' = -2 Omega delta + i conj(De) delta^2.
-static inline cd step_closed(cd g, cd De, cd z, double l) {
-    cd Om = omega_of(De, z);
-    cd gh = -De / (z + I_ * Om);
-    cd Cc = I_ * std::conj(De) / (2.0 * Om);
-    cd e = std::exp(-2.0 * Om * l);
-    cd d0 = g - gh;
+template <class C> static inline C step_closed(C g, C De, C z, double l) {
+    using std::conj; using std::exp;
+    const C I1(0.0, 1.0);
+    C Om = omega_of(De, z);
+    C gh = -De / (z + I1 * Om);
+    C Cc = I1 * conj(De) / (2.0 * Om);
+    C e = exp(-2.0 * Om * l);
+    C d0 = g - gh;
     return gh + d0 * e / (1.0 + Cc * d0 * (e - 1.0));
 }
 // Implicit mid-point rule, PAPER.md C4-C9 (:984-1001) verbatim with v_F = 1, h -> l.
-static inline cd step_midpoint(cd g, cd De, cd z, double l) {
-    cd c2 = I_ * (l / 4.0) * std::conj(De);
-    cd c1 = 2.0 * c2 * g + I_ * l * z - 1.0;
-    cd c0 = (c1 - c2 * g + 2.0) * g - 4.0 * std::conj(c2);
-    return 2.0 * c0 / (-c1 + std::sqrt(c1 * c1 - 4.0 * c2 * c0));
+template <class C> static inline C step_midpoint(C g, C De, C z, double l) {
+    using std::conj; using std::sqrt;
+    const C I1(0.0, 1.0);
+    C c2 = I1 * (l / 4.0) * conj(De);
+    C c1 = 2.0 * c2 * g + I1 * l * z - 1.0;
+    C c0 = (c1 - c2 * g + 2.0) * g - 4.0 * conj(c2);
+    return 2.0 * c0 / (-c1 + sqrt(c1 * c1 - 4.0 * c2 * c0));
 }
 static inline cd step(int stepper, cd g, cd De, cd z, double l) {
     return stepper == 1 ? step_midpoint(g, De, z, l) : step_closed(g, De, z, l);
@@ -465,6 +471,46 @@ static cd start_gammat(const Ctx& C, const Traj& T, const Pieces& P, const cd* D
 }
 
 // ---------------------------------------------------------------------------------------------------
+// Operation-counting complex scalar: runs the step templates above and tallies the REAL floating-point operations of
+// the textbook complex arithmetic (bench.py reports them as the "textbook" work of one trajectory-step update; the
+// tally is derived from the oracle's own statements, nothing is typed in).  Not used by any sweep.
+// ---------------------------------------------------------------------------------------------------
+namespace opcount {
+struct Tally { long mul, add, div, sqrt, exp, sincos; };
+static Tally T;
+struct CC {
+    double re, im;
+    CC(double r = 0.0, double i = 0.0) : re(r), im(i) {}
+};
+static inline CC operator-(CC a) { return CC(-a.re, -a.im); }
+static inline CC operator+(CC a, CC b) { T.add += 2; return CC(a.re + b.re, a.im + b.im); }
+static inline CC operator-(CC a, CC b) { T.add += 2; return CC(a.re - b.re, a.im - b.im); }
+static inline CC operator+(double a, CC b) { T.add += 1; return CC(a + b.re, b.im); }
+static inline CC operator-(CC a, double b) { T.add += 1; return CC(a.re - b, a.im); }
+static inline CC operator+(CC a, double b) { T.add += 1; return CC(a.re + b, a.im); }
+static inline CC operator*(CC a, CC b) { T.mul += 4; T.add += 2; return CC(a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re); }
+static inline CC operator*(double a, CC b) { T.mul += 2; return CC(a * b.re, a * b.im); }
+static inline CC operator*(CC a, double b) { T.mul += 2; return CC(a.re * b, a.im * b); }
+static inline CC operator/(CC a, CC b) {             // (a conj b) / |b|^2
+    T.mul += 6; T.add += 3; T.div += 2;
+    double d = b.re * b.re + b.im * b.im;
+    return CC((a.re * b.re + a.im * b.im) / d, (a.im * b.re - a.re * b.im) / d);
+}
+static inline CC conj(CC a) { return CC(a.re, -a.im); }
+static inline double norm(CC a) { T.mul += 2; T.add += 1; return a.re * a.re + a.im * a.im; }
+static inline CC sqrt(CC a) {                        // principal branch: |a|, sqrt((|a| + re)/2), im / (2 re')
+    T.mul += 4; T.add += 2; T.sqrt += 2; T.div += 1;
+    std::complex<double> r = std::sqrt(std::complex<double>(a.re, a.im));
+    return CC(r.real(), r.imag());
+}
+static inline CC exp(CC a) {                         // e^re (cos im + i sin im)
+    T.exp += 1; T.sincos += 1; T.mul += 2;
+    std::complex<double> r = std::exp(std::complex<double>(a.re, a.im));
+    return CC(r.real(), r.imag());
+}
+}  // namespace opcount
+
+// ---------------------------------------------------------------------------------------------------
 // C ABI
 // ---------------------------------------------------------------------------------------------------
 extern "C" {
@@ -524,6 +570,18 @@ void orc_step(int stepper, const double* g, const double* De, const double* z, d
 }
 void orc_gamma_h(const double* De, const double* z, double* out) {
     cd r = gamma_h(cd(De[0], De[1]), cd(z[0], z[1])); out[0] = r.real(); out[1] = r.imag();
+}
+// Real floating-point operations of ONE step (one trajectory-step update of the metric) as the oracle states it:
+// counts[6] = mul, add, div, sqrt, exp, sincos.  The step is run on the counting scalar; its value is returned in out
+// so that the caller can check it against orc_step.
+void orc_opcount(int stepper, const double* g, const double* De, const double* z, double l, long* counts, double* out) {
+    using opcount::CC;
+    opcount::T = opcount::Tally{0, 0, 0, 0, 0, 0};
+    CC r = stepper == 1 ? step_midpoint(CC(g[0], g[1]), CC(De[0], De[1]), CC(z[0], z[1]), l)
+                        : step_closed(CC(g[0], g[1]), CC(De[0], De[1]), CC(z[0], z[1]), l);
+    counts[0] = opcount::T.mul; counts[1] = opcount::T.add; counts[2] = opcount::T.div;
+    counts[3] = opcount::T.sqrt; counts[4] = opcount::T.exp; counts[5] = opcount::T.sincos;
+    out[0] = r.re; out[1] = r.im;
 }
 void orc_march(int stepper, int M, const double* len, const double* De, const double* a, const double* z0,
                const double* g_start, const double* gt_start, double* G, double* GT, double* ends) {

@@ -669,3 +669,18 @@ def test_basis_functions_are_orthonormal_on_the_angle_set():
     o1 = oracle.Oracle(4, 4, 0.1, sq, [square(0.4)], 0.5, 1, 64, crystal_rotation=0.125)
     o2 = oracle.Oracle(4, 4, 0.1, sq, [square(0.4)], 0.5, 2, 64)
     assert max(abs(o1.angle_info(k)[1] - o2.angle_info(k)[1]) for k in range(64)) < 1e-14
+
+
+def test_opcount_scalar_runs_the_same_step():
+    """bench.py's "textbook" flop count comes from running the oracle's own step statements on an operation-counting
+    scalar: it must return the step's value, and the tallies must be those of the formula as printed (closed form: one
+    complex square root, one complex exponential, three complex divisions and one real-by-complex; mid-point C4-C9: one
+    square root, one division, no exponential)."""
+    for st in (0, 1):
+        for (g, De, z, l) in ((0.2 - 0.3j, 0.3 + 0.1j, 0.04 + 0.25j, 0.05), (0.1 + 0.6j, 0.34 - 0.02j, 0.3 + 0.003j, 0.1)):
+            d = oracle.step_opcount(st, g, De, z, l)
+            assert abs(d["value"] - oracle.step(g, De, z, l, st)) < 1e-15
+    c, m = oracle.step_opcount(0), oracle.step_opcount(1)
+    assert (c["sqrt"], c["exp"], c["sincos"]) == (2, 1, 1) and (m["sqrt"], m["exp"], m["sincos"]) == (2, 0, 0)
+    assert c["div"] == 2 * 3 + 1 and m["div"] == 2 * 1 + 1          # 2 real divisions per complex division + 1 in the square root
+    assert 40 <= c["mul"] <= 70 and 25 <= c["add"] <= 45
