@@ -9,6 +9,14 @@ solve, Barzilai-Borwein mixing.  Workload at N=1: BASELINE.json configs[4] (s-wa
 1600x1600 grid, 256 angles, 512 Matsubara energies, kappa = 2, 20 vortices), the config the metric's FP64
 target is quoted on.  Inputs are seeded synthetic fields (workloads/), resident in HBM for `value`; `e2e`
 repeats the measurement with pinned HOST buffers copied in and out every step.
+
+The timed state.  The first Barzilai-Borwein iterations at kappa = 2 overshoot the induced vector potential
+(|A| up to 6 A0), which sends march rounds to dearer table tiers; from iteration ~10 on the cost of an iteration
+is constant to 0.3 % (profiles/r2_transient.md).  The run therefore first does `--burnin` untimed iterations,
+then W warm-up steps, then the K timed steps, then the K end-to-end steps: all legs sit on the same stationary
+part of the run, so `value` does not depend on --steps and e2e = value + the host copies.  The cost of the very
+first iterations is reported beside it (`config.transient`).
+
 With --gpus N > 1 (torchrun) the Matsubara energies are sharded across ranks (the march, the specular
 boundary condition and the boundary stores never couple energies) and the partial Delta_new, j, I fields are
 summed with one NCCL all-reduce per sweep; per-rank work shrinks as N grows -> "strong" scaling.
@@ -17,8 +25,8 @@ summed with one NCCL all-reduce per sweep; per-rank work shrinks as N grows -> "
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
-import math
 import os
 import subprocess
 import sys
@@ -34,29 +42,51 @@ import workloads  # noqa: E402
 
 METRIC = "riccati_trajectory_step_updates_per_s"
 UNIT = "updates/s"
-# FP64-pipe instructions the closed-form path needs per unit = (piece, energy, angle pair) = 4 logical updates
-# (gamma and gamma-tilde for angles k and k+N/2): DESIGN.md §6 tally of the kernel's own algorithm.
-#   "recompute" rounds (every piece inside the radius of the per-energy Taylor table of T): T twice 2 x 15, two Moebius
-#       steps 2 x 27, node products 26 (28 with non-unit weights; the bench's Matsubara table has unit weights and the
-#       kernel variant with the weights compiled out runs), energy reduction 8 = 118, + half a Moebius step 13.5 because
-#       only every second gamma-tilde is spilled and the other is re-stepped in pass 2 = 131.5; scratch traffic 8 B
-#       written + 8 B read = 16 B
-#   "recompute_pole" rounds (|a| beyond that table but inside the pole-subtracted one): T twice 2 x 24 (degree 5 + the
-#       pole term with one reciprocal), 54, 26, 8, 13.5 = 149.5; 16 B per unit
-#   "stored-T" rounds (strong vector potential): T once from the pole-subtracted table 36, 54, 26, 8 = 124; 64 B per unit
-# Evaluating T from its definition (sqrt, exp, sin/cos) would be 86 per evaluation — reported as context only.
-ALGO_FP64_INSTR_PER_UNIT = {"recompute": 131.5, "recompute_pole": 149.5, "stored": 124.0}
-# the least FP64 work any of these layouts could do per unit if nothing were evaluated twice: T once 15, two steps 54,
-# node products 26, reduction 8 — reported beside the roofline so that recomputation is not mistaken for useful work
-MIN_WORK_FP64_INSTR_PER_UNIT = 103.0
-ALGO_HBM_BYTES_PER_UNIT = {"recompute": 16.0, "recompute_pole": 16.0, "stored": 64.0}
-TEXTBOOK_FP64_INSTR_PER_UNIT = 184.0
-ALGO_FP64_INSTR_PER_UNIT_MIDPOINT = 2 * 66.0 + 28.0 + 8.0     # the mid-point kernels keep the weights
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE march launch at configs[4], fp64, closed-form stepper, all rounds in
-# "recompute" mode (--sweep-only: A = A_ext), from the `ncu --set full` capture summarised in profiles/
-# (profiles/r1_march_fp64_cfg4_ncu_full.md: 1.518 TB read + 1.255 TB written)
-NCU_TRAFFIC_BYTES = {(4, 64, 0): 2.773331e12}
-NCU_PIPE_FP64_ACTIVE_PCT = {(4, 64, 0): 74.3}
+
+# ---- FP64-pipe instruction tallies per unit = (piece, energy, angle pair) = 4 logical updates (gamma and gamma-tilde
+# for angles k and k + N/2; the kernel marches two of them, Eq. 13 gives the other two).  FMA = one instruction = 2 flops.
+# Each stage is derived in DESIGN.md §6; the EXECUTED tally is checked against the ncu instruction counters
+# (profiles/r2_march_ncu.json, read below when it belongs to the kernel sources in the tree).
+STAGE_FP64 = {
+    "T_table_deg5": 15.0,       # dw 1, |dw|^2 2, real-coefficient degree-5 polynomial at complex dw 10, remainder 2
+    "T_pole_table": 24.0,       # pole term (one reciprocal) + degree-5 remainder
+    "T_pole_table_deg8": 36.0,  # stored-T rounds: degree 8, warp vote
+    "moebius_step": 27.0,       # z g + De 4, N 4, z + conj(De) g 4, Q 4, |Q|^2 2, reciprocal 3, N conj(Q) / |Q|^2 6
+    "node_products": 26.0,      # P 4, 1+P 1, |.|^2 2, reciprocal 3, 1/(1+P) 2, six summands 14 (unit weights)
+    "energy_reduction": 8.0,    # column sums of the transpose stage + running sum
+}
+# least work: nothing evaluated twice — T once, gamma and gamma-tilde stepped once, products, reduction
+LEAST_WORK_FP64 = STAGE_FP64["T_table_deg5"] + 2 * STAGE_FP64["moebius_step"] + STAGE_FP64["node_products"] + STAGE_FP64["energy_reduction"]
+# what the kernel executes: T in both passes, and every second gamma-tilde re-stepped in pass 2 instead of spilled
+EXECUTED_FP64 = {
+    "recompute": LEAST_WORK_FP64 + STAGE_FP64["T_table_deg5"] + 0.5 * STAGE_FP64["moebius_step"],
+    "recompute_pole": LEAST_WORK_FP64 - STAGE_FP64["T_table_deg5"] + 2 * STAGE_FP64["T_pole_table"] + 0.5 * STAGE_FP64["moebius_step"],
+    "stored": LEAST_WORK_FP64 - STAGE_FP64["T_table_deg5"] + STAGE_FP64["T_pole_table_deg8"],
+}
+EXECUTED_FP64_MIDPOINT = 2 * 66.0 + 28.0 + 8.0
+ALGO_HBM_BYTES_PER_UNIT = {"recompute": 16.0, "recompute_pole": 16.0, "stored": 64.0}   # scratch out + back
+
+
+def source_hash():
+    """sha256 over the kernel sources: ncu figures in profiles/ are only quoted for the code they were captured from"""
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2205_15000_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh", ".hpp")):
+            h.update(f.encode()); h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()
+
+
+def ncu_capture(key):
+    """figures of the committed ncu capture `key`, or None when the kernel sources have changed since"""
+    p = os.path.join(ROOT, "profiles", "r2_march_ncu.json")
+    if not os.path.exists(p):
+        return None
+    j = json.load(open(p))
+    c = j.get("captures", {}).get(key)
+    if not c or c.get("source_sha256") != source_hash():
+        return None
+    return c
 
 
 class ClockSampler(threading.Thread):
@@ -81,13 +111,14 @@ class ClockSampler(threading.Thread):
         self.join(timeout=5)
         sm = [float(r[0]) for r in self.rows if r[0].replace(".", "").isdigit()]
         mx = [float(r[1]) for r in self.rows if r[1].replace(".", "").isdigit()]
+        pw = [float(r[2]) for r in self.rows if r[2].replace(".", "").isdigit()]
         reasons = set()
         for r in self.rows:
             for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
                 if v.lower().startswith("active"):
                     reasons.add(name)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": sorted(reasons), "samples": len(sm)}
+                "power_w": float(np.median(pw)) if pw else None, "reasons": sorted(reasons), "samples": len(sm)}
 
 
 def parse():
@@ -101,11 +132,14 @@ def parse():
     ap.add_argument("--n-angles", type=int, default=None)
     ap.add_argument("--n-energies", type=int, default=None)
     ap.add_argument("--size-scale", type=float, default=1.0)
+    ap.add_argument("--burnin", type=int, default=None, help="untimed self-consistent iterations before the warm-up (default 12 with an induced A, else 0)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--sweep-only", action="store_true", help="time sc_riccati_sweep alone (profiling aid)")
+    ap.add_argument("--sweep-only", action="store_true", help="time sc_riccati_sweep alone at the initial fields (profiling aid)")
     ap.add_argument("--stepper", type=int, default=0, help="0 closed-form step (north_star), 1 the paper's implicit mid-point rule")
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32], help="arithmetic of the march (ABI buffers stay fp64)")
     ap.add_argument("--no-fp32-leg", action="store_true", help="skip the extra FP32-mode timing that configs[4] asks for")
+    ap.add_argument("--no-ldos-leg", action="store_true", help="skip the sc_ldos timing on configs[3]")
+    ap.add_argument("--ldos-only", action="store_true", help="time sc_ldos on configs[3] alone (profiling aid)")
     return ap.parse_args()
 
 
@@ -151,14 +185,27 @@ def oracle_sample(wl, cores):
     return r["stats"]["n_updates"], dt, f"{nang} of {wl.n_angles} angles x {ne} of {wl.n_energies} energies, all trajectories, 1 sweep"
 
 
+CPU_NOTE = ("the parity checker as it stands (g++ -O2, std::complex, library sqrt/exp, no Eq. 13 symmetry, every logical update "
+            "executed): a reported baseline, not a tuned CPU implementation")
+
+
+def textbook_count():
+    """real flops of one trajectory-step update as the oracle states the closed-form step, counted by running the
+    oracle's own statements on an operation-counting scalar (oracle.step_opcount)"""
+    import oracle
+    c = oracle.step_opcount(0)
+    ops = {k: c[k] for k in ("mul", "add", "div", "sqrt", "exp", "sincos")}
+    return {"per_update": ops, "flops_per_update": sum(ops.values()), "flops_per_unit": 4 * sum(ops.values()),
+            "note": "textbook complex arithmetic, each division / square root / exponential / sin-cos pair counted as ONE flop; "
+                    "4 logical updates per unit"}
+
+
 def run_reference(a):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     wl = workload_from_args(a)
     cores = os.cpu_count() or 1
-    for _ in range(min(a.warmup, 1)):
-        pass                                        # the oracle has no warm-up state worth timing away
     tot_u, tot_t, desc = 0, 0.0, ""
     for _ in range(a.steps):
         u, t, desc = oracle_sample(wl, cores)
@@ -167,7 +214,7 @@ def run_reference(a):
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": a.gpus, "steps": a.steps,
             "warmup": a.warmup, "ms_per_step": 1e3 * tot_t / a.steps, "higher_is_better": True, "scaling": "strong",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_of(wl, a),
-            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc, "note": CPU_NOTE},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
     print(json.dumps(line))
 
@@ -175,29 +222,102 @@ def run_reference(a):
 # ------------------------------------------------------------------------------------------------
 # CUDA path
 # ------------------------------------------------------------------------------------------------
-def run_ours(a):
-    import torch
-    import paper_2205_15000_b200 as sc
+def time_iterations(ctx, torch, dist, world, devname, nsteps, step_fn):
+    """K steps between barriers + synchronize, CUDA events on the stream the library launches on; returns
+    (ms of the slowest rank, march ms per launch, launches, units (all, stored-T, pole table), kernels launched)"""
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    ctx.sc_debug_march_time(); ctx.sc_debug_march_units(); ctx.sc_debug_launch_count()
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(nsteps):
+        step_fn()
+    e1.record()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    ms = e0.elapsed_time(e1)
+    launches = ctx.sc_debug_launch_count()
+    mms, nl = ctx.sc_debug_march_time()
+    units = ctx.sc_debug_march_units()
+    if world > 1:
+        tmax = torch.tensor([ms], dtype=torch.float64, device=devname)
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        ms = float(tmax.item())
+    return ms, mms / max(nl, 1), nl, units, launches
 
-    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    import torch.distributed as dist
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    torch.cuda.set_device(local)
+
+def march_roofline(a, wl, ctx, kernel, mk_ms, nl, units, step_ms, precision, full_size, clocks):
+    """roofline object of the march kernel for one timed leg"""
+    u_all, u_st, u_pl = (v / max(nl, 1) for v in units)
+    u_rec = u_all - u_st - u_pl
+    if a.stepper == 0:
+        executed = sum(EXECUTED_FP64[k] * u for k, u in (("recompute", u_rec), ("recompute_pole", u_pl), ("stored", u_st)))
+        hbm = sum(ALGO_HBM_BYTES_PER_UNIT[k] * u for k, u in (("recompute", u_rec), ("recompute_pole", u_pl), ("stored", u_st)))
+        least = LEAST_WORK_FP64 * u_all
+    else:
+        executed = EXECUTED_FP64_MIDPOINT * u_all; hbm = 32.0 * u_all; least = executed
+    if precision == 32:
+        hbm *= 0.5
+    sec = mk_ms * 1e-3
+    if precision == 64:
+        burst = 2.0 * ctx.sc_debug_fp64_peak()[0] / 1e12
+        sustained = 2.0 * ctx.sc_debug_fp64_peak_sustained(2.0) / 1e12
+        peak_kind = "measured register-resident DFMA rate (fp64 pipe): larger of a best-of-3 11 ms burst and a 2 s sustained run"
+    else:
+        burst = sustained = 2.0 * ctx.sc_debug_pipe_peak(1, 2.0) / 1e12
+        peak_kind = "measured register-resident FFMA rate (fp32 pipe), 2 s sustained run"
+    peak = max(burst, sustained)
+    cap = ncu_capture(f"cfg{wl.cfg}_f{precision}_stepper{a.stepper}") if full_size else None
+    achieved = 2.0 * least / sec / 1e12
+    r = {"bound": "alu", "kernel": "sck::" + kernel, "launches_timed": nl,
+         "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+         "frac_basis": f"least-work count: {LEAST_WORK_FP64:.0f} fp{precision}-pipe instructions per unit (T once, two Moebius steps, node "
+                       "products, energy reduction; nothing evaluated twice) x units / march time (CUDA events around the march "
+                       "launches of the timed steps) / measured peak",
+         "traffic": cap["dram_bytes"] if cap else None,
+         "algorithmic_bytes_per_launch": hbm,
+         "peak_kind": peak_kind, "peak_burst": burst, "peak_sustained": sustained,
+         "pipe_utilisation": {"instr_per_unit_tally": executed / max(u_all, 1.0),
+                              "tflops": 2.0 * executed / sec / 1e12, "frac": 2.0 * executed / sec / 1e12 / peak,
+                              "note": "what the kernel executes on purpose: T evaluated in both passes and every second gamma-tilde "
+                                      "re-stepped instead of spilled (DESIGN.md §6)"},
+         "march_ms": mk_ms, "march_share_of_step": mk_ms / step_ms,
+         "units_per_launch": u_all, "units_share_stored_T": u_st / max(u_all, 1.0), "units_share_recompute_pole_table": u_pl / max(u_all, 1.0),
+         "hbm_bytes_per_unit_algorithmic": hbm / max(u_all, 1.0), "hbm_gbs_algorithmic": hbm / sec / 1e9}
+    if cap:     # figures of the committed ncu capture of THIS source tree (profiles/r2_march_ncu.json)
+        r["ncu"] = {k: cap[k] for k in cap if k != "source_sha256"}
+        if "fp_pipe_warp_instr_per_unit" in cap:
+            r["pipe_utilisation"]["instr_per_unit_ncu"] = cap["fp_pipe_warp_instr_per_unit"]
+    else:
+        r["ncu"] = None
+    if precision == 32:
+        mufu = ctx.sc_debug_pipe_peak(2, 1.0)
+        r["sfu"] = {"mufu_peak_per_s": mufu, "mufu_per_unit_tally": 3.5,
+                    "mufu_issue_frac": 3.5 * u_all / sec / mufu,
+                    "note": "MUFU.RCP seeds of the reciprocals: one per Moebius step and node product (3.5 per unit with the re-stepped "
+                            "gamma-tilde) against the measured MUFU issue rate"}
+    else:
+        mufu = ctx.sc_debug_pipe_peak(3, 1.0)
+        r["sfu"] = {"mufu_peak_per_s": mufu, "mufu_per_unit_tally": 3.5, "mufu_issue_frac": 3.5 * u_all / sec / mufu,
+                    "note": "MUFU.RCP64H seeds (3.5 per unit) against the measured MUFU.RCP64H issue rate"}
+    return r
+
+
+def run_leg(a, sc, torch, dist, wl, local, world, precision, burnin, full_size):
+    """burn-in, warm-up, K device-resident steps, K end-to-end steps for one arithmetic precision"""
     devname = f"cuda:{local}"
-    wl = workload_from_args(a)
-    ctx = sc.ScContext.from_workload(wl, device=local, stepper=a.stepper, precision=a.precision)
+    dev = lambda x: torch.as_tensor(np.ascontiguousarray(x), device=devname)
+    ctx = sc.ScContext.from_workload(wl, device=local, stepper=a.stepper, precision=precision)
     if world > 1:
-        # energy sharding: this rank marches its slice of the Matsubara table; one NCCL all-reduce of the
-        # five accumulator fields per sweep; A-solve and mixing are replicated (deterministic, identical on all ranks)
         from paper_2205_15000_b200 import sharding
         sharding.attach(ctx, wl.t, wl.n_energies)
-    dev = lambda x: torch.as_tensor(np.ascontiguousarray(x), device=devname)
     ng = wl.nx * wl.ny
     delta = dev(wl.delta0.astype(np.complex128))
     aix = torch.zeros((wl.ny, wl.nx), dtype=torch.float64, device=devname); aiy = torch.zeros_like(aix)
-    ctx.sc_set_external_field(dev(wl.Aext_x), dev(wl.Aext_y))
+    dev_ax, dev_ay = dev(wl.Aext_x), dev(wl.Aext_y)
+    ctx.sc_set_external_field(dev_ax, dev_ay)
     acc = wl.accelerator
     dn = torch.zeros_like(delta); jx = torch.zeros_like(aix); jy = torch.zeros_like(aix); fe = torch.zeros_like(aix)
 
@@ -208,166 +328,159 @@ def run_ours(a):
         else:
             ctx.sc_iterate(acc, 1.0, False, delta, aix, aiy)
 
-    dev_ax, dev_ay = dev(wl.Aext_x), dev(wl.Aext_y)
-
+    # the first iterations: their cost (context for `transient`), and the burn-in that takes the run past them
+    transient = []
+    for it in range(burnin):
+        ctx.sc_debug_march_time(); ctx.sc_debug_march_units()
+        t0 = time.perf_counter(); step(); torch.cuda.synchronize(); dt = time.perf_counter() - t0
+        u = ctx.sc_debug_march_units()
+        if it < 8:
+            transient.append({"iteration": it, "s": round(dt, 4), "stored_T": round(u[1] / max(u[0], 1), 4), "pole_table": round(u[2] / max(u[0], 1), 4)})
     for _ in range(max(a.warmup, 3)):
         step()
     torch.cuda.synchronize()
     sampler = ClockSampler(local); sampler.start()
-    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
-    if world > 1:
-        dist.barrier()
-    torch.cuda.synchronize()
-    ctx.sc_debug_march_time()                       # reset: count only the march launches of the timed steps
-    ctx.sc_debug_march_units()
-    ctx.sc_debug_launch_count()
-    e0.record()
-    for _ in range(a.steps):
-        step()
-    e1.record()
-    torch.cuda.synchronize()
-    if world > 1:
-        dist.barrier()
-    ms = e0.elapsed_time(e1)
+    ms, mk_ms, nl, units, launches = time_iterations(ctx, torch, dist, world, devname, a.steps, step)
     clocks = sampler.stop()
-    gpu_launches = ctx.sc_debug_launch_count()      # kernels of the library launched by the timed steps (counted at the launch sites)
-    timed_kernel = ctx.sc_debug_last_march_variant()
-    march_total_ms, march_launches = ctx.sc_debug_march_time()      # CUDA events around each march launch of the timed region
-    units_timed, units_timed_stored, units_timed_pole = ctx.sc_debug_march_units()     # units of those launches, by mode
-    if world > 1:                                   # device time of the slowest rank
-        tmax = torch.tensor([ms], dtype=torch.float64, device=devname)
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        ms = float(tmax.item())
+    kernel = ctx.sc_debug_last_march_variant()
 
-    # unit counts of one sweep (one extra sweep with stats, outside the timed region)
-    ctx.sc_set_fields(delta, dev_ax + aix, dev_ay + aiy)
-    st = ctx.sc_riccati_sweep(dn, jx, jy, fe, want_stats=True)
-    units = st.n_updates / 4.0                    # this rank's (node, energy, angle-pair) units incl. the boundary pieces
-    n_updates, n_exec = st.n_updates, st.n_updates_executed
-    if world > 1:                                 # whole-job updates = sum over the energy shards
-        tot = torch.tensor([n_updates, n_exec], dtype=torch.float64, device=devname)
-        dist.all_reduce(tot)
-        n_updates, n_exec = int(tot[0].item()), int(tot[1].item())
-    peak_dfma, clk = ctx.sc_debug_fp64_peak()
-    mk_ms = march_total_ms / max(march_launches, 1)
-    full_size = world == 1 and not (a.pts_per_xi or a.n_angles or a.n_energies or a.size_scale != 1.0)
-    # algorithmic work of ONE average march launch of the timed region (units counted by the library, by mode)
-    nl = max(march_launches, 1)
-    u_all = units_timed / nl; u_st = units_timed_stored / nl; u_pl = units_timed_pole / nl; u_rec = u_all - u_st - u_pl
-    if a.stepper == 0:
-        instr = sum(ALGO_FP64_INSTR_PER_UNIT[k] * u for k, u in (("recompute", u_rec), ("recompute_pole", u_pl), ("stored", u_st)))
-        hbm = sum(ALGO_HBM_BYTES_PER_UNIT[k] * u for k, u in (("recompute", u_rec), ("recompute_pole", u_pl), ("stored", u_st)))
-    else:
-        instr = ALGO_FP64_INSTR_PER_UNIT_MIDPOINT * u_all
-        hbm = 32.0 * u_all
-    if a.precision == 32:
-        hbm *= 0.5
-    achieved = 2.0 * instr / (mk_ms * 1e-3) / 1e12
-    peak_burst = 2.0 * peak_dfma / 1e12
-    peak_sustained = 2.0 * ctx.sc_debug_fp64_peak_sustained(2.0) / 1e12
-    peak = max(peak_burst, peak_sustained)
-    peak_kind = "measured register-resident DFMA rate (fp64 pipe)"
-    if a.precision == 32:
-        # the fp32 march runs the same instruction stream on the FP32 pipe: 128 FMA lanes per SM (twice the fp64 lanes);
-        # no measured fp32 figure exists here, so the peak is nominal (unit count x maximum SM clock)
-        peak = 2.0 * 148 * 128 * (clocks.get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
-        peak_kind = "nominal fp32 pipe: 148 SMs x 128 FMA lanes x max SM clock"
-    key = (wl.cfg, a.precision, a.stepper)
-    roofline = {"bound": "alu", "kernel": "sck::" + timed_kernel,
-                "launches_timed": march_launches, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                "frac": achieved / peak,
-                "traffic": NCU_TRAFFIC_BYTES.get(key) if full_size else None,
-                "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/) of a launch with ALL rounds in recompute mode (16 B algorithmic per unit = 2.11e12, + 0.39e12 running sums + 0.3e12 coefficient records); stored-T rounds move 64 B per unit",
-                "algorithmic_bytes_per_launch": hbm,
-                "ncu_pipe_fp64_cycles_active_pct": NCU_PIPE_FP64_ACTIVE_PCT.get(key) if full_size else None,
-                "note": "fp64 pipe: flops = 2 x FP64-pipe instructions; achieved = algorithmic count (DESIGN.md §6) x units / "
-                        "march duration (CUDA events around the march launches of the timed steps); peak = register-resident "
-                        "DFMA rate measured in this process: the larger of a best-of-3 burst (11 ms) and a 2 s sustained run",
-                "peak_kind": peak_kind, "peak_burst": peak_burst, "peak_sustained": peak_sustained,
-                "min_work_context": {"fp64_instr_per_unit": MIN_WORK_FP64_INSTR_PER_UNIT,
-                                     "tflops": 2.0 * MIN_WORK_FP64_INSTR_PER_UNIT * u_all / (mk_ms * 1e-3) / 1e12,
-                                     "frac": 2.0 * MIN_WORK_FP64_INSTR_PER_UNIT * u_all / (mk_ms * 1e-3) / 1e12 / peak,
-                                     "note": "FP64 instructions if T and every gamma-tilde were evaluated once; the kernel re-evaluates "
-                                             "them on purpose (bytes cost more watts than instructions under the 1 kW cap)"},
-                "textbook_count_context": {"fp64_instr_per_unit": TEXTBOOK_FP64_INSTR_PER_UNIT,
-                                           "tflops": 2.0 * TEXTBOOK_FP64_INSTR_PER_UNIT * u_all / (mk_ms * 1e-3) / 1e12},
-                "march_ms": mk_ms, "march_share_of_step": mk_ms / (ms / a.steps),
-                "algo_fp64_instr_per_unit": instr / max(u_all, 1.0), "units_per_launch": u_all,
-                "units_share_stored_T": u_st / max(u_all, 1.0), "units_share_recompute_pole_table": u_pl / max(u_all, 1.0),
-                "hbm_bytes_per_unit_algorithmic": hbm / max(u_all, 1.0),
-                "hbm_gbs_algorithmic": hbm / (mk_ms * 1e-3) / 1e9}
-
-    # end to end through the C ABI with HOST buffers: H2D of Delta, A_ind; iterate; D2H of Delta, A_ind + stats
+    # end to end through the C ABI with HOST buffers, continuing on the same stationary part of the run: every step copies
+    # Delta and A_ind from pinned host memory, iterates, and copies Delta, A_ind and the residuals back
     hd = torch.empty((wl.ny, wl.nx), dtype=torch.complex128).pin_memory(); hd.copy_(delta)
     hax = torch.zeros((wl.ny, wl.nx), dtype=torch.float64).pin_memory(); hay = torch.zeros_like(hax).pin_memory()
     hax.copy_(aix); hay.copy_(aiy)
     torch.cuda.synchronize()
-    t0 = time.perf_counter()
-    for _ in range(a.steps):
-        delta.copy_(hd, non_blocking=True); aix.copy_(hax, non_blocking=True); aiy.copy_(hay, non_blocking=True)
-        st2 = ctx.sc_iterate(acc, 1.0, False, delta, aix, aiy, want_stats=True)
-        hd.copy_(delta, non_blocking=True); hax.copy_(aix, non_blocking=True); hay.copy_(aiy, non_blocking=True)
-        torch.cuda.synchronize()
-    e2e_s = (time.perf_counter() - t0) / a.steps
-    if world > 1:
-        tmax = torch.tensor([e2e_s], dtype=torch.float64, device=devname)
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        e2e_s = float(tmax.item())
-    bytes_io = ng * 16 + 2 * ng * 8
-
-    # configs[4]: "... FP64, with an FP32 mode also timed": the same step with opts.precision = 32 (same inputs, same
-    # warm-up and step counts), reported beside the FP64 headline, never instead of it
-    fp32_leg = None
-    if a.precision == 64 and wl.cfg == 4 and not a.no_fp32_leg and not a.sweep_only:
-        ctx.close(); del ctx
-        torch.cuda.empty_cache()
-        c32 = sc.ScContext.from_workload(wl, device=local, stepper=a.stepper, precision=32)
-        if world > 1:
-            from paper_2205_15000_b200 import sharding
-            sharding.attach(c32, wl.t, wl.n_energies)
-        c32.sc_set_external_field(dev_ax, dev_ay)
-        d32 = dev(wl.delta0.astype(np.complex128)); ax32 = torch.zeros_like(aix); ay32 = torch.zeros_like(aix)
-        for _ in range(max(a.warmup, 3)):
-            c32.sc_iterate(acc, 1.0, False, d32, ax32, ay32)
-        torch.cuda.synchronize()
+    e2e = None
+    if not a.sweep_only:
         if world > 1:
             dist.barrier()
-        f0 = torch.cuda.Event(enable_timing=True); f1 = torch.cuda.Event(enable_timing=True)
-        c32.sc_debug_march_time()
-        f0.record()
+        ctx.sc_debug_march_units()
+        t0 = time.perf_counter()
         for _ in range(a.steps):
-            c32.sc_iterate(acc, 1.0, False, d32, ax32, ay32)
-        f1.record(); torch.cuda.synchronize()
-        ms32 = f0.elapsed_time(f1)
+            delta.copy_(hd, non_blocking=True); aix.copy_(hax, non_blocking=True); aiy.copy_(hay, non_blocking=True)
+            st2 = ctx.sc_iterate(acc, 1.0, False, delta, aix, aiy, want_stats=True)
+            hd.copy_(delta, non_blocking=True); hax.copy_(aix, non_blocking=True); hay.copy_(aiy, non_blocking=True)
+            torch.cuda.synchronize()
+        e2e_s = (time.perf_counter() - t0) / a.steps
+        ue = ctx.sc_debug_march_units()
         if world > 1:
-            tmax = torch.tensor([ms32], dtype=torch.float64, device=devname)
+            tmax = torch.tensor([e2e_s], dtype=torch.float64, device=devname)
             dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-            ms32 = float(tmax.item())
-        fp32_leg = {"dtype": "f32", "value": n_updates * a.steps / (ms32 * 1e-3), "unit": UNIT, "ms_per_step": ms32 / a.steps,
-                    "march_ms": c32.sc_debug_march_time()[0] / a.steps}
-        c32.close()
+            e2e_s = float(tmax.item())
+        e2e = {"s_per_step": e2e_s, "res_delta_last": st2.res_delta, "bytes": ng * 16 + 2 * ng * 8,
+               "units_share_stored_T": ue[1] / max(ue[0], 1), "units_share_recompute_pole_table": ue[2] / max(ue[0], 1)}
 
+    # logical / executed update counts of one sweep (one extra sweep with stats, outside the timed regions)
+    ctx.sc_set_fields(delta, dev_ax + aix, dev_ay + aiy)
+    st = ctx.sc_riccati_sweep(dn, jx, jy, fe, want_stats=True)
+    n_updates, n_exec = st.n_updates, st.n_updates_executed
+    if world > 1:
+        tot = torch.tensor([n_updates, n_exec], dtype=torch.float64, device=devname)
+        dist.all_reduce(tot)
+        n_updates, n_exec = int(tot[0].item()), int(tot[1].item())
+    roof = march_roofline(a, wl, ctx, kernel, mk_ms, nl, units, ms / a.steps, precision, full_size, clocks)
+    ctx.close()
+    del ctx
+    torch.cuda.empty_cache()
+    return dict(ms=ms, clocks=clocks, launches=launches, roofline=roof, e2e=e2e, n_updates=n_updates, n_exec=n_exec, transient=transient)
+
+
+def ldos_leg(sc, torch, local, steps):
+    """sc_ldos on configs[3] (d-wave [110] square, 512 real energies, 128 angles): 8 boundary sweeps + the LDOS sweep"""
+    wl = workloads.make_workload(3)
+    devname = f"cuda:{local}"
+    ctx = sc.ScContext.from_workload(wl, device=local)
+    ctx.sc_set_fields(torch.as_tensor(np.ascontiguousarray(wl.delta0.astype(np.complex128)), device=devname))
+    out = torch.zeros((len(wl.ldos_energies), wl.ny, wl.nx), dtype=torch.float64, device=devname)
+    iters = 8
+    st = ctx.sc_ldos(wl.ldos_energies, wl.ldos_broadening, iters, out, want_stats=True)        # warm-up (allocations, tables)
+    torch.cuda.synchronize()
+    ctx.sc_debug_march_time(); ctx.sc_debug_launch_count()
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        ctx.sc_ldos(wl.ldos_energies, wl.ldos_broadening, iters, out)
+    e1.record(); torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    mms, nl = ctx.sc_debug_march_time()
+    launches = ctx.sc_debug_launch_count()
+    kernel = ctx.sc_debug_last_march_variant()
+    ok = bool(torch.isfinite(out).all().item()) and bool((out[:, torch.as_tensor(wl.mask > 0, device=devname)] > 0).all().item())
+    ctx.close()
+    return {"workload": f"BASELINE.json configs[3]: {wl.name}", "grid": f"{wl.nx}x{wl.ny}", "n_angles": wl.n_angles,
+            "n_energies": len(wl.ldos_energies), "boundary_sweeps": iters, "dtype": "f64",
+            "value": st.n_updates / (ms * 1e-3), "unit": UNIT, "s_per_call": ms * 1e-3, "updates_per_call": st.n_updates,
+            "march_ms_per_call": mms / steps, "march_launches_per_call": nl / steps, "gpu_launches_per_call": launches / steps,
+            "last_march_kernel": "sck::" + kernel, "ldos_positive_and_finite": ok,
+            "note": "general (off-axis) energies: complex Taylor table of T (Horner, 4 instructions per term); boundary sweeps "
+                    "march for the end values only (MODE 2), the last sweep writes Re g per (node, energy) and is rotated back per energy"}
+
+
+def run_ours(a):
+    import torch
+    import torch.distributed as dist
+    import paper_2205_15000_b200 as sc
+
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    torch.cuda.set_device(local)
+    if a.ldos_only:
+        print(json.dumps({"metric": METRIC, "ldos": ldos_leg(sc, torch, local, a.steps)}))
+        return
+    wl = workload_from_args(a)
+    full_size = world == 1 and not (a.pts_per_xi or a.n_angles or a.n_energies or a.size_scale != 1.0)
+    burnin = a.burnin if a.burnin is not None else (12 if (wl.kappa > 0 and not a.sweep_only) else 0)
+    L = run_leg(a, sc, torch, dist, wl, local, world, a.precision, burnin, full_size)
+
+    # configs[4]: "... FP64, with an FP32 mode also timed": the same legs with opts.precision = 32, beside the headline
+    fp32 = None
+    if a.precision == 64 and wl.cfg == 4 and not a.no_fp32_leg and not a.sweep_only:
+        F = run_leg(a, sc, torch, dist, wl, local, world, 32, burnin, full_size)
+        fp32 = {"dtype": "f32", "value": F["n_updates"] * a.steps / (F["ms"] * 1e-3), "unit": UNIT, "ms_per_step": F["ms"] / a.steps,
+                "e2e_value": F["n_updates"] / F["e2e"]["s_per_step"], "clocks": F["clocks"], "roofline": F["roofline"]}
+    ldos = None
+    if full_size and wl.cfg == 4 and a.precision == 64 and not a.no_ldos_leg and not a.sweep_only and rank == 0:
+        ldos = ldos_leg(sc, torch, local, max(1, min(a.steps, 2)))
+
+    ms, n_updates = L["ms"], L["n_updates"]
     value = n_updates * a.steps / (ms * 1e-3)
+    cfg = config_of(wl, a, {"seconds_per_self_consistent_iteration": ms / a.steps / 1e3,
+                            "updates_per_step": n_updates, "updates_executed_per_step": L["n_exec"],
+                            "updates_counted": "LOGICAL updates (gamma and gamma-tilde, every angle, every energy, every piece: the metric's "
+                                               "unit and what the CPU oracle executes); the kernel executes half of them, Eq. 13 gives the rest",
+                            "value_executed_updates_per_s": L["n_exec"] * a.steps / (ms * 1e-3),
+                            "stepper": "closed-form" if a.stepper == 0 else "implicit mid-point",
+                            "parallelism": f"energy-sharded x{world}, 1 all-reduce/sweep" if world > 1 else "single GPU",
+                            "burnin_iterations": burnin,
+                            "timed_state": "iterations after the Barzilai-Borwein transient of A_ind (stationary cost per iteration); "
+                                           "the e2e steps follow the timed ones on the same part of the run",
+                            "transient": L["transient"]})
+    if a.sweep_only:
+        cfg["step"] = "one sc_riccati_sweep at the initial fields (A = A_ext)"
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": max(a.warmup, 3),
             "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
-            "dtype": "f64" if a.precision == 64 else "f32",
-            "data": "synthetic", "config": config_of(wl, a, {"seconds_per_self_consistent_iteration": ms / a.steps / 1e3,
-                                                             "updates_per_step": n_updates, "updates_executed_per_step": n_exec,
-                                                             "stepper": "closed-form" if a.stepper == 0 else "implicit mid-point",
-                                                             "parallelism": f"energy-sharded x{world}, 1 all-reduce/sweep" if world > 1 else "single GPU"}),
-            "clocks": clocks,
-            "e2e": {"value": n_updates / e2e_s, "unit": UNIT, "h2d_bytes_per_step": bytes_io, "d2h_bytes_per_step": bytes_io + 64,
-                    "res_delta_last": st2.res_delta,
-                    "note": "the e2e steps continue the same self-consistency run (iterations after the timed ones): as the "
-                            "Barzilai-Borwein transient of A_ind decays more rounds take the cheaper table tiers, so a step here "
-                            "can be faster than a timed one although it also pays the host copies"},
-            "gpu_launches": gpu_launches, "roofline": roofline}
-    if fp32_leg:
-        line["config"]["fp32_mode"] = fp32_leg
+            "dtype": "f64" if a.precision == 64 else "f32", "data": "synthetic", "config": cfg, "clocks": L["clocks"],
+            "gpu_launches": L["launches"], "roofline": L["roofline"]}
+    if L["e2e"]:
+        e = L["e2e"]
+        line["e2e"] = {"value": n_updates / e["s_per_step"], "unit": UNIT, "h2d_bytes_per_step": e["bytes"], "d2h_bytes_per_step": e["bytes"] + 64,
+                       "s_per_step": e["s_per_step"], "res_delta_last": e["res_delta_last"],
+                       "units_share_stored_T": e["units_share_stored_T"], "units_share_recompute_pole_table": e["units_share_recompute_pole_table"]}
+    if fp32:
+        line["config"]["fp32_mode"] = fp32
+    if ldos:
+        line["config"]["ldos"] = ldos
+    if rank == 0:
+        try:
+            line["roofline"]["textbook_count_context"] = textbook_count()
+        except Exception as ex:       # the oracle is test infrastructure: its absence must not break the bench
+            line["roofline"]["textbook_count_context"] = {"unavailable": str(ex)}
     if not a.no_cpu_baseline and rank == 0:
         cores = os.cpu_count() or 1
         u, t, desc = oracle_sample(wl, cores)
-        line["cpu_baseline"] = {"value": u / t, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+        line["cpu_baseline"] = {"value": u / t, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc, "note": CPU_NOTE}
     if rank == 0:
         print(json.dumps(line))
     if world > 1:

@@ -63,10 +63,12 @@ typedef struct {
     double crystal_rotation; /* rotation of the crystal axes in full turns (:890) */
     int device;          /* CUDA device ordinal */
     void* cuda_stream;   /* cudaStream_t; NULL = default stream */
+    int residual_norm;   /* p of the residual norms of Eq. 27 (:201; "norm" in :960): 2 (0 = default), 1, or -1 = maximum norm.
+                          * One element is one complex Delta_G(R), one vector A(R) or j(R), or one real I(R). */
 } sc_opts;
 
 typedef struct {
-    double res_delta, res_j, res_A, res_fe;   /* Eq. 27 (:201), 2-norm; filled by sc_iterate */
+    double res_delta, res_j, res_A, res_fe;   /* Eq. 27 (:201) in the norm opts.residual_norm; filled by sc_iterate */
     double min_one_minus_abs_gamma;           /* min over nodes of 1 - max(|gamma|,|gamma~|) (invariant |gamma| < 1) */
     long long n_updates;                      /* logical trajectory-step updates of the sweep: 2 * N_phi * N_eps * sum_t pieces */
     long long n_updates_executed;             /* steps actually marched (Eq. 13 symmetry halves them) */
@@ -194,6 +196,11 @@ sc_status sc_debug_fp64_peak(sc_ctx* ctx, double* dfma_per_s, double* sm_clock_m
 /* The same microbenchmark launched back to back for `seconds` (<= 30), rate of the second half: what the FP64 pipe
  * sustains once the part sits at its power limit (the march runs for seconds at a time). */
 sc_status sc_debug_fp64_peak_sustained(sc_ctx* ctx, double seconds, double* dfma_per_s);
+/* The same kind of register-resident loop for the other pipes the march uses, held for `seconds` (<= 30): pipe 1 = fp32
+ * FMA (FFMA; roofline denominator of opts.precision = 32), 2 = MUFU.RCP (fp32 reciprocal seed), 3 = MUFU.RCP64H (fp64
+ * reciprocal seed) — the special-function issue rate north_star asks about.  ops_per_s counts thread-level
+ * instructions per second over the whole device. */
+sc_status sc_debug_pipe_peak(sc_ctx* ctx, int pipe, double seconds, double* ops_per_s);
 
 /* Device time of the most recent march kernel launch (CUDA events recorded on the stream around that launch
  * alone); synchronises.  Used by bench.py for the roofline of the dominant kernel. */

@@ -452,8 +452,8 @@ class Driver:
     """Algorithm 1 (:203-205): sweep -> A-solve -> accelerator on x = (Re Delta, Im Delta, kappa^2 A_x^ind,
     kappa^2 A_y^ind) (E3 :1053) -> residual (Eq. 27 :201).  `accelerator` and the keyword parameters are Accelerator's."""
 
-    def __init__(self, orc: Oracle, Aext_x, Aext_y, ne, accelerator=0, step=1.0, **kw):
-        self.o, self.ne = orc, ne
+    def __init__(self, orc: Oracle, Aext_x, Aext_y, ne, accelerator=0, step=1.0, norm=2, **kw):
+        self.o, self.ne, self.norm = orc, ne, norm            # norm: p of Eq. 27 (:201; :960 "norm"): 1, 2, or 0 = maximum norm
         self.accel = Accelerator(accelerator, step, ncomp=4, **kw)
         self.Aext = (np.asarray(Aext_x, np.float64), np.asarray(Aext_y, np.float64))
         self.stores = None
@@ -493,7 +493,9 @@ class Driver:
             out["Aind_x"] = (xn[2 * nc * n:(2 * nc + 1) * n] / k2).reshape(shp); out["Aind_y"] = (xn[(2 * nc + 1) * n:] / k2).reshape(shp)
         else:
             out["Aind_x"], out["Aind_y"] = Aind_x, Aind_y
-        out["res_delta"] = residual(out["delta"], delta)
+        out["res_delta"] = residual(out["delta"], delta, self.norm)
+        if o.kappa > 0:       # one element of a vector field is the 2-vector at a grid point: |A| = |A_x + i A_y|
+            out["res_A"] = residual(out["Aind_x"] + 1j * out["Aind_y"], Aind_x + 1j * Aind_y, self.norm)
         out["alpha"] = self.accel.alpha if self.accel.kind != 3 else list(self.accel.alpha_c)
         out["w"] = list(self.accel.w_c)
         return out

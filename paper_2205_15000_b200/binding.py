@@ -36,7 +36,8 @@ class _Shape(C.Structure):
 class _Opts(C.Structure):
     _fields_ = [("n_angles", C.c_int), ("n_matsubara", C.c_int), ("precision", C.c_int), ("stepper", C.c_int),
                 ("quadrature", C.c_int), ("charge_sign", C.c_int), ("bc_mode", C.c_int),
-                ("crystal_rotation", C.c_double), ("device", C.c_int), ("cuda_stream", C.c_void_p)]
+                ("crystal_rotation", C.c_double), ("device", C.c_int), ("cuda_stream", C.c_void_p),
+                ("residual_norm", C.c_int)]
 
 
 class _Stats(C.Structure):
@@ -112,6 +113,7 @@ def load_library():
     L.sc_debug_fp64_peak.argtypes = [vp, C.POINTER(d), C.POINTER(d)]
     L.sc_debug_last_march_ms.argtypes = [vp, C.POINTER(C.c_float)]
     L.sc_debug_fp64_peak_sustained.argtypes = [vp, d, C.POINTER(d)]
+    L.sc_debug_pipe_peak.argtypes = [vp, i, d, C.POINTER(d)]
     L.sc_debug_march_time.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(i)]
     L.sc_debug_march_units.argtypes = [vp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
     L.sc_debug_last_march_variant.argtypes = [vp, C.c_char_p, i]
@@ -142,7 +144,8 @@ class ScContext:
     def __init__(self, nx: int, ny: int, h: float, mask: np.ndarray, shapes: Sequence, t: float, kappa: float,
                  symmetry: int, n_angles: int, n_matsubara: int, *, crystal_rotation: float = 0.0,
                  quadrature: int = 0, charge_sign: int = -1, bc_mode: int = 0, precision: int = 64,
-                 stepper: int = 0, device: int = 0, stream: Optional[int] = None, tables_only: bool = False):
+                 stepper: int = 0, device: int = 0, stream: Optional[int] = None, tables_only: bool = False,
+                 residual_norm: int = 2):
         """tables_only=True keeps a context whose sc_create stopped at SC_ERR_CUDA (no device) so that the host-built
         trajectory tables can still be read with sc_debug_tables; every compute call on it fails."""
         import torch
@@ -165,7 +168,7 @@ class ScContext:
         if stream is None:
             stream = torch.cuda.current_stream(self.device).cuda_stream if torch.cuda.is_available() else 0
         opts = _Opts(n_angles, n_matsubara, precision, stepper, quadrature, charge_sign, bc_mode, crystal_rotation,
-                     device, C.c_void_p(stream))
+                     device, C.c_void_p(stream), residual_norm)
         grid = _Grid(nx, ny, h)
         h_ = C.c_void_p()
         rc = L.sc_create(C.byref(grid), mask.ctypes.data_as(C.c_void_p), arr, len(shapes), t, kappa, symmetry,
@@ -350,6 +353,11 @@ class ScContext:
     def sc_debug_fp64_peak_sustained(self, seconds=2.0):
         a = C.c_double()
         self._check(self._L.sc_debug_fp64_peak_sustained(self._h, float(seconds), C.byref(a)))
+        return a.value
+
+    def sc_debug_pipe_peak(self, pipe, seconds=1.0):
+        a = C.c_double()
+        self._check(self._L.sc_debug_pipe_peak(self._h, int(pipe), float(seconds), C.byref(a)))
         return a.value
 
     def sc_debug_fp64_peak(self):

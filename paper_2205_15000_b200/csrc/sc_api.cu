@@ -156,6 +156,9 @@ struct sc_ctx {
     // Eq. 22 denominator sum (sum_n w_n t / eps_n over the WHOLE job's energy table) and the energy-shard hook
     double denom_sum = 0.0;
     double* hook_acc = nullptr; sc_allreduce_fn hook_fn = nullptr; void* hook_user = nullptr;
+    // sc_ldos: energy table, boundary stores, per-node Re g window and work lists stay alive after the call returns
+    // (the call only enqueues); they are re-used by the next sc_ldos and freed by sc_destroy
+    EnergySet ldos_E; DevBuf<char> ldos_st[2]; DevBuf<double> ldos_ldn; DevBuf<int> ldos_items, ldos_out_idx;
     // vector potential / driver state
     scf::FieldState fs;
 };
@@ -337,6 +340,8 @@ sc_status sc_create(const sc_grid* grid, const unsigned char* mask, const sc_sha
     if (opts->n_matsubara < 1) return fail(ctx, SC_ERR_ARG, "n_matsubara < 1");
     if (opts->precision != 64 && opts->precision != 32 && opts->precision != 0) return fail(ctx, SC_ERR_ARG, "precision must be 64 or 32");
     if (opts->stepper != 0 && opts->stepper != 1) return fail(ctx, SC_ERR_ARG, "stepper must be 0 (closed form) or 1 (implicit mid-point)");
+    if (opts->residual_norm != 0 && opts->residual_norm != 2 && opts->residual_norm != 1 && opts->residual_norm != -1)
+        return fail(ctx, SC_ERR_ARG, "residual_norm must be 2 (or 0), 1, or -1 (maximum norm)");
     ctx->opt = *opts; ctx->grid = *grid; ctx->t = T_over_Tc; ctx->kappa = kappa; ctx->sym = (int)symmetry;
     ctx->ncomp = 1; ctx->syms[0] = (int)symmetry; ctx->tc_ratio[0] = 1.0;
     ctx->f32 = opts->precision == 32;
@@ -598,7 +603,9 @@ sc_status sc_ldos(sc_ctx* ctx, const double* energies, int n_e, double broadenin
     CU(cudaMemsetAsync(ctx->d_nbad.p + 1, 0, sizeof(int), ctx->stream));
     if (sc_status st = ensure_nodes(ctx)) return st;
     // internal energy list closed under eps -> -eps (gamma-tilde_k(eps) = conj gamma_{k+N/2}(-eps), Eq. 13 :95)
-    EnergySet E;
+    CU(cudaStreamSynchronize(ctx->stream));       // an earlier sc_ldos may still be reading the tables replaced below
+    EnergySet& E = ctx->ldos_E;
+    E.zr.clear(); E.zi.clear(); E.w.clear();
     std::vector<int> out_idx(n_e);
     for (int m = 0; m < n_e; ++m) { E.zr.push_back(energies[m]); E.zi.push_back(broadening); E.w.push_back(1.0); out_idx[m] = m; }
     E.partner.assign(n_e, -1);
@@ -613,46 +620,51 @@ sc_status sc_ldos(sc_ctx* ctx, const double* energies, int n_e, double broadenin
     }
     if (sc_status st = upload_energies(ctx, E)) return st;
     const int ND = (int)ctx->geo.dt.size();
-    DevBuf<char> st0, st1;
-    CU(st0.alloc((size_t)ND * E.ne * 2 * ctx->rsz())); CU(st1.alloc((size_t)ND * E.ne * 2 * ctx->rsz()));
-    if (sc_status st = reset_stores(ctx, E, st0.p)) return st;
-    char* so = st0.p; char* sn = st1.p;
+    const size_t store_bytes = (size_t)ND * E.ne * 2 * ctx->rsz();
+    for (auto& b : ctx->ldos_st) if (b.n < store_bytes) CU(b.alloc(store_bytes));
+    if (sc_status st = reset_stores(ctx, E, ctx->ldos_st[0].p)) return st;
+    char* so = ctx->ldos_st[0].p; char* sn = ctx->ldos_st[1].p;
     for (int it = 0; it + 1 < n_boundary_iters; ++it) {
         if (sc_status st = launch_march<2>(ctx, E, so, sn, false)) return st;
         std::swap(so, sn);
     }
-    // last sweep: per-energy Re g at every node, in batches of angle pairs sized to the free memory
+    // last sweep: per-energy Re g at every node, in batches of angle pairs sized to the free memory.  Node offsets are
+    // pair-major, so the nodes of a batch are one contiguous window; all batches share one window buffer and run back to
+    // back on the stream (stream order keeps a batch's march behind the previous batch's rotate-back: no host sync).
     const int H = ctx->geo.nphi / 2;
     std::vector<long long> pair_nodes(H + 1, 0);
     for (int g = 0; g < ctx->G; ++g) pair_nodes[ctx->h_k[g] + 1] += ctx->h_nn[g];
     for (int p = 0; p < H; ++p) pair_nodes[p + 1] += pair_nodes[p];
     size_t freeb = 0, totalb = 0; CU(cudaMemGetInfo(&freeb, &totalb));
-    const size_t budget = std::min<size_t>(freeb / 2, (size_t)48 << 30);
-    DevBuf<int> d_out_idx; CU(d_out_idx.upload(out_idx, ctx->stream));
-    // items are trajectory-sorted by length, not by pair: run the march over ALL pairs writing into a node
-    // window; windows are contiguous node ranges because node offsets are pair-major.
-    std::vector<int> item_by_pair(ctx->G); std::iota(item_by_pair.begin(), item_by_pair.end(), 0);
-    DevBuf<int> d_items; DevBuf<double> d_ldn;
-    int p0 = 0; bool first = true;
-    while (p0 < H) {
+    const size_t budget = std::max(ctx->ldos_ldn.n * sizeof(double), std::min<size_t>(freeb / 2, (size_t)48 << 30));
+    std::vector<int> bounds{0};
+    long long win_max = 0;
+    for (int p0 = 0; p0 < H;) {
         int p1 = p0 + 1;
         while (p1 < H && (size_t)(pair_nodes[p1 + 1] - pair_nodes[p0]) * E.ne * sizeof(double) <= budget) ++p1;
-        const long long nwin = pair_nodes[p1] - pair_nodes[p0];
-        CU(d_ldn.alloc((size_t)nwin * E.ne));
-        std::vector<int> items;
-        for (int g : ctx->h_order) if (ctx->h_k[g] >= p0 && ctx->h_k[g] < p1) items.push_back(g);
-        CU(d_items.upload(items, ctx->stream));
-        double* const ldn = d_ldn.p - (size_t)pair_nodes[p0] * E.ne;       // node offsets are global
-        if (sc_status st = launch_march<1>(ctx, E, so, sn, false, d_items.p, (int)items.size(), ldn)) return st;
+        win_max = std::max(win_max, pair_nodes[p1] - pair_nodes[p0]);
+        bounds.push_back(p1); p0 = p1;
+    }
+    if (ctx->ldos_ldn.n < (size_t)win_max * E.ne) CU(ctx->ldos_ldn.alloc((size_t)win_max * E.ne));
+    // work lists of all batches, each longest-first, concatenated
+    std::vector<int> items; std::vector<int> item_off{0};
+    for (size_t b = 0; b + 1 < bounds.size(); ++b) {
+        for (int g : ctx->h_order) if (ctx->h_k[g] >= bounds[b] && ctx->h_k[g] < bounds[b + 1]) items.push_back(g);
+        item_off.push_back((int)items.size());
+    }
+    CU(ctx->ldos_items.upload(items, ctx->stream)); CU(ctx->ldos_out_idx.upload(out_idx, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));       // `items` / `out_idx` are stack-owned host vectors
+    for (size_t b = 0; b + 1 < bounds.size(); ++b) {
+        const int p0 = bounds[b], p1 = bounds[b + 1];
+        double* const ldn = ctx->ldos_ldn.p - (size_t)pair_nodes[p0] * E.ne;       // node offsets are global
+        if (sc_status st = launch_march<1>(ctx, E, so, sn, false, ctx->ldos_items.p + item_off[b], item_off[b + 1] - item_off[b], ldn)) return st;
         sck::BackLdosArgs L{};
         L.B = back_args(ctx, nullptr, nullptr, nullptr, nullptr);
-        L.ne_out = n_e; L.out_idx = d_out_idx.p; L.partner = E.d_partner.p; L.ne = E.ne;
-        L.ldos_nodes = ldn; L.out = ldos; L.p0 = p0; L.p1 = p1; L.accumulate = first ? 0 : 1;
+        L.ne_out = n_e; L.out_idx = ctx->ldos_out_idx.p; L.partner = E.d_partner.p; L.ne = E.ne;
+        L.ldos_nodes = ldn; L.out = ldos; L.p0 = p0; L.p1 = p1; L.accumulate = b ? 1 : 0;
         dim3 grd((n_e + 63) / 64, ctx->grid.nx, ctx->grid.ny);
         ++sck::g_launches, sck::rotate_back_ldos_kernel<<<grd, 64, 0, ctx->stream>>>(L);
         CU(cudaGetLastError());
-        CU(cudaStreamSynchronize(ctx->stream));     // d_ldn / d_items are re-used by the next batch
-        first = false; p0 = p1;
     }
     sc_status r = fill_stats(ctx, stats, E.ne, false);
     if (stats) { stats->n_updates *= n_boundary_iters; stats->n_updates_executed *= n_boundary_iters; }
@@ -704,7 +716,7 @@ sc_status sc_iterate(sc_ctx* ctx, int accelerator, double step, int burnin, void
             if (int rc = scf::vector_potential(F, nx, ny, ctx->grid.h, ctx->d_mask.p, ctx->kappa, F.jx, F.jy, F.gAx, F.gAy, nullptr, ctx->stream, e))
                 return fail(ctx, rc == 2 ? SC_ERR_NOMEM : SC_ERR_CUDA, e);
         }
-        if (int rc = scf::mix(F, accelerator, step, ctx->kappa, withA, (double2*)delta_inout, Aix, Aiy, ctx->d_mask.p, ng, ctx->stream, e))
+        if (int rc = scf::mix(F, accelerator, step, ctx->kappa, withA, (double2*)delta_inout, Aix, Aiy, ctx->d_mask.p, ng, ctx->opt.residual_norm, ctx->stream, e))
             return fail(ctx, SC_ERR_CUDA, e);
     }
     if (stats) {
@@ -950,6 +962,37 @@ sc_status sc_debug_fp64_peak_sustained(sc_ctx* ctx, double seconds, double* dfma
     CU(cudaEventSynchronize(ctx->ev1));
     float ms = 0; CU(cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1));
     *dfma_per_s = (double)(n - n / 2) * blocks * threads * (double)iters * 64.0 / (ms * 1e-3);
+    return SC_OK;
+}
+
+sc_status sc_debug_pipe_peak(sc_ctx* ctx, int pipe, double seconds, double* ops_per_s) {
+    if (!ctx || !ops_per_s || pipe < 1 || pipe > 3 || !(seconds > 0) || seconds > 30) return fail(ctx, SC_ERR_ARG, "bad argument");
+    ON_DEVICE(ctx);
+    DevBuf<float> d; CU(d.alloc(1));
+    const int blocks = ctx->n_sm * 4, threads = 256;
+    const int iters = pipe == 1 ? 20000 : 2000;
+    const double per_thread = (double)iters * 64.0;       // 8 chains x 8 per loop body, in both kernels
+    auto launch = [&]() {
+        ++sck::g_launches;
+        if (pipe == 1) sck::fp32_peak_kernel<<<blocks, threads, 0, ctx->stream>>>(iters, d.p);
+        else if (pipe == 2) sck::mufu_peak_kernel<false><<<blocks, threads, 0, ctx->stream>>>(iters, d.p);
+        else sck::mufu_peak_kernel<true><<<blocks, threads, 0, ctx->stream>>>(iters, d.p);
+    };
+    launch();
+    CU(cudaEventRecord(ctx->ev0, ctx->stream));
+    launch();
+    CU(cudaEventRecord(ctx->ev1, ctx->stream));
+    CU(cudaEventSynchronize(ctx->ev1));
+    float one = 0; CU(cudaEventElapsedTime(&one, ctx->ev0, ctx->ev1));
+    const int n = std::max(4, (int)(seconds * 1e3 / std::max(one, 1e-3f)));
+    for (int i = 0; i < n / 2; ++i) launch();                                    // reach the steady clock
+    CU(cudaEventRecord(ctx->ev0, ctx->stream));
+    for (int i = 0; i < n - n / 2; ++i) launch();
+    CU(cudaEventRecord(ctx->ev1, ctx->stream));
+    CU(cudaEventSynchronize(ctx->ev1));
+    CU(cudaGetLastError());
+    float ms = 0; CU(cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1));
+    *ops_per_s = (double)(n - n / 2) * blocks * threads * per_thread / (ms * 1e-3);
     return SC_OK;
 }
 

@@ -69,24 +69,31 @@ inline void release(FieldState& F) {
 }
 
 // ---- deterministic reductions --------------------------------------------------------------------
-template <typename Op>
+// MAXR: maximum of non-negative terms instead of their sum (max-norm residuals)
+template <typename Op, bool MAXR = false>
 __global__ void reduce_stage1(size_t n, Op op, double* partial, int nout) {
     __shared__ double sh[RED_THREADS];
     for (int c = 0; c < nout; ++c) {
         double s = 0.0;
-        for (size_t i = (size_t)blockIdx.x * RED_THREADS + threadIdx.x; i < n; i += (size_t)RED_BLOCKS * RED_THREADS) s += op(i, c);
+        for (size_t i = (size_t)blockIdx.x * RED_THREADS + threadIdx.x; i < n; i += (size_t)RED_BLOCKS * RED_THREADS) {
+            if (MAXR) s = fmax(s, op(i, c)); else s += op(i, c);
+        }
         sh[threadIdx.x] = s;
         __syncthreads();
-        for (int o = RED_THREADS / 2; o; o >>= 1) { if (threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o]; __syncthreads(); }
+        for (int o = RED_THREADS / 2; o; o >>= 1) {
+            if (threadIdx.x < o) sh[threadIdx.x] = MAXR ? fmax(sh[threadIdx.x], sh[threadIdx.x + o]) : sh[threadIdx.x] + sh[threadIdx.x + o];
+            __syncthreads();
+        }
         if (threadIdx.x == 0) partial[(size_t)c * RED_BLOCKS + blockIdx.x] = sh[0];
         __syncthreads();
     }
 }
+template <bool MAXR = false>
 __global__ void reduce_stage2(const double* partial, int nout, double* out) {
     const int c = threadIdx.x;
     if (c >= nout) return;
     double s = 0.0;
-    for (int b = 0; b < RED_BLOCKS; ++b) s += partial[(size_t)c * RED_BLOCKS + b];
+    for (int b = 0; b < RED_BLOCKS; ++b) s = MAXR ? fmax(s, partial[(size_t)c * RED_BLOCKS + b]) : s + partial[(size_t)c * RED_BLOCKS + b];
     out[c] = s;
 }
 
@@ -182,7 +189,7 @@ inline int vector_potential(FieldState& F, int nx, int ny, double h, const unsig
     const int px = 2 * nx, py = 2 * ny; const size_t nspec = (size_t)py * (px / 2 + 1);
     double* res = F.red + RED_RES;
     ++sck::g_launches, reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, MeanOp{mask, jx, jy}, F.red, 3);
-    ++sck::g_launches, reduce_stage2<<<1, 32, 0, s>>>(F.red, 3, res);
+    ++sck::g_launches, reduce_stage2<false><<<1, 32, 0, s>>>(F.red, 3, res);
     ++sck::g_launches, mean_finish_kernel<<<1, 1, 0, s>>>(res);
     if (F.vp_eps > 0.0) {      // the paper's truncated eigen-decomposition (D7-D9) instead of the exact correlation
         if (!F.lr) F.lr = new LowRank();
@@ -205,7 +212,7 @@ inline int vector_potential(FieldState& F, int nx, int ny, double h, const unsig
     SCF_CU(cudaGetLastError());
     if (fe_mag) {
         ++sck::g_launches, reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, FemagOp{mask, jx, jy, Ax, Ay}, F.red, 1);
-        ++sck::g_launches, reduce_stage2<<<1, 32, 0, s>>>(F.red, 1, res + 4);
+        ++sck::g_launches, reduce_stage2<false><<<1, 32, 0, s>>>(F.red, 1, res + 4);
         double v = 0; SCF_CU(cudaMemcpyAsync(&v, res + 4, sizeof(double), cudaMemcpyDeviceToHost, s));
         SCF_CU(cudaStreamSynchronize(s));
         *fe_mag = 0.5 * h * h * v;
@@ -315,30 +322,47 @@ __global__ void step_kernel(size_t ng, int nslice, int accelerator, const double
         aux[q] = m; upd[q] = state[ST_ALPHA + c] * m;
     } else upd[q] = state[0] * d[q];
 }
-struct NormOp {    // c: 0 |dx_delta|^2, 1 |x_delta|^2, 2 |dx_A|^2, 3 |x_A|^2 (before the update); delta = all components
+// Terms of the norms of Eq. 27 (:201; p in {1, 2, infinity}, :960).  One element of a field is one complex number
+// (Delta_G at a grid point) or one 2-vector (A, j at a grid point) or one real number (I); P2 = true gives |element|^2
+// (summed, root taken at the end), false |element| (summed for p = 1, maximised for p = infinity).
+template <bool P2> __device__ __forceinline__ double norm_term(double a, double b) { return P2 ? a * a + b * b : sqrt(a * a + b * b); }
+template <bool P2, bool MAXR> __device__ __forceinline__ double norm_join(double s, double v) { return MAXR ? fmax(s, v) : s + v; }
+template <bool P2, bool MAXR>
+struct NormOp {    // c: 0 dx_delta, 1 x_delta, 2 dx_A, 3 x_A (before the update); delta = all components
     size_t ng; int nc; const double2* delta; const double* aix; const double* aiy; const double* u; double k2; int withA;
     __device__ double operator()(size_t i, int c) const {
-        if (c == 0) { double s = 0.0; for (int g = 0; g < 2 * nc; ++g) s += u[g * ng + i] * u[g * ng + i]; return s; }
-        if (c == 1) { double s = 0.0; for (int g = 0; g < nc; ++g) s += delta[g * ng + i].x * delta[g * ng + i].x + delta[g * ng + i].y * delta[g * ng + i].y; return s; }
+        if (c == 0) { double s = 0.0; for (int g = 0; g < nc; ++g) s = norm_join<P2, MAXR>(s, norm_term<P2>(u[(2 * g) * ng + i], u[(2 * g + 1) * ng + i])); return s; }
+        if (c == 1) { double s = 0.0; for (int g = 0; g < nc; ++g) s = norm_join<P2, MAXR>(s, norm_term<P2>(delta[g * ng + i].x, delta[g * ng + i].y)); return s; }
         if (!withA) return 0.0;
-        if (c == 2) return (u[(2 * nc) * ng + i] * u[(2 * nc) * ng + i] + u[(2 * nc + 1) * ng + i] * u[(2 * nc + 1) * ng + i]) / (k2 * k2);
-        return aix[i] * aix[i] + aiy[i] * aiy[i];
+        if (c == 2) return norm_term<P2>(u[(2 * nc) * ng + i] / k2, u[(2 * nc + 1) * ng + i] / k2);
+        return norm_term<P2>(aix[i], aiy[i]);
     }
 };
-struct ObsNormOp {  // c: 0 |j - j_prev|^2, 1 |j_prev|^2, 2 |fe - fe_prev|^2, 3 |fe_prev|^2
+template <bool P2>
+struct ObsNormOp {  // c: 0 j - j_prev, 1 j_prev, 2 fe - fe_prev, 3 fe_prev
     const double *jx, *jy, *fe, *pjx, *pjy, *pfe;
     __device__ double operator()(size_t i, int c) const {
-        if (c == 0) return (jx[i] - pjx[i]) * (jx[i] - pjx[i]) + (jy[i] - pjy[i]) * (jy[i] - pjy[i]);
-        if (c == 1) return pjx[i] * pjx[i] + pjy[i] * pjy[i];
-        if (c == 2) return (fe[i] - pfe[i]) * (fe[i] - pfe[i]);
-        return pfe[i] * pfe[i];
+        if (c == 0) return norm_term<P2>(jx[i] - pjx[i], jy[i] - pjy[i]);
+        if (c == 1) return norm_term<P2>(pjx[i], pjy[i]);
+        if (c == 2) return norm_term<P2>(fe[i] - pfe[i], 0.0);
+        return norm_term<P2>(pfe[i], 0.0);
     }
 };
-__global__ void residual_kernel(double* state, const double* n1, const double* n2) {
-    state[2] = n1[1] > 0 ? sqrt(n1[0] / n1[1]) : sqrt(n1[0]);
-    state[3] = n1[3] > 0 ? sqrt(n1[2] / n1[3]) : sqrt(n1[2]);
-    state[4] = n2[1] > 0 ? sqrt(n2[0] / n2[1]) : sqrt(n2[0]);
-    state[5] = n2[3] > 0 ? sqrt(n2[2] / n2[3]) : sqrt(n2[2]);
+__global__ void residual_kernel(double* state, const double* n1, const double* n2, int p2) {
+    for (int q = 0; q < 4; ++q) {
+        const double* n = q < 2 ? n1 + 2 * q : n2 + 2 * (q - 2);
+        const double r = n[1] > 0 ? n[0] / n[1] : n[0];
+        state[2 + q] = p2 ? sqrt(r) : r;
+    }
+}
+template <bool P2, bool MAXR>
+inline void residual_norms(FieldState& F, size_t ng, int nc, const double2* delta, const double* aix, const double* aiy, double k2, bool withA, cudaStream_t s) {
+    double* res = F.red + RED_RES;
+    ++sck::g_launches, reduce_stage1<NormOp<P2, MAXR>, MAXR><<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, NormOp<P2, MAXR>{ng, nc, delta, aix, aiy, F.upd, k2 > 0 ? k2 : 1.0, withA ? 1 : 0}, F.red, 4);
+    ++sck::g_launches, reduce_stage2<MAXR><<<1, 32, 0, s>>>(F.red, 4, res + 4);
+    ++sck::g_launches, reduce_stage1<ObsNormOp<P2>, MAXR><<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, ObsNormOp<P2>{F.jx, F.jy, F.feI, F.prev_jx, F.prev_jy, F.prev_fe}, F.red, 4);
+    ++sck::g_launches, reduce_stage2<MAXR><<<1, 32, 0, s>>>(F.red, 4, res + 8);
+    ++sck::g_launches, residual_kernel<<<1, 1, 0, s>>>(F.state, res + 4, res + 8, P2 ? 1 : 0);
 }
 __global__ void update_kernel(size_t ng, int nc, double2* delta, double* aix, double* aiy, const double* u,
                               const unsigned char* mask, double k2, int withA) {
@@ -350,8 +374,9 @@ __global__ void update_kernel(size_t ng, int nc, double2* delta, double* aix, do
     if (withA) { aix[i] += u[(2 * nc) * ng + i] / k2; aiy[i] += u[(2 * nc + 1) * ng + i] / k2; }
 }
 
+// norm_p: the p of Eq. 27's residual norms: 2 (default), 1, or -1 for the maximum norm
 inline int mix(FieldState& F, int accelerator, double step, double kappa, bool withA, double2* delta, double* aix, double* aiy,
-               const unsigned char* mask, size_t ng, cudaStream_t s, std::string& err) {
+               const unsigned char* mask, size_t ng, int norm_p, cudaStream_t s, std::string& err) {
     const double k2 = withA ? kappa * kappa : 0.0;
     const int nc = F.nc, nslice = 2 * nc + 2;
     const size_t nxl = (size_t)nslice * ng;
@@ -365,20 +390,18 @@ inline int mix(FieldState& F, int accelerator, double step, double kappa, bool w
     ++sck::g_launches, diff_kernel<<<nb, 256, 0, s>>>(ng, nc, delta, F.dnew, aix, aiy, F.gAx, F.gAy, k2, withA ? 1 : 0, F.d_cur);
     if (!F.first && accelerator == 1) {
         ++sck::g_launches, reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(nxl, DotOp{F.d_cur, F.d_prev}, F.red, 3);
-        ++sck::g_launches, reduce_stage2<<<1, 32, 0, s>>>(F.red, 3, res);
+        ++sck::g_launches, reduce_stage2<false><<<1, 32, 0, s>>>(F.red, 3, res);
     }
     ++sck::g_launches, alpha_kernel<<<1, 1, 0, s>>>(F.state, res, accelerator, step, F.first ? 1 : 0, F.par);
     if (accelerator == 3) {
         ++sck::g_launches, reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, CongDotOp{ng, F.aux, F.d_cur}, F.red, 3 * nslice);
-        ++sck::g_launches, reduce_stage2<<<1, 32, 0, s>>>(F.red, 3 * nslice, res + 16);
+        ++sck::g_launches, reduce_stage2<false><<<1, 32, 0, s>>>(F.red, 3 * nslice, res + 16);
         ++sck::g_launches, congacc_kernel<<<1, 32, 0, s>>>(F.state, res + 16, nslice, F.par);
     }
     ++sck::g_launches, step_kernel<<<nbx, 256, 0, s>>>(ng, nslice, accelerator, F.d_cur, F.aux, F.state, F.par.drag, F.upd);
-    ++sck::g_launches, reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, NormOp{ng, nc, delta, aix, aiy, F.upd, k2, withA ? 1 : 0}, F.red, 4);
-    ++sck::g_launches, reduce_stage2<<<1, 32, 0, s>>>(F.red, 4, res + 4);
-    ++sck::g_launches, reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, s>>>(ng, ObsNormOp{F.jx, F.jy, F.feI, F.prev_jx, F.prev_jy, F.prev_fe}, F.red, 4);
-    ++sck::g_launches, reduce_stage2<<<1, 32, 0, s>>>(F.red, 4, res + 8);
-    ++sck::g_launches, residual_kernel<<<1, 1, 0, s>>>(F.state, res + 4, res + 8);
+    if (norm_p == 1) residual_norms<false, false>(F, ng, nc, delta, aix, aiy, k2, withA, s);
+    else if (norm_p < 0) residual_norms<false, true>(F, ng, nc, delta, aix, aiy, k2, withA, s);
+    else residual_norms<true, false>(F, ng, nc, delta, aix, aiy, k2, withA, s);
     ++sck::g_launches, update_kernel<<<nb, 256, 0, s>>>(ng, nc, delta, aix, aiy, F.upd, mask, k2 > 0 ? k2 : 1.0, withA ? 1 : 0);
     SCF_CU(cudaMemcpyAsync(F.prev_jx, F.jx, ng * sizeof(double), cudaMemcpyDeviceToDevice, s));
     SCF_CU(cudaMemcpyAsync(F.prev_jy, F.jy, ng * sizeof(double), cudaMemcpyDeviceToDevice, s));

@@ -1011,4 +1011,40 @@ __global__ void fp64_peak_kernel(int iters, double* sink) {
     if (s == 123.456) sink[0] = s;
 }
 
+// register-resident FFMA loop (fp32 pipe: the peak of the fp32 march), 8 independent chains per thread
+__global__ void fp32_peak_kernel(int iters, float* sink) {
+    float a0 = threadIdx.x * 1e-6f, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+    const float b = 0.9999f, c = 1e-4f;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            a0 = fmaf(a0, b, c); a1 = fmaf(a1, b, c); a2 = fmaf(a2, b, c); a3 = fmaf(a3, b, c);
+            a4 = fmaf(a4, b, c); a5 = fmaf(a5, b, c); a6 = fmaf(a6, b, c); a7 = fmaf(a7, b, c);
+        }
+    }
+    const float s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+    if (s == 123.456f) sink[0] = s;
+}
+// MUFU issue rate (the "SFU" of north_star): the reciprocal seeds of the march are MUFU.RCP (fp32) / MUFU.RCP64H (fp64).
+// 8 independent chains per thread of MUFU.RCP64H (F64) or MUFU.RSQ (fp32: same unit and rate as MUFU.RCP); the values stay finite.
+template <bool F64>
+__global__ void mufu_peak_kernel(int iters, float* sink) {
+    float a[8]; double d[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) { a[u] = 1.5f + threadIdx.x * 1e-3f + u; d[u] = 1.5 + threadIdx.x * 1e-3 + u; }
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int r = 0; r < 8; ++r)
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                if constexpr (F64) asm volatile("rcp.approx.ftz.f64 %0, %1;" : "=d"(d[u]) : "d"(d[u]));
+                else asm volatile("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(a[u]) : "f"(a[u]));     // (a chain of rcp.approx is folded away: 1/(1/x) = x)
+            }
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int u = 0; u < 8; ++u) s += F64 ? (float)d[u] : a[u];
+    if (s == 123.456f) sink[0] = s;
+}
+
 }  // namespace sck

@@ -745,3 +745,78 @@ def test_two_components_in_fp32_and_with_the_midpoint_stepper(sc, kw, tol):
         for c in range(2):
             assert relerr(dn.cpu().numpy()[c], ro["delta_new"][c]) < tol, (it, c)
         assert relerr(jx.cpu().numpy(), ro["jx"]) < tol and relerr(fe.cpu().numpy(), ro["fe_I"]) < tol
+
+
+@pytest.mark.parametrize("norm_gpu,norm_orc", [(1, 1), (-1, 0), (2, 2)])
+def test_residual_norms_of_eq27(sc, norm_gpu, norm_orc):
+    """Eq. 27 (:201) in the 1-, 2- and maximum norm (:960 "norm"): opts.residual_norm against oracle.residual, for Delta
+    (one element = one complex number) and A_ind (one element = the 2-vector at a grid point) over BB iterations."""
+    wl = wlmod.make_workload(1, pts_per_xi=5, n_angles=16, n_energies=24)
+    o = oracle.Oracle.from_workload(wl)
+    drv = oracle.Driver(o, wl.Aext_x, wl.Aext_y, wl.n_energies, accelerator=1, step=1.0, norm=norm_orc)
+    ctx = sc.ScContext.from_workload(wl, residual_norm=norm_gpu)
+    ctx.sc_set_external_field(dev(wl.Aext_x), dev(wl.Aext_y))
+    d_g = dev(wl.delta0.astype(np.complex128)).clone()
+    ax_g = torch.zeros((wl.ny, wl.nx), dtype=torch.float64, device="cuda"); ay_g = torch.zeros_like(ax_g)
+    d_o = wl.delta0.copy(); ax_o = np.zeros((wl.ny, wl.nx)); ay_o = np.zeros((wl.ny, wl.nx))
+    seen = []
+    for it in range(4):
+        r = drv.iterate(d_o, ax_o, ay_o)
+        d_o, ax_o, ay_o = r["delta"], r["Aind_x"], r["Aind_y"]
+        st = ctx.sc_iterate(1, 1.0, False, d_g, ax_g, ay_g, want_stats=True)
+        assert abs(st.res_delta - r["res_delta"]) < 1e-7 * r["res_delta"], (it, st.res_delta, r["res_delta"])
+        if it > 0:                                    # A_ind = 0 before the first update: the oracle's ratio is then |dA| itself
+            assert abs(st.res_A - r["res_A"]) < 1e-6 * r["res_A"], (it, st.res_A, r["res_A"])
+        seen.append(st.res_delta)
+    assert len(set(round(v, 12) for v in seen)) == 4
+    with pytest.raises(sc.ScError):
+        sc.ScContext.from_workload(wl, residual_norm=3)
+
+
+def test_pipe_peak_taps(sc):
+    """register-resident loops behind bench.py's roofline denominators: FFMA ~ 2x DFMA lanes, MUFU well below both"""
+    wl = wlmod.make_workload(0)
+    ctx = sc.ScContext.from_workload(wl)
+    dfma = ctx.sc_debug_fp64_peak_sustained(0.3)
+    ffma = ctx.sc_debug_pipe_peak(1, 0.3)
+    mufu32, mufu64 = ctx.sc_debug_pipe_peak(2, 0.3), ctx.sc_debug_pipe_peak(3, 0.3)
+    assert 1.5 * dfma < ffma < 2.6 * dfma                  # 128 vs 64 lanes per SM
+    assert 0.05 * ffma < mufu32 < 0.3 * ffma and 0.05 * ffma < mufu64 < 0.3 * ffma       # 16 MUFU lanes per SM
+    with pytest.raises(sc.ScError):
+        ctx.sc_debug_pipe_peak(7, 0.1)
+
+
+def test_single_rank_nccl_attach_and_bench_path(sc, tmp_path):
+    """`sharding.attach` — the function bench.py --gpus N calls under torchrun — on a one-rank NCCL group: the hooked
+    sweep (raw accumulators -> all-reduce on the context's stream -> finalise) must equal the plain sweep bit for bit;
+    and bench.py itself runs end to end on a reduced workload and prints one JSON line with the contract's keys."""
+    import json, os, subprocess, sys, socket
+    import torch.distributed as dist
+    from paper_2205_15000_b200 import sharding
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", 0))
+    try:
+        wl = wlmod.make_workload(1, pts_per_xi=5, n_angles=16, n_energies=64)
+        plain = GpuRun(sc, wl); plain.set_fields(wl.delta0, wl.Aext_x, wl.Aext_y)
+        ref = plain.sweep(stats=False)
+        sh = GpuRun(sc, wl)
+        acc = sharding.attach(sh.ctx, wl.t, wl.n_energies)
+        sh.set_fields(wl.delta0, wl.Aext_x, wl.Aext_y)
+        got = sh.sweep(stats=False)
+        assert float(acc.abs().max()) > 0
+        for k in ("delta_new", "jx", "jy", "fe_I"):
+            assert np.array_equal(got[k], ref[k]), k
+    finally:
+        dist.destroy_process_group()
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, RANK="0", LOCAL_RANK="0", WORLD_SIZE="1")
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--steps", "2", "--warmup", "3", "--pts-per-xi", "4", "--n-angles", "16",
+                          "--n-energies", "64", "--size-scale", "0.2", "--burnin", "3", "--no-cpu-baseline"], capture_output=True, text=True, env=env, timeout=900)
+    assert out.returncode == 0, out.stderr[-2000:]
+    line = json.loads(out.stdout.strip().splitlines()[-1])
+    for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling", "dtype", "config", "clocks", "e2e", "gpu_launches", "roofline"):
+        assert k in line, k
+    assert line["gpu_launches"] > 0 and line["roofline"]["kernel"] == "sck::" + BENCH_KERNEL[64]
+    assert 0 < line["e2e"]["value"] <= line["value"] * 1.5      # (a reduced grain is launch-bound and still in the BB transient)
+    assert line["config"]["fp32_mode"]["roofline"]["kernel"] == "sck::" + BENCH_KERNEL[32]

@@ -78,3 +78,65 @@ def test_world2_gloo_sharded_sweep_matches_full(tmp_path):
         for key in ("delta_new", "jx", "jy", "fe_I"):
             err = np.max(np.abs(got[key] - ref[key])) / max(np.max(np.abs(ref[key])), 1e-6)
             assert err < 1e-12, (rank, key, err)
+
+
+class _FakeContext:
+    """Stands in for ScContext on a box without a GPU: the same four members `sharding.attach` touches.  Its sweep
+    computes this rank's accumulators with the oracle (in place of the kernels), runs the hook, and finalises —
+    the order of operations of sc_riccati_sweep with a hook set (include/sc_riccati.h, sc_set_allreduce_hook)."""
+
+    def __init__(self, wl):
+        self.wl, self.o = wl, oracle.Oracle.from_workload(wl)
+        self.n_components, self.ny, self.nx, self.device = 1, wl.ny, wl.nx, torch.device("cpu")
+        self.stores = None
+
+    def sc_set_energies(self, z, w, denominator_sum):
+        self.z, self.w, self.dsum = np.asarray(z), np.asarray(w), denominator_sum
+
+    def sc_set_allreduce_hook(self, acc, fn):
+        self.acc, self.fn = acc, fn
+
+    def sweep(self):
+        wl = self.wl
+        if self.stores is None:
+            self.stores = self.o.reset_stores(wl.delta0, wl.Aext_x, wl.Aext_y, self.z)
+        r = self.o.raw_sweep(wl.delta0, wl.Aext_x, wl.Aext_y, self.z, self.w, self.stores)
+        self.stores = r["stores"]
+        self.acc.copy_(torch.from_numpy(np.stack([r["num"].real, r["num"].imag, r["Jx"], r["Jy"], r["I"]])))
+        self.fn()
+        a = self.acc.numpy()
+        D = np.log(wl.t) + self.dsum
+        return dict(delta_new=-2j * wl.t * (a[0] + 1j * a[1]) / D * wl.mask, jx=2.0 * wl.charge_sign * wl.t * a[2] * wl.mask,
+                    jy=2.0 * wl.charge_sign * wl.t * a[3] * wl.mask, fe_I=wl.t * a[4] * wl.mask)
+
+
+def _attach_worker(rank, world, port, out):
+    import torch.distributed as dist
+    os.environ["MASTER_ADDR"] = "127.0.0.1"; os.environ["MASTER_PORT"] = str(port)
+    os.environ["OMP_NUM_THREADS"] = "2"
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    wl = wlmod.make_workload(1, pts_per_xi=4, n_angles=8, n_energies=64)     # whole warps of energies: 32 per rank
+    ctx = _FakeContext(wl)
+    acc = sharding.attach(ctx, wl.t, wl.n_energies)          # the function bench.py --gpus N calls
+    assert acc.shape == (5, wl.ny, wl.nx) and len(ctx.z) == 32 and ctx.z.imag[0] == wl.t * (32 * rank + 0.5)
+    for _ in range(2):
+        res = ctx.sweep()
+    np.savez(out + f".{rank}.npz", **res)
+    dist.destroy_process_group()
+
+
+def test_world2_gloo_attach_runs_the_hook_path(tmp_path):
+    import torch.multiprocessing as mp
+    world, port, out = 2, _free_port(), str(tmp_path / "attach")
+    mp.spawn(_attach_worker, args=(world, port, out), nprocs=world, join=True)
+    wl = wlmod.make_workload(1, pts_per_xi=4, n_angles=8, n_energies=64)
+    o = oracle.Oracle.from_workload(wl)
+    st = None
+    for _ in range(2):
+        ref = o.sweep(wl.delta0, wl.Aext_x, wl.Aext_y, wl.n_energies, st)
+        st = ref["stores"]
+    for rank in range(world):
+        got = np.load(out + f".{rank}.npz")
+        for key in ("delta_new", "jx", "jy", "fe_I"):
+            err = np.max(np.abs(got[key] - ref[key])) / max(np.max(np.abs(ref[key])), 1e-6)
+            assert err < 1e-12, (rank, key, err)
