@@ -223,29 +223,11 @@ struct MarchArgsT {
 };
 using MarchArgs = MarchArgsT<double>;
 
-#ifndef SC_MARCH_WARPS
-#define SC_MARCH_WARPS 8
-#endif
-constexpr int MARCH_WARPS = SC_MARCH_WARPS;  // warps per CTA
-#ifndef SC_MARCH_MIN_CTAS
-#define SC_MARCH_MIN_CTAS 2
-#endif
-constexpr int MARCH_MIN_CTAS = SC_MARCH_MIN_CTAS;   // resident CTAs per SM the fp64 register budget is sized for
-#ifndef SC_P1_UNROLL
-#define SC_P1_UNROLL 2
-#endif
-constexpr int P1_UNROLL = SC_P1_UNROLL;      // pass 1: pieces per unrolled loop body
-#ifndef SC_HALF_SPILL
-#define SC_HALF_SPILL 1
-#endif
-#ifndef SC_PF_DIST
-#define SC_PF_DIST 16
-#endif
-constexpr int PF_DIST = SC_PF_DIST;          // pass 2: scratch lines are pulled into L2 this many nodes ahead
-#ifndef SC_RED_NODES
-#define SC_RED_NODES 4
-#endif
-constexpr int RED_NODES = SC_RED_NODES;      // nodes per shared-memory reduction batch
+constexpr int MARCH_WARPS = 8;               // warps per CTA
+constexpr int MARCH_MIN_CTAS = 2;            // resident CTAs per SM the fp64 register budget is sized for (128 registers per thread)
+constexpr int P1_UNROLL = 2;                 // pass 1: pieces per unrolled loop body
+constexpr int PF_DIST = 16;                  // pass 2: scratch lines are pulled into L2 this many nodes ahead
+constexpr int RED_NODES = 4;                 // nodes per shared-memory reduction batch
 constexpr int RED_VALS = 6;
 constexpr int STAGE_LD = 34;                 // padded row of the transpose stage: 16-byte aligned rows, conflict-free 128-bit column reads
 
@@ -476,7 +458,7 @@ __device__ __forceinline__ void march_round(const MarchArgsT<R>& A, const WarpJo
     // m+1 down across piece m+1 — with the T it evaluates anyway for gamma's step up across the same piece — to get
     // gamma~ at the even node m: one more Moebius step per two units (13.5 FP64 instructions per unit) for half the
     // scratch traffic (16 instead of 32 B per unit).  Entry m>>1 holds node m+1 (m even, m+1 < nn) or the last node.
-    constexpr bool HALF = !ST && STEP == 0 && SC_HALF_SPILL != 0;
+    constexpr bool HALF = !ST && STEP == 0;
     constexpr int PFROWS = HALF ? RED_NODES / 2 : RED_NODES;   // scratch rows one reduction batch consumes
     const int lane = J.lane, nn = J.nn, ne = J.ne;
     char* const scr = J.scr_w + lane * BYTES;               // entry e of this lane: scr + e*ROW
@@ -811,10 +793,7 @@ __device__ __forceinline__ int back_weights(const BackArgs& B, int p, double x, 
 
 // 2-D thread tiles (BACK_TX x BACK_TY grid points): neighbouring points share lattice nodes, so a compact tile re-uses
 // the gathered `part` lines in L1 instead of fetching them again from L2
-#ifndef SC_BACK_TY
-#define SC_BACK_TY 8
-#endif
-constexpr int BACK_TX = 16, BACK_TY = SC_BACK_TY;
+constexpr int BACK_TX = 16, BACK_TY = 8;
 __global__ void __launch_bounds__(BACK_TX * BACK_TY) rotate_back_kernel(BackArgs B) {
     const int i = blockIdx.x * BACK_TX + threadIdx.x, j = blockIdx.y * BACK_TY + threadIdx.y;
     if (i >= B.G.nx || j >= B.G.ny) return;

@@ -48,10 +48,6 @@ __device__ __forceinline__ double rcp_nr(double x) {
     double y;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
     double e = fma(-x, y, 1.0);
-#ifdef SC_MATH_EXTRA_NEWTON
-    y = fma(y, e, y);
-    e = fma(-x, y, 1.0);
-#endif
     const double t = fma(e, e, e);
     return fma(y, t, y);
 }
@@ -59,13 +55,6 @@ __device__ __forceinline__ double rcp_nr(double x) {
 __device__ __forceinline__ double rsqrt_nr(double x) {
     double y;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-#ifdef SC_MATH_EXTRA_NEWTON
-    {
-        const double t0 = x * y;
-        const double e0 = fma(-t0, y, 1.0);
-        y = fma(0.5 * y, e0, y);
-    }
-#endif
     const double t = x * y;
     const double e = fma(-t, y, 1.0);          // 1 - x y^2
     const double p = fma(0.375, e, 0.5);       // y (1 + e/2 + 3 e^2/8)
@@ -196,11 +185,8 @@ __device__ __noinline__ cplx_t<R> coef_T_slow(R d2, R zr, R zi, R len) { return 
 // bound is only approached at the highest energies (|dw| ~ 2 eps |a|), where one step already contracts a perturbation
 // of gamma by e^{-2 eps h}; at the low energies that carry a long memory |dw|/radius ~ |De|^2/wp ~ 1e-4 and the
 // truncation is below 1e-20.  The parity budget is 1e-9.
-#ifndef SC_TK
-#define SC_TK 5
-#endif
 template <typename R> struct TaylorK;
-template <> struct TaylorK<double> { static constexpr int K = SC_TK; static constexpr double RMAX = SC_TK >= 8 ? 0.024 : 0.01; };   // 0.01^6 = 1e-12, 0.024^9 = 3e-15
+template <> struct TaylorK<double> { static constexpr int K = 5; static constexpr double RMAX = 0.01; };                                // 0.01^6 = 1e-12
 template <> struct TaylorK<float> { static constexpr int K = 3; static constexpr double RMAX = 0.012; };                                // 0.012^4 = 2e-8
 template <typename R, int K>
 __device__ __forceinline__ cplx_t<R> taylor_real(const R (&c)[K + 1], R dwr, R dwi, R s) {
