@@ -16,6 +16,14 @@ TOL = 1e-9
 TOL32 = 2e-4          # north_star: "to 2e-4 in the optional FP32 mode"
 
 
+def ITER_TOL(it):
+    """Tolerance after `it` accelerated self-consistency iterations from identical starts.  One sweep agrees to TOL; an
+    accelerated update x += alpha (g(x) - x) multiplies an existing difference by up to |1 - alpha (1 - g')|, and the
+    Barzilai-Borwein / CongAcc / Polyak step sizes reach alpha ~ 3-4 in these runs (DESIGN.md §3 R-TOL, measured with
+    `ITER_TOL_PROBE=1`: the worst growth per iteration over all iteration tests is below 3, and it stops after a few)."""
+    return TOL * max(1.0, 3.0 ** min(it, 6))
+
+
 def relerr(a, b):
     a = np.asarray(a); b = np.asarray(b)
     return float(np.max(np.abs(a - b)) / max(float(np.max(np.abs(b))), 1e-6))
@@ -403,7 +411,7 @@ def test_self_consistent_iterations_match(sc, cfg, kw, acc, niter):
         torch.cuda.synchronize()
         assert ctx.sc_debug_last_march_variant() == expected_variant(wl, False)       # sc_iterate never asks the march for stats
         # the fixed-point map amplifies rounding differences by at most alpha per iteration
-        tol = TOL * max(1.0, 3.0 ** min(it, 6)) if acc == 1 else TOL
+        tol = ITER_TOL(it) if acc == 1 else TOL
         assert relerr(d_g.cpu().numpy(), d_o) < tol, it
         if wl.kappa > 0:
             assert relerr(ax_g.cpu().numpy(), ax_o) < tol * 10, it
@@ -434,7 +442,7 @@ def test_polyak_and_congacc_iterations_match(sc, cfg, kw, acc, step, niter):
         wmax = max(wmax, max(r["w"]))
         st = ctx.sc_iterate(acc, step, False, d_g, ax_g, ay_g, want_stats=True)
         torch.cuda.synchronize()
-        tol = TOL * max(1.0, 3.0 ** min(it, 6))        # rounding differences are amplified by the iteration map
+        tol = ITER_TOL(it)
         assert relerr(d_g.cpu().numpy(), d_o) < tol, it
         if wl.kappa > 0:
             assert relerr(ax_g.cpu().numpy(), ax_o) < tol * 10, it
@@ -524,7 +532,7 @@ def test_two_component_iterations_match(sc, acc, step):
         d_o, ax_o, ay_o = r["delta"], r["Aind_x"], r["Aind_y"]
         st = ctx.sc_iterate(acc, step, False, d_g, ax_g, ay_g, want_stats=True)
         torch.cuda.synchronize()
-        tol = TOL * max(1.0, 3.0 ** min(it, 6))
+        tol = ITER_TOL(it)
         assert relerr(d_g.cpu().numpy(), d_o) < tol, it
         assert relerr(ax_g.cpu().numpy(), ax_o) < tol * 10, it
         assert abs(st.res_delta - r["res_delta"]) < 1e-7 * max(r["res_delta"], 1e-3)
@@ -821,3 +829,25 @@ def test_single_rank_nccl_attach_and_bench_path(sc, tmp_path):
     assert line["gpu_launches"] > 0 and line["roofline"]["kernel"] == "sck::" + BENCH_KERNEL[64]
     assert 0 < line["e2e"]["value"] <= line["value"] * 1.5      # (a reduced grain is launch-bound and still in the BB transient)
     assert line["config"]["fp32_mode"]["roofline"]["kernel"] == "sck::" + BENCH_KERNEL[32]
+
+
+def test_annulus_self_consistent_iterations_match(sc):
+    """NEXT-3 through the driver: the annulus in the solenoid gauge (flux through the hole, matching winding, kappa = 3:
+    induced A from the hole-rim and outer-rim currents), 5 Barzilai-Borwein iterations of sc_iterate against oracle.Driver
+    — the GPU twin of the oracle's Eq. 43 / Eq. 48 runs (tests/test_oracle_pins_annulus.py)."""
+    wl = wlmod.make_annulus_workload(flux_in_hole=0.6, n_energies=32)
+    o = oracle.Oracle.from_workload(wl)
+    drv = oracle.Driver(o, wl.Aext_x, wl.Aext_y, wl.n_energies, accelerator=1, step=1.0)
+    ctx = sc.ScContext.from_workload(wl)
+    ctx.sc_set_external_field(dev(wl.Aext_x), dev(wl.Aext_y))
+    d_g = dev(wl.delta0.astype(np.complex128)).clone()
+    ax_g = torch.zeros((wl.ny, wl.nx), dtype=torch.float64, device="cuda"); ay_g = torch.zeros_like(ax_g)
+    d_o = wl.delta0.copy(); ax_o = np.zeros((wl.ny, wl.nx)); ay_o = np.zeros((wl.ny, wl.nx))
+    for it in range(5):
+        r = drv.iterate(d_o, ax_o, ay_o)
+        d_o, ax_o, ay_o = r["delta"], r["Aind_x"], r["Aind_y"]
+        st = ctx.sc_iterate(1, 1.0, False, d_g, ax_g, ay_g, want_stats=True)
+        assert ctx.sc_debug_last_march_variant() == BENCH_KERNEL[64]
+        assert relerr(d_g.cpu().numpy(), d_o) < ITER_TOL(it) and relerr(ax_g.cpu().numpy(), ax_o) < 10 * ITER_TOL(it), it
+        assert abs(st.res_delta - r["res_delta"]) < 1e-7 * max(r["res_delta"], 1e-3)
+    assert float(ax_g.abs().max()) > 1e-4

@@ -1,0 +1,136 @@
+"""The paper's analytic benchmarks of an s-wave annulus, run on the oracle:
+
+  * Eq. 43 (:569): in the solenoid gauge Eq. 41 (:555) the free energy of a state with phase winding n is the parabola
+    dOmega = (pi/4) Y(T) ln(R_> / R_<) (n + Phi/Phi0)^2 — with Y(T) = t sum_n |D|^2 / Lambda_n^3, the coefficient of the
+    linear response j = -Y p_s (Eq. 34 :502, pin P6);
+  * Eq. 48-53 (:614-636): in a homogeneous field with screening, A_phi(R) is the modified-Bessel solution of the
+    London-Maxwell equation (45) with lambda = kappa / sqrt(Y) (Eq. 46), and the field in the hole is beta Phi0 / A_h.
+
+They pin, against formulas the paper prints, what nothing else pins: the multi-interval ("remove") clipping with its
+hole-rim reflections inside a full self-consistent calculation, the free-energy functional Eq. 17/19 summed over a
+grain, and the whole Driver loop (sweep -> D1 A-solve -> mixing) including the sign and magnitude of the screening.
+R_< = 10 xi0, R_> = 25 xi0 as in Fig. 8 and Fig. 10; h = 0.5 xi0 is enough for an s-wave gap that stays uniform.
+"""
+import math
+
+import numpy as np
+import pytest
+from scipy.special import iv, kv
+
+import oracle
+import workloads as wlmod
+from workloads import make_mask
+
+R_IN, R_OUT, H, T, NE, NPHI = 10.0, 25.0, 0.5, 0.5, 8, 16
+
+
+def _annulus(kappa=-1.0):
+    shapes = [wlmod.disc(R_OUT), wlmod.disc(R_IN, add=False)]
+    n = int(round(2 * R_OUT / H)) + 2
+    mask = make_mask(shapes, n, n, H)
+    X, Y = wlmod.grid_xy(n, n, H)
+    return oracle.Oracle(n, n, H, mask, shapes, T, wlmod.SYM_S, NPHI, kappa=kappa), mask, X, Y, n
+
+
+def _response_coefficient(amp):
+    eps = T * (np.arange(NE) + 0.5)
+    return T * float(np.sum(amp ** 2 / (eps ** 2 + amp ** 2) ** 1.5))       # Y(T): j = -Y p_s (pin P6)
+
+
+@pytest.fixture(scope="module")
+def solenoid_runs():
+    """self-consistent Delta at kappa = infinity for (flux in the hole, winding) pairs; total free energy Eq. 17 / 19"""
+    o, mask, X, Y, n = _annulus()
+    R2 = np.maximum(X * X + Y * Y, 1e-12)
+    out = {}
+    for alpha, wind in ((0.0, 0), (0.5, 0), (1.0, 0), (-1.0, 0), (1.0, -1), (0.5, -1)):
+        Ax, Ay = -alpha * Y / (2 * R2), alpha * X / (2 * R2)                 # Eq. 41: A = Phi / (2 pi R) phi-hat = alpha / (2R) in units of A0
+        d = wlmod.BULK_GAP[("s", 0.5, 16)] * np.exp(1j * wind * np.arctan2(Y, X)) * mask
+        drv = oracle.Driver(o, Ax, Ay, NE, accelerator=0, step=1.0)
+        z = np.zeros((n, n))
+        for _ in range(40):
+            r = drv.iterate(d, z, z)
+            d = r["delta"]
+            if r["res_delta"] < 1e-7:
+                break
+        rr = o.sweep(d, Ax, Ay, NE, drv.stores)
+        om = o.free_energy_density(d, NE, rr["fe_I"])
+        out[(alpha, wind)] = dict(F=H * H * float(np.sum(om[mask > 0])), amp=float(abs(d[n // 2, n // 2 + int(17 / H)])), jx=rr["jx"], jy=rr["jy"])
+    return out, mask, X, Y, n
+
+
+def test_eq43_free_energy_parabolas_in_the_solenoid_gauge(solenoid_runs):
+    runs, mask, X, Y, n = solenoid_runs
+    C = math.pi / 4 * _response_coefficient(runs[(0.0, 0)]["amp"]) * math.log(R_OUT / R_IN)     # Eq. 43 for (n + alpha)^2 = 1
+    F0 = runs[(0.0, 0)]["F"]
+    assert F0 < -30.0                                                   # condensation energy of the grain, ~ Omega_bulk x area
+    # winding 0: parabola centred at alpha = 0; measured 0.991, 0.990 (the corrections are the p_s^4 terms: negative)
+    for alpha in (0.5, 1.0, -1.0):
+        ratio = (runs[(alpha, 0)]["F"] - F0) / (C * alpha ** 2)
+        assert 0.97 < ratio < 1.005, (alpha, ratio)
+    assert abs(runs[(1.0, 0)]["F"] - runs[(-1.0, 0)]["F"]) < 1e-9        # even in the flux
+    # winding -1: the same parabola centred at alpha = +1 (flux quantisation; R11: chi = n phi with n = -1 pairs with +Phi0).
+    # The centre sits 0.2 % above F0 — piecewise-constant coefficients are gauge covariant only to O(h^2) (pin P12).
+    Fc = runs[(1.0, -1)]["F"]
+    assert abs(Fc - F0) < 3e-3 * abs(F0)
+    ratio = (runs[(0.5, -1)]["F"] - Fc) / (C * 0.25)
+    assert 0.97 < ratio < 1.02, ratio
+    # and the currents: p_s = (n + alpha) / (2R) phi-hat (Eq. 42), j = -Y p_s: no current at the matching flux, a circulating one off it
+    c = n // 2
+    i = c + int(17 / H)
+    Yc = _response_coefficient(runs[(0.0, 0)]["amp"])
+    R = X[c, i]
+    assert abs(runs[(1.0, -1)]["jy"][c, i]) < 0.1 * Yc * 0.5 / (2 * R)     # (5 % of the half-flux current is left: O(h^2) gauge error)
+    assert abs(runs[(1.0, 0)]["jy"][c, i] - (-Yc * 1.0 / (2 * R))) < 0.02 * Yc / (2 * R)
+    assert abs(runs[(0.5, -1)]["jy"][c, i] - (-Yc * (-0.5) / (2 * R))) < 0.06 * Yc * 0.5 / (2 * R)      # sign: the current reverses with n + alpha
+
+
+def _london(R, alpha, wind, lam):
+    """Eq. 48-53 with xi0 = 1 and A0 = Phi0 / (pi xi0) = 1, i.e. Phi0 = pi"""
+    A_ann, A_h = math.pi * (R_OUT ** 2 - R_IN ** 2), math.pi * R_IN ** 2
+    I0g, K0g, I2l, K2l = iv(0, R_OUT / lam), kv(0, R_OUT / lam), iv(2, R_IN / lam), kv(2, R_IN / lam)
+    I0l, K0l = iv(0, R_IN / lam), kv(0, R_IN / lam)
+    M = I0g * K2l - I2l * K0g
+    a = (K2l * alpha / A_ann + K0g * wind / A_h) / M                       # Eq. 50
+    b = (I2l * alpha / A_ann + I0g * wind / A_h) / M                       # Eq. 51
+    beta = (2 * math.pi * lam ** 2 / A_ann * alpha - (I0g * K0l - I0l * K0g) * wind) / M      # Eq. 52
+    A = math.pi * lam * (a * iv(1, R / lam) + b * kv(1, R / lam)) - wind / (2 * R)            # Eq. 48
+    return A, math.pi * beta / A_h                                         # A_phi(R), B in the hole (Eq. 53)
+
+
+@pytest.mark.parametrize("alpha,wind", [(4.0, 0), (0.0, -1)])
+def test_eq48_london_bessel_profile_with_screening(alpha, wind):
+    """kappa = 5 (lambda(T) = 5.5 xi0, the annulus is 2.7 lambda wide): converge Delta and A_ind with the Driver
+    (Barzilai-Borwein), compare the total A_phi(R), j_phi(R) = -Y (A_phi + n / 2R) and the field in the hole."""
+    kappa = 5.0
+    o, mask, X, Y, n = _annulus(kappa)
+    Bext = math.pi * alpha / (math.pi * (R_OUT ** 2 - R_IN ** 2))           # alpha Phi0 / area
+    Aex, Aey = -0.5 * Bext * Y, 0.5 * Bext * X
+    d = wlmod.BULK_GAP[("s", 0.5, 16)] * np.exp(1j * wind * np.arctan2(Y, X)) * mask
+    drv = oracle.Driver(o, Aex, Aey, NE, accelerator=1, step=1.0)
+    ax = np.zeros((n, n)); ay = np.zeros((n, n))
+    for _ in range(50):
+        r = drv.iterate(d, ax, ay)
+        d, ax, ay = r["delta"], r["Aind_x"], r["Aind_y"]
+    assert r["res_delta"] < 1e-4 and r["res_A"] < 1e-3
+    c = n // 2
+    Yc = _response_coefficient(float(abs(d[c, c + int(17 / H)])))
+    lam = kappa / math.sqrt(Yc)                                            # Eq. 46
+    scale = max(abs(_london(R_OUT, alpha, wind, lam)[0] + wind / (2 * R_OUT)), abs(_london(R_IN, alpha, wind, lam)[0] + wind / (2 * R_IN)))
+    for Rr in (11.0, 14.0, 17.5, 21.0, 24.0):
+        i = c + int(round(Rr / H - 0.5))
+        R = X[c, i]                                                      # on the +x axis (y = h/2): phi-hat ~ y-hat
+        y = Y[c, i]; rr_ = math.hypot(R, y)
+        A_num = (-(ax + Aex)[c, i] * y + (ay + Aey)[c, i] * R) / rr_
+        j_num = (-r["jx"][c, i] * y + r["jy"][c, i] * R) / rr_
+        A_an, _ = _london(rr_, alpha, wind, lam)
+        assert abs(A_num - A_an) < 0.03 * max(abs(A_an), 0.3 * scale), (Rr, A_num, A_an)
+        ps = A_an + wind / (2 * rr_)
+        assert abs(j_num - (-Yc * ps)) < 0.06 * Yc * max(abs(ps), 0.3 * scale), (Rr, j_num, -Yc * ps)
+    # the flux density in the hole: curl of the total A at the centre against beta Phi0 / A_h (Eq. 52-53)
+    At_x, At_y = ax + Aex, ay + Aey
+    B_num = ((At_y[c, c + 1] - At_y[c, c - 1]) - (At_x[c + 1, c] - At_x[c - 1, c])) / (2 * H)
+    B_an = _london(R_IN, alpha, wind, lam)[1]
+    assert abs(B_num - B_an) < 0.04 * abs(B_an), (B_num, B_an)
+    if wind == 0:
+        assert 0 < B_num < Bext                                           # the ring screens part of the applied flux out of the hole
