@@ -13,11 +13,15 @@
 // Units (Table II :1204-1230): energies in 2 pi kB Tc, lengths in xi0 (v_F = 1),
 // t = T/Tc, Matsubara eps_n = t (n + 1/2), A in A0 = Phi0/(pi xi0) so that (e/c) v_F.A -> sigma_e v.A.
 //
-// Pins (tests/test_oracle_pins.py): closed-form step vs adaptive ODE solve, bulk fixed point, uniform
-// gap closed form, BCS gap 1.764 / 2.14, Doppler-shift current, bulk free energy Eq. 38, ABS kink,
-// Eq. 13 symmetry, global-phase covariance, G_{m,n} vs quadrature of D2, brute-force ray tracing.
-// Parity unpinned (fixed only by DESIGN.md readings): interpolation-weight fallbacks at corners /
-// grazing incidence (R7, R9 fallbacks).
+// Pins (tests/test_oracle_pins*.py, listed with the sabotages they catch in DESIGN.md §7): closed-form step vs adaptive
+// ODE solve, bulk fixed point, uniform gap closed form, BCS gap 1.764 / 2.14, Doppler-shift current, bulk free energy
+// Eq. 38, ABS kink, Eq. 13 symmetry, global-phase covariance, G_{m,n} vs quadrature of D2, brute-force ray tracing on and
+// off the lattice (ODE reference), gather weights against prescribed linear stores and analytic normals (square, disc,
+// annulus), rotate-in / rotate-back against a library bilinear interpolant, charge conservation at self-consistency,
+// rotation covariance P11, and the paper's annulus benchmarks Eq. 43 and Eq. 48-53.
+// Parity unpinned (fixed only by DESIGN.md readings): the interpolation FALLBACKS at corners / grazing incidence — the
+// nearest-mask-point search of R5, the "no valid candidate" branch of R6/R7 and the renormalisation of the gather
+// weights when a candidate ends on another wall.
 //
 // Build: g++ -O2 -fopenmp -shared -fPIC -std=c++17 sc_oracle.cpp -o libsc_oracle.so
 

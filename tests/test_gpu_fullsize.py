@@ -100,18 +100,15 @@ def test_full_config3_ldos_sampled_energy_planes(sc):
 
 
 def test_full_config4_production_launch_every_16th_angle_all_energies(sc):
-    """SURVEY §8(d) rule for cfg 4.  ONE production sweep (the launch bench.py times: 256 angles x 512 Matsubara energies,
-    plain table, no stats -> march_kernel<0,false,0,double,1,true>) from the reset boundary stores; the oracle sweeps every
-    16th angle (k = 0, 16, ..., 240: 8 marched pairs, both members of each) with all 512 energies.  Compared, all from
-    that one launch: SF, SG, SI at every lattice node of the 16 angles (6.25 % of the per-angle sums the grid fields are
-    made of, 16 energy rounds accumulated each) and gamma_end / gamma-tilde_end of every trajectory of those angles at
-    every energy (the march's boundary output).  Then properties of the full grid outputs."""
+    """SURVEY §8(d) rule for cfg 4, in FP64 and in FP32 mode.  ONE production sweep (the launch bench.py times: 256 angles
+    x 512 Matsubara energies, plain table, no stats -> march_kernel<0,false,0,double|float,1,true>) from the reset boundary
+    stores; the oracle sweeps every 16th angle (k = 0, 16, ..., 240: 8 marched pairs, both members of each) with all 512
+    energies, once, and both precisions are compared with it.  Compared, all from that one launch: SF, SG, SI at every
+    lattice node of the 16 angles (6.25 % of the per-angle sums the grid fields are made of, 16 energy rounds accumulated
+    each) and gamma_end / gamma-tilde_end of every trajectory of those angles at every energy (the march's boundary
+    output).  Then properties of the full grid outputs."""
     wl = wlmod.make_workload(4)
     Ax, Ay = wl.Aext_x, wl.Aext_y
-    ctx = sc.ScContext.from_workload(wl)
-    ctx.sc_set_fields(dev(wl.delta0.astype(np.complex128)), dev(Ax), dev(Ay))
-    rg = gpu_sweep(ctx, wl, stats=False)
-    assert ctx.sc_debug_last_march_variant() == BENCH_KERNEL[64]
     o = oracle.Oracle.from_workload(wl)
     z, w = o.matsubara(wl.n_energies)
     angles = list(range(0, wl.n_angles, 16))
@@ -119,30 +116,36 @@ def test_full_config4_production_launch_every_16th_angle_all_energies(sc):
     ro = o.raw_sweep(wl.delta0, Ax, Ay, z, w, stores, angle_list=angles, dbg_angle=-2)
     del stores
     assert ro["stats"]["n_bad"] == 0
-    assert ro["stats"]["n_updates"] * (wl.n_angles // len(angles)) == 4 * (ctx.n_pieces // 2) * wl.n_energies   # discs: every angle has the same pieces
-    for ia, k in enumerate(angles):
-        SF, SG, SI = ctx.sc_debug_partial(k)
-        for name, a, b in (("SF", SF, ro["dbg"]["SF"][ia]), ("SG", SG, ro["dbg"]["SG"][ia]), ("SI", SI, ro["dbg"]["SI"][ia])):
-            assert relerr(a, b) < TOL, (k, name, relerr(a, b))
-        ge, gte = ctx.sc_debug_stores(k)
-        r0, r1 = o.traj_offset(k), o.traj_offset(k) + o.ntraj_angle(k)
-        assert ge.shape == (r1 - r0, wl.n_energies)
-        assert relerr(ge, ro["stores"][0][r0:r1]) < TOL and relerr(gte, ro["stores"][1][r0:r1]) < TOL, k
-    del ro
-    # --- properties of the full outputs ---
-    for key in ("delta_new", "jx", "jy", "fe_I"):
-        assert np.all(np.isfinite(rg[key])) and np.all(rg[key][wl.mask == 0] == 0)
-    # the phase of Delta_new winds -20 times around the rim (20 vortices, R11/R19)
-    R = 0.95 * 40.0
-    th = np.linspace(0, 2 * np.pi, 4001)
-    ii = np.rint(R * np.cos(th) / wl.h + 0.5 * (wl.nx - 1)).astype(int); jj = np.rint(R * np.sin(th) / wl.h + 0.5 * (wl.ny - 1)).astype(int)
-    ph = np.unwrap(np.angle(rg["delta_new"][jj, ii]))
-    assert round((ph[-1] - ph[0]) / (2 * np.pi)) == -20
-    # a second sweep with stats: invariants of the whole launch
-    st = gpu_sweep(ctx, wl, stats=True)["stats"]
-    assert st.n_bad == 0 and st.n_updates == 4 * (ctx.n_pieces // 2) * wl.n_energies
-    assert 0.0 < st.min_one_minus_abs_gamma < 1.0
-    ctx.close()
+    for precision, tol in ((64, TOL), (32, TOL32)):
+        ctx = sc.ScContext.from_workload(wl, precision=precision)
+        ctx.sc_set_fields(dev(wl.delta0.astype(np.complex128)), dev(Ax), dev(Ay))
+        rg = gpu_sweep(ctx, wl, stats=False)
+        assert ctx.sc_debug_last_march_variant() == BENCH_KERNEL[precision]
+        assert ro["stats"]["n_updates"] * (wl.n_angles // len(angles)) == 4 * (ctx.n_pieces // 2) * wl.n_energies   # discs: every angle has the same pieces
+        for ia, k in enumerate(angles):
+            SF, SG, SI = ctx.sc_debug_partial(k)
+            for name, a, b in (("SF", SF, ro["dbg"]["SF"][ia]), ("SG", SG, ro["dbg"]["SG"][ia]), ("SI", SI, ro["dbg"]["SI"][ia])):
+                assert relerr(a, b) < tol, (precision, k, name, relerr(a, b))
+            ge, gte = ctx.sc_debug_stores(k)
+            r0, r1 = o.traj_offset(k), o.traj_offset(k) + o.ntraj_angle(k)
+            assert ge.shape == (r1 - r0, wl.n_energies)
+            assert relerr(ge, ro["stores"][0][r0:r1]) < tol and relerr(gte, ro["stores"][1][r0:r1]) < tol, (precision, k)
+        # --- properties of the full outputs ---
+        for key in ("delta_new", "jx", "jy", "fe_I"):
+            assert np.all(np.isfinite(rg[key])) and np.all(rg[key][wl.mask == 0] == 0)
+        # the phase of Delta_new winds -20 times around the rim (20 vortices, R11/R19)
+        R = 0.95 * 40.0
+        th = np.linspace(0, 2 * np.pi, 4001)
+        ii = np.rint(R * np.cos(th) / wl.h + 0.5 * (wl.nx - 1)).astype(int); jj = np.rint(R * np.sin(th) / wl.h + 0.5 * (wl.ny - 1)).astype(int)
+        ph = np.unwrap(np.angle(rg["delta_new"][jj, ii]))
+        assert round((ph[-1] - ph[0]) / (2 * np.pi)) == -20
+        # a second sweep with stats: invariants of the whole launch
+        st = gpu_sweep(ctx, wl, stats=True)["stats"]
+        assert st.n_bad == 0 and st.n_updates == 4 * (ctx.n_pieces // 2) * wl.n_energies
+        assert 0.0 < st.min_one_minus_abs_gamma < 1.0
+        ctx.close()
+        del ctx, rg
+        torch.cuda.empty_cache()
 
 
 @pytest.mark.parametrize("precision,tol", [(64, TOL), (32, TOL32)])
