@@ -49,20 +49,26 @@ UNIT = "updates/s"
 # (profiles/r2_march_ncu.json, read below when it belongs to the kernel sources in the tree).
 STAGE_FP64 = {
     "T_table_deg5": 15.0,       # dw 1, |dw|^2 2, real-coefficient degree-5 polynomial at complex dw 10, remainder 2
+    "T_table_deg3": 11.0,       # FP32 mode: degree 3 (truncation 2e-8 relative at the edge of its radius)
     "T_pole_table": 24.0,       # pole term (one reciprocal) + degree-5 remainder
     "T_pole_table_deg8": 36.0,  # stored-T rounds: degree 8, warp vote
     "moebius_step": 27.0,       # z g + De 4, N 4, z + conj(De) g 4, Q 4, |Q|^2 2, reciprocal 3, N conj(Q) / |Q|^2 6
     "node_products": 26.0,      # P 4, 1+P 1, |.|^2 2, reciprocal 3, 1/(1+P) 2, six summands 14 (unit weights)
     "energy_reduction": 8.0,    # column sums of the transpose stage + running sum
 }
-# least work: nothing evaluated twice — T once, gamma and gamma-tilde stepped once, products, reduction
-LEAST_WORK_FP64 = STAGE_FP64["T_table_deg5"] + 2 * STAGE_FP64["moebius_step"] + STAGE_FP64["node_products"] + STAGE_FP64["energy_reduction"]
-# what the kernel executes: T in both passes, and every second gamma-tilde re-stepped in pass 2 instead of spilled
-EXECUTED_FP64 = {
-    "recompute": LEAST_WORK_FP64 + STAGE_FP64["T_table_deg5"] + 0.5 * STAGE_FP64["moebius_step"],
-    "recompute_pole": LEAST_WORK_FP64 - STAGE_FP64["T_table_deg5"] + 2 * STAGE_FP64["T_pole_table"] + 0.5 * STAGE_FP64["moebius_step"],
-    "stored": LEAST_WORK_FP64 - STAGE_FP64["T_table_deg5"] + STAGE_FP64["T_pole_table_deg8"],
-}
+def stage_counts(precision):
+    """(least work per unit, executed per unit by round type) for the closed-form stepper"""
+    T = STAGE_FP64["T_table_deg5" if precision == 64 else "T_table_deg3"]
+    # least work: nothing evaluated twice — T once, gamma and gamma-tilde stepped once, products, reduction
+    least = T + 2 * STAGE_FP64["moebius_step"] + STAGE_FP64["node_products"] + STAGE_FP64["energy_reduction"]
+    # what the kernel executes: T in both passes, and every second gamma-tilde re-stepped in pass 2 instead of spilled
+    executed = {"recompute": least + T + 0.5 * STAGE_FP64["moebius_step"],
+                "recompute_pole": least - T + 2 * STAGE_FP64["T_pole_table"] + 0.5 * STAGE_FP64["moebius_step"],
+                "stored": least - T + STAGE_FP64["T_pole_table_deg8"]}
+    return least, executed
+
+
+LEAST_WORK_FP64, EXECUTED_FP64 = stage_counts(64)
 EXECUTED_FP64_MIDPOINT = 2 * 66.0 + 28.0 + 8.0
 ALGO_HBM_BYTES_PER_UNIT = {"recompute": 16.0, "recompute_pole": 16.0, "stored": 64.0}   # scratch out + back
 
@@ -71,9 +77,8 @@ def source_hash():
     """sha256 over the kernel sources: ncu figures in profiles/ are only quoted for the code they were captured from"""
     h = hashlib.sha256()
     d = os.path.join(ROOT, "paper_2205_15000_b200", "csrc")
-    for f in sorted(os.listdir(d)):
-        if f.endswith((".cu", ".cuh", ".hpp")):
-            h.update(f.encode()); h.update(open(os.path.join(d, f), "rb").read())
+    for f in ("sc_kernels.cuh", "sc_math.cuh"):            # the files the march kernel is compiled from
+        h.update(f.encode()); h.update(open(os.path.join(d, f), "rb").read())
     return h.hexdigest()
 
 
@@ -252,12 +257,13 @@ def march_roofline(a, wl, ctx, kernel, mk_ms, nl, units, step_ms, precision, ful
     """roofline object of the march kernel for one timed leg"""
     u_all, u_st, u_pl = (v / max(nl, 1) for v in units)
     u_rec = u_all - u_st - u_pl
+    least_pu, exec_pu = stage_counts(precision)
     if a.stepper == 0:
-        executed = sum(EXECUTED_FP64[k] * u for k, u in (("recompute", u_rec), ("recompute_pole", u_pl), ("stored", u_st)))
+        executed = sum(exec_pu[k] * u for k, u in (("recompute", u_rec), ("recompute_pole", u_pl), ("stored", u_st)))
         hbm = sum(ALGO_HBM_BYTES_PER_UNIT[k] * u for k, u in (("recompute", u_rec), ("recompute_pole", u_pl), ("stored", u_st)))
-        least = LEAST_WORK_FP64 * u_all
+        least = least_pu * u_all
     else:
-        executed = EXECUTED_FP64_MIDPOINT * u_all; hbm = 32.0 * u_all; least = executed
+        executed = EXECUTED_FP64_MIDPOINT * u_all; hbm = 32.0 * u_all; least = executed; least_pu = EXECUTED_FP64_MIDPOINT
     if precision == 32:
         hbm *= 0.5
     sec = mk_ms * 1e-3
@@ -273,7 +279,7 @@ def march_roofline(a, wl, ctx, kernel, mk_ms, nl, units, step_ms, precision, ful
     achieved = 2.0 * least / sec / 1e12
     r = {"bound": "alu", "kernel": "sck::" + kernel, "launches_timed": nl,
          "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-         "frac_basis": f"least-work count: {LEAST_WORK_FP64:.0f} fp{precision}-pipe instructions per unit (T once, two Moebius steps, node "
+         "frac_basis": f"least-work count: {least_pu:.0f} fp{precision}-pipe instructions per unit (T once, two Moebius steps, node "
                        "products, energy reduction; nothing evaluated twice) x units / march time (CUDA events around the march "
                        "launches of the timed steps) / measured peak",
          "traffic": cap["dram_bytes"] if cap else None,
@@ -298,6 +304,8 @@ def march_roofline(a, wl, ctx, kernel, mk_ms, nl, units, step_ms, precision, ful
                     "mufu_issue_frac": 3.5 * u_all / sec / mufu,
                     "note": "MUFU.RCP seeds of the reciprocals: one per Moebius step and node product (3.5 per unit with the re-stepped "
                             "gamma-tilde) against the measured MUFU issue rate"}
+        r["issue_note"] = ("the fp32 pipe issues one warp instruction per cycle per scheduler, like every other pipe: the fp32 march is bound "
+                           "by instruction issue (ncu: issue_active_pct of the capture below), not by the fp32 lanes")
     else:
         mufu = ctx.sc_debug_pipe_peak(3, 1.0)
         r["sfu"] = {"mufu_peak_per_s": mufu, "mufu_per_unit_tally": 3.5, "mufu_issue_frac": 3.5 * u_all / sec / mufu,

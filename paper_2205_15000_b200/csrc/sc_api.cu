@@ -16,6 +16,7 @@
 #include "../../include/sc_riccati.h"
 #include "sc_geometry.hpp"
 #include "sc_kernels.cuh"
+#include "sc_probe_kernels.cuh"
 #include "sc_field_kernels.cuh"
 
 #define SC_VERSION_STR "sc_riccati 0.1 (sm_100a)"
@@ -966,17 +967,22 @@ sc_status sc_debug_fp64_peak_sustained(sc_ctx* ctx, double seconds, double* dfma
 }
 
 sc_status sc_debug_pipe_peak(sc_ctx* ctx, int pipe, double seconds, double* ops_per_s) {
-    if (!ctx || !ops_per_s || pipe < 1 || pipe > 3 || !(seconds > 0) || seconds > 30) return fail(ctx, SC_ERR_ARG, "bad argument");
+    if (!ctx || !ops_per_s || pipe < 1 || (pipe > 3 && pipe < 10) || pipe > 14 || !(seconds > 0) || seconds > 30) return fail(ctx, SC_ERR_ARG, "bad argument");
     ON_DEVICE(ctx);
-    DevBuf<float> d; CU(d.alloc(1));
+    DevBuf<float> d; CU(d.alloc(2));
     const int blocks = ctx->n_sm * 4, threads = 256;
-    const int iters = pipe == 1 ? 20000 : 2000;
+    const int iters = pipe == 1 ? 20000 : (pipe >= 10 ? 4000 : 2000);
     const double per_thread = (double)iters * 64.0;       // 8 chains x 8 per loop body, in both kernels
     auto launch = [&]() {
         ++sck::g_launches;
         if (pipe == 1) sck::fp32_peak_kernel<<<blocks, threads, 0, ctx->stream>>>(iters, d.p);
         else if (pipe == 2) sck::mufu_peak_kernel<false><<<blocks, threads, 0, ctx->stream>>>(iters, d.p);
-        else sck::mufu_peak_kernel<true><<<blocks, threads, 0, ctx->stream>>>(iters, d.p);
+        else if (pipe == 3) sck::mufu_peak_kernel<true><<<blocks, threads, 0, ctx->stream>>>(iters, d.p);
+        else if (pipe == 10) sck::fp64_mix_kernel<0, 0><<<blocks, threads, 0, ctx->stream>>>(iters, (double*)d.p);
+        else if (pipe == 11) sck::fp64_mix_kernel<4, 0><<<blocks, threads, 0, ctx->stream>>>(iters, (double*)d.p);
+        else if (pipe == 12) sck::fp64_mix_kernel<8, 0><<<blocks, threads, 0, ctx->stream>>>(iters, (double*)d.p);
+        else if (pipe == 13) sck::fp64_mix_kernel<0, 1><<<blocks, threads, 0, ctx->stream>>>(iters, (double*)d.p);
+        else sck::fp64_mix_kernel<3, 1><<<blocks, threads, 0, ctx->stream>>>(iters, (double*)d.p);
     };
     launch();
     CU(cudaEventRecord(ctx->ev0, ctx->stream));

@@ -17,11 +17,10 @@ TOL32 = 2e-4          # north_star: "to 2e-4 in the optional FP32 mode"
 
 
 def ITER_TOL(it):
-    """Tolerance after `it` accelerated self-consistency iterations from identical starts.  One sweep agrees to TOL; an
-    accelerated update x += alpha (g(x) - x) multiplies an existing difference by up to |1 - alpha (1 - g')|, and the
-    Barzilai-Borwein / CongAcc / Polyak step sizes reach alpha ~ 3-4 in these runs (DESIGN.md §3 R-TOL, measured with
-    `ITER_TOL_PROBE=1`: the worst growth per iteration over all iteration tests is below 3, and it stops after a few)."""
-    return TOL * max(1.0, 3.0 ** min(it, 6))
+    """Tolerance after `it` accelerated self-consistency iterations from identical starts: the same 1e-9 as one sweep, with no
+    allowance for growth.  Measured over every iteration test (`ITER_TOL_PROBE=1 pytest -s -k "iterations or annulus_self"`):
+    Delta stays within 6e-15 and A_ind within 8e-14 of the oracle for up to 20 iterations with every accelerator."""
+    return TOL
 
 
 def _probe(tag, it, err_delta, err_A=None):
@@ -416,12 +415,11 @@ def test_self_consistent_iterations_match(sc, cfg, kw, acc, niter):
         st = ctx.sc_iterate(acc, 1.0, False, d_g, ax_g, ay_g, want_stats=True)
         torch.cuda.synchronize()
         assert ctx.sc_debug_last_march_variant() == expected_variant(wl, False)       # sc_iterate never asks the march for stats
-        # the fixed-point map amplifies rounding differences by at most alpha per iteration
         tol = ITER_TOL(it) if acc == 1 else TOL
         _probe(f"iter cfg{cfg} acc{acc}", it, relerr(d_g.cpu().numpy(), d_o), relerr(ax_g.cpu().numpy(), ax_o) if wl.kappa > 0 else None)
         assert relerr(d_g.cpu().numpy(), d_o) < tol, it
         if wl.kappa > 0:
-            assert relerr(ax_g.cpu().numpy(), ax_o) < tol * 10, it
+            assert relerr(ax_g.cpu().numpy(), ax_o) < tol, it
         assert abs(st.res_delta - r["res_delta"]) < 1e-7 * max(r["res_delta"], 1e-3)
     assert r["res_delta"] < (0.5 if cfg == 4 else 0.2)      # sanity: the run is converging (20 vortices relax slowly)
 
@@ -453,7 +451,7 @@ def test_polyak_and_congacc_iterations_match(sc, cfg, kw, acc, step, niter):
         _probe(f"polyak/congacc cfg{cfg} acc{acc}", it, relerr(d_g.cpu().numpy(), d_o), relerr(ax_g.cpu().numpy(), ax_o) if wl.kappa > 0 else None)
         assert relerr(d_g.cpu().numpy(), d_o) < tol, it
         if wl.kappa > 0:
-            assert relerr(ax_g.cpu().numpy(), ax_o) < tol * 10, it
+            assert relerr(ax_g.cpu().numpy(), ax_o) < tol, it
         assert abs(st.res_delta - r["res_delta"]) < 1e-7 * max(r["res_delta"], 1e-3)
     assert np.all(np.isfinite(d_o))
     if acc == 3 and wl.kappa > 0:
@@ -543,7 +541,7 @@ def test_two_component_iterations_match(sc, acc, step):
         tol = ITER_TOL(it)
         _probe(f"two-component acc{acc}", it, relerr(d_g.cpu().numpy(), d_o), relerr(ax_g.cpu().numpy(), ax_o))
         assert relerr(d_g.cpu().numpy(), d_o) < tol, it
-        assert relerr(ax_g.cpu().numpy(), ax_o) < tol * 10, it
+        assert relerr(ax_g.cpu().numpy(), ax_o) < tol, it
         assert abs(st.res_delta - r["res_delta"]) < 1e-7 * max(r["res_delta"], 1e-3)
 
 
@@ -695,7 +693,7 @@ def test_restart_with_burnin_matches(sc):
             r = drv.iterate(d_o, ax_o, ay_o); d_o, ax_o, ay_o = r["delta"], r["Aind_x"], r["Aind_y"]
             ctx.sc_iterate(0, 0.3, False, d_g, ax_g, ay_g)
         torch.cuda.synchronize()
-        assert relerr(d_g.cpu().numpy(), d_o) < 10 * TOL and relerr(ax_g.cpu().numpy(), ax_o) < 100 * TOL
+        assert relerr(d_g.cpu().numpy(), d_o) < TOL and relerr(ax_g.cpu().numpy(), ax_o) < TOL
         results[nburn] = relerr(d_o, uninterrupted)
     assert results[3] < 0.5 * results[0]
 
@@ -858,6 +856,6 @@ def test_annulus_self_consistent_iterations_match(sc):
         st = ctx.sc_iterate(1, 1.0, False, d_g, ax_g, ay_g, want_stats=True)
         assert ctx.sc_debug_last_march_variant() == BENCH_KERNEL[64]
         _probe("annulus acc1", it, relerr(d_g.cpu().numpy(), d_o), relerr(ax_g.cpu().numpy(), ax_o))
-        assert relerr(d_g.cpu().numpy(), d_o) < ITER_TOL(it) and relerr(ax_g.cpu().numpy(), ax_o) < 10 * ITER_TOL(it), it
+        assert relerr(d_g.cpu().numpy(), d_o) < ITER_TOL(it) and relerr(ax_g.cpu().numpy(), ax_o) < ITER_TOL(it), it
         assert abs(st.res_delta - r["res_delta"]) < 1e-7 * max(r["res_delta"], 1e-3)
     assert float(ax_g.abs().max()) > 1e-4
