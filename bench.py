@@ -145,6 +145,7 @@ def parse():
     ap.add_argument("--no-fp32-leg", action="store_true", help="skip the extra FP32-mode timing that configs[4] asks for")
     ap.add_argument("--no-ldos-leg", action="store_true", help="skip the sc_ldos timing on configs[3]")
     ap.add_argument("--ldos-only", action="store_true", help="time sc_ldos on configs[3] alone (profiling aid)")
+    ap.add_argument("--issue-probe", action="store_true", help="print the DFMA rate next to integer / shared-memory instructions (DESIGN.md §6) and exit")
     return ap.parse_args()
 
 
@@ -342,8 +343,8 @@ def run_leg(a, sc, torch, dist, wl, local, world, precision, burnin, full_size):
         ctx.sc_debug_march_time(); ctx.sc_debug_march_units()
         t0 = time.perf_counter(); step(); torch.cuda.synchronize(); dt = time.perf_counter() - t0
         u = ctx.sc_debug_march_units()
-        if it < 8:
-            transient.append({"iteration": it, "s": round(dt, 4), "stored_T": round(u[1] / max(u[0], 1), 4), "pole_table": round(u[2] / max(u[0], 1), 4)})
+        transient.append({"iteration": it, "s": round(dt, 4), "march_ms": round(ctx.sc_debug_march_time()[0], 1),
+                          "stored_T": round(u[1] / max(u[0], 1), 4), "pole_table": round(u[2] / max(u[0], 1), 4)})
     for _ in range(max(a.warmup, 3)):
         step()
     torch.cuda.synchronize()
@@ -436,6 +437,14 @@ def run_ours(a):
     torch.cuda.set_device(local)
     if a.ldos_only:
         print(json.dumps({"metric": METRIC, "ldos": ldos_leg(sc, torch, local, a.steps)}))
+        return
+    if a.issue_probe:
+        ctx = sc.ScContext.from_workload(workloads.make_workload(0), device=local)
+        names = {10: "DFMA only", 11: "+ 0.5 integer per DFMA", 12: "+ 1 integer per DFMA", 13: "+ 0.125 LDS (and its DADD) per DFMA",
+                 14: "+ 0.375 integer + 0.125 LDS (and its DADD) per DFMA"}
+        base = ctx.sc_debug_pipe_peak(10, 1.0)
+        print(json.dumps({"issue_probe": {names[k]: {"dfma_tflops": 2e-12 * v, "of_dfma_only": v / base}
+                                          for k, v in ((k, ctx.sc_debug_pipe_peak(k, 1.0)) for k in names)}}))
         return
     wl = workload_from_args(a)
     full_size = world == 1 and not (a.pts_per_xi or a.n_angles or a.n_energies or a.size_scale != 1.0)
