@@ -61,9 +61,12 @@ inline int ensure_lowrank(LowRank& L, int nx, int ny, double h, double eps, cuda
     std::vector<double> G((size_t)N * N);
     for (int n = 0; n < N; ++n) for (int m = n; m < N; ++m) G[(size_t)n * N + m] = G[(size_t)m * N + n] = G_closed(m, n, h);   // G_{m,n} = G_{n,m}
     double *dG = nullptr, *dW = nullptr, *work = nullptr; int* info = nullptr; int lwork = 0;
+    cusolverDnHandle_t sol = nullptr;
+    // temporaries and the solver handle are released on every return path (the error macros below return early)
+    struct Temps { double*& a; double*& b; double*& c; int*& i; cusolverDnHandle_t& h;
+                   ~Temps() { cudaFree(a); cudaFree(b); cudaFree(c); cudaFree(i); if (h) cusolverDnDestroy(h); } } temps{dG, dW, work, info, sol};
     SCL_CU(cudaMalloc((void**)&dG, G.size() * sizeof(double))); SCL_CU(cudaMalloc((void**)&dW, N * sizeof(double))); SCL_CU(cudaMalloc((void**)&info, sizeof(int)));
     SCL_CU(cudaMemcpyAsync(dG, G.data(), G.size() * sizeof(double), cudaMemcpyHostToDevice, s));
-    cusolverDnHandle_t sol = nullptr;
     SCL_LIB(cusolverDnCreate(&sol)); SCL_LIB(cusolverDnSetStream(sol, s));
     SCL_LIB(cusolverDnDsyevd_bufferSize(sol, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER, N, dG, N, dW, &lwork));
     SCL_CU(cudaMalloc((void**)&work, (size_t)lwork * sizeof(double)));
@@ -72,7 +75,6 @@ inline int ensure_lowrank(LowRank& L, int nx, int ny, double h, double eps, cuda
     SCL_CU(cudaMemcpyAsync(lam.data(), dW, N * sizeof(double), cudaMemcpyDeviceToHost, s));
     SCL_CU(cudaMemcpyAsync(&hinfo, info, sizeof(int), cudaMemcpyDeviceToHost, s));
     SCL_CU(cudaStreamSynchronize(s));
-    cusolverDnDestroy(sol);
     if (hinfo != 0) { err = "cusolverDnDsyevd did not converge"; return 1; }
     // D9 (:1036): eigenvalues sorted by |lambda| descending; N* = smallest count with sqrt(1 - kept/total) < eps
     std::vector<int> ord(N); std::iota(ord.begin(), ord.end(), 0);
@@ -94,7 +96,6 @@ inline int ensure_lowrank(LowRank& L, int nx, int ny, double h, double eps, cuda
     SCL_LIB(cublasCreate(&L.blas)); SCL_LIB(cublasSetStream(L.blas, s));
     SCL_LIB(cublasSetMathMode(L.blas, CUBLAS_PEDANTIC_MATH));      // plain fp64 DGEMM, no reduced-precision paths
     SCL_CU(cudaStreamSynchronize(s));
-    cudaFree(dG); cudaFree(dW); cudaFree(work); cudaFree(info);
     L.ready = true;
     return 0;
 }
