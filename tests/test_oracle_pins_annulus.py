@@ -132,5 +132,14 @@ def test_eq48_london_bessel_profile_with_screening(alpha, wind):
     B_num = ((At_y[c, c + 1] - At_y[c, c - 1]) - (At_x[c + 1, c] - At_x[c - 1, c])) / (2 * H)
     B_an = _london(R_IN, alpha, wind, lam)[1]
     assert abs(B_num - B_an) < 0.04 * abs(B_an), (B_num, B_an)
+    # magnetic moment per unit thickness, Eq. 56 (:667) against Eq. 59-61 (:683-689): m = A (d_alpha alpha + d_n n) in units j0 xi0^3
+    m_num = 0.5 * H * H * float(np.sum((X * r["jy"] - Y * r["jx"])[mask > 0]))
+    A_ann, A_h = math.pi * (R_OUT ** 2 - R_IN ** 2), math.pi * R_IN ** 2
+    I2g, K2g, I2l, K2l = iv(2, R_OUT / lam), kv(2, R_OUT / lam), iv(2, R_IN / lam), kv(2, R_IN / lam)
+    M = iv(0, R_OUT / lam) * K2l - I2l * kv(0, R_OUT / lam)
+    d_alpha = math.pi * kappa ** 2 / A_ann * (A_ann + A_h) / (M * A_ann) * (I2l * K2g - I2g * K2l)        # Eq. 60, lambda_0 = kappa xi0
+    d_n = math.pi * kappa ** 2 / A_ann * (2 * math.pi * lam ** 2 / (M * A_h) - 1.0)                      # Eq. 61
+    m_an = A_ann * (d_alpha * alpha + d_n * wind)
+    assert abs(m_num - m_an) < 0.05 * abs(m_an) and m_num * (alpha + wind) < 0, (m_num, m_an)            # opposes n + alpha (Eq. 42): diamagnetic in a field, reversed for n = -1
     if wind == 0:
         assert 0 < B_num < Bext                                           # the ring screens part of the applied flux out of the hole
