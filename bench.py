@@ -54,17 +54,20 @@ STAGE_FP64 = {
     "T_pole_table_deg8": 36.0,  # stored-T rounds: degree 8, warp vote
     "moebius_step": 27.0,       # z g + De 4, N 4, z + conj(De) g 4, Q 4, |Q|^2 2, reciprocal 3, N conj(Q) / |Q|^2 6
     "node_products": 26.0,      # P 4, 1+P 1, |.|^2 2, reciprocal 3, 1/(1+P) 2, six summands 14 (unit weights)
-    "energy_reduction": 8.0,    # column sums of the transpose stage + running sum
+    "energy_reduction": 8.0,    # one energy per lane: column sums of the transpose stage + running sum
+    "energy_reduction_pairs": 7.0,  # two energies per lane: their six summands added in registers (3) + half the column sums (4)
 }
 def stage_counts(precision):
     """(least work per unit, executed per unit by round type) for the closed-form stepper"""
     T = STAGE_FP64["T_table_deg5" if precision == 64 else "T_table_deg3"]
     # least work: nothing evaluated twice — T once, gamma and gamma-tilde stepped once, products, reduction
-    least = T + 2 * STAGE_FP64["moebius_step"] + STAGE_FP64["node_products"] + STAGE_FP64["energy_reduction"]
-    # what the kernel executes: T in both passes, and every second gamma-tilde re-stepped in pass 2 instead of spilled
+    least = T + 2 * STAGE_FP64["moebius_step"] + STAGE_FP64["node_products"] + STAGE_FP64["energy_reduction_pairs"]
+    # what the kernel executes: T in both passes, and every second gamma-tilde re-stepped in pass 2 instead of spilled;
+    # rounds outside the pole-free table run one energy per lane (one more addition per unit in the reduction)
+    one = STAGE_FP64["energy_reduction"] - STAGE_FP64["energy_reduction_pairs"]
     executed = {"recompute": least + T + 0.5 * STAGE_FP64["moebius_step"],
-                "recompute_pole": least - T + 2 * STAGE_FP64["T_pole_table"] + 0.5 * STAGE_FP64["moebius_step"],
-                "stored": least - T + STAGE_FP64["T_pole_table_deg8"]}
+                "recompute_pole": least + one - T + 2 * STAGE_FP64["T_pole_table"] + 0.5 * STAGE_FP64["moebius_step"],
+                "stored": least + one - T + STAGE_FP64["T_pole_table_deg8"]}
     return least, executed
 
 
@@ -281,7 +284,7 @@ def march_roofline(a, wl, ctx, kernel, mk_ms, nl, units, step_ms, precision, ful
     r = {"bound": "alu", "kernel": "sck::" + kernel, "launches_timed": nl,
          "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
          "frac_basis": f"least-work count: {least_pu:.0f} fp{precision}-pipe instructions per unit (T once, two Moebius steps, node "
-                       "products, energy reduction; nothing evaluated twice) x units / march time (CUDA events around the march "
+                       "products, energy reduction with two energies per lane; nothing evaluated twice) x units / march time (CUDA events around the march "
                        "launches of the timed steps) / measured peak",
          "traffic": cap["dram_bytes"] if cap else None,
          "algorithmic_bytes_per_launch": hbm,

@@ -238,7 +238,8 @@ sck::MarchArgsT<R> march_args(sc_ctx* ctx, const EnergySet& E, const char* store
 
 template <int MODE, bool STATS, int STEP, typename R, int TM, bool UW = false>
 sc_status launch_march_t(sc_ctx* ctx, const sck::MarchArgsT<R>& A) {
-    const int blocks = ctx->n_slots / sck::MARCH_WARPS;
+    // persistent grid: one CTA per resident slot of this instantiation (n_slots is sized for the largest, MARCH_MIN_CTAS)
+    const int blocks = ctx->n_sm * sck::kMarchCtasPerSm<MODE, STATS, STEP, TM, UW>;
     const int smem = sck::march_smem<R>();
     // the opt-in to > 48 KB of dynamic shared memory is a per-device attribute of the function: remember it per context
     const void* fn = (const void*)sck::march_kernel<MODE, STATS, STEP, R, TM, UW>;

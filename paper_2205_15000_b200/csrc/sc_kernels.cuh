@@ -660,8 +660,221 @@ __device__ __forceinline__ void march_round(const MarchArgsT<R>& A, const WarpJo
     if (act) A.store_new[(size_t)J.dF * ne + n] = mk2(gm.re, gm.im);
 }
 
+// ---- TWO energies per lane (n0 + lane and n0 + 32 + lane) of one trajectory in one pass: the warp-uniform coefficient
+// loads, the loop bookkeeping, the shared-memory transpose and the running sums are shared by the two energies (their
+// six summands are added in registers before the stage), and the two independent dependency chains of a lane interleave.
+// Only the common case: Matsubara sums (MODE 0), closed-form step, every piece inside the pole-free table for all 64
+// energies, unit weights, no stats.  gamma~ of every second node is spilled as one 256-bit entry {gt(n), gt(n+32)}.
+template <typename R>
+__device__ __forceinline__ void node_terms(cplx_t<R> gm, cplx_t<R> gt, typename VT<R>::V2 Dn, R (&o)[6]) {
+    using scm::mad;
+    const R Pr = mad(gm.re, gt.re, -gm.im * gt.im), Pi = mad(gm.re, gt.im, gm.im * gt.re);
+    const R qr = R(1) + Pr;
+    const R rq = scm::rcp_nr(mad(qr, qr, Pi * Pi));
+    const R wr = qr * rq, wi = -Pi * rq;                      // 1/(1+P)
+    o[0] = mad(gm.re, wr, -gm.im * wi);                      // SF
+    o[1] = mad(gm.re, wi, gm.im * wr);
+    o[2] = mad(gt.re, wr, -gt.im * wi);                      // X2
+    o[3] = mad(gt.re, wi, gt.im * wr);
+    o[4] = wi + wi;                                          // SG
+    o[5] = mad(Dn.x, gm.im - gt.im, -Dn.y * (gm.re + gt.re));   // SI
+}
+
+template <typename R>
+__device__ __forceinline__ void march_round2(const MarchArgsT<R>& A, const WarpJob<R>& J, int n0) {
+    using V2 = typename VT<R>::V2; using V4 = typename VT<R>::V4;
+    using TAB = TTab<R, 1>;
+    constexpr int BYTES = 4 * (int)sizeof(R), ROW = 32 * BYTES;   // one entry = both energies' gamma~ of one node
+    constexpr int PFROWS = RED_NODES / 2;
+    const int lane = J.lane, nn = J.nn, ne = J.ne;
+    char* const scr = J.scr_w + lane * BYTES;
+    const bool pf_lane = lane * 128 < PFROWS * ROW;
+    const int na = n0 + lane, nb = n0 + 32 + lane;             // both < ne (whole double rounds only)
+    TAB ta, tb; ta.load(A.E, na); tb.load(A.E, nb);
+    const R zia = (R)A.E.zi[na], zib = (R)A.E.zi[nb];
+    const int pa = A.E.partner[na], pb = A.E.partner[nb];
+    const V4* __restrict__ PC = J.PC; const V2* __restrict__ ND = J.ND;
+    V4* const pcb = J.pcb; V2* const ndb = J.ndb;
+    const int npart = nn * RED_VALS;
+
+    // ---------------- pass 1: gamma-tilde from u_out down to u_in ----------------
+    const int ctop = nn >> 5;
+    if (ctop * CHUNK + lane <= nn) cp_async<sizeof(V4)>(pcb + (ctop & 1) * CHUNK + lane, PC + ctop * CHUNK + lane);
+    cp_commit();
+    cplx_t<R> gta, gtb;
+    if (A.bc_mode == 1) {
+        const V4 c4 = ldu(PC + nn);
+        gta = hom_start<R>(-(double)c4.x, c4.y, A.E.zr[na] + c4.z, A.E.zi[na]);
+        gtb = hom_start<R>(-(double)c4.x, c4.y, A.E.zr[nb] + c4.z, A.E.zi[nb]);
+    } else if (A.ga_n[J.dB]) {
+        const cplx_t<R> sa = gather_start(A, J.dB, pa), sb = gather_start(A, J.dB, pb);
+        gta = mk(sa.re, -sa.im); gtb = mk(sb.re, -sb.im);
+    } else {
+        const cplx_t<R> sa = hom_start<R>(A.fb_D[J.dB].x, A.fb_D[J.dB].y, A.E.zr[pa] + A.fb_a[J.dB], A.E.zi[pa]);
+        const cplx_t<R> sb = hom_start<R>(A.fb_D[J.dB].x, A.fb_D[J.dB].y, A.E.zr[pb] + A.fb_a[J.dB], A.E.zi[pb]);
+        gta = mk(sa.re, -sa.im); gtb = mk(sb.re, -sb.im);
+    }
+    cplx_t<R> T0a = mk(R(0), R(0)), T0b = T0a;
+    {
+        char* e = scr + (size_t)((nn - 1) >> 1) * ROW;
+        int p = nn;
+        for (int c = ctop; c >= 0; --c) {
+            if (c > 0) {
+                cp_async<sizeof(V4)>(pcb + ((c - 1) & 1) * CHUNK + lane, PC + (c - 1) * CHUNK + lane);
+                cp_commit();
+                cp_wait<1>();
+            } else {
+                cp_wait<0>();
+            }
+            __syncwarp();
+            const V4* __restrict__ buf = pcb + (c & 1) * CHUNK;
+            const int plo = max(c * CHUNK, 1);
+            if (p == nn) {                                      // exit piece (length l1); the last node is always spilled
+                const V4 cc = buf[p & (CHUNK - 1)];
+                const cplx_t<R> Ta = end_T<R>(cc, R(0), zia, J.len1), Tb = end_T<R>(cc, R(0), zib, J.len1);
+                gta = scm::step_T(gta, -cc.x, cc.y, cc.z, zia, Ta);
+                gtb = scm::step_T(gtb, -cc.x, cc.y, cc.z, zib, Tb);
+                st_ent<true>(e, gta, gtb);
+                e -= ROW; --p;
+            }
+            const V4* __restrict__ bp = buf + (p & (CHUNK - 1));
+#pragma unroll 2
+            for (; p >= plo; --p, --bp) {
+                const V4 cc = *bp;
+                const cplx_t<R> Ta = ta.fast(cc), Tb = tb.fast(cc);
+                gta = scm::step_T(gta, -cc.x, cc.y, cc.z, zia, Ta);
+                gtb = scm::step_T(gtb, -cc.x, cc.y, cc.z, zib, Tb);
+                if (!(p & 1)) { st_ent<true>(e, gta, gtb); e -= ROW; }      // landed on the odd node p-1: row (p-1)>>1
+            }
+            if (c == 0) {                                       // entry piece (length l0)
+                const V4 cc = buf[0];
+                T0a = end_T<R>(cc, R(0), zia, J.len0); T0b = end_T<R>(cc, R(0), zib, J.len0);
+                gta = scm::step_T(gta, -cc.x, cc.y, cc.z, zia, T0a);
+                gtb = scm::step_T(gtb, -cc.x, cc.y, cc.z, zib, T0b);
+            }
+            __syncwarp();
+        }
+        A.store_new[(size_t)J.dB * ne + pa] = mk2(gta.re, -gta.im);
+        A.store_new[(size_t)J.dB * ne + pb] = mk2(gtb.re, -gtb.im);
+    }
+
+    // ---------------- pass 2: gamma from u_in up to u_out; products and energy reduction ------------
+    const int nchunk = (nn + CHUNK - 1) >> 5;
+    cplx_t<R> ga, gb;
+    {
+        const V4 c0 = pcb[0];
+        __syncwarp();
+        if (lane < nn) {
+            cp_async<sizeof(V4)>(pcb + CHUNK + lane, PC + 1 + lane);
+            cp_async<sizeof(V2)>(ndb + CHUNK + lane, ND + lane);
+        }
+        cp_commit();
+        if (A.bc_mode == 1) {
+            ga = hom_start<R>(c0.x, c0.y, A.E.zr[na] + c0.z, A.E.zi[na]);
+            gb = hom_start<R>(c0.x, c0.y, A.E.zr[nb] + c0.z, A.E.zi[nb]);
+        } else if (A.ga_n[J.dF]) {
+            ga = gather_start(A, J.dF, na); gb = gather_start(A, J.dF, nb);
+        } else {
+            ga = hom_start<R>(A.fb_D[J.dF].x, A.fb_D[J.dF].y, A.E.zr[na] + A.fb_a[J.dF], A.E.zi[na]);
+            gb = hom_start<R>(A.fb_D[J.dF].x, A.fb_D[J.dF].y, A.E.zr[nb] + A.fb_a[J.dF], A.E.zi[nb]);
+        }
+        ga = scm::step_T(ga, c0.x, c0.y, c0.z, zia, T0a);
+        gb = scm::step_T(gb, c0.x, c0.y, c0.z, zib, T0b);
+    }
+    const char* e = scr;                         // entry of nodes 0 / 1
+    for (int q = RED_NODES; q < PF_DIST && q < nn; q += RED_NODES)
+        if (pf_lane) prefetch_l2(J.scr_w + (size_t)(q >> 1) * ROW + lane * 128);
+    Ent<R> En = ld_ent<true>(e, R(0)), En2 = ld_ent<true>(e + ROW, R(0));      // {gt_a, gt_b} of the next two spilled nodes
+    cplx_t<R> oa = mk(R(0), R(0)), ob = oa;      // gamma~ of the odd node, held from the even node before it
+    double part_nxt = 0.0;
+    if (n0 && lane < RED_NODES * RED_VALS && lane < npart) part_nxt = J.PART[lane];
+    int m = 0;
+    auto node = [&](int b, const V4* pbuf, const V2* dbuf, bool exitp) {
+        const V4 cc = pbuf[b]; const V2 dc = dbuf[b];
+        const R len = exitp ? J.len1 : J.hlen;
+        const cplx_t<R> Ta = exitp ? end_T<R>(cc, R(0), zia, len) : ta.fast(cc);
+        const cplx_t<R> Tb = exitp ? end_T<R>(cc, R(0), zib, len) : tb.fast(cc);
+        cplx_t<R> ha = oa, hb = ob;
+        if (!(b & 1)) {
+            const cplx_t<R> Ga = mk(En.tr, En.ti), Gb = mk(En.gr, En.gi);      // entry (m+b)>>1: node m+b+1, or the last node itself
+            En = En2; En2 = ld_ent<true>(e + ((b >> 1) + 2) * ROW, R(0));
+            oa = Ga; ob = Gb;
+            ha = exitp ? Ga : scm::step_T(Ga, -cc.x, cc.y, cc.z, zia, Ta);
+            hb = exitp ? Gb : scm::step_T(Gb, -cc.x, cc.y, cc.z, zib, Tb);
+        }
+        R sa[6], sb[6];
+        node_terms<R>(ga, ha, dc, sa); node_terms<R>(gb, hb, dc, sb);
+        R* st = J.stage + b * RED_VALS * STAGE_LD + lane;
+#pragma unroll
+        for (int v = 0; v < 6; ++v) st[v * STAGE_LD] = sa[v] + sb[v];
+        ga = scm::step_T(ga, cc.x, cc.y, cc.z, zia, Ta);
+        gb = scm::step_T(gb, cc.x, cc.y, cc.z, zib, Tb);
+    };
+    for (int c = 0; c < nchunk; ++c) {
+        const int bsel = (c + 1) & 1;
+        if (c + 1 < nchunk) {
+            const int q = (c + 1) * CHUNK + lane;
+            if (q < nn) {
+                cp_async<sizeof(V4)>(pcb + (bsel ^ 1) * CHUNK + lane, PC + 1 + q);
+                cp_async<sizeof(V2)>(ndb + (bsel ^ 1) * CHUNK + lane, ND + q);
+            }
+            cp_commit();
+            cp_wait<1>();
+        } else {
+            cp_wait<0>();
+        }
+        __syncwarp();
+        const V4* __restrict__ pbuf = pcb + bsel * CHUNK;
+        const V2* __restrict__ dbuf = ndb + bsel * CHUNK;
+        const int mhi = min(nn, (c + 1) * CHUNK);
+        for (; m + RED_NODES <= mhi; m += RED_NODES) {
+            if (pf_lane && m + PF_DIST < nn) prefetch_l2(J.scr_w + (size_t)((m + PF_DIST) >> 1) * ROW + lane * 128);
+            const double part_old = part_nxt;
+            if (n0 && lane < RED_NODES * RED_VALS && (m + RED_NODES) * RED_VALS + lane < npart)
+                part_nxt = J.PART[(m + RED_NODES) * RED_VALS + lane];
+            const V4* __restrict__ pb = pbuf + (m & (CHUNK - 1)); const V2* __restrict__ db = dbuf + (m & (CHUNK - 1));
+            if (m + RED_NODES < nn) {
+#pragma unroll
+                for (int b = 0; b < RED_NODES; ++b) node(b, pb, db, false);
+            } else {
+#pragma unroll
+                for (int b = 0; b < RED_NODES; ++b) node(b, pb, db, b == RED_NODES - 1);
+            }
+            e += PFROWS * ROW;
+            __syncwarp();
+            if (lane < RED_NODES * RED_VALS) {
+                double s = stage_colsum(J.stage, lane);
+                if (n0) s += part_old;
+                J.PART[m * RED_VALS + lane] = s;
+            }
+            __syncwarp();
+        }
+        if (m < mhi) {                                       // ragged tail: 1..3 nodes (last chunk only)
+            const int rem = mhi - m;
+            const double part_old = part_nxt;
+            for (int b = 0; b < rem; ++b) node(b, pbuf + (m & (CHUNK - 1)), dbuf + (m & (CHUNK - 1)), m + b + 1 == nn);
+            __syncwarp();
+            if (lane < rem * RED_VALS) {
+                double s = stage_colsum(J.stage, lane);
+                if (n0) s += part_old;
+                J.PART[m * RED_VALS + lane] = s;
+            }
+            __syncwarp();
+            m = mhi;
+        }
+        __syncwarp();
+    }
+    A.store_new[(size_t)J.dF * ne + na] = mk2(ga.re, ga.im);
+    A.store_new[(size_t)J.dF * ne + nb] = mk2(gb.re, gb.im);
+}
+
+// The plain Matsubara sweep (MODE 0, closed-form step, imaginary-axis energies, unit weights, no stats) marches two
+// energies per lane (march_round2): 232 registers per thread, one CTA of 8 warps per SM.
+constexpr int E2_MIN_CTAS = 1;
+template <int MODE, bool STATS, int STEP, int TM, bool UW> constexpr bool kTwoEnergies = MODE == 0 && !STATS && STEP == 0 && TM == 1 && UW;
+template <int MODE, bool STATS, int STEP, int TM, bool UW> constexpr int kMarchCtasPerSm = kTwoEnergies<MODE, STATS, STEP, TM, UW> ? E2_MIN_CTAS : MARCH_MIN_CTAS;
 template <int MODE, bool STATS, int STEP, typename R, int TM, bool UW = false>
-__global__ void __launch_bounds__(MARCH_WARPS * 32, MARCH_MIN_CTAS) march_kernel(MarchArgsT<R> A) {
+__global__ void __launch_bounds__(MARCH_WARPS * 32, (kMarchCtasPerSm<MODE, STATS, STEP, TM, UW>)) march_kernel(MarchArgsT<R> A) {
     using V2 = typename VT<R>::V2; using V4 = typename VT<R>::V4;
     extern __shared__ double4 smem_raw[];
     WarpJob<R> J;
@@ -690,6 +903,15 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32, MARCH_MIN_CTAS) march_kernel
         const float2 pm = A.pmax[g];
 
         for (int n0 = 0; n0 < J.ne; n0 += 32) {
+            if constexpr (kTwoEnergies<MODE, STATS, STEP, TM, UW>) {
+                // a whole double round inside the pole-free table: both energies of every lane in one pass
+                if (n0 + 64 <= J.ne &&
+                    !__any_sync(0xffffffffu, !TTab<R, 1>::covers(A.E, n0 + J.lane, pm) || !TTab<R, 1>::covers(A.E, n0 + 32 + J.lane, pm))) {
+                    march_round2<R>(A, J, n0);
+                    n0 += 32;
+                    continue;
+                }
+            }
             const int n = min(n0 + J.lane, J.ne - 1);
             // STEP 0: T is re-evaluated in pass 2 if every piece is inside a table's radius for all 32 lanes, else spilled
             if (STEP == 0 && __any_sync(0xffffffffu, !TTab<R, TM>::covers(A.E, n, pm))) {
