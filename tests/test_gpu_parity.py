@@ -357,6 +357,13 @@ def test_tiny_and_thin_grains(sc):
         A = 0.05 * rng.uniform(-1, 1, (ny, nx))
         wl = wlmod.Workload("tiny", -1, nx, ny, h, shapes, mask, wlmod.SYM_DXY, 0.05, 12, 5, 0.4, -1.0, -1, d0, A, -A, 0.25)
         compare_sweeps(sc, wl, n_sweeps=2)
+        # the same grains through the two-energies-per-lane rounds (trajectories of 1, 2, 3 ... nodes: every ragged tail of a
+        # reduction batch, odd and even node counts for the half spill): 64 energies = one double round; 96 = a double round
+        # followed by a single one; 160 = two double rounds and a single one (running sums across rounds of both kinds)
+        for ne in (64, 96, 160):
+            wl2 = wlmod.Workload("tiny", -1, nx, ny, h, shapes, mask, wlmod.SYM_DXY, 0.05, 12, ne, 0.4, -1.0, -1, d0, A, -A, 0.25)
+            o, g, _, _ = compare_sweeps(sc, wl2, n_sweeps=2, stats=False)
+            assert g.ctx.sc_debug_last_march_variant() == BENCH_KERNEL[64]
 
 
 def test_repeat_sweeps_are_bitwise_deterministic(sc):
