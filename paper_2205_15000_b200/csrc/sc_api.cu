@@ -822,8 +822,8 @@ sc_status sc_debug_partial(sc_ctx* ctx, int k, void* SF, double* SG, double* SI)
         for (int m = 0; m < ctx->h_nn[g]; ++m) {
             const double* v = &buf[(size_t)(ctx->h_noff[g] - n0 + m) * sck::RED_VALS];
             int t = ctx->h_t[g], j = ctx->h_jf[g] + m;
-            if (k < H) { const size_t q = (size_t)t * NR + j; sf[2 * q] = v[0]; sf[2 * q + 1] = v[1]; SG[q] = v[4]; SI[q] = v[5]; }
-            else { const size_t q = (size_t)(NR - 1 - t) * NR + (NR - 1 - j); sf[2 * q] = v[2]; sf[2 * q + 1] = -v[3]; SG[q] = -v[4]; SI[q] = v[5]; }
+            if (k < H) { const size_t q = (size_t)t * NR + j; sf[2 * q] = v[0]; sf[2 * q + 1] = v[1]; SG[q] = 2.0 * v[4]; SI[q] = v[5]; }
+            else { const size_t q = (size_t)(NR - 1 - t) * NR + (NR - 1 - j); sf[2 * q] = v[2]; sf[2 * q + 1] = -v[3]; SG[q] = -2.0 * v[4]; SI[q] = v[5]; }
         }
     return SC_OK;
 }

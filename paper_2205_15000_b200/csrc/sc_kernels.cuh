@@ -214,7 +214,7 @@ struct MarchArgsT {
     const double2* fb_D; const double* fb_a;
     const V2* store_old; V2* store_new;
     char* scr; long long scr_stride;        // per warp slot: scr_stride bytes = (smax+2) rows of 32 entries of 4 R
-    double* part;                           // MODE 0: [node][6] = SF.re, SF.im, X2.re, X2.im, SG, SI
+    double* part;                           // MODE 0: [node][6] = SF.re, SF.im, X2.re, X2.im, SG/2, SI
     double* ldos;                           // MODE 1: [node][ne] = Re g_n
     int* counter;
     double* stat_max2;                      // per warp slot: max |gamma|^2 seen (optional)
@@ -275,7 +275,7 @@ __device__ __forceinline__ R node_products(cplx_t<R> gm, R gtr, R gti, typename 
         st[1 * STAGE_LD] = mad(gm.re, wi, gm.im * wr);
         st[2 * STAGE_LD] = mad(gtr, wr, -gti * wi);          // X2  = w gamma~/(1+P)  (SF of k+N/2 = conj)
         st[3 * STAGE_LD] = mad(gtr, wi, gti * wr);
-        st[4 * STAGE_LD] = wi + wi;                          // SG  = w Im g = 2 w Im 1/(1+P)
+        st[4 * STAGE_LD] = wi;                               // SG/2 = w Im 1/(1+P) (Im g = 2 Im 1/(1+P): doubled in rotate-back)
         const R si = mad(Dn.x, gm.im - gti, -Dn.y * (gm.re + gtr));
         st[5 * STAGE_LD] = UW ? si : wn * si;   // SI (Eq. 19 :128 numerator)
     }
@@ -676,8 +676,24 @@ __device__ __forceinline__ void node_terms(cplx_t<R> gm, cplx_t<R> gt, typename 
     o[1] = mad(gm.re, wi, gm.im * wr);
     o[2] = mad(gt.re, wr, -gt.im * wi);                      // X2
     o[3] = mad(gt.re, wi, gt.im * wr);
-    o[4] = wi + wi;                                          // SG
+    o[4] = wi;                                               // SG/2 (doubled in rotate-back)
     o[5] = mad(Dn.x, gm.im - gt.im, -Dn.y * (gm.re + gt.re));   // SI
+}
+
+// the same six terms of a second energy, accumulated onto o (each sum rides on the last FMA of its term)
+template <typename R>
+__device__ __forceinline__ void node_terms_acc(cplx_t<R> gm, cplx_t<R> gt, typename VT<R>::V2 Dn, R (&o)[6]) {
+    using scm::mad;
+    const R Pr = mad(gm.re, gt.re, -gm.im * gt.im), Pi = mad(gm.re, gt.im, gm.im * gt.re);
+    const R qr = R(1) + Pr;
+    const R rq = scm::rcp_nr(mad(qr, qr, Pi * Pi));
+    const R wr = qr * rq, wi = -Pi * rq;
+    o[0] = mad(gm.re, wr, mad(-gm.im, wi, o[0]));
+    o[1] = mad(gm.re, wi, mad(gm.im, wr, o[1]));
+    o[2] = mad(gt.re, wr, mad(-gt.im, wi, o[2]));
+    o[3] = mad(gt.re, wi, mad(gt.im, wr, o[3]));
+    o[4] += wi;
+    o[5] = mad(Dn.x, gm.im - gt.im, mad(-Dn.y, gm.re + gt.re, o[5]));
 }
 
 template <typename R>
@@ -802,11 +818,11 @@ __device__ __forceinline__ void march_round2(const MarchArgsT<R>& A, const WarpJ
             ha = exitp ? Ga : scm::step_T(Ga, -cc.x, cc.y, cc.z, zia, Ta);
             hb = exitp ? Gb : scm::step_T(Gb, -cc.x, cc.y, cc.z, zib, Tb);
         }
-        R sa[6], sb[6];
-        node_terms<R>(ga, ha, dc, sa); node_terms<R>(gb, hb, dc, sb);
+        R sa[6];
+        node_terms<R>(ga, ha, dc, sa); node_terms_acc<R>(gb, hb, dc, sa);
         R* st = J.stage + b * RED_VALS * STAGE_LD + lane;
 #pragma unroll
-        for (int v = 0; v < 6; ++v) st[v * STAGE_LD] = sa[v] + sb[v];
+        for (int v = 0; v < 6; ++v) st[v * STAGE_LD] = sa[v];
         ga = scm::step_T(ga, cc.x, cc.y, cc.z, zia, Ta);
         gb = scm::step_T(gb, cc.x, cc.y, cc.z, zib, Tb);
     };
@@ -1046,7 +1062,7 @@ __global__ void __launch_bounds__(BACK_TX * BACK_TY) rotate_back_kernel(BackArgs
                     nr[c] += Wk * ek * f0 + Wk2 * ek2 * f2;
                     ni[c] += Wk * ek * f1 - Wk2 * ek2 * f3;
                 }
-            const double wj = (Wk + Wk2) * f4;
+            const double wj = 2.0 * (Wk + Wk2) * f4;        // f4 = sum of Im 1/(1+P); Im g = 2 Im 1/(1+P)
             sjx = fma(wj, B.vx[p], sjx); sjy = fma(wj, B.vy[p], sjy);
             sI += (Wk + Wk2) * f5;
         }
