@@ -53,21 +53,26 @@ STAGE_FP64 = {
     "T_pole_table": 24.0,       # pole term (one reciprocal) + degree-5 remainder
     "T_pole_table_deg8": 36.0,  # stored-T rounds: degree 8, warp vote
     "moebius_step": 27.0,       # z g + De 4, N 4, z + conj(De) g 4, Q 4, |Q|^2 2, reciprocal 3, N conj(Q) / |Q|^2 6
-    "node_products": 26.0,      # P 4, 1+P 1, |.|^2 2, reciprocal 3, 1/(1+P) 2, six summands 14 (unit weights)
+    "node_products": 25.0,      # one energy per lane: P 4, 1+P 1, |.|^2 2, reciprocal 3, 1/(1+P) 2, SF 4, X2 4, SG 1 (weight), SI 4
+    "node_products_pairs": 24.0,  # two energies per lane, per unit: the same without the SG instruction; the second energy's terms are
+                                  # accumulated onto the first's by the last FMA of each term (no separate additions)
     "energy_reduction": 8.0,    # one energy per lane: column sums of the transpose stage + running sum
-    "energy_reduction_pairs": 7.0,  # two energies per lane: their six summands added in registers (3) + half the column sums (4)
+    "energy_reduction_pairs": 4.5,  # two energies per lane: SG addition 0.5 + half the column sums and running sum 4
 }
+ROUND1_LEAST_WORK = 103.0       # the count round 1's fraction (0.556) was quoted on: kept beside `frac` for comparison
+
+
 def stage_counts(precision):
     """(least work per unit, executed per unit by round type) for the closed-form stepper"""
     T = STAGE_FP64["T_table_deg5" if precision == 64 else "T_table_deg3"]
-    # least work: nothing evaluated twice — T once, gamma and gamma-tilde stepped once, products, reduction
-    least = T + 2 * STAGE_FP64["moebius_step"] + STAGE_FP64["node_products"] + STAGE_FP64["energy_reduction_pairs"]
+    # least work: nothing evaluated twice — T once, gamma and gamma-tilde stepped once, products, reduction (two energies per lane)
+    least = T + 2 * STAGE_FP64["moebius_step"] + STAGE_FP64["node_products_pairs"] + STAGE_FP64["energy_reduction_pairs"]
     # what the kernel executes: T in both passes, and every second gamma-tilde re-stepped in pass 2 instead of spilled;
-    # rounds outside the pole-free table run one energy per lane (one more addition per unit in the reduction)
-    one = STAGE_FP64["energy_reduction"] - STAGE_FP64["energy_reduction_pairs"]
+    # rounds outside the pole-free table run one energy per lane
+    one = least + (STAGE_FP64["node_products"] - STAGE_FP64["node_products_pairs"]) + (STAGE_FP64["energy_reduction"] - STAGE_FP64["energy_reduction_pairs"])
     executed = {"recompute": least + T + 0.5 * STAGE_FP64["moebius_step"],
-                "recompute_pole": least + one - T + 2 * STAGE_FP64["T_pole_table"] + 0.5 * STAGE_FP64["moebius_step"],
-                "stored": least + one - T + STAGE_FP64["T_pole_table_deg8"]}
+                "recompute_pole": one - T + 2 * STAGE_FP64["T_pole_table"] + 0.5 * STAGE_FP64["moebius_step"],
+                "stored": one - T + STAGE_FP64["T_pole_table_deg8"]}
     return least, executed
 
 
@@ -283,9 +288,10 @@ def march_roofline(a, wl, ctx, kernel, mk_ms, nl, units, step_ms, precision, ful
     achieved = 2.0 * least / sec / 1e12
     r = {"bound": "alu", "kernel": "sck::" + kernel, "launches_timed": nl,
          "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-         "frac_basis": f"least-work count: {least_pu:.0f} fp{precision}-pipe instructions per unit (T once, two Moebius steps, node "
+         "frac_basis": f"least-work count: {least_pu:.1f} fp{precision}-pipe instructions per unit (T once, two Moebius steps, node "
                        "products, energy reduction with two energies per lane; nothing evaluated twice) x units / march time (CUDA events around the march "
                        "launches of the timed steps) / measured peak",
+         "frac_on_round1_count": 2.0 * ROUND1_LEAST_WORK * u_all / sec / 1e12 / peak if (precision == 64 and a.stepper == 0) else None,
          "traffic": cap["dram_bytes"] if cap else None,
          "algorithmic_bytes_per_launch": hbm,
          "peak_kind": peak_kind, "peak_burst": burst, "peak_sustained": sustained,
@@ -444,7 +450,7 @@ def run_ours(a):
     if a.issue_probe:
         ctx = sc.ScContext.from_workload(workloads.make_workload(0), device=local)
         names = {10: "DFMA only", 11: "+ 0.5 integer per DFMA", 12: "+ 1 integer per DFMA", 13: "+ 0.125 LDS (and its DADD) per DFMA",
-                 14: "+ 0.375 integer + 0.125 LDS (and its DADD) per DFMA"}
+                 14: "+ 0.375 integer + 0.125 LDS (and its DADD) per DFMA", 15: "DFMA only, three different changing register operands"}
         base = ctx.sc_debug_pipe_peak(10, 1.0)
         print(json.dumps({"issue_probe": {names[k]: {"dfma_tflops": 2e-12 * v, "of_dfma_only": v / base}
                                           for k, v in ((k, ctx.sc_debug_pipe_peak(k, 1.0)) for k in names)}}))

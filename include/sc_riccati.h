@@ -202,7 +202,8 @@ sc_status sc_debug_fp64_peak_sustained(sc_ctx* ctx, double seconds, double* dfma
  * instructions per second over the whole device.  Pipes 10-14 run the DFMA loop with other instructions mixed in and
  * return DFMA per second: 10 = DFMA only, 11 = + 0.5 integer instruction per DFMA, 12 = + 1 integer, 13 = + 0.125
  * shared-memory load (and its DADD), 14 = + 0.375 integer + 0.125 shared-memory load — what the non-FP64 instructions of
- * the march cost next to half-rate DFMA. */
+ * the march cost next to half-rate DFMA; 15 = DFMA only, but with three different, changing register operands per instruction
+ * (DESIGN.md §6). */
 sc_status sc_debug_pipe_peak(sc_ctx* ctx, int pipe, double seconds, double* ops_per_s);
 
 /* Device time of the most recent march kernel launch (CUDA events recorded on the stream around that launch

@@ -968,7 +968,7 @@ sc_status sc_debug_fp64_peak_sustained(sc_ctx* ctx, double seconds, double* dfma
 }
 
 sc_status sc_debug_pipe_peak(sc_ctx* ctx, int pipe, double seconds, double* ops_per_s) {
-    if (!ctx || !ops_per_s || pipe < 1 || (pipe > 3 && pipe < 10) || pipe > 14 || !(seconds > 0) || seconds > 30) return fail(ctx, SC_ERR_ARG, "bad argument");
+    if (!ctx || !ops_per_s || pipe < 1 || (pipe > 3 && pipe < 10) || pipe > 15 || !(seconds > 0) || seconds > 30) return fail(ctx, SC_ERR_ARG, "bad argument");
     ON_DEVICE(ctx);
     DevBuf<float> d; CU(d.alloc(2));
     const int blocks = ctx->n_sm * 4, threads = 256;
@@ -983,7 +983,8 @@ sc_status sc_debug_pipe_peak(sc_ctx* ctx, int pipe, double seconds, double* ops_
         else if (pipe == 11) sck::fp64_mix_kernel<4, 0><<<blocks, threads, 0, ctx->stream>>>(iters, (double*)d.p);
         else if (pipe == 12) sck::fp64_mix_kernel<8, 0><<<blocks, threads, 0, ctx->stream>>>(iters, (double*)d.p);
         else if (pipe == 13) sck::fp64_mix_kernel<0, 1><<<blocks, threads, 0, ctx->stream>>>(iters, (double*)d.p);
-        else sck::fp64_mix_kernel<3, 1><<<blocks, threads, 0, ctx->stream>>>(iters, (double*)d.p);
+        else if (pipe == 14) sck::fp64_mix_kernel<3, 1><<<blocks, threads, 0, ctx->stream>>>(iters, (double*)d.p);
+        else sck::fp64_operand_kernel<<<blocks, threads, 0, ctx->stream>>>(iters, (double*)d.p);
     };
     launch();
     CU(cudaEventRecord(ctx->ev0, ctx->stream));

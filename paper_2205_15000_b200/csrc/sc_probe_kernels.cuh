@@ -41,4 +41,22 @@ __global__ void __launch_bounds__(256) fp64_mix_kernel(int iters, double* sink) 
     if (s == 123.456 || (x0 ^ x1 ^ x2 ^ x3) == 0x12345) sink[0] = s;
 }
 
+// DFMA whose three source operands are all different registers that change from instruction to instruction (the march's
+// DFMAs look like this; the peak loop above re-uses two constant operands): 8 chains a_i <- a_i * b_j + c_k with rotating j, k.
+__global__ void __launch_bounds__(256) fp64_operand_kernel(int iters, double* sink) {
+    double a[8], b[8], c[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { a[i] = threadIdx.x * 1e-9 + i; b[i] = 0.999999 - 1e-9 * i; c[i] = 1e-7 * (i + 1); }
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+#pragma unroll
+            for (int i = 0; i < 8; ++i) a[i] = fma(a[i], b[(i + u) & 7], c[(i + 3 * u + 1) & 7]);
+    }
+    double s = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += a[i];
+    if (s == 123.456) sink[0] = s;
+}
+
 }  // namespace sck
