@@ -696,10 +696,9 @@ __device__ __forceinline__ void node_terms_acc(cplx_t<R> gm, cplx_t<R> gt, typen
     o[5] = mad(Dn.x, gm.im - gt.im, mad(-Dn.y, gm.re + gt.re, o[5]));
 }
 
-template <typename R>
+template <typename R, typename TAB>
 __device__ __forceinline__ void march_round2(const MarchArgsT<R>& A, const WarpJob<R>& J, int n0) {
     using V2 = typename VT<R>::V2; using V4 = typename VT<R>::V4;
-    using TAB = TTab<R, 1>;
     constexpr int BYTES = 4 * (int)sizeof(R), ROW = 32 * BYTES;   // one entry = both energies' gamma~ of one node
     constexpr int PFROWS = RED_NODES / 2;
     const int lane = J.lane, nn = J.nn, ne = J.ne;
@@ -885,7 +884,8 @@ __device__ __forceinline__ void march_round2(const MarchArgsT<R>& A, const WarpJ
 }
 
 // The plain Matsubara sweep (MODE 0, closed-form step, imaginary-axis energies, unit weights, no stats) marches two
-// energies per lane (march_round2): 232 registers per thread, one CTA of 8 warps per SM.
+// energies per lane (march_round2, with the pole-free or the pole-subtracted table): 240 registers per thread, one CTA of
+// 8 warps per SM.
 constexpr int E2_MIN_CTAS = 1;
 template <int MODE, bool STATS, int STEP, int TM, bool UW> constexpr bool kTwoEnergies = MODE == 0 && !STATS && STEP == 0 && TM == 1 && UW;
 template <int MODE, bool STATS, int STEP, int TM, bool UW> constexpr int kMarchCtasPerSm = kTwoEnergies<MODE, STATS, STEP, TM, UW> ? E2_MIN_CTAS : MARCH_MIN_CTAS;
@@ -921,11 +921,21 @@ __global__ void __launch_bounds__(MARCH_WARPS * 32, (kMarchCtasPerSm<MODE, STATS
         for (int n0 = 0; n0 < J.ne; n0 += 32) {
             if constexpr (kTwoEnergies<MODE, STATS, STEP, TM, UW>) {
                 // a whole double round inside the pole-free table: both energies of every lane in one pass
-                if (n0 + 64 <= J.ne &&
-                    !__any_sync(0xffffffffu, !TTab<R, 1>::covers(A.E, n0 + J.lane, pm) || !TTab<R, 1>::covers(A.E, n0 + 32 + J.lane, pm))) {
-                    march_round2<R>(A, J, n0);
-                    n0 += 32;
-                    continue;
+                if (n0 + 64 <= J.ne) {
+                    const int na = n0 + J.lane, nb = n0 + 32 + J.lane;
+                    if (!__any_sync(0xffffffffu, !TTab<R, 1>::covers(A.E, na, pm) || !TTab<R, 1>::covers(A.E, nb, pm))) {
+                        march_round2<R, TTab<R, 1>>(A, J, n0);
+                        n0 += 32;
+                        continue;
+                    }
+                    // beyond the pole-free table but inside the pole-subtracted one: the same double round with that table
+                    using Short = TTabPole<R, scm::TaylorPoleShortK<R>>;
+                    if (!__any_sync(0xffffffffu, !Short::covers(A.E, na, pm) || !Short::covers(A.E, nb, pm))) {
+                        march_round2<R, Short>(A, J, n0);
+                        npl += (unsigned long long)(J.nn + 1) * 64;
+                        n0 += 32;
+                        continue;
+                    }
                 }
             }
             const int n = min(n0 + J.lane, J.ne - 1);
