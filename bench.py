@@ -68,10 +68,10 @@ def stage_counts(precision):
     # least work: nothing evaluated twice — T once, gamma and gamma-tilde stepped once, products, reduction (two energies per lane)
     least = T + 2 * STAGE_FP64["moebius_step"] + STAGE_FP64["node_products_pairs"] + STAGE_FP64["energy_reduction_pairs"]
     # what the kernel executes: T in both passes, and every second gamma-tilde re-stepped in pass 2 instead of spilled;
-    # rounds outside the pole-free table run one energy per lane
+    # stored-T rounds run one energy per lane
     one = least + (STAGE_FP64["node_products"] - STAGE_FP64["node_products_pairs"]) + (STAGE_FP64["energy_reduction"] - STAGE_FP64["energy_reduction_pairs"])
     executed = {"recompute": least + T + 0.5 * STAGE_FP64["moebius_step"],
-                "recompute_pole": one - T + 2 * STAGE_FP64["T_pole_table"] + 0.5 * STAGE_FP64["moebius_step"],
+                "recompute_pole": least - T + 2 * STAGE_FP64["T_pole_table"] + 0.5 * STAGE_FP64["moebius_step"],
                 "stored": one - T + STAGE_FP64["T_pole_table_deg8"]}
     return least, executed
 
