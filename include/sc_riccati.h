@@ -168,6 +168,23 @@ sc_status sc_iterate(sc_ctx* ctx, int accelerator, double step, int burnin, void
 sc_status sc_set_accelerator_params(sc_ctx* ctx, double drag, double step_factor, double cos_similarity_min,
                                     double step_min, double step_max);
 
+/* The residual of Eq. 27 (:201), ||x_new - x_old||_p / ||x_old||_p over n complex fp64 elements (the res_delta of
+ * sc_iterate for x = Delta), for callers that may not allocate: code under CUDA graph capture, tight serving loops.
+ * It needs no context and calls no cudaMalloc / cudaFree or allocating library routine: the partial sums of its
+ * reduction live in a static device array of the library (64.25 KiB, held by every GPU that loads the library until
+ * exit), which bounds the size: n <= SC_RESIDUAL_STATIC_MAX_ELEMENTS, beyond that SC_ERR_ARG.
+ *   x_new, x_old  dev, complex fp64 [n] (caller-owned, read only)
+ *   norm_p        2 (0 = default), 1, or -1 = maximum norm, as opts.residual_norm
+ *   out           dev fp64 [3] (caller-owned): ||x_new - x_old||_p, ||x_old||_p, their ratio (the numerator if x_old = 0)
+ *   device        CUDA device ordinal, made current; < 0 = the calling thread's current device
+ *   cuda_stream   cudaStream_t the work (one 8-byte memset + one kernel) is enqueued on; no host synchronisation
+ *   err, err_len  host buffer for the message of a non-zero status (may be NULL)
+ * The first call on a device looks the array's address up (cudaGetSymbolAddress): make it outside graph capture.
+ * All calls on a device share the array: calls that overlap on the GPU (two streams, two host threads) race. */
+#define SC_RESIDUAL_STATIC_MAX_ELEMENTS 8388608LL
+sc_status sc_residual_norm_static(const void* x_new, const void* x_old, long long n, int norm_p, double* out,
+                                  int device, void* cuda_stream, char* err, int err_len);
+
 /* ---- parity / debug taps (synchronise) -------------------------------------------------------- */
 /* Geometry: lattice size N_rot, number of trajectories of angle k (all N_phi angles are addressable). */
 sc_status sc_debug_geometry(sc_ctx* ctx, int* n_rot, int* n_traj_total, long long* n_pieces_total);

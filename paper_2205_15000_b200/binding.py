@@ -118,6 +118,7 @@ def load_library():
     L.sc_debug_march_units.argtypes = [vp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
     L.sc_debug_last_march_variant.argtypes = [vp, C.c_char_p, i]
     L.sc_debug_launch_count.argtypes = [vp, C.POINTER(C.c_longlong)]
+    L.sc_residual_norm_static.argtypes = [vp, vp, C.c_longlong, i, vp, i, vp, C.c_char_p, i]
     _lib = L
     return L
 
@@ -131,6 +132,30 @@ def _dev_ptr(t, dtype_name: str, numel: int):
     if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous() and t.dtype == want and t.numel() == numel):
         raise ScError(1, f"expected a contiguous CUDA {dtype_name} tensor with {numel} elements")
     return C.c_void_p(t.data_ptr())
+
+
+RESIDUAL_STATIC_MAX_ELEMENTS = 8388608     # SC_RESIDUAL_STATIC_MAX_ELEMENTS of include/sc_riccati.h
+
+
+def sc_residual_norm_static(x_new, x_old, out, norm_p: int = 2, stream: Optional[int] = None):
+    """Eq. 27's residual of two complex128 CUDA tensors into `out` (CUDA float64, 3 values: ||x_new - x_old||_p,
+    ||x_old||_p, ratio) without any allocation by the library: the scratch is a static device array (see the header).
+    Enqueues on `stream` (default: torch's current stream of the tensors' device) and does not synchronise."""
+    import torch
+    L = load_library()
+    n = x_new.numel() if isinstance(x_new, torch.Tensor) else 0
+    a, b, o = _dev_ptr(x_new, "c128", n), _dev_ptr(x_old, "c128", n), _dev_ptr(out, "f64", 3)
+    if a is None or b is None or o is None:
+        raise ScError(1, "sc_residual_norm_static: x_new, x_old and out are required")
+    if not (x_new.device == x_old.device == out.device):
+        raise ScError(1, "sc_residual_norm_static: tensors live on different devices")
+    if stream is None:
+        stream = torch.cuda.current_stream(x_new.device).cuda_stream
+    err = C.create_string_buffer(256)
+    rc = L.sc_residual_norm_static(a, b, n, int(norm_p), o, x_new.device.index, C.c_void_p(stream), err, len(err))
+    if rc:
+        raise ScError(rc, err.value.decode())
+    return out
 
 
 def _stats(s: _Stats) -> SweepStats:

@@ -7,8 +7,8 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsc_riccati.so")
-SOURCES = ["sc_api.cu"]
-DEPS = ["sc_api.cu", "sc_kernels.cuh", "sc_math.cuh", "sc_geometry.hpp", "sc_field_kernels.cuh", "sc_lowrank.cuh", "sc_probe_kernels.cuh",
+SOURCES = ["sc_api.cu", "sc_static.cu"]
+DEPS = ["sc_api.cu", "sc_static.cu", "sc_kernels.cuh", "sc_math.cuh", "sc_geometry.hpp", "sc_field_kernels.cuh", "sc_lowrank.cuh", "sc_probe_kernels.cuh",
         os.path.join("..", "..", "include", "sc_riccati.h")]
 
 
