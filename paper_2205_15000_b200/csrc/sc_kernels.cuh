@@ -799,23 +799,21 @@ __device__ __forceinline__ void march_round2(const MarchArgsT<R>& A, const WarpJ
     const char* e = scr;                         // entry of nodes 0 / 1
     for (int q = RED_NODES; q < PF_DIST && q < nn; q += RED_NODES)
         if (pf_lane) prefetch_l2(J.scr_w + (size_t)(q >> 1) * ROW + lane * 128);
-    Ent<R> En = ld_ent<true>(e, R(0)), En2 = ld_ent<true>(e + ROW, R(0));      // {gt_a, gt_b} of the next two spilled nodes
-    cplx_t<R> oa = mk(R(0), R(0)), ob = oa;      // gamma~ of the odd node, held from the even node before it
+    // {gt_a, gt_b} of the next two spilled nodes: E0 serves nodes 4i, 4i+1, E1 nodes 4i+2, 4i+3, each reloaded (two entries ahead) once
+    // its pair is done, so that neither the entries nor the gamma~ of the odd node are ever copied between registers
+    Ent<R> E0 = ld_ent<true>(e, R(0)), E1 = ld_ent<true>(e + ROW, R(0));
     double part_nxt = 0.0;
     if (n0 && lane < RED_NODES * RED_VALS && lane < npart) part_nxt = J.PART[lane];
     int m = 0;
-    auto node = [&](int b, const V4* pbuf, const V2* dbuf, bool exitp) {
+    auto node = [&](int b, const V4* pbuf, const V2* dbuf, bool exitp, const Ent<R>& E) {
         const V4 cc = pbuf[b]; const V2 dc = dbuf[b];
         const R len = exitp ? J.len1 : J.hlen;
         const cplx_t<R> Ta = exitp ? end_T<R>(cc, R(0), zia, len) : ta.fast(cc);
         const cplx_t<R> Tb = exitp ? end_T<R>(cc, R(0), zib, len) : tb.fast(cc);
-        cplx_t<R> ha = oa, hb = ob;
-        if (!(b & 1)) {
-            const cplx_t<R> Ga = mk(En.tr, En.ti), Gb = mk(En.gr, En.gi);      // entry (m+b)>>1: node m+b+1, or the last node itself
-            En = En2; En2 = ld_ent<true>(e + ((b >> 1) + 2) * ROW, R(0));
-            oa = Ga; ob = Gb;
-            ha = exitp ? Ga : scm::step_T(Ga, -cc.x, cc.y, cc.z, zia, Ta);
-            hb = exitp ? Gb : scm::step_T(Gb, -cc.x, cc.y, cc.z, zib, Tb);
+        cplx_t<R> ha = mk(E.tr, E.ti), hb = mk(E.gr, E.gi);      // entry (m+b)>>1: gamma~ of the odd node m+b | 1, or of the last node itself
+        if (!(b & 1) && !exitp) {                                 // even node: one step down from the odd node above it
+            ha = scm::step_T(ha, -cc.x, cc.y, cc.z, zia, Ta);
+            hb = scm::step_T(hb, -cc.x, cc.y, cc.z, zib, Tb);
         }
         R sa[6];
         node_terms<R>(ga, ha, dc, sa); node_terms_acc<R>(gb, hb, dc, sa);
@@ -848,12 +846,15 @@ __device__ __forceinline__ void march_round2(const MarchArgsT<R>& A, const WarpJ
             if (n0 && lane < RED_NODES * RED_VALS && (m + RED_NODES) * RED_VALS + lane < npart)
                 part_nxt = J.PART[(m + RED_NODES) * RED_VALS + lane];
             const V4* __restrict__ pb = pbuf + (m & (CHUNK - 1)); const V2* __restrict__ db = dbuf + (m & (CHUNK - 1));
+            static_assert(RED_NODES == 4, "two pairs of nodes per block");
             if (m + RED_NODES < nn) {
-#pragma unroll
-                for (int b = 0; b < RED_NODES; ++b) node(b, pb, db, false);
-            } else {
-#pragma unroll
-                for (int b = 0; b < RED_NODES; ++b) node(b, pb, db, b == RED_NODES - 1);
+                node(0, pb, db, false, E0); node(1, pb, db, false, E0);
+                E0 = ld_ent<true>(e + 2 * ROW, R(0));
+                node(2, pb, db, false, E1); node(3, pb, db, false, E1);
+                E1 = ld_ent<true>(e + 3 * ROW, R(0));
+            } else {                                             // the last block: its last piece is the exit piece
+                node(0, pb, db, false, E0); node(1, pb, db, false, E0);
+                node(2, pb, db, false, E1); node(3, pb, db, true, E1);
             }
             e += PFROWS * ROW;
             __syncwarp();
@@ -867,7 +868,7 @@ __device__ __forceinline__ void march_round2(const MarchArgsT<R>& A, const WarpJ
         if (m < mhi) {                                       // ragged tail: 1..3 nodes (last chunk only)
             const int rem = mhi - m;
             const double part_old = part_nxt;
-            for (int b = 0; b < rem; ++b) node(b, pbuf + (m & (CHUNK - 1)), dbuf + (m & (CHUNK - 1)), m + b + 1 == nn);
+            for (int b = 0; b < rem; ++b) node(b, pbuf + (m & (CHUNK - 1)), dbuf + (m & (CHUNK - 1)), m + b + 1 == nn, b < 2 ? E0 : E1);
             __syncwarp();
             if (lane < rem * RED_VALS) {
                 double s = stage_colsum(J.stage, lane);
