@@ -616,19 +616,17 @@ __device__ __forceinline__ void march_round(const MarchArgsT<R>& A, const WarpJo
         const V4* __restrict__ pbuf = pcb + bsel * CHUNK;
         const V2* __restrict__ dbuf = ndb + bsel * CHUNK;
         const int mhi = min(nn, (c + 1) * CHUNK);
-        for (; m + RED_NODES <= mhi; m += RED_NODES) {
+        // full batches that do not end the trajectory; the last batch (exit piece) goes through the compact tail code below, so
+        // that the unrolled batch exists once, not twice, in the instruction stream (rounds of different kinds share the I-cache)
+        const int mfull = min(mhi, nn - 1);
+        for (; m + RED_NODES <= mfull; m += RED_NODES) {
             if (LD && pf_lane && m + PF_DIST < nn) prefetch_l2(J.scr_w + (size_t)(HALF ? (m + PF_DIST) >> 1 : m + PF_DIST + NB) * ROW + lane * 128);
             const double part_old = part_nxt;
             if (MODE == 0 && n0 && lane < RED_NODES * RED_VALS && (m + RED_NODES) * RED_VALS + lane < npart)
                 part_nxt = J.PART[(m + RED_NODES) * RED_VALS + lane];
             const V4* __restrict__ pb = pbuf + (m & (CHUNK - 1)); const V2* __restrict__ db = dbuf + (m & (CHUNK - 1));
-            if (m + RED_NODES < nn) {
 #pragma unroll
-                for (int b = 0; b < RED_NODES; ++b) node(b, pb, db, false);
-            } else {                                             // the batch ends on the trajectory's last node
-#pragma unroll
-                for (int b = 0; b < RED_NODES; ++b) node(b, pb, db, b == RED_NODES - 1);
-            }
+            for (int b = 0; b < RED_NODES; ++b) node(b, pb, db, false);
             e += PFROWS * ROW;
             if (MODE == 0) {
                 __syncwarp();
@@ -640,10 +638,13 @@ __device__ __forceinline__ void march_round(const MarchArgsT<R>& A, const WarpJo
                 __syncwarp();
             }
         }
-        if (m < mhi) {                                       // ragged tail: 1..3 nodes (last chunk only)
+        if (m < mhi) {                                       // the last 1..4 nodes of the trajectory (last chunk only)
             const int rem = mhi - m;
             const double part_old = part_nxt;
-            for (int b = 0; b < rem; ++b) node(b, pbuf + (m & (CHUNK - 1)), dbuf + (m & (CHUNK - 1)), m + b + 1 == nn);
+            const V4* __restrict__ pb = pbuf + (m & (CHUNK - 1)); const V2* __restrict__ db = dbuf + (m & (CHUNK - 1));
+#pragma unroll 1
+            for (int b = 0; b < rem - 1; ++b) node(b, pb, db, false);
+            node(rem - 1, pb, db, true);                         // m + rem == nn: the exit piece, with its own length
             if (MODE == 0) {
                 __syncwarp();
                 if (lane < rem * RED_VALS) {
@@ -840,22 +841,18 @@ __device__ __forceinline__ void march_round2(const MarchArgsT<R>& A, const WarpJ
         const V4* __restrict__ pbuf = pcb + bsel * CHUNK;
         const V2* __restrict__ dbuf = ndb + bsel * CHUNK;
         const int mhi = min(nn, (c + 1) * CHUNK);
-        for (; m + RED_NODES <= mhi; m += RED_NODES) {
+        const int mfull = min(mhi, nn - 1);                     // the last batch goes through the tail code (see march_round)
+        for (; m + RED_NODES <= mfull; m += RED_NODES) {
             if (pf_lane && m + PF_DIST < nn) prefetch_l2(J.scr_w + (size_t)((m + PF_DIST) >> 1) * ROW + lane * 128);
             const double part_old = part_nxt;
             if (n0 && lane < RED_NODES * RED_VALS && (m + RED_NODES) * RED_VALS + lane < npart)
                 part_nxt = J.PART[(m + RED_NODES) * RED_VALS + lane];
             const V4* __restrict__ pb = pbuf + (m & (CHUNK - 1)); const V2* __restrict__ db = dbuf + (m & (CHUNK - 1));
             static_assert(RED_NODES == 4, "two pairs of nodes per block");
-            if (m + RED_NODES < nn) {
-                node(0, pb, db, false, E0); node(1, pb, db, false, E0);
-                E0 = ld_ent<true>(e + 2 * ROW, R(0));
-                node(2, pb, db, false, E1); node(3, pb, db, false, E1);
-                E1 = ld_ent<true>(e + 3 * ROW, R(0));
-            } else {                                             // the last block: its last piece is the exit piece
-                node(0, pb, db, false, E0); node(1, pb, db, false, E0);
-                node(2, pb, db, false, E1); node(3, pb, db, true, E1);
-            }
+            node(0, pb, db, false, E0); node(1, pb, db, false, E0);
+            E0 = ld_ent<true>(e + 2 * ROW, R(0));
+            node(2, pb, db, false, E1); node(3, pb, db, false, E1);
+            E1 = ld_ent<true>(e + 3 * ROW, R(0));
             e += PFROWS * ROW;
             __syncwarp();
             if (lane < RED_NODES * RED_VALS) {
@@ -865,10 +862,13 @@ __device__ __forceinline__ void march_round2(const MarchArgsT<R>& A, const WarpJ
             }
             __syncwarp();
         }
-        if (m < mhi) {                                       // ragged tail: 1..3 nodes (last chunk only)
+        if (m < mhi) {                                       // the last 1..4 nodes of the trajectory (last chunk only)
             const int rem = mhi - m;
             const double part_old = part_nxt;
-            for (int b = 0; b < rem; ++b) node(b, pbuf + (m & (CHUNK - 1)), dbuf + (m & (CHUNK - 1)), m + b + 1 == nn, b < 2 ? E0 : E1);
+            const V4* __restrict__ pb = pbuf + (m & (CHUNK - 1)); const V2* __restrict__ db = dbuf + (m & (CHUNK - 1));
+#pragma unroll 1
+            for (int b = 0; b < rem - 1; ++b) node(b, pb, db, false, b < 2 ? E0 : E1);
+            node(rem - 1, pb, db, true, rem <= 2 ? E0 : E1);     // m + rem == nn: the exit piece, with its own length
             __syncwarp();
             if (lane < rem * RED_VALS) {
                 double s = stage_colsum(J.stage, lane);
